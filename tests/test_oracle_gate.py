@@ -1,0 +1,190 @@
+"""Tier B (keyed algorithm) pinned to Tier A (plaintext semantics) and Tier A pinned to closed forms.
+Lemma 4.5 / Thm 4.6: reconstructing the two parties' outputs gives G(x) for EVERY
+x and EVERY mask r.  Exhaustive at n = 8; all x with sampled r and all r with sampled x at n = 12."""
+import os
+
+import numpy as np
+import pytest
+
+from helpers import all_r_keys, mask_of, pack_bits
+from workloads import specs
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _signed(v, n):
+    v = v.astype(np.int64)
+    return np.where(v >= (1 << (n - 1)), v - (1 << n), v)
+
+
+def _check_all_r(orc, spec, xs, seed=11):
+    P = orc.Program(spec)
+    n = spec.n
+    N = 1 << n
+    na = P.shape["n_out_a"]
+    r_out = (np.arange(N * max(1, na), dtype=np.uint64) * np.uint64(2654435761)) & mask_of(n)
+    r_in, (k0, k1) = all_r_keys(P, n, seed, r_out)
+    for x in xs:
+        xv = np.full(N, x, dtype=np.uint64)
+        xhat = (xv + r_in) & mask_of(n)
+        out = P.run_gate(k0, k1, xhat)
+        ye, ze = P.plain_G(xv, r_in)
+        if spec.mask_output:
+            ye = (ye + r_out.reshape(-1, N)[: ye.shape[0]]) & mask_of(n)
+        y = (out["y"][0] + out["y"][1]) & mask_of(n)
+        assert np.array_equal(y, ye), (spec.name, x)
+        if P.shape["n_out_b"]:
+            assert np.array_equal(out["z"][0] ^ out["z"][1], pack_bits(ze)), (spec.name, x)
+        # the two calls reconstruct to their plain definitions (Def I.1 / I.2)
+        for t in range(P.shape["T"]):
+            a = P.atom(t)
+            K = np.uint64((1 << a["k"]) - 1)
+            u = ((xhat & K) + np.uint64(a["c"])) & K
+            rk = r_in & K
+            theta = (rk + np.uint64(a["beta"])) & K if a["is_theta"] else rk
+            got = ((out["bits"][0] ^ out["bits"][1]) >> np.uint64(t)) & np.uint64(1)
+            assert np.array_equal(got, (u < theta).astype(np.uint64)), (spec.name, t)
+        if P.shape["has_lut"]:
+            c = (out["coeff"][0] + out["coeff"][1]) & mask_of(n)
+            i_star = np.searchsorted(np.array([0] + spec.alpha), np.uint64(x), side="right") - 1
+            pay = np.concatenate([spec.coeff[i_star].reshape(-1), spec.aux[i_star].reshape(-1)])
+            assert np.array_equal(c, np.repeat(pay[:, None], N, axis=1)), (spec.name, x)
+    return P
+
+
+SPECS8 = [lambda: specs.relu(8, 4), lambda: specs.toy(8, 3), lambda: specs.toy(8, 3, True),
+          lambda: specs.plain_default(8, 3), lambda: specs.single_interval(8, 3), lambda: specs.no_bits(8, 3),
+          lambda: specs.full_partition(3), lambda: specs.shift_relu(8, 3)]
+
+
+@pytest.mark.parametrize("mk", SPECS8)
+def test_reconstruct_equals_plaintext_exhaustive_n8(orc, mk):
+    spec = mk()
+    N = 1 << spec.n
+    xs = range(N) if spec.name in ("relu_n8", "shift_relu_n8", "full_n3") else list(range(0, N, 3)) + [N - 1]
+    _check_all_r(orc, spec, xs)
+
+
+@pytest.mark.parametrize("mk", [lambda: specs.relu(12, 6), lambda: specs.shift_relu(12, 4), lambda: specs.toy(12, 4)])
+def test_reconstruct_equals_plaintext_n12(orc, mk):
+    spec = mk()
+    rng = np.random.default_rng(12)
+    xs = [0, 1, 2047, 2048, 4095] + [int(v) for v in rng.integers(0, 4096, 3)]
+    _check_all_r(orc, spec, xs)
+
+
+def test_appendix_N_relu_golden(orc):
+    """App. N: shape (T, M, p, #Beaver), atoms, and semantics (max(x,0), MSB(x))."""
+    gold = {}
+    for line in open(os.path.join(GOLD, "appN_relu.txt")):
+        line = line.split("#")[0].split()
+        if line:
+            gold[line[0]] = [int(v) for v in line[1:]]
+    for n, f in ((8, 4), (12, 6), (16, 8), (64, 12)):
+        spec = specs.relu(n, f)
+        P = orc.Program(spec)
+        for key in ("T", "M", "p", "M_A", "M_B", "G_mix"):
+            assert P.shape[key] == gold[key][0], key
+        assert spec.m == gold["m"][0]
+        assert [int(v) for v in spec.coeff[0].reshape(-1)] == gold["P0"]
+        assert [int(v) for v in spec.coeff[1].reshape(-1)] == gold["P1"]
+        assert P.shape["k"] == [n, n]
+        a0, a1 = P.atom(0), P.atom(1)
+        assert (a0["is_theta"], a1["is_theta"], a1["beta"], a0["c"], a1["c"]) == (0, 1, 1 << (n - 1), 0, 0)
+    n = 8
+    P = orc.Program(specs.relu(8, 4))
+    xs = np.arange(256, dtype=np.uint64)
+    y, z = P.plain_G(xs, np.zeros(256, np.uint64))
+    assert np.array_equal(_signed(y[0], n), np.maximum(_signed(xs, n), 0))
+    assert np.array_equal(z[0], (xs >= 128).astype(np.uint8))
+
+
+@pytest.mark.parametrize("n,f", [(8, 3), (12, 4)])
+def test_shift_relu_closed_form(orc, n, f):
+    """config 4a semantics: y = max(0, floor(x_signed / 2^f)) for all x, r; wrap bit two ways agree."""
+    P = orc.Program(specs.shift_relu(n, f))
+    N = 1 << n
+    xs = np.arange(N, dtype=np.uint64)
+    for r in (range(N) if n == 8 else [0, 1, N // 2, N - 1, 1234, 3001]):
+        rv = np.full(N, r, dtype=np.uint64)
+        y, z = P.plain_G(xs, rv)
+        assert np.array_equal(y[0].astype(np.int64), np.maximum(0, _signed(xs, n) >> f))
+        assert np.array_equal(z[0], (xs >= N // 2).astype(np.uint8))
+        assert np.array_equal(z[1], z[2])                            # AND-path wrap bit == r-atom wrap bit
+        assert np.array_equal(z[1], (((xs + rv) & mask_of(n)) < rv).astype(np.uint8))
+
+
+def test_shape_is_mask_independent(orc):
+    """Prop. I.3: (T, M, p), key length and layout depend on (program, count) only."""
+    spec = specs.toy(8, 3)
+    P = orc.Program(spec)
+    sizes = {P.key_bytes(c) for c in (1, 31, 32, 33, 1000)}
+    assert len(sizes) >= 3
+    kb = P.key_bytes(16)
+    for r0 in (0, 1, 255, 224):                                      # incl. r = -alpha_i (beta_0 = 0 branch)
+        k0, k1 = P.keygen(np.full(16, r0, np.uint64), None, 3)
+        assert k0.size == kb and k1.size == kb
+    for other in (specs.relu(64, 12), specs.gelu(), specs.shift_relu()):
+        Q = orc.Program(other)
+        assert Q.key_bytes(7) == Q.key_bytes(7)
+
+
+def test_chunked_keygen_equals_one_shot(orc):
+    """randomness is derived from the GLOBAL element index, so chunks reproduce the one-shot keys."""
+    spec = specs.shift_relu(12, 4)
+    P = orc.Program(spec)
+    rng = np.random.default_rng(0)
+    r = rng.integers(0, 4096, 96, dtype=np.uint64)
+    xh = rng.integers(0, 4096, 96, dtype=np.uint64)
+    k0, k1 = P.keygen(r, None, 9)
+    full = P.run_gate(k0, k1, xh)
+    for lo, hi in ((0, 40), (40, 96)):
+        c0, c1 = P.keygen(r[lo:hi], None, 9, first_elem=lo)
+        part = P.run_gate(c0, c1, xh[lo:hi])
+        for b in (0, 1):
+            assert np.array_equal(part["y"][b], full["y"][b][:, lo:hi])
+            assert np.array_equal(part["bits"][b], full["bits"][b][lo:hi])
+            assert np.array_equal(part["coeff"][b], full["coeff"][b][:, lo:hi])
+
+
+def test_single_party_shares_look_uniform(orc):
+    """guards against a degenerate "share = value" bug: chi^2 of party-0 output share at n = 8."""
+    spec = specs.relu(8, 4)
+    P = orc.Program(spec)
+    rng = np.random.default_rng(5)
+    cnt = 8192
+    r = rng.integers(0, 256, cnt, dtype=np.uint64)
+    x = np.full(cnt, 3, np.uint64)
+    k0, k1 = P.keygen(r, None, 77)
+    out = P.run_gate(k0, k1, (x + r) & np.uint64(255))
+    for arr in (out["y"][0][0], out["coeff"][0][0], out["coeff"][1][1]):
+        h = np.bincount(arr.astype(np.int64), minlength=256)
+        chi2 = ((h - cnt / 256) ** 2 / (cnt / 256)).sum()
+        assert chi2 < 400, chi2                                       # 255 dof: mean 255, sd ~22.6
+    ones = int((out["bits"][0] & np.uint64(1)).sum())
+    assert 0.45 < ones / cnt < 0.55
+
+
+def test_complexity_accounting_table(orc):
+    """App. O counts per config, as listed in DESIGN.md."""
+    exp = {"relu16": (2, 3, 2, 1, 0, 0), "gelu": (5, 11, 3, 2, 0, 0), "nexp": (0, 19, 2, 1, 0, 0),
+           "recip": (0, 19, 3, 2, 0, 0), "shift_relu": (3, 3, 1, 1, 1, 2), "rsqrt": (0, 15, 3, 2, 0, 0),
+           "silu": (5, 27, 3, 2, 0, 0)}
+    for name, want in exp.items():
+        P = orc.Program(specs.CONFIGS[name]())
+        got = tuple(P.shape[k] for k in ("T", "M", "p", "M_A", "M_B", "G_mix"))
+        assert got == want, (name, got)
+    P = orc.Program(specs.shift_relu())
+    assert P.shape["k"] == [64, 64, 12] and P.post_rounds() == 3
+    assert P.online_bits() == 64 + 2 * 64 + 2 + 2
+
+
+def test_rejects_ill_formed(orc):
+    s = specs.relu(8, 4)
+    s.alpha = [0]
+    with pytest.raises(ValueError):
+        orc.Program(s)
+    s = specs.toy(8, 3)
+    s.alpha = [40, 40, 200]
+    with pytest.raises(ValueError):
+        orc.Program(s)
