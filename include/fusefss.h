@@ -1,0 +1,178 @@
+/*
+ * fusefss.h -- C ABI of libfusefss (B200 / sm_100a), the data-parallel hot path of FuseFSS
+ * (arxiv/paper_2606_09551).  "P:<line>" cites /root/reference/PAPER.md; "DESIGN 4.x" cites DESIGN.md.
+ *
+ * Conventions
+ *  - Every function returns 0 on success or a negative FUSEFSS_E_* code; nothing throws or aborts.
+ *    fusefss_strerror() gives text.  Size queries return 0 on a null program.
+ *  - Ring elements of Z_{2^n} (n <= 64) travel as uint64_t with bits >= n zero.
+ *  - Pointers named *_dev are DEVICE pointers owned by the caller (e.g. torch tensors); pointers without
+ *    the suffix are HOST pointers.  The library allocates no device memory of its own.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = default stream); all launches are asynchronous on it.
+ *  - party is 0 or 1.  xhat = x + r_in mod 2^n is public and identical for both parties (Protocol 1).
+ *  - A key buffer is one-time material for exactly one xhat tensor; not enforced.
+ *  - Key buffers are SoA over the chunk's elements; their size and layout depend on (program, count) only
+ *    (Prop. I.3; DESIGN 4.4).
+ */
+#ifndef FUSEFSS_H
+#define FUSEFSS_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    FUSEFSS_OK = 0,
+    FUSEFSS_E_NULL = -1,      /* a required pointer is null                                   */
+    FUSEFSS_E_SPEC = -2,      /* ill-formed operator specification or over a limit    */
+    FUSEFSS_E_PARTY = -3,     /* party not in {0,1}                                           */
+    FUSEFSS_E_COUNT = -4,     /* count == 0                                                   */
+    FUSEFSS_E_ROUND = -5,     /* round outside [0, rounds]                                    */
+    FUSEFSS_E_CUDA = -6,      /* a CUDA call failed (fusefss_last_cuda_error() has the text)  */
+    FUSEFSS_E_OMITTED = -7    /* eval_cmp with T = 0 / eval_lut with m = 1 (call omitted) */
+};
+
+/* ---- operator specification (Def 4.1; grammar App. H) ------------------ */
+/* Boolean expression DAG node.  kind: */
+enum { FUSEFSS_BN_CONST = 0,   /* value & 1                                                     */
+       FUSEFSS_BN_C = 1,       /* C_beta(x)    = I[rep(x) < value]; value_is_2k: beta = 2^n     */
+       FUSEFSS_BN_D = 2,       /* D_{gamma,k}(x) = I[(rep(x) mod 2^k) < value]; value_is_2k: 2^k */
+       FUSEFSS_BN_MSB = 3,     /* MSB(x + value)                                   */
+       FUSEFSS_BN_CARRY = 4,   /* carry of the low k bits of x + r_in (DESIGN 4.3 R1)           */
+       FUSEFSS_BN_NOT = 5, FUSEFSS_BN_XOR = 6, FUSEFSS_BN_AND = 7, FUSEFSS_BN_OR = 8 };
+typedef struct {
+    uint8_t kind, k; uint16_t lhs, rhs; uint8_t value_is_2k, pad; uint64_t value;
+} fusefss_bitnode;
+
+/* instance constants kappa derived from r_in only (Def 4.2) */
+enum { FUSEFSS_KA_R_SHR = 1 /* kappa^A = rep(r_in) >> arg */, FUSEFSS_KB_R_BIT = 2 /* kappa^B = bit arg of r_in */ };
+typedef struct { uint8_t kind, arg; } fusefss_kappa;
+
+/* post-processing program Phi (App. H): straight-line code over arithmetic registers A[]
+ * and bit registers B[] (at most 256 of each).  op: */
+enum {
+    FUSEFSS_PHI_A_CONST = 1,  /* A[dst] = imm                        */
+    FUSEFSS_PHI_A_X,          /* A[dst] = x                          */
+    FUSEFSS_PHI_A_Y,          /* A[dst] = y_a (a-th polynomial)      */
+    FUSEFSS_PHI_A_KAPPA,      /* A[dst] = kappa^A_a                  */
+    FUSEFSS_PHI_A_XHAT_SHR,   /* A[dst] = xhat >> a   (public)       */
+    FUSEFSS_PHI_A_ADD, FUSEFSS_PHI_A_SUB,     /* A[dst] = A[a] +- A[b] */
+    FUSEFSS_PHI_A_MULC,       /* A[dst] = A[a] * imm                 */
+    FUSEFSS_PHI_A_MUL,        /* A[dst] = A[a] * A[b]  (one Beaver)  */
+    FUSEFSS_PHI_A_B2A,        /* A[dst] = B[a]         (one B2A)     */
+    FUSEFSS_PHI_A_OUT,        /* output y'[dst] = A[a]               */
+    FUSEFSS_PHI_A_AUX,        /* A[dst] = aux_a of the active interval */
+    FUSEFSS_PHI_B_CONST = 32, /* B[dst] = imm & 1                    */
+    FUSEFSS_PHI_B_Z,          /* B[dst] = z_a (a-th predicate bit)   */
+    FUSEFSS_PHI_B_KAPPA,      /* B[dst] = kappa^B_a                  */
+    FUSEFSS_PHI_B_XHAT,       /* B[dst] = bit a of xhat (public)     */
+    FUSEFSS_PHI_B_NOT, FUSEFSS_PHI_B_XOR, FUSEFSS_PHI_B_AND, FUSEFSS_PHI_B_OR,
+    FUSEFSS_PHI_B_ANDPUB,     /* B[dst] = B[a] & (bit b of xhat ^ (imm&1)) */
+    FUSEFSS_PHI_B_OUT         /* output z'[dst] = B[a]               */
+};
+typedef struct { uint8_t op, dst, a, b; uint32_t pad; uint64_t imm; } fusefss_phi_op;
+
+typedef struct {
+    uint32_t n, frac_bits;            /* ring Z_{2^n}, fixed-point metadata                         */
+    uint32_t m, r, d, p_aux, ell;     /* intervals, polynomials, degree bound, aux constants, predicate bits */
+    uint32_t n_nodes, n_kappa_a, n_kappa_b, phi_len;
+    uint32_t n_out_a, n_out_b;        /* outputs of Phi (ignored when phi_len == 0: outputs are y and z)    */
+    uint32_t mask_output;             /* 1: arithmetic outputs are opened as yhat = y + r_out       */
+    const uint64_t *alpha;            /* HOST [m-1] interior boundaries, strictly increasing in (0, 2^n)    */
+    const uint64_t *coeff;            /* HOST [m][r][d+1], high degree first                                */
+    const uint64_t *aux;              /* HOST [m][p_aux]                                                    */
+    const fusefss_bitnode *nodes;     /* HOST [n_nodes]                                                     */
+    const uint16_t *bit_root;         /* HOST [m][ell] root node per interval per output bit                */
+    const fusefss_kappa *kappa_a, *kappa_b;
+    const fusefss_phi_op *phi;        /* HOST [phi_len]                                                     */
+} fusefss_spec;
+
+typedef struct fusefss_program fusefss_program;   /* opaque, library-owned */
+
+/* L_shape = (T, {k_t}, M, p, #mults, #ANDs, #B2A) -- everything that may depend on the spec only */
+typedef struct {
+    int32_t T, M, p, M_A, M_B, G_mix, rounds, n_out_a, n_out_b, has_lut, n_kb;
+    int32_t k[64];
+} fusefss_shape_t;
+
+/* ---- a0: compile (host only; Protocol 3 steps (2)-(4); DESIGN 4.3) ------------------
+ * Validates the spec (boundaries strictly increasing in (0,2^n), n in [1,64], m < 64, p <= 8, T <= 64,
+ * <= 16 rounds, <= 64 AND gates, <= 64 B2A gates) and builds the immutable compiled gate type: atom list,
+ * (T, M, p), post-processing program, message shapes.  The spec's arrays are copied; the caller may free
+ * them.  Compile once per gate type, reuse across tensors/layers (program caching). */
+int fusefss_compile(const fusefss_spec *spec, fusefss_program **out);
+void fusefss_destroy(fusefss_program *prog);
+int fusefss_shape(const fusefss_program *prog, fusefss_shape_t *out);
+/* atom t of the packed comparison instance Q = ((k_t, c_t, theta_t)) (Def I.1):
+ * out4 = { k_t, c_t, is_theta, beta_t };  theta_t = (r mod 2^k + beta_t) mod 2^k, or r mod 2^k for an r-atom */
+int fusefss_atom(const fusefss_program *prog, int t, uint64_t *out4);
+/* bytes of ONE party's key buffer for `count` elements (DESIGN 4.4); a function of (program, count) only */
+size_t fusefss_key_bytes(const fusefss_program *prog, size_t count);
+
+/* ---- a1-a4: keygen (dealer; section 5.2; Protocol 3 steps (1),(5)) ----
+ * r_in_dev[count]: fresh uniform input masks; r_out_dev[n_out_a][count]: output masks (may be NULL unless
+ * mask_output).  seed: the dealer's randomness seed (DESIGN 4.5).  first_elem: GLOBAL index of element 0 of
+ * this chunk -- randomness is derived from the global index, so chunked keygen equals one-shot keygen.
+ * Writes both parties' key buffers (fusefss_key_bytes() each, 256-byte aligned device memory). */
+int fusefss_keygen(const fusefss_program *prog, const uint64_t *r_in_dev, const uint64_t *r_out_dev,
+                   uint64_t seed, uint64_t first_elem, size_t count,
+                   void *key0_dev, void *key1_dev, void *stream);
+
+/* ---- a5: packed comparison (section 3.6, Def I.1) --------------------------------
+ * bits_out_dev[count]: bit t = this party's XOR share of I[view_{k_t,c_t}(xhat) < theta_t]. */
+int fusefss_eval_cmp(int party, const fusefss_program *prog, const void *key_dev, const uint64_t *xhat_dev,
+                     size_t count, uint64_t *bits_out_dev, void *stream);
+
+/* ---- a6: vector interval lookup (section 3.6, Def I.2) ---------------------------
+ * coeff_out_dev[p][count]: this party's additive share of the active interval's payload v_{i*} in R^p. */
+int fusefss_eval_lut(int party, const fusefss_program *prog, const void *key_dev, const uint64_t *xhat_dev,
+                     size_t count, uint64_t *coeff_out_dev, void *stream);
+
+/* ---- a7: post-processing (online steps 4-6; Horner P:895; DESIGN 4.6) ---------
+ * One call per party per round.  msg_in_dev = the OTHER party's message buffer, msg_out_dev = this party's;
+ * both cover all rounds (sum over q of fusefss_post_msg_bytes(q)).  round q in [0, rounds) writes this party's
+ * openings of round q into msg_out_dev (replaying rounds < q from both buffers); round == rounds writes
+ * y_out_dev[n_out_a][count] (shares of y, or of yhat = y + r_out when mask_output) and z_out_dev[count]
+ * (bit j = XOR share of output bit j).  bits_dev / coeff_dev may be NULL when the respective call is omitted. */
+int fusefss_post(int party, const fusefss_program *prog, const void *key_dev, const uint64_t *xhat_dev,
+                 const uint64_t *bits_dev, const uint64_t *coeff_dev, size_t count, int round,
+                 const void *msg_in_dev, void *msg_out_dev, uint64_t *y_out_dev, uint64_t *z_out_dev,
+                 void *stream);
+int fusefss_post_rounds(const fusefss_program *prog);
+size_t fusefss_post_msg_bytes(const fusefss_program *prog, size_t count, int round);
+/* algorithmic online bits per element per party: n (xhat) + 2n M_A + 2 M_B + G_mix (+ n n_out_a if masked) */
+size_t fusefss_online_bits(const fusefss_program *prog);
+/* Both parties, all rounds, one launch; outputs equal the per-round API bit for bit. */
+int fusefss_post_fused(const fusefss_program *prog, const void *key0_dev, const void *key1_dev,
+                       const uint64_t *xhat_dev, const uint64_t *bits0_dev, const uint64_t *bits1_dev,
+                       const uint64_t *coeff0_dev, const uint64_t *coeff1_dev, size_t count,
+                       uint64_t *y0_dev, uint64_t *y1_dev, uint64_t *z0_dev, uint64_t *z1_dev, void *stream);
+
+/* ---- end-to-end convenience: HOST buffers in, HOST buffers out (bench.py's e2e leg) ---------------
+ * Copies r_in/r_out/xhat to the device, runs keygen + both parties' eval_cmp/eval_lut + post_fused in chunks of
+ * `chunk` elements using the caller's device workspace, copies y0,y1 [n_out_a][count] and z0,z1 [count] back.
+ * workspace_dev must hold fusefss_gate_workspace_bytes(prog, chunk) bytes. */
+size_t fusefss_gate_workspace_bytes(const fusefss_program *prog, size_t chunk);
+int fusefss_gate_host(const fusefss_program *prog, const uint64_t *r_in, const uint64_t *r_out,
+                      const uint64_t *xhat, uint64_t seed, size_t count, size_t chunk, void *workspace_dev,
+                      uint64_t *y0, uint64_t *y1, uint64_t *z0, uint64_t *z1, void *stream);
+
+/* ---- diagnostics ---------------------------------------------------------------------------------- */
+const char *fusefss_strerror(int code);
+const char *fusefss_last_cuda_error(void);
+/* number of kernel launches this library has issued since load (bench.py's gpu_launches) */
+uint64_t fusefss_launch_count(void);
+/* PRG micro-kernel for the roofline denominator: each thread chains `iters` fixed-key AES-128 blocks starting
+ * from its index and writes the last block to out_dev[threads*16 bytes]; blocks = threads*iters. */
+int fusefss_aes_probe(size_t threads, int iters, void *out_dev, void *stream);
+/* single-block AES-128 (FIPS-197) through the device PRG core, for the known-answer test: key[16], in[16] HOST,
+ * out_dev[16] device */
+int fusefss_aes_kat(const uint8_t *key, const uint8_t *in, void *out_dev, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FUSEFSS_H */
