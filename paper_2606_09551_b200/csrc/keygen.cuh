@@ -1,0 +1,406 @@
+// keygen.cuh -- dealer kernels (section 5.2): per element, T bit-DCF Gen (a2), Protocol 3 step (1)
+// + (M-1) vector-DCF Gen + additive split of v_{M-1} (a1, a3), and the share splitting of masks,
+// instance constants and correlated randomness (a4).  DCF Gen: DESIGN 4.2; randomness slots: DESIGN 4.5;
+// key layout: DESIGN 4.4.  One lane per element, one warp per (32-element tile, tree): the level loop is
+// sequential, the four child expansions of a level run in lock-step through the shared-memory T-tables, and
+// each level's correction words are written to both parties' buffers as coalesced streaming stores.
+#pragma once
+#include "aes.cuh"
+
+namespace fsk {
+
+constexpr int kGenThreads = 512;
+
+enum : uint64_t {
+    SLOT_BIT_ROOT = 0x1000, SLOT_VEC_ROOT = 0x2000, SLOT_LUT_C = 0x3000, SLOT_RIN = 0x4000, SLOT_ROUT = 0x4100,
+    SLOT_KA = 0x5000, SLOT_KB = 0x5800, SLOT_BV_AB = 0x6000, SLOT_BV_AB0 = 0x6800, SLOT_BV_C0 = 0x7000,
+    SLOT_AND_AB = 0x8000, SLOT_AND_AB0 = 0x8001, SLOT_AND_C0 = 0x8002, SLOT_B2A = 0x9000, SLOT_B2A_A0 = 0x9100
+};
+
+__device__ __forceinline__ void st_stream16(void *p, uint4 v) { __stcs(reinterpret_cast<uint4 *>(p), v); }
+__device__ __forceinline__ void st_stream8(void *p, uint64_t v) { __stcs(reinterpret_cast<unsigned long long *>(p), (unsigned long long)v); }
+
+// R(e, slot) = AES_{seed||~seed}(LE64(e) || LE64(slot))
+template <int NTAB>
+__device__ __forceinline__ void dealer_rand(const uint32_t *tl, const RoundKeys &rk, uint64_t e, uint64_t slot, uint64_t &lo, uint64_t &hi) {
+    uint32_t s[4] = {(uint32_t)e, (uint32_t)(e >> 32), (uint32_t)slot, (uint32_t)(slot >> 32)};
+    aes_encrypt_rk<NTAB>(tl, rk, s);
+    lo = (uint64_t)s[0] | ((uint64_t)s[1] << 32);
+    hi = (uint64_t)s[2] | ((uint64_t)s[3] << 32);
+}
+
+struct GenAtomDev { uint64_t c, beta, root_off, cw_off, vb_off; int k, is_theta; };
+struct GenBitArgs {
+    uint8_t *key0, *key1; const uint64_t *r_in;
+    size_t count, s16; uint64_t first_elem, mask;
+    int T, pad;
+    RoundKeys rk;
+    GenAtomDev atom[kMaxAtoms];
+};
+
+template <int NTAB>
+__global__ void __launch_bounds__(kGenThreads, 1) k_gen_bit(const __grid_constant__ GenBitArgs a) {
+    extern __shared__ uint32_t sT[];
+    aes_fill_tables<NTAB>(sT);
+    const int lane = threadIdx.x & 31;
+    const uint32_t *tl = sT + lane;
+    const size_t tiles = (a.count + 31) / 32;
+    const size_t items = tiles * (size_t)a.T;
+    const size_t warps = (size_t)gridDim.x * (blockDim.x >> 5);
+    for (size_t it = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); it < items; it += warps) {
+        const int t = (int)(it / tiles);
+        const size_t e = (it - (size_t)t * tiles) * 32 + lane;
+        if (e >= a.count) continue;
+        const GenAtomDev &at = a.atom[t];
+        const int k = at.k;
+        const uint64_t km = k >= 64 ? ~0ull : ((1ull << k) - 1ull);
+        const uint64_t rk_ = a.r_in[e] & a.mask & km;
+        // threshold of the masked comparison (Lemma 4.3 / E.1): theta = (r_k + beta) mod 2^k, or r_k for the r-atom
+        uint64_t alpha = (at.is_theta ? (rk_ + at.beta) & km : rk_) << (64 - k);
+        uint32_t s[2][4];
+        {
+            uint64_t lo, hi;
+            dealer_rand<NTAB>(tl, a.rk, a.first_elem + e, SLOT_BIT_ROOT + 2 * t, lo, hi);
+            s[0][0] = (uint32_t)lo & ~3u; s[0][1] = (uint32_t)(lo >> 32); s[0][2] = (uint32_t)hi; s[0][3] = (uint32_t)(hi >> 32);
+            dealer_rand<NTAB>(tl, a.rk, a.first_elem + e, SLOT_BIT_ROOT + 2 * t + 1, lo, hi);
+            s[1][0] = (uint32_t)lo & ~3u; s[1][1] = (uint32_t)(lo >> 32); s[1][2] = (uint32_t)hi; s[1][3] = (uint32_t)(hi >> 32);
+        }
+        const uint4 root0 = make_uint4(s[0][0], s[0][1], s[0][2], s[0][3]);
+        const uint4 root1 = make_uint4(s[1][0], s[1][1], s[1][2], s[1][3]);
+        uint32_t t0 = 0, t1 = 1, Va = 0;
+        uint64_t vbits = 0;
+        uint8_t *cw0 = a.key0 + at.cw_off + e * 16, *cw1 = a.key1 + at.cw_off + e * 16;
+        for (int i = 0; i < k; ++i) {
+            const uint32_t abit = (uint32_t)(alpha >> 63);
+            alpha <<= 1;
+            // children: index 2*b + d
+            uint32_t x[4][4], o[4][1][4];
+#pragma unroll
+            for (int b = 0; b < 2; ++b)
+#pragma unroll
+                for (int d = 0; d < 2; ++d) { x[2 * b + d][0] = s[b][0] | (uint32_t)d; x[2 * b + d][1] = s[b][1]; x[2 * b + d][2] = s[b][2]; x[2 * b + d][3] = s[b][3]; }
+            prg_blocks<NTAB, 4, 1, 0>(tl, x, o);
+            const uint32_t am = 0u - abit;                    // keep = alpha_i, lose = 1 - alpha_i
+            uint32_t keep0[4], keep1[4], scw[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const uint32_t l0 = (o[1][0][c] & ~am) | (o[0][0][c] & am);       // lose = 1 when abit = 0
+                const uint32_t l1 = (o[3][0][c] & ~am) | (o[2][0][c] & am);
+                keep0[c] = (o[0][0][c] & ~am) | (o[1][0][c] & am);
+                keep1[c] = (o[2][0][c] & ~am) | (o[3][0][c] & am);
+                scw[c] = l0 ^ l1;
+            }
+            // word 0 carries: bit0 = control bit T, bit1 = Z_2 payload W
+            const uint32_t lose_w = ((scw[0] >> 1) & 1u);                          // W_0[lose] ^ W_1[lose]
+            const uint32_t keep_w = ((keep0[0] ^ keep1[0]) >> 1) & 1u;
+            const uint32_t vcw = lose_w ^ Va ^ (abit);                             // + beta (=1) iff lose = 0 iff alpha_i = 1
+            Va ^= keep_w ^ vcw;
+            const uint32_t tcw0 = ((o[0][0][0] ^ o[2][0][0]) & 1u) ^ abit ^ 1u;
+            const uint32_t tcw1 = ((o[1][0][0] ^ o[3][0][0]) & 1u) ^ abit;
+            const uint32_t tcw_keep = abit ? tcw1 : tcw0;
+            scw[0] = (scw[0] & ~3u) | tcw0 | (tcw1 << 1);
+            const uint4 cwv = make_uint4(scw[0], scw[1], scw[2], scw[3]);
+            st_stream16(cw0 + (size_t)i * a.s16, cwv);
+            st_stream16(cw1 + (size_t)i * a.s16, cwv);
+            vbits |= (uint64_t)vcw << i;
+            const uint32_t m0 = 0u - t0, m1 = 0u - t1;
+            const uint32_t nt0 = (keep0[0] & 1u) ^ (t0 & tcw_keep), nt1 = (keep1[0] & 1u) ^ (t1 & tcw_keep);
+            s[0][0] = (keep0[0] & ~3u) ^ (scw[0] & ~3u & m0); s[1][0] = (keep1[0] & ~3u) ^ (scw[0] & ~3u & m1);
+#pragma unroll
+            for (int c = 1; c < 4; ++c) { s[0][c] = keep0[c] ^ (scw[c] & m0); s[1][c] = keep1[c] ^ (scw[c] & m1); }
+            t0 = nt0; t1 = nt1;
+        }
+        uint32_t x[2][4], o[2][1][4];
+#pragma unroll
+        for (int b = 0; b < 2; ++b) { x[b][0] = s[b][0] | 2u; x[b][1] = s[b][1]; x[b][2] = s[b][2]; x[b][3] = s[b][3]; }
+        prg_blocks<NTAB, 2, 1, 0>(tl, x, o);
+        const uint32_t fin = (((o[0][0][0] ^ o[1][0][0]) >> 1) & 1u) ^ Va;
+        st_stream16(a.key0 + at.root_off + e * 16, make_uint4(root0.x | fin, root0.y, root0.z, root0.w));
+        st_stream16(a.key1 + at.root_off + e * 16, make_uint4(root1.x | fin, root1.y, root1.z, root1.w));
+        st_stream8(a.key0 + at.vb_off + e * 8, vbits);
+        st_stream8(a.key1 + at.vb_off + e * 8, vbits);
+    }
+}
+
+
+// ---------------------------------------------------------------------------------------------------
+// Protocol 3 step (1) for one element, evaluated per lookup interval j on demand.
+// The sort of s_i = (alpha_i + r) mod N is always the cyclic rotation pi(q) = (i0 + q) mod m with
+// i0 = #{i : alpha_i + r < N} (the non-wrapping starts stay in order and follow the wrapped ones).
+// ---------------------------------------------------------------------------------------------------
+struct P3 {
+    const uint64_t *alpha;     // interior boundaries alpha_1..alpha_{m-1}
+    uint64_t r, mask, N;       // N = 2^n (0 when n = 64: differences are taken mod 2^64)
+    int m, n, i0, beta0_zero, jstar;
+    __device__ __forceinline__ uint64_t start(int i) const { return ((i == 0 ? 0ull : alpha[i - 1]) + r) & mask; }
+    __device__ __forceinline__ int pi(int q) const { int v = i0 + q; return v >= m ? v - m : v; }
+    __device__ __forceinline__ uint64_t sorted(int q) const { return start(pi(q)); }          // beta_q
+    __device__ void init(const uint64_t *alpha_, int m_, int n_, uint64_t mask_, uint64_t r_, int M) {
+        alpha = alpha_; m = m_; n = n_; mask = mask_; r = r_; N = n_ >= 64 ? 0ull : (1ull << n_);
+        i0 = 0;
+        for (int i = 0; i < m; ++i) {
+            const uint64_t a_i = i == 0 ? 0ull : alpha[i - 1];
+            const uint64_t sum = a_i + r;
+            const bool wraps = n >= 64 ? sum < a_i : (sum >> n) != 0;
+            i0 += wraps ? 0 : 1;
+        }
+        beta0_zero = sorted(0) == 0;
+        jstar = -1;
+        if (beta0_zero && M == m + 1) {                                  // lines 12-18: dummy split at the first gap >= 2
+            for (int j = 0; j < m && jstar < 0; ++j) {
+                const uint64_t lo = sorted(j);                           // B'_j  (B'_0 = beta_0 = 0)
+                const uint64_t hi = j + 1 == m ? N : sorted(j + 1);      // B'_m = N (0 mod 2^64 when n = 64; lo >= 1 there)
+                if (hi - lo >= 2) jstar = j;
+            }
+        }
+    }
+    // boundary B_q (1 <= q <= M-1) and interval label ord_q (0 <= q <= M-1)
+    __device__ __forceinline__ uint64_t B(int q) const {
+        if (!beta0_zero) return sorted(q - 1);                           // line 19: B = (0, beta_0, .., beta_{m-1}, N)
+        if (jstar < 0 || q <= jstar) return sorted(q);
+        if (q == jstar + 1) return sorted(jstar) + 1;                    // delta = B_{j*} + 1
+        return sorted(q - 1);
+    }
+    __device__ __forceinline__ int ord(int q) const {
+        if (!beta0_zero) return q == 0 ? pi(m - 1) : pi(q - 1);
+        if (jstar < 0 || q <= jstar) return pi(q);
+        return pi(q - 1);
+    }
+};
+
+struct GenVecArgs {
+    uint8_t *key0, *key1; const uint64_t *r_in; const uint64_t *alpha; const uint64_t *payload;   // payload[m][p]
+    size_t count, s16, s8, vt_first, vt_stride, lvl_stride, vt_lvl_rel, vt_fin_rel;
+    uint64_t first_elem, mask;
+    int n, m, M, pad;
+    RoundKeys rk;
+};
+
+template <int NTAB, int P>
+__global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec(const __grid_constant__ GenVecArgs a) {
+    constexpr int Q = (P + 1) / 2;
+    extern __shared__ uint32_t sT[];
+    aes_fill_tables<NTAB>(sT);
+    const int lane = threadIdx.x & 31;
+    const uint32_t *tl = sT + lane;
+    const size_t tiles = (a.count + 31) / 32;
+    const size_t items = tiles * (size_t)(a.M - 1);
+    const size_t warps = (size_t)gridDim.x * (blockDim.x >> 5);
+    for (size_t it = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); it < items; it += warps) {
+        const int j = 1 + (int)(it / tiles);
+        const size_t e = (it - (size_t)(j - 1) * tiles) * 32 + lane;
+        if (e >= a.count) continue;
+        const uint64_t r = a.r_in[e] & a.mask;
+        P3 p3;
+        p3.init(a.alpha, a.m, a.n, a.mask, r, a.M);
+        uint64_t alpha = p3.B(j) << (64 - a.n);
+        uint64_t beta[P];                                                  // Delta_j = v_{j-1} - v_j
+        {
+            const uint64_t *va = a.payload + (size_t)p3.ord(j - 1) * P, *vb = a.payload + (size_t)p3.ord(j) * P;
+#pragma unroll
+            for (int w = 0; w < P; ++w) beta[w] = va[w] - vb[w];
+        }
+        uint32_t s[2][4];
+        {
+            uint64_t lo, hi;
+            dealer_rand<NTAB>(tl, a.rk, a.first_elem + e, SLOT_VEC_ROOT + 2 * j, lo, hi);
+            s[0][0] = (uint32_t)lo & ~3u; s[0][1] = (uint32_t)(lo >> 32); s[0][2] = (uint32_t)hi; s[0][3] = (uint32_t)(hi >> 32);
+            dealer_rand<NTAB>(tl, a.rk, a.first_elem + e, SLOT_VEC_ROOT + 2 * j + 1, lo, hi);
+            s[1][0] = (uint32_t)lo & ~3u; s[1][1] = (uint32_t)(lo >> 32); s[1][2] = (uint32_t)hi; s[1][3] = (uint32_t)(hi >> 32);
+        }
+        uint8_t *tree0 = a.key0 + a.vt_first + (size_t)(j - 1) * a.vt_stride;
+        uint8_t *tree1 = a.key1 + a.vt_first + (size_t)(j - 1) * a.vt_stride;
+        st_stream16(tree0 + e * 16, make_uint4(s[0][0], s[0][1], s[0][2], s[0][3]));
+        st_stream16(tree1 + e * 16, make_uint4(s[1][0], s[1][1], s[1][2], s[1][3]));
+        uint32_t t0 = 0, t1 = 1;
+        uint64_t Va[P];
+#pragma unroll
+        for (int w = 0; w < P; ++w) Va[w] = 0;
+        size_t lvl = a.vt_lvl_rel;
+        for (int i = 0; i < a.n; ++i, lvl += a.lvl_stride) {
+            const uint32_t abit = (uint32_t)(alpha >> 63);
+            alpha <<= 1;
+            const uint32_t am = 0u - abit;
+            const uint64_t am64 = 0ull - (uint64_t)abit;
+            uint32_t keepS[2][4], loseS[2][4], Tb[2][2];
+            uint64_t keepW[2][P], loseW[2][P];
+#pragma unroll
+            for (int b = 0; b < 2; ++b) {                                  // party b: both directions in lock-step
+                uint32_t x[2][4], o[2][1 + Q][4];
+#pragma unroll
+                for (int d = 0; d < 2; ++d) { x[d][0] = s[b][0] | (uint32_t)d; x[d][1] = s[b][1]; x[d][2] = s[b][2]; x[d][3] = s[b][3]; }
+                prg_blocks<NTAB, 2, 1 + Q, 0>(tl, x, o);
+                Tb[b][0] = o[0][0][0] & 1u; Tb[b][1] = o[1][0][0] & 1u;
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    const uint32_t v0 = c == 0 ? o[0][0][0] & ~3u : o[0][0][c], v1 = c == 0 ? o[1][0][0] & ~3u : o[1][0][c];
+                    keepS[b][c] = (v0 & ~am) | (v1 & am);
+                    loseS[b][c] = (v1 & ~am) | (v0 & am);
+                }
+#pragma unroll
+                for (int w = 0; w < P; ++w) {
+                    const uint64_t w0 = (uint64_t)o[0][1 + w / 2][2 * (w & 1)] | ((uint64_t)o[0][1 + w / 2][2 * (w & 1) + 1] << 32);
+                    const uint64_t w1 = (uint64_t)o[1][1 + w / 2][2 * (w & 1)] | ((uint64_t)o[1][1 + w / 2][2 * (w & 1) + 1] << 32);
+                    keepW[b][w] = (w0 & ~am64) | (w1 & am64);
+                    loseW[b][w] = (w1 & ~am64) | (w0 & am64);
+                }
+            }
+            uint32_t scw[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) scw[c] = loseS[0][c] ^ loseS[1][c];
+            const uint64_t sgn = 0ull - (uint64_t)t1;                       // (-1)^{t_1}: negate iff t_1 = 1
+            uint64_t vcw[P];
+#pragma unroll
+            for (int w = 0; w < P; ++w) {
+                uint64_t v = loseW[1][w] - loseW[0][w] - Va[w] + (beta[w] & am64);     // + beta iff lose = 0 iff alpha_i = 1
+                v = ((v ^ sgn) - sgn) & a.mask;
+                vcw[w] = v;
+                Va[w] = Va[w] - keepW[1][w] + keepW[0][w] + ((v ^ sgn) - sgn);
+            }
+            const uint32_t tcw0 = Tb[0][0] ^ Tb[1][0] ^ abit ^ 1u, tcw1 = Tb[0][1] ^ Tb[1][1] ^ abit;
+            const uint32_t tcw_keep = abit ? tcw1 : tcw0;
+            const uint4 cwv = make_uint4(scw[0] | tcw0 | (tcw1 << 1), scw[1], scw[2], scw[3]);
+            st_stream16(tree0 + lvl + e * 16, cwv);
+            st_stream16(tree1 + lvl + e * 16, cwv);
+#pragma unroll
+            for (int w = 0; w < P; ++w) {
+                st_stream8(tree0 + lvl + a.s16 + (size_t)w * a.s8 + e * 8, vcw[w]);
+                st_stream8(tree1 + lvl + a.s16 + (size_t)w * a.s8 + e * 8, vcw[w]);
+            }
+            const uint32_t m0 = 0u - t0, m1 = 0u - t1;
+            const uint32_t nt0 = (abit ? Tb[0][1] : Tb[0][0]) ^ (t0 & tcw_keep), nt1 = (abit ? Tb[1][1] : Tb[1][0]) ^ (t1 & tcw_keep);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) { s[0][c] = keepS[0][c] ^ (scw[c] & m0); s[1][c] = keepS[1][c] ^ (scw[c] & m1); }
+            t0 = nt0; t1 = nt1;
+        }
+        // final correction word: fin = (-1)^{t_1} (conv(s_1) - conv(s_0) - Valpha)
+        uint32_t x[2][4], o[2][Q][4];
+#pragma unroll
+        for (int b = 0; b < 2; ++b) { x[b][0] = s[b][0] | 2u; x[b][1] = s[b][1]; x[b][2] = s[b][2]; x[b][3] = s[b][3]; }
+        prg_blocks<NTAB, 2, Q, 1>(tl, x, o);
+        const uint64_t sgn = 0ull - (uint64_t)t1;
+#pragma unroll
+        for (int w = 0; w < P; ++w) {
+            const uint64_t c0 = (uint64_t)o[0][w / 2][2 * (w & 1)] | ((uint64_t)o[0][w / 2][2 * (w & 1) + 1] << 32);
+            const uint64_t c1 = (uint64_t)o[1][w / 2][2 * (w & 1)] | ((uint64_t)o[1][w / 2][2 * (w & 1) + 1] << 32);
+            uint64_t v = c1 - c0 - Va[w];
+            v = ((v ^ sgn) - sgn) & a.mask;
+            st_stream8(tree0 + a.vt_fin_rel + (size_t)w * a.s8 + e * 8, v);
+            st_stream8(tree1 + a.vt_fin_rel + (size_t)w * a.s8 + e * 8, v);
+        }
+    }
+}
+
+
+// ---------------------------------------------------------------------------------------------------
+// a4: share splitting.  One lane per element: c_b of the lookup, [r_in], [r_out], kappa^A,
+// kappa^B (theta-atom carries of Lemma 4.3 + the spec's bits), Beaver / AND / B2A material.
+// ---------------------------------------------------------------------------------------------------
+struct GenMiscArgs {
+    uint8_t *key0, *key1; const uint64_t *r_in, *r_out, *alpha, *payload;
+    size_t count, s8, lut_c, rin, rout, ka, kb, beaver, andt, b2a_bits, b2a_a;
+    uint64_t first_elem, mask;
+    int n, m, M, p, has_lut, mask_output, n_out_a, n_ka, n_kb_spec, n_carry, T, MA, MB, GMIX;
+    RoundKeys rk;
+    uint8_t ka_kind[8], ka_arg[8], kb_kind[64], kb_arg[64];
+    GenAtomDev atom[kMaxAtoms];
+};
+
+template <int NTAB>
+__global__ void __launch_bounds__(kGenThreads, 1) k_gen_misc(const __grid_constant__ GenMiscArgs a) {
+    extern __shared__ uint32_t sT[];
+    aes_fill_tables<NTAB>(sT);
+    const uint32_t *tl = sT + (threadIdx.x & 31);
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < a.count; e += (size_t)gridDim.x * blockDim.x) {
+        const uint64_t ge = a.first_elem + e;
+        const uint64_t r = a.r_in[e] & a.mask;
+        uint64_t lo, hi;
+        auto put = [&](size_t off, uint64_t v0, uint64_t v1) {
+            st_stream8(a.key0 + off + e * 8, v0);
+            st_stream8(a.key1 + off + e * 8, v1);
+        };
+        if (a.has_lut) {                                                   // additive split of v_{M-1}
+            P3 p3;
+            p3.init(a.alpha, a.m, a.n, a.mask, r, a.M);
+            const uint64_t *v = a.payload + (size_t)p3.ord(a.M - 1) * a.p;
+            for (int w = 0; w < a.p; ++w) {
+                dealer_rand<NTAB>(tl, a.rk, ge, SLOT_LUT_C + w, lo, hi);
+                const uint64_t c0 = lo & a.mask;
+                put(a.lut_c + (size_t)w * a.s8, c0, (v[w] - c0) & a.mask);
+            }
+        }
+        dealer_rand<NTAB>(tl, a.rk, ge, SLOT_RIN, lo, hi);
+        put(a.rin, lo & a.mask, (r - (lo & a.mask)) & a.mask);
+        if (a.mask_output)
+            for (int j = 0; j < a.n_out_a; ++j) {
+                dealer_rand<NTAB>(tl, a.rk, ge, SLOT_ROUT + j, lo, hi);
+                const uint64_t ro = a.r_out[(size_t)j * a.count + e] & a.mask, s0 = lo & a.mask;
+                put(a.rout + (size_t)j * a.s8, s0, (ro - s0) & a.mask);
+            }
+        for (int t = 0; t < a.n_ka; ++t) {                                 // kappa^A = rep(r) >> arg
+            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_KA + t, lo, hi);
+            uint64_t val = 0;
+            if (a.ka_kind[t] == FUSEFSS_KA_R_SHR) val = a.ka_arg[t] >= 64 ? 0ull : r >> a.ka_arg[t];
+            const uint64_t s0 = lo & a.mask;
+            put(a.ka + (size_t)t * a.s8, s0, ((val & a.mask) - s0) & a.mask);
+        }
+        const int n_kb = a.n_carry + a.n_kb_spec;
+        if (n_kb > 0) {
+            uint64_t kbits = 0;
+            int ci = 0;
+            for (int t = 0; t < a.T; ++t) {                                // w_t = I[r_k + beta >= 2^k]  (Lemma 4.3, G3)
+                if (!a.atom[t].is_theta) continue;
+                const int k = a.atom[t].k;
+                const uint64_t km = k >= 64 ? ~0ull : ((1ull << k) - 1ull);
+                const uint64_t rk_ = r & km, sum = rk_ + a.atom[t].beta;
+                const uint64_t w = k >= 64 ? (uint64_t)(sum < rk_) : (sum >> k) & 1ull;
+                kbits |= w << ci++;
+            }
+            for (int t = 0; t < a.n_kb_spec; ++t) {
+                uint64_t bit = 0;
+                if (a.kb_kind[t] == FUSEFSS_KB_R_BIT) bit = (r >> a.kb_arg[t]) & 1ull;
+                kbits |= bit << (a.n_carry + t);
+            }
+            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_KB, lo, hi);
+            const uint64_t s0 = lo & (n_kb >= 64 ? ~0ull : ((1ull << n_kb) - 1ull));
+            put(a.kb, s0, kbits ^ s0);
+        }
+        for (int i = 0; i < a.MA; ++i) {                                   // Beaver triple (a, b, c = ab)
+            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_BV_AB + i, lo, hi);
+            const uint64_t ta = lo & a.mask, tb = hi & a.mask, tc = (ta * tb) & a.mask;
+            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_BV_AB0 + i, lo, hi);
+            const uint64_t a0 = lo & a.mask, b0 = hi & a.mask;
+            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_BV_C0 + i, lo, hi);
+            const uint64_t c0 = lo & a.mask;
+            const size_t o = a.beaver + (size_t)3 * i * a.s8;
+            put(o, a0, (ta - a0) & a.mask);
+            put(o + a.s8, b0, (tb - b0) & a.mask);
+            put(o + 2 * a.s8, c0, (tc - c0) & a.mask);
+        }
+        if (a.MB > 0) {                                                    // AND triples, gate i = bit i
+            const uint64_t bm = a.MB >= 64 ? ~0ull : ((1ull << a.MB) - 1ull);
+            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_AND_AB, lo, hi);
+            const uint64_t ta = lo & bm, tb = hi & bm, tc = ta & tb;
+            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_AND_AB0, lo, hi);
+            const uint64_t a0 = lo & bm, b0 = hi & bm;
+            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_AND_C0, lo, hi);
+            const uint64_t c0 = lo & bm;
+            put(a.andt, a0, ta ^ a0);
+            put(a.andt + a.s8, b0, tb ^ b0);
+            put(a.andt + 2 * a.s8, c0, tc ^ c0);
+        }
+        if (a.GMIX > 0) {                                                  // B2A pairs (<rho>, [rho])
+            const uint64_t bm = a.GMIX >= 64 ? ~0ull : ((1ull << a.GMIX) - 1ull);
+            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_B2A, lo, hi);
+            const uint64_t rho = lo & bm, rho0 = hi & bm;
+            put(a.b2a_bits, rho0, rho ^ rho0);
+            for (int i = 0; i < a.GMIX; ++i) {
+                dealer_rand<NTAB>(tl, a.rk, ge, SLOT_B2A_A0 + i, lo, hi);
+                const uint64_t s0 = lo & a.mask, val = (rho >> i) & 1ull;
+                put(a.b2a_a + (size_t)i * a.s8, s0, (val - s0) & a.mask);
+            }
+        }
+    }
+}
+
+}  // namespace fsk

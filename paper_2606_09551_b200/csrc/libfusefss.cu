@@ -1,0 +1,513 @@
+// libfusefss.cu -- C ABI entry points (include/fusefss.h) and kernel launchers.  sm_100a only.
+#include <cuda_runtime.h>
+
+#include <atomic>
+#include <cstdio>
+#include <cstdlib>
+#include <mutex>
+
+#include "program.h"
+#include "aes.cuh"
+#include "eval.cuh"
+#include "keygen.cuh"
+#include "post.cuh"
+
+namespace fsk {
+namespace {
+
+thread_local char g_cuda_err[256] = "";
+std::atomic<uint64_t> g_launches{0};
+std::once_flag g_init_once;
+int g_init_status = 0;
+int g_ntab = 4;
+int g_sms = 148;
+int g_eval_threads = kEvalThreads;
+const HostAes &host_aes() { static HostAes h; return h; }
+
+int cuda_fail(cudaError_t e, const char *what) {
+    std::snprintf(g_cuda_err, sizeof g_cuda_err, "%s: %s", what, cudaGetErrorString(e));
+    return FUSEFSS_E_CUDA;
+}
+#define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, #call); } while (0)
+
+template <typename K> int allow_smem(K kernel, size_t bytes) {
+    CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    return 0;
+}
+
+// one-time: PRG round keys + T0 into constant memory, opt-in shared memory sizes, SM count, tuning knobs
+int init_device() {
+    std::call_once(g_init_once, [] {
+        auto body = []() -> int {
+            const HostAes &h = host_aes();
+            uint32_t rk[kNumPrgKeys][44];
+            for (int i = 0; i < kNumPrgKeys; ++i) {
+                uint8_t key[16];
+                for (int j = 0; j < 16; ++j) key[j] = (uint8_t)j;
+                key[0] = (uint8_t)i;
+                h.expand(key, rk[i]);
+            }
+            CU(cudaMemcpyToSymbol(c_T0, h.T0, sizeof h.T0));
+            CU(cudaMemcpyToSymbol(c_rk, rk, sizeof rk));
+            int dev = 0;
+            CU(cudaGetDevice(&dev));
+            CU(cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev));
+            if (const char *s = std::getenv("FUSEFSS_NTAB")) g_ntab = std::atoi(s) == 1 ? 1 : 4;
+            if (const char *s = std::getenv("FUSEFSS_EVAL_THREADS")) {
+                int v = std::atoi(s);
+                if (v >= 32 && v <= kEvalThreads && v % 32 == 0) g_eval_threads = v;
+            }
+            return 0;
+        };
+        g_init_status = body();
+    });
+    return g_init_status;
+}
+
+// number of tree groups G in [1, gmax]: the smallest G whose last wave is >= 97 % full, else the best one
+int pick_groups(size_t count, int gmax, int threads) {
+    if (const char *f = std::getenv("FUSEFSS_FORCE_G")) {          // test hook: force the tree-group count
+        int v = std::atoi(f);
+        if (v >= 1) return v < gmax ? v : gmax;
+    }
+    const double warps = (double)g_sms * (threads / 32);
+    const double tiles = (double)((count + 31) / 32);
+    int best = 1; double best_eff = 0;
+    for (int G = 1; G <= gmax; ++G) {
+        const double waves = tiles * G / warps;
+        const double eff = waves / (double)(size_t)(waves + 0.999999);
+        if (eff >= 0.97) return G;
+        if (eff > best_eff + 1e-9) { best_eff = eff; best = G; }
+    }
+    return best;
+}
+
+int grid_for(size_t warp_items, int threads) {
+    size_t blocks = (warp_items + (threads / 32) - 1) / (threads / 32);
+    if (blocks > (size_t)g_sms) blocks = (size_t)g_sms;
+    return blocks ? (int)blocks : 1;
+}
+
+// lazily upload the small per-program tables (post program, alpha, payload table)
+int ensure_blob(Program &P) {
+    if (P.dev_blob) return 0;
+    auto up = [](size_t x) { return (x + 255) & ~(size_t)255; };
+    P.dev_ins_off = 0;
+    P.dev_alpha_off = up(P.ins.size() * sizeof(Ins));
+    P.dev_payload_off = P.dev_alpha_off + up(P.alpha.size() * 8 + 8);
+    P.dev_blob_bytes = P.dev_payload_off + up(P.payload.size() * 8 + 8);
+    void *d = nullptr;
+    CU(cudaMalloc(&d, P.dev_blob_bytes));
+    std::vector<uint8_t> h(P.dev_blob_bytes, 0);
+    if (!P.ins.empty()) std::memcpy(h.data() + P.dev_ins_off, P.ins.data(), P.ins.size() * sizeof(Ins));
+    if (!P.alpha.empty()) std::memcpy(h.data() + P.dev_alpha_off, P.alpha.data(), P.alpha.size() * 8);
+    if (!P.payload.empty()) std::memcpy(h.data() + P.dev_payload_off, P.payload.data(), P.payload.size() * 8);
+    cudaError_t e = cudaMemcpy(d, h.data(), P.dev_blob_bytes, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { cudaFree(d); return cuda_fail(e, "cudaMemcpy(program tables)"); }
+    P.dev_blob = d;
+    return 0;
+}
+
+RoundKeys seed_round_keys(uint64_t seed) {
+    uint8_t key[16];
+    const uint64_t inv = ~seed;
+    for (int i = 0; i < 8; ++i) { key[i] = (uint8_t)(seed >> (8 * i)); key[8 + i] = (uint8_t)(inv >> (8 * i)); }
+    RoundKeys rk;
+    host_aes().expand(key, rk.w);
+    return rk;
+}
+
+template <typename K, typename A> int launch(K kernel, int grid, int block, size_t smem, cudaStream_t st, const A &args) {
+    if (smem > 48 * 1024) { int rc = allow_smem(kernel, smem); if (rc) return rc; }
+    kernel<<<grid, block, smem, st>>>(args);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    CU(cudaGetLastError());
+    return 0;
+}
+
+// ---- dispatch on (NTAB, P) -------------------------------------------------------------------------
+template <int NTAB> int launch_eval_lut_p(int p, int grid, int block, cudaStream_t st, const EvalLutArgs &a) {
+    const size_t sm = aes_smem_bytes<NTAB>();
+    switch (p) {
+    case 1: return launch(k_eval_lut<NTAB, 1>, grid, block, sm, st, a);
+    case 2: return launch(k_eval_lut<NTAB, 2>, grid, block, sm, st, a);
+    case 3: return launch(k_eval_lut<NTAB, 3>, grid, block, sm, st, a);
+    case 4: return launch(k_eval_lut<NTAB, 4>, grid, block, sm, st, a);
+    case 5: return launch(k_eval_lut<NTAB, 5>, grid, block, sm, st, a);
+    case 6: return launch(k_eval_lut<NTAB, 6>, grid, block, sm, st, a);
+    case 7: return launch(k_eval_lut<NTAB, 7>, grid, block, sm, st, a);
+    case 8: return launch(k_eval_lut<NTAB, 8>, grid, block, sm, st, a);
+    }
+    return FUSEFSS_E_SPEC;
+}
+template <int NTAB> int launch_gen_vec_p(int p, int grid, int block, cudaStream_t st, const GenVecArgs &a) {
+    const size_t sm = aes_smem_bytes<NTAB>();
+    switch (p) {
+    case 1: return launch(k_gen_vec<NTAB, 1>, grid, block, sm, st, a);
+    case 2: return launch(k_gen_vec<NTAB, 2>, grid, block, sm, st, a);
+    case 3: return launch(k_gen_vec<NTAB, 3>, grid, block, sm, st, a);
+    case 4: return launch(k_gen_vec<NTAB, 4>, grid, block, sm, st, a);
+    case 5: return launch(k_gen_vec<NTAB, 5>, grid, block, sm, st, a);
+    case 6: return launch(k_gen_vec<NTAB, 6>, grid, block, sm, st, a);
+    case 7: return launch(k_gen_vec<NTAB, 7>, grid, block, sm, st, a);
+    case 8: return launch(k_gen_vec<NTAB, 8>, grid, block, sm, st, a);
+    }
+    return FUSEFSS_E_SPEC;
+}
+
+PostKeyOff post_offsets(const Layout &L) {
+    return PostKeyOff{L.s8, L.rin, L.rout, L.ka, L.kb, L.beaver, L.andt, L.b2a_bits, L.b2a_a};
+}
+
+}  // namespace
+}  // namespace fsk
+
+using namespace fsk;
+
+static const Program *prog_of(const fusefss_program *p) { return p ? &p->impl : nullptr; }
+
+extern "C" {
+
+int fusefss_compile(const fusefss_spec *spec, fusefss_program **out) {
+    if (!spec || !out) return FUSEFSS_E_NULL;
+    Program *P = nullptr;
+    int rc = compile_program(spec, &P);
+    *out = rc == 0 ? reinterpret_cast<fusefss_program *>(P) : nullptr;
+    return rc;
+}
+
+void fusefss_destroy(fusefss_program *prog) {
+    if (!prog) return;
+    if (prog->impl.dev_blob) cudaFree(prog->impl.dev_blob);
+    delete prog;
+}
+
+int fusefss_shape(const fusefss_program *prog, fusefss_shape_t *out) {
+    const Program *P = prog_of(prog);
+    if (!P || !out) return FUSEFSS_E_NULL;
+    *out = fusefss_shape_t{};
+    out->T = P->T; out->M = P->M; out->p = P->p; out->M_A = P->MA; out->M_B = P->MB; out->G_mix = P->GMIX;
+    out->rounds = P->rounds; out->n_out_a = P->n_out_a; out->n_out_b = P->n_out_b; out->has_lut = P->has_lut;
+    out->n_kb = P->n_kb;
+    for (int t = 0; t < P->T; ++t) out->k[t] = P->atoms[t].k;
+    return 0;
+}
+
+int fusefss_atom(const fusefss_program *prog, int t, uint64_t *out4) {
+    const Program *P = prog_of(prog);
+    if (!P || !out4) return FUSEFSS_E_NULL;
+    if (t < 0 || t >= P->T) return FUSEFSS_E_SPEC;
+    out4[0] = (uint64_t)P->atoms[t].k; out4[1] = P->atoms[t].c; out4[2] = (uint64_t)P->atoms[t].is_theta; out4[3] = P->atoms[t].beta;
+    return 0;
+}
+
+size_t fusefss_key_bytes(const fusefss_program *prog, size_t count) {
+    const Program *P = prog_of(prog);
+    if (!P) return 0;
+    Layout L; compute_layout(*P, count, &L);
+    return L.total;
+}
+
+int fusefss_post_rounds(const fusefss_program *prog) { return prog ? prog->impl.rounds : FUSEFSS_E_NULL; }
+
+size_t fusefss_post_msg_bytes(const fusefss_program *prog, size_t count, int round) {
+    return prog ? post_msg_bytes(prog->impl, count, round) : 0;
+}
+
+size_t fusefss_online_bits(const fusefss_program *prog) {
+    const Program *P = prog_of(prog);
+    if (!P) return 0;
+    return (size_t)P->n + (size_t)2 * P->n * P->MA + (size_t)2 * P->MB + (size_t)P->GMIX +
+           (P->mask_output ? (size_t)P->n * P->n_out_a : 0);
+}
+
+const char *fusefss_strerror(int code) {
+    switch (code) {
+    case FUSEFSS_OK: return "ok";
+    case FUSEFSS_E_NULL: return "null pointer";
+    case FUSEFSS_E_SPEC: return "ill-formed operator specification or compiled limit exceeded";
+    case FUSEFSS_E_PARTY: return "party must be 0 or 1";
+    case FUSEFSS_E_COUNT: return "count must be > 0";
+    case FUSEFSS_E_ROUND: return "round out of range";
+    case FUSEFSS_E_CUDA: return "CUDA error (see fusefss_last_cuda_error)";
+    case FUSEFSS_E_OMITTED: return "call omitted for this gate type (T = 0 or m = 1)";
+    }
+    return "unknown error";
+}
+const char *fusefss_last_cuda_error(void) { return g_cuda_err; }
+uint64_t fusefss_launch_count(void) { return g_launches.load(); }
+
+int fusefss_keygen(const fusefss_program *prog, const uint64_t *r_in_dev, const uint64_t *r_out_dev, uint64_t seed,
+                   uint64_t first_elem, size_t count, void *key0_dev, void *key1_dev, void *stream) {
+    Program *P = const_cast<Program *>(prog_of(prog));
+    if (!P || !r_in_dev || !key0_dev || !key1_dev) return FUSEFSS_E_NULL;
+    if (P->mask_output && !r_out_dev) return FUSEFSS_E_NULL;
+    if (count == 0) return FUSEFSS_E_COUNT;
+    int rc = init_device(); if (rc) return rc;
+    rc = ensure_blob(*P); if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    Layout L; compute_layout(*P, count, &L);
+    const RoundKeys rk = seed_round_keys(seed);
+    const uint8_t *blob = (const uint8_t *)P->dev_blob;
+    const uint64_t *alpha_dev = (const uint64_t *)(blob + P->dev_alpha_off);
+    const uint64_t *payload_dev = (const uint64_t *)(blob + P->dev_payload_off);
+    const size_t tiles = (count + 31) / 32;
+    const size_t smem = g_ntab == 4 ? aes_smem_bytes<4>() : aes_smem_bytes<1>();
+    if (P->T > 0) {
+        GenBitArgs a{};
+        a.key0 = (uint8_t *)key0_dev; a.key1 = (uint8_t *)key1_dev; a.r_in = r_in_dev;
+        a.count = count; a.s16 = L.s16; a.first_elem = first_elem; a.mask = P->mask; a.T = P->T; a.rk = rk;
+        for (int t = 0; t < P->T; ++t)
+            a.atom[t] = GenAtomDev{P->atoms[t].c, P->atoms[t].beta, L.bt_root[t], L.bt_cw[t], L.bt_vb[t], P->atoms[t].k, P->atoms[t].is_theta};
+        const int grid = grid_for(tiles * P->T, kGenThreads);
+        rc = g_ntab == 4 ? launch(k_gen_bit<4>, grid, kGenThreads, smem, st, a) : launch(k_gen_bit<1>, grid, kGenThreads, smem, st, a);
+        if (rc) return rc;
+    }
+    if (P->has_lut) {
+        GenVecArgs a{};
+        a.key0 = (uint8_t *)key0_dev; a.key1 = (uint8_t *)key1_dev; a.r_in = r_in_dev; a.alpha = alpha_dev; a.payload = payload_dev;
+        a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.vt_first = L.vt_first; a.vt_stride = L.vt_stride; a.lvl_stride = L.lvl_stride;
+        a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel; a.first_elem = first_elem; a.mask = P->mask;
+        a.n = (int)P->n; a.m = (int)P->m; a.M = P->M; a.rk = rk;
+        const int grid = grid_for(tiles * (size_t)(P->M - 1), kGenThreads);
+        rc = g_ntab == 4 ? launch_gen_vec_p<4>(P->p, grid, kGenThreads, st, a) : launch_gen_vec_p<1>(P->p, grid, kGenThreads, st, a);
+        if (rc) return rc;
+    }
+    {
+        GenMiscArgs a{};
+        a.key0 = (uint8_t *)key0_dev; a.key1 = (uint8_t *)key1_dev; a.r_in = r_in_dev; a.r_out = r_out_dev;
+        a.alpha = alpha_dev; a.payload = payload_dev;
+        a.count = count; a.s8 = L.s8; a.lut_c = L.lut_c; a.rin = L.rin; a.rout = L.rout; a.ka = L.ka; a.kb = L.kb;
+        a.beaver = L.beaver; a.andt = L.andt; a.b2a_bits = L.b2a_bits; a.b2a_a = L.b2a_a;
+        a.first_elem = first_elem; a.mask = P->mask;
+        a.n = (int)P->n; a.m = (int)P->m; a.M = P->M; a.p = P->p; a.has_lut = P->has_lut; a.mask_output = (int)P->mask_output;
+        a.n_out_a = P->n_out_a; a.n_ka = (int)P->kappa_a.size(); a.n_kb_spec = (int)P->kappa_b.size(); a.n_carry = P->n_carry;
+        a.T = P->T; a.MA = P->MA; a.MB = P->MB; a.GMIX = P->GMIX; a.rk = rk;
+        if (a.n_ka > 8) return FUSEFSS_E_SPEC;
+        for (int t = 0; t < a.n_ka; ++t) { a.ka_kind[t] = P->kappa_a[t].kind; a.ka_arg[t] = P->kappa_a[t].arg; }
+        for (int t = 0; t < a.n_kb_spec; ++t) { a.kb_kind[t] = P->kappa_b[t].kind; a.kb_arg[t] = P->kappa_b[t].arg; }
+        for (int t = 0; t < P->T; ++t)
+            a.atom[t] = GenAtomDev{P->atoms[t].c, P->atoms[t].beta, 0, 0, 0, P->atoms[t].k, P->atoms[t].is_theta};
+        const int grid = grid_for(tiles, kGenThreads);
+        rc = g_ntab == 4 ? launch(k_gen_misc<4>, grid, kGenThreads, smem, st, a) : launch(k_gen_misc<1>, grid, kGenThreads, smem, st, a);
+        if (rc) return rc;
+    }
+    return 0;
+}
+
+int fusefss_eval_cmp(int party, const fusefss_program *prog, const void *key_dev, const uint64_t *xhat_dev, size_t count,
+                     uint64_t *bits_out_dev, void *stream) {
+    const Program *P = prog_of(prog);
+    if (!P || !key_dev || !xhat_dev || !bits_out_dev) return FUSEFSS_E_NULL;
+    if (party != 0 && party != 1) return FUSEFSS_E_PARTY;
+    if (count == 0) return FUSEFSS_E_COUNT;
+    if (P->T == 0) return FUSEFSS_E_OMITTED;
+    int rc = init_device(); if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    Layout L; compute_layout(*P, count, &L);
+    EvalCmpArgs a{};
+    a.key = (const uint8_t *)key_dev; a.xhat = xhat_dev; a.out = bits_out_dev; a.count = count; a.s16 = L.s16;
+    a.T = P->T; a.party = party;
+    a.G = pick_groups(count, P->T, g_eval_threads);
+    for (int t = 0; t < P->T; ++t) a.atom[t] = CmpAtomDev{P->atoms[t].c, L.bt_root[t], L.bt_cw[t], L.bt_vb[t], P->atoms[t].k, 0};
+    if (a.G > 1) CU(cudaMemsetAsync(bits_out_dev, 0, count * 8, st));
+    const int grid = grid_for(((count + 31) / 32) * (size_t)a.G, g_eval_threads);
+    return g_ntab == 4 ? launch(k_eval_cmp<4>, grid, g_eval_threads, aes_smem_bytes<4>(), st, a)
+                       : launch(k_eval_cmp<1>, grid, g_eval_threads, aes_smem_bytes<1>(), st, a);
+}
+
+int fusefss_eval_lut(int party, const fusefss_program *prog, const void *key_dev, const uint64_t *xhat_dev, size_t count,
+                     uint64_t *coeff_out_dev, void *stream) {
+    const Program *P = prog_of(prog);
+    if (!P || !key_dev || !xhat_dev || !coeff_out_dev) return FUSEFSS_E_NULL;
+    if (party != 0 && party != 1) return FUSEFSS_E_PARTY;
+    if (count == 0) return FUSEFSS_E_COUNT;
+    if (!P->has_lut) return FUSEFSS_E_OMITTED;
+    int rc = init_device(); if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    Layout L; compute_layout(*P, count, &L);
+    EvalLutArgs a{};
+    a.key = (const uint8_t *)key_dev; a.xhat = xhat_dev; a.out = coeff_out_dev;
+    a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.lut_c = L.lut_c; a.vt_first = L.vt_first; a.vt_stride = L.vt_stride;
+    a.lvl_stride = L.lvl_stride; a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel;
+    a.mask = P->mask; a.n = (int)P->n; a.M = P->M; a.party = party;
+    a.G = pick_groups(count, P->M - 1, g_eval_threads);
+    if (a.G > 1) CU(cudaMemsetAsync(coeff_out_dev, 0, count * 8 * (size_t)P->p, st));
+    const int grid = grid_for(((count + 31) / 32) * (size_t)a.G, g_eval_threads);
+    rc = g_ntab == 4 ? launch_eval_lut_p<4>(P->p, grid, g_eval_threads, st, a) : launch_eval_lut_p<1>(P->p, grid, g_eval_threads, st, a);
+    if (rc) return rc;
+    if (a.G > 1 && P->n < 64) {
+        const size_t words = count * (size_t)P->p;
+        return launch(k_mask_words, (int)((words + 255) / 256), 256, 0, st, MaskArgs{coeff_out_dev, words, P->mask});
+    }
+    return 0;
+}
+
+
+int fusefss_post(int party, const fusefss_program *prog, const void *key_dev, const uint64_t *xhat_dev,
+                 const uint64_t *bits_dev, const uint64_t *coeff_dev, size_t count, int round, const void *msg_in_dev,
+                 void *msg_out_dev, uint64_t *y_out_dev, uint64_t *z_out_dev, void *stream) {
+    Program *P = const_cast<Program *>(prog_of(prog));
+    if (!P || !key_dev || !xhat_dev) return FUSEFSS_E_NULL;
+    if (party != 0 && party != 1) return FUSEFSS_E_PARTY;
+    if (count == 0) return FUSEFSS_E_COUNT;
+    if (round < 0 || round > P->rounds) return FUSEFSS_E_ROUND;
+    if ((P->T > 0 && !bits_dev) || (P->has_lut && !coeff_dev)) return FUSEFSS_E_NULL;
+    if (round < P->rounds && !msg_out_dev) return FUSEFSS_E_NULL;
+    if (round > 0 && !msg_in_dev) return FUSEFSS_E_NULL;
+    if (round == P->rounds && ((P->n_out_a > 0 && !y_out_dev) || (P->n_out_b > 0 && !z_out_dev))) return FUSEFSS_E_NULL;
+    int rc = init_device(); if (rc) return rc;
+    rc = ensure_blob(*P); if (rc) return rc;
+    Layout L; compute_layout(*P, count, &L);
+    PostArgs a{};
+    a.ins = (const Ins *)((const uint8_t *)P->dev_blob + P->dev_ins_off); a.n_ins = (int)P->ins.size();
+    a.party = party; a.round = round; a.rounds = P->rounds; a.mask_output = (int)P->mask_output;
+    a.n_out_a = P->n_out_a; a.n_out_b = P->n_out_b;
+    a.key = (const uint8_t *)key_dev; a.xhat = xhat_dev; a.bits = bits_dev; a.coeff = coeff_dev;
+    a.msg_in = (const uint8_t *)msg_in_dev; a.msg_out = (uint8_t *)msg_out_dev; a.y_out = y_out_dev; a.z_out = z_out_dev;
+    a.count = count; a.mask = P->mask; a.k = post_offsets(L);
+    a.round_off[0] = 0;
+    for (int q = 0; q < kMaxRounds; ++q) {
+        a.round_off[q + 1] = a.round_off[q] + post_msg_bytes(*P, count, q);
+        a.round_mul[q] = P->round_mul[q]; a.round_bits[q] = P->round_bits[q];
+    }
+    return launch(k_post_round, (int)((count + 255) / 256), 256, 0, (cudaStream_t)stream, a);
+}
+
+int fusefss_post_fused(const fusefss_program *prog, const void *key0_dev, const void *key1_dev, const uint64_t *xhat_dev,
+                       const uint64_t *bits0_dev, const uint64_t *bits1_dev, const uint64_t *coeff0_dev,
+                       const uint64_t *coeff1_dev, size_t count, uint64_t *y0_dev, uint64_t *y1_dev, uint64_t *z0_dev,
+                       uint64_t *z1_dev, void *stream) {
+    Program *P = const_cast<Program *>(prog_of(prog));
+    if (!P || !key0_dev || !key1_dev || !xhat_dev) return FUSEFSS_E_NULL;
+    if (count == 0) return FUSEFSS_E_COUNT;
+    if ((P->T > 0 && (!bits0_dev || !bits1_dev)) || (P->has_lut && (!coeff0_dev || !coeff1_dev))) return FUSEFSS_E_NULL;
+    if ((P->n_out_a > 0 && (!y0_dev || !y1_dev)) || (P->n_out_b > 0 && (!z0_dev || !z1_dev))) return FUSEFSS_E_NULL;
+    int rc = init_device(); if (rc) return rc;
+    rc = ensure_blob(*P); if (rc) return rc;
+    Layout L; compute_layout(*P, count, &L);
+    PostFusedArgs a{};
+    a.ins = (const Ins *)((const uint8_t *)P->dev_blob + P->dev_ins_off); a.n_ins = (int)P->ins.size();
+    a.mask_output = (int)P->mask_output; a.n_out_a = P->n_out_a; a.n_out_b = P->n_out_b;
+    a.key[0] = (const uint8_t *)key0_dev; a.key[1] = (const uint8_t *)key1_dev; a.xhat = xhat_dev;
+    a.bits[0] = bits0_dev; a.bits[1] = bits1_dev; a.coeff[0] = coeff0_dev; a.coeff[1] = coeff1_dev;
+    a.y_out[0] = y0_dev; a.y_out[1] = y1_dev; a.z_out[0] = z0_dev; a.z_out[1] = z1_dev;
+    a.count = count; a.mask = P->mask; a.k = post_offsets(L);
+    return launch(k_post_fused, (int)((count + 255) / 256), 256, 0, (cudaStream_t)stream, a);
+}
+
+// workspace: key0 | key1 | r_in | r_out[n_out_a] | xhat | bits0 | bits1 | coeff0[p] | coeff1[p] | y0 | y1 [n_out_a] | z0 | z1
+static size_t ws_u64_arrays(const Program &P) { return 1 + 1 + 2 + 2 + (size_t)2 * P.p + (size_t)3 * (P.n_out_a > 0 ? P.n_out_a : 1); }
+
+size_t fusefss_gate_workspace_bytes(const fusefss_program *prog, size_t chunk) {
+    const Program *P = prog_of(prog);
+    if (!P || chunk == 0) return 0;
+    Layout L; compute_layout(*P, chunk, &L);
+    return 2 * L.total + ws_u64_arrays(*P) * L.s8;
+}
+
+int fusefss_gate_host(const fusefss_program *prog, const uint64_t *r_in, const uint64_t *r_out, const uint64_t *xhat,
+                      uint64_t seed, size_t count, size_t chunk, void *workspace_dev, uint64_t *y0, uint64_t *y1,
+                      uint64_t *z0, uint64_t *z1, void *stream) {
+    const Program *P = prog_of(prog);
+    if (!P || !r_in || !xhat || !workspace_dev) return FUSEFSS_E_NULL;
+    if (P->mask_output && !r_out) return FUSEFSS_E_NULL;
+    if ((P->n_out_a > 0 && (!y0 || !y1)) || (P->n_out_b > 0 && (!z0 || !z1))) return FUSEFSS_E_NULL;
+    if (count == 0 || chunk == 0) return FUSEFSS_E_COUNT;
+    cudaStream_t st = (cudaStream_t)stream;
+    Layout L; compute_layout(*P, chunk, &L);
+    const int na = P->n_out_a > 0 ? P->n_out_a : 1;
+    uint8_t *ws = (uint8_t *)workspace_dev;
+    uint8_t *key0 = ws, *key1 = ws + L.total;
+    uint8_t *q = ws + 2 * L.total;
+    auto take = [&](size_t arrays) { uint64_t *r = (uint64_t *)q; q += arrays * L.s8; return r; };
+    uint64_t *d_rin = take(1), *d_rout = take(na), *d_xhat = take(1), *d_b0 = take(1), *d_b1 = take(1);
+    uint64_t *d_c0 = take(P->p), *d_c1 = take(P->p), *d_y0 = take(na), *d_y1 = take(na), *d_z0 = take(1), *d_z1 = take(1);
+    for (size_t first = 0; first < count; first += chunk) {
+        const size_t c = count - first < chunk ? count - first : chunk;
+        CU(cudaMemcpyAsync(d_rin, r_in + first, c * 8, cudaMemcpyHostToDevice, st));
+        CU(cudaMemcpyAsync(d_xhat, xhat + first, c * 8, cudaMemcpyHostToDevice, st));
+        if (P->mask_output)
+            for (int j = 0; j < P->n_out_a; ++j)
+                CU(cudaMemcpyAsync(d_rout + (size_t)j * c, r_out + (size_t)j * count + first, c * 8, cudaMemcpyHostToDevice, st));
+        int rc = fusefss_keygen(prog, d_rin, d_rout, seed, first, c, key0, key1, st); if (rc) return rc;
+        if (P->T > 0) {
+            rc = fusefss_eval_cmp(0, prog, key0, d_xhat, c, d_b0, st); if (rc) return rc;
+            rc = fusefss_eval_cmp(1, prog, key1, d_xhat, c, d_b1, st); if (rc) return rc;
+        }
+        if (P->has_lut) {
+            rc = fusefss_eval_lut(0, prog, key0, d_xhat, c, d_c0, st); if (rc) return rc;
+            rc = fusefss_eval_lut(1, prog, key1, d_xhat, c, d_c1, st); if (rc) return rc;
+        }
+        rc = fusefss_post_fused(prog, key0, key1, d_xhat, d_b0, d_b1, d_c0, d_c1, c, d_y0, d_y1, d_z0, d_z1, st); if (rc) return rc;
+        for (int j = 0; j < P->n_out_a; ++j) {
+            CU(cudaMemcpyAsync(y0 + (size_t)j * count + first, d_y0 + (size_t)j * c, c * 8, cudaMemcpyDeviceToHost, st));
+            CU(cudaMemcpyAsync(y1 + (size_t)j * count + first, d_y1 + (size_t)j * c, c * 8, cudaMemcpyDeviceToHost, st));
+        }
+        if (P->n_out_b > 0) {
+            CU(cudaMemcpyAsync(z0 + first, d_z0, c * 8, cudaMemcpyDeviceToHost, st));
+            CU(cudaMemcpyAsync(z1 + first, d_z1, c * 8, cudaMemcpyDeviceToHost, st));
+        }
+    }
+    CU(cudaStreamSynchronize(st));
+    return 0;
+}
+
+}  // extern "C"
+
+// ---- PRG micro-kernels: roofline denominator probe and FIPS-197 known-answer path --------------------
+namespace fsk {
+struct ProbeArgs { uint4 *out; size_t threads; int iters; };
+template <int NTAB>
+__global__ void __launch_bounds__(kEvalThreads, 1) k_aes_probe(const ProbeArgs a) {
+    extern __shared__ uint32_t sT[];
+    aes_fill_tables<NTAB>(sT);
+    const uint32_t *tl = sT + (threadIdx.x & 31);
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < a.threads; i += (size_t)gridDim.x * blockDim.x) {
+        uint32_t x[1][4] = {{(uint32_t)i, (uint32_t)(i >> 32), 0x9e3779b9u, 0x7f4a7c15u}};
+        for (int it = 0; it < a.iters; it += 3) {                       // 3 independent keys per trip, like a p = 3 level
+            uint32_t o[1][3][4];
+            prg_blocks<NTAB, 1, 3, 0>(tl, x, o);
+#pragma unroll
+            for (int c = 0; c < 4; ++c) x[0][c] = o[0][0][c] ^ o[0][1][(c + 1) & 3] ^ o[0][2][(c + 2) & 3];
+        }
+        a.out[i] = make_uint4(x[0][0], x[0][1], x[0][2], x[0][3]);
+    }
+}
+struct KatArgs { uint4 *out; uint32_t in[4]; RoundKeys rk; };
+template <int NTAB>
+__global__ void k_aes_kat(const KatArgs a) {
+    extern __shared__ uint32_t sT[];
+    aes_fill_tables<NTAB>(sT);
+    if (threadIdx.x == 0) {
+        uint32_t s[4] = {a.in[0], a.in[1], a.in[2], a.in[3]};
+        aes_encrypt_rk<NTAB>(sT + 0, a.rk, s);
+        a.out[0] = make_uint4(s[0], s[1], s[2], s[3]);
+    }
+}
+}  // namespace fsk
+
+extern "C" {
+
+int fusefss_aes_probe(size_t threads, int iters, void *out_dev, void *stream) {
+    if (!out_dev) return FUSEFSS_E_NULL;
+    if (threads == 0 || iters <= 0) return FUSEFSS_E_COUNT;
+    int rc = init_device(); if (rc) return rc;
+    ProbeArgs a{(uint4 *)out_dev, threads, iters};
+    const int grid = grid_for((threads + 31) / 32, g_eval_threads);
+    return g_ntab == 4 ? launch(k_aes_probe<4>, grid, g_eval_threads, aes_smem_bytes<4>(), (cudaStream_t)stream, a)
+                       : launch(k_aes_probe<1>, grid, g_eval_threads, aes_smem_bytes<1>(), (cudaStream_t)stream, a);
+}
+
+int fusefss_aes_kat(const uint8_t *key, const uint8_t *in, void *out_dev, void *stream) {
+    if (!key || !in || !out_dev) return FUSEFSS_E_NULL;
+    int rc = init_device(); if (rc) return rc;
+    KatArgs a{};
+    a.out = (uint4 *)out_dev;
+    std::memcpy(a.in, in, 16);
+    host_aes().expand(key, a.rk.w);
+    return g_ntab == 4 ? launch(k_aes_kat<4>, 1, 256, aes_smem_bytes<4>(), (cudaStream_t)stream, a)
+                       : launch(k_aes_kat<1>, 1, 256, aes_smem_bytes<1>(), (cudaStream_t)stream, a);
+}
+
+}  // extern "C"

@@ -1,0 +1,83 @@
+// program.h -- compiled gate type shared by the host compiler (compile.cpp) and the kernel launchers.
+// Product code: independent of oracle/ (DESIGN.md section 3).  Format definitions: DESIGN.md section 4.
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <vector>
+
+#include "../../include/fusefss.h"
+
+namespace fsk {
+
+constexpr int kMaxAtoms = 64;      // T <= 64: one packed word of share bits per element
+constexpr int kMaxP = 8;           // payload words p
+constexpr int kMaxIntervals = 64;  // m < 64
+constexpr int kMaxRounds = 16;
+constexpr int kMaxAReg = 48;       // arithmetic registers after allocation (device local array)
+constexpr int kMaxBReg = 64;       // bit registers after allocation (one 64-bit word per party)
+
+// One query of the packed comparison instance (Def I.1).
+struct Atom {
+    int k;              // view width k_t
+    uint64_t c;         // view offset c_t
+    int is_theta;       // 0: r-atom (threshold r mod 2^k), 1: theta-atom (threshold (r_k + beta) mod 2^k)
+    uint64_t beta;
+    int carry;          // index of the carry bit w_t inside kappa^B, -1 for r-atoms
+};
+
+// Post-processing instruction (DESIGN 4.3 "post program").  Interactive gates carry their gate number
+// (`gate`), their round and their position inside that round's message (`pos`).
+enum : uint8_t {
+    I_B_CONST = 1, I_B_ATOM, I_B_KAPPA, I_B_XHAT, I_B_NOT, I_B_XOR, I_B_AND, I_B_ANDPUB, I_B_OUT,
+    I_A_CONST, I_A_X, I_A_COEFF, I_A_KAPPA, I_A_XHAT_SHR, I_A_ADD, I_A_SUB, I_A_MULC, I_A_MUL, I_A_B2A, I_A_OUT
+};
+struct Ins {
+    uint8_t op;
+    uint8_t round;      // interactive gates only
+    uint16_t dst, a, b;
+    uint16_t gate;      // Beaver / AND / B2A gate number
+    uint16_t pos;       // Beaver: pair index inside the round; AND/B2A: first bit position inside the round's bit word
+    uint32_t pad;
+    uint64_t imm;
+};
+static_assert(sizeof(Ins) == 24, "Ins is uploaded to the device as-is");
+
+// Byte offsets inside one party's key buffer (DESIGN 4.4).
+struct Layout {
+    size_t s16, s8;
+    size_t bt_root[kMaxAtoms], bt_cw[kMaxAtoms], bt_vb[kMaxAtoms];
+    size_t lut_c, vt_first, vt_stride, lvl_stride, vt_lvl_rel, vt_fin_rel;   // vector tree j at vt_first + (j-1)*vt_stride
+    size_t rin, rout, ka, kb, beaver, andt, b2a_bits, b2a_a, total;
+};
+
+struct Program {
+    // deep copy of the specification
+    uint32_t n = 0, frac_bits = 0, m = 0, r = 0, d = 0, p_aux = 0, ell = 0, mask_output = 0;
+    std::vector<uint64_t> alpha, coeff, aux;
+    std::vector<fusefss_bitnode> nodes;
+    std::vector<uint16_t> bit_root;
+    std::vector<fusefss_kappa> kappa_a, kappa_b;
+    std::vector<fusefss_phi_op> phi;
+    // compiled shape
+    uint64_t mask = 0;
+    int M = 0, p = 0, Q = 0, T = 0, has_lut = 0;
+    int n_carry = 0, n_kb = 0;
+    int MA = 0, MB = 0, GMIX = 0, rounds = 0, n_out_a = 0, n_out_b = 0;
+    Atom atoms[kMaxAtoms];
+    std::vector<Ins> ins;
+    int n_areg = 0, n_breg = 0;
+    int round_mul[kMaxRounds] = {0}, round_bits[kMaxRounds] = {0};
+    // payload table v[i][w], i < m, w < p (coefficients poly-major, high degree first, then aux), masked
+    std::vector<uint64_t> payload;
+    // device copy of the small tables (uploaded lazily by the launchers)
+    void *dev_blob = nullptr;
+    size_t dev_ins_off = 0, dev_alpha_off = 0, dev_payload_off = 0, dev_blob_bytes = 0;
+};
+
+int compile_program(const fusefss_spec *spec, Program **out);
+void compute_layout(const Program &P, size_t count, Layout *L);
+size_t post_msg_bytes(const Program &P, size_t count, int round);
+
+}  // namespace fsk
+
+struct fusefss_program { fsk::Program impl; };

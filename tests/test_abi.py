@@ -1,0 +1,107 @@
+"""Host-side checks of the C-ABI library (no GPU): it loads, exports every symbol include/fusefss.h declares,
+compiles every spec to the shape the paper / the oracle fixes, and reports errors as codes."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from workloads import specs
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def F():
+    import __graft_entry__ as g
+    g.build()
+    import paper_2606_09551_b200 as F
+    return F
+
+
+def test_exports_every_declared_symbol(F):
+    hdr = open(os.path.join(ROOT, "include", "fusefss.h")).read()
+    declared = set(re.findall(r"\b(fusefss_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(F.SYMBOLS)
+    raw = C.CDLL(F.LIB_PATH)
+    for name in declared:
+        assert hasattr(raw, name), name
+
+
+ALL = [("relu16", lambda: specs.relu(16, 8)), ("gelu", specs.gelu), ("nexp", specs.nexp), ("recip", specs.recip),
+       ("shift_relu", specs.shift_relu), ("rsqrt", specs.rsqrt), ("silu", specs.silu),
+       ("toy", lambda: specs.toy(8, 3)), ("toy_masked", lambda: specs.toy(8, 3, True)),
+       ("plain", specs.plain_default), ("single", specs.single_interval), ("nobits", specs.no_bits),
+       ("full", specs.full_partition), ("shift_relu8", lambda: specs.shift_relu(8, 3))]
+
+
+@pytest.mark.parametrize("name,mk", ALL)
+def test_compile_matches_oracle_shape(F, orc, name, mk):
+    """Two independent compilers (DESIGN 4.3): same L_shape, atoms, key size, message sizes."""
+    s = mk()
+    P, O = F.Program(s), orc.Program(s)
+    assert P.shape == O.shape
+    for t in range(P.shape["T"]):
+        assert P.atom(t) == O.atom(t)
+    for count in (1, 31, 32, 33, 4096, 100003):
+        assert P.key_bytes(count) == O.key_bytes(count)
+        for q in range(P.post_rounds() + 1):
+            assert P.post_msg_bytes(count, q) == O.post_msg_bytes(count, q)
+    assert P.post_rounds() == O.post_rounds()
+    assert P.online_bits() == O.online_bits()
+
+
+def test_appendix_N_shape(F):
+    """App. N: T = 2 atoms of width n, M = 3, p = 2, one Beaver multiplication."""
+    P = F.Program(specs.relu(16, 8))
+    assert (P.shape["T"], P.shape["M"], P.shape["p"], P.shape["M_A"], P.shape["M_B"], P.shape["G_mix"]) == (2, 3, 2, 1, 0, 0)
+    assert P.shape["k"] == [16, 16]
+    N = 1 << 16
+    assert P.atom(0) == dict(k=16, c=0, is_theta=0, beta=0)
+    assert P.atom(1) == dict(k=16, c=0, is_theta=1, beta=N // 2)
+
+
+def test_key_bytes_formula(F):
+    """DESIGN 4.4 / SURVEY 8(a): per element per party, unpadded: bitDCF(k) = 16(k+1) + 8, vecDCF(n,p) = 16 + n(16+8p) + 8p."""
+    for mk in (specs.gelu, specs.silu, specs.shift_relu):
+        s = mk()
+        P = F.Program(s)
+        sh = P.shape
+        count = 1 << 20                                          # multiple of 32: no padding
+        per = sum(16 * (k + 1) + 8 for k in sh["k"]) + 8 * sh["p"] + (sh["M"] - 1) * (16 + s.n * (16 + 8 * sh["p"]) + 8 * sh["p"])
+        per += 8 + 8 * len(s.kappa_a) + (8 if sh["n_kb"] else 0) + 24 * sh["M_A"] + (24 if sh["M_B"] else 0) + (8 if sh["G_mix"] else 0) + 8 * sh["G_mix"]
+        assert P.key_bytes(count) == per * count
+
+
+def test_rejects_ill_formed_specs(F):
+    good = specs.relu(16, 8)
+    bad = specs.relu(16, 8)
+    bad.alpha = [0]                                             # boundary must be > 0
+    with pytest.raises(F.FuseFSSError):
+        F.Program(bad)
+    bad2 = specs.toy(8, 3)
+    bad2.alpha = [5, 5, 9]                                      # not strictly increasing
+    with pytest.raises(F.FuseFSSError):
+        F.Program(bad2)
+    bad3 = specs.relu(16, 8)
+    bad3.n = 65
+    with pytest.raises(F.FuseFSSError):
+        F.Program(bad3)
+    assert F.Program(good).shape["T"] == 2
+    assert F.lib.fusefss_key_bytes(None, 10) == 0
+    assert F.lib.fusefss_strerror(-3) == b"party must be 0 or 1"
+
+
+def test_argument_errors_without_gpu(F):
+    P = F.Program(specs.relu(16, 8))
+    # null pointers / bad party / zero count are rejected before any CUDA call
+    assert F.lib.fusefss_eval_cmp(0, P._h, None, None, 10, None, None) == -1
+    assert F.lib.fusefss_eval_cmp(2, P._h, 1, 1, 10, 1, None) == -3
+    assert F.lib.fusefss_eval_lut(0, P._h, 1, 1, 0, 1, None) == -4
+    assert F.lib.fusefss_keygen(P._h, None, None, 0, 0, 10, None, None, None) == -1
+    Pn = F.Program(specs.no_bits())
+    assert F.lib.fusefss_eval_cmp(0, Pn._h, 1, 1, 10, 1, None) == -7     # T = 0: call omitted
+    Ps = F.Program(specs.single_interval())
+    assert F.lib.fusefss_eval_lut(0, Ps._h, 1, 1, 10, 1, None) == -7     # m = 1: call omitted
+    assert F.lib.fusefss_post(0, P._h, 1, 1, 1, 1, 10, 99, 1, 1, 1, 1, None) == -5
