@@ -167,15 +167,20 @@ def main():
     youts = [torch.empty((na, chunk), dtype=torch.int64, device="cuda") for _ in range(2)]
     zouts = [torch.empty(chunk, dtype=torch.int64, device="cuda") for _ in range(2)]
     ev = lambda: torch.cuda.Event(enable_timing=True)
-    t_gen, t_cmp, t_lut, t_post = [], [], [], []
+    t_gen, t_cmp, t_lut, t_post, t_genvec, t_genbit = [], [], [], [], [], []
 
     def step(record):
         for first in range(0, count, chunk):
             c = min(chunk, count - first)
             sl = slice(first, first + c)
-            e = [ev() for _ in range(5)]
+            e = [ev() for _ in range(7)]
+            ro = r_out[:, sl].contiguous() if spec.mask_output else r_out
             e[0].record()
-            P.keygen(r_in[sl], r_out[:, sl].contiguous() if spec.mask_output else r_out, step.seed, first, keys=(k0, k1))
+            P.keygen(r_in[sl], ro, step.seed, first, keys=(k0, k1), parts=1)          # T bit-DCF keys      (k_gen_bit)
+            e[5].record()
+            P.keygen(r_in[sl], ro, step.seed, first, keys=(k0, k1), parts=2)          # M-1 vector-DCF keys (k_gen_vec)
+            e[6].record()
+            P.keygen(r_in[sl], ro, step.seed, first, keys=(k0, k1), parts=4)          # share splitting     (k_gen_misc)
             e[1].record()
             if sh["T"]:
                 for b, k in ((0, k0), (1, k1)):
@@ -219,33 +224,47 @@ def main():
     for e in step.events:
         t_gen.append(e[0].elapsed_time(e[1])); t_cmp.append(e[1].elapsed_time(e[2]))
         t_lut.append(e[2].elapsed_time(e[3])); t_post.append(e[3].elapsed_time(e[4]))
+        t_genbit.append(e[0].elapsed_time(e[5])); t_genvec.append(e[5].elapsed_time(e[6]))
     per_step = lambda ts: sum(ts) / args.steps
     ms_step = ms / args.steps
     value = world * count / (ms_step * 1e-3)
 
-    # ---- roofline of the dominant kernel (k_eval_lut: two launches per chunk, one per party) ----------
+    # ---- roofline: AES-block rate of the dominant kernel against the shared-memory lookup roof (DESIGN 5.2) ----
     aes_eval, aes_gen = aes_per_elem(sh, spec.n)
     Q = (sh["p"] + 1) // 2
-    lut_aes_per_launch = (sh["M"] - 1) * (spec.n * (1 + Q) + Q) * chunk if sh["has_lut"] else 0
-    n_lut_launches = 2 * len(step.events)
-    lut_ms = sum(t_lut) / max(1, n_lut_launches)                      # average launch duration (full chunks dominate)
-    achieved = lut_aes_per_launch / (lut_ms * 1e-3) / 1e9 if lut_ms > 0 else 0.0
+    n_chunks = len(step.events)
+    full_chunk_frac = count / (chunk * ((count + chunk - 1) // chunk))      # tail chunk: fewer blocks per launch
     peak = 148 * SM_CLOCK_MAX_MHZ * 1e6 * LDS_LANES_PER_CLK_SM / LOOKUPS_PER_AES / 1e9
-    key_b = P.key_bytes(1 << 20) / (1 << 20)
-    lut_key_bytes = (8 * sh["p"] + (sh["M"] - 1) * (16 + spec.n * (16 + 8 * sh["p"]) + 8 * sh["p"])) if sh["has_lut"] else 0
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except Exception:
         pass
     hbm_peak = peaks.get("hbm_gbs", 6650.0)
-    roofline = {"bound": "alu", "kernel": "k_eval_lut", "achieved": achieved, "peak": peak, "unit": "GAES/s (AES-128 blocks; 160 conflict-free LDS.32 lookups each)",
-                "frac": achieved / peak if peak else None, "traffic": None,
-                "peak_derivation": "148 SMs x 1.965 GHz x 32 LDS lanes/clk/SM / 160 lookups per AES block (DESIGN 5.2)",
-                "hbm_achieved_gbs": lut_key_bytes * chunk / (lut_ms * 1e-3) / 1e9 if lut_ms > 0 else 0.0,
-                "hbm_peak_gbs": hbm_peak, "hbm_peak_source": "measured" if peaks else "fallback",
-                "launch_ms": lut_ms, "aes_per_launch": lut_aes_per_launch}
-    roofline["hbm_frac"] = roofline["hbm_achieved_gbs"] / hbm_peak
+    key_b = P.key_bytes(1 << 20) / (1 << 20)
+    lut_key_bytes = (8 * sh["p"] + (sh["M"] - 1) * (16 + spec.n * (16 + 8 * sh["p"]) + 8 * sh["p"])) if sh["has_lut"] else 0
+
+    def roof(kernel, aes_per_launch_elem, launches_per_chunk, times, bytes_per_elem):
+        n_launch = launches_per_chunk * n_chunks
+        launch_ms = sum(times) / max(1, n_launch)
+        per_launch = aes_per_launch_elem * chunk * full_chunk_frac
+        ach = per_launch / (launch_ms * 1e-3) / 1e9 if launch_ms > 0 else 0.0
+        gbs = bytes_per_elem * chunk * full_chunk_frac / (launch_ms * 1e-3) / 1e9 if launch_ms > 0 else 0.0
+        return {"bound": "alu", "kernel": kernel, "achieved": ach, "peak": peak,
+                "unit": "GAES/s (AES-128 blocks per second; 160 conflict-free LDS.32 table lookups each)",
+                "frac": ach / peak, "traffic": None,
+                "peak_derivation": "148 SMs x 1.965 GHz x 32 shared-memory lanes/clk/SM / 160 lookups per AES block (DESIGN 5.2)",
+                "launch_ms": launch_ms, "aes_per_launch": per_launch, "share_of_step": sum(times) / (ms_step * args.steps),
+                "hbm_achieved_gbs": gbs, "hbm_peak_gbs": hbm_peak, "hbm_frac": gbs / hbm_peak,
+                "hbm_peak_source": "measured (MEASURED_PEAKS.json)" if peaks else "fallback"}
+    vec_gen_aes = (sh["M"] - 1) * (4 * spec.n * (1 + Q) + 2 * Q + 2) if sh["has_lut"] else 0
+    vec_eval_aes = (sh["M"] - 1) * (spec.n * (1 + Q) + Q) if sh["has_lut"] else 0
+    roofs = {"k_gen_vec": roof("k_gen_vec", vec_gen_aes, 1, t_genvec, 2 * (lut_key_bytes - 8 * sh["p"])),
+             "k_eval_lut": roof("k_eval_lut", vec_eval_aes, 2, t_lut, lut_key_bytes)}
+    dominant = max(roofs.values(), key=lambda r: r["share_of_step"])
+    roofline = dict(dominant)
+    roofline["other_kernels"] = {k: {kk: v[kk] for kk in ("achieved", "frac", "launch_ms", "share_of_step", "hbm_achieved_gbs")}
+                                 for k, v in roofs.items() if v is not dominant}
 
     line = {"metric": METRIC, "value": value, "unit": "elements/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64",
@@ -256,7 +275,7 @@ def main():
             "eval_elems_per_s": world * count / ((per_step(t_cmp) + per_step(t_lut)) * 1e-3),
             "eval_post_elems_per_s": world * count / ((per_step(t_cmp) + per_step(t_lut) + per_step(t_post)) * 1e-3),
             "keygen_elems_per_s": world * count / (per_step(t_gen) * 1e-3),
-            "ms_breakdown": {"keygen": per_step(t_gen), "eval_cmp_x2": per_step(t_cmp), "eval_lut_x2": per_step(t_lut), "post_fused": per_step(t_post)},
+            "ms_breakdown": {"keygen": per_step(t_gen), "keygen_bit": per_step(t_genbit), "keygen_vec": per_step(t_genvec), "eval_cmp_x2": per_step(t_cmp), "eval_lut_x2": per_step(t_lut), "post_fused": per_step(t_post)},
             "key_bytes_per_elem_per_party": key_b, "online_bytes_per_elem_per_party": P.online_bits() / 8,
             "aes_per_elem": {"eval_one_party": aes_eval, "keygen_both": aes_gen},
             "aes_rate_gaes": {"eval": 2 * aes_eval * count / ((per_step(t_cmp) + per_step(t_lut)) * 1e-3) / 1e9,

@@ -7,7 +7,8 @@
  *    fusefss_strerror() gives text.  Size queries return 0 on a null program.
  *  - Ring elements of Z_{2^n} (n <= 64) travel as uint64_t with bits >= n zero.
  *  - Pointers named *_dev are DEVICE pointers owned by the caller (e.g. torch tensors); pointers without
- *    the suffix are HOST pointers.  The library allocates no device memory of its own.
+ *    the suffix are HOST pointers.  The library allocates no device memory of its own except a few KB per
+ *    program (its post-processing code and descriptor tables, uploaded on first use, freed by _destroy).
  *  - `stream` is a cudaStream_t passed as void* (NULL = default stream); all launches are asynchronous on it.
  *  - party is 0 or 1.  xhat = x + r_in mod 2^n is public and identical for both parties (Protocol 1).
  *  - A key buffer is one-time material for exactly one xhat tensor; not enforced.
@@ -120,6 +121,14 @@ size_t fusefss_key_bytes(const fusefss_program *prog, size_t count);
 int fusefss_keygen(const fusefss_program *prog, const uint64_t *r_in_dev, const uint64_t *r_out_dev,
                    uint64_t seed, uint64_t first_elem, size_t count,
                    void *key0_dev, void *key1_dev, void *stream);
+
+/* The same work split by key section, for per-kernel timing: parts = OR of FUSEFSS_GEN_CMP (the T bit-DCF keys),
+ * FUSEFSS_GEN_LUT (the M-1 vector-DCF keys) and FUSEFSS_GEN_SHARES (c_b, masks, kappa, Beaver/AND/B2A material).
+ * Calling the three parts in any order writes exactly what fusefss_keygen writes. */
+enum { FUSEFSS_GEN_CMP = 1, FUSEFSS_GEN_LUT = 2, FUSEFSS_GEN_SHARES = 4 };
+int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, const uint64_t *r_out_dev,
+                         uint64_t seed, uint64_t first_elem, size_t count,
+                         void *key0_dev, void *key1_dev, int parts, void *stream);
 
 /* ---- a5: packed comparison (section 3.6, Def I.1) --------------------------------
  * bits_out_dev[count]: bit t = this party's XOR share of I[view_{k_t,c_t}(xhat) < theta_t]. */

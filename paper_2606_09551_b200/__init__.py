@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libfusefss.so")
 
 # every symbol include/fusefss.h declares (tests check the library exports all of them)
 SYMBOLS = (
-    "fusefss_compile", "fusefss_destroy", "fusefss_shape", "fusefss_atom", "fusefss_key_bytes", "fusefss_keygen",
+    "fusefss_compile", "fusefss_destroy", "fusefss_shape", "fusefss_atom", "fusefss_key_bytes", "fusefss_keygen", "fusefss_keygen_parts",
     "fusefss_eval_cmp", "fusefss_eval_lut", "fusefss_post", "fusefss_post_rounds", "fusefss_post_msg_bytes",
     "fusefss_online_bits", "fusefss_post_fused", "fusefss_gate_workspace_bytes", "fusefss_gate_host",
     "fusefss_strerror", "fusefss_last_cuda_error", "fusefss_launch_count", "fusefss_aes_probe", "fusefss_aes_kat",
@@ -63,6 +63,7 @@ def _load():
         "fusefss_atom": (i32, [vp, i32, C.POINTER(u64)]),
         "fusefss_key_bytes": (sz, [vp, sz]),
         "fusefss_keygen": (i32, [vp, vp, vp, u64, u64, sz, vp, vp, vp]),
+        "fusefss_keygen_parts": (i32, [vp, vp, vp, u64, u64, sz, vp, vp, i32, vp]),
         "fusefss_eval_cmp": (i32, [i32, vp, vp, vp, sz, vp, vp]),
         "fusefss_eval_lut": (i32, [i32, vp, vp, vp, sz, vp, vp]),
         "fusefss_post": (i32, [i32, vp, vp, vp, vp, vp, sz, i32, vp, vp, vp, vp, vp]),
@@ -195,10 +196,14 @@ class Program:
         kb = self.key_bytes(count)
         return (torch.empty(kb, dtype=torch.uint8, device="cuda"), torch.empty(kb, dtype=torch.uint8, device="cuda"))
 
-    def keygen(self, r_in, r_out, seed, first_elem=0, keys=None):
+    def keygen(self, r_in, r_out, seed, first_elem=0, keys=None, parts=7):
         count = r_in.numel()
         k0, k1 = keys if keys is not None else self.alloc_keys(count)
-        _check(lib.fusefss_keygen(self._h, _ptr(r_in), _ptr(r_out), seed, first_elem, count, _ptr(k0), _ptr(k1), _stream()))
+        if parts == 7:
+            _check(lib.fusefss_keygen(self._h, _ptr(r_in), _ptr(r_out), seed, first_elem, count, _ptr(k0), _ptr(k1), _stream()))
+        else:
+            _check(lib.fusefss_keygen_parts(self._h, _ptr(r_in), _ptr(r_out), seed, first_elem, count, _ptr(k0), _ptr(k1),
+                                            parts, _stream()))
         return k0, k1
 
     def eval_cmp(self, party, key, xhat, out=None):

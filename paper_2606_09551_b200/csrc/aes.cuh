@@ -1,9 +1,12 @@
 // aes.cuh -- fixed-key AES-128 PRG core for sm_100a.
 //
-// T-table AES with the tables in shared memory, REPLICATED PER BANK: entry x of table k lives at word
-// (k*256 + x)*32 + lane, so the 32 lanes of a warp always hit 32 different banks and every LDS.32 is one
-// conflict-free wavefront whatever the (secret-dependent, random) indices are.  160 lookups per block.
-// NTAB = 4 keeps T0..T3 (128 KB); NTAB = 1 keeps T0 only (32 KB) and rotates with PRMT.
+// T-table AES with T0..T3 in shared memory, REPLICATED PER BANK so that the 32 lanes of a warp always hit 32
+// different banks: every LDS.32 is one conflict-free wavefront whatever the (secret-dependent) indices are.
+// 160 lookups per block.  Layout chosen so that ONE PRMT builds the address of a lookup: entry x of a table
+// sits at shared-window offset  block*65536 + x*256 + half*128 + lane*4  (T0/T1 = halves of block 1, T2/T3 =
+// halves of block 2), so address = PRMT(state word, tl) = [tl.b0 | state byte k << 8 | tl.b2 | tl.b3] with
+// tl = 0x00010000 | lane*4, and (block, half) ride in the LDS immediate.  Per round and block: 16 PRMT + 16 LDS +
+// 8 LOP3 (r1a used SHF + LOP3 + IMAD per lookup and was issue-bound: profiles/r1a_launches_gelu.md).
 // State: 4 little-endian 32-bit words = the 4 columns (FIPS-197 3.4: byte r of word c is s[r][c]).
 #pragma once
 #include <cstdint>
@@ -69,65 +72,63 @@ struct HostAes {
 // ---------------------------------------------------------------------------------------------------
 // device side
 // ---------------------------------------------------------------------------------------------------
-template <int NTAB>
-__device__ __forceinline__ void aes_fill_tables(uint32_t *sT) {
-    for (int i = threadIdx.x; i < NTAB * 256 * 32; i += blockDim.x) {
-        uint32_t v = c_T0[(i >> 5) & 255];
-        int rot = (i >> 13) * 8;                                      // table k = T0 rotated left by 8k bits
-        sT[i] = __funnelshift_l(v, v, rot);
+// Dynamic shared memory request: the tables occupy window offsets [65536, 196608); the dynamic region starts at
+// a small offset B0 (reserved/static shared memory), so asking for 192 KB always covers them.
+constexpr size_t kAesSmemBytes = 3 * 65536;
+
+// Fills the tables and returns tl (= 0x00010000 | lane*4), produced AFTER the barrier by a volatile asm so that
+// no table lookup (all of which consume tl) can be scheduled above it.
+__device__ __forceinline__ uint32_t aes_fill_tables(uint32_t *dyn_smem) {
+    const uint32_t b0 = (uint32_t)__cvta_generic_to_shared(dyn_smem);
+    char *win0 = reinterpret_cast<char *>(dyn_smem) - b0;                  // generic address of window offset 0
+    for (int i = threadIdx.x; i < 4 * 256 * 32; i += blockDim.x) {
+        const int tab = i >> 13, x = (i >> 5) & 255, ln = i & 31;
+        const uint32_t v = c_T0[x];
+        const uint32_t off = 65536u + (uint32_t)(tab >> 1) * 65536u + (uint32_t)x * 256u + (uint32_t)(tab & 1) * 128u + (uint32_t)ln * 4u;
+        *reinterpret_cast<uint32_t *>(win0 + off) = __funnelshift_l(v, v, tab * 8);   // T_k = T0 rotated left by 8k bits
     }
     __syncthreads();
+    uint32_t tl;
+    asm volatile("mov.u32 %0, %1;" : "=r"(tl) : "r"(0x00010000u | ((threadIdx.x & 31u) << 2)) : "memory");
+    return tl;
 }
 
-template <int NTAB> constexpr size_t aes_smem_bytes() { return (size_t)NTAB * 256 * 32 * 4; }
-
-template <int K> __device__ __forceinline__ uint32_t byte_of(uint32_t w) {
-    return K == 0 ? (w & 0xffu) : K == 3 ? (w >> 24) : ((w >> (8 * K)) & 0xffu);
+// T_TAB[ byte K of w ]
+template <int TAB, int K>
+__device__ __forceinline__ uint32_t tlu(uint32_t tl, uint32_t w) {
+    uint32_t v;
+    asm("{\n\t.reg .b32 a;\n\tprmt.b32 a, %1, %2, %3;\n\tld.shared.u32 %0, [a+%4];\n\t}"
+        : "=r"(v) : "r"(w), "r"(tl), "n"(0x7604 | (K << 4)), "n"((TAB >> 1) * 65536 + (TAB & 1) * 128));
+    return v;
 }
 
-// lookup of table TAB at the byte K of w; `tl` = shared table base already offset by the lane
-template <int NTAB, int TAB, int K>
-__device__ __forceinline__ uint32_t tlu(const uint32_t *tl, uint32_t w) {
-    if (NTAB == 4) return tl[TAB * 8192 + byte_of<K>(w) * 32];
-    uint32_t v = tl[byte_of<K>(w) * 32];
-    return TAB == 0 ? v : TAB == 1 ? __byte_perm(v, v, 0x2103) : TAB == 2 ? __byte_perm(v, v, 0x1032)
-                                                                          : __byte_perm(v, v, 0x0321);
-}
-
-template <int NTAB>
-__device__ __forceinline__ void aes_round(uint32_t (&s)[4], const uint32_t *tl, uint32_t k0, uint32_t k1,
-                                          uint32_t k2, uint32_t k3) {
-    uint32_t t0 = tlu<NTAB, 0, 0>(tl, s[0]) ^ tlu<NTAB, 1, 1>(tl, s[1]) ^ tlu<NTAB, 2, 2>(tl, s[2]) ^ tlu<NTAB, 3, 3>(tl, s[3]) ^ k0;
-    uint32_t t1 = tlu<NTAB, 0, 0>(tl, s[1]) ^ tlu<NTAB, 1, 1>(tl, s[2]) ^ tlu<NTAB, 2, 2>(tl, s[3]) ^ tlu<NTAB, 3, 3>(tl, s[0]) ^ k1;
-    uint32_t t2 = tlu<NTAB, 0, 0>(tl, s[2]) ^ tlu<NTAB, 1, 1>(tl, s[3]) ^ tlu<NTAB, 2, 2>(tl, s[0]) ^ tlu<NTAB, 3, 3>(tl, s[1]) ^ k2;
-    uint32_t t3 = tlu<NTAB, 0, 0>(tl, s[3]) ^ tlu<NTAB, 1, 1>(tl, s[0]) ^ tlu<NTAB, 2, 2>(tl, s[1]) ^ tlu<NTAB, 3, 3>(tl, s[2]) ^ k3;
+__device__ __forceinline__ void aes_round(uint32_t (&s)[4], uint32_t tl, uint32_t k0, uint32_t k1, uint32_t k2, uint32_t k3) {
+    uint32_t t0 = tlu<0, 0>(tl, s[0]) ^ tlu<1, 1>(tl, s[1]) ^ tlu<2, 2>(tl, s[2]) ^ tlu<3, 3>(tl, s[3]) ^ k0;
+    uint32_t t1 = tlu<0, 0>(tl, s[1]) ^ tlu<1, 1>(tl, s[2]) ^ tlu<2, 2>(tl, s[3]) ^ tlu<3, 3>(tl, s[0]) ^ k1;
+    uint32_t t2 = tlu<0, 0>(tl, s[2]) ^ tlu<1, 1>(tl, s[3]) ^ tlu<2, 2>(tl, s[0]) ^ tlu<3, 3>(tl, s[1]) ^ k2;
+    uint32_t t3 = tlu<0, 0>(tl, s[3]) ^ tlu<1, 1>(tl, s[0]) ^ tlu<2, 2>(tl, s[1]) ^ tlu<3, 3>(tl, s[2]) ^ k3;
     s[0] = t0; s[1] = t1; s[2] = t2; s[3] = t3;
 }
 
-// final round: SubBytes + ShiftRows + AddRoundKey; S[x] is byte 1 (and 2) of T0[x]
-template <int NTAB>
-__device__ __forceinline__ uint32_t aes_last_col(const uint32_t *tl, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
-    if (NTAB == 4) {
-        return (tl[2 * 8192 + byte_of<0>(a) * 32] & 0x000000ffu) | (tl[3 * 8192 + byte_of<1>(b) * 32] & 0x0000ff00u) |
-               (tl[0 * 8192 + byte_of<2>(c) * 32] & 0x00ff0000u) | (tl[1 * 8192 + byte_of<3>(d) * 32] & 0xff000000u);
-    }
-    uint32_t va = tl[byte_of<0>(a) * 32], vb = tl[byte_of<1>(b) * 32], vc = tl[byte_of<2>(c) * 32], vd = tl[byte_of<3>(d) * 32];
-    uint32_t lo = __byte_perm(va, vb, 0x0051);      // bytes: va.b1, vb.b1
-    uint32_t hi = __byte_perm(vc, vd, 0x0051);
-    return __byte_perm(lo, hi, 0x5410);
+// final round: SubBytes + ShiftRows (+ AddRoundKey by the caller).  S[x] = byte 0 of T2 = byte 1 of T3 = byte 2
+// of T0 = byte 3 of T1, so the column is assembled with three PRMTs.
+__device__ __forceinline__ uint32_t aes_last_col(uint32_t tl, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
+    const uint32_t va = tlu<2, 0>(tl, a), vb = tlu<3, 1>(tl, b), vc = tlu<0, 2>(tl, c), vd = tlu<1, 3>(tl, d);
+    const uint32_t lo = __byte_perm(va, vb, 0x3250);      // [va.b0, vb.b1, -, -]
+    const uint32_t hi = __byte_perm(vc, vd, 0x7210);      // [-, -, vc.b2, vd.b3]
+    return __byte_perm(lo, hi, 0x7610);
 }
-template <int NTAB>
-__device__ __forceinline__ void aes_last(uint32_t (&s)[4], const uint32_t *tl, uint32_t k0, uint32_t k1, uint32_t k2, uint32_t k3) {
-    uint32_t t0 = aes_last_col<NTAB>(tl, s[0], s[1], s[2], s[3]) ^ k0;
-    uint32_t t1 = aes_last_col<NTAB>(tl, s[1], s[2], s[3], s[0]) ^ k1;
-    uint32_t t2 = aes_last_col<NTAB>(tl, s[2], s[3], s[0], s[1]) ^ k2;
-    uint32_t t3 = aes_last_col<NTAB>(tl, s[3], s[0], s[1], s[2]) ^ k3;
+__device__ __forceinline__ void aes_last(uint32_t (&s)[4], uint32_t tl, uint32_t k0, uint32_t k1, uint32_t k2, uint32_t k3) {
+    uint32_t t0 = aes_last_col(tl, s[0], s[1], s[2], s[3]) ^ k0;
+    uint32_t t1 = aes_last_col(tl, s[1], s[2], s[3], s[0]) ^ k1;
+    uint32_t t2 = aes_last_col(tl, s[2], s[3], s[0], s[1]) ^ k2;
+    uint32_t t3 = aes_last_col(tl, s[3], s[0], s[1], s[2]) ^ k3;
     s[0] = t0; s[1] = t1; s[2] = t2; s[3] = t3;
 }
 
 // NI inputs x NK keys (K_KFIRST .. K_{KFIRST+NK-1}) in lock-step: out[i][k] = AES_{K}(x_i) ^ x_i  (the PRG of 4.1)
-template <int NTAB, int NI, int NK, int KFIRST>
-__device__ __forceinline__ void prg_blocks(const uint32_t *tl, const uint32_t (&x)[NI][4], uint32_t (&out)[NI][NK][4]) {
+template <int NI, int NK, int KFIRST>
+__device__ __forceinline__ void prg_blocks(uint32_t tl, const uint32_t (&x)[NI][4], uint32_t (&out)[NI][NK][4]) {
 #pragma unroll
     for (int i = 0; i < NI; ++i)
 #pragma unroll
@@ -140,27 +141,26 @@ __device__ __forceinline__ void prg_blocks(const uint32_t *tl, const uint32_t (&
         for (int i = 0; i < NI; ++i)
 #pragma unroll
             for (int k = 0; k < NK; ++k)
-                aes_round<NTAB>(out[i][k], tl, c_rk[KFIRST + k][4 * r], c_rk[KFIRST + k][4 * r + 1],
-                                c_rk[KFIRST + k][4 * r + 2], c_rk[KFIRST + k][4 * r + 3]);
+                aes_round(out[i][k], tl, c_rk[KFIRST + k][4 * r], c_rk[KFIRST + k][4 * r + 1],
+                          c_rk[KFIRST + k][4 * r + 2], c_rk[KFIRST + k][4 * r + 3]);
     }
 #pragma unroll
     for (int i = 0; i < NI; ++i)
 #pragma unroll
         for (int k = 0; k < NK; ++k) {
-            aes_last<NTAB>(out[i][k], tl, c_rk[KFIRST + k][40], c_rk[KFIRST + k][41], c_rk[KFIRST + k][42], c_rk[KFIRST + k][43]);
+            aes_last(out[i][k], tl, c_rk[KFIRST + k][40], c_rk[KFIRST + k][41], c_rk[KFIRST + k][42], c_rk[KFIRST + k][43]);
 #pragma unroll
             for (int c = 0; c < 4; ++c) out[i][k][c] ^= x[i][c];
         }
 }
 
 // plain AES-128 with a run-time expanded key (no feed-forward): R(e, slot) of DESIGN 4.5
-template <int NTAB>
-__device__ __forceinline__ void aes_encrypt_rk(const uint32_t *tl, const RoundKeys &rk, uint32_t (&s)[4]) {
+__device__ __forceinline__ void aes_encrypt_rk(uint32_t tl, const RoundKeys &rk, uint32_t (&s)[4]) {
 #pragma unroll
     for (int c = 0; c < 4; ++c) s[c] ^= rk.w[c];
 #pragma unroll 1
-    for (int r = 1; r < 10; ++r) aes_round<NTAB>(s, tl, rk.w[4 * r], rk.w[4 * r + 1], rk.w[4 * r + 2], rk.w[4 * r + 3]);
-    aes_last<NTAB>(s, tl, rk.w[40], rk.w[41], rk.w[42], rk.w[43]);
+    for (int r = 1; r < 10; ++r) aes_round(s, tl, rk.w[4 * r], rk.w[4 * r + 1], rk.w[4 * r + 2], rk.w[4 * r + 3]);
+    aes_last(s, tl, rk.w[40], rk.w[41], rk.w[42], rk.w[43]);
 }
 
 }  // namespace fsk

@@ -24,12 +24,10 @@ struct EvalCmpArgs {
 __device__ __forceinline__ uint4 ld_stream16(const void *p) { return __ldcs(reinterpret_cast<const uint4 *>(p)); }
 __device__ __forceinline__ uint64_t ld_stream8(const void *p) { return __ldcs(reinterpret_cast<const unsigned long long *>(p)); }
 
-template <int NTAB>
 __global__ void __launch_bounds__(kEvalThreads, 1) k_eval_cmp(const __grid_constant__ EvalCmpArgs a) {
     extern __shared__ uint32_t sT[];
-    aes_fill_tables<NTAB>(sT);
+    const uint32_t tl = aes_fill_tables(sT);
     const int lane = threadIdx.x & 31;
-    const uint32_t *tl = sT + lane;
     const size_t tiles = (a.count + 31) / 32;
     const size_t items = tiles * (size_t)a.G;
     const size_t warps = (size_t)gridDim.x * (blockDim.x >> 5);
@@ -60,7 +58,7 @@ __global__ void __launch_bounds__(kEvalThreads, 1) k_eval_cmp(const __grid_const
                 u <<= 1;
                 uint32_t x[1][4] = {{s.x | dbit, s.y, s.z, s.w}};
                 uint32_t o[1][1][4];
-                prg_blocks<NTAB, 1, 1, 0>(tl, x, o);
+                prg_blocks<1, 1, 0>(tl, x, o);
                 const uint32_t tm = 0u - tb;                                   // all-ones iff the control bit is set
                 V ^= ((o[0][0][0] >> 1) & 1u) ^ (tb & (uint32_t)((vb >> i) & 1ull));
                 const uint32_t tnew = (o[0][0][0] & 1u) ^ (tb & (cw.x >> dbit) & 1u);
@@ -73,7 +71,7 @@ __global__ void __launch_bounds__(kEvalThreads, 1) k_eval_cmp(const __grid_const
             }
             uint32_t x[1][4] = {{s.x | 2u, s.y, s.z, s.w}};                   // leaf conversion, tweak 2
             uint32_t o[1][1][4];
-            prg_blocks<NTAB, 1, 1, 0>(tl, x, o);
+            prg_blocks<1, 1, 0>(tl, x, o);
             V ^= ((o[0][0][0] >> 1) & 1u) ^ (tb & fin);
             word |= (uint64_t)(V & 1u) << t;
         }
@@ -91,13 +89,12 @@ struct EvalLutArgs {
     int n, M, G, party;
 };
 
-template <int NTAB, int P>
+template <int P>
 __global__ void __launch_bounds__(kEvalThreads, 1) k_eval_lut(const __grid_constant__ EvalLutArgs a) {
     constexpr int Q = (P + 1) / 2;
     extern __shared__ uint32_t sT[];
-    aes_fill_tables<NTAB>(sT);
+    const uint32_t tl = aes_fill_tables(sT);
     const int lane = threadIdx.x & 31;
-    const uint32_t *tl = sT + lane;
     const size_t tiles = (a.count + 31) / 32;
     const size_t items = tiles * (size_t)a.G;
     const size_t warps = (size_t)gridDim.x * (blockDim.x >> 5);
@@ -141,7 +138,7 @@ __global__ void __launch_bounds__(kEvalThreads, 1) k_eval_lut(const __grid_const
                 u <<= 1;
                 uint32_t x[1][4] = {{s.x | dbit, s.y, s.z, s.w}};
                 uint32_t o[1][1 + Q][4];
-                prg_blocks<NTAB, 1, 1 + Q, 0>(tl, x, o);
+                prg_blocks<1, 1 + Q, 0>(tl, x, o);
                 const uint32_t tm = 0u - tb;
                 const uint64_t tm64 = 0ull - (uint64_t)tb;
 #pragma unroll
@@ -162,7 +159,7 @@ __global__ void __launch_bounds__(kEvalThreads, 1) k_eval_lut(const __grid_const
             // leaf: V += conv(s) + t * fin; party 1 negates
             uint32_t x[1][4] = {{s.x | 2u, s.y, s.z, s.w}};
             uint32_t o[1][Q][4];
-            prg_blocks<NTAB, 1, Q, 1>(tl, x, o);
+            prg_blocks<1, Q, 1>(tl, x, o);
             const uint64_t tm64 = 0ull - (uint64_t)tb;
             const uint8_t *fin = tree + a.vt_fin_rel;
 #pragma unroll

@@ -21,10 +21,9 @@ __device__ __forceinline__ void st_stream16(void *p, uint4 v) { __stcs(reinterpr
 __device__ __forceinline__ void st_stream8(void *p, uint64_t v) { __stcs(reinterpret_cast<unsigned long long *>(p), (unsigned long long)v); }
 
 // R(e, slot) = AES_{seed||~seed}(LE64(e) || LE64(slot))
-template <int NTAB>
-__device__ __forceinline__ void dealer_rand(const uint32_t *tl, const RoundKeys &rk, uint64_t e, uint64_t slot, uint64_t &lo, uint64_t &hi) {
+__device__ __forceinline__ void dealer_rand(uint32_t tl, const RoundKeys &rk, uint64_t e, uint64_t slot, uint64_t &lo, uint64_t &hi) {
     uint32_t s[4] = {(uint32_t)e, (uint32_t)(e >> 32), (uint32_t)slot, (uint32_t)(slot >> 32)};
-    aes_encrypt_rk<NTAB>(tl, rk, s);
+    aes_encrypt_rk(tl, rk, s);
     lo = (uint64_t)s[0] | ((uint64_t)s[1] << 32);
     hi = (uint64_t)s[2] | ((uint64_t)s[3] << 32);
 }
@@ -38,12 +37,10 @@ struct GenBitArgs {
     GenAtomDev atom[kMaxAtoms];
 };
 
-template <int NTAB>
 __global__ void __launch_bounds__(kGenThreads, 1) k_gen_bit(const __grid_constant__ GenBitArgs a) {
     extern __shared__ uint32_t sT[];
-    aes_fill_tables<NTAB>(sT);
+    const uint32_t tl = aes_fill_tables(sT);
     const int lane = threadIdx.x & 31;
-    const uint32_t *tl = sT + lane;
     const size_t tiles = (a.count + 31) / 32;
     const size_t items = tiles * (size_t)a.T;
     const size_t warps = (size_t)gridDim.x * (blockDim.x >> 5);
@@ -60,9 +57,9 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_bit(const __grid_constan
         uint32_t s[2][4];
         {
             uint64_t lo, hi;
-            dealer_rand<NTAB>(tl, a.rk, a.first_elem + e, SLOT_BIT_ROOT + 2 * t, lo, hi);
+            dealer_rand(tl, a.rk, a.first_elem + e, SLOT_BIT_ROOT + 2 * t, lo, hi);
             s[0][0] = (uint32_t)lo & ~3u; s[0][1] = (uint32_t)(lo >> 32); s[0][2] = (uint32_t)hi; s[0][3] = (uint32_t)(hi >> 32);
-            dealer_rand<NTAB>(tl, a.rk, a.first_elem + e, SLOT_BIT_ROOT + 2 * t + 1, lo, hi);
+            dealer_rand(tl, a.rk, a.first_elem + e, SLOT_BIT_ROOT + 2 * t + 1, lo, hi);
             s[1][0] = (uint32_t)lo & ~3u; s[1][1] = (uint32_t)(lo >> 32); s[1][2] = (uint32_t)hi; s[1][3] = (uint32_t)(hi >> 32);
         }
         const uint4 root0 = make_uint4(s[0][0], s[0][1], s[0][2], s[0][3]);
@@ -79,7 +76,7 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_bit(const __grid_constan
             for (int b = 0; b < 2; ++b)
 #pragma unroll
                 for (int d = 0; d < 2; ++d) { x[2 * b + d][0] = s[b][0] | (uint32_t)d; x[2 * b + d][1] = s[b][1]; x[2 * b + d][2] = s[b][2]; x[2 * b + d][3] = s[b][3]; }
-            prg_blocks<NTAB, 4, 1, 0>(tl, x, o);
+            prg_blocks<4, 1, 0>(tl, x, o);
             const uint32_t am = 0u - abit;                    // keep = alpha_i, lose = 1 - alpha_i
             uint32_t keep0[4], keep1[4], scw[4];
 #pragma unroll
@@ -113,7 +110,7 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_bit(const __grid_constan
         uint32_t x[2][4], o[2][1][4];
 #pragma unroll
         for (int b = 0; b < 2; ++b) { x[b][0] = s[b][0] | 2u; x[b][1] = s[b][1]; x[b][2] = s[b][2]; x[b][3] = s[b][3]; }
-        prg_blocks<NTAB, 2, 1, 0>(tl, x, o);
+        prg_blocks<2, 1, 0>(tl, x, o);
         const uint32_t fin = (((o[0][0][0] ^ o[1][0][0]) >> 1) & 1u) ^ Va;
         st_stream16(a.key0 + at.root_off + e * 16, make_uint4(root0.x | fin, root0.y, root0.z, root0.w));
         st_stream16(a.key1 + at.root_off + e * 16, make_uint4(root1.x | fin, root1.y, root1.z, root1.w));
@@ -176,13 +173,12 @@ struct GenVecArgs {
     RoundKeys rk;
 };
 
-template <int NTAB, int P>
+template <int P>
 __global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec(const __grid_constant__ GenVecArgs a) {
     constexpr int Q = (P + 1) / 2;
     extern __shared__ uint32_t sT[];
-    aes_fill_tables<NTAB>(sT);
+    const uint32_t tl = aes_fill_tables(sT);
     const int lane = threadIdx.x & 31;
-    const uint32_t *tl = sT + lane;
     const size_t tiles = (a.count + 31) / 32;
     const size_t items = tiles * (size_t)(a.M - 1);
     const size_t warps = (size_t)gridDim.x * (blockDim.x >> 5);
@@ -203,9 +199,9 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec(const __grid_constan
         uint32_t s[2][4];
         {
             uint64_t lo, hi;
-            dealer_rand<NTAB>(tl, a.rk, a.first_elem + e, SLOT_VEC_ROOT + 2 * j, lo, hi);
+            dealer_rand(tl, a.rk, a.first_elem + e, SLOT_VEC_ROOT + 2 * j, lo, hi);
             s[0][0] = (uint32_t)lo & ~3u; s[0][1] = (uint32_t)(lo >> 32); s[0][2] = (uint32_t)hi; s[0][3] = (uint32_t)(hi >> 32);
-            dealer_rand<NTAB>(tl, a.rk, a.first_elem + e, SLOT_VEC_ROOT + 2 * j + 1, lo, hi);
+            dealer_rand(tl, a.rk, a.first_elem + e, SLOT_VEC_ROOT + 2 * j + 1, lo, hi);
             s[1][0] = (uint32_t)lo & ~3u; s[1][1] = (uint32_t)(lo >> 32); s[1][2] = (uint32_t)hi; s[1][3] = (uint32_t)(hi >> 32);
         }
         uint8_t *tree0 = a.key0 + a.vt_first + (size_t)(j - 1) * a.vt_stride;
@@ -229,7 +225,7 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec(const __grid_constan
                 uint32_t x[2][4], o[2][1 + Q][4];
 #pragma unroll
                 for (int d = 0; d < 2; ++d) { x[d][0] = s[b][0] | (uint32_t)d; x[d][1] = s[b][1]; x[d][2] = s[b][2]; x[d][3] = s[b][3]; }
-                prg_blocks<NTAB, 2, 1 + Q, 0>(tl, x, o);
+                prg_blocks<2, 1 + Q, 0>(tl, x, o);
                 Tb[b][0] = o[0][0][0] & 1u; Tb[b][1] = o[1][0][0] & 1u;
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
@@ -277,7 +273,7 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec(const __grid_constan
         uint32_t x[2][4], o[2][Q][4];
 #pragma unroll
         for (int b = 0; b < 2; ++b) { x[b][0] = s[b][0] | 2u; x[b][1] = s[b][1]; x[b][2] = s[b][2]; x[b][3] = s[b][3]; }
-        prg_blocks<NTAB, 2, Q, 1>(tl, x, o);
+        prg_blocks<2, Q, 1>(tl, x, o);
         const uint64_t sgn = 0ull - (uint64_t)t1;
 #pragma unroll
         for (int w = 0; w < P; ++w) {
@@ -306,11 +302,9 @@ struct GenMiscArgs {
     GenAtomDev atom[kMaxAtoms];
 };
 
-template <int NTAB>
 __global__ void __launch_bounds__(kGenThreads, 1) k_gen_misc(const __grid_constant__ GenMiscArgs a) {
     extern __shared__ uint32_t sT[];
-    aes_fill_tables<NTAB>(sT);
-    const uint32_t *tl = sT + (threadIdx.x & 31);
+    const uint32_t tl = aes_fill_tables(sT);
     for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < a.count; e += (size_t)gridDim.x * blockDim.x) {
         const uint64_t ge = a.first_elem + e;
         const uint64_t r = a.r_in[e] & a.mask;
@@ -324,21 +318,21 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_misc(const __grid_consta
             p3.init(a.alpha, a.m, a.n, a.mask, r, a.M);
             const uint64_t *v = a.payload + (size_t)p3.ord(a.M - 1) * a.p;
             for (int w = 0; w < a.p; ++w) {
-                dealer_rand<NTAB>(tl, a.rk, ge, SLOT_LUT_C + w, lo, hi);
+                dealer_rand(tl, a.rk, ge, SLOT_LUT_C + w, lo, hi);
                 const uint64_t c0 = lo & a.mask;
                 put(a.lut_c + (size_t)w * a.s8, c0, (v[w] - c0) & a.mask);
             }
         }
-        dealer_rand<NTAB>(tl, a.rk, ge, SLOT_RIN, lo, hi);
+        dealer_rand(tl, a.rk, ge, SLOT_RIN, lo, hi);
         put(a.rin, lo & a.mask, (r - (lo & a.mask)) & a.mask);
         if (a.mask_output)
             for (int j = 0; j < a.n_out_a; ++j) {
-                dealer_rand<NTAB>(tl, a.rk, ge, SLOT_ROUT + j, lo, hi);
+                dealer_rand(tl, a.rk, ge, SLOT_ROUT + j, lo, hi);
                 const uint64_t ro = a.r_out[(size_t)j * a.count + e] & a.mask, s0 = lo & a.mask;
                 put(a.rout + (size_t)j * a.s8, s0, (ro - s0) & a.mask);
             }
         for (int t = 0; t < a.n_ka; ++t) {                                 // kappa^A = rep(r) >> arg
-            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_KA + t, lo, hi);
+            dealer_rand(tl, a.rk, ge, SLOT_KA + t, lo, hi);
             uint64_t val = 0;
             if (a.ka_kind[t] == FUSEFSS_KA_R_SHR) val = a.ka_arg[t] >= 64 ? 0ull : r >> a.ka_arg[t];
             const uint64_t s0 = lo & a.mask;
@@ -361,16 +355,16 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_misc(const __grid_consta
                 if (a.kb_kind[t] == FUSEFSS_KB_R_BIT) bit = (r >> a.kb_arg[t]) & 1ull;
                 kbits |= bit << (a.n_carry + t);
             }
-            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_KB, lo, hi);
+            dealer_rand(tl, a.rk, ge, SLOT_KB, lo, hi);
             const uint64_t s0 = lo & (n_kb >= 64 ? ~0ull : ((1ull << n_kb) - 1ull));
             put(a.kb, s0, kbits ^ s0);
         }
         for (int i = 0; i < a.MA; ++i) {                                   // Beaver triple (a, b, c = ab)
-            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_BV_AB + i, lo, hi);
+            dealer_rand(tl, a.rk, ge, SLOT_BV_AB + i, lo, hi);
             const uint64_t ta = lo & a.mask, tb = hi & a.mask, tc = (ta * tb) & a.mask;
-            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_BV_AB0 + i, lo, hi);
+            dealer_rand(tl, a.rk, ge, SLOT_BV_AB0 + i, lo, hi);
             const uint64_t a0 = lo & a.mask, b0 = hi & a.mask;
-            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_BV_C0 + i, lo, hi);
+            dealer_rand(tl, a.rk, ge, SLOT_BV_C0 + i, lo, hi);
             const uint64_t c0 = lo & a.mask;
             const size_t o = a.beaver + (size_t)3 * i * a.s8;
             put(o, a0, (ta - a0) & a.mask);
@@ -379,11 +373,11 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_misc(const __grid_consta
         }
         if (a.MB > 0) {                                                    // AND triples, gate i = bit i
             const uint64_t bm = a.MB >= 64 ? ~0ull : ((1ull << a.MB) - 1ull);
-            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_AND_AB, lo, hi);
+            dealer_rand(tl, a.rk, ge, SLOT_AND_AB, lo, hi);
             const uint64_t ta = lo & bm, tb = hi & bm, tc = ta & tb;
-            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_AND_AB0, lo, hi);
+            dealer_rand(tl, a.rk, ge, SLOT_AND_AB0, lo, hi);
             const uint64_t a0 = lo & bm, b0 = hi & bm;
-            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_AND_C0, lo, hi);
+            dealer_rand(tl, a.rk, ge, SLOT_AND_C0, lo, hi);
             const uint64_t c0 = lo & bm;
             put(a.andt, a0, ta ^ a0);
             put(a.andt + a.s8, b0, tb ^ b0);
@@ -391,11 +385,11 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_misc(const __grid_consta
         }
         if (a.GMIX > 0) {                                                  // B2A pairs (<rho>, [rho])
             const uint64_t bm = a.GMIX >= 64 ? ~0ull : ((1ull << a.GMIX) - 1ull);
-            dealer_rand<NTAB>(tl, a.rk, ge, SLOT_B2A, lo, hi);
+            dealer_rand(tl, a.rk, ge, SLOT_B2A, lo, hi);
             const uint64_t rho = lo & bm, rho0 = hi & bm;
             put(a.b2a_bits, rho0, rho ^ rho0);
             for (int i = 0; i < a.GMIX; ++i) {
-                dealer_rand<NTAB>(tl, a.rk, ge, SLOT_B2A_A0 + i, lo, hi);
+                dealer_rand(tl, a.rk, ge, SLOT_B2A_A0 + i, lo, hi);
                 const uint64_t s0 = lo & a.mask, val = (rho >> i) & 1ull;
                 put(a.b2a_a + (size_t)i * a.s8, s0, (val - s0) & a.mask);
             }

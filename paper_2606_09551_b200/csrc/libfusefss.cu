@@ -19,7 +19,6 @@ thread_local char g_cuda_err[256] = "";
 std::atomic<uint64_t> g_launches{0};
 std::once_flag g_init_once;
 int g_init_status = 0;
-int g_ntab = 4;
 int g_sms = 148;
 int g_eval_threads = kEvalThreads;
 const HostAes &host_aes() { static HostAes h; return h; }
@@ -52,7 +51,6 @@ int init_device() {
             int dev = 0;
             CU(cudaGetDevice(&dev));
             CU(cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev));
-            if (const char *s = std::getenv("FUSEFSS_NTAB")) g_ntab = std::atoi(s) == 1 ? 1 : 4;
             if (const char *s = std::getenv("FUSEFSS_EVAL_THREADS")) {
                 int v = std::atoi(s);
                 if (v >= 32 && v <= kEvalThreads && v % 32 == 0) g_eval_threads = v;
@@ -125,32 +123,32 @@ template <typename K, typename A> int launch(K kernel, int grid, int block, size
     return 0;
 }
 
-// ---- dispatch on (NTAB, P) -------------------------------------------------------------------------
-template <int NTAB> int launch_eval_lut_p(int p, int grid, int block, cudaStream_t st, const EvalLutArgs &a) {
-    const size_t sm = aes_smem_bytes<NTAB>();
+// ---- dispatch on P ---------------------------------------------------------------------------------
+int launch_eval_lut_p(int p, int grid, int block, cudaStream_t st, const EvalLutArgs &a) {
+    const size_t sm = kAesSmemBytes;
     switch (p) {
-    case 1: return launch(k_eval_lut<NTAB, 1>, grid, block, sm, st, a);
-    case 2: return launch(k_eval_lut<NTAB, 2>, grid, block, sm, st, a);
-    case 3: return launch(k_eval_lut<NTAB, 3>, grid, block, sm, st, a);
-    case 4: return launch(k_eval_lut<NTAB, 4>, grid, block, sm, st, a);
-    case 5: return launch(k_eval_lut<NTAB, 5>, grid, block, sm, st, a);
-    case 6: return launch(k_eval_lut<NTAB, 6>, grid, block, sm, st, a);
-    case 7: return launch(k_eval_lut<NTAB, 7>, grid, block, sm, st, a);
-    case 8: return launch(k_eval_lut<NTAB, 8>, grid, block, sm, st, a);
+    case 1: return launch(k_eval_lut<1>, grid, block, sm, st, a);
+    case 2: return launch(k_eval_lut<2>, grid, block, sm, st, a);
+    case 3: return launch(k_eval_lut<3>, grid, block, sm, st, a);
+    case 4: return launch(k_eval_lut<4>, grid, block, sm, st, a);
+    case 5: return launch(k_eval_lut<5>, grid, block, sm, st, a);
+    case 6: return launch(k_eval_lut<6>, grid, block, sm, st, a);
+    case 7: return launch(k_eval_lut<7>, grid, block, sm, st, a);
+    case 8: return launch(k_eval_lut<8>, grid, block, sm, st, a);
     }
     return FUSEFSS_E_SPEC;
 }
-template <int NTAB> int launch_gen_vec_p(int p, int grid, int block, cudaStream_t st, const GenVecArgs &a) {
-    const size_t sm = aes_smem_bytes<NTAB>();
+int launch_gen_vec_p(int p, int grid, int block, cudaStream_t st, const GenVecArgs &a) {
+    const size_t sm = kAesSmemBytes;
     switch (p) {
-    case 1: return launch(k_gen_vec<NTAB, 1>, grid, block, sm, st, a);
-    case 2: return launch(k_gen_vec<NTAB, 2>, grid, block, sm, st, a);
-    case 3: return launch(k_gen_vec<NTAB, 3>, grid, block, sm, st, a);
-    case 4: return launch(k_gen_vec<NTAB, 4>, grid, block, sm, st, a);
-    case 5: return launch(k_gen_vec<NTAB, 5>, grid, block, sm, st, a);
-    case 6: return launch(k_gen_vec<NTAB, 6>, grid, block, sm, st, a);
-    case 7: return launch(k_gen_vec<NTAB, 7>, grid, block, sm, st, a);
-    case 8: return launch(k_gen_vec<NTAB, 8>, grid, block, sm, st, a);
+    case 1: return launch(k_gen_vec<1>, grid, block, sm, st, a);
+    case 2: return launch(k_gen_vec<2>, grid, block, sm, st, a);
+    case 3: return launch(k_gen_vec<3>, grid, block, sm, st, a);
+    case 4: return launch(k_gen_vec<4>, grid, block, sm, st, a);
+    case 5: return launch(k_gen_vec<5>, grid, block, sm, st, a);
+    case 6: return launch(k_gen_vec<6>, grid, block, sm, st, a);
+    case 7: return launch(k_gen_vec<7>, grid, block, sm, st, a);
+    case 8: return launch(k_gen_vec<8>, grid, block, sm, st, a);
     }
     return FUSEFSS_E_SPEC;
 }
@@ -239,6 +237,12 @@ uint64_t fusefss_launch_count(void) { return g_launches.load(); }
 
 int fusefss_keygen(const fusefss_program *prog, const uint64_t *r_in_dev, const uint64_t *r_out_dev, uint64_t seed,
                    uint64_t first_elem, size_t count, void *key0_dev, void *key1_dev, void *stream) {
+    return fusefss_keygen_parts(prog, r_in_dev, r_out_dev, seed, first_elem, count, key0_dev, key1_dev,
+                                FUSEFSS_GEN_CMP | FUSEFSS_GEN_LUT | FUSEFSS_GEN_SHARES, stream);
+}
+
+int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, const uint64_t *r_out_dev, uint64_t seed,
+                         uint64_t first_elem, size_t count, void *key0_dev, void *key1_dev, int parts, void *stream) {
     Program *P = const_cast<Program *>(prog_of(prog));
     if (!P || !r_in_dev || !key0_dev || !key1_dev) return FUSEFSS_E_NULL;
     if (P->mask_output && !r_out_dev) return FUSEFSS_E_NULL;
@@ -252,28 +256,28 @@ int fusefss_keygen(const fusefss_program *prog, const uint64_t *r_in_dev, const 
     const uint64_t *alpha_dev = (const uint64_t *)(blob + P->dev_alpha_off);
     const uint64_t *payload_dev = (const uint64_t *)(blob + P->dev_payload_off);
     const size_t tiles = (count + 31) / 32;
-    const size_t smem = g_ntab == 4 ? aes_smem_bytes<4>() : aes_smem_bytes<1>();
-    if (P->T > 0) {
+    const size_t smem = kAesSmemBytes;
+    if (P->T > 0 && (parts & FUSEFSS_GEN_CMP)) {
         GenBitArgs a{};
         a.key0 = (uint8_t *)key0_dev; a.key1 = (uint8_t *)key1_dev; a.r_in = r_in_dev;
         a.count = count; a.s16 = L.s16; a.first_elem = first_elem; a.mask = P->mask; a.T = P->T; a.rk = rk;
         for (int t = 0; t < P->T; ++t)
             a.atom[t] = GenAtomDev{P->atoms[t].c, P->atoms[t].beta, L.bt_root[t], L.bt_cw[t], L.bt_vb[t], P->atoms[t].k, P->atoms[t].is_theta};
         const int grid = grid_for(tiles * P->T, kGenThreads);
-        rc = g_ntab == 4 ? launch(k_gen_bit<4>, grid, kGenThreads, smem, st, a) : launch(k_gen_bit<1>, grid, kGenThreads, smem, st, a);
+        rc = launch(k_gen_bit, grid, kGenThreads, kAesSmemBytes, st, a);
         if (rc) return rc;
     }
-    if (P->has_lut) {
+    if (P->has_lut && (parts & FUSEFSS_GEN_LUT)) {
         GenVecArgs a{};
         a.key0 = (uint8_t *)key0_dev; a.key1 = (uint8_t *)key1_dev; a.r_in = r_in_dev; a.alpha = alpha_dev; a.payload = payload_dev;
         a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.vt_first = L.vt_first; a.vt_stride = L.vt_stride; a.lvl_stride = L.lvl_stride;
         a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel; a.first_elem = first_elem; a.mask = P->mask;
         a.n = (int)P->n; a.m = (int)P->m; a.M = P->M; a.rk = rk;
         const int grid = grid_for(tiles * (size_t)(P->M - 1), kGenThreads);
-        rc = g_ntab == 4 ? launch_gen_vec_p<4>(P->p, grid, kGenThreads, st, a) : launch_gen_vec_p<1>(P->p, grid, kGenThreads, st, a);
+        rc = launch_gen_vec_p(P->p, grid, kGenThreads, st, a);
         if (rc) return rc;
     }
-    {
+    if (parts & FUSEFSS_GEN_SHARES) {
         GenMiscArgs a{};
         a.key0 = (uint8_t *)key0_dev; a.key1 = (uint8_t *)key1_dev; a.r_in = r_in_dev; a.r_out = r_out_dev;
         a.alpha = alpha_dev; a.payload = payload_dev;
@@ -289,7 +293,7 @@ int fusefss_keygen(const fusefss_program *prog, const uint64_t *r_in_dev, const 
         for (int t = 0; t < P->T; ++t)
             a.atom[t] = GenAtomDev{P->atoms[t].c, P->atoms[t].beta, 0, 0, 0, P->atoms[t].k, P->atoms[t].is_theta};
         const int grid = grid_for(tiles, kGenThreads);
-        rc = g_ntab == 4 ? launch(k_gen_misc<4>, grid, kGenThreads, smem, st, a) : launch(k_gen_misc<1>, grid, kGenThreads, smem, st, a);
+        rc = launch(k_gen_misc, grid, kGenThreads, kAesSmemBytes, st, a);
         if (rc) return rc;
     }
     return 0;
@@ -312,8 +316,7 @@ int fusefss_eval_cmp(int party, const fusefss_program *prog, const void *key_dev
     for (int t = 0; t < P->T; ++t) a.atom[t] = CmpAtomDev{P->atoms[t].c, L.bt_root[t], L.bt_cw[t], L.bt_vb[t], P->atoms[t].k, 0};
     if (a.G > 1) CU(cudaMemsetAsync(bits_out_dev, 0, count * 8, st));
     const int grid = grid_for(((count + 31) / 32) * (size_t)a.G, g_eval_threads);
-    return g_ntab == 4 ? launch(k_eval_cmp<4>, grid, g_eval_threads, aes_smem_bytes<4>(), st, a)
-                       : launch(k_eval_cmp<1>, grid, g_eval_threads, aes_smem_bytes<1>(), st, a);
+    return launch(k_eval_cmp, grid, g_eval_threads, kAesSmemBytes, st, a);
 }
 
 int fusefss_eval_lut(int party, const fusefss_program *prog, const void *key_dev, const uint64_t *xhat_dev, size_t count,
@@ -334,7 +337,7 @@ int fusefss_eval_lut(int party, const fusefss_program *prog, const void *key_dev
     a.G = pick_groups(count, P->M - 1, g_eval_threads);
     if (a.G > 1) CU(cudaMemsetAsync(coeff_out_dev, 0, count * 8 * (size_t)P->p, st));
     const int grid = grid_for(((count + 31) / 32) * (size_t)a.G, g_eval_threads);
-    rc = g_ntab == 4 ? launch_eval_lut_p<4>(P->p, grid, g_eval_threads, st, a) : launch_eval_lut_p<1>(P->p, grid, g_eval_threads, st, a);
+    rc = launch_eval_lut_p(P->p, grid, g_eval_threads, st, a);
     if (rc) return rc;
     if (a.G > 1 && P->n < 64) {
         const size_t words = count * (size_t)P->p;
@@ -458,16 +461,14 @@ int fusefss_gate_host(const fusefss_program *prog, const uint64_t *r_in, const u
 // ---- PRG micro-kernels: roofline denominator probe and FIPS-197 known-answer path --------------------
 namespace fsk {
 struct ProbeArgs { uint4 *out; size_t threads; int iters; };
-template <int NTAB>
 __global__ void __launch_bounds__(kEvalThreads, 1) k_aes_probe(const ProbeArgs a) {
     extern __shared__ uint32_t sT[];
-    aes_fill_tables<NTAB>(sT);
-    const uint32_t *tl = sT + (threadIdx.x & 31);
+    const uint32_t tl = aes_fill_tables(sT);
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < a.threads; i += (size_t)gridDim.x * blockDim.x) {
         uint32_t x[1][4] = {{(uint32_t)i, (uint32_t)(i >> 32), 0x9e3779b9u, 0x7f4a7c15u}};
         for (int it = 0; it < a.iters; it += 3) {                       // 3 independent keys per trip, like a p = 3 level
             uint32_t o[1][3][4];
-            prg_blocks<NTAB, 1, 3, 0>(tl, x, o);
+            prg_blocks<1, 3, 0>(tl, x, o);
 #pragma unroll
             for (int c = 0; c < 4; ++c) x[0][c] = o[0][0][c] ^ o[0][1][(c + 1) & 3] ^ o[0][2][(c + 2) & 3];
         }
@@ -475,13 +476,12 @@ __global__ void __launch_bounds__(kEvalThreads, 1) k_aes_probe(const ProbeArgs a
     }
 }
 struct KatArgs { uint4 *out; uint32_t in[4]; RoundKeys rk; };
-template <int NTAB>
 __global__ void k_aes_kat(const KatArgs a) {
     extern __shared__ uint32_t sT[];
-    aes_fill_tables<NTAB>(sT);
+    const uint32_t tl = aes_fill_tables(sT);
     if (threadIdx.x == 0) {
         uint32_t s[4] = {a.in[0], a.in[1], a.in[2], a.in[3]};
-        aes_encrypt_rk<NTAB>(sT + 0, a.rk, s);
+        aes_encrypt_rk(tl, a.rk, s);
         a.out[0] = make_uint4(s[0], s[1], s[2], s[3]);
     }
 }
@@ -495,8 +495,7 @@ int fusefss_aes_probe(size_t threads, int iters, void *out_dev, void *stream) {
     int rc = init_device(); if (rc) return rc;
     ProbeArgs a{(uint4 *)out_dev, threads, iters};
     const int grid = grid_for((threads + 31) / 32, g_eval_threads);
-    return g_ntab == 4 ? launch(k_aes_probe<4>, grid, g_eval_threads, aes_smem_bytes<4>(), (cudaStream_t)stream, a)
-                       : launch(k_aes_probe<1>, grid, g_eval_threads, aes_smem_bytes<1>(), (cudaStream_t)stream, a);
+    return launch(k_aes_probe, grid, g_eval_threads, kAesSmemBytes, (cudaStream_t)stream, a);
 }
 
 int fusefss_aes_kat(const uint8_t *key, const uint8_t *in, void *out_dev, void *stream) {
@@ -506,8 +505,7 @@ int fusefss_aes_kat(const uint8_t *key, const uint8_t *in, void *out_dev, void *
     a.out = (uint4 *)out_dev;
     std::memcpy(a.in, in, 16);
     host_aes().expand(key, a.rk.w);
-    return g_ntab == 4 ? launch(k_aes_kat<4>, 1, 256, aes_smem_bytes<4>(), (cudaStream_t)stream, a)
-                       : launch(k_aes_kat<1>, 1, 256, aes_smem_bytes<1>(), (cudaStream_t)stream, a);
+    return launch(k_aes_kat, 1, 256, kAesSmemBytes, (cudaStream_t)stream, a);
 }
 
 }  // extern "C"
