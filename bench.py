@@ -28,6 +28,8 @@ sys.path.insert(0, ROOT)
 METRIC = "compiled-op elements/s (keygen + cmp+LUT eval both parties + post); also eval-only and keygen-only elems/s; key B/elem"
 SM_CLOCK_MAX_MHZ = 1965.0
 LOOKUPS_PER_AES = 160           # 16 table lookups x 10 rounds (DESIGN 5.2)
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` (profiles/r1b_gelu.md, r1a_launches_gelu.md)
+NCU_TRAFFIC = {("gelu", 393216, "k_gen_vec"): 20.405e9, ("gelu", 393216, "k_eval_lut"): 10.276e9}
 LDS_LANES_PER_CLK_SM = 32       # shared-memory crossbar: 128 B/clk/SM (B300_MICROARCH "LDS/STS")
 
 
@@ -173,14 +175,15 @@ def main():
         for first in range(0, count, chunk):
             c = min(chunk, count - first)
             sl = slice(first, first + c)
+            gfirst = rank * count + first                       # global element index: rank r owns [r*count, (r+1)*count)
             e = [ev() for _ in range(7)]
             ro = r_out[:, sl].contiguous() if spec.mask_output else r_out
             e[0].record()
-            P.keygen(r_in[sl], ro, step.seed, first, keys=(k0, k1), parts=1)          # T bit-DCF keys      (k_gen_bit)
+            P.keygen(r_in[sl], ro, step.seed, gfirst, keys=(k0, k1), parts=1)          # T bit-DCF keys      (k_gen_bit)
             e[5].record()
-            P.keygen(r_in[sl], ro, step.seed, first, keys=(k0, k1), parts=2)          # M-1 vector-DCF keys (k_gen_vec)
+            P.keygen(r_in[sl], ro, step.seed, gfirst, keys=(k0, k1), parts=2)          # M-1 vector-DCF keys (k_gen_vec)
             e[6].record()
-            P.keygen(r_in[sl], ro, step.seed, first, keys=(k0, k1), parts=4)          # share splitting     (k_gen_misc)
+            P.keygen(r_in[sl], ro, step.seed, gfirst, keys=(k0, k1), parts=4)          # share splitting     (k_gen_misc)
             e[1].record()
             if sh["T"]:
                 for b, k in ((0, k0), (1, k1)):
@@ -234,7 +237,6 @@ def main():
     Q = (sh["p"] + 1) // 2
     n_chunks = len(step.events)
     full_chunk_frac = count / (chunk * ((count + chunk - 1) // chunk))      # tail chunk: fewer blocks per launch
-    peak = 148 * SM_CLOCK_MAX_MHZ * 1e6 * LDS_LANES_PER_CLK_SM / LOOKUPS_PER_AES / 1e9
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
@@ -244,27 +246,37 @@ def main():
     key_b = P.key_bytes(1 << 20) / (1 << 20)
     lut_key_bytes = (8 * sh["p"] + (sh["M"] - 1) * (16 + spec.n * (16 + 8 * sh["p"]) + 8 * sh["p"])) if sh["has_lut"] else 0
 
-    def roof(kernel, aes_per_launch_elem, launches_per_chunk, times, bytes_per_elem):
+    def grp(B):                                   # table lookups of B blocks that share their round-1 input (DESIGN 5.2)
+        return 15 + B + 144 * B if B > 1 else 160
+
+    def roof(kernel, aes_per_launch_elem, launches_per_chunk, times, bytes_per_elem, lookups_per_elem):
+        lookups_per_aes = lookups_per_elem / max(1, aes_per_launch_elem)
+        peak = 148 * SM_CLOCK_MAX_MHZ * 1e6 * LDS_LANES_PER_CLK_SM / lookups_per_aes / 1e9
         n_launch = launches_per_chunk * n_chunks
         launch_ms = sum(times) / max(1, n_launch)
         per_launch = aes_per_launch_elem * chunk * full_chunk_frac
         ach = per_launch / (launch_ms * 1e-3) / 1e9 if launch_ms > 0 else 0.0
         gbs = bytes_per_elem * chunk * full_chunk_frac / (launch_ms * 1e-3) / 1e9 if launch_ms > 0 else 0.0
         return {"bound": "alu", "kernel": kernel, "achieved": ach, "peak": peak,
-                "unit": "GAES/s (AES-128 blocks per second; 160 conflict-free LDS.32 table lookups each)",
-                "frac": ach / peak, "traffic": None,
-                "peak_derivation": "148 SMs x 1.965 GHz x 32 shared-memory lanes/clk/SM / 160 lookups per AES block (DESIGN 5.2)",
+                "unit": "GAES/s (AES-128 blocks per second)", "lookups_per_aes": lookups_per_aes,
+                "frac": ach / peak, "traffic": NCU_TRAFFIC.get((name, count, kernel)),
+                "peak_derivation": "148 SMs x 1.965 GHz x 32 conflict-free shared-memory lanes/clk/SM / lookups_per_aes (160 per block, less the round-1 lookups shared by blocks of one seed; DESIGN 5.2)",
                 "launch_ms": launch_ms, "aes_per_launch": per_launch, "share_of_step": sum(times) / (ms_step * args.steps),
                 "hbm_achieved_gbs": gbs, "hbm_peak_gbs": hbm_peak, "hbm_frac": gbs / hbm_peak,
                 "hbm_peak_source": "measured (MEASURED_PEAKS.json)" if peaks else "fallback"}
     vec_gen_aes = (sh["M"] - 1) * (4 * spec.n * (1 + Q) + 2 * Q + 2) if sh["has_lut"] else 0
     vec_eval_aes = (sh["M"] - 1) * (spec.n * (1 + Q) + Q) if sh["has_lut"] else 0
-    roofs = {"k_gen_vec": roof("k_gen_vec", vec_gen_aes, 1, t_genvec, 2 * (lut_key_bytes - 8 * sh["p"])),
-             "k_eval_lut": roof("k_eval_lut", vec_eval_aes, 2, t_lut, lut_key_bytes)}
+    vec_gen_lookups = (sh["M"] - 1) * (2 * spec.n * grp(2 * (1 + Q)) + 2 * grp(Q) + 2 * 160) if sh["has_lut"] else 0
+    vec_eval_lookups = (sh["M"] - 1) * (spec.n * grp(1 + Q) + grp(Q)) if sh["has_lut"] else 0
+    roofs = {"k_gen_vec": roof("k_gen_vec", vec_gen_aes, 1, t_genvec, 2 * (lut_key_bytes - 8 * sh["p"]), vec_gen_lookups),
+             "k_eval_lut": roof("k_eval_lut", vec_eval_aes, 2, t_lut, lut_key_bytes, vec_eval_lookups)}
     dominant = max(roofs.values(), key=lambda r: r["share_of_step"])
     roofline = dict(dominant)
     roofline["other_kernels"] = {k: {kk: v[kk] for kk in ("achieved", "frac", "launch_ms", "share_of_step", "hbm_achieved_gbs")}
                                  for k, v in roofs.items() if v is not dominant}
+    for k, v in roofs.items():
+        if v is not dominant:
+            roofline["other_kernels"][k]["traffic"] = v["traffic"]
 
     line = {"metric": METRIC, "value": value, "unit": "elements/s", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64",

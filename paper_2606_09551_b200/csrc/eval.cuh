@@ -138,7 +138,7 @@ __global__ void __launch_bounds__(kEvalThreads, 1) k_eval_lut(const __grid_const
                 u <<= 1;
                 uint32_t x[1][4] = {{s.x | dbit, s.y, s.z, s.w}};
                 uint32_t o[1][1 + Q][4];
-                prg_blocks<1, 1 + Q, 0>(tl, x, o);
+                prg_blocks<1, 1 + Q, 0, true>(tl, x, o);
                 const uint32_t tm = 0u - tb;
                 const uint64_t tm64 = 0ull - (uint64_t)tb;
 #pragma unroll
@@ -159,7 +159,7 @@ __global__ void __launch_bounds__(kEvalThreads, 1) k_eval_lut(const __grid_const
             // leaf: V += conv(s) + t * fin; party 1 negates
             uint32_t x[1][4] = {{s.x | 2u, s.y, s.z, s.w}};
             uint32_t o[1][Q][4];
-            prg_blocks<1, Q, 1>(tl, x, o);
+            prg_blocks<1, Q, 1, true>(tl, x, o);
             const uint64_t tm64 = 0ull - (uint64_t)tb;
             const uint8_t *fin = tree + a.vt_fin_rel;
 #pragma unroll

@@ -71,12 +71,18 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_bit(const __grid_constan
             const uint32_t abit = (uint32_t)(alpha >> 63);
             alpha <<= 1;
             // children: index 2*b + d
-            uint32_t x[4][4], o[4][1][4];
+            uint32_t o[4][1][4];
 #pragma unroll
-            for (int b = 0; b < 2; ++b)
+            for (int b = 0; b < 2; ++b) {
+                uint32_t x[2][4], ob[2][1][4];
 #pragma unroll
-                for (int d = 0; d < 2; ++d) { x[2 * b + d][0] = s[b][0] | (uint32_t)d; x[2 * b + d][1] = s[b][1]; x[2 * b + d][2] = s[b][2]; x[2 * b + d][3] = s[b][3]; }
-            prg_blocks<4, 1, 0>(tl, x, o);
+                for (int d = 0; d < 2; ++d) { x[d][0] = s[b][0] | (uint32_t)d; x[d][1] = s[b][1]; x[d][2] = s[b][2]; x[d][3] = s[b][3]; }
+                prg_blocks<2, 1, 0, true>(tl, x, ob);
+#pragma unroll
+                for (int d = 0; d < 2; ++d)
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) o[2 * b + d][0][c] = ob[d][0][c];
+            }
             const uint32_t am = 0u - abit;                    // keep = alpha_i, lose = 1 - alpha_i
             uint32_t keep0[4], keep1[4], scw[4];
 #pragma unroll
@@ -225,7 +231,7 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec(const __grid_constan
                 uint32_t x[2][4], o[2][1 + Q][4];
 #pragma unroll
                 for (int d = 0; d < 2; ++d) { x[d][0] = s[b][0] | (uint32_t)d; x[d][1] = s[b][1]; x[d][2] = s[b][2]; x[d][3] = s[b][3]; }
-                prg_blocks<2, 1 + Q, 0>(tl, x, o);
+                prg_blocks<2, 1 + Q, 0, true>(tl, x, o);
                 Tb[b][0] = o[0][0][0] & 1u; Tb[b][1] = o[1][0][0] & 1u;
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
@@ -270,10 +276,16 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec(const __grid_constan
             t0 = nt0; t1 = nt1;
         }
         // final correction word: fin = (-1)^{t_1} (conv(s_1) - conv(s_0) - Valpha)
-        uint32_t x[2][4], o[2][Q][4];
+        uint32_t o[2][Q][4];
 #pragma unroll
-        for (int b = 0; b < 2; ++b) { x[b][0] = s[b][0] | 2u; x[b][1] = s[b][1]; x[b][2] = s[b][2]; x[b][3] = s[b][3]; }
-        prg_blocks<2, Q, 1>(tl, x, o);
+        for (int b = 0; b < 2; ++b) {
+            uint32_t x[1][4] = {{s[b][0] | 2u, s[b][1], s[b][2], s[b][3]}}, ob[1][Q][4];
+            prg_blocks<1, Q, 1, true>(tl, x, ob);
+#pragma unroll
+            for (int q = 0; q < Q; ++q)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) o[b][q][c] = ob[0][q][c];
+        }
         const uint64_t sgn = 0ull - (uint64_t)t1;
 #pragma unroll
         for (int w = 0; w < P; ++w) {

@@ -46,6 +46,9 @@ int init_device() {
                 key[0] = (uint8_t)i;
                 h.expand(key, rk[i]);
             }
+            // prg_blocks<.., SHARED> relies on the PRG keys agreeing outside byte 0 of round key 0
+            for (int i = 1; i < kNumPrgKeys; ++i)
+                if ((rk[i][0] ^ rk[0][0]) & ~0xffu || rk[i][1] != rk[0][1] || rk[i][2] != rk[0][2] || rk[i][3] != rk[0][3]) return FUSEFSS_E_SPEC;
             CU(cudaMemcpyToSymbol(c_T0, h.T0, sizeof h.T0));
             CU(cudaMemcpyToSymbol(c_rk, rk, sizeof rk));
             int dev = 0;
