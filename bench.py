@@ -28,8 +28,8 @@ sys.path.insert(0, ROOT)
 METRIC = "compiled-op elements/s (keygen + cmp+LUT eval both parties + post); also eval-only and keygen-only elems/s; key B/elem"
 SM_CLOCK_MAX_MHZ = 1965.0
 LOOKUPS_PER_AES = 160           # 16 table lookups x 10 rounds (DESIGN 5.2)
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` (profiles/r1b_gelu.md, r1a_launches_gelu.md)
-NCU_TRAFFIC = {("gelu", 393216, "k_gen_vec"): 20.405e9, ("gelu", 393216, "k_eval_lut"): 10.276e9}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` (profiles/r1c_gelu.md)
+NCU_TRAFFIC = {("gelu", 393216, "k_gen_vec"): 20.406e9, ("gelu", 393216, "k_eval_lut"): 10.279e9}
 LDS_LANES_PER_CLK_SM = 32       # shared-memory crossbar: 128 B/clk/SM (B300_MICROARCH "LDS/STS")
 
 

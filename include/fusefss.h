@@ -82,6 +82,7 @@ typedef struct {
     uint32_t n_nodes, n_kappa_a, n_kappa_b, phi_len;
     uint32_t n_out_a, n_out_b;        /* outputs of Phi (ignored when phi_len == 0: outputs are y and z)    */
     uint32_t mask_output;             /* 1: arithmetic outputs are opened as yhat = y + r_out       */
+    uint32_t variant;                 /* 0: Protocol-3 construction; 1: single-key shared-prefix (DESIGN 9) */
     const uint64_t *alpha;            /* HOST [m-1] interior boundaries, strictly increasing in (0, 2^n)    */
     const uint64_t *coeff;            /* HOST [m][r][d+1], high degree first                                */
     const uint64_t *aux;              /* HOST [m][p_aux]                                                    */

@@ -44,7 +44,7 @@ class _PhiOp(C.Structure):
 class _Spec(C.Structure):
     _fields_ = [(k, C.c_uint32) for k in (
         "n", "frac_bits", "m", "r", "d", "p_aux", "ell", "n_nodes", "n_kappa_a", "n_kappa_b", "phi_len",
-        "n_out_a", "n_out_b", "mask_output")] + [
+        "n_out_a", "n_out_b", "mask_output", "variant")] + [
         ("alpha", C.c_void_p), ("coeff", C.c_void_p), ("aux", C.c_void_p), ("nodes", C.c_void_p),
         ("bit_root", C.c_void_p), ("kappa_a", C.c_void_p), ("kappa_b", C.c_void_p), ("phi", C.c_void_p)]
 
@@ -94,7 +94,7 @@ class _SpecHolder:
         for i, (op, dst, a, b, imm) in enumerate(s.phi):
             self.phi[i] = _PhiOp(op, dst, a, b, 0, imm & 0xFFFFFFFFFFFFFFFF)
         self.c = _Spec(s.n, s.f, s.m, s.r, s.d, s.p_aux, s.ell, len(s.nodes), len(s.kappa_a), len(s.kappa_b),
-                       len(s.phi), s.n_out_a, s.n_out_b, int(s.mask_output),
+                       len(s.phi), s.n_out_a, s.n_out_b, int(s.mask_output), int(getattr(s, "variant", 0)),
                        _p(self.alpha), _p(self.coeff), _p(self.aux), C.cast(self.nodes, C.c_void_p),
                        _p(self.bit_root), C.cast(self.ka, C.c_void_p), C.cast(self.kb, C.c_void_p),
                        C.cast(self.phi, C.c_void_p))

@@ -410,7 +410,7 @@ typedef struct { u8 op, dst, a, b; u32 pad; u64 imm; } orc_phi_op;
 
 typedef struct {
     u32 n, frac_bits, m, r, d, p_aux, ell;
-    u32 n_nodes, n_kappa_a, n_kappa_b, phi_len, n_out_a, n_out_b, mask_output;
+    u32 n_nodes, n_kappa_a, n_kappa_b, phi_len, n_out_a, n_out_b, mask_output, variant;
     const u64 *alpha;            /* m-1 interior boundaries (alpha_0 = 0, alpha_m = 2^n implied) */
     const u64 *coeff;            /* [m][r][d+1], high degree first                                */
     const u64 *aux;              /* [m][p_aux]                                                    */

@@ -41,7 +41,7 @@ class PhiOp(C.Structure):
 
 class Spec(C.Structure):
     _fields_ = [(k, C.c_uint32) for k in ("n", "frac_bits", "m", "r", "d", "p_aux", "ell", "n_nodes", "n_kappa_a",
-                                          "n_kappa_b", "phi_len", "n_out_a", "n_out_b", "mask_output")] + \
+                                          "n_kappa_b", "phi_len", "n_out_a", "n_out_b", "mask_output", "variant")] + \
                [(k, C.c_void_p) for k in ("alpha", "coeff", "aux", "nodes", "bit_root", "kappa_a", "kappa_b", "phi")]
 
 
@@ -132,7 +132,7 @@ class _SpecHolder:
         self.phi = (PhiOp * max(1, len(s.phi)))(*[PhiOp(op, dst, a, b, 0, imm & 0xFFFFFFFFFFFFFFFF)
                                                   for (op, dst, a, b, imm) in s.phi])
         self.c = Spec(s.n, s.f, s.m, s.r, s.d, s.p_aux, s.ell, len(s.nodes), len(s.kappa_a), len(s.kappa_b),
-                      len(s.phi), s.n_out_a, s.n_out_b, int(s.mask_output),
+                      len(s.phi), s.n_out_a, s.n_out_b, int(s.mask_output), int(getattr(s, "variant", 0)),
                       _np_ptr(self.alpha), _np_ptr(self.coeff), _np_ptr(self.aux), C.cast(self.nodes, C.c_void_p),
                       _np_ptr(self.bit_root), C.cast(self.ka, C.c_void_p), C.cast(self.kb, C.c_void_p),
                       C.cast(self.phi, C.c_void_p))

@@ -43,6 +43,7 @@ class OpSpec:
     out_frac: int = 0      # fractional bits of the arithmetic outputs (metadata for decode)
     domain: tuple = None   # real interval on which the spline error is stated
     func: object = None    # real function approximated (metadata for tests)
+    variant: int = 0       # 0: Protocol-3 construction (one key per query / boundary); 1: single-key shared-prefix (DESIGN 9)
 
     @property
     def m(self):
@@ -330,6 +331,12 @@ def full_partition(n=3):
     """m = N: M = N, no padding possible (Protocol 3 line 2 / line 12)."""
     N = 1 << n
     return _mk(f"full_n{n}", n, 0, list(range(1, N)), [[[i * 3 + 1]] for i in range(N)], n_out_a=1)
+
+
+def shared_prefix(spec):
+    """The same operator compiled with the single-key, multi-point construction."""
+    import dataclasses
+    return dataclasses.replace(spec, variant=1, name=spec.name + "_sp")
 
 
 CONFIGS = {
