@@ -522,7 +522,7 @@ void orc_plain_G(const orc_spec *S, u64 x, u64 r, u64 *yo, u8 *zo)
 /* ------------------------------------------------------------------------- */
 /* 6. Spec-level compile (Protocol 3 steps (2)-(4))  */
 /* ------------------------------------------------------------------------- */
-typedef struct { int k; u64 c; int nbeta; u64 beta[TMAX]; int first_atom; } view_t;
+typedef struct { int k; u64 c; int nbeta; u64 beta[TMAX]; int first_atom; int want_carry; } view_t;
 typedef struct { int k; u64 c; int is_theta; u64 beta; int carry_idx; } atom_t;
 
 enum {
@@ -549,12 +549,20 @@ typedef struct orc_prog {
     /* lowering memo */
     int node_reg[4096];
     int calpha_reg[MMAX + 1];
+    /* variant 1 (single-key shared-prefix construction): one DCF key per view width,
+     * threshold r mod 2^k, evaluated at the public points (xhat + delta) mod 2^k */
+    int variant;
+    int n_w, wk[8], w_npts[8];        /* widths in first-appearance order; points per width             */
+    u64 w_delta[8][2 * TMAX + 2];     /* offsets delta, sorted by signed value                           */
+    int atom_w[TMAX], atom_ib[TMAX], atom_ia[TMAX];   /* per atom: width, point of (c), point of (c - beta) */
+    int alpha_atom[MMAX];             /* atom index of the boundary comparison C_{alpha_i}, i = 1..m-1   */
 } orc_prog;
 
 static int find_view(orc_prog *P, int k, u64 c)
 {
     for (int v = 0; v < P->nviews; v++) if (P->views[v].k == k && P->views[v].c == c) return v;
     P->views[P->nviews].k = k; P->views[P->nviews].c = c; P->views[P->nviews].nbeta = 0;
+    P->views[P->nviews].want_carry = 0;
     return P->nviews++;
 }
 static void add_pred(orc_prog *P, int k, u64 c, u64 beta)
@@ -602,6 +610,7 @@ static int e_band(orc_prog *P, int a, int b)
 static int e_pred(orc_prog *P, int k, u64 c, u64 beta)
 {
     int at = theta_atom(P, k, c, beta), ar = r_atom(P, k, c);
+    if (P->variant) { int r0 = newb(P, 0); emit(P, C_B_ATOM, r0, at, 0, 0); return r0; }   /* DESIGN 9: no carry, no r-atom */
     int r1 = newb(P, 0); emit(P, C_B_ATOM, r1, at, 0, 0);
     int r2 = newb(P, 0); emit(P, C_B_ATOM, r2, ar, 0, 0);
     int r3 = newb(P, 0); emit(P, C_B_KAPPA, r3, P->atoms[at].carry_idx, 0, 0);
@@ -669,6 +678,45 @@ void orc_destroy(orc_prog *P)
     free(P);
 }
 
+/* variant 1: evaluation points.  For a predicate atom (k, c, beta): I[view_{k,c}(x) < beta] = e - b + a with
+ * h = (xhat + c) mod 2^k, e = I[h < beta] public, b = I[h < r_k], a = I[(h - beta) mod 2^k < r_k]  (checked
+ * exhaustively in tests/test_oracle_sp.py); b and a are the ONE DCF f_{r_k,1} at the offsets c and c - beta. */
+static int sp_point(orc_prog *P, int w, u64 delta)
+{
+    for (int j = 0; j < P->w_npts[w]; j++) if (P->w_delta[w][j] == delta) return j;
+    P->w_delta[w][P->w_npts[w]] = delta;
+    return P->w_npts[w]++;
+}
+static int sp_points(orc_prog *P)
+{
+    P->n_w = 0;
+    for (int t = 0; t < P->T; t++) {                     /* widths in first-appearance order */
+        int w = -1;
+        for (int i = 0; i < P->n_w; i++) if (P->wk[i] == P->atoms[t].k) w = i;
+        if (w < 0) { if (P->n_w >= 8) return -1; w = P->n_w++; P->wk[w] = P->atoms[t].k; P->w_npts[w] = 0; }
+        P->atom_w[t] = w;
+    }
+    for (int pass = 0; pass < 2; pass++) {               /* pass 0 collects, then sort, pass 1 resolves indices */
+        for (int t = 0; t < P->T; t++) {
+            const atom_t *a = &P->atoms[t];
+            int w = P->atom_w[t];
+            u64 km = low_mask(a->k);
+            P->atom_ib[t] = sp_point(P, w, a->c & km);
+            P->atom_ia[t] = a->is_theta ? sp_point(P, w, (a->c - a->beta) & km) : -1;
+        }
+        if (pass == 0) for (int w = 0; w < P->n_w; w++) {    /* ascending as signed k-bit values */
+            int k = P->wk[w]; u64 half = (u64)1 << (k - 1);
+            for (int i = 1; i < P->w_npts[w]; i++) {
+                u64 v = P->w_delta[w][i]; int j = i;
+                while (j > 0 && ((P->w_delta[w][j - 1] ^ half) > (v ^ half))) { P->w_delta[w][j] = P->w_delta[w][j - 1]; j--; }
+                P->w_delta[w][j] = v;
+            }
+        }
+    }
+    for (int i = 1; i < P->m; i++) P->alpha_atom[i] = P->has_lut ? theta_atom(P, P->n, 0, P->S.alpha[i - 1]) : -1;
+    return 0;
+}
+
 orc_prog *orc_compile(const orc_spec *S0)
 {
     prg_init();
@@ -697,6 +745,8 @@ orc_prog *orc_compile(const orc_spec *S0)
     u128 N = (u128)1 << P->n;
     P->M = ((u128)(P->m + 1) < N) ? P->m + 1 : (int)N;
     P->has_lut = P->m > 1;                               /* single interval: lookup omitted */
+    P->variant = (int)S->variant;
+    if (P->variant) P->M = P->m;                         /* no translated partition, hence no wrap/dummy split */
     for (int i = 0; i < 4096; i++) P->node_reg[i] = -1;
     for (int i = 0; i <= MMAX; i++) P->calpha_reg[i] = -1;
 
@@ -707,25 +757,30 @@ orc_prog *orc_compile(const orc_spec *S0)
         if (nd->kind == BN_C && !nd->value_is_2k && nd->value != 0) add_pred(P, P->n, 0, nd->value);
         if (nd->kind == BN_D && !nd->value_is_2k && nd->value != 0) add_pred(P, nd->k, 0, nd->value);
         if (nd->kind == BN_MSB) add_pred(P, P->n, nd->value & P->mask, (u64)1 << (P->n - 1));
-        if (nd->kind == BN_CARRY) find_view(P, nd->k, 0);
+        if (nd->kind == BN_CARRY) P->views[find_view(P, nd->k, 0)].want_carry = 1;
     }
     int piecewise = 0;
     for (u32 j = 0; j < S->ell; j++) if (!bit_is_uniform(S, j)) piecewise = 1;
-    if (piecewise) for (int i = 1; i < P->m; i++) add_pred(P, P->n, 0, S->alpha[i - 1]);
+    if (piecewise || (S->variant && P->m > 1)) for (int i = 1; i < P->m; i++) add_pred(P, P->n, 0, S->alpha[i - 1]);
     /* flatten: per view, the r-atom then one theta-atom per distinct beta */
     P->T = 0; P->n_carry = 0;
     for (int v = 0; v < P->nviews; v++) {
         view_t *V = &P->views[v];
         V->first_atom = P->T;
         if (P->T + 1 + V->nbeta > TMAX) { orc_destroy(P); return NULL; }
-        atom_t *a = &P->atoms[P->T++];
-        a->k = V->k; a->c = V->c; a->is_theta = 0; a->beta = 0; a->carry_idx = -1;
+        atom_t *a;
+        if (!S->variant || V->want_carry) {              /* variant 1 keeps the r-atom only where a CARRY node reads it */
+            a = &P->atoms[P->T++];
+            a->k = V->k; a->c = V->c; a->is_theta = 0; a->beta = 0; a->carry_idx = -1;
+        }
         for (int j = 0; j < V->nbeta; j++) {
             a = &P->atoms[P->T++];
-            a->k = V->k; a->c = V->c; a->is_theta = 1; a->beta = V->beta[j]; a->carry_idx = P->n_carry++;
+            a->k = V->k; a->c = V->c; a->is_theta = 1; a->beta = V->beta[j];
+            a->carry_idx = S->variant ? -1 : P->n_carry++;
         }
     }
     P->n_kb = P->n_carry + (int)S->n_kappa_b;
+    if (S->variant && sp_points(P) < 0) { orc_destroy(P); return NULL; }
 
     /* program: Horner (step-major), Boolean circuit (bit-major), then Phi */
     int xreg = newa(P, 0); emit(P, C_A_X, xreg, 0, 0, 0);
@@ -907,13 +962,29 @@ static void layout(const orc_prog *P, size_t count, layout_t *L)
 {
     size_t off = 0;
     L->s16 = rup256(count * 16); L->s8 = rup256(count * 8);
-    for (int t = 0; t < P->T; t++) {
+    if (P->variant) {
+        /* one tree per view width, in width order: k < n -> bit-DCF arrays (root, k levels, VCW bits);
+         * k = n -> vector-DCF arrays with p = 1 (root, n levels of {sCW, VCW}, fin) */
+        L->lvl_stride = L->s16 + L->s8;
+        for (int w = 0; w < P->n_w; w++) {
+            if (P->wk[w] < P->n) {
+                L->bt_root[w] = off; off += L->s16;
+                L->bt_cw[w] = off; off += L->s16 * (size_t)P->wk[w];
+                L->bt_vb[w] = off; off += L->s8;
+            } else {
+                L->vt_root[1] = off; off += L->s16;
+                L->vt_lvl[1] = off; off += L->lvl_stride * (size_t)P->n;
+                L->vt_fin[1] = off; off += L->s8;
+            }
+        }
+    }
+    for (int t = 0; t < P->T && !P->variant; t++) {
         L->bt_root[t] = off; off += L->s16;
         L->bt_cw[t] = off; off += L->s16 * (size_t)P->atoms[t].k;
         L->bt_vb[t] = off; off += L->s8;
     }
-    L->lvl_stride = L->s16 + (size_t)P->p * L->s8;
-    if (P->has_lut) {
+    if (!P->variant) L->lvl_stride = L->s16 + (size_t)P->p * L->s8;
+    if (P->has_lut && !P->variant) {
         L->lut_c = off; off += (size_t)P->p * L->s8;
         for (int j = 1; j < P->M; j++) {
             L->vt_root[j] = off; off += L->s16;
@@ -980,7 +1051,36 @@ void orc_keygen(const orc_prog *P, const u64 *r_in, const u64 *r_out, u64 seed, 
         u8 rb[16], rb1[16];
         /* ---- packed comparison instance: one bit-DCF per atom ---- */
         u64 kbits = 0;
-        for (int t = 0; t < P->T; t++) {
+        if (P->variant) {                                               /* DESIGN 9: one key per view width, threshold r_k */
+            for (int w = 0; w < P->n_w; w++) {
+                int k = P->wk[w];
+                if (k < n) {
+                    rnd(&ks, ge, SLOT_BT_ROOT + 2 * w, rb); rnd(&ks, ge, SLOT_BT_ROOT + 2 * w + 1, rb1);
+                    dcf_bit_gen(k, r & low_mask(k), rb, rb1, bk0, bk1);
+                    bitkey *bk[2] = { bk0, bk1 };
+                    for (int b = 0; b < 2; b++) {
+                        st16(key[b], L.bt_root[w], e, bk[b]->root);
+                        for (int i = 0; i < k; i++) st16(key[b], L.bt_cw[w] + (size_t)i * L.s16, e, bk[b]->cw[i]);
+                        st8(key[b], L.bt_vb[w], e, bk[b]->vbits);
+                    }
+                } else {
+                    u64 one = 1 & mask;
+                    rnd(&ks, ge, SLOT_VT_ROOT + 2, rb); rnd(&ks, ge, SLOT_VT_ROOT + 3, rb1);
+                    dcf_vec_gen(n, 1, mask, r, &one, rb, rb1, vk0, vk1);
+                    veckey *vk[2] = { vk0, vk1 };
+                    for (int b = 0; b < 2; b++) {
+                        st16(key[b], L.vt_root[1], e, vk[b]->root);
+                        for (int i = 0; i < n; i++) {
+                            size_t lo = L.vt_lvl[1] + (size_t)i * L.lvl_stride;
+                            st16(key[b], lo, e, vk[b]->scw[i]);
+                            st8(key[b], lo + L.s16, e, vk[b]->vcw[i][0]);
+                        }
+                        st8(key[b], L.vt_fin[1], e, vk[b]->fin[0]);
+                    }
+                }
+            }
+        }
+        for (int t = 0; t < P->T && !P->variant; t++) {
             const atom_t *a = &P->atoms[t];
             u64 rk = r & low_mask(a->k);
             u64 theta = rk;
@@ -1001,7 +1101,7 @@ void orc_keygen(const orc_prog *P, const u64 *r_in, const u64 *r_out, u64 seed, 
         }
         for (u32 t = 0; t < S->n_kappa_b; t++) kbits |= (u64)kappa_b_value(S, (int)t, r) << (P->n_carry + t);
         /* ---- interval lookup instance (Protocol 3 (1),(5); reading S2: sum of M-1 vector DCFs) ---- */
-        if (P->has_lut) {
+        if (P->has_lut && !P->variant) {
             u128 B[MMAX + 2]; int ord[MMAX + 1], M;
             protocol3(n, P->m, S->alpha, r, B, ord, &M);
             u64 v[MMAX + 1][PMAX];
@@ -1093,8 +1193,79 @@ void orc_keygen(const orc_prog *P, const u64 *r_in, const u64 *r_out, u64 seed, 
 /* ------------------------------------------------------------------------- */
 static void ld16(const u8 *base, size_t off, size_t e, u8 *v) { memcpy(v, base + off + e * 16, 16); }
 
+/* variant 1: A[w][j] = Eval_b(key_w, (xhat + delta_j) mod 2^k), every point from the root (plain definition) */
+static void sp_eval_points(int party, const orc_prog *P, const u8 *key, const layout_t *L, size_t e, u64 xh,
+                           bitkey *bk, veckey *vk, u64 A[8][2 * TMAX + 2])
+{
+    int n = P->n;
+    for (int w = 0; w < P->n_w; w++) {
+        int k = P->wk[w];
+        u64 km = low_mask(k);
+        if (k < n) {
+            ld16(key, L->bt_root[w], e, bk->root);
+            for (int i = 0; i < k; i++) ld16(key, L->bt_cw[w] + (size_t)i * L->s16, e, bk->cw[i]);
+            bk->vbits = ld8(key, L->bt_vb[w], e);
+            for (int j = 0; j < P->w_npts[w]; j++) A[w][j] = (u64)dcf_bit_eval(party, k, bk, (xh + P->w_delta[w][j]) & km);
+        } else {
+            ld16(key, L->vt_root[1], e, vk->root);
+            for (int i = 0; i < n; i++) {
+                size_t lo = L->vt_lvl[1] + (size_t)i * L->lvl_stride;
+                ld16(key, lo, e, vk->scw[i]);
+                vk->vcw[i][0] = ld8(key, lo + L->s16, e);
+            }
+            vk->fin[0] = ld8(key, L->vt_fin[1], e);
+            for (int j = 0; j < P->w_npts[w]; j++) dcf_vec_eval(party, n, 1, P->mask, vk, (xh + P->w_delta[w][j]) & km, &A[w][j]);
+        }
+    }
+}
+/* share of the predicate atom t: e - b + a in R (k = n) or e ^ b ^ a (k < n); r-atom: b itself */
+static u64 sp_atom_share(int party, const orc_prog *P, int t, u64 xh, u64 A[8][2 * TMAX + 2])
+{
+    const atom_t *a = &P->atoms[t];
+    int w = P->atom_w[t];
+    u64 km = low_mask(a->k);
+    u64 b = A[w][P->atom_ib[t]];
+    if (!a->is_theta) return b;
+    u64 h = (xh + a->c) & km;
+    u64 pub = (party == 0 && h < a->beta) ? 1 : 0;
+    u64 av = A[w][P->atom_ia[t]];
+    return a->k < P->n ? (pub ^ b ^ av) : ((pub - b + av) & P->mask);
+}
+static void sp_eval(int party, const orc_prog *P, const u8 *key, const u64 *xhat, size_t count, u64 *bits_out, u64 *coeff_out)
+{
+    layout_t L; layout(P, count, &L);
+    bitkey *bk = malloc(sizeof *bk); veckey *vk = malloc(sizeof *vk);
+    u64 (*A)[2 * TMAX + 2] = malloc(sizeof(u64) * 8 * (2 * TMAX + 2));
+    const orc_spec *S = &P->S;
+    u32 nc = S->r * (S->d + 1);
+    for (size_t e = 0; e < count; e++) {
+        u64 xh = xhat[e] & P->mask;
+        sp_eval_points(party, P, key, &L, e, xh, bk, vk, A);
+        if (bits_out) {
+            u64 word = 0;
+            for (int t = 0; t < P->T; t++) word |= (sp_atom_share(party, P, t, xh, A) & 1) << t;   /* LSB of an additive share of a bit = XOR share */
+            bits_out[e] = word;
+        }
+        if (coeff_out && P->has_lut) {
+            /* v_{i*} = v_{m-1} + sum_{i=1}^{m-1} (v_{i-1} - v_i) I[x < alpha_i]  (Lemma D.1 telescoped); v_i public */
+            for (int wd = 0; wd < P->p; wd++) {
+                u64 acc = 0;
+                for (int i = 0; i < P->m; i++) {
+                    u64 vi = (wd < (int)nc ? S->coeff[(size_t)i * nc + wd] : S->aux[(size_t)i * S->p_aux + (wd - nc)]) & P->mask;
+                    u64 vprev = i ? ((wd < (int)nc ? S->coeff[(size_t)(i - 1) * nc + wd] : S->aux[(size_t)(i - 1) * S->p_aux + (wd - nc)]) & P->mask) : 0;
+                    if (i) acc += (vprev - vi) * sp_atom_share(party, P, P->alpha_atom[i], xh, A);
+                    if (i == P->m - 1 && party == 0) acc += vi;
+                }
+                coeff_out[(size_t)wd * count + e] = acc & P->mask;
+            }
+        }
+    }
+    free(bk); free(vk); free(A);
+}
+
 void orc_eval_cmp(int party, const orc_prog *P, const u8 *key, const u64 *xhat, size_t count, u64 *bits_out)
 {
+    if (P->variant) { if (P->T) sp_eval(party, P, key, xhat, count, bits_out, NULL); return; }
     layout_t L; layout(P, count, &L);
     bitkey *bk = malloc(sizeof *bk);
     for (size_t e = 0; e < count; e++) {
@@ -1115,6 +1286,7 @@ void orc_eval_cmp(int party, const orc_prog *P, const u8 *key, const u64 *xhat, 
 
 void orc_eval_lut(int party, const orc_prog *P, const u8 *key, const u64 *xhat, size_t count, u64 *coeff_out)
 {
+    if (P->variant) { sp_eval(party, P, key, xhat, count, NULL, coeff_out); return; }
     layout_t L; layout(P, count, &L);
     if (!P->has_lut) return;
     veckey *vk = malloc(sizeof *vk);
