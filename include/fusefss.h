@@ -141,6 +141,14 @@ int fusefss_eval_cmp(int party, const fusefss_program *prog, const void *key_dev
 int fusefss_eval_lut(int party, const fusefss_program *prog, const void *key_dev, const uint64_t *xhat_dev,
                      size_t count, uint64_t *coeff_out_dev, void *stream);
 
+/* ---- a5 + a6 in one call -------------------------------------------------------------------------
+ * Writes both outputs of the two FSS calls.  For variant 1 (single-key shared-prefix construction, DESIGN 9) both
+ * come from ONE walk of the element's key at the public points xhat + delta_j, with the tree prefix shared by
+ * nearby points; for variant 0 it is eval_cmp followed by eval_lut.  bits_out_dev may be NULL iff T = 0,
+ * coeff_out_dev iff m = 1.  (eval_cmp / eval_lut remain valid for variant 1 and each walk only the points they need.) */
+int fusefss_eval_fused(int party, const fusefss_program *prog, const void *key_dev, const uint64_t *xhat_dev,
+                       size_t count, uint64_t *bits_out_dev, uint64_t *coeff_out_dev, void *stream);
+
 /* ---- a7: post-processing (online steps 4-6; Horner P:895; DESIGN 4.6) ---------
  * One call per party per round.  msg_in_dev = the OTHER party's message buffer, msg_out_dev = this party's;
  * both cover all rounds (sum over q of fusefss_post_msg_bytes(q)).  round q in [0, rounds) writes this party's

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libfusefss.so")
 # every symbol include/fusefss.h declares (tests check the library exports all of them)
 SYMBOLS = (
     "fusefss_compile", "fusefss_destroy", "fusefss_shape", "fusefss_atom", "fusefss_key_bytes", "fusefss_keygen", "fusefss_keygen_parts",
-    "fusefss_eval_cmp", "fusefss_eval_lut", "fusefss_post", "fusefss_post_rounds", "fusefss_post_msg_bytes",
+    "fusefss_eval_cmp", "fusefss_eval_lut", "fusefss_eval_fused", "fusefss_post", "fusefss_post_rounds", "fusefss_post_msg_bytes",
     "fusefss_online_bits", "fusefss_post_fused", "fusefss_gate_workspace_bytes", "fusefss_gate_host",
     "fusefss_strerror", "fusefss_last_cuda_error", "fusefss_launch_count", "fusefss_aes_probe", "fusefss_aes_kat",
 )
@@ -66,6 +66,7 @@ def _load():
         "fusefss_keygen_parts": (i32, [vp, vp, vp, u64, u64, sz, vp, vp, i32, vp]),
         "fusefss_eval_cmp": (i32, [i32, vp, vp, vp, sz, vp, vp]),
         "fusefss_eval_lut": (i32, [i32, vp, vp, vp, sz, vp, vp]),
+        "fusefss_eval_fused": (i32, [i32, vp, vp, vp, sz, vp, vp, vp]),
         "fusefss_post": (i32, [i32, vp, vp, vp, vp, vp, sz, i32, vp, vp, vp, vp, vp]),
         "fusefss_post_rounds": (i32, [vp]),
         "fusefss_post_msg_bytes": (sz, [vp, sz, i32]),
@@ -217,6 +218,13 @@ class Program:
         out = self._empty((self.shape["p"], count)) if out is None else out
         _check(lib.fusefss_eval_lut(party, self._h, _ptr(key), _ptr(xhat), count, _ptr(out), _stream()))
         return out
+
+    def eval_fused(self, party, key, xhat, bits=None, coeff=None):
+        count = xhat.numel()
+        bits = self._empty(count) if bits is None and self.shape["T"] else bits
+        coeff = self._empty((self.shape["p"], count)) if coeff is None and self.shape["has_lut"] else coeff
+        _check(lib.fusefss_eval_fused(party, self._h, _ptr(key), _ptr(xhat), count, _ptr(bits), _ptr(coeff), _stream()))
+        return bits, coeff
 
     def post(self, party, key, xhat, bits, coeff, rnd, msg_in, msg_out, y=None, z=None):
         count = xhat.numel()

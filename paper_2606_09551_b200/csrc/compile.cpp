@@ -17,7 +17,7 @@ namespace {
 
 uint64_t ring_mask(unsigned n) { return n >= 64 ? ~0ull : ((1ull << n) - 1ull); }
 
-struct ViewRec { int k; uint64_t c; std::vector<uint64_t> betas; };
+struct ViewRec { int k; uint64_t c; std::vector<uint64_t> betas; bool want_carry = false; };
 
 // Builds the SSA program; registers are renamed to a small file afterwards.
 class Lowering {
@@ -37,7 +37,7 @@ private:
     int view_index(int k, uint64_t c) {
         for (size_t v = 0; v < views.size(); ++v)
             if (views[v].k == k && views[v].c == c) return (int)v;
-        views.push_back(ViewRec{k, c, {}});
+        views.push_back(ViewRec{k, c, {}, false});
         return (int)views.size() - 1;
     }
     void want_pred(int k, uint64_t c, uint64_t beta) {
@@ -77,6 +77,7 @@ private:
     // I[view_{k,c}(x) < beta] = A_theta xor A_r xor w   (Lemma 4.3 / E.1)
     int b_pred(int k, uint64_t c, uint64_t beta) {
         int at = find_atom(k, c, true, beta), ar = find_atom(k, c, false, 0);
+        if (P.variant) { int v0 = fresh_b(0); push(I_B_ATOM, v0, at, 0, 0); return v0; }   // variant 1: the atom is the predicate share
         int v1 = fresh_b(0); push(I_B_ATOM, v1, at, 0, 0);
         int v2 = fresh_b(0); push(I_B_ATOM, v2, ar, 0, 0);
         int v3 = fresh_b(0); push(I_B_KAPPA, v3, P.atoms[at].carry, 0, 0);
@@ -101,6 +102,7 @@ private:
     int a_bin(uint8_t op, int a, int b) { int d = fresh_a(std::max(a_ready[a], a_ready[b])); push(op, d, a, b, 0); return d; }
 
     void collect_atoms();
+    void build_sp();
     bool lower_phi(int xval, const std::vector<int> &yval, const std::vector<int> &auxval, const std::vector<int> &zval);
     bool finish();
 };
@@ -113,22 +115,108 @@ void Lowering::collect_atoms() {
         case FUSEFSS_BN_C: if (inner) want_pred(n, 0, nd.value); break;
         case FUSEFSS_BN_D: if (inner) want_pred(nd.k, 0, nd.value); break;
         case FUSEFSS_BN_MSB: want_pred(n, nd.value & P.mask, 1ull << (n - 1)); break;
-        case FUSEFSS_BN_CARRY: view_index(nd.k, 0); break;
+        case FUSEFSS_BN_CARRY: views[view_index(nd.k, 0)].want_carry = true; break;
         default: break;
         }
     }
     bool piecewise = false;
     for (uint32_t j = 0; j < P.ell; ++j) piecewise = piecewise || !uniform_bit(j);
-    if (piecewise) for (uint32_t i = 1; i < P.m; ++i) want_pred(n, 0, P.alpha[i - 1]);
+    if (piecewise || (P.variant && P.m > 1)) for (uint32_t i = 1; i < P.m; ++i) want_pred(n, 0, P.alpha[i - 1]);
     P.T = 0; P.n_carry = 0;
     for (const ViewRec &V : views) {
         if (P.T + 1 + (int)V.betas.size() > kMaxAtoms) { failed = true; return; }
-        P.atoms[P.T++] = Atom{V.k, V.c, 0, 0, -1};
-        for (uint64_t beta : V.betas) P.atoms[P.T++] = Atom{V.k, V.c, 1, beta, P.n_carry++};
+        if (!P.variant || V.want_carry) P.atoms[P.T++] = Atom{V.k, V.c, 0, 0, -1};    // variant 1: r-atom only where CARRY reads it
+        for (uint64_t beta : V.betas) P.atoms[P.T++] = Atom{V.k, V.c, 1, beta, P.variant ? -1 : P.n_carry++};
     }
     P.n_kb = P.n_carry + (int)P.kappa_b.size();
     if (P.n_kb > 64) failed = true;
+    if (P.variant && !failed) build_sp();
 }
+
+// variant 1: evaluation points of the per-width keys, their linear contributions, and the prefix clusters.
+// I[view_{k,c}(x) < beta] = e - b + a,  b = f(h), a = f(h - beta), h = (xhat + c) mod 2^k, f = I[. < r_k]  (DESIGN 9).
+void Lowering::build_sp() {
+    SpProgram &S = P.sp;
+    S = SpProgram{};
+    std::vector<std::vector<uint64_t>> deltas;
+    auto width_of = [&](int k) {
+        for (int w = 0; w < S.n_w; ++w) if (S.width[w].k == k) return w;
+        if (S.n_w >= kMaxWidths) { failed = true; return 0; }
+        S.width[S.n_w] = SpWidth{k, 0, 0, k == (int)P.n};
+        deltas.emplace_back();
+        return S.n_w++;
+    };
+    auto kmask = [](int k) { return k >= 64 ? ~0ull : ((1ull << k) - 1ull); };
+    for (int t = 0; t < P.T; ++t) {
+        const Atom &a = P.atoms[t];
+        int w = width_of(a.k);
+        if (failed) return;
+        S.atom_w[t] = w;
+        auto add = [&](uint64_t d) { if (std::find(deltas[w].begin(), deltas[w].end(), d) == deltas[w].end()) deltas[w].push_back(d); };
+        add(a.c & kmask(a.k));
+        if (a.is_theta) add((a.c - a.beta) & kmask(a.k));
+    }
+    int base = 0;
+    for (int w = 0; w < S.n_w; ++w) {
+        const uint64_t half = 1ull << (S.width[w].k - 1);
+        std::sort(deltas[w].begin(), deltas[w].end(), [half](uint64_t x, uint64_t y) { return (x ^ half) < (y ^ half); });
+        S.width[w].first_point = base; S.width[w].n_points = (int)deltas[w].size();
+        for (uint64_t d : deltas[w]) S.points.push_back(SpPoint{d, 0});
+        base += (int)deltas[w].size();
+    }
+    if (base > kMaxPoints) { failed = true; return; }
+    auto index_of = [&](int w, uint64_t d) {
+        for (int j = 0; j < S.width[w].n_points; ++j) if (S.points[S.width[w].first_point + j].delta == d) return j;
+        return -1;
+    };
+    for (int t = 0; t < P.T; ++t) {
+        const Atom &a = P.atoms[t];
+        int w = S.atom_w[t];
+        S.atom_ib[t] = index_of(w, a.c & kmask(a.k));
+        S.atom_ia[t] = a.is_theta ? index_of(w, (a.c - a.beta) & kmask(a.k)) : -1;
+        S.points[S.width[w].first_point + S.atom_ib[t]].bitmask ^= 1ull << t;      // LSB(e - b + a) = e ^ b ^ a
+        if (a.is_theta) S.points[S.width[w].first_point + S.atom_ia[t]].bitmask ^= 1ull << t;
+    }
+    // interval lookup as a public linear map of the boundary comparisons (Lemma D.1 telescoped):
+    // v_{i*} = v_{m-1} + sum_{i=1}^{m-1} (v_{i-1} - v_i) I[x < alpha_i]
+    const int p = P.p;
+    S.weights.assign((size_t)base * p, 0);
+    S.delta_tab.assign((size_t)P.m * p, 0);
+    for (int w = 0; w < p; ++w) S.delta_tab[w] = P.payload[(size_t)(P.m - 1) * p + w];
+    for (uint32_t i = 1; i < P.m && P.has_lut; ++i) {
+        int t = find_atom((int)P.n, 0, true, P.alpha[i - 1]);
+        S.alpha_atom[i] = t;
+        const int wd = S.atom_w[t];
+        for (int w = 0; w < p; ++w) {
+            const uint64_t dl = (P.payload[(size_t)(i - 1) * p + w] - P.payload[(size_t)i * p + w]) & P.mask;
+            S.delta_tab[(size_t)i * p + w] = dl;
+            S.weights[(size_t)(S.width[wd].first_point + S.atom_ia[t]) * p + w] += dl;
+            S.weights[(size_t)(S.width[wd].first_point + S.atom_ib[t]) * p + w] -= dl;
+        }
+    }
+    // clusters of the n-bit tree: greedy over the sorted offsets; a cluster spans < 2^tail_bits, so its points have
+    // at most two distinct (n - tail_bits)-bit prefixes; sharing must save at least 8 levels to be worth it
+    for (int w = 0; w < S.n_w; ++w) {
+        if (!S.width[w].is_vec) continue;
+        const int n = (int)P.n, np = S.width[w].n_points, f0 = S.width[w].first_point;
+        const uint64_t half = 1ull << (n - 1);
+        int i = 0;
+        while (i < np) {
+            int j = i, bits = 0;
+            while (j + 1 < np) {
+                const uint64_t span = ((S.points[f0 + j + 1].delta ^ half) - (S.points[f0 + i].delta ^ half));
+                int b = 0;
+                while (b < 64 && (span >> b) != 0) ++b;                 // span < 2^b
+                if (b > n - 8) break;
+                bits = b; ++j;
+            }
+            S.clusters.push_back(SpCluster{i, j - i + 1, j > i ? (bits < 1 ? 1 : bits) : n, 0});
+            i = j + 1;
+        }
+    }
+}
+
+
 
 int Lowering::lower_bit(int id) {
     if (id < 0 || id >= (int)P.nodes.size()) { failed = true; return b_const(0); }
@@ -368,6 +456,8 @@ int compile_program(const fusefss_spec *S, Program **out) {
     // M = min(m+1, 2^n)  (Protocol 3 line 2)
     P.M = (S->n >= 7 || (uint64_t)(S->m + 1) < (1ull << S->n)) ? (int)S->m + 1 : (int)(1ull << S->n);
     P.has_lut = S->m > 1;                         // a single interval needs no lookup
+    P.variant = S->variant ? 1 : 0;
+    if (P.variant) P.M = (int)S->m;               // variant 1: no translated partition, no wrap / dummy split
     P.n_out_a = (int)S->n_out_a; P.n_out_b = (int)S->n_out_b;
     if (P.n_out_a > kMaxP || P.n_out_b > 64) { delete holder; return FUSEFSS_E_SPEC; }
     P.payload.resize((size_t)S->m * p);
@@ -387,18 +477,34 @@ void compute_layout(const Program &P, size_t count, Layout *L) {
     size_t off = 0;
     L->s16 = round_up_256(count * 16);
     L->s8 = round_up_256(count * 8);
-    for (int t = 0; t < P.T; ++t) {
+    if (P.variant) {                              // one tree per view width (DESIGN 9)
+        L->lvl_stride = L->s16 + L->s8;
+        L->vt_lvl_rel = L->s16;
+        L->vt_fin_rel = L->s16 + L->lvl_stride * (size_t)P.n;
+        L->vt_stride = L->vt_fin_rel + L->s8;
+        L->lut_c = L->vt_first = 0;
+        for (int w = 0; w < P.sp.n_w; ++w) {
+            if (!P.sp.width[w].is_vec) {
+                L->bt_root[w] = off; off += L->s16;
+                L->bt_cw[w] = off;   off += L->s16 * (size_t)P.sp.width[w].k;
+                L->bt_vb[w] = off;   off += L->s8;
+            } else { L->vt_first = off; off += L->vt_stride; }
+        }
+    }
+    for (int t = 0; t < P.T && !P.variant; ++t) {
         L->bt_root[t] = off; off += L->s16;
         L->bt_cw[t] = off;   off += L->s16 * (size_t)P.atoms[t].k;
         L->bt_vb[t] = off;   off += L->s8;
     }
     const size_t pw = (size_t)P.p * L->s8;
-    L->lvl_stride = L->s16 + pw;
-    L->vt_lvl_rel = L->s16;                                   // after the root
-    L->vt_fin_rel = L->s16 + L->lvl_stride * (size_t)P.n;
-    L->vt_stride = L->vt_fin_rel + pw;
-    L->lut_c = off; L->vt_first = off;
-    if (P.has_lut) {
+    if (!P.variant) {
+        L->lvl_stride = L->s16 + pw;
+        L->vt_lvl_rel = L->s16;                               // after the root
+        L->vt_fin_rel = L->s16 + L->lvl_stride * (size_t)P.n;
+        L->vt_stride = L->vt_fin_rel + pw;
+        L->lut_c = off; L->vt_first = off;
+    }
+    if (P.has_lut && !P.variant) {
         off += pw;
         L->vt_first = off;
         off += L->vt_stride * (size_t)(P.M - 1);

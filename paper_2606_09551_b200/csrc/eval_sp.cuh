@@ -1,0 +1,203 @@
+// eval_sp.cuh -- online evaluation for variant 1 (single-key shared-prefix construction, DESIGN.md section 9;
+// SURVEY 8(f) NEXT-1; north_star: "the packed multi-threshold comparison that shares tree prefixes across the
+// predicates of one element").  Per element ONE n-bit DCF key f_{r,1} (payload in R) -- plus one bit-DCF per
+// narrower view -- is evaluated at the public points u_j = (xhat + delta_j) mod 2^k:
+//   I[view_{k,c}(x) < beta] = e - b + a,  b = f(xhat + c), a = f(xhat + c - beta), e = I[(xhat + c) mod 2^k < beta]
+// (Def I.1 with c_t = -beta_t, theta_t = r).  Predicate bits are the LSBs; the interval lookup is the
+// public linear map  v_{i*} = v_{m-1} + sum_i (v_{i-1} - v_i) I[x < alpha_i]  of the same comparisons (Def I.2).
+// Points whose offsets lie within 2^tail_bits of each other share the walk over their top n - tail_bits bits:
+// the two candidate prefixes of a cluster are walked once (in lock-step), every point then walks only its tail.
+#pragma once
+#include "aes.cuh"
+#include "program.h"
+
+namespace fsk {
+
+constexpr int kMaxClusters = 16;
+struct SpAtomDev { uint64_t c, beta; int k, is_theta; };
+struct EvalSpArgs {
+    const uint8_t *key; const uint64_t *xhat; uint64_t *bits_out, *coeff_out;       // either output may be null
+    const SpPoint *points; const uint64_t *weights, *delta_tab, *alpha;             // device tables (program blob)
+    size_t count, s16, s8, lvl_stride, vt_first, vt_lvl_rel, vt_fin_rel;
+    uint64_t mask;
+    int n, m, p, party, T, n_w, n_clusters, pad;
+    SpWidth width[kMaxWidths];
+    size_t bt_root[kMaxWidths], bt_cw[kMaxWidths], bt_vb[kMaxWidths];
+    SpCluster cluster[kMaxClusters];
+    SpAtomDev atom[kMaxAtoms];
+};
+
+struct SpState { uint32_t s[4]; uint32_t t; uint64_t V; };
+
+__device__ __forceinline__ void sp_step(uint32_t tl, const uint4 cw, const uint64_t vcw, uint32_t dbit, SpState &st) {
+    uint32_t x[1][4] = {{st.s[0] | dbit, st.s[1], st.s[2], st.s[3]}};
+    uint32_t o[1][2][4];
+    prg_blocks<1, 2, 0, true>(tl, x, o);
+    const uint32_t tm = 0u - st.t;
+    st.V += ((uint64_t)o[0][1][0] | ((uint64_t)o[0][1][1] << 32)) + (vcw & (0ull - (uint64_t)st.t));
+    const uint32_t tnew = (o[0][0][0] & 1u) ^ (st.t & (cw.x >> dbit) & 1u);
+    st.s[0] = (o[0][0][0] & ~3u) ^ (cw.x & ~3u & tm);
+    st.s[1] = o[0][0][1] ^ (cw.y & tm);
+    st.s[2] = o[0][0][2] ^ (cw.z & tm);
+    st.s[3] = o[0][0][3] ^ (cw.w & tm);
+    st.t = tnew;
+}
+
+// walk levels [from, to) of the n-bit vector tree (p = 1); ubits = the point with its level-`from` bit at bit 63
+__device__ __forceinline__ void sp_walk(uint32_t tl, const uint8_t *lvl, size_t e, size_t s16, size_t lvl_stride,
+                                        int from, int to, uint64_t ubits, SpState &st) {
+    const uint8_t *pl = lvl + (size_t)from * lvl_stride;
+    for (int i = from; i < to; ++i, pl += lvl_stride) {
+        const uint4 cw = __ldg(reinterpret_cast<const uint4 *>(pl + e * 16));
+        const uint64_t vcw = __ldg(reinterpret_cast<const unsigned long long *>(pl + s16 + e * 8));
+        sp_step(tl, cw, vcw, (uint32_t)(ubits >> 63), st);
+        ubits <<= 1;
+    }
+}
+// two prefixes in lock-step over levels [0, to): same correction words, independent PRG chains
+__device__ __forceinline__ void sp_walk2(uint32_t tl, const uint8_t *lvl, size_t e, size_t s16, size_t lvl_stride,
+                                         int to, uint64_t u1, uint64_t u2, SpState &a, SpState &b) {
+    const uint8_t *pl = lvl;
+    for (int i = 0; i < to; ++i, pl += lvl_stride) {
+        const uint4 cw = __ldg(reinterpret_cast<const uint4 *>(pl + e * 16));
+        const uint64_t vcw = __ldg(reinterpret_cast<const unsigned long long *>(pl + s16 + e * 8));
+        sp_step(tl, cw, vcw, (uint32_t)(u1 >> 63), a);
+        sp_step(tl, cw, vcw, (uint32_t)(u2 >> 63), b);
+        u1 <<= 1; u2 <<= 1;
+    }
+}
+// leaf: A = (-1)^party (V + conv(s) + t * fin)
+__device__ __forceinline__ uint64_t sp_leaf(uint32_t tl, const SpState &st, uint64_t fin, int party) {
+    uint32_t x[1][4] = {{st.s[0] | 2u, st.s[1], st.s[2], st.s[3]}};
+    uint32_t o[1][1][4];
+    prg_blocks<1, 1, 1>(tl, x, o);
+    const uint64_t v = st.V + ((uint64_t)o[0][0][0] | ((uint64_t)o[0][0][1] << 32)) + (fin & (0ull - (uint64_t)st.t));
+    return party ? 0ull - v : v;
+}
+
+// bit-DCF walk (payload Z_2) of one point; u = the k-bit point, MSB-aligned
+__device__ __forceinline__ uint32_t sp_bit_eval(uint32_t tl, const uint8_t *key, size_t root_off, size_t cw_off, size_t vb_off,
+                                                size_t e, size_t s16, int k, uint64_t u, int party) {
+    uint4 s = __ldg(reinterpret_cast<const uint4 *>(key + root_off + e * 16));
+    const uint64_t vb = __ldg(reinterpret_cast<const unsigned long long *>(key + vb_off + e * 8));
+    const uint32_t fin = s.x & 1u;
+    s.x &= ~3u;
+    uint32_t tb = (uint32_t)party, V = 0;
+    const uint8_t *cwp = key + cw_off + e * 16;
+    for (int i = 0; i < k; ++i) {
+        const uint4 cw = __ldg(reinterpret_cast<const uint4 *>(cwp + (size_t)i * s16));
+        const uint32_t dbit = (uint32_t)(u >> 63);
+        u <<= 1;
+        uint32_t x[1][4] = {{s.x | dbit, s.y, s.z, s.w}};
+        uint32_t o[1][1][4];
+        prg_blocks<1, 1, 0>(tl, x, o);
+        const uint32_t tm = 0u - tb;
+        V ^= ((o[0][0][0] >> 1) & 1u) ^ (tb & (uint32_t)((vb >> i) & 1ull));
+        const uint32_t tnew = (o[0][0][0] & 1u) ^ (tb & (cw.x >> dbit) & 1u);
+        s.x = (o[0][0][0] & ~3u) ^ (cw.x & ~3u & tm);
+        s.y = o[0][0][1] ^ (cw.y & tm);
+        s.z = o[0][0][2] ^ (cw.z & tm);
+        s.w = o[0][0][3] ^ (cw.w & tm);
+        tb = tnew;
+    }
+    uint32_t x[1][4] = {{s.x | 2u, s.y, s.z, s.w}};
+    uint32_t o[1][1][4];
+    prg_blocks<1, 1, 0>(tl, x, o);
+    return (V ^ ((o[0][0][0] >> 1) & 1u) ^ (tb & fin)) & 1u;
+}
+
+template <int P>
+__global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ EvalSpArgs a) {
+    extern __shared__ uint32_t sT[];
+    const uint32_t tl = aes_fill_tables(sT);
+    const size_t padded = (a.count + 31) & ~(size_t)31;                     // whole warps stay converged
+    for (size_t e0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e0 < padded; e0 += (size_t)gridDim.x * blockDim.x) {
+        const bool live = e0 < a.count;
+        const size_t e = live ? e0 : a.count - 1;
+        const uint64_t xh = a.xhat[e] & a.mask;
+        const bool want_bits = a.bits_out != nullptr, want_coeff = a.coeff_out != nullptr;
+        uint64_t word = 0, acc[P];
+#pragma unroll
+        for (int w = 0; w < P; ++w) acc[w] = 0;
+        if (a.party == 0) {                                                 // public parts: e_t and the plaintext table row of xhat
+            if (want_bits)
+                for (int t = 0; t < a.T; ++t) {
+                    const SpAtomDev &at = a.atom[t];
+                    const uint64_t km = at.k >= 64 ? ~0ull : ((1ull << at.k) - 1ull);
+                    if (at.is_theta) word |= (uint64_t)(((xh + at.c) & km) < at.beta) << t;
+                }
+            if (want_coeff) {
+#pragma unroll
+                for (int w = 0; w < P; ++w) acc[w] = a.delta_tab[w];
+                for (int i = 1; i < a.m; ++i)
+                    if (xh < a.alpha[i - 1]) {
+#pragma unroll
+                        for (int w = 0; w < P; ++w) acc[w] += a.delta_tab[(size_t)i * P + w];
+                    }
+            }
+        }
+        for (int wd = 0; wd < a.n_w; ++wd) {
+            const SpWidth W = a.width[wd];
+            const SpPoint *pts = a.points + W.first_point;
+            const uint64_t *wts = a.weights + (size_t)W.first_point * P;
+            if (!W.is_vec) {
+                if (!want_bits) continue;
+                const uint64_t km = (1ull << W.k) - 1ull;
+                for (int j = 0; j < W.n_points; ++j) {
+                    const uint64_t u = (((xh & km) + pts[j].delta) & km) << (64 - W.k);
+                    const uint32_t A = sp_bit_eval(tl, a.key, a.bt_root[wd], a.bt_cw[wd], a.bt_vb[wd], e, a.s16, W.k, u, a.party);
+                    word ^= pts[j].bitmask & (0ull - (uint64_t)A);
+                }
+                continue;
+            }
+            const uint8_t *tree = a.key + a.vt_first;
+            const uint8_t *lvl = tree + a.vt_lvl_rel;
+            const uint4 root = __ldg(reinterpret_cast<const uint4 *>(tree + e * 16));
+            const uint64_t fin = __ldg(reinterpret_cast<const unsigned long long *>(tree + a.vt_fin_rel + e * 8));
+            SpState r0;
+            r0.s[0] = root.x & ~3u; r0.s[1] = root.y; r0.s[2] = root.z; r0.s[3] = root.w; r0.t = (uint32_t)a.party; r0.V = 0;
+            const int n = a.n;
+            for (int c = 0; c < a.n_clusters; ++c) {
+                const SpCluster cl = a.cluster[c];
+                const int kf = n - cl.tail_bits;                            // shared levels
+                const bool share = cl.count > 1 && kf > 0;
+                SpState s1 = r0, s2 = r0;
+                uint64_t pre1 = 0;
+                if (share) {
+                    const uint64_t uf = ((xh + pts[cl.first].delta) & a.mask) << (64 - n);
+                    const uint64_t ul = ((xh + pts[cl.first + cl.count - 1].delta) & a.mask) << (64 - n);
+                    sp_walk2(tl, lvl, e, a.s16, a.lvl_stride, kf, uf, ul, s1, s2);
+                    pre1 = uf >> (64 - kf);
+                }
+                for (int j = cl.first; j < cl.first + cl.count; ++j) {
+                    bool need = want_bits && pts[j].bitmask != 0;
+                    if (want_coeff) {
+#pragma unroll
+                        for (int w = 0; w < P; ++w) need = need || wts[(size_t)j * P + w] != 0;
+                    }
+                    if (!need) continue;
+                    const uint64_t u = ((xh + pts[j].delta) & a.mask) << (64 - n);
+                    SpState st = r0;
+                    int from = 0;
+                    if (share) { st = (u >> (64 - kf)) == pre1 ? s1 : s2; from = kf; }
+                    sp_walk(tl, lvl, e, a.s16, a.lvl_stride, from, n, from ? u << from : u, st);
+                    const uint64_t A = sp_leaf(tl, st, fin, a.party);
+                    word ^= pts[j].bitmask & (0ull - (A & 1ull));
+                    if (want_coeff) {
+#pragma unroll
+                        for (int w = 0; w < P; ++w) acc[w] += wts[(size_t)j * P + w] * A;
+                    }
+                }
+            }
+        }
+        if (live) {
+            if (want_bits) a.bits_out[e] = word;
+            if (want_coeff) {
+#pragma unroll
+                for (int w = 0; w < P; ++w) a.coeff_out[(size_t)w * a.count + e] = acc[w] & a.mask;
+            }
+        }
+    }
+}
+
+}  // namespace fsk

@@ -50,6 +50,7 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_bit(const __grid_constan
         if (e >= a.count) continue;
         const GenAtomDev &at = a.atom[t];
         const int k = at.k;
+        if (k == 0) continue;                              // variant 1: slot of the n-bit view (its key is a vector tree)
         const uint64_t km = k >= 64 ? ~0ull : ((1ull << k) - 1ull);
         const uint64_t rk_ = a.r_in[e] & a.mask & km;
         // threshold of the masked comparison (Lemma 4.3 / E.1): theta = (r_k + beta) mod 2^k, or r_k for the r-atom
@@ -175,7 +176,7 @@ struct GenVecArgs {
     uint8_t *key0, *key1; const uint64_t *r_in; const uint64_t *alpha; const uint64_t *payload;   // payload[m][p]
     size_t count, s16, s8, vt_first, vt_stride, lvl_stride, vt_lvl_rel, vt_fin_rel;
     uint64_t first_elem, mask;
-    int n, m, M, pad;
+    int n, m, M, sp;           // sp = 1 (variant 1): the single tree f_{r,1}: threshold r_in, payload 1, no Protocol 3
     RoundKeys rk;
 };
 
@@ -193,14 +194,18 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec(const __grid_constan
         const size_t e = (it - (size_t)(j - 1) * tiles) * 32 + lane;
         if (e >= a.count) continue;
         const uint64_t r = a.r_in[e] & a.mask;
-        P3 p3;
-        p3.init(a.alpha, a.m, a.n, a.mask, r, a.M);
-        uint64_t alpha = p3.B(j) << (64 - a.n);
-        uint64_t beta[P];                                                  // Delta_j = v_{j-1} - v_j
-        {
+        uint64_t alpha, beta[P];
+        if (a.sp) {
+            alpha = r << (64 - a.n);
+#pragma unroll
+            for (int w = 0; w < P; ++w) beta[w] = 1;
+        } else {
+            P3 p3;
+            p3.init(a.alpha, a.m, a.n, a.mask, r, a.M);
+            alpha = p3.B(j) << (64 - a.n);
             const uint64_t *va = a.payload + (size_t)p3.ord(j - 1) * P, *vb = a.payload + (size_t)p3.ord(j) * P;
 #pragma unroll
-            for (int w = 0; w < P; ++w) beta[w] = va[w] - vb[w];
+            for (int w = 0; w < P; ++w) beta[w] = va[w] - vb[w];                // Delta_j = v_{j-1} - v_j
         }
         uint32_t s[2][4];
         {

@@ -9,6 +9,7 @@
 #include "program.h"
 #include "aes.cuh"
 #include "eval.cuh"
+#include "eval_sp.cuh"
 #include "keygen.cuh"
 #include "post.cuh"
 
@@ -96,13 +97,19 @@ int ensure_blob(Program &P) {
     P.dev_ins_off = 0;
     P.dev_alpha_off = up(P.ins.size() * sizeof(Ins));
     P.dev_payload_off = P.dev_alpha_off + up(P.alpha.size() * 8 + 8);
-    P.dev_blob_bytes = P.dev_payload_off + up(P.payload.size() * 8 + 8);
+    P.dev_sp_points_off = P.dev_payload_off + up(P.payload.size() * 8 + 8);
+    P.dev_sp_weights_off = P.dev_sp_points_off + up(P.sp.points.size() * sizeof(SpPoint) + 8);
+    P.dev_sp_delta_off = P.dev_sp_weights_off + up(P.sp.weights.size() * 8 + 8);
+    P.dev_blob_bytes = P.dev_sp_delta_off + up(P.sp.delta_tab.size() * 8 + 8);
     void *d = nullptr;
     CU(cudaMalloc(&d, P.dev_blob_bytes));
     std::vector<uint8_t> h(P.dev_blob_bytes, 0);
     if (!P.ins.empty()) std::memcpy(h.data() + P.dev_ins_off, P.ins.data(), P.ins.size() * sizeof(Ins));
     if (!P.alpha.empty()) std::memcpy(h.data() + P.dev_alpha_off, P.alpha.data(), P.alpha.size() * 8);
     if (!P.payload.empty()) std::memcpy(h.data() + P.dev_payload_off, P.payload.data(), P.payload.size() * 8);
+    if (!P.sp.points.empty()) std::memcpy(h.data() + P.dev_sp_points_off, P.sp.points.data(), P.sp.points.size() * sizeof(SpPoint));
+    if (!P.sp.weights.empty()) std::memcpy(h.data() + P.dev_sp_weights_off, P.sp.weights.data(), P.sp.weights.size() * 8);
+    if (!P.sp.delta_tab.empty()) std::memcpy(h.data() + P.dev_sp_delta_off, P.sp.delta_tab.data(), P.sp.delta_tab.size() * 8);
     cudaError_t e = cudaMemcpy(d, h.data(), P.dev_blob_bytes, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { cudaFree(d); return cuda_fail(e, "cudaMemcpy(program tables)"); }
     P.dev_blob = d;
@@ -152,6 +159,42 @@ int launch_gen_vec_p(int p, int grid, int block, cudaStream_t st, const GenVecAr
     case 6: return launch(k_gen_vec<6>, grid, block, sm, st, a);
     case 7: return launch(k_gen_vec<7>, grid, block, sm, st, a);
     case 8: return launch(k_gen_vec<8>, grid, block, sm, st, a);
+    }
+    return FUSEFSS_E_SPEC;
+}
+
+// variant 1: one kernel serves eval_cmp (bits only), eval_lut (coefficients only) and the fused call (both)
+int launch_eval_sp(Program &P, int party, const void *key, const uint64_t *xhat, size_t count, uint64_t *bits_out,
+                   uint64_t *coeff_out, cudaStream_t st) {
+    int rc = ensure_blob(P); if (rc) return rc;
+    Layout L; compute_layout(P, count, &L);
+    EvalSpArgs a{};
+    const uint8_t *blob = (const uint8_t *)P.dev_blob;
+    a.key = (const uint8_t *)key; a.xhat = xhat; a.bits_out = bits_out; a.coeff_out = coeff_out;
+    a.points = (const SpPoint *)(blob + P.dev_sp_points_off); a.weights = (const uint64_t *)(blob + P.dev_sp_weights_off);
+    a.delta_tab = (const uint64_t *)(blob + P.dev_sp_delta_off); a.alpha = (const uint64_t *)(blob + P.dev_alpha_off);
+    a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.lvl_stride = L.lvl_stride; a.vt_first = L.vt_first;
+    a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel; a.mask = P.mask;
+    a.n = (int)P.n; a.m = (int)P.m; a.p = P.p; a.party = party; a.T = P.T; a.n_w = P.sp.n_w;
+    if (P.sp.clusters.size() > (size_t)kMaxClusters) return FUSEFSS_E_SPEC;
+    a.n_clusters = (int)P.sp.clusters.size();
+    for (int c = 0; c < a.n_clusters; ++c) a.cluster[c] = P.sp.clusters[c];
+    for (int w = 0; w < P.sp.n_w; ++w) { a.width[w] = P.sp.width[w]; a.bt_root[w] = L.bt_root[w]; a.bt_cw[w] = L.bt_cw[w]; a.bt_vb[w] = L.bt_vb[w]; }
+    for (int t = 0; t < P.T; ++t) a.atom[t] = SpAtomDev{P.atoms[t].c, P.atoms[t].beta, P.atoms[t].k, P.atoms[t].is_theta};
+    // spread small tensors over the SMs: threads per CTA = count / SMs rounded up to a warp, in [64, 1024]
+    int threads = (int)(((count + g_sms - 1) / g_sms + 31) / 32 * 32);
+    threads = threads < 64 ? 64 : threads > g_eval_threads ? g_eval_threads : threads;
+    const int grid = grid_for((count + 31) / 32, threads);
+    const size_t sm = kAesSmemBytes;
+    switch (P.p) {
+    case 1: return launch(k_eval_sp<1>, grid, threads, sm, st, a);
+    case 2: return launch(k_eval_sp<2>, grid, threads, sm, st, a);
+    case 3: return launch(k_eval_sp<3>, grid, threads, sm, st, a);
+    case 4: return launch(k_eval_sp<4>, grid, threads, sm, st, a);
+    case 5: return launch(k_eval_sp<5>, grid, threads, sm, st, a);
+    case 6: return launch(k_eval_sp<6>, grid, threads, sm, st, a);
+    case 7: return launch(k_eval_sp<7>, grid, threads, sm, st, a);
+    case 8: return launch(k_eval_sp<8>, grid, threads, sm, st, a);
     }
     return FUSEFSS_E_SPEC;
 }
@@ -260,7 +303,31 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
     const uint64_t *payload_dev = (const uint64_t *)(blob + P->dev_payload_off);
     const size_t tiles = (count + 31) / 32;
     const size_t smem = kAesSmemBytes;
-    if (P->T > 0 && (parts & FUSEFSS_GEN_CMP)) {
+    if (P->variant) {                                   // variant 1: one tree per view width (DESIGN 9)
+        bool any_bit = false, any_vec = false;
+        GenBitArgs ab{};
+        ab.key0 = (uint8_t *)key0_dev; ab.key1 = (uint8_t *)key1_dev; ab.r_in = r_in_dev;
+        ab.count = count; ab.s16 = L.s16; ab.first_elem = first_elem; ab.mask = P->mask; ab.T = P->sp.n_w; ab.rk = rk;
+        for (int w = 0; w < P->sp.n_w; ++w) {
+            const bool vec = P->sp.width[w].is_vec != 0;
+            any_bit = any_bit || !vec; any_vec = any_vec || vec;
+            ab.atom[w] = GenAtomDev{0, 0, L.bt_root[w], L.bt_cw[w], L.bt_vb[w], vec ? 0 : P->sp.width[w].k, 0};
+        }
+        if (any_bit && (parts & FUSEFSS_GEN_CMP)) {
+            rc = launch(k_gen_bit, grid_for(tiles * P->sp.n_w, kGenThreads), kGenThreads, smem, st, ab);
+            if (rc) return rc;
+        }
+        if (any_vec && (parts & FUSEFSS_GEN_LUT)) {
+            GenVecArgs a{};
+            a.key0 = (uint8_t *)key0_dev; a.key1 = (uint8_t *)key1_dev; a.r_in = r_in_dev; a.alpha = alpha_dev; a.payload = payload_dev;
+            a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.vt_first = L.vt_first; a.vt_stride = L.vt_stride; a.lvl_stride = L.lvl_stride;
+            a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel; a.first_elem = first_elem; a.mask = P->mask;
+            a.n = (int)P->n; a.m = (int)P->m; a.M = 2; a.sp = 1; a.rk = rk;
+            rc = launch(k_gen_vec<1>, grid_for(tiles, kGenThreads), kGenThreads, smem, st, a);
+            if (rc) return rc;
+        }
+    }
+    if (!P->variant && P->T > 0 && (parts & FUSEFSS_GEN_CMP)) {
         GenBitArgs a{};
         a.key0 = (uint8_t *)key0_dev; a.key1 = (uint8_t *)key1_dev; a.r_in = r_in_dev;
         a.count = count; a.s16 = L.s16; a.first_elem = first_elem; a.mask = P->mask; a.T = P->T; a.rk = rk;
@@ -270,7 +337,7 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
         rc = launch(k_gen_bit, grid, kGenThreads, kAesSmemBytes, st, a);
         if (rc) return rc;
     }
-    if (P->has_lut && (parts & FUSEFSS_GEN_LUT)) {
+    if (!P->variant && P->has_lut && (parts & FUSEFSS_GEN_LUT)) {
         GenVecArgs a{};
         a.key0 = (uint8_t *)key0_dev; a.key1 = (uint8_t *)key1_dev; a.r_in = r_in_dev; a.alpha = alpha_dev; a.payload = payload_dev;
         a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.vt_first = L.vt_first; a.vt_stride = L.vt_stride; a.lvl_stride = L.lvl_stride;
@@ -287,13 +354,13 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
         a.count = count; a.s8 = L.s8; a.lut_c = L.lut_c; a.rin = L.rin; a.rout = L.rout; a.ka = L.ka; a.kb = L.kb;
         a.beaver = L.beaver; a.andt = L.andt; a.b2a_bits = L.b2a_bits; a.b2a_a = L.b2a_a;
         a.first_elem = first_elem; a.mask = P->mask;
-        a.n = (int)P->n; a.m = (int)P->m; a.M = P->M; a.p = P->p; a.has_lut = P->has_lut; a.mask_output = (int)P->mask_output;
+        a.n = (int)P->n; a.m = (int)P->m; a.M = P->M; a.p = P->p; a.has_lut = P->variant ? 0 : P->has_lut; a.mask_output = (int)P->mask_output;
         a.n_out_a = P->n_out_a; a.n_ka = (int)P->kappa_a.size(); a.n_kb_spec = (int)P->kappa_b.size(); a.n_carry = P->n_carry;
-        a.T = P->T; a.MA = P->MA; a.MB = P->MB; a.GMIX = P->GMIX; a.rk = rk;
+        a.T = P->variant ? 0 : P->T; a.MA = P->MA; a.MB = P->MB; a.GMIX = P->GMIX; a.rk = rk;
         if (a.n_ka > 8) return FUSEFSS_E_SPEC;
         for (int t = 0; t < a.n_ka; ++t) { a.ka_kind[t] = P->kappa_a[t].kind; a.ka_arg[t] = P->kappa_a[t].arg; }
         for (int t = 0; t < a.n_kb_spec; ++t) { a.kb_kind[t] = P->kappa_b[t].kind; a.kb_arg[t] = P->kappa_b[t].arg; }
-        for (int t = 0; t < P->T; ++t)
+        for (int t = 0; t < a.T; ++t)
             a.atom[t] = GenAtomDev{P->atoms[t].c, P->atoms[t].beta, 0, 0, 0, P->atoms[t].k, P->atoms[t].is_theta};
         const int grid = grid_for(tiles, kGenThreads);
         rc = launch(k_gen_misc, grid, kGenThreads, kAesSmemBytes, st, a);
@@ -311,6 +378,7 @@ int fusefss_eval_cmp(int party, const fusefss_program *prog, const void *key_dev
     if (P->T == 0) return FUSEFSS_E_OMITTED;
     int rc = init_device(); if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
+    if (P->variant) return launch_eval_sp(*const_cast<Program *>(P), party, key_dev, xhat_dev, count, bits_out_dev, nullptr, st);
     Layout L; compute_layout(*P, count, &L);
     EvalCmpArgs a{};
     a.key = (const uint8_t *)key_dev; a.xhat = xhat_dev; a.out = bits_out_dev; a.count = count; a.s16 = L.s16;
@@ -331,6 +399,7 @@ int fusefss_eval_lut(int party, const fusefss_program *prog, const void *key_dev
     if (!P->has_lut) return FUSEFSS_E_OMITTED;
     int rc = init_device(); if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
+    if (P->variant) return launch_eval_sp(*const_cast<Program *>(P), party, key_dev, xhat_dev, count, nullptr, coeff_out_dev, st);
     Layout L; compute_layout(*P, count, &L);
     EvalLutArgs a{};
     a.key = (const uint8_t *)key_dev; a.xhat = xhat_dev; a.out = coeff_out_dev;
@@ -349,6 +418,24 @@ int fusefss_eval_lut(int party, const fusefss_program *prog, const void *key_dev
     return 0;
 }
 
+
+int fusefss_eval_fused(int party, const fusefss_program *prog, const void *key_dev, const uint64_t *xhat_dev, size_t count,
+                       uint64_t *bits_out_dev, uint64_t *coeff_out_dev, void *stream) {
+    const Program *P = prog_of(prog);
+    if (!P || !key_dev || !xhat_dev) return FUSEFSS_E_NULL;
+    if ((P->T > 0 && !bits_out_dev) || (P->has_lut && !coeff_out_dev)) return FUSEFSS_E_NULL;
+    if (party != 0 && party != 1) return FUSEFSS_E_PARTY;
+    if (count == 0) return FUSEFSS_E_COUNT;
+    if (P->T == 0 && !P->has_lut) return FUSEFSS_E_OMITTED;
+    if (P->variant) {
+        int rc = init_device(); if (rc) return rc;
+        return launch_eval_sp(*const_cast<Program *>(P), party, key_dev, xhat_dev, count, P->T > 0 ? bits_out_dev : nullptr,
+                              P->has_lut ? coeff_out_dev : nullptr, (cudaStream_t)stream);
+    }
+    if (P->T > 0) { int rc = fusefss_eval_cmp(party, prog, key_dev, xhat_dev, count, bits_out_dev, stream); if (rc) return rc; }
+    if (P->has_lut) { int rc = fusefss_eval_lut(party, prog, key_dev, xhat_dev, count, coeff_out_dev, stream); if (rc) return rc; }
+    return 0;
+}
 
 int fusefss_post(int party, const fusefss_program *prog, const void *key_dev, const uint64_t *xhat_dev,
                  const uint64_t *bits_dev, const uint64_t *coeff_dev, size_t count, int round, const void *msg_in_dev,
@@ -437,13 +524,9 @@ int fusefss_gate_host(const fusefss_program *prog, const uint64_t *r_in, const u
             for (int j = 0; j < P->n_out_a; ++j)
                 CU(cudaMemcpyAsync(d_rout + (size_t)j * c, r_out + (size_t)j * count + first, c * 8, cudaMemcpyHostToDevice, st));
         int rc = fusefss_keygen(prog, d_rin, d_rout, seed, first, c, key0, key1, st); if (rc) return rc;
-        if (P->T > 0) {
-            rc = fusefss_eval_cmp(0, prog, key0, d_xhat, c, d_b0, st); if (rc) return rc;
-            rc = fusefss_eval_cmp(1, prog, key1, d_xhat, c, d_b1, st); if (rc) return rc;
-        }
-        if (P->has_lut) {
-            rc = fusefss_eval_lut(0, prog, key0, d_xhat, c, d_c0, st); if (rc) return rc;
-            rc = fusefss_eval_lut(1, prog, key1, d_xhat, c, d_c1, st); if (rc) return rc;
+        if (P->T > 0 || P->has_lut) {
+            rc = fusefss_eval_fused(0, prog, key0, d_xhat, c, d_b0, d_c0, st); if (rc) return rc;
+            rc = fusefss_eval_fused(1, prog, key1, d_xhat, c, d_b1, d_c1, st); if (rc) return rc;
         }
         rc = fusefss_post_fused(prog, key0, key1, d_xhat, d_b0, d_b1, d_c0, d_c1, c, d_y0, d_y1, d_z0, d_z1, st); if (rc) return rc;
         for (int j = 0; j < P->n_out_a; ++j) {

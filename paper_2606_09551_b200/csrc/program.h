@@ -50,9 +50,26 @@ struct Layout {
     size_t rin, rout, ka, kb, beaver, andt, b2a_bits, b2a_a, total;
 };
 
+// variant 1: single-key shared-prefix construction
+constexpr int kMaxWidths = 8;
+constexpr int kMaxPoints = 2 * kMaxAtoms + 2;
+struct SpPoint { uint64_t delta; uint64_t bitmask; };      // offset added to xhat; atoms whose bit flips with LSB(A_j)
+struct SpCluster { int first, count, tail_bits, pad; };    // points [first, first+count) share their top n - tail_bits bits (two candidate prefixes)
+struct SpWidth { int k, first_point, n_points, is_vec; };
+struct SpProgram {
+    int n_w = 0;
+    SpWidth width[kMaxWidths];
+    std::vector<SpPoint> points;        // all widths, width-major, sorted by signed delta inside a width
+    std::vector<uint64_t> weights;      // [n_points_total][p]: coefficient share += weights[j][w] * A_j
+    std::vector<uint64_t> delta_tab;    // [m][p]: row i >= 1 = v_{i-1} - v_i, row 0 = v_{m-1} (public part, party 0)
+    std::vector<SpCluster> clusters;    // of the n-bit tree
+    int atom_w[kMaxAtoms], atom_ib[kMaxAtoms], atom_ia[kMaxAtoms], alpha_atom[kMaxIntervals];
+};
+
 struct Program {
     // deep copy of the specification
-    uint32_t n = 0, frac_bits = 0, m = 0, r = 0, d = 0, p_aux = 0, ell = 0, mask_output = 0;
+    uint32_t n = 0, frac_bits = 0, m = 0, r = 0, d = 0, p_aux = 0, ell = 0, mask_output = 0, variant = 0;
+    SpProgram sp;
     std::vector<uint64_t> alpha, coeff, aux;
     std::vector<fusefss_bitnode> nodes;
     std::vector<uint16_t> bit_root;
@@ -72,6 +89,7 @@ struct Program {
     // device copy of the small tables (uploaded lazily by the launchers)
     void *dev_blob = nullptr;
     size_t dev_ins_off = 0, dev_alpha_off = 0, dev_payload_off = 0, dev_blob_bytes = 0;
+    size_t dev_sp_points_off = 0, dev_sp_weights_off = 0, dev_sp_delta_off = 0;
 };
 
 int compile_program(const fusefss_spec *spec, Program **out);

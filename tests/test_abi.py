@@ -34,6 +34,7 @@ ALL = [("relu16", lambda: specs.relu(16, 8)), ("gelu", specs.gelu), ("nexp", spe
        ("toy", lambda: specs.toy(8, 3)), ("toy_masked", lambda: specs.toy(8, 3, True)),
        ("plain", specs.plain_default), ("single", specs.single_interval), ("nobits", specs.no_bits),
        ("full", specs.full_partition), ("shift_relu8", lambda: specs.shift_relu(8, 3))]
+ALL = ALL + [(nm + "_sp", (lambda mk=mk: specs.shared_prefix(mk()))) for nm, mk in ALL]      # variant 1 (DESIGN 9)
 
 
 @pytest.mark.parametrize("name,mk", ALL)

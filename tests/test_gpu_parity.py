@@ -58,6 +58,14 @@ def _parity(F, orc, spec, x, r_in, r_out, seed, check_plain=True, first_elem=0):
         assert np.array_equal(host(got["y"][b])[:na], exp["y"][b]), spec.name + ": y shares"
         if P.shape["n_out_b"]:
             assert np.array_equal(host(got["z"][b]), exp["z"][b]), spec.name + ": z shares"
+    # the fused two-call evaluation == the separate calls, bit for bit
+    for b, k in ((0, k0), (1, k1)):
+        if P.shape["T"] or P.shape["has_lut"]:
+            fb, fc = P.eval_fused(b, k, dev(xhat))
+            if P.shape["T"]:
+                assert np.array_equal(host(fb), exp["bits"][b]), spec.name + ": eval_fused bits"
+            if P.shape["has_lut"]:
+                assert np.array_equal(host(fc), exp["coeff"][b]), spec.name + ": eval_fused coeff"
     # fused post == per-round post, bit for bit
     y0, y1, z0, z1 = P.post_fused(k0, k1, dev(xhat), got["bits"][0], got["bits"][1], got["coeff"][0], got["coeff"][1])
     assert np.array_equal(host(y0)[:na], exp["y"][0]) and np.array_equal(host(y1)[:na], exp["y"][1])
@@ -91,7 +99,10 @@ SMALL = [lambda: specs.relu(8, 4), lambda: specs.toy(8, 3), lambda: specs.toy(8,
          lambda: specs.toy(12, 4), lambda: specs.relu(12, 6)]
 
 
-@pytest.mark.parametrize("mk", SMALL)
+SMALL_SP = [(lambda mk=mk: specs.shared_prefix(mk())) for mk in SMALL]
+
+
+@pytest.mark.parametrize("mk", SMALL + SMALL_SP)
 @pytest.mark.parametrize("force_g", ["", "1"])
 def test_small_rings_all_masks(F, orc, mk, force_g, monkeypatch):
     """Every mask r (both Protocol 3 branches, incl. beta_0 = 0 and the dummy split) at n <= 8; a ragged count."""
@@ -115,22 +126,36 @@ CONFIGS = [("relu16", 4096), ("gelu", 700), ("nexp", 330), ("recip", 130), ("shi
            ("silu", 131)]
 
 
+@pytest.mark.parametrize("variant", [0, 1])
 @pytest.mark.parametrize("name,count", CONFIGS)
-def test_config_parity(F, orc, name, count):
+def test_config_parity(F, orc, name, count, variant):
     """BASELINE.json's configs on their seeded synthetic inputs (workloads/tensors.py), several 32-element tiles
-    and a ragged tail; config 1 at its full size."""
+    and a ragged tail; config 1 at its full size.  variant 1 = the single-key shared-prefix construction, whose
+    kernel shares tree prefixes between nearby points while the oracle walks every point from the root."""
     spec = specs.CONFIGS[name]()
+    if variant:
+        spec = specs.shared_prefix(spec)
+        count = min(4096, count * 4)
     inp = tensors.inputs(name, spec, count=count, seed=0)
     _parity(F, orc, spec, inp["x"], inp["r_in"], inp["r_out"], seed=0)
 
 
-def test_edge_masks_n64(F, orc):
+@pytest.mark.parametrize("variant", [0, 1])
+def test_edge_masks_n64(F, orc, variant):
     """n = 64 corner masks: r = 0 (beta_0 = 0 branch + dummy split), r = -alpha_i (a translated start lands on 0),
-    r = 2^64-1, and x at the interval boundaries."""
+    r = 2^64-1, and x at the interval boundaries; for variant 1 also xhat values whose cluster of points straddles
+    a 2^tail_bits boundary (two different prefixes) and wraps around 2^64."""
     spec = specs.gelu()
+    if variant:
+        spec = specs.shared_prefix(spec)
     a = np.array(spec.alpha, dtype=np.uint64)
     r_in = np.concatenate([np.array([0, 1, 2**64 - 1, 2**63, 2**63 - 1], dtype=np.uint64), (np.uint64(0) - a), (np.uint64(0) - a) + np.uint64(1)])
     x = np.resize(np.concatenate([a, a - np.uint64(1), np.array([0, 2**64 - 1], dtype=np.uint64)]), r_in.size)
+    if variant:                                            # xhat = x + r near multiples of 2^16 and near 0 / 2^64
+        xh = np.array([0, 1, 2**64 - 1, 2**16, 2**16 - 1, 2**16 + 1, 3 * 2**16 + 5, 2**63, 2**63 + 2**15, 2**64 - 2**14, 2**14, 5 * 2**17 - 3],
+                      dtype=np.uint64)
+        r_in = np.concatenate([r_in, np.arange(xh.size, dtype=np.uint64) * np.uint64(0x9E3779B97F4A7C15)])
+        x = np.concatenate([x, xh - r_in[-xh.size:]])
     r_out = np.arange(r_in.size, dtype=np.uint64)
     _parity(F, orc, spec, x, r_in, r_out, seed=9)
 
