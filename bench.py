@@ -118,6 +118,68 @@ def run_reference(args, rank):
     print(json.dumps(line), flush=True)
 
 
+def measure_shared_prefix(F, torch, name, base_spec, inp, rank, world, steps, warmup, barrier, max_over_ranks):
+    """The same workload compiled with variant 1 (single-key shared-prefix construction):
+    keygen (one n-bit key per element) + ONE fused evaluation per party + post, timed like the main step."""
+    from workloads import specs as _specs
+    spec = _specs.shared_prefix(base_spec)
+    P = F.Program(spec)
+    sh, cost = P.shape, P.cost()
+    count = int(inp["xhat"].size)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.int64)).cuda()
+    r_in, r_out, xhat = dev(inp["r_in"]), dev(inp["r_out"]), dev(inp["xhat"])
+    k0, k1 = P.alloc_keys(count)
+    na = max(1, sh["n_out_a"])
+    bits = [torch.empty(count, dtype=torch.int64, device="cuda") for _ in (0, 1)]
+    coeff = [torch.empty((sh["p"], count), dtype=torch.int64, device="cuda") for _ in (0, 1)]
+    outs = (torch.empty((na, count), dtype=torch.int64, device="cuda"), torch.empty((na, count), dtype=torch.int64, device="cuda"),
+            torch.empty(count, dtype=torch.int64, device="cuda"), torch.empty(count, dtype=torch.int64, device="cuda"))
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    events = []
+
+    def step(record):
+        e = [ev() for _ in range(4)]
+        e[0].record()
+        P.keygen(r_in, r_out, 0, rank * count, keys=(k0, k1))
+        e[1].record()
+        for b, k in ((0, k0), (1, k1)):
+            P.eval_fused(b, k, xhat, bits[b] if sh["T"] else None, coeff[b] if sh["has_lut"] else None)
+        e[2].record()
+        P.post_fused(k0, k1, xhat, bits[0], bits[1], coeff[0], coeff[1], outs=outs)
+        e[3].record()
+        if record:
+            events.append(e)
+    for _ in range(max(warmup, 3)):
+        step(False)
+    barrier()
+    l0 = F.launch_count()
+    start, stop = ev(), ev()
+    start.record()
+    for _ in range(steps):
+        step(True)
+    stop.record()
+    barrier()
+    ms = max_over_ranks(start.elapsed_time(stop)) / steps
+    t_gen = sum(e[0].elapsed_time(e[1]) for e in events) / steps
+    t_eval = sum(e[1].elapsed_time(e[2]) for e in events) / steps
+    t_post = sum(e[2].elapsed_time(e[3]) for e in events) / steps
+    aes_eval = cost["eval_cmp_aes"] + cost["eval_lut_aes"]
+    lk_eval = cost["eval_cmp_lookups"] + cost["eval_lut_lookups"]
+    ach = aes_eval * count / (t_eval / 2 * 1e-3) / 1e9
+    peak = 148 * SM_CLOCK_MAX_MHZ * 1e6 * LDS_LANES_PER_CLK_SM / (lk_eval / max(1, aes_eval)) / 1e9
+    key_b = P.key_bytes(1 << 20) / (1 << 20)
+    return {"construction": "variant 1: one DCF key f_{r,1} per view width, evaluated at the public points xhat + delta_j with shared tree prefixes (DESIGN 9)",
+            "value": world * count / (ms * 1e-3), "unit": "elements/s", "ms_per_step": ms,
+            "eval_elems_per_s": world * count / (t_eval * 1e-3), "keygen_elems_per_s": world * count / (t_gen * 1e-3),
+            "ms_breakdown": {"keygen": t_gen, "eval_fused_x2": t_eval, "post_fused": t_post},
+            "key_bytes_per_elem_per_party": key_b, "online_bytes_per_elem_per_party": P.online_bits() / 8,
+            "aes_per_elem": {"eval_one_party": aes_eval, "keygen_both": cost["gen_cmp_aes"] + cost["gen_lut_aes"]},
+            "gpu_launches": F.launch_count() - l0,
+            "roofline": {"bound": "alu", "kernel": "k_eval_sp", "achieved": ach, "peak": peak, "unit": "GAES/s (AES-128 blocks per second)",
+                         "frac": ach / peak, "lookups_per_aes": lk_eval / max(1, aes_eval), "launch_ms": t_eval / 2, "traffic": None,
+                         "hbm_achieved_gbs": key_b * count / (t_eval / 2 * 1e-3) / 1e9}}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -131,6 +193,7 @@ def main():
     ap.add_argument("--cpu-sample", type=int, default=2048)
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-sp", action="store_true", help="skip the variant-1 (shared-prefix) measurement")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     rank = int(os.environ.get("RANK", "0"))
@@ -200,6 +263,13 @@ def main():
             if record:
                 step.events.append(e)
     step.seed, step.events = 0, []
+
+    def _allmax(v):
+        if world > 1:
+            t = torch.tensor([v], device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            return float(t.item())
+        return v
 
     def barrier():
         torch.cuda.synchronize()
@@ -293,6 +363,14 @@ def main():
             "aes_rate_gaes": {"eval": 2 * aes_eval * count / ((per_step(t_cmp) + per_step(t_lut)) * 1e-3) / 1e9,
                               "keygen": aes_gen * count / (per_step(t_gen) * 1e-3) / 1e9},
             "gpu_launches": launches, "clocks": clocks.summary(), "roofline": roofline}
+
+    # ---- the same workload with the single-key shared-prefix construction (variant 1) ------------------
+    if not args.no_sp and chunk == count:
+        del k0, k1
+        torch.cuda.empty_cache()
+        line["shared_prefix"] = measure_shared_prefix(F, torch, name, spec, inp, rank, world, args.steps, args.warmup, barrier,
+                                                      lambda v: (float(_allmax(v))))
+        k0, k1 = None, None
 
     # ---- e2e: the public host-buffer call, pinned host memory, H2D + D2H inside the timed region -------
     if not args.no_e2e:

@@ -178,6 +178,17 @@ int fusefss_gate_host(const fusefss_program *prog, const uint64_t *r_in, const u
                       const uint64_t *xhat, uint64_t seed, size_t count, size_t chunk, void *workspace_dev,
                       uint64_t *y0, uint64_t *y1, uint64_t *z0, uint64_t *z1, void *stream);
 
+/* ---- algorithmic work per element (for the roofline; DESIGN 5.3, 9) ---------------------------------
+ * AES-128 blocks and T-table lookups of one party's evaluation (cmp part / lut part; for variant 1 "lut" = the fused
+ * walk of the n-bit tree, "cmp" = the narrower bit trees) and of the dealer's keygen (both bundles), plus the key
+ * bytes one party's evaluation reads. */
+typedef struct {
+    uint64_t eval_cmp_aes, eval_cmp_lookups, eval_lut_aes, eval_lut_lookups;
+    uint64_t gen_cmp_aes, gen_cmp_lookups, gen_lut_aes, gen_lut_lookups;
+    uint64_t eval_cmp_key_bytes, eval_lut_key_bytes;
+} fusefss_cost_t;
+int fusefss_cost(const fusefss_program *prog, fusefss_cost_t *out);
+
 /* ---- diagnostics ---------------------------------------------------------------------------------- */
 const char *fusefss_strerror(int code);
 const char *fusefss_last_cuda_error(void);

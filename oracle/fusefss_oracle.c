@@ -23,6 +23,9 @@
  * every share to F(x)/G(x), the DCF truth table, Protocol 3's post-conditions,
  * AES-128 against FIPS-197 -- is pinned in tests/ (-m "not gpu").
  *
+ * Variant 1 (spec.variant = 1): the single-key shared-prefix construction -- one DCF key
+ * f_{r_k,1} per view width, evaluated point by point from the root (sp_eval); pinned in tests/test_oracle_sp.py.
+ *
  * Arithmetic: integers only.  Ring elements are uint64_t with bits >= n zero.
  * 2^n (n = 64) is handled with unsigned __int128, never as a ring element.
  */

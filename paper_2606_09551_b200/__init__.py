@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libfusefss.so")
 SYMBOLS = (
     "fusefss_compile", "fusefss_destroy", "fusefss_shape", "fusefss_atom", "fusefss_key_bytes", "fusefss_keygen", "fusefss_keygen_parts",
     "fusefss_eval_cmp", "fusefss_eval_lut", "fusefss_eval_fused", "fusefss_post", "fusefss_post_rounds", "fusefss_post_msg_bytes",
-    "fusefss_online_bits", "fusefss_post_fused", "fusefss_gate_workspace_bytes", "fusefss_gate_host",
+    "fusefss_online_bits", "fusefss_post_fused", "fusefss_cost", "fusefss_gate_workspace_bytes", "fusefss_gate_host",
     "fusefss_strerror", "fusefss_last_cuda_error", "fusefss_launch_count", "fusefss_aes_probe", "fusefss_aes_kat",
 )
 
@@ -43,6 +43,12 @@ class Spec(C.Structure):
     _fields_ = [(k, C.c_uint32) for k in ("n", "frac_bits", "m", "r", "d", "p_aux", "ell", "n_nodes", "n_kappa_a",
                                           "n_kappa_b", "phi_len", "n_out_a", "n_out_b", "mask_output", "variant")] + \
                [(k, C.c_void_p) for k in ("alpha", "coeff", "aux", "nodes", "bit_root", "kappa_a", "kappa_b", "phi")]
+
+
+class Cost(C.Structure):
+    _fields_ = [(k, C.c_uint64) for k in ("eval_cmp_aes", "eval_cmp_lookups", "eval_lut_aes", "eval_lut_lookups", "gen_cmp_aes",
+                                          "gen_cmp_lookups", "gen_lut_aes", "gen_lut_lookups", "eval_cmp_key_bytes",
+                                          "eval_lut_key_bytes")]
 
 
 class Shape(C.Structure):
@@ -72,6 +78,7 @@ def _load():
         "fusefss_post_msg_bytes": (sz, [vp, sz, i32]),
         "fusefss_online_bits": (sz, [vp]),
         "fusefss_post_fused": (i32, [vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp, vp, vp, vp]),
+        "fusefss_cost": (i32, [vp, C.POINTER(Cost)]),
         "fusefss_gate_workspace_bytes": (sz, [vp, sz]),
         "fusefss_gate_host": (i32, [vp, vp, vp, vp, u64, sz, sz, vp, vp, vp, vp, vp, vp]),
         "fusefss_strerror": (C.c_char_p, [i32]),
@@ -182,6 +189,11 @@ class Program:
 
     def online_bits(self):
         return lib.fusefss_online_bits(self._h)
+
+    def cost(self):
+        c = Cost()
+        _check(lib.fusefss_cost(self._h, C.byref(c)))
+        return {k: int(getattr(c, k)) for k, _ in Cost._fields_}
 
     def workspace_bytes(self, chunk):
         return lib.fusefss_gate_workspace_bytes(self._h, chunk)

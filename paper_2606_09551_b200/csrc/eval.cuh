@@ -31,7 +31,7 @@ __global__ void __launch_bounds__(kEvalThreads, 1) k_eval_cmp(const __grid_const
     const size_t tiles = (a.count + 31) / 32;
     const size_t items = tiles * (size_t)a.G;
     const size_t warps = (size_t)gridDim.x * (blockDim.x >> 5);
-    for (size_t it = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); it < items; it += warps) {
+    for (size_t it = (size_t)(threadIdx.x >> 5) * gridDim.x + blockIdx.x; it < items; it += warps) {   // warp w of CTA b takes items w*grid + b: a partial last wave spreads over all SMs
         const int g = (int)(it / tiles);
         const size_t tile = it - (size_t)g * tiles;
         size_t e = tile * 32 + lane;
@@ -98,7 +98,7 @@ __global__ void __launch_bounds__(kEvalThreads, 1) k_eval_lut(const __grid_const
     const size_t tiles = (a.count + 31) / 32;
     const size_t items = tiles * (size_t)a.G;
     const size_t warps = (size_t)gridDim.x * (blockDim.x >> 5);
-    for (size_t it = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); it < items; it += warps) {
+    for (size_t it = (size_t)(threadIdx.x >> 5) * gridDim.x + blockIdx.x; it < items; it += warps) {   // warp w of CTA b takes items w*grid + b: a partial last wave spreads over all SMs
         const int g = (int)(it / tiles);
         const size_t tile = it - (size_t)g * tiles;
         size_t e = tile * 32 + lane;

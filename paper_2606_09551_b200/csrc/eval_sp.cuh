@@ -110,8 +110,10 @@ template <int P>
 __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ EvalSpArgs a) {
     extern __shared__ uint32_t sT[];
     const uint32_t tl = aes_fill_tables(sT);
-    const size_t padded = (a.count + 31) & ~(size_t)31;                     // whole warps stay converged
-    for (size_t e0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e0 < padded; e0 += (size_t)gridDim.x * blockDim.x) {
+    const size_t tiles = (a.count + 31) / 32, warps = (size_t)gridDim.x * (blockDim.x >> 5);
+    // warp w of CTA b takes tiles w*grid + b (+ k*warps): a partial last wave spreads evenly over all SMs
+    for (size_t tile = (size_t)(threadIdx.x >> 5) * gridDim.x + blockIdx.x; tile < tiles; tile += warps) {
+        const size_t e0 = tile * 32 + (threadIdx.x & 31);
         const bool live = e0 < a.count;
         const size_t e = live ? e0 : a.count - 1;
         const uint64_t xh = a.xhat[e] & a.mask;

@@ -44,7 +44,7 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_bit(const __grid_constan
     const size_t tiles = (a.count + 31) / 32;
     const size_t items = tiles * (size_t)a.T;
     const size_t warps = (size_t)gridDim.x * (blockDim.x >> 5);
-    for (size_t it = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); it < items; it += warps) {
+    for (size_t it = (size_t)(threadIdx.x >> 5) * gridDim.x + blockIdx.x; it < items; it += warps) {   // warp w of CTA b takes items w*grid + b: a partial last wave spreads over all SMs
         const int t = (int)(it / tiles);
         const size_t e = (it - (size_t)t * tiles) * 32 + lane;
         if (e >= a.count) continue;
@@ -189,7 +189,7 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec(const __grid_constan
     const size_t tiles = (a.count + 31) / 32;
     const size_t items = tiles * (size_t)(a.M - 1);
     const size_t warps = (size_t)gridDim.x * (blockDim.x >> 5);
-    for (size_t it = (size_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); it < items; it += warps) {
+    for (size_t it = (size_t)(threadIdx.x >> 5) * gridDim.x + blockIdx.x; it < items; it += warps) {   // warp w of CTA b takes items w*grid + b: a partial last wave spreads over all SMs
         const int j = 1 + (int)(it / tiles);
         const size_t e = (it - (size_t)(j - 1) * tiles) * 32 + lane;
         if (e >= a.count) continue;

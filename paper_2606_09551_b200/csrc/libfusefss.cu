@@ -265,6 +265,51 @@ size_t fusefss_online_bits(const fusefss_program *prog) {
            (P->mask_output ? (size_t)P->n * P->n_out_a : 0);
 }
 
+// Algorithmic work per element, from the compiled program (DESIGN 5.3 / 9): AES blocks and T-table lookups.
+// A group of B blocks expanded from one seed costs 15 + B + 144 B lookups (B > 1), a lone block 160.
+int fusefss_cost(const fusefss_program *prog, fusefss_cost_t *out) {
+    const Program *P = prog_of(prog);
+    if (!P || !out) return FUSEFSS_E_NULL;
+    auto grp = [](uint64_t B) { return B > 1 ? 15 + B + 144 * B : (uint64_t)160; };
+    const uint64_t n = P->n, Q = (uint64_t)P->Q;
+    fusefss_cost_t c{};
+    if (!P->variant) {
+        for (int t = 0; t < P->T; ++t) {
+            const uint64_t k = (uint64_t)P->atoms[t].k;
+            c.eval_cmp_aes += k + 1; c.eval_cmp_lookups += 160 * (k + 1);
+            c.gen_cmp_aes += 4 * k + 4; c.gen_cmp_lookups += 2 * 160 + k * 2 * grp(2) + 2 * 160;
+            c.eval_cmp_key_bytes += 16 * (k + 1) + 8;
+        }
+        if (P->has_lut) {
+            const uint64_t trees = (uint64_t)P->M - 1, p = (uint64_t)P->p;
+            c.eval_lut_aes = trees * (n * (1 + Q) + Q); c.eval_lut_lookups = trees * (n * grp(1 + Q) + grp(Q));
+            c.gen_lut_aes = trees * (4 * n * (1 + Q) + 2 * Q + 2); c.gen_lut_lookups = trees * (2 * 160 + n * 2 * grp(2 * (1 + Q)) + 2 * grp(Q));
+            c.eval_lut_key_bytes = 8 * p + trees * (16 + n * (16 + 8 * p) + 8 * p);
+        }
+    } else {
+        for (int w = 0; w < P->sp.n_w; ++w) {
+            const SpWidth &W = P->sp.width[w];
+            const uint64_t k = (uint64_t)W.k;
+            if (!W.is_vec) {
+                c.eval_cmp_aes += (uint64_t)W.n_points * (k + 1); c.eval_cmp_lookups += 160 * (uint64_t)W.n_points * (k + 1);
+                c.gen_cmp_aes += 4 * k + 4; c.gen_cmp_lookups += 2 * 160 + k * 2 * grp(2) + 2 * 160;
+                c.eval_cmp_key_bytes += 16 * (k + 1) + 8;
+                continue;
+            }
+            for (const SpCluster &cl : P->sp.clusters) {                       // fused walk: every point of the n-bit tree
+                const uint64_t kf = n - (uint64_t)cl.tail_bits;
+                const bool share = cl.count > 1 && kf > 0;
+                const uint64_t levels = share ? 2 * kf + (uint64_t)cl.count * (uint64_t)cl.tail_bits : (uint64_t)cl.count * n;
+                c.eval_lut_aes += 2 * levels + (uint64_t)cl.count; c.eval_lut_lookups += levels * grp(2) + 160 * (uint64_t)cl.count;
+            }
+            c.gen_lut_aes += 8 * n + 4; c.gen_lut_lookups += 2 * 160 + n * 2 * grp(4) + 2 * 160;
+            c.eval_lut_key_bytes += 16 + n * 24 + 8;
+        }
+    }
+    *out = c;
+    return 0;
+}
+
 const char *fusefss_strerror(int code) {
     switch (code) {
     case FUSEFSS_OK: return "ok";
