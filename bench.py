@@ -364,6 +364,22 @@ def main():
                               "keygen": aes_gen * count / (per_step(t_gen) * 1e-3) / 1e9},
             "gpu_launches": launches, "clocks": clocks.summary(), "roofline": roofline}
 
+    # ---- PRG core alone (a pure AES chain, no key traffic): what the table design sustains on this GPU ----
+    try:
+        probe_threads, probe_iters = 148 * 1024 * 4, 192
+        pout = torch.empty(probe_threads * 16, dtype=torch.uint8, device="cuda")
+        F.aes_probe(probe_threads, probe_iters, pout)
+        torch.cuda.synchronize()
+        p0, p1 = ev(), ev()
+        p0.record(); F.aes_probe(probe_threads, probe_iters, pout); p1.record()
+        torch.cuda.synchronize()
+        line["prg_probe"] = {"gaes": probe_threads * probe_iters / (p0.elapsed_time(p1) * 1e-3) / 1e9,
+                             "what": "fusefss_aes_probe: 3 blocks per trip sharing round 1 (150 lookups per block), no key loads",
+                             "lookup_roof_gaes": 148 * SM_CLOCK_MAX_MHZ * 1e6 * LDS_LANES_PER_CLK_SM / 150.0 / 1e9}
+        del pout
+    except Exception as exc:                                      # the probe is informative only
+        line["prg_probe"] = {"error": str(exc)}
+
     # ---- the same workload with the single-key shared-prefix construction (variant 1) ------------------
     if not args.no_sp and chunk == count:
         del k0, k1

@@ -599,7 +599,7 @@ __global__ void __launch_bounds__(kEvalThreads, 1) k_aes_probe(const ProbeArgs a
         uint32_t x[1][4] = {{(uint32_t)i, (uint32_t)(i >> 32), 0x9e3779b9u, 0x7f4a7c15u}};
         for (int it = 0; it < a.iters; it += 3) {                       // 3 independent keys per trip, like a p = 3 level
             uint32_t o[1][3][4];
-            prg_blocks<1, 3, 0>(tl, x, o);
+            prg_blocks<1, 3, 0, true>(tl, x, o);
 #pragma unroll
             for (int c = 0; c < 4; ++c) x[0][c] = o[0][0][c] ^ o[0][1][(c + 1) & 3] ^ o[0][2][(c + 2) & 3];
         }
