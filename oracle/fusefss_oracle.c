@@ -530,7 +530,8 @@ typedef struct { int k; u64 c; int is_theta; u64 beta; int carry_idx; } atom_t;
 
 enum {
     C_B_CONST = 1, C_B_ATOM, C_B_KAPPA, C_B_XHAT, C_B_NOT, C_B_XOR, C_B_AND, C_B_ANDPUB, C_B_OUT,
-    C_A_CONST, C_A_X, C_A_COEFF, C_A_KAPPA, C_A_XHAT_SHR, C_A_ADD, C_A_SUB, C_A_MULC, C_A_MUL, C_A_B2A, C_A_OUT
+    C_A_CONST, C_A_X, C_A_COEFF, C_A_KAPPA, C_A_XHAT_SHR, C_A_ADD, C_A_SUB, C_A_MULC, C_A_MUL, C_A_B2A, C_A_OUT,
+    C_A_MULX      /* variant bit 1: product with the gate input x = xhat - r_in, one opening (DESIGN 10) */
 };
 typedef struct { int op, dst, a, b, idx, round; u64 imm; } cop_t;
 
@@ -549,6 +550,9 @@ typedef struct orc_prog {
     int n_out_a, n_out_b;
     /* per round message shape */
     int r_nmul[16], r_nbits[16];
+    int xmul;                         /* variant bit 1 */
+    int r_narr[16];                   /* ring-element arrays opened per round: 2 per Beaver, 1 per x-product */
+    int ma_is_x[64], ma_word[65];     /* per arithmetic gate: kind, first word of its material in the key */
     /* lowering memo */
     int node_reg[4096];
     int calpha_reg[MMAX + 1];
@@ -748,7 +752,8 @@ orc_prog *orc_compile(const orc_spec *S0)
     u128 N = (u128)1 << P->n;
     P->M = ((u128)(P->m + 1) < N) ? P->m + 1 : (int)N;
     P->has_lut = P->m > 1;                               /* single interval: lookup omitted */
-    P->variant = (int)S->variant;
+    P->variant = (int)(S->variant & 1);
+    P->xmul = (int)((S->variant >> 1) & 1);
     if (P->variant) P->M = P->m;                         /* no translated partition, hence no wrap/dummy split */
     for (int i = 0; i < 4096; i++) P->node_reg[i] = -1;
     for (int i = 0; i <= MMAX; i++) P->calpha_reg[i] = -1;
@@ -764,7 +769,7 @@ orc_prog *orc_compile(const orc_spec *S0)
     }
     int piecewise = 0;
     for (u32 j = 0; j < S->ell; j++) if (!bit_is_uniform(S, j)) piecewise = 1;
-    if (piecewise || (S->variant && P->m > 1)) for (int i = 1; i < P->m; i++) add_pred(P, P->n, 0, S->alpha[i - 1]);
+    if (piecewise || ((S->variant & 1) && P->m > 1)) for (int i = 1; i < P->m; i++) add_pred(P, P->n, 0, S->alpha[i - 1]);
     /* flatten: per view, the r-atom then one theta-atom per distinct beta */
     P->T = 0; P->n_carry = 0;
     for (int v = 0; v < P->nviews; v++) {
@@ -772,18 +777,18 @@ orc_prog *orc_compile(const orc_spec *S0)
         V->first_atom = P->T;
         if (P->T + 1 + V->nbeta > TMAX) { orc_destroy(P); return NULL; }
         atom_t *a;
-        if (!S->variant || V->want_carry) {              /* variant 1 keeps the r-atom only where a CARRY node reads it */
+        if (!(S->variant & 1) || V->want_carry) {              /* variant 1 keeps the r-atom only where a CARRY node reads it */
             a = &P->atoms[P->T++];
             a->k = V->k; a->c = V->c; a->is_theta = 0; a->beta = 0; a->carry_idx = -1;
         }
         for (int j = 0; j < V->nbeta; j++) {
             a = &P->atoms[P->T++];
             a->k = V->k; a->c = V->c; a->is_theta = 1; a->beta = V->beta[j];
-            a->carry_idx = S->variant ? -1 : P->n_carry++;
+            a->carry_idx = (S->variant & 1) ? -1 : P->n_carry++;
         }
     }
     P->n_kb = P->n_carry + (int)S->n_kappa_b;
-    if (S->variant && sp_points(P) < 0) { orc_destroy(P); return NULL; }
+    if ((S->variant & 1) && sp_points(P) < 0) { orc_destroy(P); return NULL; }
 
     /* program: Horner (step-major), Boolean circuit (bit-major), then Phi */
     int xreg = newa(P, 0); emit(P, C_A_X, xreg, 0, 0, 0);
@@ -802,7 +807,7 @@ orc_prog *orc_compile(const orc_spec *S0)
         for (u32 j = 0; j < S->r; j++) {
             int rd = imax(P->ardy[yreg[j]], P->ardy[xreg]);
             int prod = newa(P, rd + 1);
-            int i = emit(P, C_A_MUL, prod, yreg[j], xreg, 0);
+            int i = emit(P, P->xmul ? C_A_MULX : C_A_MUL, prod, yreg[j], xreg, 0);
             P->ops[i].idx = P->MA++; P->ops[i].round = rd;
             int sum = newa(P, rd + 1);
             emit(P, C_A_ADD, sum, prod, creg[j * (S->d + 1) + k], 0);
@@ -845,7 +850,10 @@ orc_prog *orc_compile(const orc_spec *S0)
             case PHI_A_MULC: d = newa(P, P->ardy[ua[o->a]]); emit(P, C_A_MULC, d, ua[o->a], 0, o->imm); ua[o->dst] = d; break;
             case PHI_A_MUL: {
                 int rd = imax(P->ardy[ua[o->a]], P->ardy[ua[o->b]]);
-                d = newa(P, rd + 1); k = emit(P, C_A_MUL, d, ua[o->a], ua[o->b], 0);
+                int ax = ua[o->a] == xreg, bx = ua[o->b] == xreg;
+                d = newa(P, rd + 1);
+                if (P->xmul && ax != bx) k = emit(P, C_A_MULX, d, ax ? ua[o->b] : ua[o->a], xreg, 0);
+                else k = emit(P, C_A_MUL, d, ua[o->a], ua[o->b], 0);
                 P->ops[k].idx = P->MA++; P->ops[k].round = rd; ua[o->dst] = d; break; }
             case PHI_A_B2A: {
                 int rd = P->brdy[ub[o->a]];
@@ -868,14 +876,17 @@ orc_prog *orc_compile(const orc_spec *S0)
     }
     P->rounds = 0;
     for (int i = 0; i < P->nops; i++) if (P->ops[i].round >= 0) P->rounds = imax(P->rounds, P->ops[i].round + 1);
-    if (P->rounds > 16 || P->MB > 64 || P->GMIX > 64) { orc_destroy(P); return NULL; }
+    if (P->rounds > 16 || P->MB > 64 || P->GMIX > 64 || P->MA > 64) { orc_destroy(P); return NULL; }
     for (int i = 0; i < P->nops; i++) {
         cop_t *o = &P->ops[i];
         if (o->round < 0) continue;
-        if (o->op == C_A_MUL) P->r_nmul[o->round]++;
+        if (o->op == C_A_MUL) { P->r_nmul[o->round]++; P->r_narr[o->round] += 2; P->ma_is_x[o->idx] = 0; }
+        if (o->op == C_A_MULX) { P->r_nmul[o->round]++; P->r_narr[o->round] += 1; P->ma_is_x[o->idx] = 1; }
         if (o->op == C_B_AND) P->r_nbits[o->round] += 2;
         if (o->op == C_A_B2A) P->r_nbits[o->round] += 1;
     }
+    P->ma_word[0] = 0;
+    for (int i = 0; i < P->MA; i++) P->ma_word[i + 1] = P->ma_word[i] + (P->ma_is_x[i] ? 2 : 3);
     return P;
 }
 
@@ -999,7 +1010,7 @@ static void layout(const orc_prog *P, size_t count, layout_t *L)
     L->rout = off; if (P->S.mask_output) off += (size_t)P->n_out_a * L->s8;
     L->ka = off; off += (size_t)P->S.n_kappa_a * L->s8;
     L->kb = off; if (P->n_kb > 0) off += L->s8;
-    L->beaver = off; off += (size_t)3 * P->MA * L->s8;
+    L->beaver = off; off += (size_t)P->ma_word[P->MA] * L->s8;
     L->andt = off; if (P->MB > 0) off += 3 * L->s8;
     L->b2a_bits = off; if (P->GMIX > 0) off += L->s8;
     L->b2a_a = off; off += (size_t)P->GMIX * L->s8;
@@ -1161,7 +1172,13 @@ void orc_keygen(const orc_prog *P, const u64 *r_in, const u64 *r_out, u64 seed, 
             u64 a0 = le64(rb) & mask, b0 = le64(rb + 8) & mask;
             rnd(&ks, ge, SLOT_BV_C0 + i, rb);
             u64 c0 = le64(rb) & mask;
-            size_t o = L.beaver + (size_t)3 * i * L.s8;
+            size_t o = L.beaver + (size_t)P->ma_word[i] * L.s8;
+            if (P->ma_is_x[i]) {                                        /* (b, c = b r_in): DESIGN 10 */
+                u64 cx = (b * r) & mask;
+                st8(key0, o, e, b0); st8(key0, o + L.s8, e, c0);
+                st8(key1, o, e, (b - b0) & mask); st8(key1, o + L.s8, e, (cx - c0) & mask);
+                continue;
+            }
             st8(key0, o, e, a0); st8(key0, o + L.s8, e, b0); st8(key0, o + 2 * L.s8, e, c0);
             st8(key1, o, e, (a - a0) & mask); st8(key1, o + L.s8, e, (b - b0) & mask); st8(key1, o + 2 * L.s8, e, (c - c0) & mask);
         }
@@ -1325,14 +1342,16 @@ size_t orc_post_msg_bytes(const orc_prog *P, size_t count, int round)
 {
     size_t s8 = rup256(count * 8);
     if (round < 0 || round >= P->rounds) return 0;
-    return s8 * ((size_t)2 * P->r_nmul[round] + (P->r_nbits[round] ? 1 : 0));
+    return s8 * ((size_t)P->r_narr[round] + (P->r_nbits[round] ? 1 : 0));
 }
 int orc_post_rounds(const orc_prog *P) { return P->rounds; }
 /* algorithmic online bits per element per party: n (xhat, Protocol 1) + 2n per Beaver + 2 per AND + 1 per B2A
  * (+ n per masked output) */
 size_t orc_online_bits(const orc_prog *P)
 {
-    return (size_t)P->n + (size_t)2 * P->n * P->MA + (size_t)2 * P->MB + (size_t)P->GMIX
+    size_t arrs = 0;
+    for (int q = 0; q < P->rounds; q++) arrs += (size_t)P->r_narr[q];
+    return (size_t)P->n + (size_t)P->n * arrs + (size_t)2 * P->MB + (size_t)P->GMIX
          + (P->S.mask_output ? (size_t)P->n * P->n_out_a : 0);
 }
 
@@ -1368,7 +1387,7 @@ void orc_post(int party, const orc_prog *P, const u8 *key, const u64 *xhat, cons
                 u8 dm = Bv[o->a] ^ ta, em = Bv[o->b] ^ tb;
                 if (q == round) outbits[q] |= ((u64)dm << pos) | ((u64)em << (pos + 1));
                 if (q < round) {
-                    u64 other = ld8(msg_in, roff[q] + (size_t)2 * P->r_nmul[q] * s8, e);
+                    u64 other = ld8(msg_in, roff[q] + (size_t)P->r_narr[q] * s8, e);
                     u8 dd = dm ^ (u8)((other >> pos) & 1), ee = em ^ (u8)((other >> (pos + 1)) & 1);
                     Bv[o->dst] = (u8)((party == 0 ? (dd & ee) : 0) ^ (dd & tb) ^ (ee & ta) ^ tc);
                 } else Bv[o->dst] = 0;
@@ -1388,15 +1407,27 @@ void orc_post(int party, const orc_prog *P, const u8 *key, const u64 *xhat, cons
                 if (round == P->rounds) y_out[(size_t)o->dst * count + e] = v;
                 break; }
             case C_A_MUL: {  /* Beaver: open e = x-a, f = y-b; [xy]_b = [b=0]ef + e[b]_b + f[a]_b + [c]_b */
-                int q = o->round, pos = mulpos[q]++;
-                size_t to = L.beaver + (size_t)3 * o->idx * L.s8;
+                int q = o->round, pos = mulpos[q]; mulpos[q] += 2;      /* pos = first array of this gate in round q */
+                size_t to = L.beaver + (size_t)P->ma_word[o->idx] * L.s8;
                 u64 ta = ld8(key, to, e), tb = ld8(key, to + L.s8, e), tc = ld8(key, to + 2 * L.s8, e);
                 u64 em = (A[o->a] - ta) & mask, fm = (A[o->b] - tb) & mask;
-                if (q == round) { st8(msg_out, roff[q] + (size_t)2 * pos * s8, e, em); st8(msg_out, roff[q] + (size_t)(2 * pos + 1) * s8, e, fm); }
+                if (q == round) { st8(msg_out, roff[q] + (size_t)pos * s8, e, em); st8(msg_out, roff[q] + (size_t)(pos + 1) * s8, e, fm); }
                 if (q < round) {
-                    u64 E = (em + ld8(msg_in, roff[q] + (size_t)2 * pos * s8, e)) & mask;
-                    u64 F = (fm + ld8(msg_in, roff[q] + (size_t)(2 * pos + 1) * s8, e)) & mask;
+                    u64 E = (em + ld8(msg_in, roff[q] + (size_t)pos * s8, e)) & mask;
+                    u64 F = (fm + ld8(msg_in, roff[q] + (size_t)(pos + 1) * s8, e)) & mask;
                     A[o->dst] = ((party == 0 ? E * F : 0) + E * tb + F * ta + tc) & mask;
+                } else A[o->dst] = 0;
+                break; }
+            case C_A_MULX: { /* y * x with x = xhat - r_in, xhat public (DESIGN 10): material (b, c = b r_in); open f = y - b;
+                              * [y x]_b = xhat [y]_b - f [r_in]_b - [c]_b */
+                int q = o->round, pos = mulpos[q]; mulpos[q] += 1;
+                size_t to = L.beaver + (size_t)P->ma_word[o->idx] * L.s8;
+                u64 tb = ld8(key, to, e), tc = ld8(key, to + L.s8, e);
+                u64 fm = (A[o->a] - tb) & mask;
+                if (q == round) st8(msg_out, roff[q] + (size_t)pos * s8, e, fm);
+                if (q < round) {
+                    u64 F = (fm + ld8(msg_in, roff[q] + (size_t)pos * s8, e)) & mask;
+                    A[o->dst] = (xh * A[o->a] - F * ld8(key, L.rin, e) - tc) & mask;
                 } else A[o->dst] = 0;
                 break; }
             case C_A_B2A: {  /* open mu = z ^ rho; [z]_b = [b=0]mu + [rho]_b - 2 mu [rho]_b */
@@ -1406,7 +1437,7 @@ void orc_post(int party, const orc_prog *P, const u8 *key, const u64 *xhat, cons
                 u8 mm = Bv[o->a] ^ rb;
                 if (q == round) outbits[q] |= (u64)mm << pos;
                 if (q < round) {
-                    u64 other = ld8(msg_in, roff[q] + (size_t)2 * P->r_nmul[q] * s8, e);
+                    u64 other = ld8(msg_in, roff[q] + (size_t)P->r_narr[q] * s8, e);
                     u64 mu = (u64)(mm ^ (u8)((other >> pos) & 1));
                     A[o->dst] = ((party == 0 ? mu : 0) + ra - 2 * mu * ra) & mask;
                 } else A[o->dst] = 0;
@@ -1414,7 +1445,7 @@ void orc_post(int party, const orc_prog *P, const u8 *key, const u64 *xhat, cons
             }
         }
         if (round < P->rounds && P->r_nbits[round])
-            st8(msg_out, roff[round] + (size_t)2 * P->r_nmul[round] * s8, e, outbits[round]);
+            st8(msg_out, roff[round] + (size_t)P->r_narr[round] * s8, e, outbits[round]);
         if (round == P->rounds && P->n_out_b > 0) z_out[e] = zword;
     }
     free(A); free(Bv);

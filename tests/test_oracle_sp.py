@@ -102,3 +102,44 @@ def test_sp_share_is_not_the_value(orc):
     xhat = (np.uint64(77) + r_in) & mask_of(8)
     b0 = P.eval_cmp(0, k0, xhat) & np.uint64(1)
     assert 80 < int(b0.sum()) < 176
+
+
+# ---- variant bit 1: input-masked products ------------------------------------------
+XM = [lambda: specs.relu(8, 4), lambda: specs.toy(8, 3), lambda: specs.toy(8, 3, True), lambda: specs.plain_default(8, 3),
+      lambda: specs.no_bits(8, 3), lambda: specs.shift_relu(8, 3)]
+
+
+@pytest.mark.parametrize("sp", [0, 1])
+@pytest.mark.parametrize("mk", XM)
+def test_xmul_reconstruct_exhaustive_n8(orc, mk, sp):
+    """y * x with x = xhat - r_in opens one element instead of two; the gate still reconstructs to G(x) for
+    every x and r, with both constructions."""
+    spec = specs.input_masked_mul(specs.shared_prefix(mk()) if sp else mk())
+    N = 1 << spec.n
+    _check_all_r(orc, spec, list(range(0, N, 5)) + [N - 1]) if sp else _check_plain_only(orc, spec, list(range(0, N, 5)) + [N - 1])
+
+
+def _check_plain_only(orc, spec, xs, seed=17):
+    P = orc.Program(spec)
+    n = spec.n
+    N = 1 << n
+    na = P.shape["n_out_a"]
+    r_out = (np.arange(N * max(1, na), dtype=np.uint64) * np.uint64(40503)) & mask_of(n)
+    r_in, (k0, k1) = all_r_keys(P, n, seed, r_out)
+    for x in xs:
+        xv = np.full(N, x, dtype=np.uint64)
+        out = P.run_gate(k0, k1, (xv + r_in) & mask_of(n))
+        ye, ze = P.plain_G(xv, r_in)
+        if spec.mask_output:
+            ye = (ye + r_out.reshape(-1, N)[: ye.shape[0]]) & mask_of(n)
+        assert np.array_equal((out["y"][0] + out["y"][1]) & mask_of(n), ye), (spec.name, x)
+        if P.shape["n_out_b"]:
+            assert np.array_equal(out["z"][0] ^ out["z"][1], pack_bits(ze)), (spec.name, x)
+
+
+def test_xmul_online_bytes(orc):
+    """Online bytes per element per party: n/8 (xhat) + n/8 per product with x (2n/8 for a general Beaver)."""
+    g0, g1 = orc.Program(specs.gelu()), orc.Program(specs.input_masked_mul(specs.gelu()))
+    assert g0.online_bits() == 64 + 2 * 2 * 64 and g1.online_bits() == 64 + 2 * 64
+    assert g1.post_msg_bytes(1024, 0) * 2 == g0.post_msg_bytes(1024, 0)
+    assert g0.key_bytes(4096) - g1.key_bytes(4096) == 2 * 8 * 4096          # (b, c) instead of (a, b, c) per product

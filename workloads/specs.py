@@ -43,7 +43,7 @@ class OpSpec:
     out_frac: int = 0      # fractional bits of the arithmetic outputs (metadata for decode)
     domain: tuple = None   # real interval on which the spline error is stated
     func: object = None    # real function approximated (metadata for tests)
-    variant: int = 0       # 0: Protocol-3 construction (one key per query / boundary); 1: single-key shared-prefix (DESIGN 9)
+    variant: int = 0       # bit 0: 0 = Protocol-3 construction, 1 = single-key shared-prefix (DESIGN 9); bit 1: input-masked products (DESIGN 10)
 
     @property
     def m(self):
@@ -337,6 +337,12 @@ def shared_prefix(spec):
     """The same operator compiled with the single-key, multi-point construction."""
     import dataclasses
     return dataclasses.replace(spec, variant=1, name=spec.name + "_sp")
+
+
+def input_masked_mul(spec):
+    """The same operator with variant bit 1: products with the gate input x open ONE ring element."""
+    import dataclasses
+    return dataclasses.replace(spec, variant=spec.variant | 2, name=spec.name + "_xm")
 
 
 CONFIGS = {
