@@ -359,6 +359,7 @@ def main():
             "keygen_elems_per_s": world * count / (per_step(t_gen) * 1e-3),
             "ms_breakdown": {"keygen": per_step(t_gen), "keygen_bit": per_step(t_genbit), "keygen_vec": per_step(t_genvec), "eval_cmp_x2": per_step(t_cmp), "eval_lut_x2": per_step(t_lut), "post_fused": per_step(t_post)},
             "key_bytes_per_elem_per_party": key_b, "online_bytes_per_elem_per_party": P.online_bits() / 8,
+            "online_bytes_per_elem_per_party_input_masked_mul": F.Program(specs.input_masked_mul(spec)).online_bits() / 8,
             "aes_per_elem": {"eval_one_party": aes_eval, "keygen_both": aes_gen},
             "aes_rate_gaes": {"eval": 2 * aes_eval * count / ((per_step(t_cmp) + per_step(t_lut)) * 1e-3) / 1e9,
                               "keygen": aes_gen * count / (per_step(t_gen) * 1e-3) / 1e9},

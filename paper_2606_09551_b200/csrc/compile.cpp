@@ -33,6 +33,7 @@ private:
     std::vector<int> node_val;                   // memo: bit node -> SSA bit value
     std::vector<int> calpha_val;                 // memo: C_{alpha_i} -> SSA bit value
     bool failed = false;
+    int x_value = -1;                            // SSA value of x (Protocol 2)
 
     int view_index(int k, uint64_t c) {
         for (size_t v = 0; v < views.size(); ++v)
@@ -94,7 +95,9 @@ private:
     int a_mul(int a, int b) {                     // one Beaver multiplication, 2 opened ring elements
         int rd = std::max(a_ready[a], a_ready[b]);
         int d = fresh_a(rd + 1);
-        Ins &i = push(I_A_MUL, d, a, b, 0);
+        const bool ax = a == x_value, bx = b == x_value;
+        const bool xm = P.xmul && ax != bx;       // variant bit 1: y * x with x = xhat - r_in, 1 opened element (DESIGN 10)
+        Ins &i = xm ? push(I_A_MULX, d, ax ? b : a, 0, 0) : push(I_A_MUL, d, a, b, 0);
         i.gate = (uint16_t)P.MA++; i.round = (uint8_t)rd;
         if (rd >= kMaxRounds) failed = true;
         return d;
@@ -306,7 +309,8 @@ bool Lowering::run() {
     calpha_val.assign(P.m + 1, -1);
     const uint32_t per_poly = P.d + 1, n_coeff = P.r * per_poly;
 
-    int xval = fresh_a(0); push(I_A_X, xval, 0, 0, 0);                       // Protocol 2
+    int xval = fresh_a(0); push(I_A_X, xval, 0, 0, 0);
+    x_value = xval;                       // Protocol 2
     std::vector<int> cval(P.p);
     for (int w = 0; w < P.p; ++w) {
         cval[w] = fresh_a(0);
@@ -349,13 +353,21 @@ bool Lowering::finish() {
     P.rounds = 0;
     int mulpos[kMaxRounds] = {0}, bitpos[kMaxRounds] = {0};
     for (Ins &i : P.ins) {
-        if (i.op == I_A_MUL) { i.pos = (uint16_t)mulpos[i.round]++; P.rounds = std::max(P.rounds, i.round + 1); }
+        if (i.op == I_A_MUL || i.op == I_A_MULX) {
+            const int arrs = i.op == I_A_MUL ? 2 : 1;
+            i.pos = (uint16_t)mulpos[i.round]; mulpos[i.round] += arrs;           // pos = first opened array of the gate in its round
+            P.round_mul[i.round]++;
+            P.ma_is_x[i.gate] = i.op == I_A_MULX;
+            P.rounds = std::max(P.rounds, i.round + 1);
+        }
         else if (i.op == I_B_AND) { i.pos = (uint16_t)bitpos[i.round]; bitpos[i.round] += 2; P.rounds = std::max(P.rounds, i.round + 1); }
         else if (i.op == I_A_B2A) { i.pos = (uint16_t)bitpos[i.round]; bitpos[i.round] += 1; P.rounds = std::max(P.rounds, i.round + 1); }
     }
-    if (P.rounds > kMaxRounds || P.MB > 64 || P.GMIX > 64) return false;
+    if (P.rounds > kMaxRounds || P.MB > 64 || P.GMIX > 64 || P.MA > 64) return false;
+    for (int g = 0; g < P.MA; ++g) P.ma_word[g + 1] = P.ma_word[g] + (P.ma_is_x[g] ? 2 : 3);
+    for (Ins &i : P.ins) if (i.op == I_A_MUL || i.op == I_A_MULX) i.imm = (uint64_t)P.ma_word[i.gate];
     for (int q = 0; q < kMaxRounds; ++q) {
-        P.round_mul[q] = mulpos[q]; P.round_bits[q] = bitpos[q];
+        P.round_arr[q] = mulpos[q]; P.round_bits[q] = bitpos[q];
         if (bitpos[q] > 64) return false;
     }
     // last use of every SSA value
@@ -367,7 +379,7 @@ bool Lowering::finish() {
         case I_B_NOT: case I_B_ANDPUB: case I_B_OUT: case I_A_B2A: a_is_B = true; break;
         case I_B_XOR: case I_B_AND: a_is_B = b_is_B = true; break;
         case I_A_ADD: case I_A_SUB: case I_A_MUL: a_is_A = b_is_A = true; break;
-        case I_A_MULC: case I_A_OUT: a_is_A = true; break;
+        case I_A_MULC: case I_A_OUT: case I_A_MULX: a_is_A = true; break;
         default: break;
         }
     };
@@ -456,7 +468,8 @@ int compile_program(const fusefss_spec *S, Program **out) {
     // M = min(m+1, 2^n)  (Protocol 3 line 2)
     P.M = (S->n >= 7 || (uint64_t)(S->m + 1) < (1ull << S->n)) ? (int)S->m + 1 : (int)(1ull << S->n);
     P.has_lut = S->m > 1;                         // a single interval needs no lookup
-    P.variant = S->variant ? 1 : 0;
+    P.variant = S->variant & 1;
+    P.xmul = (S->variant >> 1) & 1;
     if (P.variant) P.M = (int)S->m;               // variant 1: no translated partition, no wrap / dummy split
     P.n_out_a = (int)S->n_out_a; P.n_out_b = (int)S->n_out_b;
     if (P.n_out_a > kMaxP || P.n_out_b > 64) { delete holder; return FUSEFSS_E_SPEC; }
@@ -513,7 +526,7 @@ void compute_layout(const Program &P, size_t count, Layout *L) {
     L->rout = off;     if (P.mask_output) off += (size_t)P.n_out_a * L->s8;
     L->ka = off;       off += P.kappa_a.size() * L->s8;
     L->kb = off;       if (P.n_kb > 0) off += L->s8;
-    L->beaver = off;   off += (size_t)3 * P.MA * L->s8;
+    L->beaver = off;   off += (size_t)P.ma_word[P.MA] * L->s8;
     L->andt = off;     if (P.MB > 0) off += 3 * L->s8;
     L->b2a_bits = off; if (P.GMIX > 0) off += L->s8;
     L->b2a_a = off;    off += (size_t)P.GMIX * L->s8;
@@ -522,7 +535,7 @@ void compute_layout(const Program &P, size_t count, Layout *L) {
 
 size_t post_msg_bytes(const Program &P, size_t count, int round) {
     if (round < 0 || round >= P.rounds) return 0;
-    return round_up_256(count * 8) * ((size_t)2 * P.round_mul[round] + (P.round_bits[round] ? 1 : 0));
+    return round_up_256(count * 8) * ((size_t)P.round_arr[round] + (P.round_bits[round] ? 1 : 0));
 }
 
 }  // namespace fsk

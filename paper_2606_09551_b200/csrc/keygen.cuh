@@ -314,6 +314,7 @@ struct GenMiscArgs {
     size_t count, s8, lut_c, rin, rout, ka, kb, beaver, andt, b2a_bits, b2a_a;
     uint64_t first_elem, mask;
     int n, m, M, p, has_lut, mask_output, n_out_a, n_ka, n_kb_spec, n_carry, T, MA, MB, GMIX;
+    uint64_t ma_is_x;          // bit i: arithmetic gate i is a product with the gate input (material (b, c = b r_in), DESIGN 10)
     RoundKeys rk;
     uint8_t ka_kind[8], ka_arg[8], kb_kind[64], kb_arg[64];
     GenAtomDev atom[kMaxAtoms];
@@ -376,6 +377,7 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_misc(const __grid_consta
             const uint64_t s0 = lo & (n_kb >= 64 ? ~0ull : ((1ull << n_kb) - 1ull));
             put(a.kb, s0, kbits ^ s0);
         }
+        int bv_word = 0;
         for (int i = 0; i < a.MA; ++i) {                                   // Beaver triple (a, b, c = ab)
             dealer_rand(tl, a.rk, ge, SLOT_BV_AB + i, lo, hi);
             const uint64_t ta = lo & a.mask, tb = hi & a.mask, tc = (ta * tb) & a.mask;
@@ -383,7 +385,15 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_misc(const __grid_consta
             const uint64_t a0 = lo & a.mask, b0 = hi & a.mask;
             dealer_rand(tl, a.rk, ge, SLOT_BV_C0 + i, lo, hi);
             const uint64_t c0 = lo & a.mask;
-            const size_t o = a.beaver + (size_t)3 * i * a.s8;
+            const size_t o = a.beaver + (size_t)bv_word * a.s8;
+            if ((a.ma_is_x >> i) & 1ull) {
+                const uint64_t cx = (tb * r) & a.mask;
+                put(o, b0, (tb - b0) & a.mask);
+                put(o + a.s8, c0, (cx - c0) & a.mask);
+                bv_word += 2;
+                continue;
+            }
+            bv_word += 3;
             put(o, a0, (ta - a0) & a.mask);
             put(o + a.s8, b0, (tb - b0) & a.mask);
             put(o + 2 * a.s8, c0, (tc - c0) & a.mask);

@@ -261,7 +261,9 @@ size_t fusefss_post_msg_bytes(const fusefss_program *prog, size_t count, int rou
 size_t fusefss_online_bits(const fusefss_program *prog) {
     const Program *P = prog_of(prog);
     if (!P) return 0;
-    return (size_t)P->n + (size_t)2 * P->n * P->MA + (size_t)2 * P->MB + (size_t)P->GMIX +
+    size_t arrs = 0;
+    for (int q = 0; q < P->rounds; ++q) arrs += (size_t)P->round_arr[q];
+    return (size_t)P->n + (size_t)P->n * arrs + (size_t)2 * P->MB + (size_t)P->GMIX +
            (P->mask_output ? (size_t)P->n * P->n_out_a : 0);
 }
 
@@ -402,6 +404,7 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
         a.n = (int)P->n; a.m = (int)P->m; a.M = P->M; a.p = P->p; a.has_lut = P->variant ? 0 : P->has_lut; a.mask_output = (int)P->mask_output;
         a.n_out_a = P->n_out_a; a.n_ka = (int)P->kappa_a.size(); a.n_kb_spec = (int)P->kappa_b.size(); a.n_carry = P->n_carry;
         a.T = P->variant ? 0 : P->T; a.MA = P->MA; a.MB = P->MB; a.GMIX = P->GMIX; a.rk = rk;
+        for (int g = 0; g < P->MA; ++g) if (P->ma_is_x[g]) a.ma_is_x |= 1ull << g;
         if (a.n_ka > 8) return FUSEFSS_E_SPEC;
         for (int t = 0; t < a.n_ka; ++t) { a.ka_kind[t] = P->kappa_a[t].kind; a.ka_arg[t] = P->kappa_a[t].arg; }
         for (int t = 0; t < a.n_kb_spec; ++t) { a.kb_kind[t] = P->kappa_b[t].kind; a.kb_arg[t] = P->kappa_b[t].arg; }
@@ -507,7 +510,7 @@ int fusefss_post(int party, const fusefss_program *prog, const void *key_dev, co
     a.round_off[0] = 0;
     for (int q = 0; q < kMaxRounds; ++q) {
         a.round_off[q + 1] = a.round_off[q] + post_msg_bytes(*P, count, q);
-        a.round_mul[q] = P->round_mul[q]; a.round_bits[q] = P->round_bits[q];
+        a.round_arr[q] = P->round_arr[q]; a.round_bits[q] = P->round_bits[q];
     }
     return launch(k_post_round, (int)((count + 255) / 256), 256, 0, (cudaStream_t)stream, a);
 }

@@ -20,7 +20,7 @@ struct PostArgs {
     size_t count; uint64_t mask;
     PostKeyOff k;
     size_t round_off[kMaxRounds + 1];
-    int round_mul[kMaxRounds];
+    int round_arr[kMaxRounds];     // ring-element arrays opened in the round (the bit word follows them)
     int round_bits[kMaxRounds];
 };
 
@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(256) k_post_round(const __grid_constant__ Post
             if (q == a.round) outbits |= (dm << o.pos) | (em << (o.pos + 1));
             uint64_t res = 0;
             if (q < a.round) {
-                const uint64_t other = kld(a.msg_in, a.round_off[q] + (size_t)2 * a.round_mul[q] * a.k.s8, e);
+                const uint64_t other = kld(a.msg_in, a.round_off[q] + (size_t)a.round_arr[q] * a.k.s8, e);
                 const uint64_t dd = dm ^ ((other >> o.pos) & 1), ee = em ^ ((other >> (o.pos + 1)) & 1);
                 res = (p0 ? (dd & ee) : 0) ^ (dd & tb) ^ (ee & ta) ^ tc;
             }
@@ -79,11 +79,11 @@ __global__ void __launch_bounds__(256) k_post_round(const __grid_constant__ Post
             }
             break;
         case I_A_MUL: {
-            const size_t to = a.k.beaver + (size_t)3 * o.gate * a.k.s8;
+            const size_t to = a.k.beaver + (size_t)o.imm * a.k.s8;
             const uint64_t ta = kld(a.key, to, e), tb = kld(a.key, to + a.k.s8, e), tc = kld(a.key, to + 2 * a.k.s8, e);
             const uint64_t em = (A[o.a] - ta) & mask, fm = (A[o.b] - tb) & mask;
             const int q = o.round;
-            const size_t mo = a.round_off[q] + (size_t)2 * o.pos * a.k.s8;
+            const size_t mo = a.round_off[q] + (size_t)o.pos * a.k.s8;
             if (q == a.round) {
                 reinterpret_cast<uint64_t *>(a.msg_out + mo)[e] = em;
                 reinterpret_cast<uint64_t *>(a.msg_out + mo + a.k.s8)[e] = fm;
@@ -95,6 +95,20 @@ __global__ void __launch_bounds__(256) k_post_round(const __grid_constant__ Post
             }
             A[o.dst] = res;
             break; }
+        case I_A_MULX: {     // y * x, x = xhat - r_in: material (b, c = b r_in), open f = y - b; [yx]_b = xhat [y]_b - f [r_in]_b - [c]_b
+            const size_t to = a.k.beaver + (size_t)o.imm * a.k.s8;
+            const uint64_t tb = kld(a.key, to, e), tc = kld(a.key, to + a.k.s8, e);
+            const uint64_t fm = (A[o.a] - tb) & mask;
+            const int q = o.round;
+            const size_t mo = a.round_off[q] + (size_t)o.pos * a.k.s8;
+            if (q == a.round) reinterpret_cast<uint64_t *>(a.msg_out + mo)[e] = fm;
+            uint64_t res = 0;
+            if (q < a.round) {
+                const uint64_t F = (fm + kld(a.msg_in, mo, e)) & mask;
+                res = (xh * A[o.a] - F * kld(a.key, a.k.rin, e) - tc) & mask;
+            }
+            A[o.dst] = res;
+            break; }
         case I_A_B2A: {
             const uint64_t rb = (kld(a.key, a.k.b2a_bits, e) >> o.gate) & 1, ra = kld(a.key, a.k.b2a_a + (size_t)o.gate * a.k.s8, e);
             const uint64_t mm = getb(o.a) ^ rb;
@@ -102,7 +116,7 @@ __global__ void __launch_bounds__(256) k_post_round(const __grid_constant__ Post
             if (q == a.round) outbits |= mm << o.pos;
             uint64_t res = 0;
             if (q < a.round) {
-                const uint64_t other = kld(a.msg_in, a.round_off[q] + (size_t)2 * a.round_mul[q] * a.k.s8, e);
+                const uint64_t other = kld(a.msg_in, a.round_off[q] + (size_t)a.round_arr[q] * a.k.s8, e);
                 const uint64_t mu = mm ^ ((other >> o.pos) & 1);
                 res = ((p0 ? mu : 0) + ra - 2 * mu * ra) & mask;
             }
@@ -112,7 +126,7 @@ __global__ void __launch_bounds__(256) k_post_round(const __grid_constant__ Post
         }
     }
     if (a.round < a.rounds && a.round_bits[a.round])
-        reinterpret_cast<uint64_t *>(a.msg_out + a.round_off[a.round] + (size_t)2 * a.round_mul[a.round] * a.k.s8)[e] = outbits;
+        reinterpret_cast<uint64_t *>(a.msg_out + a.round_off[a.round] + (size_t)a.round_arr[a.round] * a.k.s8)[e] = outbits;
     if (a.round == a.rounds && a.n_out_b > 0) a.z_out[e] = zword;
 }
 
@@ -174,7 +188,7 @@ __global__ void __launch_bounds__(256) k_post_fused(const __grid_constant__ Post
             }
             break;
         case I_A_MUL: {
-            const size_t to = a.k.beaver + (size_t)3 * o.gate * a.k.s8;
+            const size_t to = a.k.beaver + (size_t)o.imm * a.k.s8;
             uint64_t ta[2], tb[2], tc[2], em[2], fm[2];
 #pragma unroll
             for (int b = 0; b < 2; ++b) {
@@ -184,6 +198,15 @@ __global__ void __launch_bounds__(256) k_post_fused(const __grid_constant__ Post
             const uint64_t E = (em[0] + em[1]) & mask, F = (fm[0] + fm[1]) & mask;
             A[0][o.dst] = (E * F + E * tb[0] + F * ta[0] + tc[0]) & mask;
             A[1][o.dst] = (E * tb[1] + F * ta[1] + tc[1]) & mask;
+            break; }
+        case I_A_MULX: {
+            const size_t to = a.k.beaver + (size_t)o.imm * a.k.s8;
+            uint64_t tb[2], tc[2], fm[2];
+#pragma unroll
+            for (int b = 0; b < 2; ++b) { tb[b] = kld(a.key[b], to, e); tc[b] = kld(a.key[b], to + a.k.s8, e); fm[b] = (A[b][o.a] - tb[b]) & mask; }
+            const uint64_t F = (fm[0] + fm[1]) & mask;
+#pragma unroll
+            for (int b = 0; b < 2; ++b) A[b][o.dst] = (xh * A[b][o.a] - F * kld(a.key[b], a.k.rin, e) - tc[b]) & mask;
             break; }
         case I_A_B2A: {
             uint64_t rb[2], ra[2], mm[2];

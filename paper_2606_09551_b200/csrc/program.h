@@ -29,7 +29,7 @@ struct Atom {
 // (`gate`), their round and their position inside that round's message (`pos`).
 enum : uint8_t {
     I_B_CONST = 1, I_B_ATOM, I_B_KAPPA, I_B_XHAT, I_B_NOT, I_B_XOR, I_B_AND, I_B_ANDPUB, I_B_OUT,
-    I_A_CONST, I_A_X, I_A_COEFF, I_A_KAPPA, I_A_XHAT_SHR, I_A_ADD, I_A_SUB, I_A_MULC, I_A_MUL, I_A_B2A, I_A_OUT
+    I_A_CONST, I_A_X, I_A_COEFF, I_A_KAPPA, I_A_XHAT_SHR, I_A_ADD, I_A_SUB, I_A_MULC, I_A_MUL, I_A_MULX, I_A_B2A, I_A_OUT
 };
 struct Ins {
     uint8_t op;
@@ -38,7 +38,7 @@ struct Ins {
     uint16_t gate;      // Beaver / AND / B2A gate number
     uint16_t pos;       // Beaver: pair index inside the round; AND/B2A: first bit position inside the round's bit word
     uint32_t pad;
-    uint64_t imm;
+    uint64_t imm;       // constants; for I_A_MUL / I_A_MULX: first word of the gate's material inside the Beaver section
 };
 static_assert(sizeof(Ins) == 24, "Ins is uploaded to the device as-is");
 
@@ -84,6 +84,10 @@ struct Program {
     std::vector<Ins> ins;
     int n_areg = 0, n_breg = 0;
     int round_mul[kMaxRounds] = {0}, round_bits[kMaxRounds] = {0};
+    // variant bit 1 (DESIGN 10): a product with the gate input x opens one ring element and needs (b, c = b r_in)
+    uint32_t xmul = 0;
+    int round_arr[kMaxRounds] = {0};      // ring-element arrays opened per round: 2 per Beaver, 1 per x-product
+    int ma_is_x[64] = {0}, ma_word[65] = {0};
     // payload table v[i][w], i < m, w < p (coefficients poly-major, high degree first, then aux), masked
     std::vector<uint64_t> payload;
     // device copy of the small tables (uploaded lazily by the launchers)

@@ -35,6 +35,7 @@ ALL = [("relu16", lambda: specs.relu(16, 8)), ("gelu", specs.gelu), ("nexp", spe
        ("plain", specs.plain_default), ("single", specs.single_interval), ("nobits", specs.no_bits),
        ("full", specs.full_partition), ("shift_relu8", lambda: specs.shift_relu(8, 3))]
 ALL = ALL + [(nm + "_sp", (lambda mk=mk: specs.shared_prefix(mk()))) for nm, mk in ALL]      # variant 1 (DESIGN 9)
+ALL = ALL + [(nm + "_xm", (lambda mk=mk: specs.input_masked_mul(mk()))) for nm, mk in ALL]  # variant bit 1 (DESIGN 10)
 
 
 @pytest.mark.parametrize("name,mk", ALL)

@@ -102,7 +102,10 @@ SMALL = [lambda: specs.relu(8, 4), lambda: specs.toy(8, 3), lambda: specs.toy(8,
 SMALL_SP = [(lambda mk=mk: specs.shared_prefix(mk())) for mk in SMALL]
 
 
-@pytest.mark.parametrize("mk", SMALL + SMALL_SP)
+SMALL_XM = [(lambda mk=mk: specs.input_masked_mul(mk())) for mk in SMALL[:4] + SMALL[7:9] + SMALL_SP[:4] + SMALL_SP[7:9]]
+
+
+@pytest.mark.parametrize("mk", SMALL + SMALL_SP + SMALL_XM)
 @pytest.mark.parametrize("force_g", ["", "1"])
 def test_small_rings_all_masks(F, orc, mk, force_g, monkeypatch):
     """Every mask r (both Protocol 3 branches, incl. beta_0 = 0 and the dummy split) at n <= 8; a ragged count."""
@@ -126,16 +129,19 @@ CONFIGS = [("relu16", 4096), ("gelu", 700), ("nexp", 330), ("recip", 130), ("shi
            ("silu", 131)]
 
 
-@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])
 @pytest.mark.parametrize("name,count", CONFIGS)
 def test_config_parity(F, orc, name, count, variant):
     """BASELINE.json's configs on their seeded synthetic inputs (workloads/tensors.py), several 32-element tiles
     and a ragged tail; config 1 at its full size.  variant 1 = the single-key shared-prefix construction, whose
     kernel shares tree prefixes between nearby points while the oracle walks every point from the root."""
     spec = specs.CONFIGS[name]()
-    if variant:
+    if variant & 1:
         spec = specs.shared_prefix(spec)
         count = min(4096, count * 4)
+    if variant & 2:
+        spec = specs.input_masked_mul(spec)                 # one opening per product with x (DESIGN 10)
+        count = max(33, count // 4)
     inp = tensors.inputs(name, spec, count=count, seed=0)
     _parity(F, orc, spec, inp["x"], inp["r_in"], inp["r_out"], seed=0)
 
