@@ -126,6 +126,9 @@ def measure_shared_prefix(F, torch, name, base_spec, inp, rank, world, steps, wa
     P = F.Program(spec)
     sh, cost = P.shape, P.cost()
     count = int(inp["xhat"].size)
+    free_b, _ = torch.cuda.mem_get_info()
+    if 2 * P.key_bytes(count) + 8 * count * (8 + 2 * sh["p"]) > 0.85 * free_b:
+        return {"skipped": "variant-1 keys of the whole tensor do not fit resident"}
     dev = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.int64)).cuda()
     r_in, r_out, xhat = dev(inp["r_in"]), dev(inp["r_out"]), dev(inp["xhat"])
     k0, k1 = P.alloc_keys(count)
@@ -382,8 +385,8 @@ def main():
         line["prg_probe"] = {"error": str(exc)}
 
     # ---- the same workload with the single-key shared-prefix construction (variant 1) ------------------
-    if not args.no_sp and chunk == count:
-        del k0, k1
+    if not args.no_sp:
+        del k0, k1, coeff, youts, zouts
         torch.cuda.empty_cache()
         line["shared_prefix"] = measure_shared_prefix(F, torch, name, spec, inp, rank, world, args.steps, args.warmup, barrier,
                                                       lambda v: (float(_allmax(v))))
