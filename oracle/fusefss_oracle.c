@@ -531,6 +531,7 @@ typedef struct { int k; u64 c; int is_theta; u64 beta; int carry_idx; } atom_t;
 enum {
     C_B_CONST = 1, C_B_ATOM, C_B_KAPPA, C_B_XHAT, C_B_NOT, C_B_XOR, C_B_AND, C_B_ANDPUB, C_B_OUT,
     C_A_CONST, C_A_X, C_A_COEFF, C_A_KAPPA, C_A_XHAT_SHR, C_A_ADD, C_A_SUB, C_A_MULC, C_A_MUL, C_A_B2A, C_A_OUT,
+    C_A_MULXH,    /* variant bit 2: share times the PUBLIC masked input xhat, local (DESIGN 11) */
     C_A_MULX      /* variant bit 1: product with the gate input x = xhat - r_in, one opening (DESIGN 10) */
 };
 typedef struct { int op, dst, a, b, idx, round; u64 imm; } cop_t;
@@ -551,6 +552,7 @@ typedef struct orc_prog {
     /* per round message shape */
     int r_nmul[16], r_nbits[16];
     int xmul;                         /* variant bit 1 */
+    int xpoly;                        /* variant bit 2: payload = coefficients of P_i(X - r_in), Horner in the public xhat */
     int r_narr[16];                   /* ring-element arrays opened per round: 2 per Beaver, 1 per x-product */
     int ma_is_x[64], ma_word[65];     /* per arithmetic gate: kind, first word of its material in the key */
     /* lowering memo */
@@ -754,6 +756,7 @@ orc_prog *orc_compile(const orc_spec *S0)
     P->has_lut = P->m > 1;                               /* single interval: lookup omitted */
     P->variant = (int)(S->variant & 1);
     P->xmul = (int)((S->variant >> 1) & 1);
+    P->xpoly = (int)((S->variant >> 2) & 1) && S->d >= 1 && P->m > 1;
     if (P->variant) P->M = P->m;                         /* no translated partition, hence no wrap/dummy split */
     for (int i = 0; i < 4096; i++) P->node_reg[i] = -1;
     for (int i = 0; i <= MMAX; i++) P->calpha_reg[i] = -1;
@@ -805,6 +808,14 @@ orc_prog *orc_compile(const orc_spec *S0)
     for (u32 j = 0; j < S->r; j++) yreg[j] = creg[j * (S->d + 1)];
     for (u32 k = 1; k <= S->d; k++)                      /* Horner: acc = acc*x + c_k, one round per step */
         for (u32 j = 0; j < S->r; j++) {
+            if (P->xpoly) {                              /* y = (..(c'_d xhat + c'_{d-1}) xhat ..) + c'_0: no interaction (DESIGN 11) */
+                int pr = newa(P, P->ardy[yreg[j]]);
+                emit(P, C_A_MULXH, pr, yreg[j], 0, 0);
+                int sm = newa(P, P->ardy[yreg[j]]);
+                emit(P, C_A_ADD, sm, pr, creg[j * (S->d + 1) + k], 0);
+                yreg[j] = sm;
+                continue;
+            }
             int rd = imax(P->ardy[yreg[j]], P->ardy[xreg]);
             int prod = newa(P, rd + 1);
             int i = emit(P, P->xmul ? C_A_MULX : C_A_MUL, prod, yreg[j], xreg, 0);
@@ -901,6 +912,27 @@ void orc_shape(const orc_prog *P, int *out, int *ks)
 void orc_atom(const orc_prog *P, int t, u64 *out)
 {
     out[0] = (u64)P->atoms[t].k; out[1] = P->atoms[t].c; out[2] = (u64)P->atoms[t].is_theta; out[3] = P->atoms[t].beta;
+}
+
+/* variant bit 2 (DESIGN 11): coefficient of X^j of P(X - r), P = sum_k c_k X^k:
+ *   c'_j = sum_{k >= j} c_k C(k, j) (-r)^{k-j}   (binomial theorem), so that P(x) = sum_j c'_j xhat^j with xhat = x + r. */
+static u64 binom(int k, int j)
+{
+    u64 v = 1;
+    for (int i = 1; i <= j; i++) v = v * (u64)(k - j + i) / (u64)i;
+    return v;
+}
+static u64 shifted_coeff(const orc_spec *S, int i, int q, int j, u64 r, u64 mask)
+{
+    int d = (int)S->d;
+    const u64 *c = S->coeff + ((size_t)i * S->r + q) * (d + 1);           /* high degree first: c_k = c[d - k] */
+    u64 acc = 0;
+    for (int k = j; k <= d; k++) {
+        u64 pw = 1;
+        for (int t = 0; t < k - j; t++) pw = (pw * ((u64)0 - r)) & mask;
+        acc = (acc + c[d - k] * binom(k, j) * pw) & mask;
+    }
+    return acc;
 }
 
 /* ------------------------------------------------------------------------- */
@@ -1121,7 +1153,9 @@ void orc_keygen(const orc_prog *P, const u64 *r_in, const u64 *r_out, u64 seed, 
             u64 v[MMAX + 1][PMAX];
             for (int j = 0; j < M; j++) {                               /* payloads v_j (lines 31-33) */
                 int w = 0;
-                for (u32 q = 0; q < S->r * (S->d + 1); q++) v[j][w++] = S->coeff[(size_t)ord[j] * S->r * (S->d + 1) + q] & mask;
+                for (u32 q = 0; q < S->r * (S->d + 1); q++)
+                    v[j][w++] = P->xpoly ? shifted_coeff(S, ord[j], (int)(q / (S->d + 1)), (int)(S->d - q % (S->d + 1)), r, mask)
+                                         : S->coeff[(size_t)ord[j] * S->r * (S->d + 1) + q] & mask;
                 for (u32 q = 0; q < S->p_aux; q++) v[j][w++] = S->aux[(size_t)ord[j] * S->p_aux + q] & mask;
             }
             for (int w = 0; w < p; w++) {                               /* constant term v_{M-1}, additively split */
@@ -1401,6 +1435,7 @@ void orc_post(int party, const orc_prog *P, const u8 *key, const u64 *xhat, cons
             case C_A_ADD: A[o->dst] = (A[o->a] + A[o->b]) & mask; break;
             case C_A_SUB: A[o->dst] = (A[o->a] - A[o->b]) & mask; break;
             case C_A_MULC: A[o->dst] = (A[o->a] * o->imm) & mask; break;
+            case C_A_MULXH: A[o->dst] = (A[o->a] * xh) & mask; break;
             case C_A_OUT: {
                 u64 v = A[o->a];
                 if (P->S.mask_output) v = (v + ld8(key, L.rout + (size_t)o->dst * L.s8, e)) & mask;   /* yhat share */

@@ -143,3 +143,22 @@ def test_xmul_online_bytes(orc):
     assert g0.online_bits() == 64 + 2 * 2 * 64 and g1.online_bits() == 64 + 2 * 64
     assert g1.post_msg_bytes(1024, 0) * 2 == g0.post_msg_bytes(1024, 0)
     assert g0.key_bytes(4096) - g1.key_bytes(4096) == 2 * 8 * 4096          # (b, c) instead of (a, b, c) per product
+
+
+# ---- variant bit 2: payload = coefficients of P_i(X - r_in), Horner in the public xhat -------
+XP = [lambda: specs.toy(8, 3), lambda: specs.toy(8, 3, True), lambda: specs.plain_default(8, 3), lambda: specs.no_bits(8, 3)]
+
+
+@pytest.mark.parametrize("sp", [0, 1])
+@pytest.mark.parametrize("mk", XP)
+def test_xpoly_reconstruct_exhaustive_n8(orc, mk, sp):
+    spec = specs.public_point_horner(specs.shared_prefix(mk()) if sp else mk())
+    N = 1 << spec.n
+    _check_plain_only(orc, spec, list(range(0, N, 5)) + [N - 1])
+
+
+def test_xpoly_shape(orc):
+    """No Beaver multiplication and no round is left for a pure spline: online = the xhat opening only."""
+    for mk in (specs.gelu, specs.silu, specs.nexp, specs.rsqrt):
+        P = orc.Program(specs.public_point_horner(mk()))
+        assert (P.shape["M_A"], P.shape["rounds"]) == (0, 0) and P.online_bits() == 64

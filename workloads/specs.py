@@ -345,6 +345,13 @@ def input_masked_mul(spec):
     return dataclasses.replace(spec, variant=spec.variant | 2, name=spec.name + "_xm")
 
 
+def public_point_horner(spec):
+    """Variant bit 2: the lookup returns the coefficients of P_i(X - r_in), Horner runs in the public xhat -- zero
+    Beaver rounds for the spline."""
+    import dataclasses
+    return dataclasses.replace(spec, variant=spec.variant | 4, name=spec.name + "_xp")
+
+
 CONFIGS = {
     "relu16": lambda: relu(16, 8),
     "gelu": gelu,
