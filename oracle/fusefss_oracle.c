@@ -1001,7 +1001,7 @@ typedef struct {
     size_t s16, s8;
     size_t bt_root[TMAX], bt_cw[TMAX], bt_vb[TMAX];
     size_t lut_c, vt_root[MMAX], vt_lvl[MMAX], vt_fin[MMAX], lvl_stride;
-    size_t rin, rout, ka, kb, beaver, andt, b2a_bits, b2a_a, total;
+    size_t rin, rout, ka, rpow, kb, beaver, andt, b2a_bits, b2a_a, total;
 } layout_t;
 static size_t rup256(size_t x) { return (x + 255) & ~(size_t)255; }
 static void layout(const orc_prog *P, size_t count, layout_t *L)
@@ -1011,7 +1011,8 @@ static void layout(const orc_prog *P, size_t count, layout_t *L)
     if (P->variant) {
         /* one tree per view width, in width order: k < n -> bit-DCF arrays (root, k levels, VCW bits);
          * k = n -> vector-DCF arrays with p = 1 (root, n levels of {sCW, VCW}, fin) */
-        L->lvl_stride = L->s16 + L->s8;
+        int pk = P->xpoly ? (int)P->S.d + 1 : 1;          /* payload words of the n-bit key: (1, -r, .., (-r)^d) with bit 2 */
+        L->lvl_stride = L->s16 + (size_t)pk * L->s8;
         for (int w = 0; w < P->n_w; w++) {
             if (P->wk[w] < P->n) {
                 L->bt_root[w] = off; off += L->s16;
@@ -1020,7 +1021,7 @@ static void layout(const orc_prog *P, size_t count, layout_t *L)
             } else {
                 L->vt_root[1] = off; off += L->s16;
                 L->vt_lvl[1] = off; off += L->lvl_stride * (size_t)P->n;
-                L->vt_fin[1] = off; off += L->s8;
+                L->vt_fin[1] = off; off += (size_t)pk * L->s8;
             }
         }
     }
@@ -1041,6 +1042,7 @@ static void layout(const orc_prog *P, size_t count, layout_t *L)
     L->rin = off; off += L->s8;
     L->rout = off; if (P->S.mask_output) off += (size_t)P->n_out_a * L->s8;
     L->ka = off; off += (size_t)P->S.n_kappa_a * L->s8;
+    L->rpow = off; if (P->variant && P->xpoly) off += (size_t)P->S.d * L->s8;     /* [(-r)^t], t = 1..d (DESIGN 11) */
     L->kb = off; if (P->n_kb > 0) off += L->s8;
     L->beaver = off; off += (size_t)P->ma_word[P->MA] * L->s8;
     L->andt = off; if (P->MB > 0) off += 3 * L->s8;
@@ -1056,7 +1058,7 @@ size_t orc_key_bytes(const orc_prog *P, size_t count) { layout_t L; layout(P, co
 /* ------------------------------------------------------------------------- */
 enum {
     SLOT_BT_ROOT = 0x1000, SLOT_VT_ROOT = 0x2000, SLOT_LUT_C = 0x3000, SLOT_RIN = 0x4000, SLOT_ROUT = 0x4100,
-    SLOT_KA = 0x5000, SLOT_KB = 0x5800, SLOT_BV_AB = 0x6000, SLOT_BV_AB0 = 0x6800, SLOT_BV_C0 = 0x7000,
+    SLOT_KA = 0x5000, SLOT_RPOW = 0x5400, SLOT_KB = 0x5800, SLOT_BV_AB = 0x6000, SLOT_BV_AB0 = 0x6800, SLOT_BV_C0 = 0x7000,
     SLOT_AND_AB = 0x8000, SLOT_AND_AB0 = 0x8001, SLOT_AND_C0 = 0x8002, SLOT_B2A = 0x9000, SLOT_B2A_A0 = 0x9100
 };
 static void rnd(const aes_ks *ks, u64 e, u64 slot, u8 out[16])
@@ -1110,18 +1112,25 @@ void orc_keygen(const orc_prog *P, const u64 *r_in, const u64 *r_out, u64 seed, 
                         st8(key[b], L.bt_vb[w], e, bk[b]->vbits);
                     }
                 } else {
-                    u64 one = 1 & mask;
+                    int pk = P->xpoly ? (int)S->d + 1 : 1;
+                    u64 pw[PMAX]; pw[0] = 1 & mask;                      /* payload (1, -r, (-r)^2, ..) */
+                    for (int t = 1; t < pk; t++) pw[t] = (pw[t - 1] * ((u64)0 - r)) & mask;
                     rnd(&ks, ge, SLOT_VT_ROOT + 2, rb); rnd(&ks, ge, SLOT_VT_ROOT + 3, rb1);
-                    dcf_vec_gen(n, 1, mask, r, &one, rb, rb1, vk0, vk1);
+                    dcf_vec_gen(n, pk, mask, r, pw, rb, rb1, vk0, vk1);
                     veckey *vk[2] = { vk0, vk1 };
                     for (int b = 0; b < 2; b++) {
                         st16(key[b], L.vt_root[1], e, vk[b]->root);
                         for (int i = 0; i < n; i++) {
                             size_t lo = L.vt_lvl[1] + (size_t)i * L.lvl_stride;
                             st16(key[b], lo, e, vk[b]->scw[i]);
-                            st8(key[b], lo + L.s16, e, vk[b]->vcw[i][0]);
+                            for (int t = 0; t < pk; t++) st8(key[b], lo + L.s16 + (size_t)t * L.s8, e, vk[b]->vcw[i][t]);
                         }
-                        st8(key[b], L.vt_fin[1], e, vk[b]->fin[0]);
+                        for (int t = 0; t < pk; t++) st8(key[b], L.vt_fin[1] + (size_t)t * L.s8, e, vk[b]->fin[t]);
+                    }
+                    for (int t = 1; t < pk; t++) {                      /* additive shares of (-r)^t */
+                        rnd(&ks, ge, SLOT_RPOW + t, rb);
+                        u64 s0 = le64(rb) & mask;
+                        st8(key0, L.rpow + (size_t)(t - 1) * L.s8, e, s0); st8(key1, L.rpow + (size_t)(t - 1) * L.s8, e, (pw[t] - s0) & mask);
                     }
                 }
             }
@@ -1249,9 +1258,10 @@ static void ld16(const u8 *base, size_t off, size_t e, u8 *v) { memcpy(v, base +
 
 /* variant 1: A[w][j] = Eval_b(key_w, (xhat + delta_j) mod 2^k), every point from the root (plain definition) */
 static void sp_eval_points(int party, const orc_prog *P, const u8 *key, const layout_t *L, size_t e, u64 xh,
-                           bitkey *bk, veckey *vk, u64 A[8][2 * TMAX + 2])
+                           bitkey *bk, veckey *vk, u64 A[8][2 * TMAX + 2], u64 AV[2 * TMAX + 2][PMAX])
 {
     int n = P->n;
+    int pk = P->xpoly ? (int)P->S.d + 1 : 1;
     for (int w = 0; w < P->n_w; w++) {
         int k = P->wk[w];
         u64 km = low_mask(k);
@@ -1265,10 +1275,13 @@ static void sp_eval_points(int party, const orc_prog *P, const u8 *key, const la
             for (int i = 0; i < n; i++) {
                 size_t lo = L->vt_lvl[1] + (size_t)i * L->lvl_stride;
                 ld16(key, lo, e, vk->scw[i]);
-                vk->vcw[i][0] = ld8(key, lo + L->s16, e);
+                for (int t = 0; t < pk; t++) vk->vcw[i][t] = ld8(key, lo + L->s16 + (size_t)t * L->s8, e);
             }
-            vk->fin[0] = ld8(key, L->vt_fin[1], e);
-            for (int j = 0; j < P->w_npts[w]; j++) dcf_vec_eval(party, n, 1, P->mask, vk, (xh + P->w_delta[w][j]) & km, &A[w][j]);
+            for (int t = 0; t < pk; t++) vk->fin[t] = ld8(key, L->vt_fin[1] + (size_t)t * L->s8, e);
+            for (int j = 0; j < P->w_npts[w]; j++) {
+                dcf_vec_eval(party, n, pk, P->mask, vk, (xh + P->w_delta[w][j]) & km, AV[j]);
+                A[w][j] = AV[j][0];                                     /* component 0 = share of I[u_j < r] */
+            }
         }
     }
 }
@@ -1290,11 +1303,12 @@ static void sp_eval(int party, const orc_prog *P, const u8 *key, const u64 *xhat
     layout_t L; layout(P, count, &L);
     bitkey *bk = malloc(sizeof *bk); veckey *vk = malloc(sizeof *vk);
     u64 (*A)[2 * TMAX + 2] = malloc(sizeof(u64) * 8 * (2 * TMAX + 2));
+    u64 (*AV)[PMAX] = malloc(sizeof(u64) * PMAX * (2 * TMAX + 2));
     const orc_spec *S = &P->S;
     u32 nc = S->r * (S->d + 1);
     for (size_t e = 0; e < count; e++) {
         u64 xh = xhat[e] & P->mask;
-        sp_eval_points(party, P, key, &L, e, xh, bk, vk, A);
+        sp_eval_points(party, P, key, &L, e, xh, bk, vk, A, AV);
         if (bits_out) {
             u64 word = 0;
             for (int t = 0; t < P->T; t++) word |= (sp_atom_share(party, P, t, xh, A) & 1) << t;   /* LSB of an additive share of a bit = XOR share */
@@ -1302,7 +1316,31 @@ static void sp_eval(int party, const orc_prog *P, const u8 *key, const u64 *xhat
         }
         if (coeff_out && P->has_lut) {
             /* v_{i*} = v_{m-1} + sum_{i=1}^{m-1} (v_{i-1} - v_i) I[x < alpha_i]  (Lemma D.1 telescoped); v_i public */
-            for (int wd = 0; wd < P->p; wd++) {
+            for (int wd = 0; wd < P->p && P->xpoly; wd++) {
+                /* DESIGN 11: coefficient of xhat^j of P_{i*}(xhat - r):  c'_j = sum_t sum_i J_i (-r)^t c_{i,j+t} C(j+t, j), with
+                 * [I[x<alpha_i] (-r)^t] = e_i [(-r)^t] - B[t] + A_i[t]  (B, A_i = the vector key at the offsets 0, -alpha_i) */
+                int d = (int)S->d, q = wd / (d + 1), j = d - wd % (d + 1), is_aux = wd >= (int)nc;
+                u64 acc = 0;
+                for (int t = 0; t <= (is_aux ? 0 : d - j); t++) {
+                    u64 rp = t == 0 ? (party == 0 ? 1 : 0) : ld8(key, L.rpow + (size_t)(t - 1) * L.s8, e);
+                    u64 wprev = 0;
+                    for (int i = 0; i < P->m; i++) {
+                        u64 wi = is_aux ? S->aux[(size_t)i * S->p_aux + (wd - nc)]
+                                        : S->coeff[((size_t)i * S->r + q) * (d + 1) + (d - (j + t))] * binom(j + t, j);
+                        wi &= P->mask;
+                        if (i) {
+                            int ta = P->alpha_atom[i];
+                            u64 ei = (xh < S->alpha[i - 1]) ? 1 : 0;
+                            u64 sh = ei * rp - AV[P->atom_ib[ta]][t] + AV[P->atom_ia[ta]][t];
+                            acc += (wprev - wi) * sh;
+                        }
+                        if (i == P->m - 1) acc += wi * rp;
+                        wprev = wi;
+                    }
+                }
+                coeff_out[(size_t)wd * count + e] = acc & P->mask;
+            }
+            for (int wd = 0; wd < P->p && !P->xpoly; wd++) {
                 u64 acc = 0;
                 for (int i = 0; i < P->m; i++) {
                     u64 vi = (wd < (int)nc ? S->coeff[(size_t)i * nc + wd] : S->aux[(size_t)i * S->p_aux + (wd - nc)]) & P->mask;
@@ -1314,7 +1352,7 @@ static void sp_eval(int party, const orc_prog *P, const u8 *key, const u64 *xhat
             }
         }
     }
-    free(bk); free(vk); free(A);
+    free(bk); free(vk); free(A); free(AV);
 }
 
 void orc_eval_cmp(int party, const orc_prog *P, const u8 *key, const u64 *xhat, size_t count, u64 *bits_out)
