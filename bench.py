@@ -118,11 +118,13 @@ def run_reference(args, rank):
     print(json.dumps(line), flush=True)
 
 
-def measure_shared_prefix(F, torch, name, base_spec, inp, rank, world, steps, warmup, barrier, max_over_ranks):
+def measure_shared_prefix(F, torch, name, base_spec, inp, rank, world, steps, warmup, barrier, max_over_ranks, xpoly=False):
     """The same workload compiled with variant 1 (single-key shared-prefix construction):
     keygen (one n-bit key per element) + ONE fused evaluation per party + post, timed like the main step."""
     from workloads import specs as _specs
     spec = _specs.shared_prefix(base_spec)
+    if xpoly:
+        spec = _specs.public_point_horner(spec)
     P = F.Program(spec)
     sh, cost = P.shape, P.cost()
     count = int(inp["xhat"].size)
@@ -171,7 +173,9 @@ def measure_shared_prefix(F, torch, name, base_spec, inp, rank, world, steps, wa
     ach = aes_eval * count / (t_eval / 2 * 1e-3) / 1e9
     peak = 148 * SM_CLOCK_MAX_MHZ * 1e6 * LDS_LANES_PER_CLK_SM / (lk_eval / max(1, aes_eval)) / 1e9
     key_b = P.key_bytes(1 << 20) / (1 << 20)
-    return {"construction": "variant 1: one DCF key f_{r,1} per view width, evaluated at the public points xhat + delta_j with shared tree prefixes (DESIGN 9)",
+    return {"construction": ("variant 1 + bit 2: payload (1, -r, .., (-r)^d), coefficients of xhat^j, Horner in the public xhat: zero Beaver rounds (DESIGN 11)" if xpoly else
+                             "variant 1: one DCF key f_{r,1} per view width, evaluated at the public points xhat + delta_j with shared tree prefixes (DESIGN 9)"),
+            "post_rounds": P.post_rounds(),
             "value": world * count / (ms * 1e-3), "unit": "elements/s", "ms_per_step": ms,
             "eval_elems_per_s": world * count / (t_eval * 1e-3), "keygen_elems_per_s": world * count / (t_gen * 1e-3),
             "ms_breakdown": {"keygen": t_gen, "eval_fused_x2": t_eval, "post_fused": t_post},
@@ -390,6 +394,9 @@ def main():
         torch.cuda.empty_cache()
         line["shared_prefix"] = measure_shared_prefix(F, torch, name, spec, inp, rank, world, args.steps, args.warmup, barrier,
                                                       lambda v: (float(_allmax(v))))
+        if spec.d >= 1:
+            line["shared_prefix_public_horner"] = measure_shared_prefix(F, torch, name, spec, inp, rank, world, args.steps, args.warmup,
+                                                                        barrier, lambda v: (float(_allmax(v))), xpoly=True)
         k0, k1 = None, None
 
     # ---- e2e: the public host-buffer call, pinned host memory, H2D + D2H inside the timed region -------

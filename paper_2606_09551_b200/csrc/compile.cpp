@@ -182,19 +182,30 @@ void Lowering::build_sp() {
     }
     // interval lookup as a public linear map of the boundary comparisons (Lemma D.1 telescoped):
     // v_{i*} = v_{m-1} + sum_{i=1}^{m-1} (v_{i-1} - v_i) I[x < alpha_i]
-    const int p = P.p;
-    S.weights.assign((size_t)base * p, 0);
-    S.delta_tab.assign((size_t)P.m * p, 0);
-    for (int w = 0; w < p; ++w) S.delta_tab[w] = P.payload[(size_t)(P.m - 1) * p + w];
+    // With variant bit 2 the key's payload is (1, -r, .., (-r)^d) and the outputs are the coefficients of xhat^j of
+    // P_{i*}(xhat - r): c'_j = sum_t sum_i J_i (-r)^t w_{i,j,t},  w_{i,j,t} = c_{i,j+t} C(j+t, j)  (DESIGN 11).
+    const int p = P.p, d = (int)P.d, nc = (int)(P.r * (P.d + 1)), pk = P.xpoly ? d + 1 : 1;
+    S.pk = pk;
+    auto binom = [](int k, int j) { uint64_t v = 1; for (int i = 1; i <= j; ++i) v = v * (uint64_t)(k - j + i) / (uint64_t)i; return v; };
+    auto wfun = [&](uint32_t i, int w, int t) -> uint64_t {
+        if (!P.xpoly) return P.payload[(size_t)i * p + w];
+        if (w >= nc) return t == 0 ? P.payload[(size_t)i * p + w] : 0;
+        const int q = w / (d + 1), j = d - w % (d + 1);
+        if (j + t > d) return 0;
+        return (P.payload[(size_t)i * p + q * (d + 1) + (d - (j + t))] * binom(j + t, j)) & P.mask;
+    };
+    S.weights.assign((size_t)base * p * pk, 0);
+    S.delta_tab.assign((size_t)P.m * p * pk, 0);
+    for (int w = 0; w < p; ++w) for (int t = 0; t < pk; ++t) S.delta_tab[(size_t)w * pk + t] = wfun(P.m - 1, w, t);
     for (uint32_t i = 1; i < P.m && P.has_lut; ++i) {
-        int t = find_atom((int)P.n, 0, true, P.alpha[i - 1]);
-        S.alpha_atom[i] = t;
-        const int wd = S.atom_w[t];
-        for (int w = 0; w < p; ++w) {
-            const uint64_t dl = (P.payload[(size_t)(i - 1) * p + w] - P.payload[(size_t)i * p + w]) & P.mask;
-            S.delta_tab[(size_t)i * p + w] = dl;
-            S.weights[(size_t)(S.width[wd].first_point + S.atom_ia[t]) * p + w] += dl;
-            S.weights[(size_t)(S.width[wd].first_point + S.atom_ib[t]) * p + w] -= dl;
+        int ta = find_atom((int)P.n, 0, true, P.alpha[i - 1]);
+        S.alpha_atom[i] = ta;
+        const int wd = S.atom_w[ta];
+        for (int w = 0; w < p; ++w) for (int t = 0; t < pk; ++t) {
+            const uint64_t dl = (wfun(i - 1, w, t) - wfun(i, w, t)) & P.mask;
+            S.delta_tab[((size_t)i * p + w) * pk + t] = dl;
+            S.weights[((size_t)(S.width[wd].first_point + S.atom_ia[ta]) * p + w) * pk + t] += dl;
+            S.weights[((size_t)(S.width[wd].first_point + S.atom_ib[ta]) * p + w) * pk + t] -= dl;
         }
     }
     // clusters of the n-bit tree: greedy over the sorted offsets; a cluster spans < 2^tail_bits, so its points have
@@ -321,6 +332,12 @@ bool Lowering::run() {
     for (uint32_t j = 0; j < P.r; ++j) yval[j] = cval[j * per_poly];
     for (uint32_t k = 1; k <= P.d; ++k)                                      // Horner, one round per step
         for (uint32_t j = 0; j < P.r; ++j) {
+            if (P.xpoly) {                                                   // (..(c'_d xhat + c'_{d-1}) xhat ..) + c'_0, local (DESIGN 11)
+                int pr = fresh_a(a_ready[yval[j]]);
+                push(I_A_MULXH, pr, yval[j], 0, 0);
+                yval[j] = a_bin(I_A_ADD, pr, cval[j * per_poly + k]);
+                continue;
+            }
             int prod = a_mul(yval[j], xval);
             yval[j] = a_bin(I_A_ADD, prod, cval[j * per_poly + k]);
         }
@@ -379,7 +396,7 @@ bool Lowering::finish() {
         case I_B_NOT: case I_B_ANDPUB: case I_B_OUT: case I_A_B2A: a_is_B = true; break;
         case I_B_XOR: case I_B_AND: a_is_B = b_is_B = true; break;
         case I_A_ADD: case I_A_SUB: case I_A_MUL: a_is_A = b_is_A = true; break;
-        case I_A_MULC: case I_A_OUT: case I_A_MULX: a_is_A = true; break;
+        case I_A_MULC: case I_A_OUT: case I_A_MULX: case I_A_MULXH: a_is_A = true; break;
         default: break;
         }
     };
@@ -470,6 +487,8 @@ int compile_program(const fusefss_spec *S, Program **out) {
     P.has_lut = S->m > 1;                         // a single interval needs no lookup
     P.variant = S->variant & 1;
     P.xmul = (S->variant >> 1) & 1;
+    P.xpoly = ((S->variant >> 2) & 1) && S->d >= 1 && S->m > 1;
+    if (P.xpoly && S->d > 2) { delete holder; return FUSEFSS_E_SPEC; }          // kernels are instantiated for d <= 2
     if (P.variant) P.M = (int)S->m;               // variant 1: no translated partition, no wrap / dummy split
     P.n_out_a = (int)S->n_out_a; P.n_out_b = (int)S->n_out_b;
     if (P.n_out_a > kMaxP || P.n_out_b > 64) { delete holder; return FUSEFSS_E_SPEC; }
@@ -491,10 +510,10 @@ void compute_layout(const Program &P, size_t count, Layout *L) {
     L->s16 = round_up_256(count * 16);
     L->s8 = round_up_256(count * 8);
     if (P.variant) {                              // one tree per view width (DESIGN 9)
-        L->lvl_stride = L->s16 + L->s8;
+        L->lvl_stride = L->s16 + (size_t)P.sp.pk * L->s8;
         L->vt_lvl_rel = L->s16;
         L->vt_fin_rel = L->s16 + L->lvl_stride * (size_t)P.n;
-        L->vt_stride = L->vt_fin_rel + L->s8;
+        L->vt_stride = L->vt_fin_rel + (size_t)P.sp.pk * L->s8;
         L->lut_c = L->vt_first = 0;
         for (int w = 0; w < P.sp.n_w; ++w) {
             if (!P.sp.width[w].is_vec) {
@@ -525,6 +544,7 @@ void compute_layout(const Program &P, size_t count, Layout *L) {
     L->rin = off;      off += L->s8;
     L->rout = off;     if (P.mask_output) off += (size_t)P.n_out_a * L->s8;
     L->ka = off;       off += P.kappa_a.size() * L->s8;
+    L->rpow = off;     if (P.variant && P.xpoly) off += (size_t)P.d * L->s8;        // shares of (-r)^t, t = 1..d
     L->kb = off;       if (P.n_kb > 0) off += L->s8;
     L->beaver = off;   off += (size_t)P.ma_word[P.MA] * L->s8;
     L->andt = off;     if (P.MB > 0) off += 3 * L->s8;

@@ -18,7 +18,7 @@ struct SpAtomDev { uint64_t c, beta; int k, is_theta; };
 struct EvalSpArgs {
     const uint8_t *key; const uint64_t *xhat; uint64_t *bits_out, *coeff_out;       // either output may be null
     const SpPoint *points; const uint64_t *weights, *delta_tab, *alpha;             // device tables (program blob)
-    size_t count, s16, s8, lvl_stride, vt_first, vt_lvl_rel, vt_fin_rel;
+    size_t count, s16, s8, lvl_stride, vt_first, vt_lvl_rel, vt_fin_rel, rpow;
     uint64_t mask;
     int n, m, p, party, T, n_w, n_clusters, pad;
     SpWidth width[kMaxWidths];
@@ -27,14 +27,20 @@ struct EvalSpArgs {
     SpAtomDev atom[kMaxAtoms];
 };
 
-struct SpState { uint32_t s[4]; uint32_t t; uint64_t V; };
+// PK = payload words of the n-bit key: 1 (payload 1) or d+1 (payload (1, -r, .., (-r)^d), variant bit 2, DESIGN 11)
+template <int PK> struct SpState { uint32_t s[4]; uint32_t t; uint64_t V[PK]; };
 
-__device__ __forceinline__ void sp_step(uint32_t tl, const uint4 cw, const uint64_t vcw, uint32_t dbit, SpState &st) {
+template <int PK>
+__device__ __forceinline__ void sp_step(uint32_t tl, const uint4 cw, const uint64_t (&vcw)[PK], uint32_t dbit, SpState<PK> &st) {
+    constexpr int QK = (PK + 1) / 2;
     uint32_t x[1][4] = {{st.s[0] | dbit, st.s[1], st.s[2], st.s[3]}};
-    uint32_t o[1][2][4];
-    prg_blocks<1, 2, 0, true>(tl, x, o);
+    uint32_t o[1][1 + QK][4];
+    prg_blocks<1, 1 + QK, 0, true>(tl, x, o);
     const uint32_t tm = 0u - st.t;
-    st.V += ((uint64_t)o[0][1][0] | ((uint64_t)o[0][1][1] << 32)) + (vcw & (0ull - (uint64_t)st.t));
+    const uint64_t tm64 = 0ull - (uint64_t)st.t;
+#pragma unroll
+    for (int w = 0; w < PK; ++w)
+        st.V[w] += ((uint64_t)o[0][1 + w / 2][2 * (w & 1)] | ((uint64_t)o[0][1 + w / 2][2 * (w & 1) + 1] << 32)) + (vcw[w] & tm64);
     const uint32_t tnew = (o[0][0][0] & 1u) ^ (st.t & (cw.x >> dbit) & 1u);
     st.s[0] = (o[0][0][0] & ~3u) ^ (cw.x & ~3u & tm);
     st.s[1] = o[0][0][1] ^ (cw.y & tm);
@@ -43,36 +49,52 @@ __device__ __forceinline__ void sp_step(uint32_t tl, const uint4 cw, const uint6
     st.t = tnew;
 }
 
-// walk levels [from, to) of the n-bit vector tree (p = 1); ubits = the point with its level-`from` bit at bit 63
-__device__ __forceinline__ void sp_walk(uint32_t tl, const uint8_t *lvl, size_t e, size_t s16, size_t lvl_stride,
-                                        int from, int to, uint64_t ubits, SpState &st) {
+template <int PK>
+__device__ __forceinline__ void sp_load_level(const uint8_t *pl, size_t e, size_t s16, size_t s8, uint4 &cw, uint64_t (&vcw)[PK]) {
+    cw = __ldg(reinterpret_cast<const uint4 *>(pl + e * 16));
+#pragma unroll
+    for (int w = 0; w < PK; ++w) vcw[w] = __ldg(reinterpret_cast<const unsigned long long *>(pl + s16 + (size_t)w * s8 + e * 8));
+}
+
+// walk levels [from, to) of the n-bit vector tree; ubits = the point with its level-`from` bit at bit 63
+template <int PK>
+__device__ __forceinline__ void sp_walk(uint32_t tl, const uint8_t *lvl, size_t e, size_t s16, size_t s8, size_t lvl_stride,
+                                        int from, int to, uint64_t ubits, SpState<PK> &st) {
     const uint8_t *pl = lvl + (size_t)from * lvl_stride;
     for (int i = from; i < to; ++i, pl += lvl_stride) {
-        const uint4 cw = __ldg(reinterpret_cast<const uint4 *>(pl + e * 16));
-        const uint64_t vcw = __ldg(reinterpret_cast<const unsigned long long *>(pl + s16 + e * 8));
-        sp_step(tl, cw, vcw, (uint32_t)(ubits >> 63), st);
+        uint4 cw; uint64_t vcw[PK];
+        sp_load_level<PK>(pl, e, s16, s8, cw, vcw);
+        sp_step<PK>(tl, cw, vcw, (uint32_t)(ubits >> 63), st);
         ubits <<= 1;
     }
 }
 // two prefixes in lock-step over levels [0, to): same correction words, independent PRG chains
-__device__ __forceinline__ void sp_walk2(uint32_t tl, const uint8_t *lvl, size_t e, size_t s16, size_t lvl_stride,
-                                         int to, uint64_t u1, uint64_t u2, SpState &a, SpState &b) {
+template <int PK>
+__device__ __forceinline__ void sp_walk2(uint32_t tl, const uint8_t *lvl, size_t e, size_t s16, size_t s8, size_t lvl_stride,
+                                         int to, uint64_t u1, uint64_t u2, SpState<PK> &a, SpState<PK> &b) {
     const uint8_t *pl = lvl;
     for (int i = 0; i < to; ++i, pl += lvl_stride) {
-        const uint4 cw = __ldg(reinterpret_cast<const uint4 *>(pl + e * 16));
-        const uint64_t vcw = __ldg(reinterpret_cast<const unsigned long long *>(pl + s16 + e * 8));
-        sp_step(tl, cw, vcw, (uint32_t)(u1 >> 63), a);
-        sp_step(tl, cw, vcw, (uint32_t)(u2 >> 63), b);
+        uint4 cw; uint64_t vcw[PK];
+        sp_load_level<PK>(pl, e, s16, s8, cw, vcw);
+        sp_step<PK>(tl, cw, vcw, (uint32_t)(u1 >> 63), a);
+        sp_step<PK>(tl, cw, vcw, (uint32_t)(u2 >> 63), b);
         u1 <<= 1; u2 <<= 1;
     }
 }
 // leaf: A = (-1)^party (V + conv(s) + t * fin)
-__device__ __forceinline__ uint64_t sp_leaf(uint32_t tl, const SpState &st, uint64_t fin, int party) {
+template <int PK>
+__device__ __forceinline__ void sp_leaf(uint32_t tl, const SpState<PK> &st, const uint8_t *fin, size_t e, size_t s8, int party, uint64_t (&A)[PK]) {
+    constexpr int QK = (PK + 1) / 2;
     uint32_t x[1][4] = {{st.s[0] | 2u, st.s[1], st.s[2], st.s[3]}};
-    uint32_t o[1][1][4];
-    prg_blocks<1, 1, 1>(tl, x, o);
-    const uint64_t v = st.V + ((uint64_t)o[0][0][0] | ((uint64_t)o[0][0][1] << 32)) + (fin & (0ull - (uint64_t)st.t));
-    return party ? 0ull - v : v;
+    uint32_t o[1][QK][4];
+    prg_blocks<1, QK, 1, true>(tl, x, o);
+    const uint64_t tm64 = 0ull - (uint64_t)st.t;
+#pragma unroll
+    for (int w = 0; w < PK; ++w) {
+        const uint64_t f = __ldg(reinterpret_cast<const unsigned long long *>(fin + (size_t)w * s8 + e * 8));
+        const uint64_t v = st.V[w] + ((uint64_t)o[0][w / 2][2 * (w & 1)] | ((uint64_t)o[0][w / 2][2 * (w & 1) + 1] << 32)) + (f & tm64);
+        A[w] = party ? 0ull - v : v;
+    }
 }
 
 // bit-DCF walk (payload Z_2) of one point; u = the k-bit point, MSB-aligned
@@ -106,7 +128,7 @@ __device__ __forceinline__ uint32_t sp_bit_eval(uint32_t tl, const uint8_t *key,
     return (V ^ ((o[0][0][0] >> 1) & 1u) ^ (tb & fin)) & 1u;
 }
 
-template <int P>
+template <int P, int PK>
 __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ EvalSpArgs a) {
     extern __shared__ uint32_t sT[];
     const uint32_t tl = aes_fill_tables(sT);
@@ -128,20 +150,26 @@ __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ Eva
                     const uint64_t km = at.k >= 64 ? ~0ull : ((1ull << at.k) - 1ull);
                     if (at.is_theta) word |= (uint64_t)(((xh + at.c) & km) < at.beta) << t;
                 }
-            if (want_coeff) {
+        }
+        if (want_coeff) {                                                   // sum_t [(-r)^t] (w_{m-1} + sum_{i: xhat < alpha_i} (w_{i-1} - w_i))
+            uint64_t rp[PK];
+            rp[0] = a.party == 0 ? 1ull : 0ull;
 #pragma unroll
-                for (int w = 0; w < P; ++w) acc[w] = a.delta_tab[w];
-                for (int i = 1; i < a.m; ++i)
-                    if (xh < a.alpha[i - 1]) {
+            for (int t = 1; t < PK; ++t) rp[t] = __ldg(reinterpret_cast<const unsigned long long *>(a.key + a.rpow + (size_t)(t - 1) * a.s8 + e * 8));
+            if (PK > 1 || a.party == 0) {
+                for (int i = 0; i < a.m; ++i)
+                    if (i == 0 || xh < a.alpha[i - 1]) {
 #pragma unroll
-                        for (int w = 0; w < P; ++w) acc[w] += a.delta_tab[(size_t)i * P + w];
+                        for (int w = 0; w < P; ++w)
+#pragma unroll
+                            for (int t = 0; t < PK; ++t) acc[w] += a.delta_tab[((size_t)i * P + w) * PK + t] * rp[t];
                     }
             }
         }
         for (int wd = 0; wd < a.n_w; ++wd) {
             const SpWidth W = a.width[wd];
             const SpPoint *pts = a.points + W.first_point;
-            const uint64_t *wts = a.weights + (size_t)W.first_point * P;
+            const uint64_t *wts = a.weights + (size_t)W.first_point * P * PK;
             if (!W.is_vec) {
                 if (!want_bits) continue;
                 const uint64_t km = (1ull << W.k) - 1ull;
@@ -155,39 +183,44 @@ __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ Eva
             const uint8_t *tree = a.key + a.vt_first;
             const uint8_t *lvl = tree + a.vt_lvl_rel;
             const uint4 root = __ldg(reinterpret_cast<const uint4 *>(tree + e * 16));
-            const uint64_t fin = __ldg(reinterpret_cast<const unsigned long long *>(tree + a.vt_fin_rel + e * 8));
-            SpState r0;
-            r0.s[0] = root.x & ~3u; r0.s[1] = root.y; r0.s[2] = root.z; r0.s[3] = root.w; r0.t = (uint32_t)a.party; r0.V = 0;
+            const uint8_t *fin = tree + a.vt_fin_rel;
+            SpState<PK> r0;
+            r0.s[0] = root.x & ~3u; r0.s[1] = root.y; r0.s[2] = root.z; r0.s[3] = root.w; r0.t = (uint32_t)a.party;
+#pragma unroll
+            for (int t = 0; t < PK; ++t) r0.V[t] = 0;
             const int n = a.n;
             for (int c = 0; c < a.n_clusters; ++c) {
                 const SpCluster cl = a.cluster[c];
                 const int kf = n - cl.tail_bits;                            // shared levels
                 const bool share = cl.count > 1 && kf > 0;
-                SpState s1 = r0, s2 = r0;
+                SpState<PK> s1 = r0, s2 = r0;
                 uint64_t pre1 = 0;
                 if (share) {
                     const uint64_t uf = ((xh + pts[cl.first].delta) & a.mask) << (64 - n);
                     const uint64_t ul = ((xh + pts[cl.first + cl.count - 1].delta) & a.mask) << (64 - n);
-                    sp_walk2(tl, lvl, e, a.s16, a.lvl_stride, kf, uf, ul, s1, s2);
+                    sp_walk2<PK>(tl, lvl, e, a.s16, a.s8, a.lvl_stride, kf, uf, ul, s1, s2);
                     pre1 = uf >> (64 - kf);
                 }
                 for (int j = cl.first; j < cl.first + cl.count; ++j) {
                     bool need = want_bits && pts[j].bitmask != 0;
                     if (want_coeff) {
 #pragma unroll
-                        for (int w = 0; w < P; ++w) need = need || wts[(size_t)j * P + w] != 0;
+                        for (int w = 0; w < P * PK; ++w) need = need || wts[(size_t)j * P * PK + w] != 0;
                     }
                     if (!need) continue;
                     const uint64_t u = ((xh + pts[j].delta) & a.mask) << (64 - n);
-                    SpState st = r0;
+                    SpState<PK> st = r0;
                     int from = 0;
                     if (share) { st = (u >> (64 - kf)) == pre1 ? s1 : s2; from = kf; }
-                    sp_walk(tl, lvl, e, a.s16, a.lvl_stride, from, n, from ? u << from : u, st);
-                    const uint64_t A = sp_leaf(tl, st, fin, a.party);
-                    word ^= pts[j].bitmask & (0ull - (A & 1ull));
+                    sp_walk<PK>(tl, lvl, e, a.s16, a.s8, a.lvl_stride, from, n, from ? u << from : u, st);
+                    uint64_t A[PK];
+                    sp_leaf<PK>(tl, st, fin, e, a.s8, a.party, A);
+                    word ^= pts[j].bitmask & (0ull - (A[0] & 1ull));        // component 0 = share of I[u_j < r]
                     if (want_coeff) {
 #pragma unroll
-                        for (int w = 0; w < P; ++w) acc[w] += wts[(size_t)j * P + w] * A;
+                        for (int w = 0; w < P; ++w)
+#pragma unroll
+                            for (int t = 0; t < PK; ++t) acc[w] += wts[((size_t)j * P + w) * PK + t] * A[t];
                     }
                 }
             }

@@ -172,11 +172,26 @@ struct P3 {
     }
 };
 
+// variant bit 2 (DESIGN 11): replace the coefficients of every polynomial of a payload (high degree first, d+1 words
+// each, `polys` of them) by those of P(X - r): Taylor shift by synthetic division, d passes of c_idx += (-r) c_{idx-1}.
+template <int P>
+__device__ __forceinline__ void shift_payload(uint64_t (&v)[P], int polys, int d, uint64_t negr) {
+    const int nc = polys * (d + 1);
+    for (int it = 0; it < d; ++it) {
+#pragma unroll
+        for (int w = 1; w < P; ++w) {
+            const int idx = w % (d + 1);
+            if (w < nc && idx >= 1 && idx <= d - it) v[w] += negr * v[w - 1];
+        }
+    }
+}
+
 struct GenVecArgs {
     uint8_t *key0, *key1; const uint64_t *r_in; const uint64_t *alpha; const uint64_t *payload;   // payload[m][p]
     size_t count, s16, s8, vt_first, vt_stride, lvl_stride, vt_lvl_rel, vt_fin_rel;
     uint64_t first_elem, mask;
-    int n, m, M, sp;           // sp = 1 (variant 1): the single tree f_{r,1}: threshold r_in, payload 1, no Protocol 3
+    int n, m, M, sp;           // sp = 1 (variant 1): the single tree f_{r,beta}: threshold r_in, beta = (1, -r, (-r)^2, ..), no Protocol 3
+    int xpoly, polys, d, pad2; // variant bit 2 with Protocol 3: payloads are the coefficients of P_i(X - r_in)
     RoundKeys rk;
 };
 
@@ -197,8 +212,9 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec(const __grid_constan
         uint64_t alpha, beta[P];
         if (a.sp) {
             alpha = r << (64 - a.n);
+            beta[0] = 1;
 #pragma unroll
-            for (int w = 0; w < P; ++w) beta[w] = 1;
+            for (int w = 1; w < P; ++w) beta[w] = beta[w - 1] * (0ull - r);
         } else {
             P3 p3;
             p3.init(a.alpha, a.m, a.n, a.mask, r, a.M);
@@ -206,6 +222,7 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec(const __grid_constan
             const uint64_t *va = a.payload + (size_t)p3.ord(j - 1) * P, *vb = a.payload + (size_t)p3.ord(j) * P;
 #pragma unroll
             for (int w = 0; w < P; ++w) beta[w] = va[w] - vb[w];                // Delta_j = v_{j-1} - v_j
+            if (a.xpoly) shift_payload<P>(beta, a.polys, a.d, 0ull - r);        // the shift is linear: shift the difference
         }
         uint32_t s[2][4];
         {
@@ -311,7 +328,8 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec(const __grid_constan
 // ---------------------------------------------------------------------------------------------------
 struct GenMiscArgs {
     uint8_t *key0, *key1; const uint64_t *r_in, *r_out, *alpha, *payload;
-    size_t count, s8, lut_c, rin, rout, ka, kb, beaver, andt, b2a_bits, b2a_a;
+    size_t count, s8, lut_c, rin, rout, ka, kb, beaver, andt, b2a_bits, b2a_a, rpow;
+    int xpoly, polys, d, n_rpow;
     uint64_t first_elem, mask;
     int n, m, M, p, has_lut, mask_output, n_out_a, n_ka, n_kb_spec, n_carry, T, MA, MB, GMIX;
     uint64_t ma_is_x;          // bit i: arithmetic gate i is a product with the gate input (material (b, c = b r_in), DESIGN 10)
@@ -334,8 +352,14 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_misc(const __grid_consta
         if (a.has_lut) {                                                   // additive split of v_{M-1}
             P3 p3;
             p3.init(a.alpha, a.m, a.n, a.mask, r, a.M);
-            const uint64_t *v = a.payload + (size_t)p3.ord(a.M - 1) * a.p;
-            for (int w = 0; w < a.p; ++w) {
+            const uint64_t *vp = a.payload + (size_t)p3.ord(a.M - 1) * a.p;
+            uint64_t v[kMaxP];
+#pragma unroll
+            for (int w = 0; w < kMaxP; ++w) v[w] = w < a.p ? vp[w] : 0;
+            if (a.xpoly) shift_payload<kMaxP>(v, a.polys, a.d, 0ull - r);
+#pragma unroll
+            for (int w = 0; w < kMaxP; ++w) {
+                if (w >= a.p) break;
                 dealer_rand(tl, a.rk, ge, SLOT_LUT_C + w, lo, hi);
                 const uint64_t c0 = lo & a.mask;
                 put(a.lut_c + (size_t)w * a.s8, c0, (v[w] - c0) & a.mask);
@@ -355,6 +379,15 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_misc(const __grid_consta
             if (a.ka_kind[t] == FUSEFSS_KA_R_SHR) val = a.ka_arg[t] >= 64 ? 0ull : r >> a.ka_arg[t];
             const uint64_t s0 = lo & a.mask;
             put(a.ka + (size_t)t * a.s8, s0, ((val & a.mask) - s0) & a.mask);
+        }
+        {                                                                  // variant 1 + bit 2: shares of (-r)^t, t = 1..d
+            uint64_t pw = 1;
+            for (int t = 1; t <= a.n_rpow; ++t) {
+                pw = (pw * (0ull - r)) & a.mask;
+                dealer_rand(tl, a.rk, ge, 0x5400 + t, lo, hi);
+                const uint64_t s0 = lo & a.mask;
+                put(a.rpow + (size_t)(t - 1) * a.s8, s0, (pw - s0) & a.mask);
+            }
         }
         const int n_kb = a.n_carry + a.n_kb_spec;
         if (n_kb > 0) {

@@ -186,16 +186,13 @@ int launch_eval_sp(Program &P, int party, const void *key, const uint64_t *xhat,
     threads = threads < 64 ? 64 : threads > g_eval_threads ? g_eval_threads : threads;
     const int grid = grid_for((count + 31) / 32, threads);
     const size_t sm = kAesSmemBytes;
-    switch (P.p) {
-    case 1: return launch(k_eval_sp<1>, grid, threads, sm, st, a);
-    case 2: return launch(k_eval_sp<2>, grid, threads, sm, st, a);
-    case 3: return launch(k_eval_sp<3>, grid, threads, sm, st, a);
-    case 4: return launch(k_eval_sp<4>, grid, threads, sm, st, a);
-    case 5: return launch(k_eval_sp<5>, grid, threads, sm, st, a);
-    case 6: return launch(k_eval_sp<6>, grid, threads, sm, st, a);
-    case 7: return launch(k_eval_sp<7>, grid, threads, sm, st, a);
-    case 8: return launch(k_eval_sp<8>, grid, threads, sm, st, a);
-    }
+    a.rpow = L.rpow;
+#define FSK_SP_CASE(PP, KK) if (P.p == PP && P.sp.pk == KK) return launch(k_eval_sp<PP, KK>, grid, threads, sm, st, a);
+#define FSK_SP_ROW(KK) FSK_SP_CASE(1, KK) FSK_SP_CASE(2, KK) FSK_SP_CASE(3, KK) FSK_SP_CASE(4, KK) FSK_SP_CASE(5, KK) \
+                       FSK_SP_CASE(6, KK) FSK_SP_CASE(7, KK) FSK_SP_CASE(8, KK)
+    FSK_SP_ROW(1) FSK_SP_ROW(2) FSK_SP_ROW(3)
+#undef FSK_SP_ROW
+#undef FSK_SP_CASE
     return FUSEFSS_E_SPEC;
 }
 
@@ -302,10 +299,12 @@ int fusefss_cost(const fusefss_program *prog, fusefss_cost_t *out) {
                 const uint64_t kf = n - (uint64_t)cl.tail_bits;
                 const bool share = cl.count > 1 && kf > 0;
                 const uint64_t levels = share ? 2 * kf + (uint64_t)cl.count * (uint64_t)cl.tail_bits : (uint64_t)cl.count * n;
-                c.eval_lut_aes += 2 * levels + (uint64_t)cl.count; c.eval_lut_lookups += levels * grp(2) + 160 * (uint64_t)cl.count;
+                const uint64_t qk = ((uint64_t)P->sp.pk + 1) / 2;
+                c.eval_lut_aes += (1 + qk) * levels + qk * (uint64_t)cl.count; c.eval_lut_lookups += levels * grp(1 + qk) + grp(qk) * (uint64_t)cl.count;
             }
-            c.gen_lut_aes += 8 * n + 4; c.gen_lut_lookups += 2 * 160 + n * 2 * grp(4) + 2 * 160;
-            c.eval_lut_key_bytes += 16 + n * 24 + 8;
+            const uint64_t qk = ((uint64_t)P->sp.pk + 1) / 2, pk = (uint64_t)P->sp.pk;
+            c.gen_lut_aes += 4 * n * (1 + qk) + 2 * qk + 2; c.gen_lut_lookups += 2 * 160 + n * 2 * grp(2 * (1 + qk)) + 2 * grp(qk);
+            c.eval_lut_key_bytes += 16 + n * (16 + 8 * pk) + 8 * pk;
         }
     }
     *out = c;
@@ -370,7 +369,7 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
             a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.vt_first = L.vt_first; a.vt_stride = L.vt_stride; a.lvl_stride = L.lvl_stride;
             a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel; a.first_elem = first_elem; a.mask = P->mask;
             a.n = (int)P->n; a.m = (int)P->m; a.M = 2; a.sp = 1; a.rk = rk;
-            rc = launch(k_gen_vec<1>, grid_for(tiles, kGenThreads), kGenThreads, smem, st, a);
+            rc = launch_gen_vec_p(P->sp.pk, grid_for(tiles, kGenThreads), kGenThreads, st, a);
             if (rc) return rc;
         }
     }
@@ -390,6 +389,7 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
         a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.vt_first = L.vt_first; a.vt_stride = L.vt_stride; a.lvl_stride = L.lvl_stride;
         a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel; a.first_elem = first_elem; a.mask = P->mask;
         a.n = (int)P->n; a.m = (int)P->m; a.M = P->M; a.rk = rk;
+        a.xpoly = (int)P->xpoly; a.polys = (int)P->r; a.d = (int)P->d;
         const int grid = grid_for(tiles * (size_t)(P->M - 1), kGenThreads);
         rc = launch_gen_vec_p(P->p, grid, kGenThreads, st, a);
         if (rc) return rc;
@@ -403,6 +403,8 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
         a.first_elem = first_elem; a.mask = P->mask;
         a.n = (int)P->n; a.m = (int)P->m; a.M = P->M; a.p = P->p; a.has_lut = P->variant ? 0 : P->has_lut; a.mask_output = (int)P->mask_output;
         a.n_out_a = P->n_out_a; a.n_ka = (int)P->kappa_a.size(); a.n_kb_spec = (int)P->kappa_b.size(); a.n_carry = P->n_carry;
+        a.rpow = L.rpow; a.n_rpow = (P->variant && P->xpoly) ? (int)P->d : 0;
+        a.xpoly = (int)P->xpoly; a.polys = (int)P->r; a.d = (int)P->d;
         a.T = P->variant ? 0 : P->T; a.MA = P->MA; a.MB = P->MB; a.GMIX = P->GMIX; a.rk = rk;
         for (int g = 0; g < P->MA; ++g) if (P->ma_is_x[g]) a.ma_is_x |= 1ull << g;
         if (a.n_ka > 8) return FUSEFSS_E_SPEC;

@@ -9,7 +9,7 @@
 
 namespace fsk {
 
-struct PostKeyOff { size_t s8, rin, rout, ka, kb, beaver, andt, b2a_bits, b2a_a; };
+struct PostKeyOff { size_t s8, rin, rout, ka, kb, beaver, andt, b2a_bits, b2a_a; };   // (rpow is read by the eval kernel only)
 
 struct PostArgs {
     const Ins *ins; int n_ins;
@@ -71,6 +71,7 @@ __global__ void __launch_bounds__(256) k_post_round(const __grid_constant__ Post
         case I_A_ADD: A[o.dst] = (A[o.a] + A[o.b]) & mask; break;
         case I_A_SUB: A[o.dst] = (A[o.a] - A[o.b]) & mask; break;
         case I_A_MULC: A[o.dst] = (A[o.a] * o.imm) & mask; break;
+        case I_A_MULXH: A[o.dst] = (A[o.a] * xh) & mask; break;          // share times the public xhat (DESIGN 11)
         case I_A_OUT:
             if (a.round == a.rounds) {
                 uint64_t v = A[o.a];
@@ -179,6 +180,7 @@ __global__ void __launch_bounds__(256) k_post_fused(const __grid_constant__ Post
         case I_A_ADD: A[0][o.dst] = (A[0][o.a] + A[0][o.b]) & mask; A[1][o.dst] = (A[1][o.a] + A[1][o.b]) & mask; break;
         case I_A_SUB: A[0][o.dst] = (A[0][o.a] - A[0][o.b]) & mask; A[1][o.dst] = (A[1][o.a] - A[1][o.b]) & mask; break;
         case I_A_MULC: A[0][o.dst] = (A[0][o.a] * o.imm) & mask; A[1][o.dst] = (A[1][o.a] * o.imm) & mask; break;
+        case I_A_MULXH: A[0][o.dst] = (A[0][o.a] * xh) & mask; A[1][o.dst] = (A[1][o.a] * xh) & mask; break;
         case I_A_OUT:
 #pragma unroll
             for (int b = 0; b < 2; ++b) {

@@ -29,7 +29,7 @@ struct Atom {
 // (`gate`), their round and their position inside that round's message (`pos`).
 enum : uint8_t {
     I_B_CONST = 1, I_B_ATOM, I_B_KAPPA, I_B_XHAT, I_B_NOT, I_B_XOR, I_B_AND, I_B_ANDPUB, I_B_OUT,
-    I_A_CONST, I_A_X, I_A_COEFF, I_A_KAPPA, I_A_XHAT_SHR, I_A_ADD, I_A_SUB, I_A_MULC, I_A_MUL, I_A_MULX, I_A_B2A, I_A_OUT
+    I_A_CONST, I_A_X, I_A_COEFF, I_A_KAPPA, I_A_XHAT_SHR, I_A_ADD, I_A_SUB, I_A_MULC, I_A_MUL, I_A_MULX, I_A_MULXH, I_A_B2A, I_A_OUT
 };
 struct Ins {
     uint8_t op;
@@ -47,7 +47,7 @@ struct Layout {
     size_t s16, s8;
     size_t bt_root[kMaxAtoms], bt_cw[kMaxAtoms], bt_vb[kMaxAtoms];
     size_t lut_c, vt_first, vt_stride, lvl_stride, vt_lvl_rel, vt_fin_rel;   // vector tree j at vt_first + (j-1)*vt_stride
-    size_t rin, rout, ka, kb, beaver, andt, b2a_bits, b2a_a, total;
+    size_t rin, rout, ka, rpow, kb, beaver, andt, b2a_bits, b2a_a, total;
 };
 
 // variant 1: single-key shared-prefix construction
@@ -60,8 +60,9 @@ struct SpProgram {
     int n_w = 0;
     SpWidth width[kMaxWidths];
     std::vector<SpPoint> points;        // all widths, width-major, sorted by signed delta inside a width
-    std::vector<uint64_t> weights;      // [n_points_total][p]: coefficient share += weights[j][w] * A_j
-    std::vector<uint64_t> delta_tab;    // [m][p]: row i >= 1 = v_{i-1} - v_i, row 0 = v_{m-1} (public part, party 0)
+    int pk = 1;                         // payload words of the n-bit key: 1, or d+1 = (1, -r, .., (-r)^d) with variant bit 2
+    std::vector<uint64_t> weights;      // [n_points_total][p][pk]: coefficient share w += weights[j][w][t] * A_j[t]
+    std::vector<uint64_t> delta_tab;    // [m][p][pk]: row i >= 1 = w_{i-1} - w_i, row 0 = w_{m-1} (times the share of (-r)^t)
     std::vector<SpCluster> clusters;    // of the n-bit tree
     int atom_w[kMaxAtoms], atom_ib[kMaxAtoms], atom_ia[kMaxAtoms], alpha_atom[kMaxIntervals];
 };
@@ -86,6 +87,7 @@ struct Program {
     int round_mul[kMaxRounds] = {0}, round_bits[kMaxRounds] = {0};
     // variant bit 1 (DESIGN 10): a product with the gate input x opens one ring element and needs (b, c = b r_in)
     uint32_t xmul = 0;
+    uint32_t xpoly = 0;                   // variant bit 2 (DESIGN 11): Horner in the public xhat, zero Beaver rounds for the spline
     int round_arr[kMaxRounds] = {0};      // ring-element arrays opened per round: 2 per Beaver, 1 per x-product
     int ma_is_x[64] = {0}, ma_word[65] = {0};
     // payload table v[i][w], i < m, w < p (coefficients poly-major, high degree first, then aux), masked

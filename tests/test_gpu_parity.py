@@ -105,7 +105,10 @@ SMALL_SP = [(lambda mk=mk: specs.shared_prefix(mk())) for mk in SMALL]
 SMALL_XM = [(lambda mk=mk: specs.input_masked_mul(mk())) for mk in SMALL[:4] + SMALL[7:9] + SMALL_SP[:4] + SMALL_SP[7:9]]
 
 
-@pytest.mark.parametrize("mk", SMALL + SMALL_SP + SMALL_XM)
+SMALL_XP = [(lambda mk=mk: specs.public_point_horner(mk())) for mk in SMALL[1:4] + SMALL[5:6] + SMALL[8:9] + SMALL_SP[1:4] + SMALL_SP[5:6] + SMALL_SP[8:9]]
+
+
+@pytest.mark.parametrize("mk", SMALL + SMALL_SP + SMALL_XM + SMALL_XP)
 @pytest.mark.parametrize("force_g", ["", "1"])
 def test_small_rings_all_masks(F, orc, mk, force_g, monkeypatch):
     """Every mask r (both Protocol 3 branches, incl. beta_0 = 0 and the dummy split) at n <= 8; a ragged count."""
@@ -129,7 +132,7 @@ CONFIGS = [("relu16", 4096), ("gelu", 700), ("nexp", 330), ("recip", 130), ("shi
            ("silu", 131)]
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5])
 @pytest.mark.parametrize("name,count", CONFIGS)
 def test_config_parity(F, orc, name, count, variant):
     """BASELINE.json's configs on their seeded synthetic inputs (workloads/tensors.py), several 32-element tiles
@@ -142,6 +145,9 @@ def test_config_parity(F, orc, name, count, variant):
     if variant & 2:
         spec = specs.input_masked_mul(spec)                 # one opening per product with x (DESIGN 10)
         count = max(33, count // 4)
+    if variant & 4:
+        spec = specs.public_point_horner(spec)              # Horner in the public xhat, zero Beaver rounds (DESIGN 11)
+        count = max(33, count // 2)
     inp = tensors.inputs(name, spec, count=count, seed=0)
     _parity(F, orc, spec, inp["x"], inp["r_in"], inp["r_out"], seed=0)
 
