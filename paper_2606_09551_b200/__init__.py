@@ -165,7 +165,7 @@ class Program:
         self.shape["k"] = [int(sh.k[t]) for t in range(self.shape["T"])]
 
     def __del__(self):
-        if getattr(self, "_h", None):
+        if getattr(self, "_h", None) and lib is not None:       # `lib` is gone at interpreter shutdown
             lib.fusefss_destroy(self._h)
             self._h = None
 

@@ -20,7 +20,7 @@ struct EvalSpArgs {
     const SpPoint *points; const uint64_t *weights, *delta_tab, *alpha;             // device tables (program blob)
     size_t count, s16, s8, lvl_stride, vt_first, vt_lvl_rel, vt_fin_rel, rpow;
     uint64_t mask;
-    int n, m, p, party, T, n_w, n_clusters, pad;
+    int n, m, p, party, T, n_w, n_clusters, G;   // G > 1: the points of an element are dealt round-robin to G warps (small tensors)
     SpWidth width[kMaxWidths];
     size_t bt_root[kMaxWidths], bt_cw[kMaxWidths], bt_vb[kMaxWidths];
     SpCluster cluster[kMaxClusters];
@@ -132,9 +132,11 @@ template <int P, int PK>
 __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ EvalSpArgs a) {
     extern __shared__ uint32_t sT[];
     const uint32_t tl = aes_fill_tables(sT);
-    const size_t tiles = (a.count + 31) / 32, warps = (size_t)gridDim.x * (blockDim.x >> 5);
-    // warp w of CTA b takes tiles w*grid + b (+ k*warps): a partial last wave spreads evenly over all SMs
-    for (size_t tile = (size_t)(threadIdx.x >> 5) * gridDim.x + blockIdx.x; tile < tiles; tile += warps) {
+    const size_t tiles = (a.count + 31) / 32, items = tiles * (size_t)a.G, warps = (size_t)gridDim.x * (blockDim.x >> 5);
+    // warp w of CTA b takes items w*grid + b (+ k*warps): a partial last wave spreads evenly over all SMs
+    for (size_t item = (size_t)(threadIdx.x >> 5) * gridDim.x + blockIdx.x; item < items; item += warps) {
+        const int g = (int)(item / tiles);                                  // this warp's share of every element's points
+        const size_t tile = item - (size_t)g * tiles;
         const size_t e0 = tile * 32 + (threadIdx.x & 31);
         const bool live = e0 < a.count;
         const size_t e = live ? e0 : a.count - 1;
@@ -143,7 +145,7 @@ __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ Eva
         uint64_t word = 0, acc[P];
 #pragma unroll
         for (int w = 0; w < P; ++w) acc[w] = 0;
-        if (a.party == 0) {                                                 // public parts: e_t and the plaintext table row of xhat
+        if (a.party == 0 && g == 0) {                                       // public parts: e_t and the plaintext table row of xhat
             if (want_bits)
                 for (int t = 0; t < a.T; ++t) {
                     const SpAtomDev &at = a.atom[t];
@@ -151,7 +153,7 @@ __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ Eva
                     if (at.is_theta) word |= (uint64_t)(((xh + at.c) & km) < at.beta) << t;
                 }
         }
-        if (want_coeff) {                                                   // sum_t [(-r)^t] (w_{m-1} + sum_{i: xhat < alpha_i} (w_{i-1} - w_i))
+        if (want_coeff && g == 0) {                                         // sum_t [(-r)^t] (w_{m-1} + sum_{i: xhat < alpha_i} (w_{i-1} - w_i))
             uint64_t rp[PK];
             rp[0] = a.party == 0 ? 1ull : 0ull;
 #pragma unroll
@@ -173,7 +175,7 @@ __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ Eva
             if (!W.is_vec) {
                 if (!want_bits) continue;
                 const uint64_t km = (1ull << W.k) - 1ull;
-                for (int j = 0; j < W.n_points; ++j) {
+                for (int j = g; j < W.n_points; j += a.G) {
                     const uint64_t u = (((xh & km) + pts[j].delta) & km) << (64 - W.k);
                     const uint32_t A = sp_bit_eval(tl, a.key, a.bt_root[wd], a.bt_cw[wd], a.bt_vb[wd], e, a.s16, W.k, u, a.party);
                     word ^= pts[j].bitmask & (0ull - (uint64_t)A);
@@ -201,7 +203,7 @@ __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ Eva
                     sp_walk2<PK>(tl, lvl, e, a.s16, a.s8, a.lvl_stride, kf, uf, ul, s1, s2);
                     pre1 = uf >> (64 - kf);
                 }
-                for (int j = cl.first; j < cl.first + cl.count; ++j) {
+                for (int j = cl.first + g; j < cl.first + cl.count; j += a.G) {
                     bool need = want_bits && pts[j].bitmask != 0;
                     if (want_coeff) {
 #pragma unroll
@@ -226,10 +228,18 @@ __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ Eva
             }
         }
         if (live) {
-            if (want_bits) a.bits_out[e] = word;
-            if (want_coeff) {
+            if (a.G == 1) {
+                if (want_bits) a.bits_out[e] = word;
+                if (want_coeff) {
 #pragma unroll
-                for (int w = 0; w < P; ++w) a.coeff_out[(size_t)w * a.count + e] = acc[w] & a.mask;
+                    for (int w = 0; w < P; ++w) a.coeff_out[(size_t)w * a.count + e] = acc[w] & a.mask;
+                }
+            } else {                                                        // integer xor / add: order-independent, still bit-exact
+                if (want_bits) atomicXor(reinterpret_cast<unsigned long long *>(a.bits_out + e), (unsigned long long)word);
+                if (want_coeff) {
+#pragma unroll
+                    for (int w = 0; w < P; ++w) atomicAdd(reinterpret_cast<unsigned long long *>(a.coeff_out + (size_t)w * a.count + e), (unsigned long long)acc[w]);
+                }
             }
         }
     }

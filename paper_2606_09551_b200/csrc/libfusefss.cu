@@ -84,6 +84,16 @@ int pick_groups(size_t count, int gmax, int threads) {
     return best;
 }
 
+// CTA size for `warp_items` warp-sized work items: small launches use small CTAs so that the warps spread over all
+// SMs (the AES kernels are bound by the per-SM shared-memory pipe), large ones use max_threads per CTA.
+int threads_for(size_t warp_items, int max_threads) {
+    size_t per_sm = (warp_items + (size_t)g_sms - 1) / (size_t)g_sms;
+    size_t t = per_sm * 32;
+    if (t < 64) t = 64;
+    if (t > (size_t)max_threads) t = (size_t)max_threads;
+    return (int)t;
+}
+
 int grid_for(size_t warp_items, int threads) {
     size_t blocks = (warp_items + (threads / 32) - 1) / (threads / 32);
     if (blocks > (size_t)g_sms) blocks = (size_t)g_sms;
@@ -181,19 +191,36 @@ int launch_eval_sp(Program &P, int party, const void *key, const uint64_t *xhat,
     for (int c = 0; c < a.n_clusters; ++c) a.cluster[c] = P.sp.clusters[c];
     for (int w = 0; w < P.sp.n_w; ++w) { a.width[w] = P.sp.width[w]; a.bt_root[w] = L.bt_root[w]; a.bt_cw[w] = L.bt_cw[w]; a.bt_vb[w] = L.bt_vb[w]; }
     for (int t = 0; t < P.T; ++t) a.atom[t] = SpAtomDev{P.atoms[t].c, P.atoms[t].beta, P.atoms[t].k, P.atoms[t].is_theta};
-    // spread small tensors over the SMs: threads per CTA = count / SMs rounded up to a warp, in [64, 1024]
-    int threads = (int)(((count + g_sms - 1) / g_sms + 31) / 32 * 32);
-    threads = threads < 64 ? 64 : threads > g_eval_threads ? g_eval_threads : threads;
-    const int grid = grid_for((count + 31) / 32, threads);
+    // small tensors: deal the points of an element to G warps so that the machine has >= ~8 warps per SM, then
+    // spread the warps over the SMs (threads per CTA = items / SMs rounded up to a warp, in [64, 1024])
+    const size_t tiles = (count + 31) / 32;
+    int maxpts = 1;
+    for (int w = 0; w < P.sp.n_w; ++w) if (P.sp.width[w].n_points > maxpts) maxpts = P.sp.width[w].n_points;
+    int G = (int)(((size_t)g_sms * 8 + tiles - 1) / tiles);
+    G = G < 1 ? 1 : G > 8 ? 8 : G;
+    if (G > maxpts) G = maxpts;
+    if (const char *f = std::getenv("FUSEFSS_FORCE_G")) { int v = std::atoi(f); if (v >= 1) G = v < maxpts ? v : maxpts; }
+    a.G = G;
+    if (G > 1) {
+        if (bits_out) CU(cudaMemsetAsync(bits_out, 0, count * 8, st));
+        if (coeff_out) CU(cudaMemsetAsync(coeff_out, 0, count * 8 * (size_t)P.p, st));
+    }
+    const int threads = threads_for(tiles * G, g_eval_threads);
+    const int grid = grid_for(tiles * G, threads);
     const size_t sm = kAesSmemBytes;
     a.rpow = L.rpow;
-#define FSK_SP_CASE(PP, KK) if (P.p == PP && P.sp.pk == KK) return launch(k_eval_sp<PP, KK>, grid, threads, sm, st, a);
+    int lrc = FUSEFSS_E_SPEC;
+#define FSK_SP_CASE(PP, KK) if (P.p == PP && P.sp.pk == KK) lrc = launch(k_eval_sp<PP, KK>, grid, threads, sm, st, a);
 #define FSK_SP_ROW(KK) FSK_SP_CASE(1, KK) FSK_SP_CASE(2, KK) FSK_SP_CASE(3, KK) FSK_SP_CASE(4, KK) FSK_SP_CASE(5, KK) \
                        FSK_SP_CASE(6, KK) FSK_SP_CASE(7, KK) FSK_SP_CASE(8, KK)
     FSK_SP_ROW(1) FSK_SP_ROW(2) FSK_SP_ROW(3)
 #undef FSK_SP_ROW
 #undef FSK_SP_CASE
-    return FUSEFSS_E_SPEC;
+    if (lrc == 0 && G > 1 && P.n < 64 && coeff_out) {                      // the atomics accumulated mod 2^64: reduce to the ring
+        const size_t words = count * (size_t)P.p;
+        return launch(k_mask_words, (int)((words + 255) / 256), 256, 0, st, MaskArgs{coeff_out, words, P.mask});
+    }
+    return lrc;
 }
 
 PostKeyOff post_offsets(const Layout &L) {
@@ -360,7 +387,7 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
             ab.atom[w] = GenAtomDev{0, 0, L.bt_root[w], L.bt_cw[w], L.bt_vb[w], vec ? 0 : P->sp.width[w].k, 0};
         }
         if (any_bit && (parts & FUSEFSS_GEN_CMP)) {
-            rc = launch(k_gen_bit, grid_for(tiles * P->sp.n_w, kGenThreads), kGenThreads, smem, st, ab);
+            { const int th = threads_for(tiles * P->sp.n_w, kGenThreads); rc = launch(k_gen_bit, grid_for(tiles * P->sp.n_w, th), th, smem, st, ab); }
             if (rc) return rc;
         }
         if (any_vec && (parts & FUSEFSS_GEN_LUT)) {
@@ -369,7 +396,7 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
             a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.vt_first = L.vt_first; a.vt_stride = L.vt_stride; a.lvl_stride = L.lvl_stride;
             a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel; a.first_elem = first_elem; a.mask = P->mask;
             a.n = (int)P->n; a.m = (int)P->m; a.M = 2; a.sp = 1; a.rk = rk;
-            rc = launch_gen_vec_p(P->sp.pk, grid_for(tiles, kGenThreads), kGenThreads, st, a);
+            { const int th = threads_for(tiles, kGenThreads); rc = launch_gen_vec_p(P->sp.pk, grid_for(tiles, th), th, st, a); }
             if (rc) return rc;
         }
     }
@@ -379,8 +406,8 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
         a.count = count; a.s16 = L.s16; a.first_elem = first_elem; a.mask = P->mask; a.T = P->T; a.rk = rk;
         for (int t = 0; t < P->T; ++t)
             a.atom[t] = GenAtomDev{P->atoms[t].c, P->atoms[t].beta, L.bt_root[t], L.bt_cw[t], L.bt_vb[t], P->atoms[t].k, P->atoms[t].is_theta};
-        const int grid = grid_for(tiles * P->T, kGenThreads);
-        rc = launch(k_gen_bit, grid, kGenThreads, kAesSmemBytes, st, a);
+        const int th = threads_for(tiles * P->T, kGenThreads), grid = grid_for(tiles * P->T, th);
+        rc = launch(k_gen_bit, grid, th, kAesSmemBytes, st, a);
         if (rc) return rc;
     }
     if (!P->variant && P->has_lut && (parts & FUSEFSS_GEN_LUT)) {
@@ -390,8 +417,8 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
         a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel; a.first_elem = first_elem; a.mask = P->mask;
         a.n = (int)P->n; a.m = (int)P->m; a.M = P->M; a.rk = rk;
         a.xpoly = (int)P->xpoly; a.polys = (int)P->r; a.d = (int)P->d;
-        const int grid = grid_for(tiles * (size_t)(P->M - 1), kGenThreads);
-        rc = launch_gen_vec_p(P->p, grid, kGenThreads, st, a);
+        const int th = threads_for(tiles * (size_t)(P->M - 1), kGenThreads), grid = grid_for(tiles * (size_t)(P->M - 1), th);
+        rc = launch_gen_vec_p(P->p, grid, th, st, a);
         if (rc) return rc;
     }
     if (parts & FUSEFSS_GEN_SHARES) {
@@ -412,8 +439,8 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
         for (int t = 0; t < a.n_kb_spec; ++t) { a.kb_kind[t] = P->kappa_b[t].kind; a.kb_arg[t] = P->kappa_b[t].arg; }
         for (int t = 0; t < a.T; ++t)
             a.atom[t] = GenAtomDev{P->atoms[t].c, P->atoms[t].beta, 0, 0, 0, P->atoms[t].k, P->atoms[t].is_theta};
-        const int grid = grid_for(tiles, kGenThreads);
-        rc = launch(k_gen_misc, grid, kGenThreads, kAesSmemBytes, st, a);
+        const int th = threads_for(tiles, kGenThreads), grid = grid_for(tiles, th);
+        rc = launch(k_gen_misc, grid, th, kAesSmemBytes, st, a);
         if (rc) return rc;
     }
     return 0;
@@ -436,8 +463,8 @@ int fusefss_eval_cmp(int party, const fusefss_program *prog, const void *key_dev
     a.G = pick_groups(count, P->T, g_eval_threads);
     for (int t = 0; t < P->T; ++t) a.atom[t] = CmpAtomDev{P->atoms[t].c, L.bt_root[t], L.bt_cw[t], L.bt_vb[t], P->atoms[t].k, 0};
     if (a.G > 1) CU(cudaMemsetAsync(bits_out_dev, 0, count * 8, st));
-    const int grid = grid_for(((count + 31) / 32) * (size_t)a.G, g_eval_threads);
-    return launch(k_eval_cmp, grid, g_eval_threads, kAesSmemBytes, st, a);
+    const int th = threads_for(((count + 31) / 32) * (size_t)a.G, g_eval_threads), grid = grid_for(((count + 31) / 32) * (size_t)a.G, th);
+    return launch(k_eval_cmp, grid, th, kAesSmemBytes, st, a);
 }
 
 int fusefss_eval_lut(int party, const fusefss_program *prog, const void *key_dev, const uint64_t *xhat_dev, size_t count,
@@ -458,8 +485,8 @@ int fusefss_eval_lut(int party, const fusefss_program *prog, const void *key_dev
     a.mask = P->mask; a.n = (int)P->n; a.M = P->M; a.party = party;
     a.G = pick_groups(count, P->M - 1, g_eval_threads);
     if (a.G > 1) CU(cudaMemsetAsync(coeff_out_dev, 0, count * 8 * (size_t)P->p, st));
-    const int grid = grid_for(((count + 31) / 32) * (size_t)a.G, g_eval_threads);
-    rc = launch_eval_lut_p(P->p, grid, g_eval_threads, st, a);
+    const int th = threads_for(((count + 31) / 32) * (size_t)a.G, g_eval_threads), grid = grid_for(((count + 31) / 32) * (size_t)a.G, th);
+    rc = launch_eval_lut_p(P->p, grid, th, st, a);
     if (rc) return rc;
     if (a.G > 1 && P->n < 64) {
         const size_t words = count * (size_t)P->p;
