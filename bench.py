@@ -429,6 +429,25 @@ def main():
                        "d2h_bytes_per_step": d2h, "api": "fusefss_gate_host (pinned host buffers, chunk=%d)" % e2e_chunk}
         # sanity: the e2e outputs reconstruct (first elements) -- not timed
         line["e2e"]["checksum_y"] = int((hy[0][0, :4] + hy[1][0, :4]).sum().item()) & 0xFFFFFFFF
+        if not args.no_sp:                                              # the same public call on the variant-1 program
+            Psp = F.Program(specs.shared_prefix(spec))
+            sp_chunk = min(count, 1 << 20)
+            ws2 = torch.empty(Psp.workspace_bytes(sp_chunk), dtype=torch.uint8, device="cuda")
+
+            def e2e_sp():
+                F._check(F.lib.fusefss_gate_host(Psp._h, h_rin.data_ptr(), h_rout.data_ptr(), h_xhat.data_ptr(), 0, count, sp_chunk,
+                                                 ws2.data_ptr(), hy[0].data_ptr(), hy[1].data_ptr(), hz[0].data_ptr(), hz[1].data_ptr(),
+                                                 torch.cuda.current_stream().cuda_stream))
+            e2e_sp()
+            barrier()
+            t0 = time.perf_counter()
+            for _ in range(args.steps):
+                e2e_sp()
+            barrier()
+            dt2 = _allmax(time.perf_counter() - t0)
+            line["shared_prefix"]["e2e"] = {"value": world * count * args.steps / dt2, "unit": "elements/s", "h2d_bytes_per_step": h2d,
+                                            "d2h_bytes_per_step": d2h, "api": "fusefss_gate_host (pinned host buffers, chunk=%d)" % sp_chunk,
+                                            "checksum_y": int((hy[0][0, :4] + hy[1][0, :4]).sum().item()) & 0xFFFFFFFF}
     if rank == 0 and not args.no_cpu and world >= 1:
         v, extra = cpu_oracle_rate(name, args.cpu_sample)
         line["cpu_baseline"] = {"value": v, "unit": "elements/s", "cores": 1, "kind": "oracle",
