@@ -81,6 +81,34 @@ __device__ __forceinline__ void sp_walk2(uint32_t tl, const uint8_t *lvl, size_t
         u1 <<= 1; u2 <<= 1;
     }
 }
+// The two candidate prefixes u1, u2 of a cluster (top kf bits) usually differ only in their last few bits: walk u1
+// once, snapshot the state at the level where u2 leaves u1's path (per lane), then walk u2's few remaining levels.
+// On return a / b = the states after kf levels along u1 / u2 (b = a when the prefixes are equal).
+template <int PK>
+__device__ __forceinline__ void sp_walk_fork(uint32_t tl, const uint8_t *lvl, size_t e, size_t s16, size_t s8, size_t lvl_stride,
+                                             int kf, uint64_t u1, uint64_t u2, SpState<PK> &a, SpState<PK> &b) {
+    const uint64_t diff = (u1 ^ u2) >> (64 - kf);
+    const int ldiv = diff ? kf - (64 - __clzll((long long)diff)) : kf;       // first level at which the prefixes differ
+    const uint8_t *pl = lvl;
+    uint64_t ub = u1;
+    for (int i = 0; i < kf; ++i, pl += lvl_stride) {
+        if (i == ldiv) b = a;
+        uint4 cw; uint64_t vcw[PK];
+        sp_load_level<PK>(pl, e, s16, s8, cw, vcw);
+        sp_step<PK>(tl, cw, vcw, (uint32_t)(ub >> 63), a);
+        ub <<= 1;
+    }
+    if (ldiv >= kf) { b = a; return; }
+    ub = u2 << ldiv;
+    pl = lvl + (size_t)ldiv * lvl_stride;
+    for (int i = ldiv; i < kf; ++i, pl += lvl_stride) {                       // per-lane trip count (expected ~2 levels)
+        uint4 cw; uint64_t vcw[PK];
+        sp_load_level<PK>(pl, e, s16, s8, cw, vcw);
+        sp_step<PK>(tl, cw, vcw, (uint32_t)(ub >> 63), b);
+        ub <<= 1;
+    }
+}
+
 // leaf: A = (-1)^party (V + conv(s) + t * fin)
 template <int PK>
 __device__ __forceinline__ void sp_leaf(uint32_t tl, const SpState<PK> &st, const uint8_t *fin, size_t e, size_t s8, int party, uint64_t (&A)[PK]) {
@@ -200,7 +228,7 @@ __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ Eva
                 if (share) {
                     const uint64_t uf = ((xh + pts[cl.first].delta) & a.mask) << (64 - n);
                     const uint64_t ul = ((xh + pts[cl.first + cl.count - 1].delta) & a.mask) << (64 - n);
-                    sp_walk2<PK>(tl, lvl, e, a.s16, a.s8, a.lvl_stride, kf, uf, ul, s1, s2);
+                    sp_walk_fork<PK>(tl, lvl, e, a.s16, a.s8, a.lvl_stride, kf, uf, ul, s1, s2);
                     pre1 = uf >> (64 - kf);
                 }
                 for (int j = cl.first + g; j < cl.first + cl.count; j += a.G) {

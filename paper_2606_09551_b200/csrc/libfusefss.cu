@@ -325,7 +325,9 @@ int fusefss_cost(const fusefss_program *prog, fusefss_cost_t *out) {
             for (const SpCluster &cl : P->sp.clusters) {                       // fused walk: every point of the n-bit tree
                 const uint64_t kf = n - (uint64_t)cl.tail_bits;
                 const bool share = cl.count > 1 && kf > 0;
-                const uint64_t levels = share ? 2 * kf + (uint64_t)cl.count * (uint64_t)cl.tail_bits : (uint64_t)cl.count * n;
+                // the shared prefix is counted once: the few levels re-walked where the cluster's second prefix forks
+                // off (data dependent, ~2 per straddling lane) are overhead, not algorithmic work
+                const uint64_t levels = share ? kf + (uint64_t)cl.count * (uint64_t)cl.tail_bits : (uint64_t)cl.count * n;
                 const uint64_t qk = ((uint64_t)P->sp.pk + 1) / 2;
                 c.eval_lut_aes += (1 + qk) * levels + qk * (uint64_t)cl.count; c.eval_lut_lookups += levels * grp(1 + qk) + grp(qk) * (uint64_t)cl.count;
             }
