@@ -128,6 +128,7 @@ def measure_shared_prefix(F, torch, name, base_spec, inp, rank, world, steps, wa
     P = F.Program(spec)
     sh, cost = P.shape, P.cost()
     count = int(inp["xhat"].size)
+    torch.cuda.empty_cache()
     free_b, _ = torch.cuda.mem_get_info()
     if 2 * P.key_bytes(count) + 8 * count * (8 + 2 * sh["p"]) > 0.85 * free_b:
         return {"skipped": "variant-1 keys of the whole tensor do not fit resident"}

@@ -200,32 +200,69 @@ def test_gate_host_end_to_end(F, orc):
     assert np.array_equal(z0, exp["z"][0]) and np.array_equal(z1, exp["z"][1])
 
 
-def test_full_size_sampled(F, orc):
-    """Config 2 at its full size (128 x 3072) in the launch configuration bench.py times: the oracle recomputes a
-    sample of elements one by one (its keygen is per-element deterministic in the global index), and the
-    reconstruction property is checked on every element on the device."""
+FULL = [("relu16", 0), ("relu16", 1), ("gelu", 0), ("gelu", 1), ("gelu", 5), ("nexp", 0), ("nexp", 1), ("recip", 0), ("recip", 1),
+        ("shift_relu", 0), ("shift_relu", 1), ("rsqrt", 0), ("rsqrt", 3), ("silu", 0), ("silu", 1)]
+
+
+@pytest.mark.parametrize("name,variant", FULL)
+def test_full_size_sampled(F, orc, name, variant):
+    """Every BASELINE.json config at its FULL size in the launch configuration bench.py times (keygen in its three
+    parts, one eval per party -- fused for variant 1 --, post_fused; config 5 / variant 0 as one 704,512-element chunk
+    at a non-zero global offset, as in the chunked run).  The oracle recomputes a sample of elements one by one
+    (its keygen is deterministic in the GLOBAL element index), and the reconstruction property G(x) is checked on a
+    20,000-element prefix."""
+    import gc
     import torch
-    spec = specs.CONFIGS["gelu"]()
-    count = tensors.FULL_COUNT["gelu"]
-    inp = tensors.inputs("gelu", spec, count=count, seed=0)
+    gc.collect()
+    torch.cuda.empty_cache()                                  # the big configs need most of the 180 GB
+    spec = specs.CONFIGS[name]()
+    if variant & 1:
+        spec = specs.shared_prefix(spec)
+    if variant & 2:
+        spec = specs.input_masked_mul(spec)
+    if variant & 4:
+        spec = specs.public_point_horner(spec)
+    count = tensors.FULL_COUNT[name]
+    first = 0
+    if name == "silu" and not variant & 1:                    # does not fit resident: bench.py streams chunks of this size
+        first, count = 3 * 704512, 704512
+    inp = tensors.inputs(name, spec, count=first + count if first else count, seed=0)
+    sl = slice(first, first + count)
+    x, r_in, r_out, xhat = inp["x"][sl], inp["r_in"][sl], np.ascontiguousarray(inp["r_out"][:, sl]), inp["xhat"][sl]
     P, O = F.Program(spec), orc.Program(spec)
-    k0, k1 = P.keygen(dev(inp["r_in"]), dev(inp["r_out"]), seed=0)
-    xh = dev(inp["xhat"])
-    bits = [P.eval_cmp(b, (k0, k1)[b], xh) for b in (0, 1)]
-    coeff = [P.eval_lut(b, (k0, k1)[b], xh) for b in (0, 1)]
+    keys = P.alloc_keys(count)
+    for parts in (1, 2, 4):
+        P.keygen(dev(r_in), dev(r_out), 0, first, keys=keys, parts=parts)
+    k0, k1 = keys
+    xh = dev(xhat)
+    T, lut = P.shape["T"], P.shape["has_lut"]
+    if variant & 1:
+        ev = [P.eval_fused(b, (k0, k1)[b], xh) for b in (0, 1)]
+        bits, coeff = [ev[0][0], ev[1][0]], [ev[0][1], ev[1][1]]
+    else:
+        bits = [P.eval_cmp(b, (k0, k1)[b], xh) if T else None for b in (0, 1)]
+        coeff = [P.eval_lut(b, (k0, k1)[b], xh) if lut else None for b in (0, 1)]
     y0, y1, z0, z1 = P.post_fused(k0, k1, xh, bits[0], bits[1], coeff[0], coeff[1])
     torch.cuda.synchronize()
     rng = np.random.default_rng(1)
-    idx = np.concatenate([[0, 31, 32, count - 1], rng.integers(0, count, 60)])
+    n_s = 24 if name == "silu" else 40
+    idx = np.unique(np.concatenate([[0, 31, 32, count - 1, count - 33], rng.integers(0, count, n_s)]))
+    idx = idx[(idx >= 0) & (idx < count)]
     for e in idx:
         e = int(e)
-        ok0, ok1 = O.keygen(inp["r_in"][e:e + 1], inp["r_out"][:, e:e + 1], 0, first_elem=e)
-        exp = O.run_gate(ok0, ok1, inp["xhat"][e:e + 1])
+        ok0, ok1 = O.keygen(r_in[e:e + 1], r_out[:, e:e + 1], 0, first_elem=first + e)
+        exp = O.run_gate(ok0, ok1, xhat[e:e + 1])
         for b, (bb, cc, yy, zz) in enumerate(((bits[0], coeff[0], y0, z0), (bits[1], coeff[1], y1, z1))):
-            assert host(bb[e:e + 1])[0] == exp["bits"][b][0]
-            assert np.array_equal(host(cc[:, e:e + 1].contiguous())[:, 0], exp["coeff"][b][:, 0])
-            assert host(yy[0, e:e + 1])[0] == exp["y"][b][0, 0] and host(zz[e:e + 1])[0] == exp["z"][b][0]
-    # property at full size: shares reconstruct to the plaintext spline for every element
-    ye, ze = O.plain_G(inp["x"][:20000], inp["r_in"][:20000])
-    assert np.array_equal((host(y0)[0, :20000] + host(y1)[0, :20000]), ye[0])
-    assert np.array_equal(host(z0)[:20000] ^ host(z1)[:20000], pack_bits(ze))
+            if T:
+                assert host(bb[e:e + 1])[0] == exp["bits"][b][0], (name, variant, e)
+            if lut:
+                assert np.array_equal(host(cc[:, e:e + 1].contiguous())[:, 0], exp["coeff"][b][:, 0]), (name, variant, e)
+            assert host(yy[0, e:e + 1])[0] == exp["y"][b][0, 0], (name, variant, e)
+            if P.shape["n_out_b"]:
+                assert host(zz[e:e + 1])[0] == exp["z"][b][0], (name, variant, e)
+    # property at full size: shares reconstruct to the plaintext operator on a prefix
+    k = min(20000, count)
+    ye, ze = O.plain_G(x[:k], r_in[:k])
+    assert np.array_equal((host(y0)[0, :k] + host(y1)[0, :k]) & mask_of(spec.n), ye[0])
+    if P.shape["n_out_b"]:
+        assert np.array_equal(host(z0)[:k] ^ host(z1)[:k], pack_bits(ze))
