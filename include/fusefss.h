@@ -169,6 +169,23 @@ int fusefss_post_fused(const fusefss_program *prog, const void *key0_dev, const 
                        const uint64_t *coeff0_dev, const uint64_t *coeff1_dev, size_t count,
                        uint64_t *y0_dev, uint64_t *y1_dev, uint64_t *z0_dev, uint64_t *z1_dev, void *stream);
 
+/* ---- vector-block glue (App. G: blocks = linear ops on shares + compiled scalar gates) ----------
+ * fusefss_share_open: Protocol 1 for the input of gate `prog`: xhat = (x_0 + [r_in]_0) + (x_1 + [r_in]_1),
+ *   the [r_in] shares are read from the two key buffers generated for these `count` elements (n/8 bytes per party).
+ * fusefss_row_sum: out[r] = sum_c in[r*cols + c] mod 2^n, local on additive shares.
+ * fusefss_mul_keygen / fusefss_mul_fused: element-wise Beaver products z = x * y (formulas DESIGN 4.6) with y
+ *   broadcast over `cols` consecutive elements (cols = 1: plain element-wise; y has count/cols entries); the dealer's
+ *   triples (fusefss_mul_triple_bytes(count) per party) come from R(e, 0xA000..0xA002); both parties in one launch,
+ *   2n/8 online bytes per party per product. */
+int fusefss_share_open(const fusefss_program *prog, const void *key0_dev, const void *key1_dev, const uint64_t *x0_dev,
+                       const uint64_t *x1_dev, size_t count, uint64_t *xhat_out_dev, void *stream);
+int fusefss_row_sum(uint32_t n_bits, const uint64_t *in_dev, size_t rows, size_t cols, uint64_t *out_dev, void *stream);
+size_t fusefss_mul_triple_bytes(size_t count);
+int fusefss_mul_keygen(uint32_t n_bits, uint64_t seed, uint64_t first_elem, size_t count, void *t0_dev, void *t1_dev, void *stream);
+int fusefss_mul_fused(uint32_t n_bits, const uint64_t *x0_dev, const uint64_t *x1_dev, const uint64_t *y0_dev,
+                      const uint64_t *y1_dev, const void *t0_dev, const void *t1_dev, size_t count, size_t cols,
+                      uint64_t *z0_dev, uint64_t *z1_dev, void *stream);
+
 /* ---- end-to-end convenience: HOST buffers in, HOST buffers out (bench.py's e2e leg) ---------------
  * Copies r_in/r_out/xhat to the device, runs keygen + both parties' eval_cmp/eval_lut + post_fused in chunks of
  * `chunk` elements using the caller's device workspace, copies y0,y1 [n_out_a][count] and z0,z1 [count] back.

@@ -194,6 +194,11 @@ class Program:
         outs = [self.post(b, keys[b], xhat, bits[b], coeff[b], R, msg[1 - b], msg[b]) for b in (0, 1)]
         return dict(bits=bits, coeff=coeff, msg=msg, y=[outs[0][0], outs[1][0]], z=[outs[0][1], outs[1][1]])
 
+    def rin_shares(self, key, count):
+        out = np.zeros(count, np.uint64)
+        lib().orc_rin_shares(C.c_void_p(self._p), _p(key), C.c_size_t(count), _p(out))
+        return out
+
     # ---- Tier A -------------------------------------------------------------------------------
     def plain_G(self, x, r):
         x = _u64(x)
@@ -244,6 +249,13 @@ def dcf_vec_pair(k, n, p, alpha, beta, seed0: bytes, seed1: bytes, us):
     o1 = np.zeros((us.size, p), np.uint64)
     lib().orc_dcf_vec_pair(k, n, p, C.c_uint64(alpha), _p(beta), seed0, seed1, _p(us), us.size, _p(o0), _p(o1))
     return o0, o1
+
+
+def dealer_rand(seed, first, count, slot):
+    lo = np.zeros(count, np.uint64)
+    hi = np.zeros(count, np.uint64)
+    lib().orc_dealer_rand(C.c_uint64(seed), C.c_uint64(first), C.c_size_t(count), C.c_uint64(slot), _p(lo), _p(hi))
+    return lo, hi
 
 
 def protocol3(n, alpha_interior, r):

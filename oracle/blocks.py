@@ -1,0 +1,63 @@
+"""Oracle composition of the softmax vector block (TEST INFRASTRUCTURE; App. G):
+e_i = nExp(x_i) -> truncate -> s = sum_i e_i -> t = Recip(s) -> truncate -> y_i = e_i * t (Beaver) -> truncate.
+Every scalar gate is the oracle's own Program (keygen, the two FSS calls, post-processing); the linear steps and
+the Beaver product are written out in numpy.  The max reduction is not part of the method: inputs are
+max-subtracted scores."""
+from __future__ import annotations
+
+import numpy as np
+
+import oracle
+
+SLOT_MUL_AB, SLOT_MUL_AB0, SLOT_MUL_C0 = 0xA000, 0xA001, 0xA002
+
+
+def gate(P, x0, x1, r_in, seed, first=0):
+    """One compiled gate on additively shared inputs: Protocol 1 (masked opening), then the online procedure."""
+    count = x0.size
+    k0, k1 = P.keygen(r_in, None, seed, first)
+    xhat = x0 + P.rin_shares(k0, count) + x1 + P.rin_shares(k1, count)          # n = 64: wraps mod 2^64
+    out = P.run_gate(k0, k1, xhat)
+    return out["y"][0][0], out["y"][1][0], xhat
+
+
+def beaver_mul(x0, x1, y0, y1, cols, seed, first=0):
+    """z = x * y with y broadcast over `cols` consecutive elements; triples from R(e, 0xA000..)."""
+    count = x0.size
+    a, b = oracle.dealer_rand(seed, first, count, SLOT_MUL_AB)
+    a0, b0 = oracle.dealer_rand(seed, first, count, SLOT_MUL_AB0)
+    c0, _ = oracle.dealer_rand(seed, first, count, SLOT_MUL_C0)
+    c = a * b
+    a1, b1, c1 = a - a0, b - b0, c - c0
+    yi = np.arange(count) // cols
+    E = (x0 - a0) + (x1 - a1)
+    Fv = (y0[yi] - b0) + (y1[yi] - b1)
+    return E * Fv + E * b0 + Fv * a0 + c0, E * b1 + Fv * a1 + c1
+
+
+def softmax(progs, x0, x1, masks, rows, cols, seed):
+    """progs / masks: dicts with the stages 'nexp', 'tr_e', 'recip', 'tr_t', 'tr_y' (oracle Programs / r_in arrays)."""
+    with np.errstate(over="ignore"):
+        e0, e1, _ = gate(progs["nexp"], x0, x1, masks["nexp"], seed + 1)
+        f0, f1, _ = gate(progs["tr_e"], e0, e1, masks["tr_e"], seed + 2)
+        s0, s1 = f0.reshape(rows, cols).sum(axis=1, dtype=np.uint64), f1.reshape(rows, cols).sum(axis=1, dtype=np.uint64)
+        t0, t1, _ = gate(progs["recip"], s0, s1, masks["recip"], seed + 3)
+        u0, u1, _ = gate(progs["tr_t"], t0, t1, masks["tr_t"], seed + 4)
+        p0, p1 = beaver_mul(f0, f1, u0, u1, cols, seed + 5)
+        y0, y1, _ = gate(progs["tr_y"], p0, p1, masks["tr_y"], seed + 6)
+    return dict(e=(e0, e1), f=(f0, f1), s=(s0, s1), t=(t0, t1), u=(u0, u1), p=(p0, p1), y=(y0, y1))
+
+
+def softmax_plain(progs, x, rows, cols):
+    """Tier A: the same pipeline on cleartext fixed-point values (exact integer semantics of every stage)."""
+    z = np.zeros(x.size, np.uint64)
+    with np.errstate(over="ignore"):
+        e = progs["nexp"].plain_G(x, z)[0][0]
+        f = progs["tr_e"].plain_G(e, z)[0][0]
+        s = f.reshape(rows, cols).sum(axis=1, dtype=np.uint64)
+        zr = np.zeros(rows, np.uint64)
+        t = progs["recip"].plain_G(s, zr)[0][0]
+        u = progs["tr_t"].plain_G(t, zr)[0][0]
+        p = f * np.repeat(u, cols)
+        y = progs["tr_y"].plain_G(p, z)[0][0]
+    return dict(e=e, f=f, s=s, t=t, u=u, p=p, y=y)

@@ -1523,3 +1523,23 @@ void orc_post(int party, const orc_prog *P, const u8 *key, const u64 *xhat, cons
     }
     free(A); free(Bv);
 }
+
+/* ------------------------------------------------------------------------- */
+/* 13. Dealer randomness for the vector-block glue (oracle/blocks.py):         */
+/*     lo/hi words of R(e, slot), e = first .. first+count-1 (DESIGN 4.5)      */
+/* ------------------------------------------------------------------------- */
+void orc_dealer_rand(u64 seed, u64 first, size_t count, u64 slot, u64 *lo, u64 *hi)
+{
+    aes_ks ks; seed_ks(seed, &ks);
+    for (size_t i = 0; i < count; i++) {
+        u8 rb[16];
+        rnd(&ks, first + i, slot, rb);
+        lo[i] = le64(rb); hi[i] = le64(rb + 8);
+    }
+}
+/* [r_in] share of element e in a key buffer (for Protocol 1 in the block composition) */
+void orc_rin_shares(const orc_prog *P, const u8 *key, size_t count, u64 *out)
+{
+    layout_t L; layout(P, count, &L);
+    for (size_t e = 0; e < count; e++) out[e] = ld8(key, L.rin, e);
+}

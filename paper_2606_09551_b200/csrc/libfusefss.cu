@@ -12,6 +12,7 @@
 #include "eval_sp.cuh"
 #include "keygen.cuh"
 #include "post.cuh"
+#include "blocks.cuh"
 
 namespace fsk {
 namespace {
@@ -566,6 +567,50 @@ int fusefss_post_fused(const fusefss_program *prog, const void *key0_dev, const 
     a.y_out[0] = y0_dev; a.y_out[1] = y1_dev; a.z_out[0] = z0_dev; a.z_out[1] = z1_dev;
     a.count = count; a.mask = P->mask; a.k = post_offsets(L);
     return launch(k_post_fused, (int)((count + 255) / 256), 256, 0, (cudaStream_t)stream, a);
+}
+
+// ---- vector-block glue (App. G) -------------------------------------------
+int fusefss_share_open(const fusefss_program *prog, const void *key0_dev, const void *key1_dev, const uint64_t *x0_dev,
+                       const uint64_t *x1_dev, size_t count, uint64_t *xhat_out_dev, void *stream) {
+    const Program *P = prog_of(prog);
+    if (!P || !key0_dev || !key1_dev || !x0_dev || !x1_dev || !xhat_out_dev) return FUSEFSS_E_NULL;
+    if (count == 0) return FUSEFSS_E_COUNT;
+    Layout L; compute_layout(*P, count, &L);
+    OpenArgs a{x0_dev, x1_dev, (const uint8_t *)key0_dev, (const uint8_t *)key1_dev, L.rin, count, P->mask, xhat_out_dev};
+    return launch(k_share_open, (int)((count + 255) / 256), 256, 0, (cudaStream_t)stream, a);
+}
+
+int fusefss_row_sum(uint32_t n_bits, const uint64_t *in_dev, size_t rows, size_t cols, uint64_t *out_dev, void *stream) {
+    if (!in_dev || !out_dev) return FUSEFSS_E_NULL;
+    if (rows == 0 || cols == 0) return FUSEFSS_E_COUNT;
+    if (n_bits < 1 || n_bits > 64) return FUSEFSS_E_SPEC;
+    RowSumArgs a{in_dev, out_dev, rows, cols, n_bits >= 64 ? ~0ull : ((1ull << n_bits) - 1ull)};
+    return launch(k_row_sum, (int)((rows * 32 + 255) / 256), 256, 0, (cudaStream_t)stream, a);
+}
+
+size_t fusefss_mul_triple_bytes(size_t count) { return 3 * ((count * 8 + 255) & ~(size_t)255); }
+
+int fusefss_mul_keygen(uint32_t n_bits, uint64_t seed, uint64_t first_elem, size_t count, void *t0_dev, void *t1_dev, void *stream) {
+    if (!t0_dev || !t1_dev) return FUSEFSS_E_NULL;
+    if (count == 0) return FUSEFSS_E_COUNT;
+    if (n_bits < 1 || n_bits > 64) return FUSEFSS_E_SPEC;
+    int rc = init_device(); if (rc) return rc;
+    MulGenArgs a{};
+    a.t0 = (uint8_t *)t0_dev; a.t1 = (uint8_t *)t1_dev; a.count = count; a.s8 = (count * 8 + 255) & ~(size_t)255;
+    a.first_elem = first_elem; a.mask = n_bits >= 64 ? ~0ull : ((1ull << n_bits) - 1ull); a.rk = seed_round_keys(seed);
+    const size_t tiles = (count + 31) / 32;
+    const int th = threads_for(tiles, kGenThreads);
+    return launch(k_mul_gen, grid_for(tiles, th), th, kAesSmemBytes, (cudaStream_t)stream, a);
+}
+
+int fusefss_mul_fused(uint32_t n_bits, const uint64_t *x0_dev, const uint64_t *x1_dev, const uint64_t *y0_dev, const uint64_t *y1_dev,
+                      const void *t0_dev, const void *t1_dev, size_t count, size_t cols, uint64_t *z0_dev, uint64_t *z1_dev, void *stream) {
+    if (!x0_dev || !x1_dev || !y0_dev || !y1_dev || !t0_dev || !t1_dev || !z0_dev || !z1_dev) return FUSEFSS_E_NULL;
+    if (count == 0 || cols == 0) return FUSEFSS_E_COUNT;
+    if (n_bits < 1 || n_bits > 64) return FUSEFSS_E_SPEC;
+    MulArgs a{x0_dev, x1_dev, y0_dev, y1_dev, (const uint8_t *)t0_dev, (const uint8_t *)t1_dev, z0_dev, z1_dev, count, cols,
+              (count * 8 + 255) & ~(size_t)255, n_bits >= 64 ? ~0ull : ((1ull << n_bits) - 1ull)};
+    return launch(k_mul_fused, (int)((count + 255) / 256), 256, 0, (cudaStream_t)stream, a);
 }
 
 // workspace: key0 | key1 | r_in | r_out[n_out_a] | xhat | bits0 | bits1 | coeff0[p] | coeff1[p] | y0 | y1 [n_out_a] | z0 | z1
