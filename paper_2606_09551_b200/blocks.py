@@ -1,0 +1,96 @@
+"""Vector blocks composed from compiled gates (App. G).
+
+softmax over max-subtracted scores:  e = nExp(x) -> truncate -> s = sum_i e_i -> t = Recip(s) -> truncate ->
+y_i = e_i * t (Beaver) -> truncate.  The max reduction is not compiled by the method and is not here.
+This module only ORCHESTRATES C-ABI calls (argument marshalling): every step -- masked openings, the gates'
+keygen / FSS evaluation / post-processing, row sums, Beaver products -- runs in libfusefss kernels.
+Both parties run on one GPU; the bytes they would exchange are counted.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+from . import Program, _check, _ptr, _stream, lib
+
+STAGES = ("nexp", "tr_e", "recip", "tr_t", "tr_y")
+
+
+def softmax_specs(variant: int = 3, n: int = 64, f: int = 12):
+    """Gate types of the block: nExp (out scale 2f+8), arithmetic shifts by 20 / 28 / 24 bits (as shift+ReLU gates:
+    every value here is non-negative), Recip (out scale 3f+16).  Scales: e at 32 -> 12; t at 52 -> 24; e*t at 36 -> 12."""
+    from workloads import specs as S
+    mk = {"nexp": S.nexp(n, f), "tr_e": S.shift_relu(n, 20), "recip": S.recip(n, f), "tr_t": S.shift_relu(n, 28),
+          "tr_y": S.shift_relu(n, 24)}
+    out = {}
+    for k, s in mk.items():
+        if variant & 1:
+            s = S.shared_prefix(s)
+        if variant & 2:
+            s = S.input_masked_mul(s)
+        if variant & 4:
+            s = S.public_point_horner(s)
+        out[k] = s
+    return out
+
+
+class Softmax:
+    """rows x cols block.  `keygen(masks, seed)` is the dealer; `run(x0, x1)` the online phase of both parties."""
+
+    def __init__(self, rows: int, cols: int, variant: int = 3):
+        import torch
+        self.rows, self.cols, self.N = rows, cols, rows * cols
+        self.specs = softmax_specs(variant)
+        self.progs = {k: Program(s) for k, s in self.specs.items()}
+        self.n = 64
+        self.counts = {"nexp": self.N, "tr_e": self.N, "recip": rows, "tr_t": rows, "tr_y": self.N}
+        self.keys = {k: self.progs[k].alloc_keys(c) for k, c in self.counts.items()}
+        tb = lib.fusefss_mul_triple_bytes(self.N)
+        self.triples = (torch.empty(tb, dtype=torch.uint8, device="cuda"), torch.empty(tb, dtype=torch.uint8, device="cuda"))
+        i64 = lambda *shape: torch.empty(shape, dtype=torch.int64, device="cuda")
+        self.buf = {k: dict(xhat=i64(c), bits=[i64(c), i64(c)], coeff=[i64(self.progs[k].shape["p"], c) for _ in (0, 1)],
+                            out=(i64(1, c), i64(1, c), i64(c), i64(c))) for k, c in self.counts.items()}
+        self.s = [i64(rows), i64(rows)]
+        self.prod = [i64(self.N), i64(self.N)]
+
+    # ---- dealer ----------------------------------------------------------------------------------
+    def keygen(self, masks, seed: int):
+        """masks[stage] = device uint64 tensor of fresh input masks r_in for that gate instance."""
+        for i, k in enumerate(STAGES):
+            st_seed = seed + (1, 2, 3, 4, 6)[i]
+            self.progs[k].keygen(masks[k], None, st_seed, 0, keys=self.keys[k])
+        _check(lib.fusefss_mul_keygen(self.n, seed + 5, 0, self.N, _ptr(self.triples[0]), _ptr(self.triples[1]), _stream()))
+
+    # ---- online ----------------------------------------------------------------------------------
+    def _gate(self, k, x0, x1):
+        P, (k0, k1), b, c = self.progs[k], self.keys[k], self.buf[k], self.counts[k]
+        _check(lib.fusefss_share_open(P._h, _ptr(k0), _ptr(k1), _ptr(x0), _ptr(x1), c, _ptr(b["xhat"]), _stream()))
+        for party, key in ((0, k0), (1, k1)):
+            P.eval_fused(party, key, b["xhat"], b["bits"][party] if P.shape["T"] else None,
+                         b["coeff"][party] if P.shape["has_lut"] else None)
+        y0, y1, _, _ = P.post_fused(k0, k1, b["xhat"], b["bits"][0], b["bits"][1], b["coeff"][0], b["coeff"][1], outs=b["out"])
+        return y0[0], y1[0]
+
+    def run(self, x0, x1):
+        """x0, x1: additive shares [rows*cols] of the max-subtracted scores at scale 2^12.  Returns shares of softmax at 2^12."""
+        e0, e1 = self._gate("nexp", x0, x1)
+        f0, f1 = self._gate("tr_e", e0, e1)
+        for b, fb in ((0, f0), (1, f1)):
+            _check(lib.fusefss_row_sum(self.n, _ptr(fb), self.rows, self.cols, _ptr(self.s[b]), _stream()))
+        t0, t1 = self._gate("recip", self.s[0], self.s[1])
+        u0, u1 = self._gate("tr_t", t0, t1)
+        _check(lib.fusefss_mul_fused(self.n, _ptr(f0), _ptr(f1), _ptr(u0), _ptr(u1), _ptr(self.triples[0]), _ptr(self.triples[1]),
+                                     self.N, self.cols, _ptr(self.prod[0]), _ptr(self.prod[1]), _stream()))
+        y0, y1 = self._gate("tr_y", self.prod[0], self.prod[1])
+        return dict(e=(e0, e1), f=(f0, f1), s=tuple(self.s), t=(t0, t1), u=(u0, u1), p=tuple(self.prod), y=(y0, y1))
+
+    # ---- accounting ------------------------------------------------------------------------------
+    def online_bytes_per_party(self) -> int:
+        """openings of every gate input + the gates' own post-processing messages + 2 ring elements per Beaver product"""
+        total = sum(self.progs[k].online_bits() // 8 * c for k, c in self.counts.items())
+        return total + 16 * self.N
+
+    def key_bytes_per_party(self) -> int:
+        return sum(self.progs[k].key_bytes(c) for k, c in self.counts.items()) + lib.fusefss_mul_triple_bytes(self.N)
+
+    def rounds(self) -> int:
+        return sum(1 + self.progs[k].post_rounds() for k in STAGES) + 1

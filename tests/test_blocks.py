@@ -1,0 +1,74 @@
+"""Softmax vector block composed from compiled gates (App. G).
+CPU: the oracle composition (oracle/blocks.py) reconstructs, stage by stage, the plaintext fixed-point pipeline,
+and that pipeline approximates the real softmax within a stated bound.  GPU: the library's block
+(paper_2606_09551_b200/blocks.py: C-ABI calls only) matches the oracle composition share for share."""
+import numpy as np
+import pytest
+
+from workloads import specs
+
+
+def _specs(variant):
+    mk = {"nexp": specs.nexp(), "tr_e": specs.shift_relu(64, 20), "recip": specs.recip(), "tr_t": specs.shift_relu(64, 28),
+          "tr_y": specs.shift_relu(64, 24)}
+    out = {}
+    for k, s in mk.items():
+        if variant & 1:
+            s = specs.shared_prefix(s)
+        if variant & 2:
+            s = specs.input_masked_mul(s)
+        out[k] = s
+    return out
+
+
+def _inputs(rows, cols, seed):
+    rng = np.random.default_rng(seed)
+    xr = np.maximum(-20.0, -4.0 * rng.exponential(1.0, size=(rows, cols)))      # config 3: max-subtracted scores
+    xr[:, 0] = 0.0                                                               # the row maximum
+    x = np.floor(xr.reshape(-1) * 4096 + 0.5).astype(np.int64).view(np.uint64)
+    U = lambda k: rng.integers(0, 1 << 63, size=k, dtype=np.uint64) * np.uint64(2) + rng.integers(0, 2, size=k, dtype=np.uint64)
+    x0 = U(x.size)
+    masks = dict(nexp=U(x.size), tr_e=U(x.size), recip=U(rows), tr_t=U(rows), tr_y=U(x.size))
+    return xr, x, x0, x - x0, masks
+
+
+@pytest.mark.parametrize("variant", [0, 3])
+def test_oracle_block_reconstructs_plaintext_pipeline(orc, variant):
+    from oracle import blocks
+    rows, cols = 4, 24
+    progs = {k: orc.Program(s) for k, s in _specs(variant).items()}
+    xr, x, x0, x1, masks = _inputs(rows, cols, 3)
+    out = blocks.softmax(progs, x0, x1, masks, rows, cols, seed=100)
+    pl = blocks.softmax_plain(progs, x, rows, cols)
+    for k in ("e", "f", "s", "t", "u", "p", "y"):
+        assert np.array_equal(out[k][0] + out[k][1], pl[k]), k
+    y = pl["y"].astype(np.float64).reshape(rows, cols) / 4096.0
+    ref = np.exp(xr) / np.exp(xr).sum(axis=1, keepdims=True)
+    assert np.abs(y - ref).max() <= 2.0 ** -9                                    # stated bound of the fixed-point block
+    assert np.all(np.abs(y.sum(axis=1) - 1.0) <= 2.0 ** -7)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("variant,rows,cols", [(3, 5, 40), (0, 3, 33), (1, 12, 128)])
+def test_gpu_block_matches_oracle_composition(orc, variant, rows, cols):
+    import torch
+    import __graft_entry__ as g
+    g.build()
+    from oracle import blocks as oblocks
+    from paper_2606_09551_b200 import blocks as gblocks
+    assert torch.cuda.is_available()
+    xr, x, x0, x1, masks = _inputs(rows, cols, 7)
+    progs = {k: orc.Program(s) for k, s in _specs(variant).items()}
+    exp = oblocks.softmax(progs, x0, x1, masks, rows, cols, seed=40)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.int64)).cuda()
+    B = gblocks.Softmax(rows, cols, variant)
+    B.keygen({k: dev(v) for k, v in masks.items()}, seed=40)
+    got = B.run(dev(x0), dev(x1))
+    torch.cuda.synchronize()
+    host = lambda t: t.cpu().numpy().view(np.uint64).reshape(-1)
+    for k in ("e", "f", "s", "t", "u", "p", "y"):
+        for b in (0, 1):
+            assert np.array_equal(host(got[k][b]), exp[k][b]), (k, b)
+    pl = oblocks.softmax_plain(progs, x, rows, cols)
+    assert np.array_equal(host(got["y"][0]) + host(got["y"][1]), pl["y"])
+    assert B.rounds() > 0 and B.online_bytes_per_party() > 0 and B.key_bytes_per_party() > 0
