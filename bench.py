@@ -202,6 +202,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-sp", action="store_true", help="skip the variant-1 (shared-prefix) measurement")
+    ap.add_argument("--blocks", action="store_true", help="also time the softmax vector block (config 3 shape: 12 x 128 rows of 128)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     rank = int(os.environ.get("RANK", "0"))
@@ -399,6 +400,44 @@ def main():
             line["shared_prefix_public_horner"] = measure_shared_prefix(F, torch, name, spec, inp, rank, world, args.steps, args.warmup,
                                                                         barrier, lambda v: (float(_allmax(v))), xpoly=True)
         k0, k1 = None, None
+
+    # ---- softmax vector block built from compiled gates (NEXT-3; DESIGN 12) ---------------------------------
+    if args.blocks:
+        from paper_2606_09551_b200 import blocks as gblocks
+        rows, cols = 12 * 128, 128
+        rngb = np.random.default_rng(5)
+        xr = np.maximum(-20.0, -4.0 * rngb.exponential(1.0, size=(rows, cols))); xr[:, 0] = 0.0
+        xq = np.floor(xr.reshape(-1) * 4096 + 0.5).astype(np.int64).view(np.uint64)
+        U = lambda k: rngb.integers(0, 1 << 63, size=k, dtype=np.uint64) * np.uint64(2) + rngb.integers(0, 2, size=k, dtype=np.uint64)
+        x0h = U(xq.size)
+        masks = {k: dev(U(c)) for k, c in (("nexp", xq.size), ("tr_e", xq.size), ("recip", rows), ("tr_t", rows), ("tr_y", xq.size))}
+        blk = {}
+        for v in (3, 0):
+            B = gblocks.Softmax(rows, cols, v)
+            x0d, x1d = dev(x0h), dev(xq - x0h)
+            for _ in range(3):
+                B.keygen(masks, 9); out = B.run(x0d, x1d)
+            torch.cuda.synchronize()
+            eb = [ev() for _ in range(3)]
+            eb[0].record()
+            for _ in range(args.steps):
+                B.keygen(masks, 9)
+            eb[1].record()
+            for _ in range(args.steps):
+                out = B.run(x0d, x1d)
+            eb[2].record()
+            torch.cuda.synchronize()
+            y = (out["y"][0] + out["y"][1]).cpu().numpy().astype(np.float64).reshape(rows, cols) / 4096.0
+            ref = np.exp(xr) / np.exp(xr).sum(axis=1, keepdims=True)
+            blk["variant_%d" % v] = {"rows": rows, "cols": cols, "dealer_ms": eb[0].elapsed_time(eb[1]) / args.steps,
+                                     "online_ms": eb[1].elapsed_time(eb[2]) / args.steps,
+                                     "online_elems_per_s": rows * cols / (eb[1].elapsed_time(eb[2]) / args.steps * 1e-3),
+                                     "key_bytes_per_elem_per_party": B.key_bytes_per_party() / (rows * cols),
+                                     "online_bytes_per_elem_per_party": B.online_bytes_per_party() / (rows * cols), "rounds": B.rounds(),
+                                     "max_abs_err_vs_float_softmax": float(np.abs(y - ref).max())}
+            del B
+            torch.cuda.empty_cache()
+        line["softmax_block"] = blk
 
     # ---- e2e: the public host-buffer call, pinned host memory, H2D + D2H inside the timed region -------
     if not args.no_e2e:
