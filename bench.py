@@ -29,7 +29,15 @@ METRIC = "compiled-op elements/s (keygen + cmp+LUT eval both parties + post); al
 SM_CLOCK_MAX_MHZ = 1965.0
 LOOKUPS_PER_AES = 160           # 16 table lookups x 10 rounds (DESIGN 5.2)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` (profiles/r1c_gelu.md)
-NCU_TRAFFIC = {("gelu", 393216, "k_gen_vec"): 20.406e9, ("gelu", 393216, "k_eval_lut"): 10.279e9}
+NCU_TRAFFIC = {("gelu", 393216, "k_gen_vec"): 20.406e9, ("gelu", 393216, "k_eval_lut"): 10.279e9,
+               ("gelu", 393216, "k_eval_sp"): 1.389e9}           # k_eval_sp<3,1>: profiles/r1h_gelu.md
+
+
+def project(t_comp_ms, bytes_per_party, rounds):
+    """Eq. 1 of the paper: T_proj = T_comp + 2 B_comm / BW + R RTT, with its LAN / WAN parameters."""
+    return {"t_comp_ms": t_comp_ms, "bytes_per_party": bytes_per_party, "rounds": rounds,
+            "lan_ms": t_comp_ms + 2e3 * bytes_per_party / 1e9 + rounds * 0.5,
+            "wan_ms": t_comp_ms + 2e3 * bytes_per_party / 400e6 + rounds * 4.0}
 LDS_LANES_PER_CLK_SM = 32       # shared-memory crossbar: 128 B/clk/SM (B300_MICROARCH "LDS/STS")
 
 
@@ -183,8 +191,10 @@ def measure_shared_prefix(F, torch, name, base_spec, inp, rank, world, steps, wa
             "key_bytes_per_elem_per_party": key_b, "online_bytes_per_elem_per_party": P.online_bits() / 8,
             "aes_per_elem": {"eval_one_party": aes_eval, "keygen_both": cost["gen_cmp_aes"] + cost["gen_lut_aes"]},
             "gpu_launches": F.launch_count() - l0,
+            "projection": project((t_eval + t_post) / 2, P.online_bits() / 8 * count, 1 + P.post_rounds()),
             "roofline": {"bound": "alu", "kernel": "k_eval_sp", "achieved": ach, "peak": peak, "unit": "GAES/s (AES-128 blocks per second)",
-                         "frac": ach / peak, "lookups_per_aes": lk_eval / max(1, aes_eval), "launch_ms": t_eval / 2, "traffic": None,
+                         "frac": ach / peak, "lookups_per_aes": lk_eval / max(1, aes_eval), "launch_ms": t_eval / 2,
+                         "traffic": None if xpoly else NCU_TRAFFIC.get((name, count, "k_eval_sp")),
                          "hbm_achieved_gbs": key_b * count / (t_eval / 2 * 1e-3) / 1e9}}
 
 
@@ -372,6 +382,7 @@ def main():
             "aes_per_elem": {"eval_one_party": aes_eval, "keygen_both": aes_gen},
             "aes_rate_gaes": {"eval": 2 * aes_eval * count / ((per_step(t_cmp) + per_step(t_lut)) * 1e-3) / 1e9,
                               "keygen": aes_gen * count / (per_step(t_gen) * 1e-3) / 1e9},
+            "projection": project((per_step(t_cmp) + per_step(t_lut) + per_step(t_post)) / 2, P.online_bits() / 8 * count, 1 + P.post_rounds()),
             "gpu_launches": launches, "clocks": clocks.summary(), "roofline": roofline}
 
     # ---- PRG core alone (a pure AES chain, no key traffic): what the table design sustains on this GPU ----
