@@ -398,6 +398,18 @@ def main():
                              "what": "fusefss_aes_probe: 3 blocks per trip sharing round 1 (150 lookups per block), no key loads",
                              "lookup_roof_gaes": 148 * SM_CLOCK_MAX_MHZ * 1e6 * LDS_LANES_PER_CLK_SM / 150.0 / 1e9}
         del pout
+        sms = torch.cuda.get_device_properties(local).multi_processor_count
+        pbuf = torch.empty(sms * 1024, dtype=torch.int32, device="cuda")
+        for kind, key in ((0, "lop3_lane_ops_per_clk_per_sm"), (1, "lds32_lanes_per_clk_per_sm")):
+            it = 4096
+            F._check(F.lib.fusefss_pipe_probe(kind, it, pbuf.data_ptr(), torch.cuda.current_stream().cuda_stream))
+            torch.cuda.synchronize()
+            p0.record()
+            F._check(F.lib.fusefss_pipe_probe(kind, it, pbuf.data_ptr(), torch.cuda.current_stream().cuda_stream))
+            p1.record()
+            torch.cuda.synchronize()
+            line["prg_probe"][key] = sms * 1024 * 8 * it / (p0.elapsed_time(p1) * 1e-3) / (SM_CLOCK_MAX_MHZ * 1e6) / sms
+        line["prg_probe"]["pipes"] = "fusefss_pipe_probe at 1.965 GHz: LOP3 chains (nominal 64 lanes/clk/SM) and conflict-free LDS.32 (nominal 32 lanes/clk/SM)"
     except Exception as exc:                                      # the probe is informative only
         line["prg_probe"] = {"error": str(exc)}
 

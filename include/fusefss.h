@@ -214,6 +214,10 @@ uint64_t fusefss_launch_count(void);
 /* PRG micro-kernel for the roofline denominator: each thread chains `iters` fixed-key AES-128 blocks starting
  * from its index and writes the last block to out_dev[threads*16 bytes]; blocks = threads*iters. */
 int fusefss_aes_probe(size_t threads, int iters, void *out_dev, void *stream);
+/* Pipe micro-probes for the roofline denominators: kind 0 = LOP3 issue (8 independent chains per thread), kind 1 =
+ * conflict-free LDS.32 wavefronts (8 dependent-lookup chains per thread through the bank-replicated table).  One CTA of
+ * 1024 threads per SM; out_dev holds SMs*1024 uint32.  Operations executed = SMs * 1024 * 8 * iters (lane-ops). */
+int fusefss_pipe_probe(int kind, int iters, void *out_dev, void *stream);
 /* single-block AES-128 (FIPS-197) through the device PRG core, for the known-answer test: key[16], in[16] HOST,
  * out_dev[16] device */
 int fusefss_aes_kat(const uint8_t *key, const uint8_t *in, void *out_dev, void *stream);

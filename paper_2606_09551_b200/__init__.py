@@ -22,7 +22,7 @@ SYMBOLS = (
     "fusefss_eval_cmp", "fusefss_eval_lut", "fusefss_eval_fused", "fusefss_post", "fusefss_post_rounds", "fusefss_post_msg_bytes",
     "fusefss_online_bits", "fusefss_post_fused", "fusefss_cost", "fusefss_gate_workspace_bytes", "fusefss_gate_host",
     "fusefss_share_open", "fusefss_row_sum", "fusefss_mul_triple_bytes", "fusefss_mul_keygen", "fusefss_mul_fused",
-    "fusefss_strerror", "fusefss_last_cuda_error", "fusefss_launch_count", "fusefss_aes_probe", "fusefss_aes_kat",
+    "fusefss_strerror", "fusefss_last_cuda_error", "fusefss_launch_count", "fusefss_aes_probe", "fusefss_aes_kat", "fusefss_pipe_probe",
 )
 
 
@@ -92,6 +92,7 @@ def _load():
         "fusefss_launch_count": (u64, []),
         "fusefss_aes_probe": (i32, [sz, i32, vp, vp]),
         "fusefss_aes_kat": (i32, [C.c_char_p, C.c_char_p, vp, vp]),
+        "fusefss_pipe_probe": (i32, [i32, i32, vp, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)

@@ -685,6 +685,33 @@ __global__ void __launch_bounds__(kEvalThreads, 1) k_aes_probe(const ProbeArgs a
         a.out[i] = make_uint4(x[0][0], x[0][1], x[0][2], x[0][3]);
     }
 }
+// Pipe probes for the roofline denominators: kind 0 = LOP3 issue rate (8 independent 3-input XOR chains
+// per thread), kind 1 = conflict-free LDS.32 wavefront rate (8 independent dependent-lookup chains per thread through
+// the bank-replicated table, PRMT-addressed exactly like the AES lookups).
+struct PipeArgs { uint32_t *out; int iters, kind; };
+__global__ void __launch_bounds__(kEvalThreads, 1) k_pipe_probe(const PipeArgs a) {
+    extern __shared__ uint32_t sT[];
+    const uint32_t tl = aes_fill_tables(sT);
+    uint32_t v[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) v[j] = threadIdx.x * 2654435761u + j * 40503u + blockIdx.x;
+    if (a.kind == 0) {
+        const uint32_t k1 = tl | 0x55aa55aau, k2 = tl * 3u + 1u;
+        for (int i = 0; i < a.iters; ++i) {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) asm("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(v[j]) : "r"(k1), "r"(k2 + j));
+        }
+    } else {
+        for (int i = 0; i < a.iters; ++i) {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) v[j] = tlu<0, 0>(tl, v[j]) + j;
+        }
+    }
+    uint32_t acc = 0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) acc ^= v[j];
+    a.out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = acc;
+}
 struct KatArgs { uint4 *out; uint32_t in[4]; RoundKeys rk; };
 __global__ void k_aes_kat(const KatArgs a) {
     extern __shared__ uint32_t sT[];
@@ -706,6 +733,14 @@ int fusefss_aes_probe(size_t threads, int iters, void *out_dev, void *stream) {
     ProbeArgs a{(uint4 *)out_dev, threads, iters};
     const int grid = grid_for((threads + 31) / 32, g_eval_threads);
     return launch(k_aes_probe, grid, g_eval_threads, kAesSmemBytes, (cudaStream_t)stream, a);
+}
+
+int fusefss_pipe_probe(int kind, int iters, void *out_dev, void *stream) {
+    if (!out_dev) return FUSEFSS_E_NULL;
+    if (iters <= 0 || (kind != 0 && kind != 1)) return FUSEFSS_E_COUNT;
+    int rc = init_device(); if (rc) return rc;
+    PipeArgs a{(uint32_t *)out_dev, iters, kind};
+    return launch(k_pipe_probe, g_sms, kEvalThreads, kAesSmemBytes, (cudaStream_t)stream, a);
 }
 
 int fusefss_aes_kat(const uint8_t *key, const uint8_t *in, void *out_dev, void *stream) {
