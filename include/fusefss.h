@@ -170,15 +170,19 @@ int fusefss_post_fused(const fusefss_program *prog, const void *key0_dev, const 
                        uint64_t *y0_dev, uint64_t *y1_dev, uint64_t *z0_dev, uint64_t *z1_dev, void *stream);
 
 /* ---- vector-block glue (App. G: blocks = linear ops on shares + compiled scalar gates) ----------
- * fusefss_share_open: Protocol 1 for the input of gate `prog`: xhat = (x_0 + [r_in]_0) + (x_1 + [r_in]_1),
- *   the [r_in] shares are read from the two key buffers generated for these `count` elements (n/8 bytes per party).
+ * fusefss_share_open: Protocol 1 for the input of gate `prog`: xhat = (x_0 + [r_in]_0) + (x_1 + [r_in]_1)
+ *   + public_offset; the [r_in] shares are read from the two key buffers generated for these `count` elements (n/8 bytes
+ *   per party).  public_offset = 2^{n-1} feeds the signed-truncation gate (workloads.specs.ars), 0 otherwise.
+ * fusefss_sub_bcast: out[i] = x[i] - mu[i / cols] mod 2^n, local on additive shares.
  * fusefss_row_sum: out[r] = sum_c in[r*cols + c] mod 2^n, local on additive shares.
  * fusefss_mul_keygen / fusefss_mul_fused: element-wise Beaver products z = x * y (formulas DESIGN 4.6) with y
  *   broadcast over `cols` consecutive elements (cols = 1: plain element-wise; y has count/cols entries); the dealer's
  *   triples (fusefss_mul_triple_bytes(count) per party) come from R(e, 0xA000..0xA002); both parties in one launch,
  *   2n/8 online bytes per party per product. */
 int fusefss_share_open(const fusefss_program *prog, const void *key0_dev, const void *key1_dev, const uint64_t *x0_dev,
-                       const uint64_t *x1_dev, size_t count, uint64_t *xhat_out_dev, void *stream);
+                       const uint64_t *x1_dev, size_t count, uint64_t public_offset, uint64_t *xhat_out_dev, void *stream);
+int fusefss_sub_bcast(uint32_t n_bits, const uint64_t *x_dev, const uint64_t *mu_dev, size_t count, size_t cols,
+                      uint64_t *out_dev, void *stream);
 int fusefss_row_sum(uint32_t n_bits, const uint64_t *in_dev, size_t rows, size_t cols, uint64_t *out_dev, void *stream);
 size_t fusefss_mul_triple_bytes(size_t count);
 int fusefss_mul_keygen(uint32_t n_bits, uint64_t seed, uint64_t first_elem, size_t count, void *t0_dev, void *t1_dev, void *stream);

@@ -12,11 +12,12 @@ import oracle
 SLOT_MUL_AB, SLOT_MUL_AB0, SLOT_MUL_C0 = 0xA000, 0xA001, 0xA002
 
 
-def gate(P, x0, x1, r_in, seed, first=0):
-    """One compiled gate on additively shared inputs: Protocol 1 (masked opening), then the online procedure."""
+def gate(P, x0, x1, r_in, seed, first=0, offset=0):
+    """One compiled gate on additively shared inputs: Protocol 1 (masked opening), then the online procedure.
+    `offset` = public constant added to the gate input (2^63 for the signed truncation gate workloads.specs.ars)."""
     count = x0.size
     k0, k1 = P.keygen(r_in, None, seed, first)
-    xhat = x0 + P.rin_shares(k0, count) + x1 + P.rin_shares(k1, count)          # n = 64: wraps mod 2^64
+    xhat = x0 + P.rin_shares(k0, count) + x1 + P.rin_shares(k1, count) + np.uint64(offset)   # n = 64: wraps mod 2^64
     out = P.run_gate(k0, k1, xhat)
     return out["y"][0][0], out["y"][1][0], xhat
 
@@ -61,3 +62,40 @@ def softmax_plain(progs, x, rows, cols):
         p = f * np.repeat(u, cols)
         y = progs["tr_y"].plain_G(p, z)[0][0]
     return dict(e=e, f=f, s=s, t=t, u=u, p=p, y=y)
+
+
+HALF = 1 << 63
+
+
+def layernorm(progs, x0, x1, masks, rows, d, seed):
+    """LayerNorm without affine parameters on rows of length d = 2^k at scale 2^12 (App. G: mean / variance reductions
+    are linear, rsqrt is a compiled gate):  mu = ARS_k(sum x); c = x - mu; v = ARS_{k+12}(sum c^2); g = rsqrt(v) (scale
+    2^48) -> ARS_24; y = ARS_24(c * g).  progs / masks: stages 'mean', 'var', 'rsqrt', 'tr_g', 'tr_y'."""
+    with np.errstate(over="ignore"):
+        rs = lambda a: a.reshape(rows, d).sum(axis=1, dtype=np.uint64)
+        m0, m1, _ = gate(progs["mean"], rs(x0), rs(x1), masks["mean"], seed + 1, offset=HALF)
+        c0, c1 = x0 - np.repeat(m0, d), x1 - np.repeat(m1, d)
+        q0, q1 = beaver_mul(c0, c1, c0, c1, 1, seed + 2)
+        v0, v1, _ = gate(progs["var"], rs(q0), rs(q1), masks["var"], seed + 3, offset=HALF)
+        g0, g1, _ = gate(progs["rsqrt"], v0, v1, masks["rsqrt"], seed + 4)
+        h0, h1, _ = gate(progs["tr_g"], g0, g1, masks["tr_g"], seed + 5, offset=HALF)
+        p0, p1 = beaver_mul(c0, c1, h0, h1, d, seed + 6)
+        y0, y1, _ = gate(progs["tr_y"], p0, p1, masks["tr_y"], seed + 7, offset=HALF)
+    return dict(m=(m0, m1), c=(c0, c1), q=(q0, q1), v=(v0, v1), g=(g0, g1), h=(h0, h1), p=(p0, p1), y=(y0, y1))
+
+
+def layernorm_plain(progs, x, rows, d):
+    """Tier A: the same pipeline on cleartext fixed-point values."""
+    zr, z = np.zeros(rows, np.uint64), np.zeros(x.size, np.uint64)
+    H = np.uint64(HALF)
+    with np.errstate(over="ignore"):
+        rs = lambda a: a.reshape(rows, d).sum(axis=1, dtype=np.uint64)
+        m = progs["mean"].plain_G(rs(x) + H, zr)[0][0]
+        c = x - np.repeat(m, d)
+        q = c * c
+        v = progs["var"].plain_G(rs(q) + H, zr)[0][0]
+        g = progs["rsqrt"].plain_G(v, zr)[0][0]
+        h = progs["tr_g"].plain_G(g + H, zr)[0][0]
+        p = c * np.repeat(h, d)
+        y = progs["tr_y"].plain_G(p + H, z)[0][0]
+    return dict(m=m, c=c, q=q, v=v, g=g, h=h, p=p, y=y)

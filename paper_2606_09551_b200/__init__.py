@@ -21,7 +21,7 @@ SYMBOLS = (
     "fusefss_compile", "fusefss_destroy", "fusefss_shape", "fusefss_atom", "fusefss_key_bytes", "fusefss_keygen", "fusefss_keygen_parts",
     "fusefss_eval_cmp", "fusefss_eval_lut", "fusefss_eval_fused", "fusefss_post", "fusefss_post_rounds", "fusefss_post_msg_bytes",
     "fusefss_online_bits", "fusefss_post_fused", "fusefss_cost", "fusefss_gate_workspace_bytes", "fusefss_gate_host",
-    "fusefss_share_open", "fusefss_row_sum", "fusefss_mul_triple_bytes", "fusefss_mul_keygen", "fusefss_mul_fused",
+    "fusefss_share_open", "fusefss_sub_bcast", "fusefss_row_sum", "fusefss_mul_triple_bytes", "fusefss_mul_keygen", "fusefss_mul_fused",
     "fusefss_strerror", "fusefss_last_cuda_error", "fusefss_launch_count", "fusefss_aes_probe", "fusefss_aes_kat", "fusefss_pipe_probe",
 )
 
@@ -82,7 +82,8 @@ def _load():
         "fusefss_cost": (i32, [vp, C.POINTER(Cost)]),
         "fusefss_gate_workspace_bytes": (sz, [vp, sz]),
         "fusefss_gate_host": (i32, [vp, vp, vp, vp, u64, sz, sz, vp, vp, vp, vp, vp, vp]),
-        "fusefss_share_open": (i32, [vp, vp, vp, vp, vp, sz, vp, vp]),
+        "fusefss_share_open": (i32, [vp, vp, vp, vp, vp, sz, u64, vp, vp]),
+        "fusefss_sub_bcast": (i32, [C.c_uint32, vp, vp, sz, sz, vp, vp]),
         "fusefss_row_sum": (i32, [C.c_uint32, vp, sz, sz, vp, vp]),
         "fusefss_mul_triple_bytes": (sz, [sz]),
         "fusefss_mul_keygen": (i32, [C.c_uint32, u64, u64, sz, vp, vp, vp]),

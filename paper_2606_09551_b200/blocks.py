@@ -61,9 +61,9 @@ class Softmax:
         _check(lib.fusefss_mul_keygen(self.n, seed + 5, 0, self.N, _ptr(self.triples[0]), _ptr(self.triples[1]), _stream()))
 
     # ---- online ----------------------------------------------------------------------------------
-    def _gate(self, k, x0, x1):
+    def _gate(self, k, x0, x1, offset=0):
         P, (k0, k1), b, c = self.progs[k], self.keys[k], self.buf[k], self.counts[k]
-        _check(lib.fusefss_share_open(P._h, _ptr(k0), _ptr(k1), _ptr(x0), _ptr(x1), c, _ptr(b["xhat"]), _stream()))
+        _check(lib.fusefss_share_open(P._h, _ptr(k0), _ptr(k1), _ptr(x0), _ptr(x1), c, offset, _ptr(b["xhat"]), _stream()))
         for party, key in ((0, k0), (1, k1)):
             P.eval_fused(party, key, b["xhat"], b["bits"][party] if P.shape["T"] else None,
                          b["coeff"][party] if P.shape["has_lut"] else None)
@@ -94,3 +94,81 @@ class Softmax:
 
     def rounds(self) -> int:
         return sum(1 + self.progs[k].post_rounds() for k in STAGES) + 1
+
+
+def _apply_variant(s, variant):
+    from workloads import specs as S
+    if variant & 1:
+        s = S.shared_prefix(s)
+    if variant & 2:
+        s = S.input_masked_mul(s)
+    if variant & 4:
+        s = S.public_point_horner(s)
+    return s
+
+
+class LayerNorm(Softmax):
+    """rows x d block, d = 2^k, no affine parameters, inputs at scale 2^12 (App. G: mean / variance reductions are linear,
+    rsqrt is a compiled gate; config 4b):  mu = ARS_k(sum x); c = x - mu; v = ARS_{k+12}(sum c^2); g = rsqrt(v) (scale 2^48)
+    -> ARS_24; y = ARS_24(c * g).  The signed truncations are `workloads.specs.ars` gates fed with xhat + 2^63."""
+    LN_STAGES = ("mean", "var", "rsqrt", "tr_g", "tr_y")
+    HALF = 1 << 63
+
+    def __init__(self, rows: int, d: int, variant: int = 3):
+        import torch
+        from workloads import specs as S
+        k = d.bit_length() - 1
+        if d != 1 << k:
+            raise ValueError("LayerNorm block: d must be a power of two (the mean is a truncation gate)")
+        self.rows, self.cols, self.N, self.n = rows, d, rows * d, 64
+        mk = {"mean": S.ars(64, k), "var": S.ars(64, k + 12), "rsqrt": S.rsqrt(64, 12), "tr_g": S.ars(64, 24), "tr_y": S.ars(64, 24)}
+        self.specs = {kk: _apply_variant(s, variant) for kk, s in mk.items()}
+        self.progs = {kk: Program(s) for kk, s in self.specs.items()}
+        self.counts = {"mean": rows, "var": rows, "rsqrt": rows, "tr_g": rows, "tr_y": self.N}
+        self.keys = {kk: self.progs[kk].alloc_keys(c) for kk, c in self.counts.items()}
+        tb = lib.fusefss_mul_triple_bytes(self.N)
+        u8 = lambda: torch.empty(tb, dtype=torch.uint8, device="cuda")
+        self.triples_sq, self.triples = (u8(), u8()), (u8(), u8())
+        i64 = lambda *shape: torch.empty(shape, dtype=torch.int64, device="cuda")
+        self.buf = {kk: dict(xhat=i64(c), bits=[i64(c), i64(c)], coeff=[i64(self.progs[kk].shape["p"], c) for _ in (0, 1)],
+                             out=(i64(1, c), i64(1, c), i64(c), i64(c))) for kk, c in self.counts.items()}
+        self.s = [i64(rows), i64(rows)]
+        self.ssq = [i64(rows), i64(rows)]
+        self.c = [i64(self.N), i64(self.N)]
+        self.sq = [i64(self.N), i64(self.N)]
+        self.prod = [i64(self.N), i64(self.N)]
+
+    def keygen(self, masks, seed: int):
+        for kk, off in zip(self.LN_STAGES, (1, 3, 4, 5, 7)):
+            self.progs[kk].keygen(masks[kk], None, seed + off, 0, keys=self.keys[kk])
+        _check(lib.fusefss_mul_keygen(self.n, seed + 2, 0, self.N, _ptr(self.triples_sq[0]), _ptr(self.triples_sq[1]), _stream()))
+        _check(lib.fusefss_mul_keygen(self.n, seed + 6, 0, self.N, _ptr(self.triples[0]), _ptr(self.triples[1]), _stream()))
+
+    def run(self, x0, x1):
+        H, st = self.HALF, _stream()
+        for b, xb in ((0, x0), (1, x1)):
+            _check(lib.fusefss_row_sum(self.n, _ptr(xb), self.rows, self.cols, _ptr(self.s[b]), st))
+        m0, m1 = self._gate("mean", self.s[0], self.s[1], H)
+        for b, (xb, mb) in enumerate(((x0, m0), (x1, m1))):
+            _check(lib.fusefss_sub_bcast(self.n, _ptr(xb), _ptr(mb), self.N, self.cols, _ptr(self.c[b]), st))
+        c0, c1 = self.c
+        _check(lib.fusefss_mul_fused(self.n, _ptr(c0), _ptr(c1), _ptr(c0), _ptr(c1), _ptr(self.triples_sq[0]), _ptr(self.triples_sq[1]),
+                                     self.N, 1, _ptr(self.sq[0]), _ptr(self.sq[1]), st))
+        for b in (0, 1):
+            _check(lib.fusefss_row_sum(self.n, _ptr(self.sq[b]), self.rows, self.cols, _ptr(self.ssq[b]), st))
+        v0, v1 = self._gate("var", self.ssq[0], self.ssq[1], H)
+        g0, g1 = self._gate("rsqrt", v0, v1)
+        h0, h1 = self._gate("tr_g", g0, g1, H)
+        _check(lib.fusefss_mul_fused(self.n, _ptr(c0), _ptr(c1), _ptr(h0), _ptr(h1), _ptr(self.triples[0]), _ptr(self.triples[1]),
+                                     self.N, self.cols, _ptr(self.prod[0]), _ptr(self.prod[1]), st))
+        y0, y1 = self._gate("tr_y", self.prod[0], self.prod[1], H)
+        return dict(m=(m0, m1), c=(c0, c1), q=tuple(self.sq), v=(v0, v1), g=(g0, g1), h=(h0, h1), p=tuple(self.prod), y=(y0, y1))
+
+    def online_bytes_per_party(self) -> int:
+        return sum(self.progs[k].online_bits() // 8 * c for k, c in self.counts.items()) + 2 * 16 * self.N
+
+    def key_bytes_per_party(self) -> int:
+        return sum(self.progs[k].key_bytes(c) for k, c in self.counts.items()) + 2 * lib.fusefss_mul_triple_bytes(self.N)
+
+    def rounds(self) -> int:
+        return sum(1 + self.progs[k].post_rounds() for k in self.LN_STAGES) + 2

@@ -11,12 +11,12 @@
 namespace fsk {
 
 // Protocol 1: xhat = (x_0 + [r_in]_0) + (x_1 + [r_in]_1) mod 2^n; each party sends one ring element.
-struct OpenArgs { const uint64_t *x0, *x1; const uint8_t *key0, *key1; size_t rin_off, count; uint64_t mask; uint64_t *xhat; };
+struct OpenArgs { const uint64_t *x0, *x1; const uint8_t *key0, *key1; size_t rin_off, count; uint64_t mask, offset; uint64_t *xhat; };
 __global__ void k_share_open(const OpenArgs a) {
     const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (e >= a.count) return;
     const uint64_t r0 = reinterpret_cast<const uint64_t *>(a.key0 + a.rin_off)[e], r1 = reinterpret_cast<const uint64_t *>(a.key1 + a.rin_off)[e];
-    a.xhat[e] = (a.x0[e] + r0 + a.x1[e] + r1) & a.mask;
+    a.xhat[e] = (a.x0[e] + r0 + a.x1[e] + r1 + a.offset) & a.mask;      // offset: public constant added to the gate input
 }
 
 // out[r] = sum_c in[r*cols + c] mod 2^n (local on additive shares): one warp per row
@@ -30,6 +30,13 @@ __global__ void k_row_sum(const RowSumArgs a) {
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
     if (lane == 0) a.out[row] = acc & a.mask;
+}
+
+// out[i] = x[i] - mu[i / cols] mod 2^n (local on additive shares): centring by a per-row value
+struct SubBcastArgs { const uint64_t *x, *mu; uint64_t *out; size_t count, cols; uint64_t mask; };
+__global__ void k_sub_bcast(const SubBcastArgs a) {
+    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e < a.count) a.out[e] = (a.x[e] - a.mu[e / a.cols]) & a.mask;
 }
 
 // Beaver triples for `count` products: per party [a][b][c] arrays of s8 bytes each; randomness R(e, 0xA000..0xA002)

@@ -571,12 +571,12 @@ int fusefss_post_fused(const fusefss_program *prog, const void *key0_dev, const 
 
 // ---- vector-block glue (App. G) -------------------------------------------
 int fusefss_share_open(const fusefss_program *prog, const void *key0_dev, const void *key1_dev, const uint64_t *x0_dev,
-                       const uint64_t *x1_dev, size_t count, uint64_t *xhat_out_dev, void *stream) {
+                       const uint64_t *x1_dev, size_t count, uint64_t public_offset, uint64_t *xhat_out_dev, void *stream) {
     const Program *P = prog_of(prog);
     if (!P || !key0_dev || !key1_dev || !x0_dev || !x1_dev || !xhat_out_dev) return FUSEFSS_E_NULL;
     if (count == 0) return FUSEFSS_E_COUNT;
     Layout L; compute_layout(*P, count, &L);
-    OpenArgs a{x0_dev, x1_dev, (const uint8_t *)key0_dev, (const uint8_t *)key1_dev, L.rin, count, P->mask, xhat_out_dev};
+    OpenArgs a{x0_dev, x1_dev, (const uint8_t *)key0_dev, (const uint8_t *)key1_dev, L.rin, count, P->mask, public_offset & P->mask, xhat_out_dev};
     return launch(k_share_open, (int)((count + 255) / 256), 256, 0, (cudaStream_t)stream, a);
 }
 
@@ -586,6 +586,14 @@ int fusefss_row_sum(uint32_t n_bits, const uint64_t *in_dev, size_t rows, size_t
     if (n_bits < 1 || n_bits > 64) return FUSEFSS_E_SPEC;
     RowSumArgs a{in_dev, out_dev, rows, cols, n_bits >= 64 ? ~0ull : ((1ull << n_bits) - 1ull)};
     return launch(k_row_sum, (int)((rows * 32 + 255) / 256), 256, 0, (cudaStream_t)stream, a);
+}
+
+int fusefss_sub_bcast(uint32_t n_bits, const uint64_t *x_dev, const uint64_t *mu_dev, size_t count, size_t cols, uint64_t *out_dev, void *stream) {
+    if (!x_dev || !mu_dev || !out_dev) return FUSEFSS_E_NULL;
+    if (count == 0 || cols == 0) return FUSEFSS_E_COUNT;
+    if (n_bits < 1 || n_bits > 64) return FUSEFSS_E_SPEC;
+    SubBcastArgs a{x_dev, mu_dev, out_dev, count, cols, n_bits >= 64 ? ~0ull : ((1ull << n_bits) - 1ull)};
+    return launch(k_sub_bcast, (int)((count + 255) / 256), 256, 0, (cudaStream_t)stream, a);
 }
 
 size_t fusefss_mul_triple_bytes(size_t count) { return 3 * ((count * 8 + 255) & ~(size_t)255); }

@@ -33,10 +33,11 @@ ALL = [("relu16", lambda: specs.relu(16, 8)), ("gelu", specs.gelu), ("nexp", spe
        ("shift_relu", specs.shift_relu), ("rsqrt", specs.rsqrt), ("silu", specs.silu),
        ("toy", lambda: specs.toy(8, 3)), ("toy_masked", lambda: specs.toy(8, 3, True)),
        ("plain", specs.plain_default), ("single", specs.single_interval), ("nobits", specs.no_bits),
-       ("full", specs.full_partition), ("shift_relu8", lambda: specs.shift_relu(8, 3))]
+       ("full", specs.full_partition), ("shift_relu8", lambda: specs.shift_relu(8, 3)), ("ars", lambda: specs.ars(64, 12)),
+       ("ars8", lambda: specs.ars(8, 3))]
 ALL = ALL + [(nm + "_sp", (lambda mk=mk: specs.shared_prefix(mk()))) for nm, mk in ALL]      # variant 1 (DESIGN 9)
 ALL = ALL + [(nm + "_xm", (lambda mk=mk: specs.input_masked_mul(mk()))) for nm, mk in ALL]  # variant bit 1 (DESIGN 10)
-ALL = ALL + [(nm + "_xp", (lambda mk=mk: specs.public_point_horner(mk()))) for nm, mk in ALL[:28]]  # variant bit 2 (DESIGN 11)
+ALL = ALL + [(nm + "_xp", (lambda mk=mk: specs.public_point_horner(mk()))) for nm, mk in ALL[:32]]  # variant bit 2 (DESIGN 11)
 
 
 @pytest.mark.parametrize("name,mk", ALL)

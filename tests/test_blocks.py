@@ -72,3 +72,67 @@ def test_gpu_block_matches_oracle_composition(orc, variant, rows, cols):
     pl = oblocks.softmax_plain(progs, x, rows, cols)
     assert np.array_equal(host(got["y"][0]) + host(got["y"][1]), pl["y"])
     assert B.rounds() > 0 and B.online_bytes_per_party() > 0 and B.key_bytes_per_party() > 0
+
+
+# ---- LayerNorm block (mean / variance reductions + rsqrt gate + signed truncation gates) ---------------------------
+def _ln_specs(variant, k):
+    mk = {"mean": specs.ars(64, k), "var": specs.ars(64, k + 12), "rsqrt": specs.rsqrt(), "tr_g": specs.ars(64, 24),
+          "tr_y": specs.ars(64, 24)}
+    out = {}
+    for kk, s in mk.items():
+        if variant & 1:
+            s = specs.shared_prefix(s)
+        if variant & 2:
+            s = specs.input_masked_mul(s)
+        out[kk] = s
+    return out
+
+
+def _ln_inputs(rows, d, seed):
+    rng = np.random.default_rng(seed)
+    xr = rng.normal(rng.normal(0.0, 1.0, size=(rows, 1)), rng.uniform(0.5, 3.0, size=(rows, 1)), size=(rows, d))
+    x = np.floor(xr.reshape(-1) * 4096 + 0.5).astype(np.int64).view(np.uint64)
+    U = lambda k: rng.integers(0, 1 << 63, size=k, dtype=np.uint64) * np.uint64(2) + rng.integers(0, 2, size=k, dtype=np.uint64)
+    x0 = U(x.size)
+    masks = dict(mean=U(rows), var=U(rows), rsqrt=U(rows), tr_g=U(rows), tr_y=U(x.size))
+    return x, x0, x - x0, masks
+
+
+@pytest.mark.parametrize("variant", [0, 3])
+def test_oracle_layernorm_reconstructs_plaintext_pipeline(orc, variant):
+    from oracle import blocks
+    rows, d = 4, 32
+    progs = {k: orc.Program(s) for k, s in _ln_specs(variant, 5).items()}
+    x, x0, x1, masks = _ln_inputs(rows, d, 5)
+    out = blocks.layernorm(progs, x0, x1, masks, rows, d, seed=77)
+    pl = blocks.layernorm_plain(progs, x, rows, d)
+    for k in ("m", "c", "q", "v", "g", "h", "p", "y"):
+        assert np.array_equal(out[k][0] + out[k][1], pl[k]), k
+    y = pl["y"].view(np.int64).astype(np.float64).reshape(rows, d) / 4096.0
+    xq = x.view(np.int64).astype(np.float64).reshape(rows, d) / 4096.0
+    ref = (xq - xq.mean(axis=1, keepdims=True)) / xq.std(axis=1, keepdims=True)
+    assert np.abs(y - ref).max() <= 0.03                     # rsqrt spline: <= 0.5 % relative on a value of magnitude <= ~4
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("variant,rows,d", [(3, 5, 64), (0, 2, 32), (1, 9, 1024)])
+def test_gpu_layernorm_matches_oracle_composition(orc, variant, rows, d):
+    import torch
+    import __graft_entry__ as g
+    g.build()
+    from oracle import blocks as oblocks
+    from paper_2606_09551_b200 import blocks as gblocks
+    x, x0, x1, masks = _ln_inputs(rows, d, 11)
+    progs = {k: orc.Program(s) for k, s in _ln_specs(variant, d.bit_length() - 1).items()}
+    exp = oblocks.layernorm(progs, x0, x1, masks, rows, d, seed=21)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.int64)).cuda()
+    B = gblocks.LayerNorm(rows, d, variant)
+    B.keygen({k: dev(v) for k, v in masks.items()}, seed=21)
+    got = B.run(dev(x0), dev(x1))
+    torch.cuda.synchronize()
+    host = lambda t: t.cpu().numpy().view(np.uint64).reshape(-1)
+    for k in ("m", "c", "q", "v", "g", "h", "p", "y"):
+        for b in (0, 1):
+            assert np.array_equal(host(got[k][b]), exp[k][b]), (k, b)
+    pl = oblocks.layernorm_plain(progs, x, rows, d)
+    assert np.array_equal(host(got["y"][0]) + host(got["y"][1]), pl["y"])

@@ -96,7 +96,7 @@ def test_aes_core_fips197(F):
 
 SMALL = [lambda: specs.relu(8, 4), lambda: specs.toy(8, 3), lambda: specs.toy(8, 3, True), specs.plain_default,
          specs.single_interval, specs.no_bits, specs.full_partition, lambda: specs.shift_relu(8, 3),
-         lambda: specs.toy(12, 4), lambda: specs.relu(12, 6)]
+         lambda: specs.toy(12, 4), lambda: specs.relu(12, 6), lambda: specs.ars(8, 3), lambda: specs.ars(12, 5)]
 
 
 SMALL_SP = [(lambda mk=mk: specs.shared_prefix(mk())) for mk in SMALL]

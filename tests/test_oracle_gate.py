@@ -188,3 +188,22 @@ def test_rejects_ill_formed(orc):
     s.alpha = [40, 40, 200]
     with pytest.raises(ValueError):
         orc.Program(s)
+
+
+@pytest.mark.parametrize("variant", [0, 1])
+@pytest.mark.parametrize("n,f", [(8, 3), (12, 5)])
+def test_ars_gate_closed_form(orc, n, f, variant):
+    """Signed truncation gate (workloads.specs.ars): with the gate input x' = x + 2^{n-1}, the shares reconstruct to
+    floor(x_signed / 2^f) for every x and every mask r (closed form; SURVEY C7 truncation identity)."""
+    spec = specs.ars(n, f)
+    if variant:
+        spec = specs.shared_prefix(spec)
+    P = orc.Program(spec)
+    N = 1 << n
+    r_in, (k0, k1) = all_r_keys(P, n, 21)
+    for x in (range(N) if n == 8 else list(range(0, N, 37)) + [N - 1, N // 2, N // 2 - 1]):
+        xs = x - N if x >= N // 2 else x
+        want = np.uint64((xs >> f) % N)
+        xp = np.full(N, (x + N // 2) % N, dtype=np.uint64)               # x' = x + 2^{n-1}
+        out = P.run_gate(k0, k1, (xp + r_in) & mask_of(n))
+        assert np.all(((out["y"][0] + out["y"][1]) & mask_of(n)) == want), (n, f, x)

@@ -266,6 +266,25 @@ def shift_relu(n=64, f=12):
                kappa_a=[(KA_R_SHR, f)], kappa_b=[(KB_R_BIT, n - 1)], phi=phi, n_out_a=1, n_out_b=3, out_frac=f)
 
 
+def ars(n=64, f=12):
+    """Signed truncation y = x >>_arith f (the rescale between fixed-point multiplications):
+    ARS_f(x) = LRS_f(x + 2^{n-1}) - 2^{n-1-f}.  The gate's input is x' = x + 2^{n-1}: the caller adds the public
+    constant 2^{n-1} to the masked value (xhat' = xhat + 2^{n-1}, same mask).  No interval lookup (m = 1).
+    LRS_f(x') = (xhat' >> f) - (r >> f) - t + 2^{n-f} w with t = carry of the low f bits, w = wrap of x' + r."""
+    nodes = [(BN_MSB, 0, 0, 0, 0, 0), (BN_CARRY, f, 0, 0, 0, 0), (BN_CARRY, n, 0, 0, 0, 0)]
+    phi = [
+        (PHI_B_Z, 0, 0, 0, 0), (PHI_B_KAPPA, 1, 0, 0, 0),
+        (PHI_B_AND, 2, 0, 1, 0), (PHI_B_XOR, 3, 0, 1, 0), (PHI_B_ANDPUB, 4, 3, n - 1, 1), (PHI_B_XOR, 5, 2, 4, 0),
+        (PHI_B_Z, 6, 1, 0, 0),
+        (PHI_A_XHAT_SHR, 0, f, 0, 0), (PHI_A_KAPPA, 1, 0, 0, 0), (PHI_A_B2A, 2, 6, 0, 0), (PHI_A_B2A, 3, 5, 0, 0),
+        (PHI_A_MULC, 4, 3, 0, (1 << (n - f)) & U64),
+        (PHI_A_SUB, 5, 0, 1, 0), (PHI_A_SUB, 6, 5, 2, 0), (PHI_A_ADD, 7, 6, 4, 0),
+        (PHI_A_CONST, 8, 0, 0, 1 << (n - 1 - f)), (PHI_A_SUB, 9, 7, 8, 0), (PHI_A_OUT, 0, 9, 0, 0),
+    ]
+    return _mk(f"ars{f}_n{n}", n, f, [], [[[0]]], nodes=nodes, bit_root=[[0, 1, 2]],
+               kappa_a=[(KA_R_SHR, f)], kappa_b=[(KB_R_BIT, n - 1)], phi=phi, n_out_a=1, n_out_b=0, out_frac=0)
+
+
 # ---- a small "kitchen sink" spec for the exhaustive n = 8 / 12 brute force -------------------------
 def toy(n=8, f=3, mask_output=False):
     """Exercises everything the grammar allows at brute-force size: 4 uneven intervals, r = 2 degree-2
