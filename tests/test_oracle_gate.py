@@ -201,7 +201,7 @@ def test_ars_gate_closed_form(orc, n, f, variant):
     P = orc.Program(spec)
     N = 1 << n
     r_in, (k0, k1) = all_r_keys(P, n, 21)
-    for x in (range(N) if n == 8 else list(range(0, N, 37)) + [N - 1, N // 2, N // 2 - 1]):
+    for x in (range(N) if n == 8 else list(range(0, N, 331)) + [N - 1, N // 2, N // 2 - 1]):
         xs = x - N if x >= N // 2 else x
         want = np.uint64((xs >> f) % N)
         xp = np.full(N, (x + N // 2) % N, dtype=np.uint64)               # x' = x + 2^{n-1}
