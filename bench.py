@@ -229,7 +229,10 @@ def main():
 
     assert torch.cuda.is_available(), "bench.py needs a CUDA device: the product has no CPU fallback"
     torch.cuda.set_device(local)
-    if world > 1:
+    use_dist = world > 1 or "LOCAL_RANK" in os.environ          # under torchrun the group exists even for one rank
+    if use_dist:
+        if os.environ.get("NCCL_DEBUG", "VERSION").upper() == "VERSION":
+            os.environ["NCCL_DEBUG"] = "WARN"                 # keep stdout to the one JSON line (no NCCL version banner)
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     name = args.workload
     spec = specs.CONFIGS[name]()
@@ -284,7 +287,7 @@ def main():
     step.seed, step.events = 0, []
 
     def _allmax(v):
-        if world > 1:
+        if use_dist:
             t = torch.tensor([v], device="cuda")
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             return float(t.item())
@@ -292,7 +295,7 @@ def main():
 
     def barrier():
         torch.cuda.synchronize()
-        if world > 1:
+        if use_dist:
             dist.barrier()
         torch.cuda.synchronize()
 
@@ -309,7 +312,7 @@ def main():
         barrier()
     launches = F.launch_count() - launches0
     ms = start.elapsed_time(stop)
-    if world > 1:
+    if use_dist:
         t = torch.tensor([ms], device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms = float(t.item())
@@ -512,7 +515,7 @@ def main():
             e2e_step()                                                  # synchronises its stream before returning
         barrier()
         dt = time.perf_counter() - t0
-        if world > 1:
+        if use_dist:
             t = torch.tensor([dt], device="cuda")
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             dt = float(t.item())
@@ -548,7 +551,7 @@ def main():
                                 "keygen_elems_per_s": extra["keygen_elems_per_s"], "eval_post_elems_per_s": extra["eval_post_elems_per_s"]}
     if rank == 0:
         print(json.dumps(line), flush=True)
-    if world > 1:
+    if use_dist:
         dist.barrier()
         dist.destroy_process_group()
 
