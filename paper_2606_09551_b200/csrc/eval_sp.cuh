@@ -13,17 +13,16 @@
 
 namespace fsk {
 
-constexpr int kMaxClusters = 16;
 struct SpAtomDev { uint64_t c, beta; int k, is_theta; };
 struct EvalSpArgs {
     const uint8_t *key; const uint64_t *xhat; uint64_t *bits_out, *coeff_out;       // either output may be null
     const SpPoint *points; const uint64_t *weights, *delta_tab, *alpha;             // device tables (program blob)
+    const SpCluster *cluster;
     size_t count, s16, s8, lvl_stride, vt_first, vt_lvl_rel, vt_fin_rel, rpow;
     uint64_t mask;
     int n, m, p, party, T, n_w, n_clusters, G;   // G > 1: the points of an element are dealt round-robin to G warps (small tensors)
     SpWidth width[kMaxWidths];
     size_t bt_root[kMaxWidths], bt_cw[kMaxWidths], bt_vb[kMaxWidths];
-    SpCluster cluster[kMaxClusters];
     SpAtomDev atom[kMaxAtoms];
 };
 

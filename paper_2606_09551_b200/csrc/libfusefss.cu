@@ -111,7 +111,8 @@ int ensure_blob(Program &P) {
     P.dev_sp_points_off = P.dev_payload_off + up(P.payload.size() * 8 + 8);
     P.dev_sp_weights_off = P.dev_sp_points_off + up(P.sp.points.size() * sizeof(SpPoint) + 8);
     P.dev_sp_delta_off = P.dev_sp_weights_off + up(P.sp.weights.size() * 8 + 8);
-    P.dev_blob_bytes = P.dev_sp_delta_off + up(P.sp.delta_tab.size() * 8 + 8);
+    P.dev_sp_clusters_off = P.dev_sp_delta_off + up(P.sp.delta_tab.size() * 8 + 8);
+    P.dev_blob_bytes = P.dev_sp_clusters_off + up(P.sp.clusters.size() * sizeof(SpCluster) + 8);
     void *d = nullptr;
     CU(cudaMalloc(&d, P.dev_blob_bytes));
     std::vector<uint8_t> h(P.dev_blob_bytes, 0);
@@ -121,6 +122,7 @@ int ensure_blob(Program &P) {
     if (!P.sp.points.empty()) std::memcpy(h.data() + P.dev_sp_points_off, P.sp.points.data(), P.sp.points.size() * sizeof(SpPoint));
     if (!P.sp.weights.empty()) std::memcpy(h.data() + P.dev_sp_weights_off, P.sp.weights.data(), P.sp.weights.size() * 8);
     if (!P.sp.delta_tab.empty()) std::memcpy(h.data() + P.dev_sp_delta_off, P.sp.delta_tab.data(), P.sp.delta_tab.size() * 8);
+    if (!P.sp.clusters.empty()) std::memcpy(h.data() + P.dev_sp_clusters_off, P.sp.clusters.data(), P.sp.clusters.size() * sizeof(SpCluster));
     cudaError_t e = cudaMemcpy(d, h.data(), P.dev_blob_bytes, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { cudaFree(d); return cuda_fail(e, "cudaMemcpy(program tables)"); }
     P.dev_blob = d;
@@ -187,9 +189,8 @@ int launch_eval_sp(Program &P, int party, const void *key, const uint64_t *xhat,
     a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.lvl_stride = L.lvl_stride; a.vt_first = L.vt_first;
     a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel; a.mask = P.mask;
     a.n = (int)P.n; a.m = (int)P.m; a.p = P.p; a.party = party; a.T = P.T; a.n_w = P.sp.n_w;
-    if (P.sp.clusters.size() > (size_t)kMaxClusters) return FUSEFSS_E_SPEC;
     a.n_clusters = (int)P.sp.clusters.size();
-    for (int c = 0; c < a.n_clusters; ++c) a.cluster[c] = P.sp.clusters[c];
+    a.cluster = (const SpCluster *)(blob + P.dev_sp_clusters_off);
     for (int w = 0; w < P.sp.n_w; ++w) { a.width[w] = P.sp.width[w]; a.bt_root[w] = L.bt_root[w]; a.bt_cw[w] = L.bt_cw[w]; a.bt_vb[w] = L.bt_vb[w]; }
     for (int t = 0; t < P.T; ++t) a.atom[t] = SpAtomDev{P.atoms[t].c, P.atoms[t].beta, P.atoms[t].k, P.atoms[t].is_theta};
     // small tensors: deal the points of an element to G warps so that the machine has >= ~8 warps per SM, then

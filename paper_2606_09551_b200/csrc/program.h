@@ -95,7 +95,7 @@ struct Program {
     // device copy of the small tables (uploaded lazily by the launchers)
     void *dev_blob = nullptr;
     size_t dev_ins_off = 0, dev_alpha_off = 0, dev_payload_off = 0, dev_blob_bytes = 0;
-    size_t dev_sp_points_off = 0, dev_sp_weights_off = 0, dev_sp_delta_off = 0;
+    size_t dev_sp_points_off = 0, dev_sp_weights_off = 0, dev_sp_delta_off = 0, dev_sp_clusters_off = 0;
 };
 
 int compile_program(const fusefss_spec *spec, Program **out);

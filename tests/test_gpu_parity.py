@@ -266,3 +266,22 @@ def test_full_size_sampled(F, orc, name, variant):
     assert np.array_equal((host(y0)[0, :k] + host(y1)[0, :k]) & mask_of(spec.n), ye[0])
     if P.shape["n_out_b"]:
         assert np.array_equal(host(z0)[:k] ^ host(z1)[:k], pack_bits(ze))
+
+
+@pytest.mark.parametrize("variant", [0, 1, 5])
+def test_many_scattered_boundaries(F, orc, variant):
+    """m = 39 intervals spread over the whole ring (M = 40 lookup intervals for Protocol 3; 39 single-point clusters for
+    the single-key construction -- no prefix to share): parity on a ragged count."""
+    N = 1 << 64
+    alpha = [(i + 1) * (N // 40) + 17 * i for i in range(38)]
+    spec = specs._mk("many", 64, 12, alpha, [[[3 * i + 1, i]] for i in range(39)], n_out_a=1)
+    if variant & 1:
+        spec = specs.shared_prefix(spec)
+    if variant & 4:
+        spec = specs.public_point_horner(spec)
+    rng = np.random.default_rng(8)
+    u = lambda k: rng.integers(0, 1 << 63, size=k, dtype=np.uint64) * np.uint64(2) + rng.integers(0, 2, size=k, dtype=np.uint64)
+    count = 45
+    x = u(count)
+    x[:38] = np.array(alpha, dtype=np.uint64) - np.uint64(1)
+    _parity(F, orc, spec, x, u(count), u(count), seed=2)
