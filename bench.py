@@ -208,7 +208,7 @@ def main():
     ap.add_argument("--count", type=int, default=0, help="override the element count (0 = the config's full tensor)")
     ap.add_argument("--chunk", type=int, default=0, help="elements per keygen/eval chunk (0 = whole tensor resident)")
     ap.add_argument("--ref-sample", type=int, default=512)
-    ap.add_argument("--cpu-sample", type=int, default=2048)
+    ap.add_argument("--cpu-sample", type=int, default=4096)
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-sp", action="store_true", help="skip the variant-1 (shared-prefix) measurement")
