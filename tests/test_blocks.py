@@ -17,6 +17,8 @@ def _specs(variant):
             s = specs.shared_prefix(s)
         if variant & 2:
             s = specs.input_masked_mul(s)
+        if variant & 4:
+            s = specs.public_point_horner(s)
         out[k] = s
     return out
 
@@ -32,7 +34,7 @@ def _inputs(rows, cols, seed):
     return xr, x, x0, x - x0, masks
 
 
-@pytest.mark.parametrize("variant", [0, 3])
+@pytest.mark.parametrize("variant", [0, 3, 7])
 def test_oracle_block_reconstructs_plaintext_pipeline(orc, variant):
     from oracle import blocks
     rows, cols = 4, 24
@@ -49,7 +51,7 @@ def test_oracle_block_reconstructs_plaintext_pipeline(orc, variant):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("variant,rows,cols", [(3, 5, 40), (0, 3, 33), (1, 12, 128)])
+@pytest.mark.parametrize("variant,rows,cols", [(3, 5, 40), (0, 3, 33), (1, 12, 128), (7, 4, 48)])
 def test_gpu_block_matches_oracle_composition(orc, variant, rows, cols):
     import torch
     import __graft_entry__ as g
