@@ -4,7 +4,9 @@
 A "step" = one pass of the WHOLE hot path over one tensor of the workload: fusefss_keygen (both key bundles),
 fusefss_eval_cmp + fusefss_eval_lut for party 0 and party 1, fusefss_post_fused.  `value` = elements/s of that
 whole step, inputs resident in HBM; eval-only and keygen-only rates, key and online bytes per element and the
-roofline of the dominant kernel (k_eval_lut) ride along.  `e2e` = the same gate through fusefss_gate_host with
+roofline of the dominant kernel (k_gen_vec; k_eval_lut beside it) ride along, as do the same workload compiled with the
+single-key shared-prefix construction (`shared_prefix`, `shared_prefix_public_horner`), the PRG / pipe probes and the
+Eq. 1 LAN/WAN projection.  `e2e` = the same gate through fusefss_gate_host with
 pinned HOST buffers (H2D + D2H inside the timed region).  `--impl reference` times the CPU oracle instead.
 N > 1 (torchrun): every rank runs the full tensor on its own GPU (elements are independent gate instances,
 no collective); value = N * count / max-over-ranks time; scaling = "weak".

@@ -6,7 +6,8 @@
 // (Def I.1 with c_t = -beta_t, theta_t = r).  Predicate bits are the LSBs; the interval lookup is the
 // public linear map  v_{i*} = v_{m-1} + sum_i (v_{i-1} - v_i) I[x < alpha_i]  of the same comparisons (Def I.2).
 // Points whose offsets lie within 2^tail_bits of each other share the walk over their top n - tail_bits bits:
-// the two candidate prefixes of a cluster are walked once (in lock-step), every point then walks only its tail.
+// the cluster's first candidate prefix is walked once, the second one forks off it for its last few levels
+// (sp_walk_fork), every point then walks only its tail from the matching saved state.
 #pragma once
 #include "aes.cuh"
 #include "program.h"
@@ -65,19 +66,6 @@ __device__ __forceinline__ void sp_walk(uint32_t tl, const uint8_t *lvl, size_t 
         sp_load_level<PK>(pl, e, s16, s8, cw, vcw);
         sp_step<PK>(tl, cw, vcw, (uint32_t)(ubits >> 63), st);
         ubits <<= 1;
-    }
-}
-// two prefixes in lock-step over levels [0, to): same correction words, independent PRG chains
-template <int PK>
-__device__ __forceinline__ void sp_walk2(uint32_t tl, const uint8_t *lvl, size_t e, size_t s16, size_t s8, size_t lvl_stride,
-                                         int to, uint64_t u1, uint64_t u2, SpState<PK> &a, SpState<PK> &b) {
-    const uint8_t *pl = lvl;
-    for (int i = 0; i < to; ++i, pl += lvl_stride) {
-        uint4 cw; uint64_t vcw[PK];
-        sp_load_level<PK>(pl, e, s16, s8, cw, vcw);
-        sp_step<PK>(tl, cw, vcw, (uint32_t)(u1 >> 63), a);
-        sp_step<PK>(tl, cw, vcw, (uint32_t)(u2 >> 63), b);
-        u1 <<= 1; u2 <<= 1;
     }
 }
 // The two candidate prefixes u1, u2 of a cluster (top kf bits) usually differ only in their last few bits: walk u1
