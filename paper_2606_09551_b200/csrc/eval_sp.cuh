@@ -199,6 +199,13 @@ __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ Eva
             }
             const uint8_t *tree = a.key + a.vt_first;
             const uint8_t *lvl = tree + a.vt_lvl_rel;
+            if (a.G > 1) {                                                   // small tensors: too few warps to hide DRAM latency level by level,
+                for (int i = 0; i < a.n; ++i) {                              // so pull the element's correction words towards L2 up front
+                    const uint8_t *pl = lvl + (size_t)i * a.lvl_stride;
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(pl + e * 16));
+                    asm volatile("prefetch.global.L2 [%0];" ::"l"(pl + a.s16 + e * 8));
+                }
+            }
             const uint4 root = __ldg(reinterpret_cast<const uint4 *>(tree + e * 16));
             const uint8_t *fin = tree + a.vt_fin_rel;
             SpState<PK> r0;
