@@ -158,8 +158,7 @@ def measure_shared_prefix(F, torch, name, base_spec, inp, rank, world, steps, wa
         e[0].record()
         P.keygen(r_in, r_out, 0, rank * count, keys=(k0, k1))
         e[1].record()
-        for b, k in ((0, k0), (1, k1)):
-            P.eval_fused(b, k, xhat, bits[b] if sh["T"] else None, coeff[b] if sh["has_lut"] else None)
+        P.eval_fused_both(k0, k1, xhat, bits if sh["T"] else None, coeff if sh["has_lut"] else None)
         e[2].record()
         P.post_fused(k0, k1, xhat, bits[0], bits[1], coeff[0], coeff[1], outs=outs)
         e[3].record()

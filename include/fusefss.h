@@ -148,6 +148,12 @@ int fusefss_eval_lut(int party, const fusefss_program *prog, const void *key_dev
  * coeff_out_dev iff m = 1.  (eval_cmp / eval_lut remain valid for variant 1 and each walk only the points they need.) */
 int fusefss_eval_fused(int party, const fusefss_program *prog, const void *key_dev, const uint64_t *xhat_dev,
                        size_t count, uint64_t *bits_out_dev, uint64_t *coeff_out_dev, void *stream);
+/* The same for BOTH parties (one GPU runs both, north_star): for variant 1 a single launch walks both parties' keys
+ * (half the launches, twice the parallelism for small tensors); otherwise two fusefss_eval_fused calls.  Outputs equal
+ * the per-party calls bit for bit. */
+int fusefss_eval_fused_both(const fusefss_program *prog, const void *key0_dev, const void *key1_dev,
+                            const uint64_t *xhat_dev, size_t count, uint64_t *bits0_dev, uint64_t *bits1_dev,
+                            uint64_t *coeff0_dev, uint64_t *coeff1_dev, void *stream);
 
 /* ---- a7: post-processing (online steps 4-6; Horner P:895; DESIGN 4.6) ---------
  * One call per party per round.  msg_in_dev = the OTHER party's message buffer, msg_out_dev = this party's;

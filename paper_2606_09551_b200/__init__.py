@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libfusefss.so")
 # every symbol include/fusefss.h declares (tests check the library exports all of them)
 SYMBOLS = (
     "fusefss_compile", "fusefss_destroy", "fusefss_shape", "fusefss_atom", "fusefss_key_bytes", "fusefss_keygen", "fusefss_keygen_parts",
-    "fusefss_eval_cmp", "fusefss_eval_lut", "fusefss_eval_fused", "fusefss_post", "fusefss_post_rounds", "fusefss_post_msg_bytes",
+    "fusefss_eval_cmp", "fusefss_eval_lut", "fusefss_eval_fused", "fusefss_eval_fused_both", "fusefss_post", "fusefss_post_rounds", "fusefss_post_msg_bytes",
     "fusefss_online_bits", "fusefss_post_fused", "fusefss_cost", "fusefss_gate_workspace_bytes", "fusefss_gate_host",
     "fusefss_share_open", "fusefss_sub_bcast", "fusefss_row_sum", "fusefss_mul_triple_bytes", "fusefss_mul_keygen", "fusefss_mul_fused",
     "fusefss_strerror", "fusefss_last_cuda_error", "fusefss_launch_count", "fusefss_aes_probe", "fusefss_aes_kat", "fusefss_pipe_probe",
@@ -74,6 +74,7 @@ def _load():
         "fusefss_eval_cmp": (i32, [i32, vp, vp, vp, sz, vp, vp]),
         "fusefss_eval_lut": (i32, [i32, vp, vp, vp, sz, vp, vp]),
         "fusefss_eval_fused": (i32, [i32, vp, vp, vp, sz, vp, vp, vp]),
+        "fusefss_eval_fused_both": (i32, [vp, vp, vp, vp, sz, vp, vp, vp, vp, vp]),
         "fusefss_post": (i32, [i32, vp, vp, vp, vp, vp, sz, i32, vp, vp, vp, vp, vp]),
         "fusefss_post_rounds": (i32, [vp]),
         "fusefss_post_msg_bytes": (sz, [vp, sz, i32]),
@@ -244,6 +245,15 @@ class Program:
         bits = self._empty(count) if bits is None and self.shape["T"] else bits
         coeff = self._empty((self.shape["p"], count)) if coeff is None and self.shape["has_lut"] else coeff
         _check(lib.fusefss_eval_fused(party, self._h, _ptr(key), _ptr(xhat), count, _ptr(bits), _ptr(coeff), _stream()))
+        return bits, coeff
+
+    def eval_fused_both(self, key0, key1, xhat, bits=None, coeff=None):
+        count = xhat.numel()
+        bits = [self._empty(count), self._empty(count)] if bits is None and self.shape["T"] else (bits or [None, None])
+        coeff = ([self._empty((self.shape["p"], count)) for _ in (0, 1)] if coeff is None and self.shape["has_lut"]
+                 else (coeff or [None, None]))
+        _check(lib.fusefss_eval_fused_both(self._h, _ptr(key0), _ptr(key1), _ptr(xhat), count, _ptr(bits[0]), _ptr(bits[1]),
+                                           _ptr(coeff[0]), _ptr(coeff[1]), _stream()))
         return bits, coeff
 
     def post(self, party, key, xhat, bits, coeff, rnd, msg_in, msg_out, y=None, z=None):

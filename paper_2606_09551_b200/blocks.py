@@ -64,9 +64,7 @@ class Softmax:
     def _gate(self, k, x0, x1, offset=0):
         P, (k0, k1), b, c = self.progs[k], self.keys[k], self.buf[k], self.counts[k]
         _check(lib.fusefss_share_open(P._h, _ptr(k0), _ptr(k1), _ptr(x0), _ptr(x1), c, offset, _ptr(b["xhat"]), _stream()))
-        for party, key in ((0, k0), (1, k1)):
-            P.eval_fused(party, key, b["xhat"], b["bits"][party] if P.shape["T"] else None,
-                         b["coeff"][party] if P.shape["has_lut"] else None)
+        P.eval_fused_both(k0, k1, b["xhat"], b["bits"] if P.shape["T"] else None, b["coeff"] if P.shape["has_lut"] else None)
         y0, y1, _, _ = P.post_fused(k0, k1, b["xhat"], b["bits"][0], b["bits"][1], b["coeff"][0], b["coeff"][1], outs=b["out"])
         return y0[0], y1[0]
 

@@ -16,12 +16,13 @@ namespace fsk {
 
 struct SpAtomDev { uint64_t c, beta; int k, is_theta; };
 struct EvalSpArgs {
-    const uint8_t *key; const uint64_t *xhat; uint64_t *bits_out, *coeff_out;       // either output may be null
+    const uint8_t *key2[2]; const uint64_t *xhat; uint64_t *bits_out2[2], *coeff_out2[2];   // per party; either output may be null
+    int n_parties, party0;      // 1 party (party0) or both parties in one launch (items = parties x groups x tiles)
     const SpPoint *points; const uint64_t *weights, *delta_tab, *alpha;             // device tables (program blob)
     const SpCluster *cluster;
     size_t count, s16, s8, lvl_stride, vt_first, vt_lvl_rel, vt_fin_rel, rpow;
     uint64_t mask;
-    int n, m, p, party, T, n_w, n_clusters, G;   // G > 1: the points of an element are dealt round-robin to G warps (small tensors)
+    int n, m, p, pad0, T, n_w, n_clusters, G;   // G > 1: the points of an element are dealt round-robin to G warps (small tensors)
     SpWidth width[kMaxWidths];
     size_t bt_root[kMaxWidths], bt_cw[kMaxWidths], bt_vb[kMaxWidths];
     SpAtomDev atom[kMaxAtoms];
@@ -147,20 +148,24 @@ template <int P, int PK>
 __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ EvalSpArgs a) {
     extern __shared__ uint32_t sT[];
     const uint32_t tl = aes_fill_tables(sT);
-    const size_t tiles = (a.count + 31) / 32, items = tiles * (size_t)a.G, warps = (size_t)gridDim.x * (blockDim.x >> 5);
+    const size_t tiles = (a.count + 31) / 32, items = tiles * (size_t)a.G * (size_t)a.n_parties, warps = (size_t)gridDim.x * (blockDim.x >> 5);
     // warp w of CTA b takes items w*grid + b (+ k*warps): a partial last wave spreads evenly over all SMs
     for (size_t item = (size_t)(threadIdx.x >> 5) * gridDim.x + blockIdx.x; item < items; item += warps) {
-        const int g = (int)(item / tiles);                                  // this warp's share of every element's points
-        const size_t tile = item - (size_t)g * tiles;
+        const int pg = (int)(item / tiles);                                 // (party slot, group): warp-uniform
+        const size_t tile = item - (size_t)pg * tiles;
+        const int slot = pg / a.G, g = pg - slot * a.G;                     // g = this warp's share of every element's points
+        const int party = a.n_parties == 2 ? slot : a.party0;
+        const uint8_t *key = a.key2[slot];
+        uint64_t *bits_out = a.bits_out2[slot], *coeff_out = a.coeff_out2[slot];
         const size_t e0 = tile * 32 + (threadIdx.x & 31);
         const bool live = e0 < a.count;
         const size_t e = live ? e0 : a.count - 1;
         const uint64_t xh = a.xhat[e] & a.mask;
-        const bool want_bits = a.bits_out != nullptr, want_coeff = a.coeff_out != nullptr;
+        const bool want_bits = bits_out != nullptr, want_coeff = coeff_out != nullptr;
         uint64_t word = 0, acc[P];
 #pragma unroll
         for (int w = 0; w < P; ++w) acc[w] = 0;
-        if (a.party == 0 && g == 0) {                                       // public parts: e_t and the plaintext table row of xhat
+        if (party == 0 && g == 0) {                                       // public parts: e_t and the plaintext table row of xhat
             if (want_bits)
                 for (int t = 0; t < a.T; ++t) {
                     const SpAtomDev &at = a.atom[t];
@@ -170,10 +175,10 @@ __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ Eva
         }
         if (want_coeff && g == 0) {                                         // sum_t [(-r)^t] (w_{m-1} + sum_{i: xhat < alpha_i} (w_{i-1} - w_i))
             uint64_t rp[PK];
-            rp[0] = a.party == 0 ? 1ull : 0ull;
+            rp[0] = party == 0 ? 1ull : 0ull;
 #pragma unroll
-            for (int t = 1; t < PK; ++t) rp[t] = __ldg(reinterpret_cast<const unsigned long long *>(a.key + a.rpow + (size_t)(t - 1) * a.s8 + e * 8));
-            if (PK > 1 || a.party == 0) {
+            for (int t = 1; t < PK; ++t) rp[t] = __ldg(reinterpret_cast<const unsigned long long *>(key + a.rpow + (size_t)(t - 1) * a.s8 + e * 8));
+            if (PK > 1 || party == 0) {
                 for (int i = 0; i < a.m; ++i)
                     if (i == 0 || xh < a.alpha[i - 1]) {
 #pragma unroll
@@ -192,12 +197,12 @@ __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ Eva
                 const uint64_t km = (1ull << W.k) - 1ull;
                 for (int j = g; j < W.n_points; j += a.G) {
                     const uint64_t u = (((xh & km) + pts[j].delta) & km) << (64 - W.k);
-                    const uint32_t A = sp_bit_eval(tl, a.key, a.bt_root[wd], a.bt_cw[wd], a.bt_vb[wd], e, a.s16, W.k, u, a.party);
+                    const uint32_t A = sp_bit_eval(tl, key, a.bt_root[wd], a.bt_cw[wd], a.bt_vb[wd], e, a.s16, W.k, u, party);
                     word ^= pts[j].bitmask & (0ull - (uint64_t)A);
                 }
                 continue;
             }
-            const uint8_t *tree = a.key + a.vt_first;
+            const uint8_t *tree = key + a.vt_first;
             const uint8_t *lvl = tree + a.vt_lvl_rel;
             if (a.G > 1) {                                                   // small tensors: too few warps to hide DRAM latency level by level,
                 for (int i = 0; i < a.n; ++i) {                              // so pull the element's correction words towards L2 up front
@@ -209,7 +214,7 @@ __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ Eva
             const uint4 root = __ldg(reinterpret_cast<const uint4 *>(tree + e * 16));
             const uint8_t *fin = tree + a.vt_fin_rel;
             SpState<PK> r0;
-            r0.s[0] = root.x & ~3u; r0.s[1] = root.y; r0.s[2] = root.z; r0.s[3] = root.w; r0.t = (uint32_t)a.party;
+            r0.s[0] = root.x & ~3u; r0.s[1] = root.y; r0.s[2] = root.z; r0.s[3] = root.w; r0.t = (uint32_t)party;
 #pragma unroll
             for (int t = 0; t < PK; ++t) r0.V[t] = 0;
             const int n = a.n;
@@ -238,7 +243,7 @@ __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ Eva
                     if (share) { st = (u >> (64 - kf)) == pre1 ? s1 : s2; from = kf; }
                     sp_walk<PK>(tl, lvl, e, a.s16, a.s8, a.lvl_stride, from, n, from ? u << from : u, st);
                     uint64_t A[PK];
-                    sp_leaf<PK>(tl, st, fin, e, a.s8, a.party, A);
+                    sp_leaf<PK>(tl, st, fin, e, a.s8, party, A);
                     word ^= pts[j].bitmask & (0ull - (A[0] & 1ull));        // component 0 = share of I[u_j < r]
                     if (want_coeff) {
 #pragma unroll
@@ -251,16 +256,16 @@ __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ Eva
         }
         if (live) {
             if (a.G == 1) {
-                if (want_bits) a.bits_out[e] = word;
+                if (want_bits) bits_out[e] = word;
                 if (want_coeff) {
 #pragma unroll
-                    for (int w = 0; w < P; ++w) a.coeff_out[(size_t)w * a.count + e] = acc[w] & a.mask;
+                    for (int w = 0; w < P; ++w) coeff_out[(size_t)w * a.count + e] = acc[w] & a.mask;
                 }
             } else {                                                        // integer xor / add: order-independent, still bit-exact
-                if (want_bits) atomicXor(reinterpret_cast<unsigned long long *>(a.bits_out + e), (unsigned long long)word);
+                if (want_bits) atomicXor(reinterpret_cast<unsigned long long *>(bits_out + e), (unsigned long long)word);
                 if (want_coeff) {
 #pragma unroll
-                    for (int w = 0; w < P; ++w) atomicAdd(reinterpret_cast<unsigned long long *>(a.coeff_out + (size_t)w * a.count + e), (unsigned long long)acc[w]);
+                    for (int w = 0; w < P; ++w) atomicAdd(reinterpret_cast<unsigned long long *>(coeff_out + (size_t)w * a.count + e), (unsigned long long)acc[w]);
                 }
             }
         }

@@ -177,18 +177,23 @@ int launch_gen_vec_p(int p, int grid, int block, cudaStream_t st, const GenVecAr
 }
 
 // variant 1: one kernel serves eval_cmp (bits only), eval_lut (coefficients only) and the fused call (both)
+// party = 0 / 1: that party only (key, bits_out, coeff_out); party = 2: both parties in ONE launch (the *_b arguments
+// are party 1's) -- half the launches and twice the parallelism for small tensors.
 int launch_eval_sp(Program &P, int party, const void *key, const uint64_t *xhat, size_t count, uint64_t *bits_out,
-                   uint64_t *coeff_out, cudaStream_t st) {
+                   uint64_t *coeff_out, cudaStream_t st, const void *key_b = nullptr, uint64_t *bits_out_b = nullptr,
+                   uint64_t *coeff_out_b = nullptr) {
     int rc = ensure_blob(P); if (rc) return rc;
     Layout L; compute_layout(P, count, &L);
     EvalSpArgs a{};
     const uint8_t *blob = (const uint8_t *)P.dev_blob;
-    a.key = (const uint8_t *)key; a.xhat = xhat; a.bits_out = bits_out; a.coeff_out = coeff_out;
+    a.n_parties = party == 2 ? 2 : 1; a.party0 = party == 2 ? 0 : party; a.xhat = xhat;
+    a.key2[0] = (const uint8_t *)key; a.bits_out2[0] = bits_out; a.coeff_out2[0] = coeff_out;
+    a.key2[1] = (const uint8_t *)key_b; a.bits_out2[1] = bits_out_b; a.coeff_out2[1] = coeff_out_b;
     a.points = (const SpPoint *)(blob + P.dev_sp_points_off); a.weights = (const uint64_t *)(blob + P.dev_sp_weights_off);
     a.delta_tab = (const uint64_t *)(blob + P.dev_sp_delta_off); a.alpha = (const uint64_t *)(blob + P.dev_alpha_off);
     a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.lvl_stride = L.lvl_stride; a.vt_first = L.vt_first;
     a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel; a.mask = P.mask;
-    a.n = (int)P.n; a.m = (int)P.m; a.p = P.p; a.party = party; a.T = P.T; a.n_w = P.sp.n_w;
+    a.n = (int)P.n; a.m = (int)P.m; a.p = P.p; a.T = P.T; a.n_w = P.sp.n_w;
     a.n_clusters = (int)P.sp.clusters.size();
     a.cluster = (const SpCluster *)(blob + P.dev_sp_clusters_off);
     for (int w = 0; w < P.sp.n_w; ++w) { a.width[w] = P.sp.width[w]; a.bt_root[w] = L.bt_root[w]; a.bt_cw[w] = L.bt_cw[w]; a.bt_vb[w] = L.bt_vb[w]; }
@@ -198,7 +203,7 @@ int launch_eval_sp(Program &P, int party, const void *key, const uint64_t *xhat,
     const size_t tiles = (count + 31) / 32;
     int maxpts = 1;
     for (int w = 0; w < P.sp.n_w; ++w) if (P.sp.width[w].n_points > maxpts) maxpts = P.sp.width[w].n_points;
-    int G = (int)(((size_t)g_sms * 8 + tiles - 1) / tiles);
+    int G = (int)(((size_t)g_sms * 8 + tiles * a.n_parties - 1) / (tiles * a.n_parties));
     G = G < 1 ? 1 : G > 8 ? 8 : G;
     if (G > maxpts) G = maxpts;
     if (const char *f = std::getenv("FUSEFSS_FORCE_G")) { int v = std::atoi(f); if (v >= 1) G = v < maxpts ? v : maxpts; }
@@ -206,9 +211,11 @@ int launch_eval_sp(Program &P, int party, const void *key, const uint64_t *xhat,
     if (G > 1) {
         if (bits_out) CU(cudaMemsetAsync(bits_out, 0, count * 8, st));
         if (coeff_out) CU(cudaMemsetAsync(coeff_out, 0, count * 8 * (size_t)P.p, st));
+        if (bits_out_b) CU(cudaMemsetAsync(bits_out_b, 0, count * 8, st));
+        if (coeff_out_b) CU(cudaMemsetAsync(coeff_out_b, 0, count * 8 * (size_t)P.p, st));
     }
-    const int threads = threads_for(tiles * G, g_eval_threads);
-    const int grid = grid_for(tiles * G, threads);
+    const int threads = threads_for(tiles * G * a.n_parties, g_eval_threads);
+    const int grid = grid_for(tiles * G * a.n_parties, threads);
     const size_t sm = kAesSmemBytes;
     a.rpow = L.rpow;
     int lrc = FUSEFSS_E_SPEC;
@@ -218,9 +225,10 @@ int launch_eval_sp(Program &P, int party, const void *key, const uint64_t *xhat,
     FSK_SP_ROW(1) FSK_SP_ROW(2) FSK_SP_ROW(3)
 #undef FSK_SP_ROW
 #undef FSK_SP_CASE
-    if (lrc == 0 && G > 1 && P.n < 64 && coeff_out) {                      // the atomics accumulated mod 2^64: reduce to the ring
+    if (lrc == 0 && G > 1 && P.n < 64) {                                   // the atomics accumulated mod 2^64: reduce to the ring
         const size_t words = count * (size_t)P.p;
-        return launch(k_mask_words, (int)((words + 255) / 256), 256, 0, st, MaskArgs{coeff_out, words, P.mask});
+        for (uint64_t *c : {coeff_out, coeff_out_b})
+            if (c && lrc == 0) lrc = launch(k_mask_words, (int)((words + 255) / 256), 256, 0, st, MaskArgs{c, words, P.mask});
     }
     return lrc;
 }
@@ -518,6 +526,25 @@ int fusefss_eval_fused(int party, const fusefss_program *prog, const void *key_d
     return 0;
 }
 
+int fusefss_eval_fused_both(const fusefss_program *prog, const void *key0_dev, const void *key1_dev, const uint64_t *xhat_dev,
+                            size_t count, uint64_t *bits0_dev, uint64_t *bits1_dev, uint64_t *coeff0_dev, uint64_t *coeff1_dev,
+                            void *stream) {
+    const Program *P = prog_of(prog);
+    if (!P || !key0_dev || !key1_dev || !xhat_dev) return FUSEFSS_E_NULL;
+    if ((P->T > 0 && (!bits0_dev || !bits1_dev)) || (P->has_lut && (!coeff0_dev || !coeff1_dev))) return FUSEFSS_E_NULL;
+    if (count == 0) return FUSEFSS_E_COUNT;
+    if (P->T == 0 && !P->has_lut) return FUSEFSS_E_OMITTED;
+    // one launch for both parties only while a single party cannot fill the machine (less than one wave of warps)
+    if (P->variant && (count + 31) / 32 <= (size_t)g_sms * (kEvalThreads / 32)) {
+        int rc = init_device(); if (rc) return rc;
+        return launch_eval_sp(*const_cast<Program *>(P), 2, key0_dev, xhat_dev, count, P->T > 0 ? bits0_dev : nullptr,
+                              P->has_lut ? coeff0_dev : nullptr, (cudaStream_t)stream, key1_dev, P->T > 0 ? bits1_dev : nullptr,
+                              P->has_lut ? coeff1_dev : nullptr);
+    }
+    int rc = fusefss_eval_fused(0, prog, key0_dev, xhat_dev, count, bits0_dev, coeff0_dev, stream); if (rc) return rc;
+    return fusefss_eval_fused(1, prog, key1_dev, xhat_dev, count, bits1_dev, coeff1_dev, stream);
+}
+
 int fusefss_post(int party, const fusefss_program *prog, const void *key_dev, const uint64_t *xhat_dev,
                  const uint64_t *bits_dev, const uint64_t *coeff_dev, size_t count, int round, const void *msg_in_dev,
                  void *msg_out_dev, uint64_t *y_out_dev, uint64_t *z_out_dev, void *stream) {
@@ -658,8 +685,7 @@ int fusefss_gate_host(const fusefss_program *prog, const uint64_t *r_in, const u
                 CU(cudaMemcpyAsync(d_rout + (size_t)j * c, r_out + (size_t)j * count + first, c * 8, cudaMemcpyHostToDevice, st));
         int rc = fusefss_keygen(prog, d_rin, d_rout, seed, first, c, key0, key1, st); if (rc) return rc;
         if (P->T > 0 || P->has_lut) {
-            rc = fusefss_eval_fused(0, prog, key0, d_xhat, c, d_b0, d_c0, st); if (rc) return rc;
-            rc = fusefss_eval_fused(1, prog, key1, d_xhat, c, d_b1, d_c1, st); if (rc) return rc;
+            rc = fusefss_eval_fused_both(prog, key0, key1, d_xhat, c, d_b0, d_b1, d_c0, d_c1, st); if (rc) return rc;
         }
         rc = fusefss_post_fused(prog, key0, key1, d_xhat, d_b0, d_b1, d_c0, d_c1, c, d_y0, d_y1, d_z0, d_z1, st); if (rc) return rc;
         for (int j = 0; j < P->n_out_a; ++j) {

@@ -66,6 +66,13 @@ def _parity(F, orc, spec, x, r_in, r_out, seed, check_plain=True, first_elem=0):
                 assert np.array_equal(host(fb), exp["bits"][b]), spec.name + ": eval_fused bits"
             if P.shape["has_lut"]:
                 assert np.array_equal(host(fc), exp["coeff"][b]), spec.name + ": eval_fused coeff"
+    if P.shape["T"] or P.shape["has_lut"]:                  # both parties in one call
+        bb, cc = P.eval_fused_both(k0, k1, dev(xhat))
+        for b in (0, 1):
+            if P.shape["T"]:
+                assert np.array_equal(host(bb[b]), exp["bits"][b]), spec.name + ": eval_fused_both bits"
+            if P.shape["has_lut"]:
+                assert np.array_equal(host(cc[b]), exp["coeff"][b]), spec.name + ": eval_fused_both coeff"
     # fused post == per-round post, bit for bit
     y0, y1, z0, z1 = P.post_fused(k0, k1, dev(xhat), got["bits"][0], got["bits"][1], got["coeff"][0], got["coeff"][1])
     assert np.array_equal(host(y0)[:na], exp["y"][0]) and np.array_equal(host(y1)[:na], exp["y"][1])
