@@ -225,6 +225,10 @@ def main():
 
     import torch
     import torch.distributed as dist
+    if not os.path.exists(os.path.join(ROOT, "paper_2606_09551_b200", "libfusefss.so")):
+        import __graft_entry__
+        if rank == 0:
+            __graft_entry__.build()                                   # source-only checkout: compile the library first (no fallback)
     import paper_2606_09551_b200 as F
     from workloads import specs, tensors
 
