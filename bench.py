@@ -227,8 +227,14 @@ def main():
     import torch.distributed as dist
     if not os.path.exists(os.path.join(ROOT, "paper_2606_09551_b200", "libfusefss.so")):
         import __graft_entry__
-        if rank == 0:
+        if local == 0:
             __graft_entry__.build()                                   # source-only checkout: compile the library first (no fallback)
+        else:
+            for _ in range(600):                                      # other ranks of this node wait for local rank 0's build
+                if os.path.exists(os.path.join(ROOT, "paper_2606_09551_b200", "libfusefss.so")):
+                    break
+                time.sleep(1.0)
+            time.sleep(2.0)
     import paper_2606_09551_b200 as F
     from workloads import specs, tensors
 
