@@ -4,7 +4,10 @@
 #include <atomic>
 #include <cstdio>
 #include <cstdlib>
+#include <algorithm>
 #include <mutex>
+#include <utility>
+#include <vector>
 
 #include "program.h"
 #include "aes.cuh"
@@ -139,7 +142,18 @@ RoundKeys seed_round_keys(uint64_t seed) {
 }
 
 template <typename K, typename A> int launch(K kernel, int grid, int block, size_t smem, cudaStream_t st, const A &args) {
-    if (smem > 48 * 1024) { int rc = allow_smem(kernel, smem); if (rc) return rc; }
+    if (smem > 48 * 1024) {                       // opt in to > 48 KB of dynamic shared memory once per kernel (and device)
+        static std::mutex mu;
+        static std::vector<std::pair<const void *, int>> done;
+        int dev = 0;
+        CU(cudaGetDevice(&dev));
+        std::lock_guard<std::mutex> lock(mu);
+        const std::pair<const void *, int> id{reinterpret_cast<const void *>(kernel), dev};
+        if (std::find(done.begin(), done.end(), id) == done.end()) {
+            int rc = allow_smem(kernel, smem); if (rc) return rc;
+            done.push_back(id);
+        }
+    }
     kernel<<<grid, block, smem, st>>>(args);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     CU(cudaGetLastError());
