@@ -131,7 +131,9 @@ __device__ __forceinline__ void aes_last(uint32_t (&s)[4], uint32_t tl, uint32_t
 // K_i = (i, 01, .., 0f) differ only in byte 0 too, so after the initial AddRoundKey all NI*NK states agree except
 // in that byte, which feeds a single lookup of round 1 (column 0, T0): the other 15 lookups of round 1 are done
 // once and shared -- 15 + NI*NK lookups instead of 16*NI*NK.
-template <int NI, int NK, int KFIRST, bool SHARED = false>
+// UNR = rounds unrolled per loop trip: 1 for the register-hungry kernels (k_gen_vec, k_eval_lut), 3 where it measured
+// faster (k_eval_sp, k_gen_bit): profiles/r1l_unroll.md.
+template <int NI, int NK, int KFIRST, bool SHARED = false, int UNR = kAesUnroll>
 __device__ __forceinline__ void prg_blocks(uint32_t tl, const uint32_t (&x)[NI][4], uint32_t (&out)[NI][NK][4]) {
     if (SHARED && NI * NK > 1) {
         uint32_t w[4];
@@ -160,7 +162,7 @@ __device__ __forceinline__ void prg_blocks(uint32_t tl, const uint32_t (&x)[NI][
                 aes_round(out[i][k], tl, c_rk[KFIRST + k][4], c_rk[KFIRST + k][5], c_rk[KFIRST + k][6], c_rk[KFIRST + k][7]);
             }
     }
-#pragma unroll kAesUnroll
+#pragma unroll UNR
     for (int r = 2; r < 10; ++r) {
 #pragma unroll
         for (int i = 0; i < NI; ++i)

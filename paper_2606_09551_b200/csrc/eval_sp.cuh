@@ -36,7 +36,7 @@ __device__ __forceinline__ void sp_step(uint32_t tl, const uint4 cw, const uint6
     constexpr int QK = (PK + 1) / 2;
     uint32_t x[1][4] = {{st.s[0] | dbit, st.s[1], st.s[2], st.s[3]}};
     uint32_t o[1][1 + QK][4];
-    prg_blocks<1, 1 + QK, 0, true>(tl, x, o);
+    prg_blocks<1, 1 + QK, 0, true, 3>(tl, x, o);
     const uint32_t tm = 0u - st.t;
     const uint64_t tm64 = 0ull - (uint64_t)st.t;
 #pragma unroll
@@ -103,7 +103,7 @@ __device__ __forceinline__ void sp_leaf(uint32_t tl, const SpState<PK> &st, cons
     constexpr int QK = (PK + 1) / 2;
     uint32_t x[1][4] = {{st.s[0] | 2u, st.s[1], st.s[2], st.s[3]}};
     uint32_t o[1][QK][4];
-    prg_blocks<1, QK, 1, true>(tl, x, o);
+    prg_blocks<1, QK, 1, true, 3>(tl, x, o);
     const uint64_t tm64 = 0ull - (uint64_t)st.t;
 #pragma unroll
     for (int w = 0; w < PK; ++w) {
@@ -128,7 +128,7 @@ __device__ __forceinline__ uint32_t sp_bit_eval(uint32_t tl, const uint8_t *key,
         u <<= 1;
         uint32_t x[1][4] = {{s.x | dbit, s.y, s.z, s.w}};
         uint32_t o[1][1][4];
-        prg_blocks<1, 1, 0>(tl, x, o);
+        prg_blocks<1, 1, 0, false, 3>(tl, x, o);
         const uint32_t tm = 0u - tb;
         V ^= ((o[0][0][0] >> 1) & 1u) ^ (tb & (uint32_t)((vb >> i) & 1ull));
         const uint32_t tnew = (o[0][0][0] & 1u) ^ (tb & (cw.x >> dbit) & 1u);
@@ -140,7 +140,7 @@ __device__ __forceinline__ uint32_t sp_bit_eval(uint32_t tl, const uint8_t *key,
     }
     uint32_t x[1][4] = {{s.x | 2u, s.y, s.z, s.w}};
     uint32_t o[1][1][4];
-    prg_blocks<1, 1, 0>(tl, x, o);
+    prg_blocks<1, 1, 0, false, 3>(tl, x, o);
     return (V ^ ((o[0][0][0] >> 1) & 1u) ^ (tb & fin)) & 1u;
 }
 

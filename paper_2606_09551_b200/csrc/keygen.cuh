@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_bit(const __grid_constan
                 uint32_t x[2][4], ob[2][1][4];
 #pragma unroll
                 for (int d = 0; d < 2; ++d) { x[d][0] = s[b][0] | (uint32_t)d; x[d][1] = s[b][1]; x[d][2] = s[b][2]; x[d][3] = s[b][3]; }
-                prg_blocks<2, 1, 0, true>(tl, x, ob);
+                prg_blocks<2, 1, 0, true, 3>(tl, x, ob);
 #pragma unroll
                 for (int d = 0; d < 2; ++d)
 #pragma unroll
