@@ -242,6 +242,15 @@ def dcf_bit_pair(k, alpha, seed0: bytes, seed1: bytes, us):
     return o0, o1
 
 
+def dcf_bit_pair_et(k, alpha, seed0: bytes, seed1: bytes, us):
+    """early-terminated bit-DCF (variant bit 3)"""
+    us = _u64(us)
+    o0 = np.zeros(us.size, np.uint8)
+    o1 = np.zeros(us.size, np.uint8)
+    lib().orc_dcf_bit_pair_et(k, C.c_uint64(alpha), seed0, seed1, _p(us), us.size, _p(o0), _p(o1))
+    return o0, o1
+
+
 def dcf_vec_pair(k, n, p, alpha, beta, seed0: bytes, seed1: bytes, us):
     us = _u64(us)
     beta = _u64(beta)

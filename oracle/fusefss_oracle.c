@@ -23,6 +23,8 @@
  * every share to F(x)/G(x), the DCF truth table, Protocol 3's post-conditions,
  * AES-128 against FIPS-197 -- is pinned in tests/ (-m "not gpu").
  *
+ * Variant bit 3 (spec.variant & 8): early-terminated bit trees (dcf_bit_gen_et / dcf_bit_eval_et),
+ * pinned by the brute-force truth table at k = 1..12 and by exhaustive reconstruction at n = 8.
  * Variant 1 (spec.variant = 1): the single-key shared-prefix construction -- one DCF key
  * f_{r_k,1} per view width, evaluated point by point from the root (sp_eval); pinned in tests/test_oracle_sp.py.
  *
@@ -278,6 +280,101 @@ static int dcf_bit_eval(int b, int k, const bitkey *K, u64 u)
     }
     V ^= conv_bit(s) ^ (t & fin);
     return V;
+}
+
+/* Early-terminated bit-DCF (variant bit 3; SURVEY 8(f)-4 "early termination of the GGM tree").
+ * A Z_2 payload needs one bit per leaf, a PRG block has 128: the tree is cut nu = max(k-7, 0) levels deep and walks only the
+ * top nu input bits u_hi; the leaf seed expands to ONE 128-bit block whose bit u_lo (the remaining lam = min(k,7) input bits)
+ * is the leaf's output.  Levels are unchanged (scalar Z_2 contributions W, VCW; all leaves left of alpha_hi output 1 on their
+ * whole sub-range, i.e. the level payload is the scalar 1).  Leaf correction block (replaces the one-bit final CW):
+ *   L = conv128(s_0) ^ conv128(s_1) ^ X,   X_j = Valpha ^ I[j < alpha_lo],  j = 0..127,   conv128(s) = PRG_0(s, 2),
+ * so that on the alpha path (t_0 ^ t_1 = 1) the two leaf blocks differ by X and the output is I[u_lo < alpha_lo], and off the
+ * path they cancel.  Bit j of a block = bit (j mod 8) of byte (j div 8).  K->cw[nu] holds L; K->vbits bit i = VCW of level i. */
+static int et_levels(int k) { return k > 7 ? k - 7 : 0; }
+static void dcf_bit_gen_et(int k, u64 alpha, const u8 r0[16], const u8 r1[16], bitkey *K0, bitkey *K1)
+{
+    int nu = et_levels(k), lam = k - nu;
+    u64 alpha_hi = lam >= 64 ? 0 : alpha >> lam, alpha_lo = alpha & low_mask(lam);
+    u8 s[2][16];
+    memcpy(s[0], r0, 16); memcpy(s[1], r1, 16);
+    s[0][0] &= 0xFC; s[1][0] &= 0xFC;
+    memset(K0, 0, sizeof *K0); memset(K1, 0, sizeof *K1);
+    memcpy(K0->root, s[0], 16); memcpy(K1->root, s[1], 16);
+    int t[2] = { 0, 1 };
+    int Va = 0;
+    u64 vbits = 0;
+    for (int i = 0; i < nu; i++) {                       /* identical to dcf_bit_gen over the nu bits of alpha_hi */
+        int a = (int)((alpha_hi >> (nu - 1 - i)) & 1);
+        u8 S[2][2][16]; int T[2][2], W[2][2];
+        for (int b = 0; b < 2; b++) for (int d = 0; d < 2; d++) child(s[b], d, S[b][d], &T[b][d], &W[b][d]);
+        int keep = a, lose = 1 - a;
+        u8 sCW[16];
+        xor16(sCW, S[0][lose], S[1][lose]);
+        int VCW = W[1][lose] ^ W[0][lose] ^ Va ^ (lose == 0 ? 1 : 0);
+        Va = Va ^ W[1][keep] ^ W[0][keep] ^ VCW;
+        int tCW[2];
+        tCW[0] = T[0][0] ^ T[1][0] ^ a ^ 1;
+        tCW[1] = T[0][1] ^ T[1][1] ^ a;
+        memcpy(K0->cw[i], sCW, 16);
+        K0->cw[i][0] |= (u8)(tCW[0] | (tCW[1] << 1));
+        vbits |= (u64)VCW << i;
+        for (int b = 0; b < 2; b++) {
+            u8 ns[16];
+            memcpy(ns, S[b][keep], 16);
+            if (t[b]) xor16(ns, ns, sCW);
+            int nt = T[b][keep] ^ (t[b] & tCW[keep]);
+            memcpy(s[b], ns, 16);
+            t[b] = nt;
+        }
+    }
+    u8 c0[16], c1[16], L[16];
+    prg(0, s[0], 2, c0); prg(0, s[1], 2, c1);
+    xor16(L, c0, c1);
+    for (int j = 0; j < 128; j++) {
+        int xj = Va ^ ((u64)j < alpha_lo ? 1 : 0);
+        L[j >> 3] ^= (u8)(xj << (j & 7));
+    }
+    memcpy(K0->cw[nu], L, 16);
+    K0->vbits = vbits;
+    memcpy(K1->cw, K0->cw, sizeof K0->cw);
+    K1->vbits = vbits;
+}
+static int dcf_bit_eval_et(int b, int k, const bitkey *K, u64 u)
+{
+    int nu = et_levels(k), lam = k - nu;
+    u64 u_hi = lam >= 64 ? 0 : u >> lam, u_lo = u & low_mask(lam);
+    u8 s[16];
+    memcpy(s, K->root, 16);
+    s[0] &= 0xFC;
+    int t = b, V = 0;
+    for (int i = 0; i < nu; i++) {
+        int d = (int)((u_hi >> (nu - 1 - i)) & 1);
+        u8 S[16]; int T, W;
+        child(s, d, S, &T, &W);
+        V ^= W ^ (t & (int)((K->vbits >> i) & 1));
+        if (t) {
+            u8 scw[16];
+            memcpy(scw, K->cw[i], 16);
+            int tcw = (scw[0] >> d) & 1;
+            scw[0] &= 0xFC;
+            xor16(S, S, scw);
+            T ^= tcw;
+        }
+        memcpy(s, S, 16);
+        t = T;
+    }
+    u8 blk[16];
+    prg(0, s, 2, blk);
+    if (t) xor16(blk, blk, K->cw[nu]);
+    return V ^ ((blk[u_lo >> 3] >> (u_lo & 7)) & 1);
+}
+void orc_dcf_bit_pair_et(int k, u64 alpha, const u8 *seed0, const u8 *seed1, const u64 *us, int nu_, u8 *out0, u8 *out1)
+{
+    prg_init();
+    bitkey *K0 = malloc(sizeof *K0), *K1 = malloc(sizeof *K1);
+    dcf_bit_gen_et(k, alpha, seed0, seed1, K0, K1);
+    for (int i = 0; i < nu_; i++) { out0[i] = (u8)dcf_bit_eval_et(0, k, K0, us[i]); out1[i] = (u8)dcf_bit_eval_et(1, k, K1, us[i]); }
+    free(K0); free(K1);
 }
 
 /* payload group R^p = (Z_{2^n})^p */
@@ -553,6 +650,7 @@ typedef struct orc_prog {
     int r_nmul[16], r_nbits[16];
     int xmul;                         /* variant bit 1 */
     int xpoly;                        /* variant bit 2: payload = coefficients of P_i(X - r_in), Horner in the public xhat */
+    int et;                           /* variant bit 3: bit trees are early-terminated (DESIGN 13) */
     int r_narr[16];                   /* ring-element arrays opened per round: 2 per Beaver, 1 per x-product */
     int ma_is_x[64], ma_word[65];     /* per arithmetic gate: kind, first word of its material in the key */
     /* lowering memo */
@@ -757,6 +855,7 @@ orc_prog *orc_compile(const orc_spec *S0)
     P->variant = (int)(S->variant & 1);
     P->xmul = (int)((S->variant >> 1) & 1);
     P->xpoly = (int)((S->variant >> 2) & 1) && S->d >= 1 && P->m > 1;
+    P->et = (int)((S->variant >> 3) & 1);
     if (P->variant) P->M = P->m;                         /* no translated partition, hence no wrap/dummy split */
     for (int i = 0; i < 4096; i++) P->node_reg[i] = -1;
     for (int i = 0; i <= MMAX; i++) P->calpha_reg[i] = -1;
@@ -1004,6 +1103,8 @@ typedef struct {
     size_t rin, rout, ka, rpow, kb, beaver, andt, b2a_bits, b2a_a, total;
 } layout_t;
 static size_t rup256(size_t x) { return (x + 255) & ~(size_t)255; }
+/* 16-byte correction arrays of a bit tree on k bits: k levels, or (early termination) max(k-7,0) levels + the leaf block */
+static size_t bit_arrays(const struct orc_prog *P, int k);
 static void layout(const orc_prog *P, size_t count, layout_t *L)
 {
     size_t off = 0;
@@ -1016,7 +1117,7 @@ static void layout(const orc_prog *P, size_t count, layout_t *L)
         for (int w = 0; w < P->n_w; w++) {
             if (P->wk[w] < P->n) {
                 L->bt_root[w] = off; off += L->s16;
-                L->bt_cw[w] = off; off += L->s16 * (size_t)P->wk[w];
+                L->bt_cw[w] = off; off += L->s16 * bit_arrays(P, P->wk[w]);
                 L->bt_vb[w] = off; off += L->s8;
             } else {
                 L->vt_root[1] = off; off += L->s16;
@@ -1027,7 +1128,7 @@ static void layout(const orc_prog *P, size_t count, layout_t *L)
     }
     for (int t = 0; t < P->T && !P->variant; t++) {
         L->bt_root[t] = off; off += L->s16;
-        L->bt_cw[t] = off; off += L->s16 * (size_t)P->atoms[t].k;
+        L->bt_cw[t] = off; off += L->s16 * bit_arrays(P, P->atoms[t].k);
         L->bt_vb[t] = off; off += L->s8;
     }
     if (!P->variant) L->lvl_stride = L->s16 + (size_t)P->p * L->s8;
@@ -1050,6 +1151,7 @@ static void layout(const orc_prog *P, size_t count, layout_t *L)
     L->b2a_a = off; off += (size_t)P->GMIX * L->s8;
     L->total = off;
 }
+static size_t bit_arrays(const orc_prog *P, int k) { return P->et ? (size_t)et_levels(k) + 1 : (size_t)k; }
 size_t orc_key_bytes(const orc_prog *P, size_t count) { layout_t L; layout(P, count, &L); return L.total; }
 
 /* ------------------------------------------------------------------------- */
@@ -1104,11 +1206,12 @@ void orc_keygen(const orc_prog *P, const u64 *r_in, const u64 *r_out, u64 seed, 
                 int k = P->wk[w];
                 if (k < n) {
                     rnd(&ks, ge, SLOT_BT_ROOT + 2 * w, rb); rnd(&ks, ge, SLOT_BT_ROOT + 2 * w + 1, rb1);
-                    dcf_bit_gen(k, r & low_mask(k), rb, rb1, bk0, bk1);
+                    if (P->et) dcf_bit_gen_et(k, r & low_mask(k), rb, rb1, bk0, bk1);
+                    else dcf_bit_gen(k, r & low_mask(k), rb, rb1, bk0, bk1);
                     bitkey *bk[2] = { bk0, bk1 };
                     for (int b = 0; b < 2; b++) {
                         st16(key[b], L.bt_root[w], e, bk[b]->root);
-                        for (int i = 0; i < k; i++) st16(key[b], L.bt_cw[w] + (size_t)i * L.s16, e, bk[b]->cw[i]);
+                        for (int i = 0; i < (int)bit_arrays(P, k); i++) st16(key[b], L.bt_cw[w] + (size_t)i * L.s16, e, bk[b]->cw[i]);
                         st8(key[b], L.bt_vb[w], e, bk[b]->vbits);
                     }
                 } else {
@@ -1146,11 +1249,12 @@ void orc_keygen(const orc_prog *P, const u64 *r_in, const u64 *r_out, u64 seed, 
                 kbits |= (u64)w << a->carry_idx;
             }
             rnd(&ks, ge, SLOT_BT_ROOT + 2 * t, rb); rnd(&ks, ge, SLOT_BT_ROOT + 2 * t + 1, rb1);
-            dcf_bit_gen(a->k, theta, rb, rb1, bk0, bk1);
+            if (P->et) dcf_bit_gen_et(a->k, theta, rb, rb1, bk0, bk1);
+            else dcf_bit_gen(a->k, theta, rb, rb1, bk0, bk1);
             bitkey *bk[2] = { bk0, bk1 };
             for (int b = 0; b < 2; b++) {
                 st16(key[b], L.bt_root[t], e, bk[b]->root);
-                for (int i = 0; i < a->k; i++) st16(key[b], L.bt_cw[t] + (size_t)i * L.s16, e, bk[b]->cw[i]);
+                for (int i = 0; i < (int)bit_arrays(P, a->k); i++) st16(key[b], L.bt_cw[t] + (size_t)i * L.s16, e, bk[b]->cw[i]);
                 st8(key[b], L.bt_vb[t], e, bk[b]->vbits);
             }
         }
@@ -1267,9 +1371,10 @@ static void sp_eval_points(int party, const orc_prog *P, const u8 *key, const la
         u64 km = low_mask(k);
         if (k < n) {
             ld16(key, L->bt_root[w], e, bk->root);
-            for (int i = 0; i < k; i++) ld16(key, L->bt_cw[w] + (size_t)i * L->s16, e, bk->cw[i]);
+            for (int i = 0; i < (int)bit_arrays(P, k); i++) ld16(key, L->bt_cw[w] + (size_t)i * L->s16, e, bk->cw[i]);
             bk->vbits = ld8(key, L->bt_vb[w], e);
-            for (int j = 0; j < P->w_npts[w]; j++) A[w][j] = (u64)dcf_bit_eval(party, k, bk, (xh + P->w_delta[w][j]) & km);
+            for (int j = 0; j < P->w_npts[w]; j++)
+                A[w][j] = (u64)(P->et ? dcf_bit_eval_et(party, k, bk, (xh + P->w_delta[w][j]) & km) : dcf_bit_eval(party, k, bk, (xh + P->w_delta[w][j]) & km));
         } else {
             ld16(key, L->vt_root[1], e, vk->root);
             for (int i = 0; i < n; i++) {
@@ -1365,11 +1470,11 @@ void orc_eval_cmp(int party, const orc_prog *P, const u8 *key, const u64 *xhat, 
         for (int t = 0; t < P->T; t++) {
             const atom_t *a = &P->atoms[t];
             ld16(key, L.bt_root[t], e, bk->root);
-            for (int i = 0; i < a->k; i++) ld16(key, L.bt_cw[t] + (size_t)i * L.s16, e, bk->cw[i]);
+            for (int i = 0; i < (int)bit_arrays(P, a->k); i++) ld16(key, L.bt_cw[t] + (size_t)i * L.s16, e, bk->cw[i]);
             bk->vbits = ld8(key, L.bt_vb[t], e);
             /* view_{k,c}(xhat) = ((xhat mod 2^k) + c) mod 2^k */
             u64 u = ((xhat[e] & low_mask(a->k)) + a->c) & low_mask(a->k);
-            word |= (u64)dcf_bit_eval(party, a->k, bk, u) << t;
+            word |= (u64)(P->et ? dcf_bit_eval_et(party, a->k, bk, u) : dcf_bit_eval(party, a->k, bk, u)) << t;
         }
         bits_out[e] = word;
     }

@@ -100,3 +100,131 @@ def random_spec(seed, variant=0):
                  mask_output=bool(rng.random() < 0.3), out_frac=f)
     spec.variant = variant if (not (variant & 4) or d <= 2) else variant & 3
     return spec
+
+
+# ---- brute-force harness shared by test_oracle_gate.py / test_oracle_sp.py ------------------------------------------
+def pmap(fn, items, workers=None):
+    """Run fn over items on a thread pool.  The oracle is plain single-threaded C behind ctypes, which releases the GIL for
+    the duration of every call, and it keeps no mutable global state after orc_compile() (its AES tables are filled
+    there), so independent calls run on all host cores.  This is what makes the exhaustive pins affordable; the
+    oracle's arithmetic itself stays single-threaded.  Exceptions (assertion failures) propagate."""
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    items = list(items)
+    workers = workers or min(len(items), os.cpu_count() or 1)
+    if workers <= 1:
+        return [fn(it) for it in items]
+    with ThreadPoolExecutor(max_workers=workers) as ex:
+        return list(ex.map(fn, items))
+
+
+def expected_atoms(P, x, r_in, n):
+    """The T bits the packed comparison must reconstruct to, from their plain definitions (Def I.1).
+    Protocol-3 construction: atom t = I[view_{k,c}(xhat) < theta_t], theta_t = (r_k + beta_t) mod 2^k (r-atom: r_k).
+    Single-key construction (variant bit 0): a theta-atom IS the predicate I[view_{k,c}(x) < beta_t]; r-atoms as above."""
+    xhat = (x + r_in) & mask_of(n)
+    sp = bool(getattr(P.spec, "variant", 0) & 1)
+    rows = []
+    for t in range(P.shape["T"]):
+        a = P.atom(t)
+        K = np.uint64((1 << a["k"]) - 1) if a["k"] < 64 else np.uint64(0xFFFFFFFFFFFFFFFF)
+        u = ((xhat & K) + np.uint64(a["c"])) & K
+        rk = r_in & K
+        if not a["is_theta"]:
+            rows.append(u < rk)
+        elif sp:
+            rows.append((((x & K) + np.uint64(a["c"])) & K) < np.uint64(a["beta"]))
+        else:
+            rows.append(u < ((rk + np.uint64(a["beta"])) & K))
+    return rows
+
+
+def check_gate_outputs(P, spec, x, r_in, r_out, out, calls=True):
+    """Lemma 4.5 / Thm 4.6: the two parties' outputs reconstruct to the plaintext G(x) (Tier A), and
+    (calls=True) each of the two FSS calls reconstructs to its plain definition: Def I.1 bits, Def I.2 = the payload of
+    the interval that contains x.  x, r_in: arrays of the same length; r_out: [n_out_a, count] or None."""
+    n = spec.n
+    M = mask_of(n)
+    ye, ze = P.plain_G(x, r_in)
+    if spec.mask_output:
+        ye = (ye + r_out[: ye.shape[0]]) & M
+    assert np.array_equal((out["y"][0] + out["y"][1]) & M, ye), (spec.name, "y")
+    if P.shape["n_out_b"]:
+        assert np.array_equal(out["z"][0] ^ out["z"][1], pack_bits(ze)), (spec.name, "z")
+    if not calls:
+        return
+    word = out["bits"][0] ^ out["bits"][1]
+    for t, want in enumerate(expected_atoms(P, x, r_in, n)):
+        got = (word >> np.uint64(t)) & np.uint64(1)
+        assert np.array_equal(got, want.astype(np.uint64)), (spec.name, "atom", t)
+    if P.shape["has_lut"] and not (getattr(spec, "variant", 0) & 4):
+        c = (out["coeff"][0] + out["coeff"][1]) & M
+        i_star = np.searchsorted(np.array([0] + spec.alpha, dtype=np.uint64), x, side="right") - 1
+        pay = np.concatenate([spec.coeff.reshape(spec.m, -1), spec.aux.reshape(spec.m, -1)], axis=1) & M
+        assert np.array_equal(c, pay[i_star].T), (spec.name, "lookup")
+
+
+def r_out_for(P, n, count):
+    na = max(1, P.shape["n_out_a"])
+    return ((np.arange(count * na, dtype=np.uint64) * np.uint64(2654435761)) & mask_of(n)).reshape(na, count)
+
+
+def check_all_r(orc, spec, xs, seed=11, calls=True):
+    """Every mask r in Z_{2^n} (both Protocol 3 branches) for each x in xs.  The keys depend on r only, so they
+    are generated once (in parallel chunks: the dealer's randomness is indexed by the global element) and every x
+    re-uses them."""
+    P = orc.Program(spec)
+    n = spec.n
+    N = 1 << n
+    r_in = np.arange(N, dtype=np.uint64)
+    r_out = r_out_for(P, n, N)
+    step = max(32, N // 8)
+    parts = pmap(lambda lo: P.keygen(r_in[lo:lo + step], np.ascontiguousarray(r_out[:, lo:lo + step]), seed, first_elem=lo),
+                 range(0, N, step))
+
+    def one(x):
+        xv = np.full(N, x, dtype=np.uint64)
+        xhat = (xv + r_in) & mask_of(n)
+        for lo, (k0, k1) in zip(range(0, N, step), parts):
+            sl = slice(lo, lo + step)
+            out = P.run_gate(k0, k1, xhat[sl])
+            check_gate_outputs(P, spec, xv[sl], r_in[sl], r_out[:, sl], out, calls)
+    pmap(one, xs)
+    return P
+
+
+def check_pairs(orc, spec, x, r_in, seed=11, calls=True, chunk=2048):
+    """Arbitrary (x, r) pairs: keygen + both calls + post for every pair, in parallel chunks."""
+    P = orc.Program(spec)
+    n = spec.n
+    count = x.size
+    r_out = r_out_for(P, n, count)
+
+    def one(lo):
+        sl = slice(lo, min(count, lo + chunk))
+        ro = np.ascontiguousarray(r_out[:, sl])
+        k0, k1 = P.keygen(r_in[sl], ro, seed, first_elem=lo)
+        out = P.run_gate(k0, k1, (x[sl] + r_in[sl]) & mask_of(n))
+        check_gate_outputs(P, spec, x[sl], r_in[sl], ro, out, calls)
+    pmap(one, range(0, count, chunk))
+    return P
+
+
+def corner_masks(spec, extra=3, seed=0):
+    """Masks that hit Protocol 3's corner cases: r = 0 and r = -alpha_i (a translated start lands on 0: the beta_0 = 0
+    branch with its dummy split), r = N-1, r = N/2, plus a few seeded random ones."""
+    N = 1 << spec.n
+    rng = np.random.default_rng(seed)
+    rs = [0, N - 1, N // 2, 1] + [(N - a) % N for a in spec.alpha] + [int(v) for v in rng.integers(0, N, extra)]
+    return sorted(set(rs))
+
+
+def corner_inputs(spec, extra=3, seed=0):
+    """x on, just below and just above every interval boundary, the ring's ends and the sign change, plus random ones."""
+    N = 1 << spec.n
+    rng = np.random.default_rng(seed + 100)
+    xs = [0, 1, N - 1, N // 2, N // 2 - 1]
+    for a in spec.alpha:
+        xs += [a, (a - 1) % N, (a + 1) % N]
+    xs += [int(v) for v in rng.integers(0, N, extra)]
+    return sorted(set(xs))

@@ -1,12 +1,14 @@
 """Tier B (keyed algorithm) pinned to Tier A (plaintext semantics) and Tier A pinned to closed forms.
 Lemma 4.5 / Thm 4.6: reconstructing the two parties' outputs gives G(x) for EVERY
-x and EVERY mask r.  Exhaustive at n = 8; all x with sampled r and all r with sampled x at n = 12."""
+x and EVERY mask r.  Exhaustive (every x, every r) at n = 8 for every spec; at n = 12 all x with sampled r (incl. r = 0,
+r = -alpha_i, r = N-1) and all r with sampled x (incl. every alpha_i, alpha_i - 1).  The loops run on all host cores
+(tests/helpers.pmap: the oracle's C calls release the GIL); the oracle itself is single-threaded."""
 import os
 
 import numpy as np
 import pytest
 
-from helpers import all_r_keys, mask_of, pack_bits
+from helpers import all_r_keys, check_all_r, check_pairs, corner_inputs, corner_masks, mask_of, pack_bits, pmap
 from workloads import specs
 
 GOLD = os.path.join(os.path.dirname(__file__), "golden")
@@ -17,60 +19,37 @@ def _signed(v, n):
     return np.where(v >= (1 << (n - 1)), v - (1 << n), v)
 
 
-def _check_all_r(orc, spec, xs, seed=11):
-    P = orc.Program(spec)
-    n = spec.n
-    N = 1 << n
-    na = P.shape["n_out_a"]
-    r_out = (np.arange(N * max(1, na), dtype=np.uint64) * np.uint64(2654435761)) & mask_of(n)
-    r_in, (k0, k1) = all_r_keys(P, n, seed, r_out)
-    for x in xs:
-        xv = np.full(N, x, dtype=np.uint64)
-        xhat = (xv + r_in) & mask_of(n)
-        out = P.run_gate(k0, k1, xhat)
-        ye, ze = P.plain_G(xv, r_in)
-        if spec.mask_output:
-            ye = (ye + r_out.reshape(-1, N)[: ye.shape[0]]) & mask_of(n)
-        y = (out["y"][0] + out["y"][1]) & mask_of(n)
-        assert np.array_equal(y, ye), (spec.name, x)
-        if P.shape["n_out_b"]:
-            assert np.array_equal(out["z"][0] ^ out["z"][1], pack_bits(ze)), (spec.name, x)
-        # the two calls reconstruct to their plain definitions (Def I.1 / I.2)
-        for t in range(P.shape["T"]):
-            a = P.atom(t)
-            K = np.uint64((1 << a["k"]) - 1)
-            u = ((xhat & K) + np.uint64(a["c"])) & K
-            rk = r_in & K
-            theta = (rk + np.uint64(a["beta"])) & K if a["is_theta"] else rk
-            got = ((out["bits"][0] ^ out["bits"][1]) >> np.uint64(t)) & np.uint64(1)
-            assert np.array_equal(got, (u < theta).astype(np.uint64)), (spec.name, t)
-        if P.shape["has_lut"]:
-            c = (out["coeff"][0] + out["coeff"][1]) & mask_of(n)
-            i_star = np.searchsorted(np.array([0] + spec.alpha), np.uint64(x), side="right") - 1
-            pay = np.concatenate([spec.coeff[i_star].reshape(-1), spec.aux[i_star].reshape(-1)])
-            assert np.array_equal(c, np.repeat(pay[:, None], N, axis=1)), (spec.name, x)
-    return P
-
-
 SPECS8 = [lambda: specs.relu(8, 4), lambda: specs.toy(8, 3), lambda: specs.toy(8, 3, True),
           lambda: specs.plain_default(8, 3), lambda: specs.single_interval(8, 3), lambda: specs.no_bits(8, 3),
           lambda: specs.full_partition(3), lambda: specs.shift_relu(8, 3)]
+SPECS12 = [lambda: specs.relu(12, 6), lambda: specs.shift_relu(12, 4), lambda: specs.toy(12, 4)]
 
 
 @pytest.mark.parametrize("mk", SPECS8)
 def test_reconstruct_equals_plaintext_exhaustive_n8(orc, mk):
+    """EVERY x and EVERY mask r at n = 8 (65,536 instances per spec; full_partition: n = 3): the gate's outputs, the packed
+    comparison's bits and the interval lookup's payload all reconstruct to their plain definitions."""
+    spec = mk()
+    check_all_r(orc, spec, range(1 << spec.n))
+
+
+@pytest.mark.parametrize("mk", SPECS12)
+def test_reconstruct_all_x_sampled_r_n12(orc, mk):
+    """n = 12: all 4,096 x for each of >= 8 masks, among them r = 0, r = -alpha_i (beta_0 = 0 branch), r = N-1."""
     spec = mk()
     N = 1 << spec.n
-    xs = range(N) if spec.name in ("relu_n8", "shift_relu_n8", "full_n3") else list(range(0, N, 5)) + [N - 1, N // 2, N // 2 - 1]
-    _check_all_r(orc, spec, xs)
+    rs = corner_masks(spec, extra=4, seed=12)
+    assert len(rs) >= 8
+    x = np.tile(np.arange(N, dtype=np.uint64), len(rs))
+    r = np.repeat(np.array(rs, dtype=np.uint64), N)
+    check_pairs(orc, spec, x, r)
 
 
-@pytest.mark.parametrize("mk", [lambda: specs.relu(12, 6), lambda: specs.shift_relu(12, 4), lambda: specs.toy(12, 4)])
-def test_reconstruct_equals_plaintext_n12(orc, mk):
+@pytest.mark.parametrize("mk", SPECS12)
+def test_reconstruct_all_r_sampled_x_n12(orc, mk):
+    """n = 12: all 4,096 masks r for x on / just below / just above every alpha_i, the ring's ends, the sign change."""
     spec = mk()
-    rng = np.random.default_rng(12)
-    xs = [0, 2047, 2048, 4095] + [int(v) for v in rng.integers(0, 4096, 1)]
-    _check_all_r(orc, spec, xs)
+    check_all_r(orc, spec, corner_inputs(spec, extra=3, seed=12))
 
 
 def test_appendix_N_relu_golden(orc):
@@ -201,9 +180,20 @@ def test_ars_gate_closed_form(orc, n, f, variant):
     P = orc.Program(spec)
     N = 1 << n
     r_in, (k0, k1) = all_r_keys(P, n, 21)
-    for x in (range(N) if n == 8 else list(range(0, N, 331)) + [N - 1, N // 2, N // 2 - 1]):
+
+    def one(x):
         xs = x - N if x >= N // 2 else x
         want = np.uint64((xs >> f) % N)
         xp = np.full(N, (x + N // 2) % N, dtype=np.uint64)               # x' = x + 2^{n-1}
         out = P.run_gate(k0, k1, (xp + r_in) & mask_of(n))
         assert np.all(((out["y"][0] + out["y"][1]) & mask_of(n)) == want), (n, f, x)
+    pmap(one, range(N) if n == 8 else sorted(set(list(range(0, N, 37)) + [N - 1, N // 2, N // 2 - 1, N // 2 + 1, (1 << f) - 1, 1 << f])))
+    if n == 12:                                                          # and every x for a few masks
+        rs = np.array([0, 1, N - 1, N // 2, N // 2 - 1, 1234, 3001, (1 << f) - 1], dtype=np.uint64)
+        x = np.tile(np.arange(N, dtype=np.uint64), rs.size)
+        r = np.repeat(rs, N)
+        ka, kb = P.keygen(r, None, 22)
+        out = P.run_gate(ka, kb, (((x + np.uint64(N // 2)) & mask_of(n)) + r) & mask_of(n))
+        xs = x.astype(np.int64)
+        xs = np.where(xs >= N // 2, xs - N, xs)
+        assert np.array_equal((out["y"][0][0] + out["y"][1][0]) & mask_of(n), ((xs >> f) % N).astype(np.uint64))

@@ -50,6 +50,36 @@ def test_dcf_bit_other_widths(orc, k):
         assert np.array_equal(o0 ^ o1, (us < int(alpha)).astype(np.uint8))
 
 
+@pytest.mark.parametrize("k", [1, 2, 3, 5, 6, 7, 8, 9, 10, 12])
+def test_dcf_bit_early_termination_truth_table(orc, k):
+    """Early-terminated bit-DCF (variant bit 3, DESIGN 13): Eval_0 xor Eval_1 = I[u < alpha] for every (alpha, u) at k <= 9
+    (k <= 7: the whole function is one leaf block; k = 8, 9: 1-2 levels + leaf), all u for sampled alpha at k = 10, 12."""
+    from helpers import pmap
+    K = 1 << k
+    us = np.arange(K, dtype=np.uint64)
+    rng0 = np.random.default_rng(k)
+    alphas = range(K) if k <= 9 else sorted({0, 1, K - 1, K // 2, 127, 128, 129, K - 128, K - 127} | {int(v) for v in rng0.integers(0, K, 40)})
+
+    def one(alpha):
+        rng = np.random.default_rng([k, alpha])
+        o0, o1 = orc.dcf_bit_pair_et(k, int(alpha), rng.bytes(16), rng.bytes(16), us)
+        assert np.array_equal(o0 ^ o1, (us < int(alpha)).astype(np.uint8)), (k, alpha)
+        return int(o0.sum())
+    ones = sum(pmap(one, alphas))
+    if k >= 5:
+        assert 0.35 < ones / (len(alphas) * K) < 0.65    # a single party's share is not the value itself
+
+
+def test_dcf_bit_early_termination_k64_edges(orc):
+    rng = np.random.default_rng(17)
+    top = (1 << 64) - 1
+    for alpha in [0, 1, 127, 128, 1 << 63, top, top - 127, (1 << 63) + 12345, 0x0123456789ABCDEF]:
+        near = [alpha + d for d in range(-130, 131, 13) if 0 <= alpha + d <= top]
+        us = np.array([0, 1, 127, 128, 1 << 63, top] + near, dtype=np.uint64)
+        o0, o1 = orc.dcf_bit_pair_et(64, alpha, rng.bytes(16), rng.bytes(16), us)
+        assert np.array_equal(o0 ^ o1, np.array([int(int(u) < alpha) for u in us], dtype=np.uint8)), alpha
+
+
 def test_dcf_bit_k64_edges(orc):
     rng = np.random.default_rng(7)
     top = (1 << 64) - 1
@@ -63,14 +93,38 @@ def test_dcf_bit_k64_edges(orc):
 @pytest.mark.parametrize("n,p", [(8, 1), (8, 2), (8, 3), (8, 7), (16, 2)])
 def test_dcf_vec_exhaustive_k8(orc, n, p):
     """every (alpha, u) at k = 8, payload in (Z_2^n)^p: Eval_0 + Eval_1 = beta * I[u < alpha]."""
+    from helpers import pmap
     us = np.arange(256, dtype=np.uint64)
-    rng = np.random.default_rng(n * 10 + p)
     mask = np.uint64((1 << n) - 1)
-    for alpha in range(0, 256, 1 if p <= 2 and n == 8 else 5):
+
+    def one(alpha):
+        rng = np.random.default_rng([n, p, alpha])
         beta = rng.integers(0, 1 << n, p, dtype=np.uint64)
         o0, o1 = orc.dcf_vec_pair(8, n, p, alpha, beta, rng.bytes(16), rng.bytes(16), us)
         exp = np.where((us < alpha)[:, None], beta[None, :], np.uint64(0))
         assert np.array_equal((o0 + o1) & mask, exp), alpha
+        return int(o0[:, 0].sum() & mask)
+    shares = pmap(one, range(256))
+    assert len(set(shares)) > 100            # a single party's share is not the value itself (256 draws mod 2^n)
+
+
+@pytest.mark.parametrize("n,p,k", [(12, 3, 12), (64, 3, 12), (64, 8, 10)])
+def test_dcf_vec_all_u_sampled_alpha(orc, n, p, k):
+    """k = 10 / 12 input bits: all u for sampled alpha (incl. 0, 1, 2^k - 1, 2^{k-1})."""
+    from helpers import pmap
+    K = 1 << k
+    us = np.arange(K, dtype=np.uint64)
+    mask = np.uint64((1 << n) - 1) if n < 64 else np.uint64(0xFFFFFFFFFFFFFFFF)
+    rng0 = np.random.default_rng(k * 100 + p)
+
+    def one(alpha):
+        rng = np.random.default_rng([n, p, alpha])
+        beta = rng.integers(0, 1 << 63, p, dtype=np.uint64) * np.uint64(2) + np.uint64(1)
+        beta &= mask
+        o0, o1 = orc.dcf_vec_pair(k, n, p, alpha, beta, rng.bytes(16), rng.bytes(16), us)
+        exp = np.where((us < alpha)[:, None], beta[None, :], np.uint64(0))
+        assert np.array_equal((o0 + o1) & mask, exp), alpha
+    pmap(one, [0, 1, K - 1, K // 2, K // 2 - 1] + [int(v) for v in rng0.integers(0, K, 11)])
 
 
 def test_dcf_vec_k64(orc):

@@ -2,11 +2,12 @@
 One DCF key f_{r_k,1} per view width, evaluated at the public points (xhat + delta) mod 2^k:
   I[view_{k,c}(x) < beta] = e - b + a,  h = (xhat + c) mod 2^k, e = I[h < beta], b = I[h < r_k], a = I[(h - beta) mod 2^k < r_k].
 Pinned by brute force: the identity itself, and reconstruction of both calls and of the whole gate to the
-plaintext F(x) / G(x) for every x and every mask r at n = 8 (sampled at n = 12)."""
+plaintext F(x) / G(x) for EVERY x and EVERY mask r at n = 8 (all specs, all variant bits); at n = 12 all x for the corner
+masks and all r for the corner inputs (tests/helpers.py: corner_masks, corner_inputs)."""
 import numpy as np
 import pytest
 
-from helpers import all_r_keys, mask_of, pack_bits
+from helpers import all_r_keys, check_all_r, check_pairs, corner_inputs, corner_masks, mask_of, pack_bits
 from workloads import specs
 
 
@@ -26,59 +27,33 @@ def test_identity_exhaustive():
             assert np.array_equal(want, e ^ b ^ a)
 
 
-def _check_all_r(orc, spec, xs, seed=13):
-    P = orc.Program(spec)
-    n = spec.n
-    N = 1 << n
-    na = P.shape["n_out_a"]
-    r_out = (np.arange(N * max(1, na), dtype=np.uint64) * np.uint64(2654435761)) & mask_of(n)
-    r_in, (k0, k1) = all_r_keys(P, n, seed, r_out)
-    for x in xs:
-        xv = np.full(N, x, dtype=np.uint64)
-        xhat = (xv + r_in) & mask_of(n)
-        out = P.run_gate(k0, k1, xhat)
-        ye, ze = P.plain_G(xv, r_in)
-        if spec.mask_output:
-            ye = (ye + r_out.reshape(-1, N)[: ye.shape[0]]) & mask_of(n)
-        assert np.array_equal((out["y"][0] + out["y"][1]) & mask_of(n), ye), (spec.name, x)
-        if P.shape["n_out_b"]:
-            assert np.array_equal(out["z"][0] ^ out["z"][1], pack_bits(ze)), (spec.name, x)
-        for t in range(P.shape["T"]):                       # Def I.1 with c_t = -beta_t, theta = r
-            a = P.atom(t)
-            K = np.uint64((1 << a["k"]) - 1)
-            got = ((out["bits"][0] ^ out["bits"][1]) >> np.uint64(t)) & np.uint64(1)
-            if a["is_theta"]:
-                want = (((xv & K) + np.uint64(a["c"])) & K) < np.uint64(a["beta"])
-            else:
-                want = (((xhat & K) + np.uint64(a["c"])) & K) < (r_in & K)
-            assert np.array_equal(got, want.astype(np.uint64)), (spec.name, t)
-        if P.shape["has_lut"]:                               # Def I.2: the active interval's payload
-            c = (out["coeff"][0] + out["coeff"][1]) & mask_of(n)
-            i_star = np.searchsorted(np.array([0] + spec.alpha), np.uint64(x), side="right") - 1
-            pay = np.concatenate([spec.coeff[i_star].reshape(-1), spec.aux[i_star].reshape(-1)]) & mask_of(n)
-            assert np.array_equal(c, np.repeat(pay[:, None], N, axis=1)), (spec.name, x)
-    return P
-
-
 SPECS8 = [lambda: specs.relu(8, 4), lambda: specs.toy(8, 3), lambda: specs.toy(8, 3, True),
           lambda: specs.plain_default(8, 3), lambda: specs.single_interval(8, 3), lambda: specs.no_bits(8, 3),
           lambda: specs.full_partition(3), lambda: specs.shift_relu(8, 3)]
+SPECS12 = [lambda: specs.relu(12, 6), lambda: specs.shift_relu(12, 4), lambda: specs.toy(12, 4)]
 
 
 @pytest.mark.parametrize("mk", SPECS8)
 def test_sp_reconstruct_equals_plaintext_exhaustive_n8(orc, mk):
+    """EVERY x and EVERY mask r at n = 8: gate outputs = G(x); atoms = the predicates themselves (Def I.1 with c_t = -beta_t,
+    theta_t = r); the lookup = the active interval's payload (Def I.2)."""
+    spec = specs.shared_prefix(mk())
+    check_all_r(orc, spec, range(1 << spec.n), seed=13)
+
+
+@pytest.mark.parametrize("mk", SPECS12)
+def test_sp_reconstruct_all_x_sampled_r_n12(orc, mk):
     spec = specs.shared_prefix(mk())
     N = 1 << spec.n
-    xs = range(N) if spec.name.startswith(("relu_n8", "shift_relu_n8", "full_n3")) else list(range(0, N, 5)) + [N - 1, N // 2, N // 2 - 1]
-    _check_all_r(orc, spec, xs)
+    rs = corner_masks(spec, extra=4, seed=13)
+    assert len(rs) >= 8
+    check_pairs(orc, spec, np.tile(np.arange(N, dtype=np.uint64), len(rs)), np.repeat(np.array(rs, dtype=np.uint64), N), seed=13)
 
 
-@pytest.mark.parametrize("mk", [lambda: specs.relu(12, 6), lambda: specs.shift_relu(12, 4), lambda: specs.toy(12, 4)])
-def test_sp_reconstruct_n12(orc, mk):
+@pytest.mark.parametrize("mk", SPECS12)
+def test_sp_reconstruct_all_r_sampled_x_n12(orc, mk):
     spec = specs.shared_prefix(mk())
-    rng = np.random.default_rng(12)
-    xs = [0, 2047, 2048, 4095] + [int(v) for v in rng.integers(0, 4096, 1)]
-    _check_all_r(orc, spec, xs)
+    check_all_r(orc, spec, corner_inputs(spec, extra=3, seed=13), seed=13)
 
 
 def test_sp_shapes_and_key_size(orc):
@@ -115,26 +90,7 @@ def test_xmul_reconstruct_exhaustive_n8(orc, mk, sp):
     """y * x with x = xhat - r_in opens one element instead of two; the gate still reconstructs to G(x) for
     every x and r, with both constructions."""
     spec = specs.input_masked_mul(specs.shared_prefix(mk()) if sp else mk())
-    N = 1 << spec.n
-    _check_all_r(orc, spec, list(range(0, N, 5)) + [N - 1]) if sp else _check_plain_only(orc, spec, list(range(0, N, 5)) + [N - 1])
-
-
-def _check_plain_only(orc, spec, xs, seed=17):
-    P = orc.Program(spec)
-    n = spec.n
-    N = 1 << n
-    na = P.shape["n_out_a"]
-    r_out = (np.arange(N * max(1, na), dtype=np.uint64) * np.uint64(40503)) & mask_of(n)
-    r_in, (k0, k1) = all_r_keys(P, n, seed, r_out)
-    for x in xs:
-        xv = np.full(N, x, dtype=np.uint64)
-        out = P.run_gate(k0, k1, (xv + r_in) & mask_of(n))
-        ye, ze = P.plain_G(xv, r_in)
-        if spec.mask_output:
-            ye = (ye + r_out.reshape(-1, N)[: ye.shape[0]]) & mask_of(n)
-        assert np.array_equal((out["y"][0] + out["y"][1]) & mask_of(n), ye), (spec.name, x)
-        if P.shape["n_out_b"]:
-            assert np.array_equal(out["z"][0] ^ out["z"][1], pack_bits(ze)), (spec.name, x)
+    check_all_r(orc, spec, range(1 << spec.n), seed=17)
 
 
 def test_xmul_online_bytes(orc):
@@ -153,8 +109,68 @@ XP = [lambda: specs.toy(8, 3), lambda: specs.toy(8, 3, True), lambda: specs.plai
 @pytest.mark.parametrize("mk", XP)
 def test_xpoly_reconstruct_exhaustive_n8(orc, mk, sp):
     spec = specs.public_point_horner(specs.shared_prefix(mk()) if sp else mk())
+    check_all_r(orc, spec, range(1 << spec.n), seed=17)      # the lookup returns shifted coefficients: only atoms + outputs are pinned
+
+
+@pytest.mark.parametrize("variant", [2, 3, 4, 5])
+def test_variant_bits_n12(orc, variant):
+    """variant bits 1 / 2 at n = 12: every x for the corner masks, every r for the corner inputs."""
+    spec = specs.toy(12, 4)
+    if variant & 1:
+        spec = specs.shared_prefix(spec)
+    if variant & 2:
+        spec = specs.input_masked_mul(spec)
+    if variant & 4:
+        spec = specs.public_point_horner(spec)
     N = 1 << spec.n
-    _check_plain_only(orc, spec, list(range(0, N, 5)) + [N - 1])
+    rs = corner_masks(spec, extra=1, seed=variant)
+    check_pairs(orc, spec, np.tile(np.arange(N, dtype=np.uint64), len(rs)), np.repeat(np.array(rs, dtype=np.uint64), N), seed=19)
+    check_all_r(orc, spec, corner_inputs(spec, extra=0, seed=variant)[::2], seed=19)
+
+
+# ---- variant bit 3: early-terminated bit trees (DESIGN.md section 13) ------------------------------------------------
+ET = [lambda: specs.relu(8, 4), lambda: specs.toy(8, 3), lambda: specs.toy(8, 3, True), lambda: specs.plain_default(8, 3),
+      lambda: specs.single_interval(8, 3), lambda: specs.shift_relu(8, 3)]
+
+
+@pytest.mark.parametrize("sp", [0, 1])
+@pytest.mark.parametrize("mk", ET)
+def test_early_termination_reconstruct_exhaustive_n8(orc, mk, sp):
+    """Every x and every r at n = 8 with early-terminated bit trees (k = 8: one level + leaf block; k = 3: leaf block only):
+    gate outputs, atoms and lookup reconstruct to their plain definitions, with both constructions."""
+    spec = specs.early_termination(specs.shared_prefix(mk()) if sp else mk())
+    check_all_r(orc, spec, range(1 << spec.n), seed=23)
+
+
+@pytest.mark.parametrize("variant", [8, 9, 15])
+def test_early_termination_n12(orc, variant):
+    spec = specs.toy(12, 4)
+    if variant & 1:
+        spec = specs.shared_prefix(spec)
+    if variant & 2:
+        spec = specs.input_masked_mul(spec)
+    if variant & 4:
+        spec = specs.public_point_horner(spec)
+    spec = specs.early_termination(spec)
+    N = 1 << spec.n
+    rs = corner_masks(spec, extra=1, seed=variant)
+    check_pairs(orc, spec, np.tile(np.arange(N, dtype=np.uint64), len(rs)), np.repeat(np.array(rs, dtype=np.uint64), N), seed=29)
+    check_all_r(orc, spec, corner_inputs(spec, extra=0, seed=variant)[::2], seed=29)
+
+
+def test_early_termination_key_size(orc):
+    """bit tree on k bits: 16 (root) + 16 max(k-7,0) (levels) + 16 (leaf block) + 8 (VCW bits) bytes instead of 16(k+1) + 8;
+    shape (T, M, p, rounds, online bits) unchanged."""
+    for mk in (specs.gelu, specs.shift_relu, lambda: specs.shared_prefix(specs.shift_relu())):
+        s0 = mk()
+        P0, P1 = orc.Program(s0), orc.Program(specs.early_termination(s0))
+        assert P0.shape == P1.shape and P0.online_bits() == P1.online_bits()
+        c = 1 << 16
+        if s0.variant & 1:
+            saved = 16 * (12 - 5 - 1)                                  # the 12-bit tree: 5 levels + leaf instead of 12
+        else:
+            saved = sum(16 * (k - max(k - 7, 0) - 1) for k in P0.shape["k"])
+        assert P0.key_bytes(c) - P1.key_bytes(c) == saved * c
 
 
 def test_xpoly_shape(orc):

@@ -43,7 +43,7 @@ class OpSpec:
     out_frac: int = 0      # fractional bits of the arithmetic outputs (metadata for decode)
     domain: tuple = None   # real interval on which the spline error is stated
     func: object = None    # real function approximated (metadata for tests)
-    variant: int = 0       # bit 0: 0 = Protocol-3 construction, 1 = single-key shared-prefix (DESIGN 9); bit 1: input-masked products (DESIGN 10)
+    variant: int = 0       # bit 0: single-key shared-prefix construction (DESIGN 9); bit 1: input-masked products (10); bit 2: Horner in xhat (11); bit 3: early-terminated bit trees (13)
 
     @property
     def m(self):
@@ -369,6 +369,13 @@ def public_point_horner(spec):
     Beaver rounds for the spline."""
     import dataclasses
     return dataclasses.replace(spec, variant=spec.variant | 4, name=spec.name + "_xp")
+
+
+def early_termination(spec):
+    """Variant bit 3: the bit-DCF trees stop max(k-7, 0) levels deep and read the output bit out of a 128-bit leaf block
+    (DESIGN.md section 13)."""
+    import dataclasses
+    return dataclasses.replace(spec, variant=spec.variant | 8, name=spec.name + "_et")
 
 
 CONFIGS = {
