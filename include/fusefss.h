@@ -33,7 +33,9 @@ enum {
     FUSEFSS_E_COUNT = -4,     /* count == 0                                                   */
     FUSEFSS_E_ROUND = -5,     /* round outside [0, rounds]                                    */
     FUSEFSS_E_CUDA = -6,      /* a CUDA call failed (fusefss_last_cuda_error() has the text)  */
-    FUSEFSS_E_OMITTED = -7    /* eval_cmp with T = 0 / eval_lut with m = 1 (call omitted) */
+    FUSEFSS_E_OMITTED = -7,   /* eval_cmp with T = 0 / eval_lut with m = 1 (call omitted) */
+    FUSEFSS_E_WORKSPACE = -8, /* fusefss_gate_host: workspace_bytes < fusefss_gate_workspace_bytes()  */
+    FUSEFSS_E_DEBUG = -9      /* fusefss_debug_set: unknown knob                                      */
 };
 
 /* ---- operator specification (Def 4.1; grammar App. H) ------------------ */
@@ -82,7 +84,9 @@ typedef struct {
     uint32_t n_nodes, n_kappa_a, n_kappa_b, phi_len;
     uint32_t n_out_a, n_out_b;        /* outputs of Phi (ignored when phi_len == 0: outputs are y and z)    */
     uint32_t mask_output;             /* 1: arithmetic outputs are opened as yhat = y + r_out       */
-    uint32_t variant;                 /* 0: Protocol-3 construction; 1: single-key shared-prefix (DESIGN 9) */
+    uint32_t variant;                 /* bit 0: single-key shared-prefix construction (DESIGN 9); bit 1: input-masked products
+                                         (DESIGN 10); bit 2: Horner in the public xhat (DESIGN 11); bit 3: early-terminated bit trees
+                                         (DESIGN 13).  0 = the paper's Protocol 3 with textbook subprotocols. */
     const uint64_t *alpha;            /* HOST [m-1] interior boundaries, strictly increasing in (0, 2^n)    */
     const uint64_t *coeff;            /* HOST [m][r][d+1], high degree first                                */
     const uint64_t *aux;              /* HOST [m][p_aux]                                                    */
@@ -199,11 +203,12 @@ int fusefss_mul_fused(uint32_t n_bits, const uint64_t *x0_dev, const uint64_t *x
 /* ---- end-to-end convenience: HOST buffers in, HOST buffers out (bench.py's e2e leg) ---------------
  * Copies r_in/r_out/xhat to the device, runs keygen + both parties' eval_cmp/eval_lut + post_fused in chunks of
  * `chunk` elements using the caller's device workspace, copies y0,y1 [n_out_a][count] and z0,z1 [count] back.
- * workspace_dev must hold fusefss_gate_workspace_bytes(prog, chunk) bytes. */
+ * workspace_dev must hold fusefss_gate_workspace_bytes(prog, chunk) bytes; workspace_bytes is what the caller allocated
+ * (FUSEFSS_E_WORKSPACE if it is too small). */
 size_t fusefss_gate_workspace_bytes(const fusefss_program *prog, size_t chunk);
 int fusefss_gate_host(const fusefss_program *prog, const uint64_t *r_in, const uint64_t *r_out,
                       const uint64_t *xhat, uint64_t seed, size_t count, size_t chunk, void *workspace_dev,
-                      uint64_t *y0, uint64_t *y1, uint64_t *z0, uint64_t *z1, void *stream);
+                      size_t workspace_bytes, uint64_t *y0, uint64_t *y1, uint64_t *z0, uint64_t *z1, void *stream);
 
 /* ---- algorithmic work per element (for the roofline; DESIGN 5.3, 9) ---------------------------------
  * AES-128 blocks and T-table lookups of one party's evaluation (cmp part / lut part; for variant 1 "lut" = the fused
@@ -219,6 +224,10 @@ int fusefss_cost(const fusefss_program *prog, fusefss_cost_t *out);
 /* ---- diagnostics ---------------------------------------------------------------------------------- */
 const char *fusefss_strerror(int code);
 const char *fusefss_last_cuda_error(void);
+/* Test / tuning knobs (process-wide, not part of the method): "force_g" = v >= 1 forces the number of warps the trees / points of an
+ * element are dealt to (0 = automatic); "eval_threads" = CTA size of the large evaluation launches (default 1024); "small_kernels"
+ * = 0 disables the 256-thread instantiations used for small launches.  Unknown knob: FUSEFSS_E_DEBUG. */
+int fusefss_debug_set(const char *knob, long value);
 /* number of kernel launches this library has issued since load (bench.py's gpu_launches) */
 uint64_t fusefss_launch_count(void);
 /* PRG micro-kernel for the roofline denominator: each thread chains `iters` fixed-key AES-128 blocks starting

@@ -836,6 +836,34 @@ orc_prog *orc_compile(const orc_spec *S0)
         if (a == 0 || (a & ~ring_mask((int)S->n))) return NULL;
         if (i && a <= S->alpha[i - 1]) return NULL;
     }
+    /* well-formedness of the rest of the descriptor ("boundaries, polynomials, constants and gates must be well formed") */
+    for (u32 i = 0; i < S->n_nodes; i++) {
+        const orc_bitnode *nd = &S->nodes[i];
+        if (nd->kind > BN_OR) return NULL;
+        if ((nd->kind == BN_D || nd->kind == BN_CARRY) && (nd->k < 1 || nd->k > S->n)) return NULL;
+        if (nd->kind == BN_C && !nd->value_is_2k && nd->value > ring_mask((int)S->n)) return NULL;      /* beta in [0, 2^n] */
+        if (nd->kind == BN_D && !nd->value_is_2k && nd->value > low_mask(nd->k)) return NULL;          /* gamma in [0, 2^k] */
+        if (nd->kind >= BN_NOT && nd->lhs >= i) return NULL;                                           /* operands precede (DAG) */
+        if (nd->kind >= BN_XOR && nd->rhs >= i) return NULL;
+    }
+    for (u32 i = 0; i < S->m * S->ell; i++) if (S->bit_root[i] >= S->n_nodes) return NULL;
+    if (S->n_kappa_a > 8 || S->n_kappa_b > 64) return NULL;
+    for (u32 i = 0; i < S->n_kappa_a; i++) if (S->kappa_a[i].kind != KA_R_SHR || S->kappa_a[i].arg > 63) return NULL;
+    for (u32 i = 0; i < S->n_kappa_b; i++) if (S->kappa_b[i].kind != KB_R_BIT || S->kappa_b[i].arg >= S->n) return NULL;
+    if (S->phi_len) {
+        int seen_a[256] = { 0 }, seen_b[256] = { 0 };
+        for (u32 i = 0; i < S->phi_len; i++) {
+            const orc_phi_op *o = &S->phi[i];
+            if ((o->op == PHI_B_XHAT && o->a >= S->n) || (o->op == PHI_B_ANDPUB && o->b >= S->n)) return NULL;   /* public bit index < n */
+            if (o->op == PHI_A_XHAT_SHR && o->a > 64) return NULL;
+            if (o->op == PHI_A_OUT) seen_a[o->dst]++;
+            if (o->op == PHI_B_OUT) seen_b[o->dst]++;
+        }
+        for (u32 j = 0; j < 256; j++) {                       /* every declared output is written exactly once */
+            if (seen_a[j] != (j < S->n_out_a)) return NULL;
+            if (seen_b[j] != (j < S->n_out_b)) return NULL;
+        }
+    }
     orc_prog *P = calloc(1, sizeof *P);
     P->S = *S;
     P->S.alpha = dup_mem(S->alpha, sizeof(u64) * (S->m - 1));

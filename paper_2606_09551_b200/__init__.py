@@ -22,7 +22,7 @@ SYMBOLS = (
     "fusefss_eval_cmp", "fusefss_eval_lut", "fusefss_eval_fused", "fusefss_eval_fused_both", "fusefss_post", "fusefss_post_rounds", "fusefss_post_msg_bytes",
     "fusefss_online_bits", "fusefss_post_fused", "fusefss_cost", "fusefss_gate_workspace_bytes", "fusefss_gate_host",
     "fusefss_share_open", "fusefss_sub_bcast", "fusefss_row_sum", "fusefss_mul_triple_bytes", "fusefss_mul_keygen", "fusefss_mul_fused",
-    "fusefss_strerror", "fusefss_last_cuda_error", "fusefss_launch_count", "fusefss_aes_probe", "fusefss_aes_kat", "fusefss_pipe_probe",
+    "fusefss_strerror", "fusefss_last_cuda_error", "fusefss_debug_set", "fusefss_launch_count", "fusefss_aes_probe", "fusefss_aes_kat", "fusefss_pipe_probe",
 )
 
 
@@ -82,7 +82,7 @@ def _load():
         "fusefss_post_fused": (i32, [vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp, vp, vp, vp]),
         "fusefss_cost": (i32, [vp, C.POINTER(Cost)]),
         "fusefss_gate_workspace_bytes": (sz, [vp, sz]),
-        "fusefss_gate_host": (i32, [vp, vp, vp, vp, u64, sz, sz, vp, vp, vp, vp, vp, vp]),
+        "fusefss_gate_host": (i32, [vp, vp, vp, vp, u64, sz, sz, vp, sz, vp, vp, vp, vp, vp]),
         "fusefss_share_open": (i32, [vp, vp, vp, vp, vp, sz, u64, vp, vp]),
         "fusefss_sub_bcast": (i32, [C.c_uint32, vp, vp, sz, sz, vp, vp]),
         "fusefss_row_sum": (i32, [C.c_uint32, vp, sz, sz, vp, vp]),
@@ -91,6 +91,7 @@ def _load():
         "fusefss_mul_fused": (i32, [C.c_uint32, vp, vp, vp, vp, vp, vp, sz, sz, vp, vp, vp]),
         "fusefss_strerror": (C.c_char_p, [i32]),
         "fusefss_last_cuda_error": (C.c_char_p, []),
+        "fusefss_debug_set": (i32, [C.c_char_p, C.c_long]),
         "fusefss_launch_count": (u64, []),
         "fusefss_aes_probe": (i32, [sz, i32, vp, vp]),
         "fusefss_aes_kat": (i32, [C.c_char_p, C.c_char_p, vp, vp]),
@@ -298,8 +299,12 @@ class Program:
         y0 = np.empty((na, count), np.uint64); y1 = np.empty((na, count), np.uint64)
         z0 = np.zeros(count, np.uint64); z1 = np.zeros(count, np.uint64)
         _check(lib.fusefss_gate_host(self._h, _ptr(r_in), _ptr(r_out), _ptr(xhat), seed, count, chunk, _ptr(workspace),
-                                     _ptr(y0), _ptr(y1), _ptr(z0), _ptr(z1), _stream()))
+                                     workspace.numel() * workspace.element_size(), _ptr(y0), _ptr(y1), _ptr(z0), _ptr(z1), _stream()))
         return y0, y1, z0, z1
+
+
+def debug_set(knob: str, value: int):
+    _check(lib.fusefss_debug_set(knob.encode(), int(value)))
 
 
 def launch_count() -> int:

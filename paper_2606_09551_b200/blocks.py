@@ -170,3 +170,64 @@ class LayerNorm(Softmax):
 
     def rounds(self) -> int:
         return sum(1 + self.progs[k].post_rounds() for k in self.LN_STAGES) + 2
+
+
+def bench(F, torch, steps: int = 3):
+    """bench.py --blocks: dealer and online time of the softmax block (config 3's shape, 12 heads x 128 rows of 128) and of the
+    LayerNorm block (config 4b's shape, 1024 tokens x d = 1024); CUDA events, both parties on one GPU."""
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.int64)).cuda()
+    rng = np.random.default_rng(5)
+    U = lambda k: rng.integers(0, 1 << 63, size=k, dtype=np.uint64) * np.uint64(2) + rng.integers(0, 2, size=k, dtype=np.uint64)
+    out = {}
+
+    def time_block(B, masks, x0d, x1d):
+        for _ in range(3):
+            B.keygen(masks, 9); res = B.run(x0d, x1d)
+        torch.cuda.synchronize()
+        e = [ev() for _ in range(3)]
+        e[0].record()
+        for _ in range(steps):
+            B.keygen(masks, 9)
+        e[1].record()
+        for _ in range(steps):
+            res = B.run(x0d, x1d)
+        e[2].record()
+        torch.cuda.synchronize()
+        return res, e[0].elapsed_time(e[1]) / steps, e[1].elapsed_time(e[2]) / steps
+
+    rows, cols = 12 * 128, 128
+    xr = np.maximum(-20.0, -4.0 * rng.exponential(1.0, size=(rows, cols))); xr[:, 0] = 0.0
+    xq = np.floor(xr.reshape(-1) * 4096 + 0.5).astype(np.int64).view(np.uint64)
+    x0h = U(xq.size)
+    masks = {k: dev(U(c)) for k, c in (("nexp", xq.size), ("tr_e", xq.size), ("recip", rows), ("tr_t", rows), ("tr_y", xq.size))}
+    blk = {}
+    for v in (3, 0):
+        B = Softmax(rows, cols, v)
+        res, t_deal, t_on = time_block(B, masks, dev(x0h), dev(xq - x0h))
+        y = (res["y"][0] + res["y"][1]).cpu().numpy().astype(np.float64).reshape(rows, cols) / 4096.0
+        ref = np.exp(xr) / np.exp(xr).sum(axis=1, keepdims=True)
+        blk["variant_%d" % v] = {"rows": rows, "cols": cols, "dealer_ms": t_deal, "online_ms": t_on, "online_elems_per_s": rows * cols / (t_on * 1e-3),
+                                 "key_bytes_per_elem_per_party": B.key_bytes_per_party() / (rows * cols),
+                                 "online_bytes_per_elem_per_party": B.online_bytes_per_party() / (rows * cols), "rounds": B.rounds(),
+                                 "max_abs_err_vs_float_softmax": float(np.abs(y - ref).max())}
+        del B
+        torch.cuda.empty_cache()
+    out["softmax_block"] = blk
+    rows, d = 1024, 1024
+    xr = rng.normal(0.0, 2.0, size=(rows, d))
+    xq = np.floor(xr.reshape(-1) * 4096 + 0.5).astype(np.int64).view(np.uint64)
+    x0h = U(xq.size)
+    masks = {k: dev(U(c)) for k, c in (("mean", rows), ("var", rows), ("rsqrt", rows), ("tr_g", rows), ("tr_y", xq.size))}
+    B = LayerNorm(rows, d, 3)
+    res, t_deal, t_on = time_block(B, masks, dev(x0h), dev(xq - x0h))
+    y = (res["y"][0] + res["y"][1]).cpu().numpy().astype(np.float64).reshape(rows, d) / 4096.0
+    xf = xq.view(np.int64).astype(np.float64).reshape(rows, d) / 4096.0
+    ref = (xf - xf.mean(axis=1, keepdims=True)) / xf.std(axis=1, keepdims=True)
+    out["layernorm_block"] = {"variant_3": {"rows": rows, "d": d, "dealer_ms": t_deal, "online_ms": t_on, "online_elems_per_s": rows * d / (t_on * 1e-3),
+                                            "key_bytes_per_elem_per_party": B.key_bytes_per_party() / (rows * d),
+                                            "online_bytes_per_elem_per_party": B.online_bytes_per_party() / (rows * d), "rounds": B.rounds(),
+                                            "max_abs_err_vs_float_layernorm": float(np.abs(y - ref).max())}}
+    del B
+    torch.cuda.empty_cache()
+    return out

@@ -7,12 +7,18 @@ import subprocess
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libfusefss.so")
+import glob
+
 SOURCES = ["libfusefss.cu", "compile.cpp"]
-DEPS = SOURCES + ["aes.cuh", "eval.cuh", "keygen.cuh", "post.cuh", "program.h", "../../include/fusefss.h"]
+
+
+def deps():
+    """every file the library is built from: all of csrc/ plus the public header"""
+    return sorted(glob.glob(os.path.join(_CSRC, "*"))) + [os.path.join(_HERE, "..", "include", "fusefss.h")]
 
 
 def build(force: bool = False, verbose: bool = False, extra=()) -> str:
-    newest = max(os.path.getmtime(os.path.join(_CSRC, d)) for d in DEPS)
+    newest = max(os.path.getmtime(d) for d in deps())
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")

@@ -81,11 +81,14 @@ constexpr size_t kAesSmemBytes = 3 * 65536;
 __device__ __forceinline__ uint32_t aes_fill_tables(uint32_t *dyn_smem) {
     const uint32_t b0 = (uint32_t)__cvta_generic_to_shared(dyn_smem);
     char *win0 = reinterpret_cast<char *>(dyn_smem) - b0;                  // generic address of window offset 0
-    for (int i = threadIdx.x; i < 4 * 256 * 32; i += blockDim.x) {
-        const int tab = i >> 13, x = (i >> 5) & 255, ln = i & 31;
+    for (int i = threadIdx.x; i < 256 * 32; i += blockDim.x) {            // one constant load feeds the four rotations
+        const int x = i >> 5, ln = i & 31;
         const uint32_t v = c_T0[x];
-        const uint32_t off = 65536u + (uint32_t)(tab >> 1) * 65536u + (uint32_t)x * 256u + (uint32_t)(tab & 1) * 128u + (uint32_t)ln * 4u;
-        *reinterpret_cast<uint32_t *>(win0 + off) = __funnelshift_l(v, v, tab * 8);   // T_k = T0 rotated left by 8k bits
+        char *p = win0 + 65536u + (uint32_t)x * 256u + (uint32_t)ln * 4u;
+        *reinterpret_cast<uint32_t *>(p) = v;                                         // T0
+        *reinterpret_cast<uint32_t *>(p + 128) = __funnelshift_l(v, v, 8);            // T1 = T0 rotated left by 8 bits
+        *reinterpret_cast<uint32_t *>(p + 65536) = __funnelshift_l(v, v, 16);         // T2
+        *reinterpret_cast<uint32_t *>(p + 65536 + 128) = __funnelshift_l(v, v, 24);   // T3
     }
     __syncthreads();
     uint32_t tl;

@@ -466,6 +466,31 @@ int compile_program(const fusefss_spec *S, Program **out) {
         if (nd.kind >= FUSEFSS_BN_XOR && nd.rhs >= i) return FUSEFSS_E_SPEC;
     }
     for (size_t i = 0; i < (size_t)S->m * S->ell; ++i) if (S->bit_root[i] >= S->n_nodes) return FUSEFSS_E_SPEC;
+    for (uint32_t i = 0; i < S->n_nodes; ++i) {   // values in range: beta in [0, 2^n] / gamma in [0, 2^k] (the upper ends via value_is_2k)
+        const fusefss_bitnode &nd = S->nodes[i];
+        if (nd.kind == FUSEFSS_BN_C && !nd.value_is_2k && (nd.value & ~mask)) return FUSEFSS_E_SPEC;
+        if (nd.kind == FUSEFSS_BN_D && !nd.value_is_2k && (nd.value & ~ring_mask(nd.k))) return FUSEFSS_E_SPEC;
+    }
+    if (S->n_kappa_a > 8 || S->n_kappa_b > 64) return FUSEFSS_E_SPEC;
+    for (uint32_t i = 0; i < S->n_kappa_a; ++i)
+        if (S->kappa_a[i].kind != FUSEFSS_KA_R_SHR || S->kappa_a[i].arg >= 64) return FUSEFSS_E_SPEC;
+    for (uint32_t i = 0; i < S->n_kappa_b; ++i)
+        if (S->kappa_b[i].kind != FUSEFSS_KB_R_BIT || S->kappa_b[i].arg >= S->n) return FUSEFSS_E_SPEC;
+    if (S->phi_len) {                             // Phi: public bit indices below n, every declared output written exactly once
+        uint32_t wa[256] = {0}, wb[256] = {0};
+        for (uint32_t i = 0; i < S->phi_len; ++i) {
+            const fusefss_phi_op &o = S->phi[i];
+            if (o.op == FUSEFSS_PHI_B_XHAT && o.a >= S->n) return FUSEFSS_E_SPEC;
+            if (o.op == FUSEFSS_PHI_B_ANDPUB && o.b >= S->n) return FUSEFSS_E_SPEC;
+            if (o.op == FUSEFSS_PHI_A_XHAT_SHR && o.a > 64) return FUSEFSS_E_SPEC;
+            if (o.op == FUSEFSS_PHI_A_OUT) ++wa[o.dst];
+            if (o.op == FUSEFSS_PHI_B_OUT) ++wb[o.dst];
+        }
+        for (uint32_t j = 0; j < 256; ++j) {
+            if (wa[j] != (j < S->n_out_a ? 1u : 0u)) return FUSEFSS_E_SPEC;
+            if (wb[j] != (j < S->n_out_b ? 1u : 0u)) return FUSEFSS_E_SPEC;
+        }
+    }
 
     fusefss_program *holder = new (std::nothrow) fusefss_program();
     if (!holder) return FUSEFSS_E_SPEC;
@@ -488,6 +513,7 @@ int compile_program(const fusefss_spec *S, Program **out) {
     P.variant = S->variant & 1;
     P.xmul = (S->variant >> 1) & 1;
     P.xpoly = ((S->variant >> 2) & 1) && S->d >= 1 && S->m > 1;
+    P.et = (S->variant >> 3) & 1;
     if (P.xpoly && S->d > 2) { delete holder; return FUSEFSS_E_SPEC; }          // kernels are instantiated for d <= 2
     if (P.variant) P.M = (int)S->m;               // variant 1: no translated partition, no wrap / dummy split
     P.n_out_a = (int)S->n_out_a; P.n_out_b = (int)S->n_out_b;
@@ -499,6 +525,17 @@ int compile_program(const fusefss_spec *S, Program **out) {
     }
     Lowering low(P);
     if (!low.run()) { delete holder; return FUSEFSS_E_SPEC; }
+    {   // layout of the small device tables (uploaded per device on first use)
+        auto up = [](size_t x) { return (x + 255) & ~(size_t)255; };
+        P.dev_ins_off = 0;
+        P.dev_alpha_off = up(P.ins.size() * sizeof(Ins));
+        P.dev_payload_off = P.dev_alpha_off + up(P.alpha.size() * 8 + 8);
+        P.dev_sp_points_off = P.dev_payload_off + up(P.payload.size() * 8 + 8);
+        P.dev_sp_weights_off = P.dev_sp_points_off + up(P.sp.points.size() * sizeof(SpPoint) + 8);
+        P.dev_sp_delta_off = P.dev_sp_weights_off + up(P.sp.weights.size() * 8 + 8);
+        P.dev_sp_clusters_off = P.dev_sp_delta_off + up(P.sp.delta_tab.size() * 8 + 8);
+        P.dev_blob_bytes = P.dev_sp_clusters_off + up(P.sp.clusters.size() * sizeof(SpCluster) + 8);
+    }
     *out = &holder->impl;
     return FUSEFSS_OK;
 }
@@ -518,14 +555,14 @@ void compute_layout(const Program &P, size_t count, Layout *L) {
         for (int w = 0; w < P.sp.n_w; ++w) {
             if (!P.sp.width[w].is_vec) {
                 L->bt_root[w] = off; off += L->s16;
-                L->bt_cw[w] = off;   off += L->s16 * (size_t)P.sp.width[w].k;
+                L->bt_cw[w] = off;   off += L->s16 * (size_t)bit_tree_arrays(P, P.sp.width[w].k);
                 L->bt_vb[w] = off;   off += L->s8;
             } else { L->vt_first = off; off += L->vt_stride; }
         }
     }
     for (int t = 0; t < P.T && !P.variant; ++t) {
         L->bt_root[t] = off; off += L->s16;
-        L->bt_cw[t] = off;   off += L->s16 * (size_t)P.atoms[t].k;
+        L->bt_cw[t] = off;   off += L->s16 * (size_t)bit_tree_arrays(P, P.atoms[t].k);
         L->bt_vb[t] = off;   off += L->s8;
     }
     const size_t pw = (size_t)P.p * L->s8;

@@ -10,6 +10,7 @@
 // (sp_walk_fork), every point then walks only its tail from the matching saved state.
 #pragma once
 #include "aes.cuh"
+#include "eval.cuh"
 #include "program.h"
 
 namespace fsk {
@@ -22,7 +23,8 @@ struct EvalSpArgs {
     const SpCluster *cluster;
     size_t count, s16, s8, lvl_stride, vt_first, vt_lvl_rel, vt_fin_rel, rpow;
     uint64_t mask;
-    int n, m, p, pad0, T, n_w, n_clusters, G;   // G > 1: the points of an element are dealt round-robin to G warps (small tensors)
+    int n, m, p, et, T, n_w, n_clusters, G;     // G > 1: the points of an element are dealt round-robin to G warps (small tensors); et: early-terminated bit trees
+    int zero_first, pad1;                       // G > 1: outputs are zeroed in-kernel before the atomics (cooperative launch)
     SpWidth width[kMaxWidths];
     size_t bt_root[kMaxWidths], bt_cw[kMaxWidths], bt_vb[kMaxWidths];
     SpAtomDev atom[kMaxAtoms];
@@ -113,41 +115,11 @@ __device__ __forceinline__ void sp_leaf(uint32_t tl, const SpState<PK> &st, cons
     }
 }
 
-// bit-DCF walk (payload Z_2) of one point; u = the k-bit point, MSB-aligned
-__device__ __forceinline__ uint32_t sp_bit_eval(uint32_t tl, const uint8_t *key, size_t root_off, size_t cw_off, size_t vb_off,
-                                                size_t e, size_t s16, int k, uint64_t u, int party) {
-    uint4 s = __ldg(reinterpret_cast<const uint4 *>(key + root_off + e * 16));
-    const uint64_t vb = __ldg(reinterpret_cast<const unsigned long long *>(key + vb_off + e * 8));
-    const uint32_t fin = s.x & 1u;
-    s.x &= ~3u;
-    uint32_t tb = (uint32_t)party, V = 0;
-    const uint8_t *cwp = key + cw_off + e * 16;
-    for (int i = 0; i < k; ++i) {
-        const uint4 cw = __ldg(reinterpret_cast<const uint4 *>(cwp + (size_t)i * s16));
-        const uint32_t dbit = (uint32_t)(u >> 63);
-        u <<= 1;
-        uint32_t x[1][4] = {{s.x | dbit, s.y, s.z, s.w}};
-        uint32_t o[1][1][4];
-        prg_blocks<1, 1, 0, false, 3>(tl, x, o);
-        const uint32_t tm = 0u - tb;
-        V ^= ((o[0][0][0] >> 1) & 1u) ^ (tb & (uint32_t)((vb >> i) & 1ull));
-        const uint32_t tnew = (o[0][0][0] & 1u) ^ (tb & (cw.x >> dbit) & 1u);
-        s.x = (o[0][0][0] & ~3u) ^ (cw.x & ~3u & tm);
-        s.y = o[0][0][1] ^ (cw.y & tm);
-        s.z = o[0][0][2] ^ (cw.z & tm);
-        s.w = o[0][0][3] ^ (cw.w & tm);
-        tb = tnew;
-    }
-    uint32_t x[1][4] = {{s.x | 2u, s.y, s.z, s.w}};
-    uint32_t o[1][1][4];
-    prg_blocks<1, 1, 0, false, 3>(tl, x, o);
-    return (V ^ ((o[0][0][0] >> 1) & 1u) ^ (tb & fin)) & 1u;
-}
-
-template <int P, int PK>
-__global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ EvalSpArgs a) {
+template <int P, int PK, int THREADS>
+__global__ void __launch_bounds__(THREADS, 1) k_eval_sp(const __grid_constant__ EvalSpArgs a) {
     extern __shared__ uint32_t sT[];
     const uint32_t tl = aes_fill_tables(sT);
+    if (a.zero_first) zero_outputs_and_sync(a.bits_out2, true, a.coeff_out2, true, a.count, P);
     const size_t tiles = (a.count + 31) / 32, items = tiles * (size_t)a.G * (size_t)a.n_parties, warps = (size_t)gridDim.x * (blockDim.x >> 5);
     // warp w of CTA b takes items w*grid + b (+ k*warps): a partial last wave spreads evenly over all SMs
     for (size_t item = (size_t)(threadIdx.x >> 5) * gridDim.x + blockIdx.x; item < items; item += warps) {
@@ -197,7 +169,7 @@ __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ Eva
                 const uint64_t km = (1ull << W.k) - 1ull;
                 for (int j = g; j < W.n_points; j += a.G) {
                     const uint64_t u = (((xh & km) + pts[j].delta) & km) << (64 - W.k);
-                    const uint32_t A = sp_bit_eval(tl, key, a.bt_root[wd], a.bt_cw[wd], a.bt_vb[wd], e, a.s16, W.k, u, party);
+                    const uint32_t A = bit_tree_eval<false>(tl, key, a.bt_root[wd], a.bt_cw[wd], a.bt_vb[wd], e, a.s16, W.k, u, party, a.et);
                     word ^= pts[j].bitmask & (0ull - (uint64_t)A);
                 }
                 continue;
@@ -265,7 +237,7 @@ __global__ void __launch_bounds__(1024, 1) k_eval_sp(const __grid_constant__ Eva
                 if (want_bits) atomicXor(reinterpret_cast<unsigned long long *>(bits_out + e), (unsigned long long)word);
                 if (want_coeff) {
 #pragma unroll
-                    for (int w = 0; w < P; ++w) atomicAdd(reinterpret_cast<unsigned long long *>(coeff_out + (size_t)w * a.count + e), (unsigned long long)acc[w]);
+                    for (int w = 0; w < P; ++w) atomic_add_ring(coeff_out + (size_t)w * a.count + e, acc[w] & a.mask, a.mask);
                 }
             }
         }

@@ -32,7 +32,7 @@ struct GenAtomDev { uint64_t c, beta, root_off, cw_off, vb_off; int k, is_theta;
 struct GenBitArgs {
     uint8_t *key0, *key1; const uint64_t *r_in;
     size_t count, s16; uint64_t first_elem, mask;
-    int T, pad;
+    int T, et;                 // et: early-terminated trees (variant bit 3, DESIGN 13): max(k-7,0) levels + a 128-bit leaf block
     RoundKeys rk;
     GenAtomDev atom[kMaxAtoms];
 };
@@ -68,7 +68,8 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_bit(const __grid_constan
         uint32_t t0 = 0, t1 = 1, Va = 0;
         uint64_t vbits = 0;
         uint8_t *cw0 = a.key0 + at.cw_off + e * 16, *cw1 = a.key1 + at.cw_off + e * 16;
-        for (int i = 0; i < k; ++i) {
+        const int levels = a.et ? (k > 7 ? k - 7 : 0) : k;             // the tree walks the top `levels` bits of alpha
+        for (int i = 0; i < levels; ++i) {
             const uint32_t abit = (uint32_t)(alpha >> 63);
             alpha <<= 1;
             // children: index 2*b + d
@@ -118,7 +119,23 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_bit(const __grid_constan
 #pragma unroll
         for (int b = 0; b < 2; ++b) { x[b][0] = s[b][0] | 2u; x[b][1] = s[b][1]; x[b][2] = s[b][2]; x[b][3] = s[b][3]; }
         prg_blocks<2, 1, 0>(tl, x, o);
-        const uint32_t fin = (((o[0][0][0] ^ o[1][0][0]) >> 1) & 1u) ^ Va;
+        uint32_t fin = (((o[0][0][0] ^ o[1][0][0]) >> 1) & 1u) ^ Va;
+        if (a.et) {
+            // leaf correction block L = conv128(s_0) ^ conv128(s_1) ^ X, X_j = Valpha ^ I[j < alpha_lo], alpha_lo = the remaining low bits
+            const int lam = k - levels;
+            const uint32_t alo = (uint32_t)(alpha >> (64 - lam));
+            const uint32_t vm = 0u - Va;
+            uint32_t L[4];
+#pragma unroll
+            for (int w = 0; w < 4; ++w) {
+                const uint32_t below = alo >= 32u * (w + 1) ? ~0u : alo <= 32u * w ? 0u : ((1u << (alo - 32u * w)) - 1u);
+                L[w] = o[0][0][w] ^ o[1][0][w] ^ below ^ vm;
+            }
+            const uint4 lv = make_uint4(L[0], L[1], L[2], L[3]);
+            st_stream16(cw0 + (size_t)levels * a.s16, lv);
+            st_stream16(cw1 + (size_t)levels * a.s16, lv);
+            fin = 0;
+        }
         st_stream16(a.key0 + at.root_off + e * 16, make_uint4(root0.x | fin, root0.y, root0.z, root0.w));
         st_stream16(a.key1 + at.root_off + e * 16, make_uint4(root1.x | fin, root1.y, root1.z, root1.w));
         st_stream8(a.key0 + at.vb_off + e * 8, vbits);

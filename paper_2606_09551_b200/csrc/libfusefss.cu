@@ -5,7 +5,9 @@
 #include <cstdio>
 #include <cstdlib>
 #include <algorithm>
+#include <map>
 #include <mutex>
+#include <string>
 #include <utility>
 #include <vector>
 
@@ -22,10 +24,10 @@ namespace {
 
 thread_local char g_cuda_err[256] = "";
 std::atomic<uint64_t> g_launches{0};
-std::once_flag g_init_once;
-int g_init_status = 0;
-int g_sms = 148;
-int g_eval_threads = kEvalThreads;
+thread_local int g_sms = 148;                 // SM count of the calling thread's current device (set by init_device)
+std::atomic<int> g_force_g{0};                // fusefss_debug_set("force_g", v): v >= 1 forces the tree-group count (tests)
+std::atomic<int> g_eval_threads{kEvalThreads};// fusefss_debug_set("eval_threads", v): CTA size of the large eval launches
+std::atomic<int> g_small_regs{1};             // fusefss_debug_set("small_kernels", 0): never pick the 256-thread instantiations
 const HostAes &host_aes() { static HostAes h; return h; }
 
 int cuda_fail(cudaError_t e, const char *what) {
@@ -39,61 +41,59 @@ template <typename K> int allow_smem(K kernel, size_t bytes) {
     return 0;
 }
 
-// one-time: PRG round keys + T0 into constant memory, opt-in shared memory sizes, SM count, tuning knobs
+// Per DEVICE, once: the PRG round keys and T0 go to that device's constant memory (__constant__ symbols are per device), and its
+// SM count is recorded.  Every entry point calls this first; it also refreshes the thread-local g_sms for the current device.
+struct DeviceState { bool ready = false; int sms = 0; };
 int init_device() {
-    std::call_once(g_init_once, [] {
-        auto body = []() -> int {
-            const HostAes &h = host_aes();
-            uint32_t rk[kNumPrgKeys][44];
-            for (int i = 0; i < kNumPrgKeys; ++i) {
-                uint8_t key[16];
-                for (int j = 0; j < 16; ++j) key[j] = (uint8_t)j;
-                key[0] = (uint8_t)i;
-                h.expand(key, rk[i]);
-            }
-            // prg_blocks<.., SHARED> relies on the PRG keys agreeing outside byte 0 of round key 0
-            for (int i = 1; i < kNumPrgKeys; ++i)
-                if ((rk[i][0] ^ rk[0][0]) & ~0xffu || rk[i][1] != rk[0][1] || rk[i][2] != rk[0][2] || rk[i][3] != rk[0][3]) return FUSEFSS_E_SPEC;
-            CU(cudaMemcpyToSymbol(c_T0, h.T0, sizeof h.T0));
-            CU(cudaMemcpyToSymbol(c_rk, rk, sizeof rk));
-            int dev = 0;
-            CU(cudaGetDevice(&dev));
-            CU(cudaDeviceGetAttribute(&g_sms, cudaDevAttrMultiProcessorCount, dev));
-            if (const char *s = std::getenv("FUSEFSS_EVAL_THREADS")) {
-                int v = std::atoi(s);
-                if (v >= 32 && v <= kEvalThreads && v % 32 == 0) g_eval_threads = v;
-            }
-            return 0;
-        };
-        g_init_status = body();
-    });
-    return g_init_status;
+    static std::mutex mu;
+    static std::map<int, DeviceState> devs;
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lock(mu);
+    DeviceState &D = devs[dev];
+    if (!D.ready) {
+        const HostAes &h = host_aes();
+        uint32_t rk[kNumPrgKeys][44];
+        for (int i = 0; i < kNumPrgKeys; ++i) {
+            uint8_t key[16];
+            for (int j = 0; j < 16; ++j) key[j] = (uint8_t)j;
+            key[0] = (uint8_t)i;
+            h.expand(key, rk[i]);
+        }
+        // prg_blocks<.., SHARED> relies on the PRG keys agreeing outside byte 0 of round key 0
+        for (int i = 1; i < kNumPrgKeys; ++i)
+            if ((rk[i][0] ^ rk[0][0]) & ~0xffu || rk[i][1] != rk[0][1] || rk[i][2] != rk[0][2] || rk[i][3] != rk[0][3]) return FUSEFSS_E_SPEC;
+        CU(cudaMemcpyToSymbol(c_T0, h.T0, sizeof h.T0));
+        CU(cudaMemcpyToSymbol(c_rk, rk, sizeof rk));
+        CU(cudaDeviceGetAttribute(&D.sms, cudaDevAttrMultiProcessorCount, dev));
+        D.ready = true;
+    }
+    g_sms = D.sms;
+    return 0;
 }
 
-// number of tree groups G in [1, gmax]: the smallest G whose last wave is >= 97 % full, else the best one
-int pick_groups(size_t count, int gmax, int threads) {
-    if (const char *f = std::getenv("FUSEFSS_FORCE_G")) {          // test hook: force the tree-group count
-        int v = std::atoi(f);
-        if (v >= 1) return v < gmax ? v : gmax;
-    }
-    const double warps = (double)g_sms * (threads / 32);
-    const double tiles = (double)((count + 31) / 32);
-    int best = 1; double best_eff = 0;
-    for (int G = 1; G <= gmax; ++G) {
-        const double waves = tiles * G / warps;
-        const double eff = waves / (double)(size_t)(waves + 0.999999);
-        if (eff >= 0.97) return G;
-        if (eff > best_eff + 1e-9) { best_eff = eff; best = G; }
-    }
-    return best;
+// Number of tree groups G in [1, gmax] for `units` (party, tile) pairs with `ntrees` trees each on `warps` persistent warps.
+// A warp takes every warps-th item, so the slowest warp walks ceil(units G / warps) items of ceil(ntrees / G) trees: minimise
+// that product (the launch's critical path in tree walks) and take the smallest G within 3 % of the minimum (fewer atomics).
+int pick_groups(size_t units, int ntrees, int warps) {
+    if (ntrees < 1) return 1;
+    if (const int f = g_force_g.load()) return f < ntrees ? f : ntrees;
+    auto cost = [&](int G) {
+        const size_t per_warp = (units * (size_t)G + (size_t)warps - 1) / (size_t)warps;
+        return per_warp * (size_t)((ntrees + G - 1) / G);
+    };
+    size_t best = ~(size_t)0;
+    for (int G = 1; G <= ntrees; ++G) best = cost(G) < best ? cost(G) : best;
+    for (int G = 1; G <= ntrees; ++G) if ((double)cost(G) <= 1.03 * (double)best) return G;
+    return 1;
 }
 
 // CTA size for `warp_items` warp-sized work items: small launches use small CTAs so that the warps spread over all
 // SMs (the AES kernels are bound by the per-SM shared-memory pipe), large ones use max_threads per CTA.
-int threads_for(size_t warp_items, int max_threads) {
+int threads_for(size_t warp_items, int max_threads, int min_threads = 64) {
     size_t per_sm = (warp_items + (size_t)g_sms - 1) / (size_t)g_sms;
     size_t t = per_sm * 32;
-    if (t < 64) t = 64;
+    if (t < (size_t)min_threads) t = (size_t)min_threads;
     if (t > (size_t)max_threads) t = (size_t)max_threads;
     return (int)t;
 }
@@ -104,18 +104,13 @@ int grid_for(size_t warp_items, int threads) {
     return blocks ? (int)blocks : 1;
 }
 
-// lazily upload the small per-program tables (post program, alpha, payload table)
-int ensure_blob(Program &P) {
-    if (P.dev_blob) return 0;
-    auto up = [](size_t x) { return (x + 255) & ~(size_t)255; };
-    P.dev_ins_off = 0;
-    P.dev_alpha_off = up(P.ins.size() * sizeof(Ins));
-    P.dev_payload_off = P.dev_alpha_off + up(P.alpha.size() * 8 + 8);
-    P.dev_sp_points_off = P.dev_payload_off + up(P.payload.size() * 8 + 8);
-    P.dev_sp_weights_off = P.dev_sp_points_off + up(P.sp.points.size() * sizeof(SpPoint) + 8);
-    P.dev_sp_delta_off = P.dev_sp_weights_off + up(P.sp.weights.size() * 8 + 8);
-    P.dev_sp_clusters_off = P.dev_sp_delta_off + up(P.sp.delta_tab.size() * 8 + 8);
-    P.dev_blob_bytes = P.dev_sp_clusters_off + up(P.sp.clusters.size() * sizeof(SpCluster) + 8);
+// the small per-program tables (post program, alpha, payload table, variant-1 tables) on the CURRENT device; uploaded on first use
+int ensure_blob(const Program &P, const uint8_t **out) {
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lock(P.blob_mu);
+    auto it = P.dev_blobs.find(dev);
+    if (it != P.dev_blobs.end()) { *out = (const uint8_t *)it->second; return 0; }
     void *d = nullptr;
     CU(cudaMalloc(&d, P.dev_blob_bytes));
     std::vector<uint8_t> h(P.dev_blob_bytes, 0);
@@ -128,7 +123,8 @@ int ensure_blob(Program &P) {
     if (!P.sp.clusters.empty()) std::memcpy(h.data() + P.dev_sp_clusters_off, P.sp.clusters.data(), P.sp.clusters.size() * sizeof(SpCluster));
     cudaError_t e = cudaMemcpy(d, h.data(), P.dev_blob_bytes, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { cudaFree(d); return cuda_fail(e, "cudaMemcpy(program tables)"); }
-    P.dev_blob = d;
+    P.dev_blobs[dev] = d;
+    *out = (const uint8_t *)d;
     return 0;
 }
 
@@ -141,7 +137,7 @@ RoundKeys seed_round_keys(uint64_t seed) {
     return rk;
 }
 
-template <typename K, typename A> int launch(K kernel, int grid, int block, size_t smem, cudaStream_t st, const A &args) {
+template <typename K, typename A> int launch(K kernel, int grid, int block, size_t smem, cudaStream_t st, const A &args, bool cooperative = false) {
     if (smem > 48 * 1024) {                       // opt in to > 48 KB of dynamic shared memory once per kernel (and device)
         static std::mutex mu;
         static std::vector<std::pair<const void *, int>> done;
@@ -154,27 +150,18 @@ template <typename K, typename A> int launch(K kernel, int grid, int block, size
             done.push_back(id);
         }
     }
-    kernel<<<grid, block, smem, st>>>(args);
+    if (cooperative) {                            // the kernel uses one grid-wide barrier: all CTAs must be co-resident (grid <= #SMs)
+        void *params[] = {const_cast<A *>(&args)};
+        CU(cudaLaunchCooperativeKernel(reinterpret_cast<const void *>(kernel), dim3(grid), dim3(block), params, smem, st));
+    } else {
+        kernel<<<grid, block, smem, st>>>(args);
+    }
     g_launches.fetch_add(1, std::memory_order_relaxed);
     CU(cudaGetLastError());
     return 0;
 }
 
 // ---- dispatch on P ---------------------------------------------------------------------------------
-int launch_eval_lut_p(int p, int grid, int block, cudaStream_t st, const EvalLutArgs &a) {
-    const size_t sm = kAesSmemBytes;
-    switch (p) {
-    case 1: return launch(k_eval_lut<1>, grid, block, sm, st, a);
-    case 2: return launch(k_eval_lut<2>, grid, block, sm, st, a);
-    case 3: return launch(k_eval_lut<3>, grid, block, sm, st, a);
-    case 4: return launch(k_eval_lut<4>, grid, block, sm, st, a);
-    case 5: return launch(k_eval_lut<5>, grid, block, sm, st, a);
-    case 6: return launch(k_eval_lut<6>, grid, block, sm, st, a);
-    case 7: return launch(k_eval_lut<7>, grid, block, sm, st, a);
-    case 8: return launch(k_eval_lut<8>, grid, block, sm, st, a);
-    }
-    return FUSEFSS_E_SPEC;
-}
 int launch_gen_vec_p(int p, int grid, int block, cudaStream_t st, const GenVecArgs &a) {
     const size_t sm = kAesSmemBytes;
     switch (p) {
@@ -190,61 +177,103 @@ int launch_gen_vec_p(int p, int grid, int block, cudaStream_t st, const GenVecAr
     return FUSEFSS_E_SPEC;
 }
 
+// A launch is "small" when even with every tree of every element on its own warp it leaves at most 8 warps per SM: then the
+// 256-thread instantiation (255 registers per thread instead of 64) is used -- such launches live on the instruction-level
+// parallelism inside a warp, not on occupancy.
+bool small_launch(size_t warp_items) { return g_small_regs.load() && warp_items <= (size_t)g_sms * (kEvalThreadsSmall / 32); }
+
+// Protocol-3 construction: ONE kernel serves eval_cmp, eval_lut, the fused call and the both-parties call.
+// party = 0 / 1: that party only (slot 0); party = 2: both parties in one launch (slot b = party b).
+int launch_eval_p3(const Program &P, int party, const void *const key[2], const uint64_t *xhat, size_t count,
+                   uint64_t *const bits[2], uint64_t *const coeff[2], cudaStream_t st) {
+    Layout L; compute_layout(P, count, &L);
+    EvalArgs a{};
+    a.n_slots = party == 2 ? 2 : 1; a.party0 = party == 2 ? 0 : party; a.xhat = xhat;
+    for (int sl = 0; sl < a.n_slots; ++sl) { a.key[sl] = (const uint8_t *)key[sl]; a.bits_out[sl] = P.T > 0 ? bits[sl] : nullptr; a.coeff_out[sl] = P.has_lut ? coeff[sl] : nullptr; }
+    a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.lut_c = L.lut_c; a.vt_first = L.vt_first; a.vt_stride = L.vt_stride;
+    a.lvl_stride = L.lvl_stride; a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel;
+    a.mask = P.mask; a.n = (int)P.n; a.M = P.has_lut ? P.M : 1; a.T = P.T; a.et = (int)P.et;
+    for (int t = 0; t < P.T; ++t) a.atom[t] = CmpAtomDev{P.atoms[t].c, L.bt_root[t], L.bt_cw[t], L.bt_vb[t], P.atoms[t].k, 0};
+    const bool want_cmp = P.T > 0 && (a.bits_out[0] || a.bits_out[1]), want_lut = P.has_lut && (a.coeff_out[0] || a.coeff_out[1]);
+    const size_t tiles = (count + 31) / 32, units = tiles * (size_t)a.n_slots;
+    const size_t max_items = units * (size_t)((want_cmp ? P.T : 0) + (want_lut ? P.M - 1 : 0));
+    const bool small = small_launch(max_items);
+    const int cap = small ? kEvalThreadsSmall : g_eval_threads.load();
+    if (small) {                                   // every tree on its own warp: the chain of one tree is the critical path
+        a.Gc = want_cmp ? P.T : 1; a.Gl = want_lut ? P.M - 1 : 1;
+        if (const int f = g_force_g.load()) { a.Gc = f < a.Gc ? f : a.Gc; a.Gl = f < a.Gl ? f : a.Gl; }
+    } else {
+        a.Gc = want_cmp ? pick_groups(units, P.T, g_sms * (cap / 32)) : 1;
+        a.Gl = want_lut ? pick_groups(units, P.M - 1, g_sms * (cap / 32)) : 1;
+    }
+    const size_t items = units * (size_t)((want_cmp ? a.Gc : 0) + (want_lut ? a.Gl : 0));
+    a.zero_first = (want_cmp && a.Gc > 1) || (want_lut && a.Gl > 1);
+    const int threads = small ? kEvalThreadsSmall : threads_for(items, cap);
+    const int grid = grid_for(items, threads);
+    const size_t sm = kAesSmemBytes;
+    const bool coop = a.zero_first != 0;
+#define FSK_P3_CASE(PP) case PP: return small ? launch(k_eval_p3<PP, kEvalThreadsSmall>, grid, threads, sm, st, a, coop) \
+                                              : launch(k_eval_p3<PP, kEvalThreads>, grid, threads, sm, st, a, coop);
+    switch (P.p) { FSK_P3_CASE(1) FSK_P3_CASE(2) FSK_P3_CASE(3) FSK_P3_CASE(4) FSK_P3_CASE(5) FSK_P3_CASE(6) FSK_P3_CASE(7) FSK_P3_CASE(8) }
+#undef FSK_P3_CASE
+    return FUSEFSS_E_SPEC;
+}
+
 // variant 1: one kernel serves eval_cmp (bits only), eval_lut (coefficients only) and the fused call (both)
-// party = 0 / 1: that party only (key, bits_out, coeff_out); party = 2: both parties in ONE launch (the *_b arguments
-// are party 1's) -- half the launches and twice the parallelism for small tensors.
-int launch_eval_sp(Program &P, int party, const void *key, const uint64_t *xhat, size_t count, uint64_t *bits_out,
-                   uint64_t *coeff_out, cudaStream_t st, const void *key_b = nullptr, uint64_t *bits_out_b = nullptr,
-                   uint64_t *coeff_out_b = nullptr) {
-    int rc = ensure_blob(P); if (rc) return rc;
+// party = 0 / 1: that party only (key, bits_out, coeff_out); party = 2: both parties in ONE launch (slot b = party b)
+// -- half the launches and twice the parallelism for small tensors.
+int launch_eval_sp(const Program &P, int party, const void *const key[2], const uint64_t *xhat, size_t count,
+                   uint64_t *const bits[2], uint64_t *const coeff[2], cudaStream_t st) {
+    const uint8_t *blob = nullptr;
+    int rc = ensure_blob(P, &blob); if (rc) return rc;
     Layout L; compute_layout(P, count, &L);
     EvalSpArgs a{};
-    const uint8_t *blob = (const uint8_t *)P.dev_blob;
     a.n_parties = party == 2 ? 2 : 1; a.party0 = party == 2 ? 0 : party; a.xhat = xhat;
-    a.key2[0] = (const uint8_t *)key; a.bits_out2[0] = bits_out; a.coeff_out2[0] = coeff_out;
-    a.key2[1] = (const uint8_t *)key_b; a.bits_out2[1] = bits_out_b; a.coeff_out2[1] = coeff_out_b;
+    for (int sl = 0; sl < a.n_parties; ++sl) { a.key2[sl] = (const uint8_t *)key[sl]; a.bits_out2[sl] = P.T > 0 ? bits[sl] : nullptr; a.coeff_out2[sl] = P.has_lut ? coeff[sl] : nullptr; }
     a.points = (const SpPoint *)(blob + P.dev_sp_points_off); a.weights = (const uint64_t *)(blob + P.dev_sp_weights_off);
     a.delta_tab = (const uint64_t *)(blob + P.dev_sp_delta_off); a.alpha = (const uint64_t *)(blob + P.dev_alpha_off);
     a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.lvl_stride = L.lvl_stride; a.vt_first = L.vt_first;
     a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel; a.mask = P.mask;
-    a.n = (int)P.n; a.m = (int)P.m; a.p = P.p; a.T = P.T; a.n_w = P.sp.n_w;
+    a.n = (int)P.n; a.m = (int)P.m; a.p = P.p; a.T = P.T; a.n_w = P.sp.n_w; a.et = (int)P.et;
     a.n_clusters = (int)P.sp.clusters.size();
     a.cluster = (const SpCluster *)(blob + P.dev_sp_clusters_off);
     for (int w = 0; w < P.sp.n_w; ++w) { a.width[w] = P.sp.width[w]; a.bt_root[w] = L.bt_root[w]; a.bt_cw[w] = L.bt_cw[w]; a.bt_vb[w] = L.bt_vb[w]; }
     for (int t = 0; t < P.T; ++t) a.atom[t] = SpAtomDev{P.atoms[t].c, P.atoms[t].beta, P.atoms[t].k, P.atoms[t].is_theta};
     // small tensors: deal the points of an element to G warps so that the machine has >= ~8 warps per SM, then
-    // spread the warps over the SMs (threads per CTA = items / SMs rounded up to a warp, in [64, 1024])
+    // spread the warps over the SMs
     const size_t tiles = (count + 31) / 32;
     int maxpts = 1;
     for (int w = 0; w < P.sp.n_w; ++w) if (P.sp.width[w].n_points > maxpts) maxpts = P.sp.width[w].n_points;
     int G = (int)(((size_t)g_sms * 8 + tiles * a.n_parties - 1) / (tiles * a.n_parties));
     G = G < 1 ? 1 : G > 8 ? 8 : G;
     if (G > maxpts) G = maxpts;
-    if (const char *f = std::getenv("FUSEFSS_FORCE_G")) { int v = std::atoi(f); if (v >= 1) G = v < maxpts ? v : maxpts; }
+    if (const int f = g_force_g.load()) G = f < maxpts ? f : maxpts;
     a.G = G;
-    if (G > 1) {
-        if (bits_out) CU(cudaMemsetAsync(bits_out, 0, count * 8, st));
-        if (coeff_out) CU(cudaMemsetAsync(coeff_out, 0, count * 8 * (size_t)P.p, st));
-        if (bits_out_b) CU(cudaMemsetAsync(bits_out_b, 0, count * 8, st));
-        if (coeff_out_b) CU(cudaMemsetAsync(coeff_out_b, 0, count * 8 * (size_t)P.p, st));
-    }
-    const int threads = threads_for(tiles * G * a.n_parties, g_eval_threads);
-    const int grid = grid_for(tiles * G * a.n_parties, threads);
+    a.zero_first = G > 1;
+    const size_t items = tiles * (size_t)G * (size_t)a.n_parties;
+    const bool small = small_launch(items);
+    const int threads = small ? kEvalThreadsSmall : threads_for(items, g_eval_threads.load());
+    const int grid = grid_for(items, threads);
     const size_t sm = kAesSmemBytes;
     a.rpow = L.rpow;
-    int lrc = FUSEFSS_E_SPEC;
-#define FSK_SP_CASE(PP, KK) if (P.p == PP && P.sp.pk == KK) lrc = launch(k_eval_sp<PP, KK>, grid, threads, sm, st, a);
+    const bool coop = a.zero_first != 0;
+#define FSK_SP_CASE(PP, KK) if (P.p == PP && P.sp.pk == KK) return small ? launch(k_eval_sp<PP, KK, kEvalThreadsSmall>, grid, threads, sm, st, a, coop) \
+                                                                         : launch(k_eval_sp<PP, KK, kEvalThreads>, grid, threads, sm, st, a, coop);
 #define FSK_SP_ROW(KK) FSK_SP_CASE(1, KK) FSK_SP_CASE(2, KK) FSK_SP_CASE(3, KK) FSK_SP_CASE(4, KK) FSK_SP_CASE(5, KK) \
                        FSK_SP_CASE(6, KK) FSK_SP_CASE(7, KK) FSK_SP_CASE(8, KK)
     FSK_SP_ROW(1) FSK_SP_ROW(2) FSK_SP_ROW(3)
 #undef FSK_SP_ROW
 #undef FSK_SP_CASE
-    if (lrc == 0 && G > 1 && P.n < 64) {                                   // the atomics accumulated mod 2^64: reduce to the ring
-        const size_t words = count * (size_t)P.p;
-        for (uint64_t *c : {coeff_out, coeff_out_b})
-            if (c && lrc == 0) lrc = launch(k_mask_words, (int)((words + 255) / 256), 256, 0, st, MaskArgs{c, words, P.mask});
-    }
-    return lrc;
+    return FUSEFSS_E_SPEC;
+}
+
+// all four evaluation entry points end here
+int launch_eval(const Program &P, int party, const void *k0, const void *k1, const uint64_t *xhat, size_t count,
+                uint64_t *b0, uint64_t *b1, uint64_t *c0, uint64_t *c1, cudaStream_t st) {
+    const void *const key[2] = {k0, k1};
+    uint64_t *const bits[2] = {b0, b1};
+    uint64_t *const coeff[2] = {c0, c1};
+    return P.variant ? launch_eval_sp(P, party, key, xhat, count, bits, coeff, st) : launch_eval_p3(P, party, key, xhat, count, bits, coeff, st);
 }
 
 PostKeyOff post_offsets(const Layout &L) {
@@ -270,7 +299,7 @@ int fusefss_compile(const fusefss_spec *spec, fusefss_program **out) {
 
 void fusefss_destroy(fusefss_program *prog) {
     if (!prog) return;
-    if (prog->impl.dev_blob) cudaFree(prog->impl.dev_blob);
+    for (auto &kv : prog->impl.dev_blobs) cudaFree(kv.second);
     delete prog;
 }
 
@@ -325,10 +354,10 @@ int fusefss_cost(const fusefss_program *prog, fusefss_cost_t *out) {
     fusefss_cost_t c{};
     if (!P->variant) {
         for (int t = 0; t < P->T; ++t) {
-            const uint64_t k = (uint64_t)P->atoms[t].k;
+            const uint64_t k = (uint64_t)bit_tree_levels(*P, P->atoms[t].k);          // levels walked (early termination: k - 7)
             c.eval_cmp_aes += k + 1; c.eval_cmp_lookups += 160 * (k + 1);
             c.gen_cmp_aes += 4 * k + 4; c.gen_cmp_lookups += 2 * 160 + k * 2 * grp(2) + 2 * 160;
-            c.eval_cmp_key_bytes += 16 * (k + 1) + 8;
+            c.eval_cmp_key_bytes += 16 * ((uint64_t)bit_tree_arrays(*P, P->atoms[t].k) + 1) + 8;
         }
         if (P->has_lut) {
             const uint64_t trees = (uint64_t)P->M - 1, p = (uint64_t)P->p;
@@ -339,11 +368,11 @@ int fusefss_cost(const fusefss_program *prog, fusefss_cost_t *out) {
     } else {
         for (int w = 0; w < P->sp.n_w; ++w) {
             const SpWidth &W = P->sp.width[w];
-            const uint64_t k = (uint64_t)W.k;
             if (!W.is_vec) {
+                const uint64_t k = (uint64_t)bit_tree_levels(*P, W.k);
                 c.eval_cmp_aes += (uint64_t)W.n_points * (k + 1); c.eval_cmp_lookups += 160 * (uint64_t)W.n_points * (k + 1);
                 c.gen_cmp_aes += 4 * k + 4; c.gen_cmp_lookups += 2 * 160 + k * 2 * grp(2) + 2 * 160;
-                c.eval_cmp_key_bytes += 16 * (k + 1) + 8;
+                c.eval_cmp_key_bytes += 16 * ((uint64_t)bit_tree_arrays(*P, W.k) + 1) + 8;
                 continue;
             }
             for (const SpCluster &cl : P->sp.clusters) {                       // fused walk: every point of the n-bit tree
@@ -374,10 +403,20 @@ const char *fusefss_strerror(int code) {
     case FUSEFSS_E_ROUND: return "round out of range";
     case FUSEFSS_E_CUDA: return "CUDA error (see fusefss_last_cuda_error)";
     case FUSEFSS_E_OMITTED: return "call omitted for this gate type (T = 0 or m = 1)";
+    case FUSEFSS_E_WORKSPACE: return "workspace smaller than fusefss_gate_workspace_bytes()";
+    case FUSEFSS_E_DEBUG: return "unknown debug knob";
     }
     return "unknown error";
 }
 const char *fusefss_last_cuda_error(void) { return g_cuda_err; }
+int fusefss_debug_set(const char *knob, long value) {
+    if (!knob) return FUSEFSS_E_NULL;
+    const std::string k(knob);
+    if (k == "force_g") { g_force_g.store(value >= 1 ? (int)value : 0); return 0; }
+    if (k == "eval_threads") { g_eval_threads.store(value >= 32 && value <= kEvalThreads && value % 32 == 0 ? (int)value : kEvalThreads); return 0; }
+    if (k == "small_kernels") { g_small_regs.store(value ? 1 : 0); return 0; }
+    return FUSEFSS_E_DEBUG;
+}
 uint64_t fusefss_launch_count(void) { return g_launches.load(); }
 
 int fusefss_keygen(const fusefss_program *prog, const uint64_t *r_in_dev, const uint64_t *r_out_dev, uint64_t seed,
@@ -388,16 +427,16 @@ int fusefss_keygen(const fusefss_program *prog, const uint64_t *r_in_dev, const 
 
 int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, const uint64_t *r_out_dev, uint64_t seed,
                          uint64_t first_elem, size_t count, void *key0_dev, void *key1_dev, int parts, void *stream) {
-    Program *P = const_cast<Program *>(prog_of(prog));
+    const Program *P = prog_of(prog);
     if (!P || !r_in_dev || !key0_dev || !key1_dev) return FUSEFSS_E_NULL;
     if (P->mask_output && !r_out_dev) return FUSEFSS_E_NULL;
     if (count == 0) return FUSEFSS_E_COUNT;
     int rc = init_device(); if (rc) return rc;
-    rc = ensure_blob(*P); if (rc) return rc;
+    const uint8_t *blob = nullptr;
+    rc = ensure_blob(*P, &blob); if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     Layout L; compute_layout(*P, count, &L);
     const RoundKeys rk = seed_round_keys(seed);
-    const uint8_t *blob = (const uint8_t *)P->dev_blob;
     const uint64_t *alpha_dev = (const uint64_t *)(blob + P->dev_alpha_off);
     const uint64_t *payload_dev = (const uint64_t *)(blob + P->dev_payload_off);
     const size_t tiles = (count + 31) / 32;
@@ -406,7 +445,7 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
         bool any_bit = false, any_vec = false;
         GenBitArgs ab{};
         ab.key0 = (uint8_t *)key0_dev; ab.key1 = (uint8_t *)key1_dev; ab.r_in = r_in_dev;
-        ab.count = count; ab.s16 = L.s16; ab.first_elem = first_elem; ab.mask = P->mask; ab.T = P->sp.n_w; ab.rk = rk;
+        ab.count = count; ab.s16 = L.s16; ab.first_elem = first_elem; ab.mask = P->mask; ab.T = P->sp.n_w; ab.rk = rk; ab.et = (int)P->et;
         for (int w = 0; w < P->sp.n_w; ++w) {
             const bool vec = P->sp.width[w].is_vec != 0;
             any_bit = any_bit || !vec; any_vec = any_vec || vec;
@@ -429,7 +468,7 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
     if (!P->variant && P->T > 0 && (parts & FUSEFSS_GEN_CMP)) {
         GenBitArgs a{};
         a.key0 = (uint8_t *)key0_dev; a.key1 = (uint8_t *)key1_dev; a.r_in = r_in_dev;
-        a.count = count; a.s16 = L.s16; a.first_elem = first_elem; a.mask = P->mask; a.T = P->T; a.rk = rk;
+        a.count = count; a.s16 = L.s16; a.first_elem = first_elem; a.mask = P->mask; a.T = P->T; a.rk = rk; a.et = (int)P->et;
         for (int t = 0; t < P->T; ++t)
             a.atom[t] = GenAtomDev{P->atoms[t].c, P->atoms[t].beta, L.bt_root[t], L.bt_cw[t], L.bt_vb[t], P->atoms[t].k, P->atoms[t].is_theta};
         const int th = threads_for(tiles * P->T, kGenThreads), grid = grid_for(tiles * P->T, th);
@@ -460,7 +499,6 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
         a.xpoly = (int)P->xpoly; a.polys = (int)P->r; a.d = (int)P->d;
         a.T = P->variant ? 0 : P->T; a.MA = P->MA; a.MB = P->MB; a.GMIX = P->GMIX; a.rk = rk;
         for (int g = 0; g < P->MA; ++g) if (P->ma_is_x[g]) a.ma_is_x |= 1ull << g;
-        if (a.n_ka > 8) return FUSEFSS_E_SPEC;
         for (int t = 0; t < a.n_ka; ++t) { a.ka_kind[t] = P->kappa_a[t].kind; a.ka_arg[t] = P->kappa_a[t].arg; }
         for (int t = 0; t < a.n_kb_spec; ++t) { a.kb_kind[t] = P->kappa_b[t].kind; a.kb_arg[t] = P->kappa_b[t].arg; }
         for (int t = 0; t < a.T; ++t)
@@ -480,17 +518,7 @@ int fusefss_eval_cmp(int party, const fusefss_program *prog, const void *key_dev
     if (count == 0) return FUSEFSS_E_COUNT;
     if (P->T == 0) return FUSEFSS_E_OMITTED;
     int rc = init_device(); if (rc) return rc;
-    cudaStream_t st = (cudaStream_t)stream;
-    if (P->variant) return launch_eval_sp(*const_cast<Program *>(P), party, key_dev, xhat_dev, count, bits_out_dev, nullptr, st);
-    Layout L; compute_layout(*P, count, &L);
-    EvalCmpArgs a{};
-    a.key = (const uint8_t *)key_dev; a.xhat = xhat_dev; a.out = bits_out_dev; a.count = count; a.s16 = L.s16;
-    a.T = P->T; a.party = party;
-    a.G = pick_groups(count, P->T, g_eval_threads);
-    for (int t = 0; t < P->T; ++t) a.atom[t] = CmpAtomDev{P->atoms[t].c, L.bt_root[t], L.bt_cw[t], L.bt_vb[t], P->atoms[t].k, 0};
-    if (a.G > 1) CU(cudaMemsetAsync(bits_out_dev, 0, count * 8, st));
-    const int th = threads_for(((count + 31) / 32) * (size_t)a.G, g_eval_threads), grid = grid_for(((count + 31) / 32) * (size_t)a.G, th);
-    return launch(k_eval_cmp, grid, th, kAesSmemBytes, st, a);
+    return launch_eval(*P, party, key_dev, nullptr, xhat_dev, count, bits_out_dev, nullptr, nullptr, nullptr, (cudaStream_t)stream);
 }
 
 int fusefss_eval_lut(int party, const fusefss_program *prog, const void *key_dev, const uint64_t *xhat_dev, size_t count,
@@ -501,26 +529,8 @@ int fusefss_eval_lut(int party, const fusefss_program *prog, const void *key_dev
     if (count == 0) return FUSEFSS_E_COUNT;
     if (!P->has_lut) return FUSEFSS_E_OMITTED;
     int rc = init_device(); if (rc) return rc;
-    cudaStream_t st = (cudaStream_t)stream;
-    if (P->variant) return launch_eval_sp(*const_cast<Program *>(P), party, key_dev, xhat_dev, count, nullptr, coeff_out_dev, st);
-    Layout L; compute_layout(*P, count, &L);
-    EvalLutArgs a{};
-    a.key = (const uint8_t *)key_dev; a.xhat = xhat_dev; a.out = coeff_out_dev;
-    a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.lut_c = L.lut_c; a.vt_first = L.vt_first; a.vt_stride = L.vt_stride;
-    a.lvl_stride = L.lvl_stride; a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel;
-    a.mask = P->mask; a.n = (int)P->n; a.M = P->M; a.party = party;
-    a.G = pick_groups(count, P->M - 1, g_eval_threads);
-    if (a.G > 1) CU(cudaMemsetAsync(coeff_out_dev, 0, count * 8 * (size_t)P->p, st));
-    const int th = threads_for(((count + 31) / 32) * (size_t)a.G, g_eval_threads), grid = grid_for(((count + 31) / 32) * (size_t)a.G, th);
-    rc = launch_eval_lut_p(P->p, grid, th, st, a);
-    if (rc) return rc;
-    if (a.G > 1 && P->n < 64) {
-        const size_t words = count * (size_t)P->p;
-        return launch(k_mask_words, (int)((words + 255) / 256), 256, 0, st, MaskArgs{coeff_out_dev, words, P->mask});
-    }
-    return 0;
+    return launch_eval(*P, party, key_dev, nullptr, xhat_dev, count, nullptr, nullptr, coeff_out_dev, nullptr, (cudaStream_t)stream);
 }
-
 
 int fusefss_eval_fused(int party, const fusefss_program *prog, const void *key_dev, const uint64_t *xhat_dev, size_t count,
                        uint64_t *bits_out_dev, uint64_t *coeff_out_dev, void *stream) {
@@ -530,14 +540,8 @@ int fusefss_eval_fused(int party, const fusefss_program *prog, const void *key_d
     if (party != 0 && party != 1) return FUSEFSS_E_PARTY;
     if (count == 0) return FUSEFSS_E_COUNT;
     if (P->T == 0 && !P->has_lut) return FUSEFSS_E_OMITTED;
-    if (P->variant) {
-        int rc = init_device(); if (rc) return rc;
-        return launch_eval_sp(*const_cast<Program *>(P), party, key_dev, xhat_dev, count, P->T > 0 ? bits_out_dev : nullptr,
-                              P->has_lut ? coeff_out_dev : nullptr, (cudaStream_t)stream);
-    }
-    if (P->T > 0) { int rc = fusefss_eval_cmp(party, prog, key_dev, xhat_dev, count, bits_out_dev, stream); if (rc) return rc; }
-    if (P->has_lut) { int rc = fusefss_eval_lut(party, prog, key_dev, xhat_dev, count, coeff_out_dev, stream); if (rc) return rc; }
-    return 0;
+    int rc = init_device(); if (rc) return rc;
+    return launch_eval(*P, party, key_dev, nullptr, xhat_dev, count, bits_out_dev, nullptr, coeff_out_dev, nullptr, (cudaStream_t)stream);
 }
 
 int fusefss_eval_fused_both(const fusefss_program *prog, const void *key0_dev, const void *key1_dev, const uint64_t *xhat_dev,
@@ -548,21 +552,14 @@ int fusefss_eval_fused_both(const fusefss_program *prog, const void *key0_dev, c
     if ((P->T > 0 && (!bits0_dev || !bits1_dev)) || (P->has_lut && (!coeff0_dev || !coeff1_dev))) return FUSEFSS_E_NULL;
     if (count == 0) return FUSEFSS_E_COUNT;
     if (P->T == 0 && !P->has_lut) return FUSEFSS_E_OMITTED;
-    // one launch for both parties only while a single party cannot fill the machine (less than one wave of warps)
-    if (P->variant && (count + 31) / 32 <= (size_t)g_sms * (kEvalThreads / 32)) {
-        int rc = init_device(); if (rc) return rc;
-        return launch_eval_sp(*const_cast<Program *>(P), 2, key0_dev, xhat_dev, count, P->T > 0 ? bits0_dev : nullptr,
-                              P->has_lut ? coeff0_dev : nullptr, (cudaStream_t)stream, key1_dev, P->T > 0 ? bits1_dev : nullptr,
-                              P->has_lut ? coeff1_dev : nullptr);
-    }
-    int rc = fusefss_eval_fused(0, prog, key0_dev, xhat_dev, count, bits0_dev, coeff0_dev, stream); if (rc) return rc;
-    return fusefss_eval_fused(1, prog, key1_dev, xhat_dev, count, bits1_dev, coeff1_dev, stream);
+    int rc = init_device(); if (rc) return rc;
+    return launch_eval(*P, 2, key0_dev, key1_dev, xhat_dev, count, bits0_dev, bits1_dev, coeff0_dev, coeff1_dev, (cudaStream_t)stream);
 }
 
 int fusefss_post(int party, const fusefss_program *prog, const void *key_dev, const uint64_t *xhat_dev,
                  const uint64_t *bits_dev, const uint64_t *coeff_dev, size_t count, int round, const void *msg_in_dev,
                  void *msg_out_dev, uint64_t *y_out_dev, uint64_t *z_out_dev, void *stream) {
-    Program *P = const_cast<Program *>(prog_of(prog));
+    const Program *P = prog_of(prog);
     if (!P || !key_dev || !xhat_dev) return FUSEFSS_E_NULL;
     if (party != 0 && party != 1) return FUSEFSS_E_PARTY;
     if (count == 0) return FUSEFSS_E_COUNT;
@@ -572,10 +569,11 @@ int fusefss_post(int party, const fusefss_program *prog, const void *key_dev, co
     if (round > 0 && !msg_in_dev) return FUSEFSS_E_NULL;
     if (round == P->rounds && ((P->n_out_a > 0 && !y_out_dev) || (P->n_out_b > 0 && !z_out_dev))) return FUSEFSS_E_NULL;
     int rc = init_device(); if (rc) return rc;
-    rc = ensure_blob(*P); if (rc) return rc;
+    const uint8_t *blob = nullptr;
+    rc = ensure_blob(*P, &blob); if (rc) return rc;
     Layout L; compute_layout(*P, count, &L);
     PostArgs a{};
-    a.ins = (const Ins *)((const uint8_t *)P->dev_blob + P->dev_ins_off); a.n_ins = (int)P->ins.size();
+    a.ins = (const Ins *)(blob + P->dev_ins_off); a.n_ins = (int)P->ins.size();
     a.party = party; a.round = round; a.rounds = P->rounds; a.mask_output = (int)P->mask_output;
     a.n_out_a = P->n_out_a; a.n_out_b = P->n_out_b;
     a.key = (const uint8_t *)key_dev; a.xhat = xhat_dev; a.bits = bits_dev; a.coeff = coeff_dev;
@@ -593,16 +591,17 @@ int fusefss_post_fused(const fusefss_program *prog, const void *key0_dev, const 
                        const uint64_t *bits0_dev, const uint64_t *bits1_dev, const uint64_t *coeff0_dev,
                        const uint64_t *coeff1_dev, size_t count, uint64_t *y0_dev, uint64_t *y1_dev, uint64_t *z0_dev,
                        uint64_t *z1_dev, void *stream) {
-    Program *P = const_cast<Program *>(prog_of(prog));
+    const Program *P = prog_of(prog);
     if (!P || !key0_dev || !key1_dev || !xhat_dev) return FUSEFSS_E_NULL;
     if (count == 0) return FUSEFSS_E_COUNT;
     if ((P->T > 0 && (!bits0_dev || !bits1_dev)) || (P->has_lut && (!coeff0_dev || !coeff1_dev))) return FUSEFSS_E_NULL;
     if ((P->n_out_a > 0 && (!y0_dev || !y1_dev)) || (P->n_out_b > 0 && (!z0_dev || !z1_dev))) return FUSEFSS_E_NULL;
     int rc = init_device(); if (rc) return rc;
-    rc = ensure_blob(*P); if (rc) return rc;
+    const uint8_t *blob = nullptr;
+    rc = ensure_blob(*P, &blob); if (rc) return rc;
     Layout L; compute_layout(*P, count, &L);
     PostFusedArgs a{};
-    a.ins = (const Ins *)((const uint8_t *)P->dev_blob + P->dev_ins_off); a.n_ins = (int)P->ins.size();
+    a.ins = (const Ins *)(blob + P->dev_ins_off); a.n_ins = (int)P->ins.size();
     a.mask_output = (int)P->mask_output; a.n_out_a = P->n_out_a; a.n_out_b = P->n_out_b;
     a.key[0] = (const uint8_t *)key0_dev; a.key[1] = (const uint8_t *)key1_dev; a.xhat = xhat_dev;
     a.bits[0] = bits0_dev; a.bits[1] = bits1_dev; a.coeff[0] = coeff0_dev; a.coeff[1] = coeff1_dev;
@@ -674,10 +673,11 @@ size_t fusefss_gate_workspace_bytes(const fusefss_program *prog, size_t chunk) {
 }
 
 int fusefss_gate_host(const fusefss_program *prog, const uint64_t *r_in, const uint64_t *r_out, const uint64_t *xhat,
-                      uint64_t seed, size_t count, size_t chunk, void *workspace_dev, uint64_t *y0, uint64_t *y1,
-                      uint64_t *z0, uint64_t *z1, void *stream) {
+                      uint64_t seed, size_t count, size_t chunk, void *workspace_dev, size_t workspace_bytes, uint64_t *y0,
+                      uint64_t *y1, uint64_t *z0, uint64_t *z1, void *stream) {
     const Program *P = prog_of(prog);
     if (!P || !r_in || !xhat || !workspace_dev) return FUSEFSS_E_NULL;
+    if (chunk && workspace_bytes < fusefss_gate_workspace_bytes(prog, chunk)) return FUSEFSS_E_WORKSPACE;
     if (P->mask_output && !r_out) return FUSEFSS_E_NULL;
     if ((P->n_out_a > 0 && (!y0 || !y1)) || (P->n_out_b > 0 && (!z0 || !z1))) return FUSEFSS_E_NULL;
     if (count == 0 || chunk == 0) return FUSEFSS_E_COUNT;
@@ -780,8 +780,8 @@ int fusefss_aes_probe(size_t threads, int iters, void *out_dev, void *stream) {
     if (threads == 0 || iters <= 0) return FUSEFSS_E_COUNT;
     int rc = init_device(); if (rc) return rc;
     ProbeArgs a{(uint4 *)out_dev, threads, iters};
-    const int grid = grid_for((threads + 31) / 32, g_eval_threads);
-    return launch(k_aes_probe, grid, g_eval_threads, kAesSmemBytes, (cudaStream_t)stream, a);
+    const int grid = grid_for((threads + 31) / 32, kEvalThreads);
+    return launch(k_aes_probe, grid, kEvalThreads, kAesSmemBytes, (cudaStream_t)stream, a);
 }
 
 int fusefss_pipe_probe(int kind, int iters, void *out_dev, void *stream) {

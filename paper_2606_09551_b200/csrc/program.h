@@ -3,6 +3,8 @@
 #pragma once
 #include <cstddef>
 #include <cstdint>
+#include <map>
+#include <mutex>
 #include <vector>
 
 #include "../../include/fusefss.h"
@@ -88,15 +90,22 @@ struct Program {
     // variant bit 1 (DESIGN 10): a product with the gate input x opens one ring element and needs (b, c = b r_in)
     uint32_t xmul = 0;
     uint32_t xpoly = 0;                   // variant bit 2 (DESIGN 11): Horner in the public xhat, zero Beaver rounds for the spline
+    uint32_t et = 0;                      // variant bit 3 (DESIGN 13): bit trees stop max(k-7,0) levels deep, 128-bit leaf block
     int round_arr[kMaxRounds] = {0};      // ring-element arrays opened per round: 2 per Beaver, 1 per x-product
     int ma_is_x[64] = {0}, ma_word[65] = {0};
     // payload table v[i][w], i < m, w < p (coefficients poly-major, high degree first, then aux), masked
     std::vector<uint64_t> payload;
-    // device copy of the small tables (uploaded lazily by the launchers)
-    void *dev_blob = nullptr;
+    // device copies of the small tables: one per device, uploaded on first use there (launchers), freed by fusefss_destroy.
+    // The offsets inside the blob are fixed by compile_program.
+    mutable std::mutex blob_mu;
+    mutable std::map<int, void *> dev_blobs;
     size_t dev_ins_off = 0, dev_alpha_off = 0, dev_payload_off = 0, dev_blob_bytes = 0;
     size_t dev_sp_points_off = 0, dev_sp_weights_off = 0, dev_sp_delta_off = 0, dev_sp_clusters_off = 0;
 };
+
+// 16-byte correction arrays of a bit tree on k input bits: k levels, or max(k-7,0) levels + the leaf block (DESIGN 13)
+inline int bit_tree_levels(const Program &P, int k) { return P.et ? (k > 7 ? k - 7 : 0) : k; }
+inline int bit_tree_arrays(const Program &P, int k) { return bit_tree_levels(P, k) + (P.et ? 1 : 0); }
 
 int compile_program(const fusefss_spec *spec, Program **out);
 void compute_layout(const Program &P, size_t count, Layout *L);

@@ -98,7 +98,7 @@ def random_spec(seed, variant=0):
     spec = S._mk(f"rand{seed}_n{n}", n, f, cuts, coeff, nodes=nodes, bit_root=bit_root if ell else None, aux=aux if p_aux else None,
                  kappa_a=kappa_a, kappa_b=kappa_b, phi=phi, n_out_a=n_out_a, n_out_b=n_out_b,
                  mask_output=bool(rng.random() < 0.3), out_frac=f)
-    spec.variant = variant if (not (variant & 4) or d <= 2) else variant & 3
+    spec.variant = variant if (not (variant & 4) or d <= 2) else variant & ~4
     return spec
 
 

@@ -38,6 +38,7 @@ ALL = [("relu16", lambda: specs.relu(16, 8)), ("gelu", specs.gelu), ("nexp", spe
 ALL = ALL + [(nm + "_sp", (lambda mk=mk: specs.shared_prefix(mk()))) for nm, mk in ALL]      # variant 1 (DESIGN 9)
 ALL = ALL + [(nm + "_xm", (lambda mk=mk: specs.input_masked_mul(mk()))) for nm, mk in ALL]  # variant bit 1 (DESIGN 10)
 ALL = ALL + [(nm + "_xp", (lambda mk=mk: specs.public_point_horner(mk()))) for nm, mk in ALL[:32]]  # variant bit 2 (DESIGN 11)
+ALL = ALL + [(nm + "_et", (lambda mk=mk: specs.early_termination(mk()))) for nm, mk in ALL[:32] + ALL[-4:]]  # variant bit 3 (DESIGN 13)
 
 
 @pytest.mark.parametrize("name,mk", ALL)
@@ -92,6 +93,11 @@ def test_rejects_ill_formed_specs(F):
     bad3.n = 65
     with pytest.raises(F.FuseFSSError):
         F.Program(bad3)
+    from test_oracle_gate import ill_formed_specs
+    for why, s in ill_formed_specs():                           # the same list the oracle's compiler rejects
+        with pytest.raises(F.FuseFSSError):
+            F.Program(s)
+            pytest.fail("accepted: " + why)
     assert F.Program(good).shape["T"] == 2
     assert F.lib.fusefss_key_bytes(None, 10) == 0
     assert F.lib.fusefss_strerror(-3) == b"party must be 0 or 1"
@@ -109,3 +115,5 @@ def test_argument_errors_without_gpu(F):
     Ps = F.Program(specs.single_interval())
     assert F.lib.fusefss_eval_lut(0, Ps._h, 1, 1, 10, 1, None) == -7     # m = 1: call omitted
     assert F.lib.fusefss_post(0, P._h, 1, 1, 1, 1, 10, 99, 1, 1, 1, 1, None) == -5
+    assert F.lib.fusefss_gate_host(P._h, 1, 1, 1, 0, 10, 10, 1, 16, 1, 1, 1, 1, None) == -8    # workspace too small
+    assert F.lib.fusefss_debug_set(b"no_such_knob", 1) == -9 and F.lib.fusefss_debug_set(b"force_g", 0) == 0

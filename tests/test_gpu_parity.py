@@ -115,12 +115,30 @@ SMALL_XM = [(lambda mk=mk: specs.input_masked_mul(mk())) for mk in SMALL[:4] + S
 SMALL_XP = [(lambda mk=mk: specs.public_point_horner(mk())) for mk in SMALL[1:4] + SMALL[5:6] + SMALL[8:9] + SMALL_SP[1:4] + SMALL_SP[5:6] + SMALL_SP[8:9]]
 
 
-@pytest.mark.parametrize("mk", SMALL + SMALL_SP + SMALL_XM + SMALL_XP)
-@pytest.mark.parametrize("force_g", ["", "1"])
-def test_small_rings_all_masks(F, orc, mk, force_g, monkeypatch):
-    """Every mask r (both Protocol 3 branches, incl. beta_0 = 0 and the dummy split) at n <= 8; a ragged count."""
-    if force_g:
-        monkeypatch.setenv("FUSEFSS_FORCE_G", force_g)
+SMALL_ET = [(lambda mk=mk: specs.early_termination(mk())) for mk in SMALL[:5] + SMALL[7:] + SMALL_SP[:5] + SMALL_SP[7:] + SMALL_XM[:2] + SMALL_XP[-2:]]
+
+
+@pytest.fixture
+def knobs(F):
+    """fusefss_debug_set knobs, restored after the test"""
+    def set_(**kw):
+        for k, v in kw.items():
+            F.debug_set(k, v)
+    yield set_
+    F.debug_set("force_g", 0); F.debug_set("small_kernels", 1); F.debug_set("eval_threads", 1024)
+
+
+@pytest.mark.parametrize("mk", SMALL + SMALL_SP + SMALL_XM + SMALL_XP + SMALL_ET)
+@pytest.mark.parametrize("mode", ["auto", "g1", "g2_big"])
+def test_small_rings_all_masks(F, orc, mk, mode, knobs):
+    """Every mask r (both Protocol 3 branches, incl. beta_0 = 0 and the dummy split) at n <= 8; a ragged count.
+    auto: the launch configuration the library picks (small launches: every tree on its own warp, 256-thread kernels, in-kernel
+    zeroing + atomics); g1: one warp walks all trees of an element (no atomics); g2_big: two tree groups with the 1024-thread
+    instantiations (the code path of large tensors whose last wave is split)."""
+    if mode == "g1":
+        knobs(force_g=1)
+    if mode == "g2_big":
+        knobs(force_g=2, small_kernels=0)
     spec = mk()
     N = 1 << spec.n
     rng = np.random.default_rng(5)
@@ -139,7 +157,7 @@ CONFIGS = [("relu16", 4096), ("gelu", 700), ("nexp", 330), ("recip", 130), ("shi
            ("silu", 131)]
 
 
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 8, 9])
 @pytest.mark.parametrize("name,count", CONFIGS)
 def test_config_parity(F, orc, name, count, variant):
     """BASELINE.json's configs on their seeded synthetic inputs (workloads/tensors.py), several 32-element tiles
@@ -155,6 +173,8 @@ def test_config_parity(F, orc, name, count, variant):
     if variant & 4:
         spec = specs.public_point_horner(spec)              # Horner in the public xhat, zero Beaver rounds (DESIGN 11)
         count = max(33, count // 2)
+    if variant & 8:
+        spec = specs.early_termination(spec)                # bit trees cut 7 levels early (DESIGN 13)
     inp = tensors.inputs(name, spec, count=count, seed=0)
     _parity(F, orc, spec, inp["x"], inp["r_in"], inp["r_out"], seed=0)
 
@@ -207,7 +227,7 @@ def test_gate_host_end_to_end(F, orc):
     assert np.array_equal(z0, exp["z"][0]) and np.array_equal(z1, exp["z"][1])
 
 
-FULL = [("relu16", 0), ("relu16", 1), ("gelu", 0), ("gelu", 1), ("gelu", 5), ("nexp", 0), ("nexp", 1), ("recip", 0), ("recip", 1),
+FULL = [("relu16", 0), ("relu16", 1), ("relu16", 8), ("shift_relu", 8), ("shift_relu", 9), ("gelu", 8), ("gelu", 0), ("gelu", 1), ("gelu", 5), ("nexp", 0), ("nexp", 1), ("recip", 0), ("recip", 1),
         ("shift_relu", 0), ("shift_relu", 1), ("rsqrt", 0), ("rsqrt", 3), ("silu", 0), ("silu", 1)]
 
 
@@ -229,6 +249,8 @@ def test_full_size_sampled(F, orc, name, variant):
         spec = specs.input_masked_mul(spec)
     if variant & 4:
         spec = specs.public_point_horner(spec)
+    if variant & 8:
+        spec = specs.early_termination(spec)
     count = tensors.FULL_COUNT[name]
     first = 0
     if name == "silu" and not variant & 1:                    # does not fit resident: bench.py streams chunks of this size

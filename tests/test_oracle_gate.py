@@ -158,15 +158,35 @@ def test_complexity_accounting_table(orc):
     assert P.online_bits() == 64 + 2 * 64 + 2 + 2
 
 
+def ill_formed_specs():
+    """(why, spec) pairs that both compilers must reject."""
+    import copy
+    out = []
+    s = specs.relu(8, 4); s.alpha = [0]; out.append(("boundary 0", s))
+    s = specs.toy(8, 3); s.alpha = [40, 40, 200]; out.append(("boundaries not strictly increasing", s))
+    s = specs.toy(8, 3); s.alpha = [40, 100, 256]; out.append(("boundary >= 2^n", s))
+    s = specs.toy(8, 3); s.nodes = list(s.nodes); s.nodes[2] = (specs.BN_C, 0, 0, 0, 0, 300); out.append(("C_beta with beta > 2^n", s))
+    s = specs.toy(8, 3); s.nodes = list(s.nodes); s.nodes[0] = (specs.BN_D, 3, 0, 0, 0, 9); out.append(("D_gamma with gamma > 2^f", s))
+    s = specs.toy(8, 3); s.nodes = list(s.nodes); s.nodes[0] = (specs.BN_D, 9, 0, 0, 0, 1); out.append(("D width > n", s))
+    s = specs.toy(8, 3); s.nodes = list(s.nodes); s.nodes[3] = (specs.BN_AND, 0, 0, 5, 0, 0); out.append(("operand does not precede", s))
+    s = specs.toy(8, 3); s.kappa_b = [(specs.KB_R_BIT, 8)]; out.append(("kappa^B bit index >= n", s))
+    s = specs.toy(8, 3); s.kappa_a = [(specs.KA_R_SHR, 64)]; out.append(("kappa^A shift >= 64", s))
+    s = specs.toy(8, 3); s.kappa_a = [(specs.KA_R_SHR, 1)] * 9; out.append(("more than 8 kappa^A", s))
+    s = specs.toy(8, 3); s.phi = [(specs.PHI_B_XHAT, d, 8, b, i) if (op, a) == (specs.PHI_B_XHAT, 1) else (op, d, a, b, i) for (op, d, a, b, i) in s.phi]
+    out.append(("xhat bit index >= n", s))
+    s = specs.shift_relu(8, 3); s.phi = [(op, d, a, 8 if op == specs.PHI_B_ANDPUB else b, i) for (op, d, a, b, i) in s.phi]; out.append(("ANDPUB bit index >= n", s))
+    s = specs.toy(8, 3); s.phi = [o for o in s.phi if not (o[0] == specs.PHI_A_OUT and o[1] == 1)]; out.append(("arithmetic output never written", s))
+    s = specs.toy(8, 3); s.phi = s.phi + [(specs.PHI_B_OUT, 0, 7, 0, 0)]; out.append(("bit output written twice", s))
+    s = specs.toy(8, 3); s.phi = s.phi + [(99, 0, 0, 0, 0)]; out.append(("unknown Phi op", s))
+    return out
+
+
 def test_rejects_ill_formed(orc):
-    s = specs.relu(8, 4)
-    s.alpha = [0]
-    with pytest.raises(ValueError):
-        orc.Program(s)
-    s = specs.toy(8, 3)
-    s.alpha = [40, 40, 200]
-    with pytest.raises(ValueError):
-        orc.Program(s)
+    for why, s in ill_formed_specs():
+        with pytest.raises(ValueError):
+            orc.Program(s)
+            pytest.fail("accepted: " + why)
+    orc.Program(specs.toy(8, 3))
 
 
 @pytest.mark.parametrize("variant", [0, 1])

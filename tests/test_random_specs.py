@@ -7,7 +7,7 @@ import pytest
 
 from helpers import mask_of, pack_bits, random_spec
 
-VARIANTS = [0, 1, 2, 3, 4, 5, 7]
+VARIANTS = [0, 1, 2, 3, 4, 5, 7, 8, 9, 15]
 
 
 @pytest.fixture(scope="module")
@@ -47,7 +47,7 @@ def _inputs(spec, count, seed):
 
 @pytest.mark.parametrize("seed", range(24))
 def test_oracle_reconstructs_random_specs(orc, seed):
-    for v in (0, 1, 3, 5):
+    for v in (0, 1, 3, 5, 8, 15):
         spec = random_spec(seed, v)
         P = orc.Program(spec)
         count = 48
