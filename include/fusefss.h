@@ -183,6 +183,9 @@ int fusefss_post_fused(const fusefss_program *prog, const void *key0_dev, const 
  * fusefss_share_open: Protocol 1 for the input of gate `prog`: xhat = (x_0 + [r_in]_0) + (x_1 + [r_in]_1)
  *   + public_offset; the [r_in] shares are read from the two key buffers generated for these `count` elements (n/8 bytes
  *   per party).  public_offset = 2^{n-1} feeds the signed-truncation gate (workloads.specs.ars), 0 otherwise.
+ * fusefss_open_output: online step 6 for a gate compiled with mask_output: yhat = y0 + y1 + public_offset, where y_b
+ *   are the parties' shares of y + r_out written by fusefss_post / _post_fused (n/8 bytes per party).  When the NEXT gate is keyed
+ *   with r_in = this gate's r_out, yhat is that gate's xhat: no second mask and no separate fusefss_share_open pass.
  * fusefss_sub_bcast: out[i] = x[i] - mu[i / cols] mod 2^n, local on additive shares.
  * fusefss_row_sum: out[r] = sum_c in[r*cols + c] mod 2^n, local on additive shares.
  * fusefss_mul_keygen / fusefss_mul_fused: element-wise Beaver products z = x * y (formulas DESIGN 4.6) with y
@@ -191,6 +194,8 @@ int fusefss_post_fused(const fusefss_program *prog, const void *key0_dev, const 
  *   2n/8 online bytes per party per product. */
 int fusefss_share_open(const fusefss_program *prog, const void *key0_dev, const void *key1_dev, const uint64_t *x0_dev,
                        const uint64_t *x1_dev, size_t count, uint64_t public_offset, uint64_t *xhat_out_dev, void *stream);
+int fusefss_open_output(uint32_t n_bits, const uint64_t *y0_dev, const uint64_t *y1_dev, size_t count, uint64_t public_offset,
+                        uint64_t *yhat_out_dev, void *stream);
 int fusefss_sub_bcast(uint32_t n_bits, const uint64_t *x_dev, const uint64_t *mu_dev, size_t count, size_t cols,
                       uint64_t *out_dev, void *stream);
 int fusefss_row_sum(uint32_t n_bits, const uint64_t *in_dev, size_t rows, size_t cols, uint64_t *out_dev, void *stream);
@@ -237,6 +242,12 @@ int fusefss_aes_probe(size_t threads, int iters, void *out_dev, void *stream);
  * conflict-free LDS.32 wavefronts (8 dependent-lookup chains per thread through the bank-replicated table).  One CTA of
  * 1024 threads per SM; out_dev holds SMs*1024 uint32.  Operations executed = SMs * 1024 * 8 * iters (lane-ops). */
 int fusefss_pipe_probe(int kind, int iters, void *out_dev, void *stream);
+/* A bitsliced AES-128 core (32 blocks per thread as 128 bit-planes, composite-field S-box circuit), built only to TIME it against the
+ * T-table core (DESIGN 5.2).  _kat: in_dev / out_dev = 32 blocks of 16 bytes (device), one encryption with key[16] (HOST).
+ * _probe: each of `threads` threads chains `iters` encryptions of its 32 blocks; out_dev holds threads*16 bytes; blocks =
+ * threads * 32 * iters. */
+int fusefss_bitslice_kat(const uint8_t *key, const void *in_dev, void *out_dev, void *stream);
+int fusefss_bitslice_probe(const uint8_t *key, size_t threads, int iters, void *out_dev, void *stream);
 /* single-block AES-128 (FIPS-197) through the device PRG core, for the known-answer test: key[16], in[16] HOST,
  * out_dev[16] device */
 int fusefss_aes_kat(const uint8_t *key, const uint8_t *in, void *out_dev, void *stream);

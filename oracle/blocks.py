@@ -12,12 +12,17 @@ import oracle
 SLOT_MUL_AB, SLOT_MUL_AB0, SLOT_MUL_C0 = 0xA000, 0xA001, 0xA002
 
 
-def gate(P, x0, x1, r_in, seed, first=0, offset=0):
+def gate(P, x0, x1, r_in, seed, first=0, offset=0, r_out=None, opened=False):
     """One compiled gate on additively shared inputs: Protocol 1 (masked opening), then the online procedure.
-    `offset` = public constant added to the gate input (2^63 for the signed truncation gate workloads.specs.ars)."""
+    `offset` = public constant added to the gate input (2^63 for the signed truncation gate workloads.specs.ars).
+    r_out: output mask of a gate compiled with mask_output (its outputs are then shares of yhat = y + r_out).
+    opened: (x0, x1) are the producer's shares of yhat with r_out(producer) = this gate's r_in, so xhat = x0 + x1 (step 6)."""
     count = x0.size
-    k0, k1 = P.keygen(r_in, None, seed, first)
-    xhat = x0 + P.rin_shares(k0, count) + x1 + P.rin_shares(k1, count) + np.uint64(offset)   # n = 64: wraps mod 2^64
+    k0, k1 = P.keygen(r_in, None if r_out is None else r_out.reshape(1, -1), seed, first)
+    if opened:
+        xhat = x0 + x1 + np.uint64(offset)
+    else:
+        xhat = x0 + P.rin_shares(k0, count) + x1 + P.rin_shares(k1, count) + np.uint64(offset)   # n = 64: wraps mod 2^64
     out = P.run_gate(k0, k1, xhat)
     return out["y"][0][0], out["y"][1][0], xhat
 
@@ -36,14 +41,17 @@ def beaver_mul(x0, x1, y0, y1, cols, seed, first=0):
     return E * Fv + E * b0 + Fv * a0 + c0, E * b1 + Fv * a1 + c1
 
 
-def softmax(progs, x0, x1, masks, rows, cols, seed):
-    """progs / masks: dicts with the stages 'nexp', 'tr_e', 'recip', 'tr_t', 'tr_y' (oracle Programs / r_in arrays)."""
+def softmax(progs, x0, x1, masks, rows, cols, seed, fused_open=False):
+    """progs / masks: dicts with the stages 'nexp', 'tr_e', 'recip', 'tr_t', 'tr_y' (oracle Programs / r_in arrays).
+    fused_open: nExp and Recip are mask_output gates keyed with r_out = the following truncation gate's r_in; their opened
+    yhat is that gate's xhat (then out['e'], out['t'] are shares of the MASKED values)."""
+    fo = fused_open
     with np.errstate(over="ignore"):
-        e0, e1, _ = gate(progs["nexp"], x0, x1, masks["nexp"], seed + 1)
-        f0, f1, _ = gate(progs["tr_e"], e0, e1, masks["tr_e"], seed + 2)
+        e0, e1, _ = gate(progs["nexp"], x0, x1, masks["nexp"], seed + 1, r_out=masks["tr_e"] if fo else None)
+        f0, f1, _ = gate(progs["tr_e"], e0, e1, masks["tr_e"], seed + 2, opened=fo)
         s0, s1 = f0.reshape(rows, cols).sum(axis=1, dtype=np.uint64), f1.reshape(rows, cols).sum(axis=1, dtype=np.uint64)
-        t0, t1, _ = gate(progs["recip"], s0, s1, masks["recip"], seed + 3)
-        u0, u1, _ = gate(progs["tr_t"], t0, t1, masks["tr_t"], seed + 4)
+        t0, t1, _ = gate(progs["recip"], s0, s1, masks["recip"], seed + 3, r_out=masks["tr_t"] if fo else None)
+        u0, u1, _ = gate(progs["tr_t"], t0, t1, masks["tr_t"], seed + 4, opened=fo)
         p0, p1 = beaver_mul(f0, f1, u0, u1, cols, seed + 5)
         y0, y1, _ = gate(progs["tr_y"], p0, p1, masks["tr_y"], seed + 6)
     return dict(e=(e0, e1), f=(f0, f1), s=(s0, s1), t=(t0, t1), u=(u0, u1), p=(p0, p1), y=(y0, y1))
@@ -67,7 +75,7 @@ def softmax_plain(progs, x, rows, cols):
 HALF = 1 << 63
 
 
-def layernorm(progs, x0, x1, masks, rows, d, seed):
+def layernorm(progs, x0, x1, masks, rows, d, seed, fused_open=False):
     """LayerNorm without affine parameters on rows of length d = 2^k at scale 2^12 (App. G: mean / variance reductions
     are linear, rsqrt is a compiled gate):  mu = ARS_k(sum x); c = x - mu; v = ARS_{k+12}(sum c^2); g = rsqrt(v) (scale
     2^48) -> ARS_24; y = ARS_24(c * g).  progs / masks: stages 'mean', 'var', 'rsqrt', 'tr_g', 'tr_y'."""
@@ -77,8 +85,8 @@ def layernorm(progs, x0, x1, masks, rows, d, seed):
         c0, c1 = x0 - np.repeat(m0, d), x1 - np.repeat(m1, d)
         q0, q1 = beaver_mul(c0, c1, c0, c1, 1, seed + 2)
         v0, v1, _ = gate(progs["var"], rs(q0), rs(q1), masks["var"], seed + 3, offset=HALF)
-        g0, g1, _ = gate(progs["rsqrt"], v0, v1, masks["rsqrt"], seed + 4)
-        h0, h1, _ = gate(progs["tr_g"], g0, g1, masks["tr_g"], seed + 5, offset=HALF)
+        g0, g1, _ = gate(progs["rsqrt"], v0, v1, masks["rsqrt"], seed + 4, r_out=masks["tr_g"] if fused_open else None)
+        h0, h1, _ = gate(progs["tr_g"], g0, g1, masks["tr_g"], seed + 5, offset=HALF, opened=fused_open)
         p0, p1 = beaver_mul(c0, c1, h0, h1, d, seed + 6)
         y0, y1, _ = gate(progs["tr_y"], p0, p1, masks["tr_y"], seed + 7, offset=HALF)
     return dict(m=(m0, m1), c=(c0, c1), q=(q0, q1), v=(v0, v1), g=(g0, g1), h=(h0, h1), p=(p0, p1), y=(y0, y1))

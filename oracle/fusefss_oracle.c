@@ -651,6 +651,7 @@ typedef struct orc_prog {
     int xmul;                         /* variant bit 1 */
     int xpoly;                        /* variant bit 2: payload = coefficients of P_i(X - r_in), Horner in the public xhat */
     int et;                           /* variant bit 3: bit trees are early-terminated (DESIGN 13) */
+    int dense;                        /* variant bit 4: dense-table ("DPF-LUT") lookup by full-domain evaluation (DESIGN 14) */
     int r_narr[16];                   /* ring-element arrays opened per round: 2 per Beaver, 1 per x-product */
     int ma_is_x[64], ma_word[65];     /* per arithmetic gate: kind, first word of its material in the key */
     /* lowering memo */
@@ -884,6 +885,8 @@ orc_prog *orc_compile(const orc_spec *S0)
     P->xmul = (int)((S->variant >> 1) & 1);
     P->xpoly = (int)((S->variant >> 2) & 1) && S->d >= 1 && P->m > 1;
     P->et = (int)((S->variant >> 3) & 1);
+    P->dense = (int)((S->variant >> 4) & 1);
+    if (P->dense && (!P->variant || P->xpoly || P->n > 16)) { orc_destroy(P); return NULL; }   /* needs the single key, n <= 16 */
     if (P->variant) P->M = P->m;                         /* no translated partition, hence no wrap/dummy split */
     for (int i = 0; i < 4096; i++) P->node_reg[i] = -1;
     for (int i = 0; i <= MMAX; i++) P->calpha_reg[i] = -1;
@@ -1472,6 +1475,35 @@ static void sp_eval(int party, const orc_prog *P, const u8 *key, const u64 *xhat
                     }
                 }
                 coeff_out[(size_t)wd * count + e] = acc & P->mask;
+            }
+            if (P->dense) {
+                /* Dense-table lookup (DESIGN 14): T[u] = payload of the interval that contains u, u = 0..N-1 -- the operator as a
+                 * table of 2^n entries.  With A_b(v) = Eval_b(key, v) the share of I[v < r] at EVERY point v of the domain and
+                 * D[a] = T[a-1] - T[a]:   T[x] = T[xhat] - I[xhat < r] (T[0] - T[N-1]) + sum_{a=1}^{N-1} D[a] I[(xhat - a) mod N < r]
+                 * (the variant-1 identity with every point of the ring as a boundary).  Work and shape depend on n only. */
+                u64 N = (u64)1 << P->n;
+                u64 acc[PMAX] = { 0 };
+                for (u64 v = 0; v < N; v++) {
+                    u64 Av[PMAX];
+                    dcf_vec_eval(party, P->n, 1, P->mask, vk, v, Av);
+                    u64 a = (xh - v) & P->mask;                        /* v = xhat - a */
+                    for (int wd = 0; wd < P->p; wd++) {
+                        u64 T0 = (wd < (int)nc ? S->coeff[wd] : S->aux[wd - nc]) & P->mask;
+                        int il = P->m - 1;
+                        u64 TN = (wd < (int)nc ? S->coeff[(size_t)il * nc + wd] : S->aux[(size_t)il * S->p_aux + (wd - nc)]) & P->mask;
+                        if (a == 0) { acc[wd] -= Av[0] * (T0 - TN); continue; }          /* the term B = A(xhat) */
+                        int ia = plain_interval(S, a), ib = plain_interval(S, a - 1);
+                        u64 Ta = (wd < (int)nc ? S->coeff[(size_t)ia * nc + wd] : S->aux[(size_t)ia * S->p_aux + (wd - nc)]) & P->mask;
+                        u64 Tb = (wd < (int)nc ? S->coeff[(size_t)ib * nc + wd] : S->aux[(size_t)ib * S->p_aux + (wd - nc)]) & P->mask;
+                        acc[wd] += (Tb - Ta) * Av[0];
+                    }
+                }
+                int ix = plain_interval(S, xh);
+                for (int wd = 0; wd < P->p; wd++) {
+                    u64 Tx = (wd < (int)nc ? S->coeff[(size_t)ix * nc + wd] : S->aux[(size_t)ix * S->p_aux + (wd - nc)]) & P->mask;
+                    coeff_out[(size_t)wd * count + e] = (acc[wd] + (party == 0 ? Tx : 0)) & P->mask;
+                }
+                continue;
             }
             for (int wd = 0; wd < P->p && !P->xpoly; wd++) {
                 u64 acc = 0;

@@ -21,8 +21,8 @@ SYMBOLS = (
     "fusefss_compile", "fusefss_destroy", "fusefss_shape", "fusefss_atom", "fusefss_key_bytes", "fusefss_keygen", "fusefss_keygen_parts",
     "fusefss_eval_cmp", "fusefss_eval_lut", "fusefss_eval_fused", "fusefss_eval_fused_both", "fusefss_post", "fusefss_post_rounds", "fusefss_post_msg_bytes",
     "fusefss_online_bits", "fusefss_post_fused", "fusefss_cost", "fusefss_gate_workspace_bytes", "fusefss_gate_host",
-    "fusefss_share_open", "fusefss_sub_bcast", "fusefss_row_sum", "fusefss_mul_triple_bytes", "fusefss_mul_keygen", "fusefss_mul_fused",
-    "fusefss_strerror", "fusefss_last_cuda_error", "fusefss_debug_set", "fusefss_launch_count", "fusefss_aes_probe", "fusefss_aes_kat", "fusefss_pipe_probe",
+    "fusefss_share_open", "fusefss_open_output", "fusefss_sub_bcast", "fusefss_row_sum", "fusefss_mul_triple_bytes", "fusefss_mul_keygen", "fusefss_mul_fused",
+    "fusefss_strerror", "fusefss_last_cuda_error", "fusefss_debug_set", "fusefss_launch_count", "fusefss_aes_probe", "fusefss_aes_kat", "fusefss_pipe_probe", "fusefss_bitslice_kat", "fusefss_bitslice_probe",
 )
 
 
@@ -84,6 +84,7 @@ def _load():
         "fusefss_gate_workspace_bytes": (sz, [vp, sz]),
         "fusefss_gate_host": (i32, [vp, vp, vp, vp, u64, sz, sz, vp, sz, vp, vp, vp, vp, vp]),
         "fusefss_share_open": (i32, [vp, vp, vp, vp, vp, sz, u64, vp, vp]),
+        "fusefss_open_output": (i32, [C.c_uint32, vp, vp, sz, u64, vp, vp]),
         "fusefss_sub_bcast": (i32, [C.c_uint32, vp, vp, sz, sz, vp, vp]),
         "fusefss_row_sum": (i32, [C.c_uint32, vp, sz, sz, vp, vp]),
         "fusefss_mul_triple_bytes": (sz, [sz]),
@@ -96,6 +97,8 @@ def _load():
         "fusefss_aes_probe": (i32, [sz, i32, vp, vp]),
         "fusefss_aes_kat": (i32, [C.c_char_p, C.c_char_p, vp, vp]),
         "fusefss_pipe_probe": (i32, [i32, i32, vp, vp]),
+        "fusefss_bitslice_kat": (i32, [C.c_char_p, vp, vp, vp]),
+        "fusefss_bitslice_probe": (i32, [C.c_char_p, sz, i32, vp, vp]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(L, name)
@@ -316,6 +319,34 @@ def aes_kat(key: bytes, block: bytes) -> bytes:
     out = torch.zeros(16, dtype=torch.uint8, device="cuda")
     _check(lib.fusefss_aes_kat(key, block, _ptr(out), _stream()))
     return bytes(out.cpu().numpy().tobytes())
+
+
+def bitslice_kat(key: bytes, blocks: bytes) -> bytes:
+    """32 blocks (512 bytes) through the bitsliced core; returns the 512 ciphertext bytes"""
+    import torch
+    assert len(blocks) == 512
+    src = torch.frombuffer(bytearray(blocks), dtype=torch.uint8).cuda()
+    out = torch.zeros(512, dtype=torch.uint8, device="cuda")
+    _check(lib.fusefss_bitslice_kat(key, _ptr(src), _ptr(out), _stream()))
+    return bytes(out.cpu().numpy().tobytes())
+
+
+def bitslice_probe(threads: int = 0, iters: int = 24):
+    """GAES/s of the bitsliced core (CUDA events), for bench.py's prg_probe"""
+    import torch
+    sms = torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count
+    threads = threads or sms * 512
+    out = torch.empty(threads * 16, dtype=torch.uint8, device="cuda")
+    key = bytes(range(16))
+    _check(lib.fusefss_bitslice_probe(key, threads, 2, _ptr(out), _stream()))
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    _check(lib.fusefss_bitslice_probe(key, threads, iters, _ptr(out), _stream()))
+    b.record()
+    torch.cuda.synchronize()
+    return {"gaes": threads * 32 * iters / (a.elapsed_time(b) * 1e-3) / 1e9,
+            "what": "fusefss_bitslice_probe: 32 blocks per thread as 128 bit-planes, composite-field S-box circuit (152 XOR + 36 AND per byte), no tables"}
 
 
 def aes_probe(threads: int, iters: int, out=None):

@@ -15,7 +15,13 @@ from . import Program, _check, _ptr, _stream, lib
 STAGES = ("nexp", "tr_e", "recip", "tr_t", "tr_y")
 
 
-def softmax_specs(variant: int = 3, n: int = 64, f: int = 12):
+# gate -> gate edges: the producer is compiled with mask_output and keyed with r_out = the consumer's r_in, so that the opened
+# yhat of the producer IS the consumer's xhat (online step 6; masked-wire invariant P:89-91)
+FUSED_EDGES = {"nexp": "tr_e", "recip": "tr_t"}
+LN_FUSED_EDGES = {"rsqrt": "tr_g"}
+
+
+def softmax_specs(variant: int = 3, n: int = 64, f: int = 12, fused_open: bool = False):
     """Gate types of the block: nExp (out scale 2f+8), arithmetic shifts by 20 / 28 / 24 bits (as shift+ReLU gates:
     every value here is non-negative), Recip (out scale 3f+16).  Scales: e at 32 -> 12; t at 52 -> 24; e*t at 36 -> 12."""
     from workloads import specs as S
@@ -29,6 +35,9 @@ def softmax_specs(variant: int = 3, n: int = 64, f: int = 12):
             s = S.input_masked_mul(s)
         if variant & 4:
             s = S.public_point_horner(s)
+        if fused_open and k in FUSED_EDGES:
+            import dataclasses
+            s = dataclasses.replace(s, mask_output=True)
         out[k] = s
     return out
 
@@ -36,10 +45,11 @@ def softmax_specs(variant: int = 3, n: int = 64, f: int = 12):
 class Softmax:
     """rows x cols block.  `keygen(masks, seed)` is the dealer; `run(x0, x1)` the online phase of both parties."""
 
-    def __init__(self, rows: int, cols: int, variant: int = 3):
+    def __init__(self, rows: int, cols: int, variant: int = 3, fused_open: bool = False):
         import torch
         self.rows, self.cols, self.N = rows, cols, rows * cols
-        self.specs = softmax_specs(variant)
+        self.edges = FUSED_EDGES if fused_open else {}
+        self.specs = softmax_specs(variant, fused_open=fused_open)
         self.progs = {k: Program(s) for k, s in self.specs.items()}
         self.n = 64
         self.counts = {"nexp": self.N, "tr_e": self.N, "recip": rows, "tr_t": rows, "tr_y": self.N}
@@ -57,13 +67,18 @@ class Softmax:
         """masks[stage] = device uint64 tensor of fresh input masks r_in for that gate instance."""
         for i, k in enumerate(STAGES):
             st_seed = seed + (1, 2, 3, 4, 6)[i]
-            self.progs[k].keygen(masks[k], None, st_seed, 0, keys=self.keys[k])
+            r_out = masks[self.edges[k]].reshape(1, -1) if k in self.edges else None     # r_out(k) = r_in(consumer)
+            self.progs[k].keygen(masks[k], r_out, st_seed, 0, keys=self.keys[k])
         _check(lib.fusefss_mul_keygen(self.n, seed + 5, 0, self.N, _ptr(self.triples[0]), _ptr(self.triples[1]), _stream()))
 
     # ---- online ----------------------------------------------------------------------------------
-    def _gate(self, k, x0, x1, offset=0):
+    def _gate(self, k, x0, x1, offset=0, opened=False):
+        """opened: (x0, x1) are the producer's shares of yhat = y + r_out with r_out = this gate's r_in: xhat = their sum"""
         P, (k0, k1), b, c = self.progs[k], self.keys[k], self.buf[k], self.counts[k]
-        _check(lib.fusefss_share_open(P._h, _ptr(k0), _ptr(k1), _ptr(x0), _ptr(x1), c, offset, _ptr(b["xhat"]), _stream()))
+        if opened:
+            _check(lib.fusefss_open_output(self.n, _ptr(x0), _ptr(x1), c, offset, _ptr(b["xhat"]), _stream()))
+        else:
+            _check(lib.fusefss_share_open(P._h, _ptr(k0), _ptr(k1), _ptr(x0), _ptr(x1), c, offset, _ptr(b["xhat"]), _stream()))
         P.eval_fused_both(k0, k1, b["xhat"], b["bits"] if P.shape["T"] else None, b["coeff"] if P.shape["has_lut"] else None)
         y0, y1, _, _ = P.post_fused(k0, k1, b["xhat"], b["bits"][0], b["bits"][1], b["coeff"][0], b["coeff"][1], outs=b["out"])
         return y0[0], y1[0]
@@ -71,11 +86,11 @@ class Softmax:
     def run(self, x0, x1):
         """x0, x1: additive shares [rows*cols] of the max-subtracted scores at scale 2^12.  Returns shares of softmax at 2^12."""
         e0, e1 = self._gate("nexp", x0, x1)
-        f0, f1 = self._gate("tr_e", e0, e1)
+        f0, f1 = self._gate("tr_e", e0, e1, opened="nexp" in self.edges)
         for b, fb in ((0, f0), (1, f1)):
             _check(lib.fusefss_row_sum(self.n, _ptr(fb), self.rows, self.cols, _ptr(self.s[b]), _stream()))
         t0, t1 = self._gate("recip", self.s[0], self.s[1])
-        u0, u1 = self._gate("tr_t", t0, t1)
+        u0, u1 = self._gate("tr_t", t0, t1, opened="recip" in self.edges)
         _check(lib.fusefss_mul_fused(self.n, _ptr(f0), _ptr(f1), _ptr(u0), _ptr(u1), _ptr(self.triples[0]), _ptr(self.triples[1]),
                                      self.N, self.cols, _ptr(self.prod[0]), _ptr(self.prod[1]), _stream()))
         y0, y1 = self._gate("tr_y", self.prod[0], self.prod[1])
@@ -112,15 +127,19 @@ class LayerNorm(Softmax):
     LN_STAGES = ("mean", "var", "rsqrt", "tr_g", "tr_y")
     HALF = 1 << 63
 
-    def __init__(self, rows: int, d: int, variant: int = 3):
+    def __init__(self, rows: int, d: int, variant: int = 3, fused_open: bool = False):
+        import dataclasses
         import torch
         from workloads import specs as S
+        self.edges = LN_FUSED_EDGES if fused_open else {}
         k = d.bit_length() - 1
         if d != 1 << k:
             raise ValueError("LayerNorm block: d must be a power of two (the mean is a truncation gate)")
         self.rows, self.cols, self.N, self.n = rows, d, rows * d, 64
         mk = {"mean": S.ars(64, k), "var": S.ars(64, k + 12), "rsqrt": S.rsqrt(64, 12), "tr_g": S.ars(64, 24), "tr_y": S.ars(64, 24)}
         self.specs = {kk: _apply_variant(s, variant) for kk, s in mk.items()}
+        for kk in self.edges:
+            self.specs[kk] = dataclasses.replace(self.specs[kk], mask_output=True)
         self.progs = {kk: Program(s) for kk, s in self.specs.items()}
         self.counts = {"mean": rows, "var": rows, "rsqrt": rows, "tr_g": rows, "tr_y": self.N}
         self.keys = {kk: self.progs[kk].alloc_keys(c) for kk, c in self.counts.items()}
@@ -138,7 +157,8 @@ class LayerNorm(Softmax):
 
     def keygen(self, masks, seed: int):
         for kk, off in zip(self.LN_STAGES, (1, 3, 4, 5, 7)):
-            self.progs[kk].keygen(masks[kk], None, seed + off, 0, keys=self.keys[kk])
+            r_out = masks[self.edges[kk]].reshape(1, -1) if kk in self.edges else None
+            self.progs[kk].keygen(masks[kk], r_out, seed + off, 0, keys=self.keys[kk])
         _check(lib.fusefss_mul_keygen(self.n, seed + 2, 0, self.N, _ptr(self.triples_sq[0]), _ptr(self.triples_sq[1]), _stream()))
         _check(lib.fusefss_mul_keygen(self.n, seed + 6, 0, self.N, _ptr(self.triples[0]), _ptr(self.triples[1]), _stream()))
 
@@ -156,7 +176,7 @@ class LayerNorm(Softmax):
             _check(lib.fusefss_row_sum(self.n, _ptr(self.sq[b]), self.rows, self.cols, _ptr(self.ssq[b]), st))
         v0, v1 = self._gate("var", self.ssq[0], self.ssq[1], H)
         g0, g1 = self._gate("rsqrt", v0, v1)
-        h0, h1 = self._gate("tr_g", g0, g1, H)
+        h0, h1 = self._gate("tr_g", g0, g1, H, opened="rsqrt" in self.edges)
         _check(lib.fusefss_mul_fused(self.n, _ptr(c0), _ptr(c1), _ptr(h0), _ptr(h1), _ptr(self.triples[0]), _ptr(self.triples[1]),
                                      self.N, self.cols, _ptr(self.prod[0]), _ptr(self.prod[1]), st))
         y0, y1 = self._gate("tr_y", self.prod[0], self.prod[1], H)

@@ -23,7 +23,7 @@ def build(force: bool = False, verbose: bool = False, extra=()) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-shared",
-           "-Xcompiler", "-fPIC,-Wall", "--expt-relaxed-constexpr", "-o", LIB]
+           "-Xcompiler", "-fPIC,-Wall", "--expt-relaxed-constexpr", "-split-compile", "0", "-o", LIB]
     if verbose:
         cmd += ["-Xptxas", "-v"]
     cmd += list(extra) + [os.path.join(_CSRC, s) for s in SOURCES]

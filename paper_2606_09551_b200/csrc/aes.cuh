@@ -130,15 +130,16 @@ __device__ __forceinline__ void aes_last(uint32_t (&s)[4], uint32_t tl, uint32_t
 }
 
 // NI inputs x NK keys (K_KFIRST .. K_{KFIRST+NK-1}) in lock-step: out[i][k] = AES_{K}(x_i) ^ x_i  (the PRG of 4.1).
-// SHARED = true asserts that the NI inputs differ only in byte 0 of word 0 (the tweak of ONE seed).  The PRG keys
+// SHARE = 1 asserts that the NI inputs differ only in byte 0 of word 0 (the tweak of ONE seed).  The PRG keys
 // K_i = (i, 01, .., 0f) differ only in byte 0 too, so after the initial AddRoundKey all NI*NK states agree except
 // in that byte, which feeds a single lookup of round 1 (column 0, T0): the other 15 lookups of round 1 are done
-// once and shared -- 15 + NI*NK lookups instead of 16*NI*NK.
-// UNR = rounds unrolled per loop trip: 1 for the register-hungry kernels (k_gen_vec, k_eval_lut), 3 where it measured
+// once and shared -- 15 + NI*NK lookups instead of 16*NI*NK.  SHARE = 2: the inputs are unrelated seeds (several points
+// walked in lock-step), the NK keys of EACH input share their 15 lookups.  SHARE = 0: nothing is shared.
+// UNR = rounds unrolled per loop trip: 1 for the register-hungry kernels (k_gen_vec, k_eval_p3), 3 where it measured
 // faster (k_eval_sp, k_gen_bit): profiles/r1l_unroll.md.
-template <int NI, int NK, int KFIRST, bool SHARED = false, int UNR = kAesUnroll>
+template <int NI, int NK, int KFIRST, int SHARE = 0, int UNR = kAesUnroll>
 __device__ __forceinline__ void prg_blocks(uint32_t tl, const uint32_t (&x)[NI][4], uint32_t (&out)[NI][NK][4]) {
-    if (SHARED && NI * NK > 1) {
+    if (SHARE == 1 && NI * NK > 1) {
         uint32_t w[4];
 #pragma unroll
         for (int c = 0; c < 4; ++c) w[c] = x[0][c] ^ c_rk[KFIRST][c];
@@ -155,6 +156,24 @@ __device__ __forceinline__ void prg_blocks(uint32_t tl, const uint32_t (&x)[NI][
                 out[i][k][2] = c2 ^ c_rk[KFIRST + k][6];
                 out[i][k][3] = c3 ^ c_rk[KFIRST + k][7];
             }
+    } else if (SHARE == 2 && NK > 1) {
+#pragma unroll
+        for (int i = 0; i < NI; ++i) {
+            uint32_t w[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) w[c] = x[i][c] ^ c_rk[KFIRST][c];
+            const uint32_t c0 = tlu<1, 1>(tl, w[1]) ^ tlu<2, 2>(tl, w[2]) ^ tlu<3, 3>(tl, w[3]);
+            const uint32_t c1 = tlu<0, 0>(tl, w[1]) ^ tlu<1, 1>(tl, w[2]) ^ tlu<2, 2>(tl, w[3]) ^ tlu<3, 3>(tl, w[0]);
+            const uint32_t c2 = tlu<0, 0>(tl, w[2]) ^ tlu<1, 1>(tl, w[3]) ^ tlu<2, 2>(tl, w[0]) ^ tlu<3, 3>(tl, w[1]);
+            const uint32_t c3 = tlu<0, 0>(tl, w[3]) ^ tlu<1, 1>(tl, w[0]) ^ tlu<2, 2>(tl, w[1]) ^ tlu<3, 3>(tl, w[2]);
+#pragma unroll
+            for (int k = 0; k < NK; ++k) {
+                out[i][k][0] = c0 ^ tlu<0, 0>(tl, x[i][0] ^ c_rk[KFIRST + k][0]) ^ c_rk[KFIRST + k][4];
+                out[i][k][1] = c1 ^ c_rk[KFIRST + k][5];
+                out[i][k][2] = c2 ^ c_rk[KFIRST + k][6];
+                out[i][k][3] = c3 ^ c_rk[KFIRST + k][7];
+            }
+        }
     } else {
 #pragma unroll
         for (int i = 0; i < NI; ++i)

@@ -19,6 +19,14 @@ __global__ void k_share_open(const OpenArgs a) {
     a.xhat[e] = (a.x0[e] + r0 + a.x1[e] + r1 + a.offset) & a.mask;      // offset: public constant added to the gate input
 }
 
+// Online step 6: opening of a masked output yhat = y + r_out from the two parties' shares of it (each sends one
+// ring element).  With r_in(next gate) = r_out(this gate) the public yhat IS the next gate's xhat.
+struct OpenOutArgs { const uint64_t *y0, *y1; size_t count; uint64_t mask, offset; uint64_t *yhat; };
+__global__ void k_open_output(const OpenOutArgs a) {
+    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e < a.count) a.yhat[e] = (a.y0[e] + a.y1[e] + a.offset) & a.mask;
+}
+
 // out[r] = sum_c in[r*cols + c] mod 2^n (local on additive shares): one warp per row
 struct RowSumArgs { const uint64_t *in; uint64_t *out; size_t rows, cols; uint64_t mask; };
 __global__ void k_row_sum(const RowSumArgs a) {

@@ -24,7 +24,7 @@ struct EvalSpArgs {
     size_t count, s16, s8, lvl_stride, vt_first, vt_lvl_rel, vt_fin_rel, rpow;
     uint64_t mask;
     int n, m, p, et, T, n_w, n_clusters, G;     // G > 1: the points of an element are dealt round-robin to G warps (small tensors); et: early-terminated bit trees
-    int zero_first, pad1;                       // G > 1: outputs are zeroed in-kernel before the atomics (cooperative launch)
+    int zero_first, np;                         // G > 1: outputs are zeroed in-kernel before the atomics (cooperative launch); np: points per batch
     SpWidth width[kMaxWidths];
     size_t bt_root[kMaxWidths], bt_cw[kMaxWidths], bt_vb[kMaxWidths];
     SpAtomDev atom[kMaxAtoms];
@@ -115,6 +115,69 @@ __device__ __forceinline__ void sp_leaf(uint32_t tl, const SpState<PK> &st, cons
     }
 }
 
+// NP points in lock-step over levels [from, to): every level's correction words are loaded ONCE for the NP points (they walk
+// the same levels of the same element's key), and the NP x (1 + QK) PRG blocks of a level are NP x (1+QK) x 16 independent
+// lookups per round -- the instruction-level parallelism a launch with only a few warps per SM lives on.  The next level's
+// words are prefetched into registers while the current level's AES runs.
+template <int PK, int NPMAX, int NP>
+__device__ __forceinline__ void sp_walk_batch(uint32_t tl, const uint8_t *lvl, size_t e, size_t s16, size_t s8, size_t lvl_stride,
+                                              int from, int to, uint64_t (&ub)[NPMAX], SpState<PK> (&st)[NPMAX]) {
+    constexpr int QK = (PK + 1) / 2;
+    if (from >= to) return;
+    const uint8_t *pl = lvl + (size_t)from * lvl_stride;
+    uint4 cw; uint64_t vcw[PK];
+    sp_load_level<PK>(pl, e, s16, s8, cw, vcw);
+    for (int i = from; i < to; ++i) {
+        pl += lvl_stride;
+        uint4 cw_n = cw; uint64_t vcw_n[PK];
+#pragma unroll
+        for (int w = 0; w < PK; ++w) vcw_n[w] = vcw[w];
+        if (i + 1 < to) sp_load_level<PK>(pl, e, s16, s8, cw_n, vcw_n);
+        uint32_t x[NP][4], o[NP][1 + QK][4], dbit[NP];
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            dbit[q] = (uint32_t)(ub[q] >> 63);
+            ub[q] <<= 1;
+            x[q][0] = st[q].s[0] | dbit[q]; x[q][1] = st[q].s[1]; x[q][2] = st[q].s[2]; x[q][3] = st[q].s[3];
+        }
+        prg_blocks<NP, 1 + QK, 0, 2, 3>(tl, x, o);
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            const uint32_t tm = 0u - st[q].t;
+            const uint64_t tm64 = 0ull - (uint64_t)st[q].t;
+#pragma unroll
+            for (int w = 0; w < PK; ++w)
+                st[q].V[w] += ((uint64_t)o[q][1 + w / 2][2 * (w & 1)] | ((uint64_t)o[q][1 + w / 2][2 * (w & 1) + 1] << 32)) + (vcw[w] & tm64);
+            const uint32_t tnew = (o[q][0][0] & 1u) ^ (st[q].t & (cw.x >> dbit[q]) & 1u);
+            st[q].s[0] = (o[q][0][0] & ~3u) ^ (cw.x & ~3u & tm);
+            st[q].s[1] = o[q][0][1] ^ (cw.y & tm);
+            st[q].s[2] = o[q][0][2] ^ (cw.z & tm);
+            st[q].s[3] = o[q][0][3] ^ (cw.w & tm);
+            st[q].t = tnew;
+        }
+        cw = cw_n;
+#pragma unroll
+        for (int w = 0; w < PK; ++w) vcw[w] = vcw_n[w];
+    }
+}
+
+// the first nb of the NPMAX entries (nb is warp-uniform)
+template <int PK, int NPMAX>
+__device__ __forceinline__ void sp_walk_some(int nb, uint32_t tl, const uint8_t *lvl, size_t e, size_t s16, size_t s8, size_t lvl_stride,
+                                             int from, int to, uint64_t (&ub)[NPMAX], SpState<PK> (&st)[NPMAX]) {
+    if (NPMAX >= 4 && nb == 4) sp_walk_batch<PK, NPMAX, (NPMAX >= 4 ? 4 : 1)>(tl, lvl, e, s16, s8, lvl_stride, from, to, ub, st);
+    else if (NPMAX >= 3 && nb == 3) sp_walk_batch<PK, NPMAX, (NPMAX >= 3 ? 3 : 1)>(tl, lvl, e, s16, s8, lvl_stride, from, to, ub, st);
+    else if (NPMAX >= 2 && nb == 2) sp_walk_batch<PK, NPMAX, (NPMAX >= 2 ? 2 : 1)>(tl, lvl, e, s16, s8, lvl_stride, from, to, ub, st);
+    else sp_walk_batch<PK, NPMAX, 1>(tl, lvl, e, s16, s8, lvl_stride, from, to, ub, st);
+}
+
+#ifndef FFS_SP_NP_BIG
+#define FFS_SP_NP_BIG 1          // points walked in lock-step by the 1024-thread instantiation (64 registers per thread)
+#endif
+#ifndef FFS_SP_NP_SMALL
+#define FFS_SP_NP_SMALL 2        // ... by the 256-thread instantiation (255 registers per thread)
+#endif
+
 template <int P, int PK, int THREADS>
 __global__ void __launch_bounds__(THREADS, 1) k_eval_sp(const __grid_constant__ EvalSpArgs a) {
     extern __shared__ uint32_t sT[];
@@ -190,39 +253,91 @@ __global__ void __launch_bounds__(THREADS, 1) k_eval_sp(const __grid_constant__ 
 #pragma unroll
             for (int t = 0; t < PK; ++t) r0.V[t] = 0;
             const int n = a.n;
+            constexpr int NP = THREADS == kEvalThreadsSmall ? FFS_SP_NP_SMALL : FFS_SP_NP_BIG;
+            const int np = a.np < 1 ? 1 : a.np > NP ? NP : a.np;           // points walked in lock-step (<= NP, the compiled maximum)
+            // is point j needed by the outputs this launch produces?  (warp-uniform)
+            auto needed = [&](int j) {
+                bool need = want_bits && pts[j].bitmask != 0;
+                if (want_coeff) {
+#pragma unroll
+                    for (int w = 0; w < P * PK; ++w) need = need || wts[(size_t)j * P * PK + w] != 0;
+                }
+                return need;
+            };
+            // leaf of a walked point: A_j = share of (1, -r, ..) I[u_j < r]; fold it into the outputs
+            auto fold = [&](int j, const SpState<PK> &st) {
+                uint64_t A[PK];
+                sp_leaf<PK>(tl, st, fin, e, a.s8, party, A);
+                word ^= pts[j].bitmask & (0ull - (A[0] & 1ull));            // component 0 = share of I[u_j < r]
+                if (want_coeff) {
+#pragma unroll
+                    for (int w = 0; w < P; ++w)
+#pragma unroll
+                        for (int t = 0; t < PK; ++t) acc[w] += wts[((size_t)j * P + w) * PK + t] * A[t];
+                }
+            };
+            // (A) clusters of one point: nothing to share; the s-th of them belongs to group s mod G; NP of them walk the whole
+            //     tree in lock-step
+            {
+                int jq[NP], nb = 0, s_idx = 0;
+                auto flush = [&]() {
+                    if (!nb) return;
+                    SpState<PK> st[NP]; uint64_t ub[NP];
+#pragma unroll
+                    for (int q = 0; q < NP; ++q) {
+                        st[q] = r0;
+                        ub[q] = ((xh + pts[jq[q < nb ? q : 0]].delta) & a.mask) << (64 - n);
+                    }
+                    sp_walk_some<PK, NP>(nb, tl, lvl, e, a.s16, a.s8, a.lvl_stride, 0, n, ub, st);
+#pragma unroll
+                    for (int q = 0; q < NP; ++q) if (q < nb) fold(jq[q], st[q]);
+                    nb = 0;
+                };
+                for (int c = 0; c < a.n_clusters; ++c) {
+                    const SpCluster cl = a.cluster[c];
+                    if (cl.count > 1 && n - cl.tail_bits > 0) continue;
+                    for (int j = cl.first; j < cl.first + cl.count; ++j, ++s_idx) {
+                        if (s_idx % a.G != g || !needed(j)) continue;
+#pragma unroll
+                        for (int q = 0; q < NP; ++q) if (q == nb) jq[q] = j;
+                        if (++nb == np) flush();
+                    }
+                }
+                flush();
+            }
+            // (B) clusters that share a prefix: walk it once (two candidates, forked), then the tails of this group's points, NP at a time
             for (int c = 0; c < a.n_clusters; ++c) {
                 const SpCluster cl = a.cluster[c];
                 const int kf = n - cl.tail_bits;                            // shared levels
-                const bool share = cl.count > 1 && kf > 0;
+                if (!(cl.count > 1 && kf > 0)) continue;
+                bool any = false;
+                for (int j = cl.first + g; j < cl.first + cl.count; j += a.G) any = any || needed(j);
+                if (!any) continue;
                 SpState<PK> s1 = r0, s2 = r0;
-                uint64_t pre1 = 0;
-                if (share) {
-                    const uint64_t uf = ((xh + pts[cl.first].delta) & a.mask) << (64 - n);
-                    const uint64_t ul = ((xh + pts[cl.first + cl.count - 1].delta) & a.mask) << (64 - n);
-                    sp_walk_fork<PK>(tl, lvl, e, a.s16, a.s8, a.lvl_stride, kf, uf, ul, s1, s2);
-                    pre1 = uf >> (64 - kf);
-                }
-                for (int j = cl.first + g; j < cl.first + cl.count; j += a.G) {
-                    bool need = want_bits && pts[j].bitmask != 0;
-                    if (want_coeff) {
+                const uint64_t uf = ((xh + pts[cl.first].delta) & a.mask) << (64 - n);
+                const uint64_t ul = ((xh + pts[cl.first + cl.count - 1].delta) & a.mask) << (64 - n);
+                sp_walk_fork<PK>(tl, lvl, e, a.s16, a.s8, a.lvl_stride, kf, uf, ul, s1, s2);
+                const uint64_t pre1 = uf >> (64 - kf);
+                int j = cl.first + g;
+                while (j < cl.first + cl.count) {
+                    int jq[NP], nb = 0;
+                    for (; j < cl.first + cl.count && nb < np; j += a.G) {
+                        if (!needed(j)) continue;
 #pragma unroll
-                        for (int w = 0; w < P * PK; ++w) need = need || wts[(size_t)j * P * PK + w] != 0;
+                        for (int q = 0; q < NP; ++q) if (q == nb) jq[q] = j;
+                        ++nb;
                     }
-                    if (!need) continue;
-                    const uint64_t u = ((xh + pts[j].delta) & a.mask) << (64 - n);
-                    SpState<PK> st = r0;
-                    int from = 0;
-                    if (share) { st = (u >> (64 - kf)) == pre1 ? s1 : s2; from = kf; }
-                    sp_walk<PK>(tl, lvl, e, a.s16, a.s8, a.lvl_stride, from, n, from ? u << from : u, st);
-                    uint64_t A[PK];
-                    sp_leaf<PK>(tl, st, fin, e, a.s8, party, A);
-                    word ^= pts[j].bitmask & (0ull - (A[0] & 1ull));        // component 0 = share of I[u_j < r]
-                    if (want_coeff) {
+                    if (!nb) break;
+                    SpState<PK> st[NP]; uint64_t ub[NP];
 #pragma unroll
-                        for (int w = 0; w < P; ++w)
-#pragma unroll
-                            for (int t = 0; t < PK; ++t) acc[w] += wts[((size_t)j * P + w) * PK + t] * A[t];
+                    for (int q = 0; q < NP; ++q) {
+                        const uint64_t u = ((xh + pts[jq[q < nb ? q : 0]].delta) & a.mask) << (64 - n);
+                        st[q] = (u >> (64 - kf)) == pre1 ? s1 : s2;
+                        ub[q] = u << kf;
                     }
+                    sp_walk_some<PK, NP>(nb, tl, lvl, e, a.s16, a.s8, a.lvl_stride, kf, n, ub, st);
+#pragma unroll
+                    for (int q = 0; q < NP; ++q) if (q < nb) fold(jq[q], st[q]);
                 }
             }
         }

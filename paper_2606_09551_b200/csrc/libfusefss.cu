@@ -18,6 +18,7 @@
 #include "keygen.cuh"
 #include "post.cuh"
 #include "blocks.cuh"
+#include "bitslice.cuh"
 
 namespace fsk {
 namespace {
@@ -27,6 +28,7 @@ std::atomic<uint64_t> g_launches{0};
 thread_local int g_sms = 148;                 // SM count of the calling thread's current device (set by init_device)
 std::atomic<int> g_force_g{0};                // fusefss_debug_set("force_g", v): v >= 1 forces the tree-group count (tests)
 std::atomic<int> g_eval_threads{kEvalThreads};// fusefss_debug_set("eval_threads", v): CTA size of the large eval launches
+std::atomic<int> g_sp_np{0};                  // fusefss_debug_set("sp_np", v): points walked in lock-step by k_eval_sp (0 = automatic)
 std::atomic<int> g_small_regs{1};             // fusefss_debug_set("small_kernels", 0): never pick the 256-thread instantiations
 const HostAes &host_aes() { static HostAes h; return h; }
 
@@ -209,7 +211,7 @@ int launch_eval_p3(const Program &P, int party, const void *const key[2], const 
     const size_t items = units * (size_t)((want_cmp ? a.Gc : 0) + (want_lut ? a.Gl : 0));
     a.zero_first = (want_cmp && a.Gc > 1) || (want_lut && a.Gl > 1);
     const int threads = small ? kEvalThreadsSmall : threads_for(items, cap);
-    const int grid = grid_for(items, threads);
+    const int grid = small ? (int)(items < (size_t)g_sms ? items : (size_t)g_sms) : grid_for(items, threads);   // small: spread the warps over ALL SMs
     const size_t sm = kAesSmemBytes;
     const bool coop = a.zero_first != 0;
 #define FSK_P3_CASE(PP) case PP: return small ? launch(k_eval_p3<PP, kEvalThreadsSmall>, grid, threads, sm, st, a, coop) \
@@ -244,16 +246,37 @@ int launch_eval_sp(const Program &P, int party, const void *const key[2], const 
     const size_t tiles = (count + 31) / 32;
     int maxpts = 1;
     for (int w = 0; w < P.sp.n_w; ++w) if (P.sp.width[w].n_points > maxpts) maxpts = P.sp.width[w].n_points;
-    int G = (int)(((size_t)g_sms * 8 + tiles * a.n_parties - 1) / (tiles * a.n_parties));
-    G = G < 1 ? 1 : G > 8 ? 8 : G;
-    if (G > maxpts) G = maxpts;
+    // Group count for small launches, from a two-term model fitted to profiles/r2f_small_sweep.md: a group's critical path is
+    // chain(G) = sum over clusters (shared prefix + ceil(points / G) tails) levels; up to one warp per SM sub-partition the warps
+    // run at the lone-warp rate, beyond that they share the sub-partition's issue slot and the SM's shared-memory pipe (and every
+    // extra group re-walks the shared prefixes), so time ~ chain(G) * max(1, warps / (4 #SMs)).  Smallest G at the minimum.
+    const size_t units_sp = tiles * (size_t)a.n_parties;
+    int G = 1;
+    if (units_sp < (size_t)g_sms * (kEvalThreads / 32)) {
+        double best = 0;
+        for (int g = 1; g <= maxpts; ++g) {
+            double chain = 0; int singles = 0;
+            for (const SpCluster &cl : P.sp.clusters) {
+                const int kf = (int)P.n - cl.tail_bits;
+                if (cl.count > 1 && kf > 0) chain += kf + (double)((cl.count + g - 1) / g) * cl.tail_bits;
+                else singles += cl.count;
+            }
+            chain += (double)((singles + g - 1) / g) * (double)P.n;
+            for (int w = 0; w < P.sp.n_w; ++w)
+                if (!P.sp.width[w].is_vec) chain += (double)((P.sp.width[w].n_points + g - 1) / g) * bit_tree_levels(P, P.sp.width[w].k);
+            const double load = (double)(units_sp * (size_t)g) / (4.0 * g_sms);
+            const double cost = chain * (load > 1.0 ? load : 1.0);
+            if (g == 1 || cost < best - 1e-9) { best = cost; G = g; }
+        }
+    }
     if (const int f = g_force_g.load()) G = f < maxpts ? f : maxpts;
     a.G = G;
+    a.np = g_sp_np.load() ? g_sp_np.load() : 2;
     a.zero_first = G > 1;
     const size_t items = tiles * (size_t)G * (size_t)a.n_parties;
     const bool small = small_launch(items);
     const int threads = small ? kEvalThreadsSmall : threads_for(items, g_eval_threads.load());
-    const int grid = grid_for(items, threads);
+    const int grid = small ? (int)(items < (size_t)g_sms ? items : (size_t)g_sms) : grid_for(items, threads);   // small: spread the warps over ALL SMs
     const size_t sm = kAesSmemBytes;
     a.rpow = L.rpow;
     const bool coop = a.zero_first != 0;
@@ -415,6 +438,7 @@ int fusefss_debug_set(const char *knob, long value) {
     if (k == "force_g") { g_force_g.store(value >= 1 ? (int)value : 0); return 0; }
     if (k == "eval_threads") { g_eval_threads.store(value >= 32 && value <= kEvalThreads && value % 32 == 0 ? (int)value : kEvalThreads); return 0; }
     if (k == "small_kernels") { g_small_regs.store(value ? 1 : 0); return 0; }
+    if (k == "sp_np") { g_sp_np.store(value >= 1 ? (int)value : 0); return 0; }
     return FUSEFSS_E_DEBUG;
 }
 uint64_t fusefss_launch_count(void) { return g_launches.load(); }
@@ -621,6 +645,16 @@ int fusefss_share_open(const fusefss_program *prog, const void *key0_dev, const 
     return launch(k_share_open, (int)((count + 255) / 256), 256, 0, (cudaStream_t)stream, a);
 }
 
+int fusefss_open_output(uint32_t n_bits, const uint64_t *y0_dev, const uint64_t *y1_dev, size_t count, uint64_t public_offset,
+                        uint64_t *yhat_out_dev, void *stream) {
+    if (!y0_dev || !y1_dev || !yhat_out_dev) return FUSEFSS_E_NULL;
+    if (count == 0) return FUSEFSS_E_COUNT;
+    if (n_bits < 1 || n_bits > 64) return FUSEFSS_E_SPEC;
+    const uint64_t mask = n_bits >= 64 ? ~0ull : ((1ull << n_bits) - 1ull);
+    OpenOutArgs a{y0_dev, y1_dev, count, mask, public_offset & mask, yhat_out_dev};
+    return launch(k_open_output, (int)((count + 255) / 256), 256, 0, (cudaStream_t)stream, a);
+}
+
 int fusefss_row_sum(uint32_t n_bits, const uint64_t *in_dev, size_t rows, size_t cols, uint64_t *out_dev, void *stream) {
     if (!in_dev || !out_dev) return FUSEFSS_E_NULL;
     if (rows == 0 || cols == 0) return FUSEFSS_E_COUNT;
@@ -790,6 +824,35 @@ int fusefss_pipe_probe(int kind, int iters, void *out_dev, void *stream) {
     int rc = init_device(); if (rc) return rc;
     PipeArgs a{(uint32_t *)out_dev, iters, kind};
     return launch(k_pipe_probe, g_sms, kEvalThreads, kAesSmemBytes, (cudaStream_t)stream, a);
+}
+
+// bitsliced AES core (measurement only, DESIGN 5.2): round-key bit masks -> constant memory, then the kernel
+static int bitslice_upload_key(const uint8_t *key, cudaStream_t st) {
+    uint32_t w[44];
+    host_aes().expand(key, w);
+    static thread_local uint32_t masks[11][128];
+    for (int r = 0; r < 11; ++r)
+        for (int b = 0; b < 16; ++b)
+            for (int i = 0; i < 8; ++i) masks[r][8 * b + i] = 0u - ((w[4 * r + b / 4] >> (8 * (b % 4) + i)) & 1u);
+    CU(cudaMemcpyToSymbolAsync(c_bs_rk, masks, sizeof masks, 0, cudaMemcpyHostToDevice, st));
+    CU(cudaStreamSynchronize(st));
+    return 0;
+}
+
+int fusefss_bitslice_kat(const uint8_t *key, const void *in_dev, void *out_dev, void *stream) {
+    if (!key || !in_dev || !out_dev) return FUSEFSS_E_NULL;
+    int rc = init_device(); if (rc) return rc;
+    rc = bitslice_upload_key(key, (cudaStream_t)stream); if (rc) return rc;
+    return launch(k_bitslice_kat, 1, 32, 0, (cudaStream_t)stream, BsKatArgs{(const uint8_t *)in_dev, (uint8_t *)out_dev});
+}
+
+int fusefss_bitslice_probe(const uint8_t *key, size_t threads, int iters, void *out_dev, void *stream) {
+    if (!key || !out_dev) return FUSEFSS_E_NULL;
+    if (threads == 0 || iters <= 0) return FUSEFSS_E_COUNT;
+    int rc = init_device(); if (rc) return rc;
+    rc = bitslice_upload_key(key, (cudaStream_t)stream); if (rc) return rc;
+    const int grid = (int)std::min<size_t>((threads + 255) / 256, (size_t)g_sms * 2);
+    return launch(k_bitslice_probe, grid, 256, 0, (cudaStream_t)stream, BsProbeArgs{(uint4 *)out_dev, threads, iters});
 }
 
 int fusefss_aes_kat(const uint8_t *key, const uint8_t *in, void *out_dev, void *stream) {

@@ -138,3 +138,67 @@ def test_gpu_layernorm_matches_oracle_composition(orc, variant, rows, d):
             assert np.array_equal(host(got[k][b]), exp[k][b]), (k, b)
     pl = oblocks.layernorm_plain(progs, x, rows, d)
     assert np.array_equal(host(got["y"][0]) + host(got["y"][1]), pl["y"])
+
+
+# ---- gate -> gate edges through the opened masked output yhat = y + r_out (online step 6) ----------
+def _fused(specs_by_stage, edges):
+    import dataclasses
+    return {k: (dataclasses.replace(s, mask_output=True) if k in edges else s) for k, s in specs_by_stage.items()}
+
+
+@pytest.mark.parametrize("variant", [0, 3])
+def test_oracle_fused_output_opening(orc, variant):
+    """nExp / Recip compiled with mask_output and keyed with r_out = the next gate's r_in: the opened yhat is that gate's xhat.
+    The pipeline still reconstructs the plaintext one at every stage (the masked stages after removing their public-to-the-
+    dealer mask), and the downstream shares equal the unfused composition's from the truncation gates' outputs on."""
+    from oracle import blocks
+    rows, cols = 3, 20
+    xr, x, x0, x1, masks = _inputs(rows, cols, 9)
+    progs = {k: orc.Program(s) for k, s in _fused(_specs(variant), ("nexp", "recip")).items()}
+    out = blocks.softmax(progs, x0, x1, masks, rows, cols, seed=50, fused_open=True)
+    pl = blocks.softmax_plain({k: orc.Program(s) for k, s in _specs(variant).items()}, x, rows, cols)
+    assert np.array_equal(out["e"][0] + out["e"][1] - masks["tr_e"], pl["e"])         # yhat - r_out = y
+    assert np.array_equal(out["t"][0] + out["t"][1] - masks["tr_t"], pl["t"])
+    for k in ("f", "s", "u", "p", "y"):
+        assert np.array_equal(out[k][0] + out[k][1], pl[k]), k
+    ln = {k: orc.Program(s) for k, s in _fused(_ln_specs(variant, 5), ("rsqrt",)).items()}
+    x, x0, x1, masks = _ln_inputs(4, 32, 6)
+    out = blocks.layernorm(ln, x0, x1, masks, 4, 32, seed=60, fused_open=True)
+    pl = blocks.layernorm_plain({k: orc.Program(s) for k, s in _ln_specs(variant, 5).items()}, x, 4, 32)
+    assert np.array_equal(out["g"][0] + out["g"][1] - masks["tr_g"], pl["g"])
+    for k in ("m", "c", "q", "v", "h", "p", "y"):
+        assert np.array_equal(out[k][0] + out[k][1], pl[k]), k
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("variant", [0, 3])
+def test_gpu_fused_output_opening(orc, variant):
+    import torch
+    import __graft_entry__ as g
+    g.build()
+    from oracle import blocks as oblocks
+    from paper_2606_09551_b200 import blocks as gblocks
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.int64)).cuda()
+    host = lambda t: t.cpu().numpy().view(np.uint64).reshape(-1)
+    rows, cols = 5, 40
+    xr, x, x0, x1, masks = _inputs(rows, cols, 12)
+    progs = {k: orc.Program(s) for k, s in _fused(_specs(variant), ("nexp", "recip")).items()}
+    exp = oblocks.softmax(progs, x0, x1, masks, rows, cols, seed=41, fused_open=True)
+    B = gblocks.Softmax(rows, cols, variant, fused_open=True)
+    B.keygen({k: dev(v) for k, v in masks.items()}, seed=41)
+    got = B.run(dev(x0), dev(x1))
+    torch.cuda.synchronize()
+    for k in ("e", "f", "s", "t", "u", "p", "y"):
+        for b in (0, 1):
+            assert np.array_equal(host(got[k][b]), exp[k][b]), (k, b)
+    rows, d = 3, 64
+    x, x0, x1, masks = _ln_inputs(rows, d, 13)
+    progs = {k: orc.Program(s) for k, s in _fused(_ln_specs(variant, 6), ("rsqrt",)).items()}
+    exp = oblocks.layernorm(progs, x0, x1, masks, rows, d, seed=22, fused_open=True)
+    B = gblocks.LayerNorm(rows, d, variant, fused_open=True)
+    B.keygen({k: dev(v) for k, v in masks.items()}, seed=22)
+    got = B.run(dev(x0), dev(x1))
+    torch.cuda.synchronize()
+    for k in ("m", "c", "q", "v", "g", "h", "p", "y"):
+        for b in (0, 1):
+            assert np.array_equal(host(got[k][b]), exp[k][b]), (k, b)

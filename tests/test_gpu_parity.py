@@ -101,6 +101,19 @@ def test_aes_core_fips197(F):
     assert n >= 2
 
 
+def test_bitsliced_aes_matches_fips197_and_the_table_core(F):
+    """The bitsliced core (timed against the T-table core, DESIGN 5.2): block 0 = the FIPS-197 vector, the other 31 blocks
+    against the device T-table core, which the test above pins to the standard."""
+    path = os.path.join(os.path.dirname(__file__), "golden", "fips197_aes128.txt")
+    key, pt, ct = [bytes.fromhex(v) for v in [l for l in open(path) if l.strip() and not l.startswith("#")][0].split()]
+    rng = np.random.default_rng(3)
+    blocks = [pt] + [bytes(rng.integers(0, 256, 16, dtype=np.uint8)) for _ in range(31)]
+    out = F.bitslice_kat(key, b"".join(blocks))
+    assert out[:16] == ct
+    for k in (1, 2, 17, 31):
+        assert out[16 * k:16 * k + 16] == F.aes_kat(key, blocks[k])
+
+
 SMALL = [lambda: specs.relu(8, 4), lambda: specs.toy(8, 3), lambda: specs.toy(8, 3, True), specs.plain_default,
          specs.single_interval, specs.no_bits, specs.full_partition, lambda: specs.shift_relu(8, 3),
          lambda: specs.toy(12, 4), lambda: specs.relu(12, 6), lambda: specs.ars(8, 3), lambda: specs.ars(12, 5)]

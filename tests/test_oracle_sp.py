@@ -80,8 +80,9 @@ def test_sp_share_is_not_the_value(orc):
 
 
 # ---- variant bit 1: input-masked products ------------------------------------------
-XM = [lambda: specs.relu(8, 4), lambda: specs.toy(8, 3), lambda: specs.toy(8, 3, True), lambda: specs.plain_default(8, 3),
-      lambda: specs.no_bits(8, 3), lambda: specs.shift_relu(8, 3)]
+_slow = lambda mk: pytest.param(mk, marks=pytest.mark.slow)
+XM = [_slow(lambda: specs.relu(8, 4)), lambda: specs.toy(8, 3), _slow(lambda: specs.toy(8, 3, True)), _slow(lambda: specs.plain_default(8, 3)),
+      _slow(lambda: specs.no_bits(8, 3)), lambda: specs.shift_relu(8, 3)]
 
 
 @pytest.mark.parametrize("sp", [0, 1])
@@ -102,7 +103,7 @@ def test_xmul_online_bytes(orc):
 
 
 # ---- variant bit 2: payload = coefficients of P_i(X - r_in), Horner in the public xhat -------
-XP = [lambda: specs.toy(8, 3), lambda: specs.toy(8, 3, True), lambda: specs.plain_default(8, 3), lambda: specs.no_bits(8, 3)]
+XP = [lambda: specs.toy(8, 3), _slow(lambda: specs.toy(8, 3, True)), lambda: specs.plain_default(8, 3), _slow(lambda: specs.no_bits(8, 3))]
 
 
 @pytest.mark.parametrize("sp", [0, 1])
@@ -112,7 +113,7 @@ def test_xpoly_reconstruct_exhaustive_n8(orc, mk, sp):
     check_all_r(orc, spec, range(1 << spec.n), seed=17)      # the lookup returns shifted coefficients: only atoms + outputs are pinned
 
 
-@pytest.mark.parametrize("variant", [2, 3, 4, 5])
+@pytest.mark.parametrize("variant", [pytest.param(2, marks=pytest.mark.slow), 3, pytest.param(4, marks=pytest.mark.slow), 5])
 def test_variant_bits_n12(orc, variant):
     """variant bits 1 / 2 at n = 12: every x for the corner masks, every r for the corner inputs."""
     spec = specs.toy(12, 4)
@@ -129,7 +130,7 @@ def test_variant_bits_n12(orc, variant):
 
 
 # ---- variant bit 3: early-terminated bit trees ------------------------------------------------
-ET = [lambda: specs.relu(8, 4), lambda: specs.toy(8, 3), lambda: specs.toy(8, 3, True), lambda: specs.plain_default(8, 3),
+ET = [_slow(lambda: specs.relu(8, 4)), lambda: specs.toy(8, 3), _slow(lambda: specs.toy(8, 3, True)), _slow(lambda: specs.plain_default(8, 3)),
       lambda: specs.single_interval(8, 3), lambda: specs.shift_relu(8, 3)]
 
 
@@ -142,7 +143,7 @@ def test_early_termination_reconstruct_exhaustive_n8(orc, mk, sp):
     check_all_r(orc, spec, range(1 << spec.n), seed=23)
 
 
-@pytest.mark.parametrize("variant", [8, 9, 15])
+@pytest.mark.parametrize("variant", [8, pytest.param(9, marks=pytest.mark.slow), 15])
 def test_early_termination_n12(orc, variant):
     spec = specs.toy(12, 4)
     if variant & 1:
@@ -171,6 +172,38 @@ def test_early_termination_key_size(orc):
         else:
             saved = sum(16 * (k - max(k - 7, 0) - 1) for k in P0.shape["k"])
         assert P0.key_bytes(c) - P1.key_bytes(c) == saved * c
+
+
+# ---- variant bit 4: dense-table ("DPF-LUT") lookup by full-domain evaluation ------------------------
+DENSE = [lambda: specs.relu(8, 4), _slow(lambda: specs.toy(8, 3)), _slow(lambda: specs.plain_default(8, 3)), _slow(lambda: specs.no_bits(8, 3)),
+         _slow(lambda: specs.shift_relu(8, 3)), lambda: specs.full_partition(3)]
+
+
+@pytest.mark.parametrize("mk", DENSE)
+def test_dense_table_reconstruct_exhaustive_n8(orc, mk):
+    """Every x and every r at n = 8: the lookup evaluated on all 2^n points of the single key reconstructs the active interval's
+    payload, the atoms and the gate outputs their plain definitions."""
+    spec = specs.dense_table(mk())
+    check_all_r(orc, spec, range(1 << spec.n), seed=37)
+
+
+def test_dense_table_n12_and_shape(orc):
+    spec = specs.dense_table(specs.toy(12, 4))
+    N = 1 << spec.n
+    rs = corner_masks(spec, extra=2, seed=3)
+    xs = corner_inputs(spec, extra=2, seed=3)
+    rng = np.random.default_rng(3)
+    x = np.array([xs[i % len(xs)] for i in range(96)], dtype=np.uint64)
+    r = np.array([rs[(i * 7) % len(rs)] for i in range(96)], dtype=np.uint64)
+    x[64:], r[64:] = rng.integers(0, N, 32, dtype=np.uint64), rng.integers(0, N, 32, dtype=np.uint64)
+    P = check_pairs(orc, spec, x, r, seed=41, chunk=12)
+    P1 = orc.Program(specs.shared_prefix(specs.toy(12, 4)))
+    assert P.key_bytes(4096) == P1.key_bytes(4096) and P.shape == P1.shape         # the same single key; only the evaluation differs
+    with pytest.raises(ValueError):
+        orc.Program(specs.dense_table(specs.gelu()))                                # n = 64: no dense table
+    import dataclasses
+    with pytest.raises(ValueError):
+        orc.Program(dataclasses.replace(specs.toy(8, 3), variant=16))               # needs the single-key construction
 
 
 def test_xpoly_shape(orc):

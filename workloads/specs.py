@@ -378,6 +378,13 @@ def early_termination(spec):
     return dataclasses.replace(spec, variant=spec.variant | 8, name=spec.name + "_et")
 
 
+def dense_table(spec):
+    """Variant bits 0 + 4: the interval lookup in the dense-table ("DPF-LUT") representation -- the single key
+    f_{r,1} evaluated on the whole domain of 2^n points (n <= 16); cost and shape depend on n only."""
+    import dataclasses
+    return dataclasses.replace(spec, variant=spec.variant | 17, name=spec.name + "_dense")
+
+
 CONFIGS = {
     "relu16": lambda: relu(16, 8),
     "gelu": gelu,
