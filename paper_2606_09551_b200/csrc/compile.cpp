@@ -514,6 +514,8 @@ int compile_program(const fusefss_spec *S, Program **out) {
     P.xmul = (S->variant >> 1) & 1;
     P.xpoly = ((S->variant >> 2) & 1) && S->d >= 1 && S->m > 1;
     P.et = (S->variant >> 3) & 1;
+    P.dense = (S->variant >> 4) & 1;
+    if (P.dense && (!P.variant || P.xpoly || S->n > 16)) { delete holder; return FUSEFSS_E_SPEC; }   // needs the single key, n <= 16
     if (P.xpoly && S->d > 2) { delete holder; return FUSEFSS_E_SPEC; }          // kernels are instantiated for d <= 2
     if (P.variant) P.M = (int)S->m;               // variant 1: no translated partition, no wrap / dummy split
     P.n_out_a = (int)S->n_out_a; P.n_out_b = (int)S->n_out_b;
@@ -525,6 +527,19 @@ int compile_program(const fusefss_spec *S, Program **out) {
     }
     Lowering low(P);
     if (!low.run()) { delete holder; return FUSEFSS_E_SPEC; }
+    if (P.dense && P.has_lut) {                  // the operator as a table of 2^n entries and its cyclic differences (DESIGN 14)
+        const size_t N = (size_t)1 << P.n, pp = (size_t)P.p;
+        P.sp.dense_t.resize(N * pp);
+        P.sp.dense_d.resize(N * pp);
+        size_t i = 0;
+        for (size_t u = 0; u < N; ++u) {
+            while (i + 1 < P.m && u >= P.alpha[i]) ++i;
+            for (size_t w = 0; w < pp; ++w) P.sp.dense_t[u * pp + w] = P.payload[i * pp + w];
+        }
+        for (size_t a = 0; a < N; ++a)
+            for (size_t w = 0; w < pp; ++w)
+                P.sp.dense_d[a * pp + w] = (P.sp.dense_t[((a + N - 1) % N) * pp + w] - P.sp.dense_t[a * pp + w]) & P.mask;
+    }
     {   // layout of the small device tables (uploaded per device on first use)
         auto up = [](size_t x) { return (x + 255) & ~(size_t)255; };
         P.dev_ins_off = 0;
@@ -534,7 +549,9 @@ int compile_program(const fusefss_spec *S, Program **out) {
         P.dev_sp_weights_off = P.dev_sp_points_off + up(P.sp.points.size() * sizeof(SpPoint) + 8);
         P.dev_sp_delta_off = P.dev_sp_weights_off + up(P.sp.weights.size() * 8 + 8);
         P.dev_sp_clusters_off = P.dev_sp_delta_off + up(P.sp.delta_tab.size() * 8 + 8);
-        P.dev_blob_bytes = P.dev_sp_clusters_off + up(P.sp.clusters.size() * sizeof(SpCluster) + 8);
+        P.dev_dense_t_off = P.dev_sp_clusters_off + up(P.sp.clusters.size() * sizeof(SpCluster) + 8);
+        P.dev_dense_d_off = P.dev_dense_t_off + up(P.sp.dense_t.size() * 8 + 8);
+        P.dev_blob_bytes = P.dev_dense_d_off + up(P.sp.dense_d.size() * 8 + 8);
     }
     *out = &holder->impl;
     return FUSEFSS_OK;

@@ -359,4 +359,72 @@ __global__ void __launch_bounds__(THREADS, 1) k_eval_sp(const __grid_constant__ 
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------------------
+// Variant bit 4 (DESIGN 14; "the dense table bit-width k (DPF-LUT representation)"): the interval lookup with the
+// operator as a dense table of 2^n entries.  The single key f_{r,1} is evaluated on the WHOLE domain -- a traversal of its GGM
+// tree that shares every prefix -- and  share_b = [b=0] T[xhat] + sum_v D[(xhat - v) mod N] A_b(v),  D[a] = T[a-1] - T[a],
+// A_b(v) = Eval_b(key, v).  One warp per (party, element): lane l owns the subtree under the top min(5, n) bits = l, walks it
+// depth-first (a node is expanded once: 2 (2^(n+1) - 2) + 2^n PRG blocks per element per party), and the 32 partial sums are
+// combined with shuffles.  Work and shape depend on n only.
+struct EvalDenseArgs {
+    const uint8_t *key2[2]; const uint64_t *xhat; uint64_t *coeff_out2[2];
+    const uint64_t *dense_t, *dense_d;
+    size_t count, s16, s8, lvl_stride, vt_first, vt_lvl_rel, vt_fin_rel;
+    uint64_t mask;
+    int n, n_parties, party0, pad;
+};
+
+template <int P>
+__global__ void __launch_bounds__(kEvalThreadsSmall, 1) k_eval_dense(const __grid_constant__ EvalDenseArgs a) {
+    extern __shared__ uint32_t sT[];
+    const uint32_t tl = aes_fill_tables(sT);
+    const int lane = threadIdx.x & 31, n = a.n;
+    const int top = n < 5 ? n : 5, m = n - top;
+    const size_t items = a.count * (size_t)a.n_parties, warps = (size_t)gridDim.x * (blockDim.x >> 5);
+    for (size_t item = (size_t)(threadIdx.x >> 5) * gridDim.x + blockIdx.x; item < items; item += warps) {
+        const int slot = (int)(item / a.count);
+        const size_t e = item - (size_t)slot * a.count;
+        const int party = a.n_parties == 2 ? slot : a.party0;
+        const uint8_t *tree = a.key2[slot] + a.vt_first, *lvl = tree + a.vt_lvl_rel, *fin = tree + a.vt_fin_rel;
+        const uint64_t xh = a.xhat[e] & a.mask;
+        const bool active = lane < (1 << top);
+        const uint32_t sub = active ? (uint32_t)lane : 0u;                 // idle lanes (n < 5) shadow lane 0 and contribute nothing
+        const uint4 root = __ldg(reinterpret_cast<const uint4 *>(tree + e * 16));
+        SpState<1> stack[12];                                              // stack[l] = the node after top + l levels (m <= 11)
+        stack[0].s[0] = root.x & ~3u; stack[0].s[1] = root.y; stack[0].s[2] = root.z; stack[0].s[3] = root.w;
+        stack[0].t = (uint32_t)party; stack[0].V[0] = 0;
+        for (int i = 0; i < top; ++i) {                                    // this lane's path through the top levels
+            uint4 cw; uint64_t vcw[1];
+            sp_load_level<1>(lvl + (size_t)i * a.lvl_stride, e, a.s16, a.s8, cw, vcw);
+            sp_step<1>(tl, cw, vcw, (sub >> (top - 1 - i)) & 1u, stack[0]);
+        }
+        uint64_t acc[P];
+#pragma unroll
+        for (int w = 0; w < P; ++w) acc[w] = 0;
+        for (uint32_t j = 0; j < (1u << m); ++j) {                        // leaves of the subtree, left to right
+            const int L = j == 0 ? 0 : m - 1 - (__ffs((int)j) - 1);       // first level whose node changes: the bit that flipped to 1
+            for (int l = L; l < m; ++l) {
+                uint4 cw; uint64_t vcw[1];
+                sp_load_level<1>(lvl + (size_t)(top + l) * a.lvl_stride, e, a.s16, a.s8, cw, vcw);
+                SpState<1> st = stack[l];
+                sp_step<1>(tl, cw, vcw, (j >> (m - 1 - l)) & 1u, st);
+                stack[l + 1] = st;
+            }
+            uint64_t A[1];
+            sp_leaf<1>(tl, stack[m], fin, e, a.s8, party, A);
+            const uint64_t v = ((uint64_t)sub << m) | j;
+            const uint64_t *d = a.dense_d + (size_t)((xh - v) & a.mask) * P;
+#pragma unroll
+            for (int w = 0; w < P; ++w) acc[w] += __ldg(d + w) * A[0];
+        }
+#pragma unroll
+        for (int w = 0; w < P; ++w) {
+            uint64_t s = active ? acc[w] : 0ull;
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+            if (lane == 0) a.coeff_out2[slot][(size_t)w * a.count + e] = (s + (party == 0 ? __ldg(a.dense_t + (size_t)xh * P + w) : 0ull)) & a.mask;
+        }
+    }
+}
+
 }  // namespace fsk

@@ -123,6 +123,8 @@ int ensure_blob(const Program &P, const uint8_t **out) {
     if (!P.sp.weights.empty()) std::memcpy(h.data() + P.dev_sp_weights_off, P.sp.weights.data(), P.sp.weights.size() * 8);
     if (!P.sp.delta_tab.empty()) std::memcpy(h.data() + P.dev_sp_delta_off, P.sp.delta_tab.data(), P.sp.delta_tab.size() * 8);
     if (!P.sp.clusters.empty()) std::memcpy(h.data() + P.dev_sp_clusters_off, P.sp.clusters.data(), P.sp.clusters.size() * sizeof(SpCluster));
+    if (!P.sp.dense_t.empty()) std::memcpy(h.data() + P.dev_dense_t_off, P.sp.dense_t.data(), P.sp.dense_t.size() * 8);
+    if (!P.sp.dense_d.empty()) std::memcpy(h.data() + P.dev_dense_d_off, P.sp.dense_d.data(), P.sp.dense_d.size() * 8);
     cudaError_t e = cudaMemcpy(d, h.data(), P.dev_blob_bytes, cudaMemcpyHostToDevice);
     if (e != cudaSuccess) { cudaFree(d); return cuda_fail(e, "cudaMemcpy(program tables)"); }
     P.dev_blobs[dev] = d;
@@ -290,12 +292,40 @@ int launch_eval_sp(const Program &P, int party, const void *const key[2], const 
     return FUSEFSS_E_SPEC;
 }
 
+// variant bit 4: the lookup by full-domain evaluation of the single key (the predicate bits still come from k_eval_sp's points)
+int launch_eval_dense(const Program &P, int party, const void *const key[2], const uint64_t *xhat, size_t count,
+                      uint64_t *const coeff[2], cudaStream_t st) {
+    const uint8_t *blob = nullptr;
+    int rc = ensure_blob(P, &blob); if (rc) return rc;
+    Layout L; compute_layout(P, count, &L);
+    EvalDenseArgs a{};
+    a.n_parties = party == 2 ? 2 : 1; a.party0 = party == 2 ? 0 : party; a.xhat = xhat;
+    for (int sl = 0; sl < a.n_parties; ++sl) { a.key2[sl] = (const uint8_t *)key[sl]; a.coeff_out2[sl] = coeff[sl]; }
+    a.dense_t = (const uint64_t *)(blob + P.dev_dense_t_off); a.dense_d = (const uint64_t *)(blob + P.dev_dense_d_off);
+    a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.lvl_stride = L.lvl_stride; a.vt_first = L.vt_first;
+    a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel; a.mask = P.mask; a.n = (int)P.n;
+    const size_t items = count * (size_t)a.n_parties;
+    const int grid = (int)(items < (size_t)g_sms ? items : (size_t)g_sms);
+    switch (P.p) {
+#define FSK_DN_CASE(PP) case PP: return launch(k_eval_dense<PP>, grid, kEvalThreadsSmall, kAesSmemBytes, st, a);
+    FSK_DN_CASE(1) FSK_DN_CASE(2) FSK_DN_CASE(3) FSK_DN_CASE(4) FSK_DN_CASE(5) FSK_DN_CASE(6) FSK_DN_CASE(7) FSK_DN_CASE(8)
+#undef FSK_DN_CASE
+    }
+    return FUSEFSS_E_SPEC;
+}
+
 // all four evaluation entry points end here
 int launch_eval(const Program &P, int party, const void *k0, const void *k1, const uint64_t *xhat, size_t count,
                 uint64_t *b0, uint64_t *b1, uint64_t *c0, uint64_t *c1, cudaStream_t st) {
     const void *const key[2] = {k0, k1};
     uint64_t *const bits[2] = {b0, b1};
     uint64_t *const coeff[2] = {c0, c1};
+    if (P.dense && P.has_lut) {                     // bits from the point walks, coefficients from the full-domain traversal
+        uint64_t *const none[2] = {nullptr, nullptr};
+        const bool want_bits = P.T > 0 && (b0 || b1), want_coeff = c0 || c1;
+        if (want_bits) { int rc = launch_eval_sp(P, party, key, xhat, count, bits, none, st); if (rc) return rc; }
+        return want_coeff ? launch_eval_dense(P, party, key, xhat, count, coeff, st) : 0;
+    }
     return P.variant ? launch_eval_sp(P, party, key, xhat, count, bits, coeff, st) : launch_eval_p3(P, party, key, xhat, count, bits, coeff, st);
 }
 
@@ -398,7 +428,12 @@ int fusefss_cost(const fusefss_program *prog, fusefss_cost_t *out) {
                 c.eval_cmp_key_bytes += 16 * ((uint64_t)bit_tree_arrays(*P, W.k) + 1) + 8;
                 continue;
             }
+            if (P->dense && P->has_lut) {                                       // full-domain traversal: every node expanded once
+                const uint64_t N = 1ull << n;
+                c.eval_lut_aes += 2 * (2 * N - 2) + N; c.eval_lut_lookups += (2 * N - 2) * grp(2) + 160 * N;
+            }
             for (const SpCluster &cl : P->sp.clusters) {                       // fused walk: every point of the n-bit tree
+                if (P->dense && P->has_lut) break;
                 const uint64_t kf = n - (uint64_t)cl.tail_bits;
                 const bool share = cl.count > 1 && kf > 0;
                 // the shared prefix is counted once: the few levels re-walked where the cluster's second prefix forks

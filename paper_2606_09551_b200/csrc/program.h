@@ -66,6 +66,9 @@ struct SpProgram {
     std::vector<uint64_t> weights;      // [n_points_total][p][pk]: coefficient share w += weights[j][w][t] * A_j[t]
     std::vector<uint64_t> delta_tab;    // [m][p][pk]: row i >= 1 = w_{i-1} - w_i, row 0 = w_{m-1} (times the share of (-r)^t)
     std::vector<SpCluster> clusters;    // of the n-bit tree
+    // variant bit 4 (DESIGN 14): the operator as a dense table of 2^n entries, T[u][w] = payload word w of the interval that
+    // contains u, and its cyclic differences D[a][w] = T[(a-1) mod N][w] - T[a][w]
+    std::vector<uint64_t> dense_t, dense_d;
     int atom_w[kMaxAtoms], atom_ib[kMaxAtoms], atom_ia[kMaxAtoms], alpha_atom[kMaxIntervals];
 };
 
@@ -90,6 +93,7 @@ struct Program {
     // variant bit 1 (DESIGN 10): a product with the gate input x opens one ring element and needs (b, c = b r_in)
     uint32_t xmul = 0;
     uint32_t xpoly = 0;                   // variant bit 2 (DESIGN 11): Horner in the public xhat, zero Beaver rounds for the spline
+    uint32_t dense = 0;                   // variant bit 4 (DESIGN 14): dense-table lookup by full-domain evaluation of the single key
     uint32_t et = 0;                      // variant bit 3 (DESIGN 13): bit trees stop max(k-7,0) levels deep, 128-bit leaf block
     int round_arr[kMaxRounds] = {0};      // ring-element arrays opened per round: 2 per Beaver, 1 per x-product
     int ma_is_x[64] = {0}, ma_word[65] = {0};
@@ -101,6 +105,7 @@ struct Program {
     mutable std::map<int, void *> dev_blobs;
     size_t dev_ins_off = 0, dev_alpha_off = 0, dev_payload_off = 0, dev_blob_bytes = 0;
     size_t dev_sp_points_off = 0, dev_sp_weights_off = 0, dev_sp_delta_off = 0, dev_sp_clusters_off = 0;
+    size_t dev_dense_t_off = 0, dev_dense_d_off = 0;
 };
 
 // 16-byte correction arrays of a bit tree on k input bits: k levels, or max(k-7,0) levels + the leaf block (DESIGN 13)

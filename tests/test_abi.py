@@ -38,6 +38,7 @@ ALL = [("relu16", lambda: specs.relu(16, 8)), ("gelu", specs.gelu), ("nexp", spe
 ALL = ALL + [(nm + "_sp", (lambda mk=mk: specs.shared_prefix(mk()))) for nm, mk in ALL]      # variant 1 (DESIGN 9)
 ALL = ALL + [(nm + "_xm", (lambda mk=mk: specs.input_masked_mul(mk()))) for nm, mk in ALL]  # variant bit 1 (DESIGN 10)
 ALL = ALL + [(nm + "_xp", (lambda mk=mk: specs.public_point_horner(mk()))) for nm, mk in ALL[:32]]  # variant bit 2 (DESIGN 11)
+ALL = ALL + [(nm + "_dense", (lambda mk=mk: specs.dense_table(mk()))) for nm, mk in ALL[:16] if nm in ("relu16", "toy", "toy_masked", "plain", "nobits", "full", "shift_relu8", "ars8")]  # variant bit 4 (DESIGN 14)
 ALL = ALL + [(nm + "_et", (lambda mk=mk: specs.early_termination(mk()))) for nm, mk in ALL[:32] + ALL[-4:]]  # variant bit 3 (DESIGN 13)
 
 
@@ -98,6 +99,8 @@ def test_rejects_ill_formed_specs(F):
         with pytest.raises(F.FuseFSSError):
             F.Program(s)
             pytest.fail("accepted: " + why)
+    with pytest.raises(F.FuseFSSError):
+        F.Program(specs.dense_table(specs.gelu()))             # dense table: n <= 16 only
     assert F.Program(good).shape["T"] == 2
     assert F.lib.fusefss_key_bytes(None, 10) == 0
     assert F.lib.fusefss_strerror(-3) == b"party must be 0 or 1"

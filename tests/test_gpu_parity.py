@@ -131,6 +131,10 @@ SMALL_XP = [(lambda mk=mk: specs.public_point_horner(mk())) for mk in SMALL[1:4]
 SMALL_ET = [(lambda mk=mk: specs.early_termination(mk())) for mk in SMALL[:5] + SMALL[7:] + SMALL_SP[:5] + SMALL_SP[7:] + SMALL_XM[:2] + SMALL_XP[-2:]]
 
 
+SMALL_DENSE = [(lambda mk=mk: specs.dense_table(mk())) for mk in SMALL[:4] + SMALL[5:9]] + \
+              [lambda: specs.early_termination(specs.dense_table(specs.shift_relu(8, 3))), lambda: specs.input_masked_mul(specs.dense_table(specs.toy(8, 3)))]
+
+
 @pytest.fixture
 def knobs(F):
     """fusefss_debug_set knobs, restored after the test"""
@@ -141,7 +145,7 @@ def knobs(F):
     F.debug_set("force_g", 0); F.debug_set("small_kernels", 1); F.debug_set("eval_threads", 1024)
 
 
-@pytest.mark.parametrize("mk", SMALL + SMALL_SP + SMALL_XM + SMALL_XP + SMALL_ET)
+@pytest.mark.parametrize("mk", SMALL + SMALL_SP + SMALL_XM + SMALL_XP + SMALL_ET + SMALL_DENSE)
 @pytest.mark.parametrize("mode", ["auto", "g1", "g2_big"])
 def test_small_rings_all_masks(F, orc, mk, mode, knobs):
     """Every mask r (both Protocol 3 branches, incl. beta_0 = 0 and the dummy split) at n <= 8; a ragged count.
@@ -190,6 +194,16 @@ def test_config_parity(F, orc, name, count, variant):
         spec = specs.early_termination(spec)                # bit trees cut 7 levels early (DESIGN 13)
     inp = tensors.inputs(name, spec, count=count, seed=0)
     _parity(F, orc, spec, inp["x"], inp["r_in"], inp["r_out"], seed=0)
+
+
+def test_dense_table_relu16(F, orc):
+    """config 1 (ReLU, n = 16) in the dense-table representation: 65,536-point full-domain evaluation per element and party; the
+    oracle walks every point from the root, so a few dozen elements (a tile, a ragged tail, both parties in one launch)."""
+    spec = specs.dense_table(specs.relu(16, 8))
+    inp = tensors.inputs("relu16", spec, count=41, seed=4)
+    inp["x"][:4] = np.array([0, 1 << 15, (1 << 15) - 1, (1 << 16) - 1], dtype=np.uint64)
+    inp["r_in"][4:8] = np.array([0, 1, (1 << 16) - 1, 1 << 15], dtype=np.uint64)
+    _parity(F, orc, spec, inp["x"], inp["r_in"], inp["r_out"], seed=3)
 
 
 @pytest.mark.parametrize("variant", [0, 1])
