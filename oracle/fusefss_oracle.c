@@ -504,7 +504,8 @@ enum {
     PHI_A_CONST = 1, PHI_A_X, PHI_A_Y, PHI_A_KAPPA, PHI_A_XHAT_SHR, PHI_A_ADD, PHI_A_SUB, PHI_A_MULC,
     PHI_A_MUL, PHI_A_B2A, PHI_A_OUT, PHI_A_AUX,
     PHI_B_CONST = 32, PHI_B_Z, PHI_B_KAPPA, PHI_B_XHAT, PHI_B_NOT, PHI_B_XOR, PHI_B_AND, PHI_B_OR,
-    PHI_B_ANDPUB, PHI_B_OUT
+    PHI_B_ANDPUB, PHI_B_OUT,
+    PHI_B_A2B     /* B[dst] = bit b of the ring element A[a]  (A2B: [x] -> <b>; reading DESIGN 15) */
 };
 typedef struct { u8 op, dst, a, b; u32 pad; u64 imm; } orc_phi_op;
 
@@ -615,6 +616,7 @@ void orc_plain_G(const orc_spec *S, u64 x, u64 r, u64 *yo, u8 *zo)
         case PHI_B_OR: B[o->dst] = B[o->a] | B[o->b]; break;
         case PHI_B_ANDPUB: B[o->dst] = B[o->a] & (u8)(((xhat >> o->b) & 1) ^ (o->imm & 1)); break;
         case PHI_B_OUT: zo[o->dst] = B[o->a]; break;
+        case PHI_B_A2B: B[o->dst] = (u8)((A[o->a] >> o->b) & 1); break;
         }
     }
 }
@@ -629,7 +631,9 @@ enum {
     C_B_CONST = 1, C_B_ATOM, C_B_KAPPA, C_B_XHAT, C_B_NOT, C_B_XOR, C_B_AND, C_B_ANDPUB, C_B_OUT,
     C_A_CONST, C_A_X, C_A_COEFF, C_A_KAPPA, C_A_XHAT_SHR, C_A_ADD, C_A_SUB, C_A_MULC, C_A_MUL, C_A_B2A, C_A_OUT,
     C_A_MULXH,    /* variant bit 2: share times the PUBLIC masked input xhat, local (DESIGN 11) */
-    C_A_MULX      /* variant bit 1: product with the gate input x = xhat - r_in, one opening (DESIGN 10) */
+    C_A_MULX,     /* variant bit 1: product with the gate input x = xhat - r_in, one opening (DESIGN 10) */
+    C_B_A2B,      /* bit j >= 1 of a shared ring element: masked opening + a j-bit comparison key (DESIGN 15) */
+    C_B_LSB       /* bit 0 of a shared ring element: the XOR of the shares' low bits, local */
 };
 typedef struct { int op, dst, a, b, idx, round; u64 imm; } cop_t;
 
@@ -642,6 +646,7 @@ typedef struct orc_prog {
     int n_carry;                      /* theta-atoms; kappa^B = carries ++ user bits */
     int n_kb;                         /* total kappa^B bits */
     int MA, MB, GMIX, rounds;
+    int GA2B, a2b_bit[64];            /* A2B nodes with bit index j >= 1 (each: one opened ring element, one j-bit bit-DCF) */
     int nops; cop_t ops[OPMAX];
     int nbreg, nareg;
     int brdy[REGMAX], ardy[REGMAX];
@@ -1011,6 +1016,13 @@ orc_prog *orc_compile(const orc_spec *S0)
             case PHI_B_OR: ub[o->dst] = e_bnot(P, e_band(P, e_bnot(P, ub[o->a]), e_bnot(P, ub[o->b]))); break;
             case PHI_B_ANDPUB: d = newb(P, P->brdy[ub[o->a]]); emit(P, C_B_ANDPUB, d, ub[o->a], o->b, o->imm & 1); ub[o->dst] = d; break;
             case PHI_B_OUT: emit(P, C_B_OUT, o->dst, ub[o->a], 0, 0); break;
+            case PHI_B_A2B: {
+                if (o->b >= S->n || ua[o->a] < 0) { orc_destroy(P); return NULL; }
+                if (o->b == 0) { d = newb(P, P->ardy[ua[o->a]]); emit(P, C_B_LSB, d, ua[o->a], 0, 0); ub[o->dst] = d; break; }
+                int rd = P->ardy[ua[o->a]];
+                if (P->GA2B >= 8) { orc_destroy(P); return NULL; }
+                d = newb(P, rd + 1); k = emit(P, C_B_A2B, d, ua[o->a], 0, (u64)o->b);
+                P->a2b_bit[P->GA2B] = o->b; P->ops[k].idx = P->GA2B++; P->ops[k].round = rd; ub[o->dst] = d; break; }
             default: orc_destroy(P); return NULL;
             }
         }
@@ -1025,6 +1037,7 @@ orc_prog *orc_compile(const orc_spec *S0)
         if (o->op == C_A_MULX) { P->r_nmul[o->round]++; P->r_narr[o->round] += 1; P->ma_is_x[o->idx] = 1; }
         if (o->op == C_B_AND) P->r_nbits[o->round] += 2;
         if (o->op == C_A_B2A) P->r_nbits[o->round] += 1;
+        if (o->op == C_B_A2B) P->r_narr[o->round] += 1;
     }
     P->ma_word[0] = 0;
     for (int i = 0; i < P->MA; i++) P->ma_word[i + 1] = P->ma_word[i] + (P->ma_is_x[i] ? 2 : 3);
@@ -1034,7 +1047,7 @@ orc_prog *orc_compile(const orc_spec *S0)
 /* L_shape: out = T, M, p, M_A, M_B, G_mix, rounds, n_out_a, n_out_b, has_lut, n_kb ; ks[t] = k_t */
 void orc_shape(const orc_prog *P, int *out, int *ks)
 {
-    out[0] = P->T; out[1] = P->M; out[2] = P->p; out[3] = P->MA; out[4] = P->MB; out[5] = P->GMIX;
+    out[0] = P->T; out[1] = P->M; out[2] = P->p; out[3] = P->MA; out[4] = P->MB; out[5] = P->GMIX + P->GA2B;     /* G_mix = mixed-domain conversions, B2A and A2B */
     out[6] = P->rounds; out[7] = P->n_out_a; out[8] = P->n_out_b; out[9] = P->has_lut; out[10] = P->n_kb;
     for (int t = 0; t < P->T; t++) ks[t] = P->atoms[t].k;
 }
@@ -1132,6 +1145,7 @@ typedef struct {
     size_t bt_root[TMAX], bt_cw[TMAX], bt_vb[TMAX];
     size_t lut_c, vt_root[MMAX], vt_lvl[MMAX], vt_fin[MMAX], lvl_stride;
     size_t rin, rout, ka, rpow, kb, beaver, andt, b2a_bits, b2a_a, total;
+    size_t a2b_rho, a2b_bits, a2b_root[8], a2b_cw[8], a2b_vb[8];
 } layout_t;
 static size_t rup256(size_t x) { return (x + 255) & ~(size_t)255; }
 /* 16-byte correction arrays of a bit tree on k bits: k levels, or (early termination) max(k-7,0) levels + the leaf block */
@@ -1180,6 +1194,13 @@ static void layout(const orc_prog *P, size_t count, layout_t *L)
     L->andt = off; if (P->MB > 0) off += 3 * L->s8;
     L->b2a_bits = off; if (P->GMIX > 0) off += L->s8;
     L->b2a_a = off; off += (size_t)P->GMIX * L->s8;
+    L->a2b_rho = off; off += (size_t)P->GA2B * L->s8;                      /* A2B (DESIGN 15): [rho_i], one word of <bit_j(rho_i)>, */
+    L->a2b_bits = off; if (P->GA2B > 0) off += L->s8;                      /* then one j_i-bit comparison key per node             */
+    for (int i = 0; i < P->GA2B; i++) {
+        L->a2b_root[i] = off; off += L->s16;
+        L->a2b_cw[i] = off; off += L->s16 * bit_arrays(P, P->a2b_bit[i]);
+        L->a2b_vb[i] = off; off += L->s8;
+    }
     L->total = off;
 }
 static size_t bit_arrays(const orc_prog *P, int k) { return P->et ? (size_t)et_levels(k) + 1 : (size_t)k; }
@@ -1192,7 +1213,8 @@ size_t orc_key_bytes(const orc_prog *P, size_t count) { layout_t L; layout(P, co
 enum {
     SLOT_BT_ROOT = 0x1000, SLOT_VT_ROOT = 0x2000, SLOT_LUT_C = 0x3000, SLOT_RIN = 0x4000, SLOT_ROUT = 0x4100,
     SLOT_KA = 0x5000, SLOT_RPOW = 0x5400, SLOT_KB = 0x5800, SLOT_BV_AB = 0x6000, SLOT_BV_AB0 = 0x6800, SLOT_BV_C0 = 0x7000,
-    SLOT_AND_AB = 0x8000, SLOT_AND_AB0 = 0x8001, SLOT_AND_C0 = 0x8002, SLOT_B2A = 0x9000, SLOT_B2A_A0 = 0x9100
+    SLOT_AND_AB = 0x8000, SLOT_AND_AB0 = 0x8001, SLOT_AND_C0 = 0x8002, SLOT_B2A = 0x9000, SLOT_B2A_A0 = 0x9100,
+    SLOT_A2B_RHO = 0xB000, SLOT_A2B_RHO0 = 0xB100, SLOT_A2B_BITS = 0xB200, SLOT_A2B_ROOT = 0x1800
 };
 static void rnd(const aes_ks *ks, u64 e, u64 slot, u8 out[16])
 {
@@ -1381,6 +1403,30 @@ void orc_keygen(const orc_prog *P, const u64 *r_in, const u64 *r_out, u64 seed, 
                 u64 s0 = le64(rb) & mask, val = (rho >> i) & 1;
                 st8(key0, L.b2a_a + (size_t)i * L.s8, e, s0); st8(key1, L.b2a_a + (size_t)i * L.s8, e, (val - s0) & mask);
             }
+        }
+        if (P->GA2B > 0) {                                              /* A2B material (DESIGN 15): mask rho, <bit_j(rho)>, f_{rho mod 2^j, 1} */
+            u64 rbits = 0;
+            for (int i = 0; i < P->GA2B; i++) {
+                int j = P->a2b_bit[i];
+                rnd(&ks, ge, SLOT_A2B_RHO + i, rb);
+                u64 rho = le64(rb) & mask;
+                rnd(&ks, ge, SLOT_A2B_RHO0 + i, rb);
+                u64 s0 = le64(rb) & mask;
+                st8(key0, L.a2b_rho + (size_t)i * L.s8, e, s0); st8(key1, L.a2b_rho + (size_t)i * L.s8, e, (rho - s0) & mask);
+                rbits |= ((rho >> j) & 1) << i;
+                rnd(&ks, ge, SLOT_A2B_ROOT + 2 * i, rb); rnd(&ks, ge, SLOT_A2B_ROOT + 2 * i + 1, rb1);
+                if (P->et) dcf_bit_gen_et(j, rho & low_mask(j), rb, rb1, bk0, bk1);
+                else dcf_bit_gen(j, rho & low_mask(j), rb, rb1, bk0, bk1);
+                bitkey *bk[2] = { bk0, bk1 };
+                for (int b = 0; b < 2; b++) {
+                    st16(key[b], L.a2b_root[i], e, bk[b]->root);
+                    for (int l = 0; l < (int)bit_arrays(P, j); l++) st16(key[b], L.a2b_cw[i] + (size_t)l * L.s16, e, bk[b]->cw[l]);
+                    st8(key[b], L.a2b_vb[i], e, bk[b]->vbits);
+                }
+            }
+            rnd(&ks, ge, SLOT_A2B_BITS, rb);
+            u64 b0 = le64(rb) & low_mask(P->GA2B);
+            st8(key0, L.a2b_bits, e, b0); st8(key1, L.a2b_bits, e, rbits ^ b0);
         }
     }
     free(bk0); free(bk1); free(vk0); free(vk1);
@@ -1667,6 +1713,24 @@ void orc_post(int party, const orc_prog *P, const u8 *key, const u64 *xhat, cons
                     u64 F = (fm + ld8(msg_in, roff[q] + (size_t)pos * s8, e)) & mask;
                     A[o->dst] = (xh * A[o->a] - F * ld8(key, L.rin, e) - tc) & mask;
                 } else A[o->dst] = 0;
+                break; }
+            case C_B_LSB: Bv[o->dst] = (u8)(A[o->a] & 1); break;             /* (e_0 + e_1) mod 2 = e_0 ^ e_1 on the low bit */
+            case C_B_A2B: {  /* bit j of e (DESIGN 15): open ehat = e + rho; bit_j(e) = bit_j(ehat) ^ bit_j(rho) ^ I[ehat mod 2^j < rho mod 2^j] */
+                int q = o->round, pos = mulpos[q]; mulpos[q] += 1;
+                int j = (int)o->imm;
+                u64 em = (A[o->a] + ld8(key, L.a2b_rho + (size_t)o->idx * L.s8, e)) & mask;
+                if (q == round) st8(msg_out, roff[q] + (size_t)pos * s8, e, em);
+                if (q < round) {
+                    u64 E = (em + ld8(msg_in, roff[q] + (size_t)pos * s8, e)) & mask;
+                    bitkey *bk = malloc(sizeof *bk);
+                    ld16(key, L.a2b_root[o->idx], e, bk->root);
+                    for (int l = 0; l < (int)bit_arrays(P, j); l++) ld16(key, L.a2b_cw[o->idx] + (size_t)l * L.s16, e, bk->cw[l]);
+                    bk->vbits = ld8(key, L.a2b_vb[o->idx], e);
+                    int c = P->et ? dcf_bit_eval_et(party, j, bk, E & low_mask(j)) : dcf_bit_eval(party, j, bk, E & low_mask(j));
+                    free(bk);
+                    u8 rb_ = (u8)((ld8(key, L.a2b_bits, e) >> o->idx) & 1);
+                    Bv[o->dst] = (u8)((party == 0 ? (int)((E >> j) & 1) : 0) ^ rb_ ^ c);
+                } else Bv[o->dst] = 0;
                 break; }
             case C_A_B2A: {  /* open mu = z ^ rho; [z]_b = [b=0]mu + [rho]_b - 2 mu [rho]_b */
                 int q = o->round, pos = bitpos[q]; bitpos[q] += 1;

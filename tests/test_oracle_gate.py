@@ -93,6 +93,28 @@ def test_shift_relu_closed_form(orc, n, f):
         assert np.array_equal(z[1], (((xs + rv) & mask_of(n)) < rv).astype(np.uint8))
 
 
+@pytest.mark.parametrize("variant", [0, 9])
+def test_a2b_node(orc, variant):
+    """A2B (reading DESIGN 15 = bit extraction): every x and every r at n = 8 reconstructs Tier A, and Tier A's
+    extracted bits are what they claim to be (closed forms on the cleartext: MSB(x), bit f of y_0, LSB(x + y_0))."""
+    spec = specs.a2b_demo(8, 3)
+    if variant & 1:
+        spec = specs.shared_prefix(spec)
+    if variant & 8:
+        spec = specs.early_termination(spec)
+    P = check_all_r(orc, spec, range(256), seed=43)
+    assert P.shape["G_mix"] == 1 + 3 and P.post_rounds() == 4            # one B2A + three preprocessed A2B (the LSB one is local)
+    assert P.online_bits() == 8 + 2 * 8 + 3 * 8 + 1                       # xhat + the Horner Beaver product + three A2B openings + one B2A bit
+    x = np.arange(256, dtype=np.uint64)
+    y, z = P.plain_G(x, np.zeros(256, np.uint64))
+    y0 = np.array([int(P.plain_F(int(v))[0][0]) for v in x], dtype=np.uint64)
+    assert np.array_equal(z[0], (x >= 128).astype(np.uint8))
+    assert np.array_equal(z[1], ((y0 >> np.uint64(3)) & np.uint64(1)).astype(np.uint8))
+    assert np.array_equal(z[2], (((x + y0) & np.uint64(255)) & np.uint64(1)).astype(np.uint8))
+    check_pairs(orc, specs.a2b_demo(12, 4) if not variant else specs.early_termination(specs.shared_prefix(specs.a2b_demo(12, 4))),
+                np.tile(np.arange(0, 4096, 7, dtype=np.uint64), 3), np.repeat(np.array([0, 4095, 1234], dtype=np.uint64), 586), seed=44)
+
+
 def test_shape_is_mask_independent(orc):
     """Prop. I.3: (T, M, p), key length and layout depend on (program, count) only."""
     spec = specs.toy(8, 3)

@@ -19,7 +19,7 @@ KA_R_SHR, KB_R_BIT = 1, 2
 (PHI_A_CONST, PHI_A_X, PHI_A_Y, PHI_A_KAPPA, PHI_A_XHAT_SHR, PHI_A_ADD, PHI_A_SUB, PHI_A_MULC, PHI_A_MUL,
  PHI_A_B2A, PHI_A_OUT, PHI_A_AUX) = range(1, 13)
 (PHI_B_CONST, PHI_B_Z, PHI_B_KAPPA, PHI_B_XHAT, PHI_B_NOT, PHI_B_XOR, PHI_B_AND, PHI_B_OR, PHI_B_ANDPUB,
- PHI_B_OUT) = range(32, 42)
+ PHI_B_OUT, PHI_B_A2B) = range(32, 43)
 
 U64 = (1 << 64) - 1
 
@@ -323,6 +323,27 @@ def toy(n=8, f=3, mask_output=False):
     return _mk(f"toy_n{n}", n, f, [a1, a2, a3], coeff, nodes=nodes, bit_root=bit_root, aux=aux,
                kappa_a=[(KA_R_SHR, 2)], kappa_b=[(KB_R_BIT, 1)], phi=phi, n_out_a=2, n_out_b=4,
                mask_output=mask_output, out_frac=f)
+
+
+def a2b_demo(n=8, f=3):
+    """Exercises the A2B node (App. H: "A2B : [x] -> <b> for a suitable extracted bit b"; DESIGN 15): Phi extracts
+    the sign of the gate input itself (bit n-1 of x), bit f of the degree-1 spline output y_0, the low bit of y_0 + x (local), and
+    feeds an extracted bit back into arithmetic through B2A.  m = 3 intervals, one predicate bit."""
+    N = 1 << n
+    nodes = [(BN_C, 0, 0, 0, 0, N // 3)]
+    phi = [
+        (PHI_A_X, 0, 0, 0, 0), (PHI_A_Y, 1, 0, 0, 0), (PHI_A_ADD, 2, 0, 1, 0),
+        (PHI_B_A2B, 0, 0, n - 1, 0),          # B0 = MSB(x)
+        (PHI_B_A2B, 1, 1, f, 0),              # B1 = bit f of y_0
+        (PHI_B_A2B, 2, 2, 0, 0),              # B2 = LSB(x + y_0)   (local)
+        (PHI_B_Z, 3, 0, 0, 0), (PHI_B_XOR, 4, 0, 3, 0),
+        (PHI_A_B2A, 3, 1, 0, 0), (PHI_A_MULC, 4, 3, 0, 5), (PHI_A_ADD, 5, 4, 1, 0),
+        (PHI_B_A2B, 5, 5, 1, 0),              # B5 = bit 1 of (5 B1 + y_0): an A2B after a B2A, two rounds later
+        (PHI_A_OUT, 0, 5, 0, 0),
+        (PHI_B_OUT, 0, 0, 0, 0), (PHI_B_OUT, 1, 1, 0, 0), (PHI_B_OUT, 2, 2, 0, 0), (PHI_B_OUT, 3, 4, 0, 0), (PHI_B_OUT, 4, 5, 0, 0),
+    ]
+    return _mk(f"a2b_n{n}", n, f, [N // 4, N // 2 + 3], [[[3, 1]], [[-2, 7]], [[1, -5]]], nodes=nodes, bit_root=[[0]] * 3,
+               phi=phi, n_out_a=1, n_out_b=5, out_frac=2 * f)
 
 
 def plain_default(n=8, f=3):
