@@ -74,7 +74,10 @@ enum {
     FUSEFSS_PHI_B_XHAT,       /* B[dst] = bit a of xhat (public)     */
     FUSEFSS_PHI_B_NOT, FUSEFSS_PHI_B_XOR, FUSEFSS_PHI_B_AND, FUSEFSS_PHI_B_OR,
     FUSEFSS_PHI_B_ANDPUB,     /* B[dst] = B[a] & (bit b of xhat ^ (imm&1)) */
-    FUSEFSS_PHI_B_OUT         /* output z'[dst] = B[a]               */
+    FUSEFSS_PHI_B_OUT,        /* output z'[dst] = B[a]               */
+    FUSEFSS_PHI_B_A2B         /* B[dst] = bit b of the ring element A[a]: the A2B node ([x] -> <b> "for a suitable extracted bit b",
+                                 P:81, 683-685).  b = 0 is local (XOR of the shares' low bits); b >= 1 costs one opened ring
+                                 element and one b-bit comparison key from the dealer, one round (DESIGN 15); at most 8 per gate */
 };
 typedef struct { uint8_t op, dst, a, b; uint32_t pad; uint64_t imm; } fusefss_phi_op;
 
@@ -86,7 +89,8 @@ typedef struct {
     uint32_t mask_output;             /* 1: arithmetic outputs are opened as yhat = y + r_out       */
     uint32_t variant;                 /* bit 0: single-key shared-prefix construction (DESIGN 9); bit 1: input-masked products
                                          (DESIGN 10); bit 2: Horner in the public xhat (DESIGN 11); bit 3: early-terminated bit trees
-                                         (DESIGN 13).  0 = the paper's Protocol 3 with textbook subprotocols. */
+                                         (DESIGN 13); bit 4: dense-table lookup by full-domain evaluation, needs bit 0 and n <= 16
+                                         (DESIGN 14).  0 = the paper's Protocol 3 with textbook subprotocols. */
     const uint64_t *alpha;            /* HOST [m-1] interior boundaries, strictly increasing in (0, 2^n)    */
     const uint64_t *coeff;            /* HOST [m][r][d+1], high degree first                                */
     const uint64_t *aux;              /* HOST [m][p_aux]                                                    */
@@ -98,7 +102,8 @@ typedef struct {
 
 typedef struct fusefss_program fusefss_program;   /* opaque, library-owned */
 
-/* L_shape = (T, {k_t}, M, p, #mults, #ANDs, #B2A) -- everything that may depend on the spec only */
+/* L_shape = (T, {k_t}, M, p, #mults, #ANDs, #mixed-domain conversions) -- everything that may depend on the spec only
+ * (P:195, 905-909); G_mix counts B2A and (interactive) A2B conversions */
 typedef struct {
     int32_t T, M, p, M_A, M_B, G_mix, rounds, n_out_a, n_out_b, has_lut, n_kb;
     int32_t k[64];
@@ -171,7 +176,8 @@ int fusefss_post(int party, const fusefss_program *prog, const void *key_dev, co
                  void *stream);
 int fusefss_post_rounds(const fusefss_program *prog);
 size_t fusefss_post_msg_bytes(const fusefss_program *prog, size_t count, int round);
-/* algorithmic online bits per element per party: n (xhat) + 2n M_A + 2 M_B + G_mix (+ n n_out_a if masked) */
+/* algorithmic online bits per element per party: n (xhat) + n per opened ring element (2 per Beaver product, 1 per x-product,
+ * 1 per interactive A2B) + 2 M_B + #B2A (+ n n_out_a if masked) */
 size_t fusefss_online_bits(const fusefss_program *prog);
 /* Both parties, all rounds, one launch; outputs equal the per-round API bit for bit. */
 int fusefss_post_fused(const fusefss_program *prog, const void *key0_dev, const void *key1_dev,

@@ -100,6 +100,7 @@ class Softmax:
     def online_bytes_per_party(self) -> int:
         """openings of every gate input + the gates' own post-processing messages + 2 ring elements per Beaver product"""
         total = sum(self.progs[k].online_bits() // 8 * c for k, c in self.counts.items())
+        total -= sum(self.n // 8 * self.counts[consumer] for consumer in self.edges.values())   # a fused wire is opened once: the producer's yhat IS the consumer's xhat
         return total + 16 * self.N
 
     def key_bytes_per_party(self) -> int:
@@ -183,7 +184,8 @@ class LayerNorm(Softmax):
         return dict(m=(m0, m1), c=(c0, c1), q=tuple(self.sq), v=(v0, v1), g=(g0, g1), h=(h0, h1), p=tuple(self.prod), y=(y0, y1))
 
     def online_bytes_per_party(self) -> int:
-        return sum(self.progs[k].online_bits() // 8 * c for k, c in self.counts.items()) + 2 * 16 * self.N
+        fused = sum(self.n // 8 * self.counts[consumer] for consumer in self.edges.values())     # a fused wire is opened once
+        return sum(self.progs[k].online_bits() // 8 * c for k, c in self.counts.items()) - fused + 2 * 16 * self.N
 
     def key_bytes_per_party(self) -> int:
         return sum(self.progs[k].key_bytes(c) for k, c in self.counts.items()) + 2 * lib.fusefss_mul_triple_bytes(self.N)

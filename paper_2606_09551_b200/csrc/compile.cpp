@@ -306,6 +306,18 @@ bool Lowering::lower_phi(int xval, const std::vector<int> &yval, const std::vect
         case FUSEFSS_PHI_B_ANDPUB: {
             int a = B(o.a); int d = fresh_b(b_ready[a]); push(I_B_ANDPUB, d, a, o.b, o.imm & 1); ub[o.dst] = d; break; }
         case FUSEFSS_PHI_B_OUT: if ((int)o.dst >= P.n_out_b || o.dst >= 64) return false; push(I_B_OUT, o.dst, B(o.a), 0, 0); break;
+        case FUSEFSS_PHI_B_A2B: {                 // bit o.b of a shared ring element (DESIGN 15)
+            if (o.b >= P.n) return false;
+            const int s = A(o.a);
+            if (failed) return false;
+            if (o.b == 0) { int d = fresh_b(a_ready[s]); push(I_B_LSB, d, s, 0, 0); ub[o.dst] = d; break; }   // (e_0 + e_1) mod 2: local
+            if (P.GA2B >= kMaxA2B) return false;
+            const int rd = a_ready[s];
+            int d = fresh_b(rd + 1);
+            Ins &i = push(I_B_A2B, d, s, 0, (uint64_t)o.b);
+            P.a2b_bit[P.GA2B] = (int)o.b; i.gate = (uint16_t)P.GA2B++; i.round = (uint8_t)rd;
+            if (rd >= kMaxRounds) failed = true;
+            ub[o.dst] = d; break; }
         default: return false;
         }
         if (failed) return false;
@@ -377,6 +389,7 @@ bool Lowering::finish() {
             P.ma_is_x[i.gate] = i.op == I_A_MULX;
             P.rounds = std::max(P.rounds, i.round + 1);
         }
+        else if (i.op == I_B_A2B) { i.pos = (uint16_t)mulpos[i.round]; mulpos[i.round] += 1; P.rounds = std::max(P.rounds, i.round + 1); }
         else if (i.op == I_B_AND) { i.pos = (uint16_t)bitpos[i.round]; bitpos[i.round] += 2; P.rounds = std::max(P.rounds, i.round + 1); }
         else if (i.op == I_A_B2A) { i.pos = (uint16_t)bitpos[i.round]; bitpos[i.round] += 1; P.rounds = std::max(P.rounds, i.round + 1); }
     }
@@ -396,7 +409,7 @@ bool Lowering::finish() {
         case I_B_NOT: case I_B_ANDPUB: case I_B_OUT: case I_A_B2A: a_is_B = true; break;
         case I_B_XOR: case I_B_AND: a_is_B = b_is_B = true; break;
         case I_A_ADD: case I_A_SUB: case I_A_MUL: a_is_A = b_is_A = true; break;
-        case I_A_MULC: case I_A_OUT: case I_A_MULX: case I_A_MULXH: a_is_A = true; break;
+        case I_A_MULC: case I_A_OUT: case I_A_MULX: case I_A_MULXH: case I_B_LSB: case I_B_A2B: a_is_A = true; break;
         default: break;
         }
     };
@@ -410,7 +423,7 @@ bool Lowering::finish() {
     std::vector<int> a_map(a_ready.size(), -1), b_map(b_ready.size(), -1), a_free, b_free;
     int a_next = 0, b_next = 0;
     auto writes_a = [](uint8_t op) { return op >= I_A_CONST && op <= I_A_B2A; };
-    auto writes_b = [](uint8_t op) { return op >= I_B_CONST && op <= I_B_ANDPUB; };
+    auto writes_b = [](uint8_t op) { return (op >= I_B_CONST && op <= I_B_ANDPUB) || op == I_B_LSB || op == I_B_A2B; };
     for (int t = 0; t < NI; ++t) {
         Ins &i = P.ins[t];
         bool aA, aB, bA, bB; reads(i, aA, aB, bA, bB);
@@ -604,6 +617,13 @@ void compute_layout(const Program &P, size_t count, Layout *L) {
     L->andt = off;     if (P.MB > 0) off += 3 * L->s8;
     L->b2a_bits = off; if (P.GMIX > 0) off += L->s8;
     L->b2a_a = off;    off += (size_t)P.GMIX * L->s8;
+    L->a2b_rho = off;  off += (size_t)P.GA2B * L->s8;                             // [rho_i], one word of <bit_j(rho_i)>, then one
+    L->a2b_bits = off; if (P.GA2B > 0) off += L->s8;                              // j_i-bit comparison key per node (DESIGN 15)
+    for (int i = 0; i < P.GA2B; ++i) {
+        L->a2b_root[i] = off; off += L->s16;
+        L->a2b_cw[i] = off;   off += L->s16 * (size_t)bit_tree_arrays(P, P.a2b_bit[i]);
+        L->a2b_vb[i] = off;   off += L->s8;
+    }
     L->total = off;
 }
 

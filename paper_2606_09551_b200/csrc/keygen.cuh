@@ -14,7 +14,8 @@ constexpr int kGenThreads = 512;
 enum : uint64_t {
     SLOT_BIT_ROOT = 0x1000, SLOT_VEC_ROOT = 0x2000, SLOT_LUT_C = 0x3000, SLOT_RIN = 0x4000, SLOT_ROUT = 0x4100,
     SLOT_KA = 0x5000, SLOT_KB = 0x5800, SLOT_BV_AB = 0x6000, SLOT_BV_AB0 = 0x6800, SLOT_BV_C0 = 0x7000,
-    SLOT_AND_AB = 0x8000, SLOT_AND_AB0 = 0x8001, SLOT_AND_C0 = 0x8002, SLOT_B2A = 0x9000, SLOT_B2A_A0 = 0x9100
+    SLOT_AND_AB = 0x8000, SLOT_AND_AB0 = 0x8001, SLOT_AND_C0 = 0x8002, SLOT_B2A = 0x9000, SLOT_B2A_A0 = 0x9100,
+    SLOT_A2B_RHO = 0xB000, SLOT_A2B_RHO0 = 0xB100, SLOT_A2B_BITS = 0xB200       // A2B (DESIGN 15); its tree roots: 0x1800 + 2i + b
 };
 
 __device__ __forceinline__ void st_stream16(void *p, uint4 v) { __stcs(reinterpret_cast<uint4 *>(p), v); }
@@ -28,11 +29,13 @@ __device__ __forceinline__ void dealer_rand(uint32_t tl, const RoundKeys &rk, ui
     hi = (uint64_t)s[2] | ((uint64_t)s[3] << 32);
 }
 
+// is_theta: 0 = r-atom (threshold r_k), 1 = theta-atom (r_k + beta), 2 = A2B key i (threshold rho_i mod 2^k, rho_i = R(e, 0xB000 + i))
 struct GenAtomDev { uint64_t c, beta, root_off, cw_off, vb_off; int k, is_theta; };
 struct GenBitArgs {
     uint8_t *key0, *key1; const uint64_t *r_in;
     size_t count, s16; uint64_t first_elem, mask;
     int T, et;                 // et: early-terminated trees (variant bit 3, DESIGN 13): max(k-7,0) levels + a 128-bit leaf block
+    int slot_t0, pad;          // tree t draws its roots from R(e, 0x1000 + 2 (slot_t0 + t) + b): 0 for the atoms, 0x400 for the A2B keys
     RoundKeys rk;
     GenAtomDev atom[kMaxAtoms];
 };
@@ -52,15 +55,20 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_bit(const __grid_constan
         const int k = at.k;
         if (k == 0) continue;                              // variant 1: slot of the n-bit view (its key is a vector tree)
         const uint64_t km = k >= 64 ? ~0ull : ((1ull << k) - 1ull);
-        const uint64_t rk_ = a.r_in[e] & a.mask & km;
+        uint64_t rk_ = a.r_in[e] & a.mask & km;
+        if (at.is_theta == 2) {                            // A2B key t: the threshold is the low k bits of the dealer's mask rho_t
+            uint64_t lo, hi;
+            dealer_rand(tl, a.rk, a.first_elem + e, SLOT_A2B_RHO + t, lo, hi);
+            rk_ = lo & a.mask & km;
+        }
         // threshold of the masked comparison (Lemma 4.3 / E.1): theta = (r_k + beta) mod 2^k, or r_k for the r-atom
-        uint64_t alpha = (at.is_theta ? (rk_ + at.beta) & km : rk_) << (64 - k);
+        uint64_t alpha = (at.is_theta == 1 ? (rk_ + at.beta) & km : rk_) << (64 - k);
         uint32_t s[2][4];
         {
             uint64_t lo, hi;
-            dealer_rand(tl, a.rk, a.first_elem + e, SLOT_BIT_ROOT + 2 * t, lo, hi);
+            dealer_rand(tl, a.rk, a.first_elem + e, SLOT_BIT_ROOT + 2 * (a.slot_t0 + t), lo, hi);
             s[0][0] = (uint32_t)lo & ~3u; s[0][1] = (uint32_t)(lo >> 32); s[0][2] = (uint32_t)hi; s[0][3] = (uint32_t)(hi >> 32);
-            dealer_rand(tl, a.rk, a.first_elem + e, SLOT_BIT_ROOT + 2 * t + 1, lo, hi);
+            dealer_rand(tl, a.rk, a.first_elem + e, SLOT_BIT_ROOT + 2 * (a.slot_t0 + t) + 1, lo, hi);
             s[1][0] = (uint32_t)lo & ~3u; s[1][1] = (uint32_t)(lo >> 32); s[1][2] = (uint32_t)hi; s[1][3] = (uint32_t)(hi >> 32);
         }
         const uint4 root0 = make_uint4(s[0][0], s[0][1], s[0][2], s[0][3]);
@@ -345,8 +353,9 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec(const __grid_constan
 // ---------------------------------------------------------------------------------------------------
 struct GenMiscArgs {
     uint8_t *key0, *key1; const uint64_t *r_in, *r_out, *alpha, *payload;
-    size_t count, s8, lut_c, rin, rout, ka, kb, beaver, andt, b2a_bits, b2a_a, rpow;
+    size_t count, s8, lut_c, rin, rout, ka, kb, beaver, andt, b2a_bits, b2a_a, rpow, a2b_rho, a2b_bits;
     int xpoly, polys, d, n_rpow;
+    int GA2B, a2b_bit[kMaxA2B], pad3;
     uint64_t first_elem, mask;
     int n, m, M, p, has_lut, mask_output, n_out_a, n_ka, n_kb_spec, n_carry, T, MA, MB, GMIX;
     uint64_t ma_is_x;          // bit i: arithmetic gate i is a product with the gate input (material (b, c = b r_in), DESIGN 10)
@@ -470,6 +479,20 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_misc(const __grid_consta
                 const uint64_t s0 = lo & a.mask, val = (rho >> i) & 1ull;
                 put(a.b2a_a + (size_t)i * a.s8, s0, (val - s0) & a.mask);
             }
+        }
+        if (a.GA2B > 0) {                                                  // A2B (DESIGN 15): [rho_i] and <bit_j(rho_i)>; the keys f_{rho_i mod 2^j, 1} are k_gen_bit's
+            uint64_t rbits = 0;
+            for (int i = 0; i < a.GA2B; ++i) {
+                dealer_rand(tl, a.rk, ge, SLOT_A2B_RHO + i, lo, hi);
+                const uint64_t rho = lo & a.mask;
+                dealer_rand(tl, a.rk, ge, SLOT_A2B_RHO0 + i, lo, hi);
+                const uint64_t s0 = lo & a.mask;
+                put(a.a2b_rho + (size_t)i * a.s8, s0, (rho - s0) & a.mask);
+                rbits |= ((rho >> a.a2b_bit[i]) & 1ull) << i;
+            }
+            dealer_rand(tl, a.rk, ge, SLOT_A2B_BITS, lo, hi);
+            const uint64_t b0 = lo & ((1ull << a.GA2B) - 1ull);
+            put(a.a2b_bits, b0, rbits ^ b0);
         }
     }
 }

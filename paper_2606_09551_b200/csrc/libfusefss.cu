@@ -329,8 +329,21 @@ int launch_eval(const Program &P, int party, const void *k0, const void *k1, con
     return P.variant ? launch_eval_sp(P, party, key, xhat, count, bits, coeff, st) : launch_eval_p3(P, party, key, xhat, count, bits, coeff, st);
 }
 
-PostKeyOff post_offsets(const Layout &L) {
-    return PostKeyOff{L.s8, L.rin, L.rout, L.ka, L.kb, L.beaver, L.andt, L.b2a_bits, L.b2a_a};
+PostKeyOff post_offsets(const Program &P, const Layout &L) {
+    PostKeyOff k{};
+    k.s8 = L.s8; k.rin = L.rin; k.rout = L.rout; k.ka = L.ka; k.kb = L.kb; k.beaver = L.beaver; k.andt = L.andt;
+    k.b2a_bits = L.b2a_bits; k.b2a_a = L.b2a_a; k.s16 = L.s16; k.a2b_rho = L.a2b_rho; k.a2b_bits = L.a2b_bits; k.et = (int)P.et;
+    for (int i = 0; i < P.GA2B; ++i) { k.a2b_root[i] = L.a2b_root[i]; k.a2b_cw[i] = L.a2b_cw[i]; k.a2b_vb[i] = L.a2b_vb[i]; }
+    return k;
+}
+
+// post-processing launch geometry: one lane per element; programs with interactive A2B nodes walk comparison keys, so they run as
+// persistent CTAs (one per SM) with the PRG tables in shared memory
+template <typename K0, typename K1, typename A>
+int launch_post(const Program &P, K0 plain, K1 with_a2b, size_t count, cudaStream_t st, const A &a) {
+    const size_t blocks = (count + 255) / 256;
+    if (P.GA2B == 0) return launch(plain, (int)blocks, 256, 0, st, a);
+    return launch(with_a2b, (int)(blocks < (size_t)g_sms ? blocks : (size_t)g_sms), 256, kAesSmemBytes, st, a);
 }
 
 }  // namespace
@@ -360,7 +373,7 @@ int fusefss_shape(const fusefss_program *prog, fusefss_shape_t *out) {
     const Program *P = prog_of(prog);
     if (!P || !out) return FUSEFSS_E_NULL;
     *out = fusefss_shape_t{};
-    out->T = P->T; out->M = P->M; out->p = P->p; out->M_A = P->MA; out->M_B = P->MB; out->G_mix = P->GMIX;
+    out->T = P->T; out->M = P->M; out->p = P->p; out->M_A = P->MA; out->M_B = P->MB; out->G_mix = P->GMIX + P->GA2B;
     out->rounds = P->rounds; out->n_out_a = P->n_out_a; out->n_out_b = P->n_out_b; out->has_lut = P->has_lut;
     out->n_kb = P->n_kb;
     for (int t = 0; t < P->T; ++t) out->k[t] = P->atoms[t].k;
@@ -562,9 +575,21 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
         for (int t = 0; t < a.n_kb_spec; ++t) { a.kb_kind[t] = P->kappa_b[t].kind; a.kb_arg[t] = P->kappa_b[t].arg; }
         for (int t = 0; t < a.T; ++t)
             a.atom[t] = GenAtomDev{P->atoms[t].c, P->atoms[t].beta, 0, 0, 0, P->atoms[t].k, P->atoms[t].is_theta};
+        a.a2b_rho = L.a2b_rho; a.a2b_bits = L.a2b_bits; a.GA2B = P->GA2B;
+        for (int i = 0; i < P->GA2B; ++i) a.a2b_bit[i] = P->a2b_bit[i];
         const int th = threads_for(tiles, kGenThreads), grid = grid_for(tiles, th);
         rc = launch(k_gen_misc, grid, th, kAesSmemBytes, st, a);
         if (rc) return rc;
+        if (P->GA2B > 0) {                              // the A2B nodes' comparison keys f_{rho_i mod 2^j, 1} (DESIGN 15): part of the shares section
+            GenBitArgs ab{};
+            ab.key0 = (uint8_t *)key0_dev; ab.key1 = (uint8_t *)key1_dev; ab.r_in = r_in_dev;
+            ab.count = count; ab.s16 = L.s16; ab.first_elem = first_elem; ab.mask = P->mask; ab.T = P->GA2B; ab.rk = rk; ab.et = (int)P->et;
+            ab.slot_t0 = 0x400;
+            for (int i = 0; i < P->GA2B; ++i) ab.atom[i] = GenAtomDev{0, 0, L.a2b_root[i], L.a2b_cw[i], L.a2b_vb[i], P->a2b_bit[i], 2};
+            const int th2 = threads_for(tiles * P->GA2B, kGenThreads);
+            rc = launch(k_gen_bit, grid_for(tiles * P->GA2B, th2), th2, kAesSmemBytes, st, ab);
+            if (rc) return rc;
+        }
     }
     return 0;
 }
@@ -637,13 +662,13 @@ int fusefss_post(int party, const fusefss_program *prog, const void *key_dev, co
     a.n_out_a = P->n_out_a; a.n_out_b = P->n_out_b;
     a.key = (const uint8_t *)key_dev; a.xhat = xhat_dev; a.bits = bits_dev; a.coeff = coeff_dev;
     a.msg_in = (const uint8_t *)msg_in_dev; a.msg_out = (uint8_t *)msg_out_dev; a.y_out = y_out_dev; a.z_out = z_out_dev;
-    a.count = count; a.mask = P->mask; a.k = post_offsets(L);
+    a.count = count; a.mask = P->mask; a.k = post_offsets(*P, L);
     a.round_off[0] = 0;
     for (int q = 0; q < kMaxRounds; ++q) {
         a.round_off[q + 1] = a.round_off[q] + post_msg_bytes(*P, count, q);
         a.round_arr[q] = P->round_arr[q]; a.round_bits[q] = P->round_bits[q];
     }
-    return launch(k_post_round, (int)((count + 255) / 256), 256, 0, (cudaStream_t)stream, a);
+    return launch_post(*P, k_post_round<false>, k_post_round<true>, count, (cudaStream_t)stream, a);
 }
 
 int fusefss_post_fused(const fusefss_program *prog, const void *key0_dev, const void *key1_dev, const uint64_t *xhat_dev,
@@ -665,8 +690,8 @@ int fusefss_post_fused(const fusefss_program *prog, const void *key0_dev, const 
     a.key[0] = (const uint8_t *)key0_dev; a.key[1] = (const uint8_t *)key1_dev; a.xhat = xhat_dev;
     a.bits[0] = bits0_dev; a.bits[1] = bits1_dev; a.coeff[0] = coeff0_dev; a.coeff[1] = coeff1_dev;
     a.y_out[0] = y0_dev; a.y_out[1] = y1_dev; a.z_out[0] = z0_dev; a.z_out[1] = z1_dev;
-    a.count = count; a.mask = P->mask; a.k = post_offsets(L);
-    return launch(k_post_fused, (int)((count + 255) / 256), 256, 0, (cudaStream_t)stream, a);
+    a.count = count; a.mask = P->mask; a.k = post_offsets(*P, L);
+    return launch_post(*P, k_post_fused<false>, k_post_fused<true>, count, (cudaStream_t)stream, a);
 }
 
 // ---- vector-block glue (App. G) -------------------------------------------

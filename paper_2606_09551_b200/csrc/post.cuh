@@ -4,12 +4,20 @@
 // Subprotocol formulas and message layout: DESIGN 4.6.  One lane per element interprets the compiled
 // straight-line program (program.h Ins) out of global memory (uniform across the warp); arithmetic registers
 // live in a small per-thread array, bit registers in one 64-bit word.
+// A2B nodes (DESIGN 15): bit 0 of a shared value is local; bit j >= 1 opens ehat = e + rho and evaluates the dealer's
+// j-bit comparison key at ehat mod 2^j: bit_j(e) = bit_j(ehat) ^ bit_j(rho) ^ I[ehat mod 2^j < rho mod 2^j].  Programs with such
+// nodes run the <true> instantiations: persistent CTAs with the PRG tables in shared memory (grid-stride over elements).
 #pragma once
+#include "eval.cuh"
 #include "program.h"
 
 namespace fsk {
 
-struct PostKeyOff { size_t s8, rin, rout, ka, kb, beaver, andt, b2a_bits, b2a_a; };   // (rpow is read by the eval kernel only)
+struct PostKeyOff {                                                                  // (rpow is read by the eval kernel only)
+    size_t s8, rin, rout, ka, kb, beaver, andt, b2a_bits, b2a_a;
+    size_t s16, a2b_rho, a2b_bits, a2b_root[kMaxA2B], a2b_cw[kMaxA2B], a2b_vb[kMaxA2B];
+    int et, pad;
+};
 
 struct PostArgs {
     const Ins *ins; int n_ins;
@@ -29,9 +37,12 @@ __device__ __forceinline__ uint64_t kld(const uint8_t *key, size_t off, size_t e
 }
 
 // one party, one round; stateless replay of earlier rounds from the two message buffers
+template <bool A2B>
 __global__ void __launch_bounds__(256) k_post_round(const __grid_constant__ PostArgs a) {
-    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= a.count) return;
+    extern __shared__ uint32_t sT[];
+    uint32_t tl = 0;
+    if (A2B) tl = aes_fill_tables(sT);
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < a.count; e += (size_t)gridDim.x * blockDim.x) {
     const uint64_t mask = a.mask, xh = a.xhat[e] & mask;
     const bool p0 = a.party == 0;
     uint64_t A[kMaxAReg];
@@ -123,12 +134,30 @@ __global__ void __launch_bounds__(256) k_post_round(const __grid_constant__ Post
             }
             A[o.dst] = res;
             break; }
+        case I_B_LSB: setb(o.dst, A[o.a]); break;                          // (e_0 + e_1) mod 2 = e_0 ^ e_1 on the low bit
+        case I_B_A2B: {
+            uint64_t res = 0;
+            if (A2B) {
+                const int q = o.round, j = (int)o.imm, g = o.gate;
+                const uint64_t em = (A[o.a] + kld(a.key, a.k.a2b_rho + (size_t)g * a.k.s8, e)) & mask;
+                const size_t mo = a.round_off[q] + (size_t)o.pos * a.k.s8;
+                if (q == a.round) reinterpret_cast<uint64_t *>(a.msg_out + mo)[e] = em;
+                if (q < a.round) {
+                    const uint64_t E = (em + kld(a.msg_in, mo, e)) & mask;
+                    const uint32_t c = bit_tree_eval<false>(tl, a.key, a.k.a2b_root[g], a.k.a2b_cw[g], a.k.a2b_vb[g], e, a.k.s16, j,
+                                                            E << (64 - j), a.party, a.k.et);
+                    res = (p0 ? (E >> j) : 0ull) ^ (kld(a.key, a.k.a2b_bits, e) >> g) ^ (uint64_t)c;
+                }
+            }
+            setb(o.dst, res);
+            break; }
         default: break;
         }
     }
     if (a.round < a.rounds && a.round_bits[a.round])
         reinterpret_cast<uint64_t *>(a.msg_out + a.round_off[a.round] + (size_t)a.round_arr[a.round] * a.k.s8)[e] = outbits;
     if (a.round == a.rounds && a.n_out_b > 0) a.z_out[e] = zword;
+    }
 }
 
 struct PostFusedArgs {
@@ -141,9 +170,12 @@ struct PostFusedArgs {
 };
 
 // both parties, all rounds, one pass: the openings are combined in registers instead of message buffers
+template <bool A2B>
 __global__ void __launch_bounds__(256) k_post_fused(const __grid_constant__ PostFusedArgs a) {
-    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= a.count) return;
+    extern __shared__ uint32_t sT[];
+    uint32_t tl = 0;
+    if (A2B) tl = aes_fill_tables(sT);
+    for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < a.count; e += (size_t)gridDim.x * blockDim.x) {
     const uint64_t mask = a.mask, xh = a.xhat[e] & mask;
     uint64_t A[2][kMaxAReg];
     uint64_t Bw[2] = {0, 0}, zword[2] = {0, 0};
@@ -221,10 +253,25 @@ __global__ void __launch_bounds__(256) k_post_fused(const __grid_constant__ Post
             A[0][o.dst] = (mu + ra[0] - 2 * mu * ra[0]) & mask;
             A[1][o.dst] = (ra[1] - 2 * mu * ra[1]) & mask;
             break; }
+        case I_B_LSB: setb(0, o.dst, A[0][o.a]); setb(1, o.dst, A[1][o.a]); break;
+        case I_B_A2B:
+            if (A2B) {
+                const int j = (int)o.imm, g = o.gate;
+                const uint64_t E = (A[0][o.a] + A[1][o.a] + kld(a.key[0], a.k.a2b_rho + (size_t)g * a.k.s8, e) +
+                                    kld(a.key[1], a.k.a2b_rho + (size_t)g * a.k.s8, e)) & mask;
+#pragma unroll
+                for (int b = 0; b < 2; ++b) {
+                    const uint32_t c = bit_tree_eval<false>(tl, a.key[b], a.k.a2b_root[g], a.k.a2b_cw[g], a.k.a2b_vb[g], e, a.k.s16, j,
+                                                            E << (64 - j), b, a.k.et);
+                    setb(b, o.dst, (b == 0 ? (E >> j) : 0ull) ^ (kld(a.key[b], a.k.a2b_bits, e) >> g) ^ (uint64_t)c);
+                }
+            }
+            break;
         default: break;
         }
     }
     if (a.n_out_b > 0) { a.z_out[0][e] = zword[0]; a.z_out[1][e] = zword[1]; }
+    }
 }
 
 }  // namespace fsk

@@ -17,6 +17,7 @@ constexpr int kMaxIntervals = 64;  // m < 64
 constexpr int kMaxRounds = 16;
 constexpr int kMaxAReg = 48;       // arithmetic registers after allocation (device local array)
 constexpr int kMaxBReg = 64;       // bit registers after allocation (one 64-bit word per party)
+constexpr int kMaxA2B = 8;         // interactive A2B nodes per gate
 
 // One query of the packed comparison instance (Def I.1).
 struct Atom {
@@ -31,7 +32,9 @@ struct Atom {
 // (`gate`), their round and their position inside that round's message (`pos`).
 enum : uint8_t {
     I_B_CONST = 1, I_B_ATOM, I_B_KAPPA, I_B_XHAT, I_B_NOT, I_B_XOR, I_B_AND, I_B_ANDPUB, I_B_OUT,
-    I_A_CONST, I_A_X, I_A_COEFF, I_A_KAPPA, I_A_XHAT_SHR, I_A_ADD, I_A_SUB, I_A_MULC, I_A_MUL, I_A_MULX, I_A_MULXH, I_A_B2A, I_A_OUT
+    I_A_CONST, I_A_X, I_A_COEFF, I_A_KAPPA, I_A_XHAT_SHR, I_A_ADD, I_A_SUB, I_A_MULC, I_A_MUL, I_A_MULX, I_A_MULXH, I_A_B2A, I_A_OUT,
+    I_B_LSB,            // B[dst] = bit 0 of the shared ring element A[a]: local (DESIGN 15)
+    I_B_A2B             // B[dst] = bit imm >= 1 of A[a]: open A[a] + rho, then one imm-bit comparison key (DESIGN 15); gate = A2B index
 };
 struct Ins {
     uint8_t op;
@@ -50,6 +53,7 @@ struct Layout {
     size_t bt_root[kMaxAtoms], bt_cw[kMaxAtoms], bt_vb[kMaxAtoms];
     size_t lut_c, vt_first, vt_stride, lvl_stride, vt_lvl_rel, vt_fin_rel;   // vector tree j at vt_first + (j-1)*vt_stride
     size_t rin, rout, ka, rpow, kb, beaver, andt, b2a_bits, b2a_a, total;
+    size_t a2b_rho, a2b_bits, a2b_root[kMaxA2B], a2b_cw[kMaxA2B], a2b_vb[kMaxA2B];   // A2B material (DESIGN 15), after the B2A section
 };
 
 // variant 1: single-key shared-prefix construction
@@ -86,6 +90,7 @@ struct Program {
     int M = 0, p = 0, Q = 0, T = 0, has_lut = 0;
     int n_carry = 0, n_kb = 0;
     int MA = 0, MB = 0, GMIX = 0, rounds = 0, n_out_a = 0, n_out_b = 0;
+    int GA2B = 0, a2b_bit[kMaxA2B] = {0};   // A2B nodes with bit index j >= 1: one opened ring element + one j-bit bit-DCF key each (DESIGN 15)
     Atom atoms[kMaxAtoms];
     std::vector<Ins> ins;
     int n_areg = 0, n_breg = 0;

@@ -103,17 +103,36 @@ def random_spec(seed, variant=0):
 
 
 # ---- brute-force harness shared by test_oracle_gate.py / test_oracle_sp.py ------------------------------------------
+_PMAP_JOB = None        # (fn, items) of the running pmap: forked workers inherit it, so closures need no pickling
+
+
+def _pmap_call(i):
+    fn, items = _PMAP_JOB
+    return fn(items[i])
+
+
 def pmap(fn, items, workers=None):
-    """Run fn over items on a thread pool.  The oracle is plain single-threaded C behind ctypes, which releases the GIL for
-    the duration of every call, and it keeps no mutable global state after orc_compile() (its AES tables are filled
-    there), so independent calls run on all host cores.  This is what makes the exhaustive pins affordable; the
-    oracle's arithmetic itself stays single-threaded.  Exceptions (assertion failures) propagate."""
+    """Run fn over items on all host cores.  The oracle is plain single-threaded C behind ctypes and keeps no mutable global
+    state after orc_compile() (its AES tables are filled there), so independent calls can run side by side; this is what makes
+    the exhaustive pins affordable -- the oracle's arithmetic itself stays single-threaded.  Workers are FORKED processes (they
+    inherit the compiled program and the closure; the numpy checks around each oracle call would serialise threads on the GIL);
+    where fork is unavailable, a thread pool (ctypes releases the GIL during the C calls).  Exceptions (assertion failures)
+    propagate; results come back in order."""
+    global _PMAP_JOB
+    import multiprocessing as mp
     import os
-    from concurrent.futures import ThreadPoolExecutor
     items = list(items)
     workers = workers or min(len(items), os.cpu_count() or 1)
-    if workers <= 1:
+    if workers <= 1 or _PMAP_JOB is not None:                  # serial, or already inside a worker
         return [fn(it) for it in items]
+    if "fork" in mp.get_all_start_methods():
+        _PMAP_JOB = (fn, items)
+        try:
+            with mp.get_context("fork").Pool(workers) as pool:
+                return pool.map(_pmap_call, range(len(items)), chunksize=max(1, len(items) // (4 * workers)))
+        finally:
+            _PMAP_JOB = None
+    from concurrent.futures import ThreadPoolExecutor
     with ThreadPoolExecutor(max_workers=workers) as ex:
         return list(ex.map(fn, items))
 

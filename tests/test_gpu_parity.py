@@ -135,6 +135,11 @@ SMALL_DENSE = [(lambda mk=mk: specs.dense_table(mk())) for mk in SMALL[:4] + SMA
               [lambda: specs.early_termination(specs.dense_table(specs.shift_relu(8, 3))), lambda: specs.input_masked_mul(specs.dense_table(specs.toy(8, 3)))]
 
 
+# the A2B node (DESIGN 15): bit 0 local, bits j >= 1 through a masked opening and a j-bit comparison key
+SMALL_A2B = [lambda: specs.a2b_demo(8, 3), lambda: specs.shared_prefix(specs.a2b_demo(8, 3)), lambda: specs.early_termination(specs.a2b_demo(8, 3)),
+             lambda: specs.early_termination(specs.shared_prefix(specs.a2b_demo(12, 4))), lambda: specs.input_masked_mul(specs.a2b_demo(12, 4))]
+
+
 @pytest.fixture
 def knobs(F):
     """fusefss_debug_set knobs, restored after the test"""
@@ -145,7 +150,7 @@ def knobs(F):
     F.debug_set("force_g", 0); F.debug_set("small_kernels", 1); F.debug_set("eval_threads", 1024)
 
 
-@pytest.mark.parametrize("mk", SMALL + SMALL_SP + SMALL_XM + SMALL_XP + SMALL_ET + SMALL_DENSE)
+@pytest.mark.parametrize("mk", SMALL + SMALL_SP + SMALL_XM + SMALL_XP + SMALL_ET + SMALL_DENSE + SMALL_A2B)
 @pytest.mark.parametrize("mode", ["auto", "g1", "g2_big"])
 def test_small_rings_all_masks(F, orc, mk, mode, knobs):
     """Every mask r (both Protocol 3 branches, incl. beta_0 = 0 and the dummy split) at n <= 8; a ragged count.
@@ -204,6 +209,26 @@ def test_dense_table_relu16(F, orc):
     inp["x"][:4] = np.array([0, 1 << 15, (1 << 15) - 1, (1 << 16) - 1], dtype=np.uint64)
     inp["r_in"][4:8] = np.array([0, 1, (1 << 16) - 1, 1 << 15], dtype=np.uint64)
     _parity(F, orc, spec, inp["x"], inp["r_in"], inp["r_out"], seed=3)
+
+
+@pytest.mark.parametrize("variant", [0, 1, 8, 9])
+def test_a2b_n64(F, orc, variant):
+    """A2B nodes on the 64-bit ring (63-, 12- and 1-bit comparison keys inside the post-processing kernels), several tiles and a
+    ragged tail; x on the interval boundaries and around the sign change."""
+    spec = specs.a2b_demo(64, 12)
+    if variant & 1:
+        spec = specs.shared_prefix(spec)
+    if variant & 8:
+        spec = specs.early_termination(spec)
+    rng = np.random.default_rng(21)
+    u = lambda k: rng.integers(0, 1 << 63, size=k, dtype=np.uint64) * np.uint64(2) + rng.integers(0, 2, size=k, dtype=np.uint64)
+    count = 333
+    x, r_in = u(count), u(count)
+    a = np.array(spec.alpha, dtype=np.uint64)
+    edge = np.concatenate([a, a - np.uint64(1), np.array([0, 1, 2**63, 2**63 - 1, 2**64 - 1], dtype=np.uint64)])
+    x[: edge.size] = edge
+    r_in[edge.size: edge.size + 3] = np.array([0, 2**64 - 1, 2**63], dtype=np.uint64)
+    _parity(F, orc, spec, x, r_in, u(count), seed=6)
 
 
 @pytest.mark.parametrize("variant", [0, 1])
