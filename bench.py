@@ -157,11 +157,13 @@ def run_reference(args, rank):
         if i >= args.warmup:
             vals.append(sample / v)
     value = sample * len(vals) / sum(vals)
-    from workloads import tensors
+    from workloads import specs, tensors
+    spec = specs.CONFIGS[args.workload]()
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": "elements/s", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(vals) / len(vals),
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
-            "config": {"workload": f"{args.workload} count={tensors.FULL_COUNT[args.workload]}", "sample": f"first {sample} elements per step"},
+            "config": {"workload": f"{args.workload} n={spec.n} f={spec.f} count={args.count or tensors.FULL_COUNT[args.workload]}",
+                       "construction": "variant 0 (the paper's Protocol 3)", "sample": f"first {sample} elements per step"},
             "cpu_baseline": {"value": value, "unit": "elements/s", "cores": cores, "kind": "oracle",
                              "sample": f"{sample} elements of {args.workload} per step, whole gate (keygen + eval both parties + post), {cores} threads over elements"},
             "e2e": {"value": value, "unit": "elements/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}

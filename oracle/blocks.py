@@ -10,6 +10,18 @@ import numpy as np
 import oracle
 
 SLOT_MUL_AB, SLOT_MUL_AB0, SLOT_MUL_C0 = 0xA000, 0xA001, 0xA002
+BLOCK_SOFTMAX, BLOCK_LAYERNORM = 1, 2
+
+
+def stage_seed(seed, block, stage):
+    """Dealer seed of stage `stage` of a block instance (DESIGN 12): a counter-based derivation -- the splitmix64 output function
+    applied to seed + golden * (16 block + stage + 1) -- so that stages of one block, and the softmax and LayerNorm blocks keyed with
+    the same block seed, draw unrelated randomness (seed + small offsets collided across blocks)."""
+    m = (1 << 64) - 1
+    z = (int(seed) + 0x9E3779B97F4A7C15 * (16 * block + stage + 1)) & m
+    z = ((z ^ (z >> 30)) * 0xBF58476D1CE4E5B9) & m
+    z = ((z ^ (z >> 27)) * 0x94D049BB133111EB) & m
+    return z ^ (z >> 31)
 
 
 def gate(P, x0, x1, r_in, seed, first=0, offset=0, r_out=None, opened=False):
@@ -46,14 +58,15 @@ def softmax(progs, x0, x1, masks, rows, cols, seed, fused_open=False):
     fused_open: nExp and Recip are mask_output gates keyed with r_out = the following truncation gate's r_in; their opened
     yhat is that gate's xhat (then out['e'], out['t'] are shares of the MASKED values)."""
     fo = fused_open
+    SS = lambda stage: stage_seed(seed, BLOCK_SOFTMAX, stage)
     with np.errstate(over="ignore"):
-        e0, e1, _ = gate(progs["nexp"], x0, x1, masks["nexp"], seed + 1, r_out=masks["tr_e"] if fo else None)
-        f0, f1, _ = gate(progs["tr_e"], e0, e1, masks["tr_e"], seed + 2, opened=fo)
+        e0, e1, _ = gate(progs["nexp"], x0, x1, masks["nexp"], SS(1), r_out=masks["tr_e"] if fo else None)
+        f0, f1, _ = gate(progs["tr_e"], e0, e1, masks["tr_e"], SS(2), opened=fo)
         s0, s1 = f0.reshape(rows, cols).sum(axis=1, dtype=np.uint64), f1.reshape(rows, cols).sum(axis=1, dtype=np.uint64)
-        t0, t1, _ = gate(progs["recip"], s0, s1, masks["recip"], seed + 3, r_out=masks["tr_t"] if fo else None)
-        u0, u1, _ = gate(progs["tr_t"], t0, t1, masks["tr_t"], seed + 4, opened=fo)
-        p0, p1 = beaver_mul(f0, f1, u0, u1, cols, seed + 5)
-        y0, y1, _ = gate(progs["tr_y"], p0, p1, masks["tr_y"], seed + 6)
+        t0, t1, _ = gate(progs["recip"], s0, s1, masks["recip"], SS(3), r_out=masks["tr_t"] if fo else None)
+        u0, u1, _ = gate(progs["tr_t"], t0, t1, masks["tr_t"], SS(4), opened=fo)
+        p0, p1 = beaver_mul(f0, f1, u0, u1, cols, SS(5))
+        y0, y1, _ = gate(progs["tr_y"], p0, p1, masks["tr_y"], SS(6))
     return dict(e=(e0, e1), f=(f0, f1), s=(s0, s1), t=(t0, t1), u=(u0, u1), p=(p0, p1), y=(y0, y1))
 
 
@@ -79,16 +92,17 @@ def layernorm(progs, x0, x1, masks, rows, d, seed, fused_open=False):
     """LayerNorm without affine parameters on rows of length d = 2^k at scale 2^12 (App. G: mean / variance reductions
     are linear, rsqrt is a compiled gate):  mu = ARS_k(sum x); c = x - mu; v = ARS_{k+12}(sum c^2); g = rsqrt(v) (scale
     2^48) -> ARS_24; y = ARS_24(c * g).  progs / masks: stages 'mean', 'var', 'rsqrt', 'tr_g', 'tr_y'."""
+    SS = lambda stage: stage_seed(seed, BLOCK_LAYERNORM, stage)
     with np.errstate(over="ignore"):
         rs = lambda a: a.reshape(rows, d).sum(axis=1, dtype=np.uint64)
-        m0, m1, _ = gate(progs["mean"], rs(x0), rs(x1), masks["mean"], seed + 1, offset=HALF)
+        m0, m1, _ = gate(progs["mean"], rs(x0), rs(x1), masks["mean"], SS(1), offset=HALF)
         c0, c1 = x0 - np.repeat(m0, d), x1 - np.repeat(m1, d)
-        q0, q1 = beaver_mul(c0, c1, c0, c1, 1, seed + 2)
-        v0, v1, _ = gate(progs["var"], rs(q0), rs(q1), masks["var"], seed + 3, offset=HALF)
-        g0, g1, _ = gate(progs["rsqrt"], v0, v1, masks["rsqrt"], seed + 4, r_out=masks["tr_g"] if fused_open else None)
-        h0, h1, _ = gate(progs["tr_g"], g0, g1, masks["tr_g"], seed + 5, offset=HALF, opened=fused_open)
-        p0, p1 = beaver_mul(c0, c1, h0, h1, d, seed + 6)
-        y0, y1, _ = gate(progs["tr_y"], p0, p1, masks["tr_y"], seed + 7, offset=HALF)
+        q0, q1 = beaver_mul(c0, c1, c0, c1, 1, SS(2))
+        v0, v1, _ = gate(progs["var"], rs(q0), rs(q1), masks["var"], SS(3), offset=HALF)
+        g0, g1, _ = gate(progs["rsqrt"], v0, v1, masks["rsqrt"], SS(4), r_out=masks["tr_g"] if fused_open else None)
+        h0, h1, _ = gate(progs["tr_g"], g0, g1, masks["tr_g"], SS(5), offset=HALF, opened=fused_open)
+        p0, p1 = beaver_mul(c0, c1, h0, h1, d, SS(6))
+        y0, y1, _ = gate(progs["tr_y"], p0, p1, masks["tr_y"], SS(7), offset=HALF)
     return dict(m=(m0, m1), c=(c0, c1), q=(q0, q1), v=(v0, v1), g=(g0, g1), h=(h0, h1), p=(p0, p1), y=(y0, y1))
 
 

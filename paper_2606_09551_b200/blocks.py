@@ -14,6 +14,17 @@ from . import Program, _check, _ptr, _stream, lib
 
 STAGES = ("nexp", "tr_e", "recip", "tr_t", "tr_y")
 
+_M64 = (1 << 64) - 1
+
+
+def _stage_seed(seed: int, block: int, stage: int) -> int:
+    """Per-stage dealer seed (DESIGN 12): splitmix64's finaliser over seed + 0x9E3779B97F4A7C15 (16 block + stage + 1); block 1 =
+    softmax, 2 = LayerNorm.  Keeps the stages of a block and different blocks under one block seed on unrelated randomness."""
+    z = (seed + 0x9E3779B97F4A7C15 * (16 * block + stage + 1)) & _M64
+    z = ((z ^ (z >> 30)) * 0xBF58476D1CE4E5B9) & _M64
+    z = ((z ^ (z >> 27)) * 0x94D049BB133111EB) & _M64
+    return z ^ (z >> 31)
+
 
 # gate -> gate edges: the producer is compiled with mask_output and keyed with r_out = the consumer's r_in, so that the opened
 # yhat of the producer IS the consumer's xhat (online step 6, P:237; masked-wire invariant P:89-91)
@@ -66,10 +77,10 @@ class Softmax:
     def keygen(self, masks, seed: int):
         """masks[stage] = device uint64 tensor of fresh input masks r_in for that gate instance."""
         for i, k in enumerate(STAGES):
-            st_seed = seed + (1, 2, 3, 4, 6)[i]
+            st_seed = _stage_seed(seed, 1, (1, 2, 3, 4, 6)[i])
             r_out = masks[self.edges[k]].reshape(1, -1) if k in self.edges else None     # r_out(k) = r_in(consumer)
             self.progs[k].keygen(masks[k], r_out, st_seed, 0, keys=self.keys[k])
-        _check(lib.fusefss_mul_keygen(self.n, seed + 5, 0, self.N, _ptr(self.triples[0]), _ptr(self.triples[1]), _stream()))
+        _check(lib.fusefss_mul_keygen(self.n, _stage_seed(seed, 1, 5), 0, self.N, _ptr(self.triples[0]), _ptr(self.triples[1]), _stream()))
 
     # ---- online ----------------------------------------------------------------------------------
     def _gate(self, k, x0, x1, offset=0, opened=False):
@@ -159,9 +170,9 @@ class LayerNorm(Softmax):
     def keygen(self, masks, seed: int):
         for kk, off in zip(self.LN_STAGES, (1, 3, 4, 5, 7)):
             r_out = masks[self.edges[kk]].reshape(1, -1) if kk in self.edges else None
-            self.progs[kk].keygen(masks[kk], r_out, seed + off, 0, keys=self.keys[kk])
-        _check(lib.fusefss_mul_keygen(self.n, seed + 2, 0, self.N, _ptr(self.triples_sq[0]), _ptr(self.triples_sq[1]), _stream()))
-        _check(lib.fusefss_mul_keygen(self.n, seed + 6, 0, self.N, _ptr(self.triples[0]), _ptr(self.triples[1]), _stream()))
+            self.progs[kk].keygen(masks[kk], r_out, _stage_seed(seed, 2, off), 0, keys=self.keys[kk])
+        _check(lib.fusefss_mul_keygen(self.n, _stage_seed(seed, 2, 2), 0, self.N, _ptr(self.triples_sq[0]), _ptr(self.triples_sq[1]), _stream()))
+        _check(lib.fusefss_mul_keygen(self.n, _stage_seed(seed, 2, 6), 0, self.N, _ptr(self.triples[0]), _ptr(self.triples[1]), _stream()))
 
     def run(self, x0, x1):
         H, st = self.HALF, _stream()

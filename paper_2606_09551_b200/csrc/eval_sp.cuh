@@ -52,25 +52,40 @@ __device__ __forceinline__ void sp_step(uint32_t tl, const uint4 cw, const uint6
     st.t = tnew;
 }
 
-template <int PK>
-__device__ __forceinline__ void sp_load_level(const uint8_t *pl, size_t e, size_t s16, size_t s8, uint4 &cw, uint64_t (&vcw)[PK]) {
-    cw = __ldg(reinterpret_cast<const uint4 *>(pl + e * 16));
+// Cache behaviour of a level's correction words (HINT): the levels of a cluster's shared prefix (and every level of a lone point)
+// are read exactly once per element -- streamed (ld.global.cs, evict-first); the tail levels of a cluster are re-read once per
+// point of the cluster -- kept in L2 with an evict_last policy, so that the streamed prefix levels of the other 150,000 resident
+// lanes do not push them out to DRAM between two points (profiles/r2_eval_sp.md: DRAM reads 2.2x -> 1.0x the key size).
+#ifndef FFS_SP_L2HINT
+#define FFS_SP_L2HINT 1
+#endif
+enum { SP_LD_PLAIN = 0, SP_LD_STREAM = 1, SP_LD_KEEP = 2 };
+__device__ __forceinline__ uint64_t sp_keep_policy() {
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+    return pol;
+}
+template <int HINT> __device__ __forceinline__ uint4 sp_ld16(const void *p, uint64_t pol) {
+    if (!FFS_SP_L2HINT || HINT == SP_LD_PLAIN) return __ldg(reinterpret_cast<const uint4 *>(p));
+    if (HINT == SP_LD_STREAM) return __ldcs(reinterpret_cast<const uint4 *>(p));
+    uint4 v;
+    asm volatile("ld.global.nc.L2::cache_hint.v4.u32 {%0, %1, %2, %3}, [%4], %5;" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p), "l"(pol));
+    return v;
+}
+template <int HINT> __device__ __forceinline__ uint64_t sp_ld8(const void *p, uint64_t pol) {
+    if (!FFS_SP_L2HINT || HINT == SP_LD_PLAIN) return __ldg(reinterpret_cast<const unsigned long long *>(p));
+    if (HINT == SP_LD_STREAM) return __ldcs(reinterpret_cast<const unsigned long long *>(p));
+    uint64_t v;
+    asm volatile("ld.global.nc.L2::cache_hint.u64 %0, [%1], %2;" : "=l"(v) : "l"(p), "l"(pol));
+    return v;
+}
+template <int PK, int HINT = SP_LD_PLAIN>
+__device__ __forceinline__ void sp_load_level(const uint8_t *pl, size_t e, size_t s16, size_t s8, uint4 &cw, uint64_t (&vcw)[PK], uint64_t pol = 0) {
+    cw = sp_ld16<HINT>(pl + e * 16, pol);
 #pragma unroll
-    for (int w = 0; w < PK; ++w) vcw[w] = __ldg(reinterpret_cast<const unsigned long long *>(pl + s16 + (size_t)w * s8 + e * 8));
+    for (int w = 0; w < PK; ++w) vcw[w] = sp_ld8<HINT>(pl + s16 + (size_t)w * s8 + e * 8, pol);
 }
 
-// walk levels [from, to) of the n-bit vector tree; ubits = the point with its level-`from` bit at bit 63
-template <int PK>
-__device__ __forceinline__ void sp_walk(uint32_t tl, const uint8_t *lvl, size_t e, size_t s16, size_t s8, size_t lvl_stride,
-                                        int from, int to, uint64_t ubits, SpState<PK> &st) {
-    const uint8_t *pl = lvl + (size_t)from * lvl_stride;
-    for (int i = from; i < to; ++i, pl += lvl_stride) {
-        uint4 cw; uint64_t vcw[PK];
-        sp_load_level<PK>(pl, e, s16, s8, cw, vcw);
-        sp_step<PK>(tl, cw, vcw, (uint32_t)(ubits >> 63), st);
-        ubits <<= 1;
-    }
-}
 // The two candidate prefixes u1, u2 of a cluster (top kf bits) usually differ only in their last few bits: walk u1
 // once, snapshot the state at the level where u2 leaves u1's path (per lane), then walk u2's few remaining levels.
 // On return a / b = the states after kf levels along u1 / u2 (b = a when the prefixes are equal).
@@ -84,7 +99,7 @@ __device__ __forceinline__ void sp_walk_fork(uint32_t tl, const uint8_t *lvl, si
     for (int i = 0; i < kf; ++i, pl += lvl_stride) {
         if (i == ldiv) b = a;
         uint4 cw; uint64_t vcw[PK];
-        sp_load_level<PK>(pl, e, s16, s8, cw, vcw);
+        sp_load_level<PK, SP_LD_STREAM>(pl, e, s16, s8, cw, vcw);
         sp_step<PK>(tl, cw, vcw, (uint32_t)(ub >> 63), a);
         ub <<= 1;
     }
@@ -93,7 +108,7 @@ __device__ __forceinline__ void sp_walk_fork(uint32_t tl, const uint8_t *lvl, si
     pl = lvl + (size_t)ldiv * lvl_stride;
     for (int i = ldiv; i < kf; ++i, pl += lvl_stride) {                       // per-lane trip count (expected ~2 levels)
         uint4 cw; uint64_t vcw[PK];
-        sp_load_level<PK>(pl, e, s16, s8, cw, vcw);
+        sp_load_level<PK, SP_LD_STREAM>(pl, e, s16, s8, cw, vcw);
         sp_step<PK>(tl, cw, vcw, (uint32_t)(ub >> 63), b);
         ub <<= 1;
     }
@@ -119,20 +134,20 @@ __device__ __forceinline__ void sp_leaf(uint32_t tl, const SpState<PK> &st, cons
 // the same levels of the same element's key), and the NP x (1 + QK) PRG blocks of a level are NP x (1+QK) x 16 independent
 // lookups per round -- the instruction-level parallelism a launch with only a few warps per SM lives on.  The next level's
 // words are prefetched into registers while the current level's AES runs.
-template <int PK, int NPMAX, int NP>
+template <int PK, int NPMAX, int NP, int HINT>
 __device__ __forceinline__ void sp_walk_batch(uint32_t tl, const uint8_t *lvl, size_t e, size_t s16, size_t s8, size_t lvl_stride,
-                                              int from, int to, uint64_t (&ub)[NPMAX], SpState<PK> (&st)[NPMAX]) {
+                                              int from, int to, uint64_t (&ub)[NPMAX], SpState<PK> (&st)[NPMAX], uint64_t pol) {
     constexpr int QK = (PK + 1) / 2;
     if (from >= to) return;
     const uint8_t *pl = lvl + (size_t)from * lvl_stride;
     uint4 cw; uint64_t vcw[PK];
-    sp_load_level<PK>(pl, e, s16, s8, cw, vcw);
+    sp_load_level<PK, HINT>(pl, e, s16, s8, cw, vcw, pol);
     for (int i = from; i < to; ++i) {
         pl += lvl_stride;
         uint4 cw_n = cw; uint64_t vcw_n[PK];
 #pragma unroll
         for (int w = 0; w < PK; ++w) vcw_n[w] = vcw[w];
-        if (i + 1 < to) sp_load_level<PK>(pl, e, s16, s8, cw_n, vcw_n);
+        if (i + 1 < to) sp_load_level<PK, HINT>(pl, e, s16, s8, cw_n, vcw_n, pol);
         uint32_t x[NP][4], o[NP][1 + QK][4], dbit[NP];
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
@@ -162,18 +177,22 @@ __device__ __forceinline__ void sp_walk_batch(uint32_t tl, const uint8_t *lvl, s
 }
 
 // the first nb of the NPMAX entries (nb is warp-uniform)
-template <int PK, int NPMAX>
+template <int PK, int NPMAX, int HINT>
 __device__ __forceinline__ void sp_walk_some(int nb, uint32_t tl, const uint8_t *lvl, size_t e, size_t s16, size_t s8, size_t lvl_stride,
-                                             int from, int to, uint64_t (&ub)[NPMAX], SpState<PK> (&st)[NPMAX]) {
-    if (NPMAX >= 4 && nb == 4) sp_walk_batch<PK, NPMAX, (NPMAX >= 4 ? 4 : 1)>(tl, lvl, e, s16, s8, lvl_stride, from, to, ub, st);
-    else if (NPMAX >= 3 && nb == 3) sp_walk_batch<PK, NPMAX, (NPMAX >= 3 ? 3 : 1)>(tl, lvl, e, s16, s8, lvl_stride, from, to, ub, st);
-    else if (NPMAX >= 2 && nb == 2) sp_walk_batch<PK, NPMAX, (NPMAX >= 2 ? 2 : 1)>(tl, lvl, e, s16, s8, lvl_stride, from, to, ub, st);
-    else sp_walk_batch<PK, NPMAX, 1>(tl, lvl, e, s16, s8, lvl_stride, from, to, ub, st);
+                                             int from, int to, uint64_t (&ub)[NPMAX], SpState<PK> (&st)[NPMAX], uint64_t pol) {
+    if (NPMAX >= 4 && nb == 4) sp_walk_batch<PK, NPMAX, (NPMAX >= 4 ? 4 : 1), HINT>(tl, lvl, e, s16, s8, lvl_stride, from, to, ub, st, pol);
+    else if (NPMAX >= 3 && nb == 3) sp_walk_batch<PK, NPMAX, (NPMAX >= 3 ? 3 : 1), HINT>(tl, lvl, e, s16, s8, lvl_stride, from, to, ub, st, pol);
+    else if (NPMAX >= 2 && nb == 2) sp_walk_batch<PK, NPMAX, (NPMAX >= 2 ? 2 : 1), HINT>(tl, lvl, e, s16, s8, lvl_stride, from, to, ub, st, pol);
+    else sp_walk_batch<PK, NPMAX, 1, HINT>(tl, lvl, e, s16, s8, lvl_stride, from, to, ub, st, pol);
 }
 
-#ifndef FFS_SP_NP_BIG
-#define FFS_SP_NP_BIG 1          // points walked in lock-step by the 1024-thread instantiation (64 registers per thread)
+#ifndef FFS_SP_THREADS
+#define FFS_SP_THREADS 1024      // CTA size of the large launches of k_eval_sp (registers per thread = 65536 / this)
 #endif
+#ifndef FFS_SP_NP_BIG
+#define FFS_SP_NP_BIG 1          // points walked in lock-step by the large-launch instantiation
+#endif
+constexpr int kEvalSpThreads = FFS_SP_THREADS;
 #ifndef FFS_SP_NP_SMALL
 #define FFS_SP_NP_SMALL 2        // ... by the 256-thread instantiation (255 registers per thread)
 #endif
@@ -182,6 +201,7 @@ template <int P, int PK, int THREADS>
 __global__ void __launch_bounds__(THREADS, 1) k_eval_sp(const __grid_constant__ EvalSpArgs a) {
     extern __shared__ uint32_t sT[];
     const uint32_t tl = aes_fill_tables(sT);
+    const uint64_t keep_pol = sp_keep_policy();
     if (a.zero_first) zero_outputs_and_sync(a.bits_out2, true, a.coeff_out2, true, a.count, P);
     const size_t tiles = (a.count + 31) / 32, items = tiles * (size_t)a.G * (size_t)a.n_parties, warps = (size_t)gridDim.x * (blockDim.x >> 5);
     // warp w of CTA b takes items w*grid + b (+ k*warps): a partial last wave spreads evenly over all SMs
@@ -288,7 +308,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_eval_sp(const __grid_constant__ 
                         st[q] = r0;
                         ub[q] = ((xh + pts[jq[q < nb ? q : 0]].delta) & a.mask) << (64 - n);
                     }
-                    sp_walk_some<PK, NP>(nb, tl, lvl, e, a.s16, a.s8, a.lvl_stride, 0, n, ub, st);
+                    sp_walk_some<PK, NP, SP_LD_STREAM>(nb, tl, lvl, e, a.s16, a.s8, a.lvl_stride, 0, n, ub, st, 0);
 #pragma unroll
                     for (int q = 0; q < NP; ++q) if (q < nb) fold(jq[q], st[q]);
                     nb = 0;
@@ -335,7 +355,7 @@ __global__ void __launch_bounds__(THREADS, 1) k_eval_sp(const __grid_constant__ 
                         st[q] = (u >> (64 - kf)) == pre1 ? s1 : s2;
                         ub[q] = u << kf;
                     }
-                    sp_walk_some<PK, NP>(nb, tl, lvl, e, a.s16, a.s8, a.lvl_stride, kf, n, ub, st);
+                    sp_walk_some<PK, NP, SP_LD_KEEP>(nb, tl, lvl, e, a.s16, a.s8, a.lvl_stride, kf, n, ub, st, keep_pol);
 #pragma unroll
                     for (int q = 0; q < NP; ++q) if (q < nb) fold(jq[q], st[q]);
                 }

@@ -254,7 +254,7 @@ int launch_eval_sp(const Program &P, int party, const void *const key[2], const 
     // extra group re-walks the shared prefixes), so time ~ chain(G) * max(1, warps / (4 #SMs)).  Smallest G at the minimum.
     const size_t units_sp = tiles * (size_t)a.n_parties;
     int G = 1;
-    if (units_sp < (size_t)g_sms * (kEvalThreads / 32)) {
+    if (units_sp < (size_t)g_sms * (kEvalSpThreads / 32)) {
         double best = 0;
         for (int g = 1; g <= maxpts; ++g) {
             double chain = 0; int singles = 0;
@@ -277,13 +277,14 @@ int launch_eval_sp(const Program &P, int party, const void *const key[2], const 
     a.zero_first = G > 1;
     const size_t items = tiles * (size_t)G * (size_t)a.n_parties;
     const bool small = small_launch(items);
-    const int threads = small ? kEvalThreadsSmall : threads_for(items, g_eval_threads.load());
+    const int cap_sp = g_eval_threads.load() < kEvalSpThreads ? g_eval_threads.load() : kEvalSpThreads;
+    const int threads = small ? kEvalThreadsSmall : threads_for(items, cap_sp);
     const int grid = small ? (int)(items < (size_t)g_sms ? items : (size_t)g_sms) : grid_for(items, threads);   // small: spread the warps over ALL SMs
     const size_t sm = kAesSmemBytes;
     a.rpow = L.rpow;
     const bool coop = a.zero_first != 0;
 #define FSK_SP_CASE(PP, KK) if (P.p == PP && P.sp.pk == KK) return small ? launch(k_eval_sp<PP, KK, kEvalThreadsSmall>, grid, threads, sm, st, a, coop) \
-                                                                         : launch(k_eval_sp<PP, KK, kEvalThreads>, grid, threads, sm, st, a, coop);
+                                                                         : launch(k_eval_sp<PP, KK, kEvalSpThreads>, grid, threads, sm, st, a, coop);
 #define FSK_SP_ROW(KK) FSK_SP_CASE(1, KK) FSK_SP_CASE(2, KK) FSK_SP_CASE(3, KK) FSK_SP_CASE(4, KK) FSK_SP_CASE(5, KK) \
                        FSK_SP_CASE(6, KK) FSK_SP_CASE(7, KK) FSK_SP_CASE(8, KK)
     FSK_SP_ROW(1) FSK_SP_ROW(2) FSK_SP_ROW(3)

@@ -111,8 +111,9 @@ def _pmap_call(i):
     return fn(items[i])
 
 
-def pmap(fn, items, workers=None):
-    """Run fn over items on all host cores.  The oracle is plain single-threaded C behind ctypes and keeps no mutable global
+def pmap(fn, items, workers=None, threads=False):
+    """Run fn over items on all host cores (threads=True: a thread pool -- for callers that hold a CUDA context, which must not
+    be forked).  The oracle is plain single-threaded C behind ctypes and keeps no mutable global
     state after orc_compile() (its AES tables are filled there), so independent calls can run side by side; this is what makes
     the exhaustive pins affordable -- the oracle's arithmetic itself stays single-threaded.  Workers are FORKED processes (they
     inherit the compiled program and the closure; the numpy checks around each oracle call would serialise threads on the GIL);
@@ -125,11 +126,15 @@ def pmap(fn, items, workers=None):
     workers = workers or min(len(items), os.cpu_count() or 1)
     if workers <= 1 or _PMAP_JOB is not None:                  # serial, or already inside a worker
         return [fn(it) for it in items]
-    if "fork" in mp.get_all_start_methods():
+    if not threads and "fork" in mp.get_all_start_methods():
         _PMAP_JOB = (fn, items)
+        import warnings
         try:
-            with mp.get_context("fork").Pool(workers) as pool:
-                return pool.map(_pmap_call, range(len(items)), chunksize=max(1, len(items) // (4 * workers)))
+            with warnings.catch_warnings():
+                # the parent may hold idle library threads (BLAS, torch); the workers only call the oracle's C and element-wise numpy
+                warnings.filterwarnings("ignore", message=".*multi-threaded, use of fork.*", category=DeprecationWarning)
+                with mp.get_context("fork").Pool(workers) as pool:
+                    return pool.map(_pmap_call, range(len(items)), chunksize=max(1, len(items) // (4 * workers)))
         finally:
             _PMAP_JOB = None
     from concurrent.futures import ThreadPoolExecutor

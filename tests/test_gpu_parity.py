@@ -7,7 +7,7 @@ import os
 import numpy as np
 import pytest
 
-from helpers import mask_of, pack_bits
+from helpers import mask_of, pack_bits, pmap
 from workloads import specs, tensors
 
 pytestmark = pytest.mark.gpu
@@ -286,10 +286,10 @@ FULL = [("relu16", 0), ("relu16", 1), ("relu16", 8), ("shift_relu", 8), ("shift_
 @pytest.mark.parametrize("name,variant", FULL)
 def test_full_size_sampled(F, orc, name, variant):
     """Every BASELINE.json config at its FULL size in the launch configuration bench.py times (keygen in its three
-    parts, one eval per party -- fused for variant 1 --, post_fused; config 5 / variant 0 as one 704,512-element chunk
-    at a non-zero global offset, as in the chunked run).  The oracle recomputes a sample of elements one by one
-    (its keygen is deterministic in the GLOBAL element index), and the reconstruction property G(x) is checked on a
-    20,000-element prefix."""
+    parts, fusefss_eval_fused_both, post_fused; config 5 / variant 0 as one 704,512-element chunk at a non-zero global
+    offset, as in the chunked run -- test_silu_all_chunks covers every chunk).  The oracle recomputes a sample of several
+    hundred elements one by one on all host cores (its keygen is deterministic in the GLOBAL element index), and the
+    reconstruction property G(x) is checked on a 20,000-element prefix."""
     import gc
     import torch
     gc.collect()
@@ -317,36 +317,94 @@ def test_full_size_sampled(F, orc, name, variant):
     k0, k1 = keys
     xh = dev(xhat)
     T, lut = P.shape["T"], P.shape["has_lut"]
-    if variant & 1:
-        ev = [P.eval_fused(b, (k0, k1)[b], xh) for b in (0, 1)]
-        bits, coeff = [ev[0][0], ev[1][0]], [ev[0][1], ev[1][1]]
-    else:
-        bits = [P.eval_cmp(b, (k0, k1)[b], xh) if T else None for b in (0, 1)]
-        coeff = [P.eval_lut(b, (k0, k1)[b], xh) if lut else None for b in (0, 1)]
+    bits, coeff = P.eval_fused_both(k0, k1, xh)              # ONE launch: both parties, both FSS calls (what bench.py times)
     y0, y1, z0, z1 = P.post_fused(k0, k1, xh, bits[0], bits[1], coeff[0], coeff[1])
     torch.cuda.synchronize()
+    # the oracle recomputes a sample element by element on all host cores (its keygen is deterministic in the GLOBAL index):
+    # the tile edges at both ends, a 96-element run across the middle, and a few hundred random elements
     rng = np.random.default_rng(1)
-    n_s = 24 if name == "silu" else 40
-    idx = np.unique(np.concatenate([[0, 31, 32, count - 1, count - 33], rng.integers(0, count, n_s)]))
+    n_s = {"silu": 160, "gelu": 320, "nexp": 320}.get(name, 480)
+    mid = count // 2 // 32 * 32
+    idx = np.unique(np.concatenate([[0, 1, 31, 32, 33, count - 1, count - 2, count - 33], np.arange(mid - 48, mid + 48), rng.integers(0, count, n_s)]))
     idx = idx[(idx >= 0) & (idx < count)]
-    for e in idx:
+    hb = [host(t) if t is not None else None for t in bits]
+    hc = [host(t) if t is not None else None for t in coeff]
+    hy, hz = [host(y0), host(y1)], [host(z0), host(z1)]
+
+    def one(e):
         e = int(e)
         ok0, ok1 = O.keygen(r_in[e:e + 1], r_out[:, e:e + 1], 0, first_elem=first + e)
         exp = O.run_gate(ok0, ok1, xhat[e:e + 1])
-        for b, (bb, cc, yy, zz) in enumerate(((bits[0], coeff[0], y0, z0), (bits[1], coeff[1], y1, z1))):
+        for b in (0, 1):
             if T:
-                assert host(bb[e:e + 1])[0] == exp["bits"][b][0], (name, variant, e)
+                assert hb[b][e] == exp["bits"][b][0], (name, variant, e)
             if lut:
-                assert np.array_equal(host(cc[:, e:e + 1].contiguous())[:, 0], exp["coeff"][b][:, 0]), (name, variant, e)
-            assert host(yy[0, e:e + 1])[0] == exp["y"][b][0, 0], (name, variant, e)
+                assert np.array_equal(hc[b].reshape(P.shape["p"], -1)[:, e], exp["coeff"][b][:, 0]), (name, variant, e)
+            assert hy[b].reshape(-1, count)[0, e] == exp["y"][b][0, 0], (name, variant, e)
             if P.shape["n_out_b"]:
-                assert host(zz[e:e + 1])[0] == exp["z"][b][0], (name, variant, e)
+                assert hz[b][e] == exp["z"][b][0], (name, variant, e)
+    pmap(one, idx, threads=True)
     # property at full size: shares reconstruct to the plaintext operator on a prefix
     k = min(20000, count)
     ye, ze = O.plain_G(x[:k], r_in[:k])
     assert np.array_equal((host(y0)[0, :k] + host(y1)[0, :k]) & mask_of(spec.n), ye[0])
     if P.shape["n_out_b"]:
         assert np.array_equal(host(z0)[:k] ^ host(z1)[:k], pack_bits(ze))
+
+
+def test_silu_all_chunks(F, orc):
+    """config 5 (SiLU, 22,544,384 elements, Protocol 3) exactly as bench.py streams it: 32 chunks of 704,512 elements through ONE
+    pair of key buffers (overwritten per chunk), global element indices.  From every chunk the first and last tile edges and a few
+    random elements are kept and recomputed by the oracle one by one (~700 elements across all 31 chunk boundaries); the
+    reconstruction property G(x) is checked on a 65,536-element stride sample of the whole tensor."""
+    import gc
+    import torch
+    gc.collect()
+    torch.cuda.empty_cache()
+    spec = specs.CONFIGS["silu"]()
+    total, chunk = tensors.FULL_COUNT["silu"], 704512
+    inp = tensors.inputs("silu", spec, count=total, seed=0)
+    P, O = F.Program(spec), orc.Program(spec)
+    k0, k1 = P.alloc_keys(chunk)
+    rng = np.random.default_rng(7)
+    stride = total // 65536
+    keep_idx, keep = [], {"bits": [[], []], "coeff": [[], []], "y": [[], []], "z": [[], []]}
+    prop_y, prop_z, prop_idx = [], [], []
+    for first in range(0, total, chunk):
+        c = min(chunk, total - first)
+        sl = slice(first, first + c)
+        r_in, r_out, xh = dev(inp["r_in"][sl]), dev(np.ascontiguousarray(inp["r_out"][:, sl])), dev(inp["xhat"][sl])
+        P.keygen(r_in, r_out, 0, first, keys=(k0, k1))
+        bits, coeff = P.eval_fused_both(k0, k1, xh)
+        y0, y1, z0, z1 = P.post_fused(k0, k1, xh, bits[0], bits[1], coeff[0], coeff[1])
+        loc = np.unique(np.concatenate([[0, 1, 31, 32, c - 33, c - 32, c - 2, c - 1], rng.integers(0, c, 14)]))
+        li = torch.from_numpy(loc).cuda()
+        keep_idx.append(first + loc)
+        for b, (bb, cc, yy, zz) in enumerate(((bits[0], coeff[0], y0, z0), (bits[1], coeff[1], y1, z1))):
+            keep["bits"][b].append(host(bb[li])); keep["coeff"][b].append(host(cc[:, li].contiguous()))
+            keep["y"][b].append(host(yy[0, li])); keep["z"][b].append(host(zz[li]))
+        pl = np.arange((-first) % stride, c, stride)
+        pi = torch.from_numpy(pl).cuda()
+        prop_idx.append(first + pl)
+        prop_y.append((host(y0[0, pi]) + host(y1[0, pi])) & mask_of(spec.n)); prop_z.append(host(z0[pi]) ^ host(z1[pi]))
+    torch.cuda.synchronize()
+    idx = np.concatenate(keep_idx)
+    got = {k: [np.concatenate(v[b], axis=-1) for b in (0, 1)] for k, v in keep.items()}
+
+    def one(i):
+        e = int(idx[i])
+        ok0, ok1 = O.keygen(inp["r_in"][e:e + 1], np.ascontiguousarray(inp["r_out"][:, e:e + 1]), 0, first_elem=e)
+        exp = O.run_gate(ok0, ok1, inp["xhat"][e:e + 1])
+        for b in (0, 1):
+            assert got["bits"][b][i] == exp["bits"][b][0], (e, "bits")
+            assert np.array_equal(got["coeff"][b][:, i], exp["coeff"][b][:, 0]), (e, "coeff")
+            assert got["y"][b][i] == exp["y"][b][0, 0], (e, "y")
+            assert got["z"][b][i] == exp["z"][b][0], (e, "z")
+    pmap(one, range(idx.size), threads=True)
+    pidx = np.concatenate(prop_idx)
+    ye, ze = O.plain_G(inp["x"][pidx], inp["r_in"][pidx])
+    assert np.array_equal(np.concatenate(prop_y), ye[0])
+    assert np.array_equal(np.concatenate(prop_z), pack_bits(ze))
 
 
 @pytest.mark.parametrize("variant", [0, 1, 5])
