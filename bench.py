@@ -257,6 +257,60 @@ class Gate:
                 events.append(e)
 
 
+def _graph_of(torch, fn):
+    """capture fn (library calls on torch's current stream) in a CUDA graph, after two eager warm-up calls on a side stream"""
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        for _ in range(2):
+            fn()
+    torch.cuda.current_stream().wait_stream(s)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        fn()
+    return g
+
+
+def _timed_graph(torch, g, flush, warmup, steps, median=False):
+    """mean (or median) ms of `steps` replays, each bracketed by its own event pair with an L2 flush (a write larger than L2) before it"""
+    for _ in range(warmup):
+        g.replay()
+    ts = []
+    for _ in range(steps):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); g.replay(); b.record()
+        ts.append((a, b))
+    torch.cuda.synchronize()
+    v = sorted(a.elapsed_time(b) for a, b in ts)
+    return v[len(v) // 2] if median else sum(v) / steps
+
+
+def small_sweep(F, torch):
+    """--small-sweep: evaluation latency of BASELINE's small tensors against the forced number of warps an element's trees / points
+    are dealt to (fusefss_debug_set force_g, sp_np) and the library's automatic choice; one JSON line per (tensor, construction).
+    Evidence for the launch-geometry model in launch_eval_sp / pick_groups (profiles/r2e_small_sweep.md)."""
+    from workloads import tensors
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    for name in ("recip", "rsqrt", "relu16"):
+        for variant in (1, 0):
+            gate = Gate(F, torch, name, variant, tensors.FULL_COUNT[name], seed=0)
+            gate.keygen(0, 7)
+            run = lambda: _timed_graph(torch, _graph_of(torch, lambda: gate.evaluate(0)), flush, 3, 20, median=True)
+            F.debug_set("force_g", 0); F.debug_set("sp_np", 0)
+            line = {"name": name, "variant": variant, "count": gate.count, "auto_us": round(run() * 1e3, 1), "forced": {}}
+            gmax = 20 if variant else max(gate.sh["M"] - 1, gate.sh["T"], 1)
+            for g in range(1, gmax + 1):
+                F.debug_set("force_g", g)
+                for np_ in ((1, 2) if variant else (0,)):
+                    F.debug_set("sp_np", np_)
+                    line["forced"]["G%d_np%d" % (g, np_)] = round(run() * 1e3, 1)
+            F.debug_set("force_g", 0); F.debug_set("sp_np", 0)
+            print(json.dumps(line), flush=True)
+            gate.free()
+
+
 def measure(gate, M, steps, warmup, barrier, allmax, world=1, clocks_index=None):
     """Times `steps` steps of `gate`.  Large tensors: K steps inside one bracket (barrier + synchronize on both sides), per-kernel
     CUDA events inside.  Small tensors (<= SMALL_COUNT elements): the step is captured in a CUDA graph (launch-bound otherwise),
@@ -296,30 +350,8 @@ def measure(gate, M, steps, warmup, barrier, allmax, world=1, clocks_index=None)
     else:
         flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
 
-        def graph_of(fn):
-            s = torch.cuda.Stream()
-            s.wait_stream(torch.cuda.current_stream())
-            with torch.cuda.stream(s):
-                for _ in range(2):
-                    fn()
-            torch.cuda.current_stream().wait_stream(s)
-            torch.cuda.synchronize()
-            g = torch.cuda.CUDAGraph()
-            with torch.cuda.graph(g):
-                fn()
-            return g
-
-        def timed(g):
-            for _ in range(warmup):
-                g.replay()
-            ts = []
-            for _ in range(steps):
-                flush.zero_()
-                a, b = ev(), ev()
-                a.record(); g.replay(); b.record()
-                ts.append((a, b))
-            torch.cuda.synchronize()
-            return sum(a.elapsed_time(b) for a, b in ts) / steps
+        graph_of = lambda fn: _graph_of(torch, fn)
+        timed = lambda g: _timed_graph(torch, g, flush, warmup, steps)
         held = {}
 
         def ev_fn():
@@ -464,6 +496,7 @@ def main():
     ap.add_argument("--no-configs", action="store_true", help="skip the other BASELINE tensors")
     ap.add_argument("--no-probes", action="store_true")
     ap.add_argument("--blocks", action="store_true", help="also time the softmax / LayerNorm vector blocks")
+    ap.add_argument("--small-sweep", action="store_true", help="sweep the launch geometry of the small tensors' evaluation call (tuning evidence) and exit")
     ap.add_argument("--two-party", action="store_true", help="N = 2: party b on GPU b, real exchange of the opening buffers (two_party.run_party)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)                               # timing rule: W >= 3
@@ -513,6 +546,9 @@ def main():
         torch.cuda.synchronize()
 
     M = Machine(torch, local)
+    if args.small_sweep:
+        small_sweep(F, torch)
+        return
     if args.two_party:
         from paper_2606_09551_b200 import two_party
         line = two_party.bench(F, torch, dist, args, rank, world, M)

@@ -125,7 +125,8 @@ size_t fusefss_key_bytes(const fusefss_program *prog, size_t count);
 
 /* ---- a1-a4: keygen (dealer; section 5.2; Protocol 3 steps (1),(5)) ----
  * r_in_dev[count]: fresh uniform input masks; r_out_dev[n_out_a][count]: output masks (may be NULL unless
- * mask_output).  seed: the dealer's randomness seed (DESIGN 4.5).  first_elem: GLOBAL index of element 0 of
+ * mask_output).  seed: the dealer's randomness seed (DESIGN 4.5) -- a reproducibility handle with 64 bits of entropy, one per
+ * gate instance; a deployment draws the dealer's 128-bit AES key from a CSPRNG instead.  first_elem: GLOBAL index of element 0 of
  * this chunk -- randomness is derived from the global index, so chunked keygen equals one-shot keygen.
  * Writes both parties' key buffers (fusefss_key_bytes() each, 256-byte aligned device memory). */
 int fusefss_keygen(const fusefss_program *prog, const uint64_t *r_in_dev, const uint64_t *r_out_dev,
@@ -237,7 +238,8 @@ const char *fusefss_strerror(int code);
 const char *fusefss_last_cuda_error(void);
 /* Test / tuning knobs (process-wide, not part of the method): "force_g" = v >= 1 forces the number of warps the trees / points of an
  * element are dealt to (0 = automatic); "eval_threads" = CTA size of the large evaluation launches (default 1024); "small_kernels"
- * = 0 disables the 256-thread instantiations used for small launches.  Unknown knob: FUSEFSS_E_DEBUG. */
+ * = 0 disables the 256-thread instantiations used for small launches; "sp_np" = points the single-key evaluation walks in lock-step per
+ * warp (0 = automatic).  Unknown knob: FUSEFSS_E_DEBUG. */
 int fusefss_debug_set(const char *knob, long value);
 /* number of kernel launches this library has issued since load (bench.py's gpu_launches) */
 uint64_t fusefss_launch_count(void);

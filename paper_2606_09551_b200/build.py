@@ -19,7 +19,9 @@ def deps():
 
 def build(force: bool = False, verbose: bool = False, extra=()) -> str:
     newest = max(os.path.getmtime(d) for d in deps())
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest:
+    flags_file, want = LIB + ".flags", " ".join(extra)
+    have = open(flags_file).read() if os.path.exists(flags_file) else ""
+    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= newest and have == want:   # up to date AND built with these switches
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-shared",
@@ -28,9 +30,13 @@ def build(force: bool = False, verbose: bool = False, extra=()) -> str:
         cmd += ["-Xptxas", "-v"]
     cmd += list(extra) + [os.path.join(_CSRC, s) for s in SOURCES]
     subprocess.check_call(cmd)
+    with open(flags_file, "w") as f:
+        f.write(want)
     return LIB
 
 
 if __name__ == "__main__":
+    # python paper_2606_09551_b200/build.py [-v] [-DNAME=VALUE ...]   (the -D switches: tuning macros such as FFS_SP_THREADS,
+    # FFS_P3_THREADS, FFS_SP_NP_BIG, FFS_SP_L2HINT -- see profiles/r2d_eval_sp_sweep.md; a plain build() restores the defaults)
     import sys
-    print(build(force=True, verbose="-v" in sys.argv))
+    print(build(force=True, verbose="-v" in sys.argv, extra=[a for a in sys.argv[1:] if a.startswith("-D")]))

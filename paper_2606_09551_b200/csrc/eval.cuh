@@ -20,6 +20,15 @@
 namespace fsk {
 
 constexpr int kEvalThreads = 1024;     // large launches: 32 warps per SM hide every latency at 64 registers per thread
+// CTA size of the large k_eval_p3 launches (registers per thread = 65536 / this), chosen per payload width by measurement
+// (profiles/r2f_p3_threads.md): with p >= 2 a level expands 1 + ceil(p/2) >= 2 blocks in lock-step and keeps p 64-bit accumulators and p
+// correction words live -- 64 registers spill; 512 threads x 128 registers run 2-3 % faster (gelu / nexp / silu).  p = 1 (shift_relu) has
+// one payload block and is faster with 32 warps.  -DFFS_P3_THREADS=N forces one size for every p.
+#ifdef FFS_P3_THREADS
+constexpr int p3_threads_for(int) { return FFS_P3_THREADS; }
+#else
+constexpr int p3_threads_for(int p) { return p >= 2 ? 512 : 1024; }
+#endif
 constexpr int kEvalThreadsSmall = 256; // small launches (a few warps per SM): 255 registers per thread let ptxas schedule a round's lookups back to back
 
 struct CmpAtomDev { uint64_t c; uint64_t root_off, cw_off, vb_off; int k; int pad; };

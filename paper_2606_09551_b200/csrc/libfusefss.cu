@@ -202,7 +202,7 @@ int launch_eval_p3(const Program &P, int party, const void *const key[2], const 
     const size_t tiles = (count + 31) / 32, units = tiles * (size_t)a.n_slots;
     const size_t max_items = units * (size_t)((want_cmp ? P.T : 0) + (want_lut ? P.M - 1 : 0));
     const bool small = small_launch(max_items);
-    const int cap = small ? kEvalThreadsSmall : g_eval_threads.load();
+    const int cap = small ? kEvalThreadsSmall : (g_eval_threads.load() < p3_threads_for(P.p) ? g_eval_threads.load() : p3_threads_for(P.p));
     if (small) {                                   // every tree on its own warp: the chain of one tree is the critical path
         a.Gc = want_cmp ? P.T : 1; a.Gl = want_lut ? P.M - 1 : 1;
         if (const int f = g_force_g.load()) { a.Gc = f < a.Gc ? f : a.Gc; a.Gl = f < a.Gl ? f : a.Gl; }
@@ -217,7 +217,7 @@ int launch_eval_p3(const Program &P, int party, const void *const key[2], const 
     const size_t sm = kAesSmemBytes;
     const bool coop = a.zero_first != 0;
 #define FSK_P3_CASE(PP) case PP: return small ? launch(k_eval_p3<PP, kEvalThreadsSmall>, grid, threads, sm, st, a, coop) \
-                                              : launch(k_eval_p3<PP, kEvalThreads>, grid, threads, sm, st, a, coop);
+                                              : launch(k_eval_p3<PP, p3_threads_for(PP)>, grid, threads, sm, st, a, coop);
     switch (P.p) { FSK_P3_CASE(1) FSK_P3_CASE(2) FSK_P3_CASE(3) FSK_P3_CASE(4) FSK_P3_CASE(5) FSK_P3_CASE(6) FSK_P3_CASE(7) FSK_P3_CASE(8) }
 #undef FSK_P3_CASE
     return FUSEFSS_E_SPEC;
@@ -248,7 +248,7 @@ int launch_eval_sp(const Program &P, int party, const void *const key[2], const 
     const size_t tiles = (count + 31) / 32;
     int maxpts = 1;
     for (int w = 0; w < P.sp.n_w; ++w) if (P.sp.width[w].n_points > maxpts) maxpts = P.sp.width[w].n_points;
-    // Group count for small launches, from a two-term model fitted to profiles/r2f_small_sweep.md: a group's critical path is
+    // Group count for small launches, from a two-term model fitted to profiles/r2e_small_sweep.md: a group's critical path is
     // chain(G) = sum over clusters (shared prefix + ceil(points / G) tails) levels; up to one warp per SM sub-partition the warps
     // run at the lone-warp rate, beyond that they share the sub-partition's issue slot and the SM's shared-memory pipe (and every
     // extra group re-walks the shared prefixes), so time ~ chain(G) * max(1, warps / (4 #SMs)).  Smallest G at the minimum.
