@@ -213,10 +213,11 @@ int fusefss_mul_fused(uint32_t n_bits, const uint64_t *x0_dev, const uint64_t *x
                       uint64_t *z0_dev, uint64_t *z1_dev, void *stream);
 
 /* ---- end-to-end convenience: HOST buffers in, HOST buffers out (bench.py's e2e leg) ---------------
- * Copies r_in/r_out/xhat to the device, runs keygen + both parties' eval_cmp/eval_lut + post_fused in chunks of
- * `chunk` elements using the caller's device workspace, copies y0,y1 [n_out_a][count] and z0,z1 [count] back.
- * workspace_dev must hold fusefss_gate_workspace_bytes(prog, chunk) bytes; workspace_bytes is what the caller allocated
- * (FUSEFSS_E_WORKSPACE if it is too small). */
+ * Runs keygen + both parties' evaluation (one launch) + post_fused in chunks of `chunk` elements on `stream`, using the caller's
+ * device workspace; r_in / r_out / xhat are copied to the device and y0, y1 [n_out_a][count], z0, z1 [count] back on an internal
+ * copy stream, double-buffered, so the copies of chunk i+1 (in) and i-1 (out) overlap the kernels of chunk i (pin the host
+ * buffers for that).  Returns after everything has completed.  workspace_dev must hold fusefss_gate_workspace_bytes(prog, chunk)
+ * bytes; workspace_bytes is what the caller allocated (FUSEFSS_E_WORKSPACE if it is too small).  One call at a time per process. */
 size_t fusefss_gate_workspace_bytes(const fusefss_program *prog, size_t chunk);
 int fusefss_gate_host(const fusefss_program *prog, const uint64_t *r_in, const uint64_t *r_out,
                       const uint64_t *xhat, uint64_t seed, size_t count, size_t chunk, void *workspace_dev,

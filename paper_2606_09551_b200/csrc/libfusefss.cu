@@ -757,8 +757,10 @@ int fusefss_mul_fused(uint32_t n_bits, const uint64_t *x0_dev, const uint64_t *x
     return launch(k_mul_fused, (int)((count + 255) / 256), 256, 0, (cudaStream_t)stream, a);
 }
 
-// workspace: key0 | key1 | r_in | r_out[n_out_a] | xhat | bits0 | bits1 | coeff0[p] | coeff1[p] | y0 | y1 [n_out_a] | z0 | z1
-static size_t ws_u64_arrays(const Program &P) { return 1 + 1 + 2 + 2 + (size_t)2 * P.p + (size_t)3 * (P.n_out_a > 0 ? P.n_out_a : 1); }
+// workspace: key0 | key1 | bits0 | bits1 | coeff0[p] | coeff1[p] | 2 x { r_in | r_out[na] | xhat | y0[na] | y1[na] | z0 | z1 }
+// (the input / output arrays are double-buffered so that the copies of chunk i+1 / i-1 overlap the kernels of chunk i)
+static size_t ws_io_arrays(const Program &P) { return 4 + (size_t)3 * (P.n_out_a > 0 ? P.n_out_a : 1); }
+static size_t ws_u64_arrays(const Program &P) { return 2 + (size_t)2 * P.p + 2 * ws_io_arrays(P); }
 
 size_t fusefss_gate_workspace_bytes(const fusefss_program *prog, size_t chunk) {
     const Program *P = prog_of(prog);
@@ -767,6 +769,32 @@ size_t fusefss_gate_workspace_bytes(const fusefss_program *prog, size_t chunk) {
     return 2 * L.total + ws_u64_arrays(*P) * L.s8;
 }
 
+namespace {
+// one copy stream and a few events per device for fusefss_gate_host, created on first use and kept for the life of the process
+struct HostPipe { cudaStream_t copy = nullptr; cudaEvent_t in_ready[2] = {}, in_free[2] = {}, out_ready[2] = {}, out_free[2] = {}; };
+int host_pipe(HostPipe **out) {
+    static std::mutex mu;
+    static std::map<int, HostPipe> pipes;
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lock(mu);
+    HostPipe &hp = pipes[dev];
+    if (!hp.copy) {
+        cudaStream_t cs = nullptr;
+        CU(cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            CU(cudaEventCreateWithFlags(&hp.in_ready[i], cudaEventDisableTiming)); CU(cudaEventCreateWithFlags(&hp.in_free[i], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&hp.out_ready[i], cudaEventDisableTiming)); CU(cudaEventCreateWithFlags(&hp.out_free[i], cudaEventDisableTiming));
+        }
+        hp.copy = cs;
+    }
+    *out = &hp;
+    return 0;
+}
+}  // namespace
+
+// Chunk i: [copy stream] H2D of its inputs into buffer i % 2 -> [caller's stream] keygen, evaluation, post-processing -> [copy stream]
+// D2H of its outputs.  The copies of chunks i+1 (in) and i-1 (out) run while chunk i computes; one call at a time per device.
 int fusefss_gate_host(const fusefss_program *prog, const uint64_t *r_in, const uint64_t *r_out, const uint64_t *xhat,
                       uint64_t seed, size_t count, size_t chunk, void *workspace_dev, size_t workspace_bytes, uint64_t *y0,
                       uint64_t *y1, uint64_t *z0, uint64_t *z1, void *stream) {
@@ -776,36 +804,63 @@ int fusefss_gate_host(const fusefss_program *prog, const uint64_t *r_in, const u
     if (P->mask_output && !r_out) return FUSEFSS_E_NULL;
     if ((P->n_out_a > 0 && (!y0 || !y1)) || (P->n_out_b > 0 && (!z0 || !z1))) return FUSEFSS_E_NULL;
     if (count == 0 || chunk == 0) return FUSEFSS_E_COUNT;
-    cudaStream_t st = (cudaStream_t)stream;
+    int rc = init_device(); if (rc) return rc;
+    HostPipe *hp = nullptr;
+    rc = host_pipe(&hp); if (rc) return rc;
+    static std::mutex call_mu;                                 // the pipe's events are shared: serialise calls
+    std::lock_guard<std::mutex> call_lock(call_mu);
+    cudaStream_t st = (cudaStream_t)stream, cs = hp->copy;
     Layout L; compute_layout(*P, chunk, &L);
     const int na = P->n_out_a > 0 ? P->n_out_a : 1;
     uint8_t *ws = (uint8_t *)workspace_dev;
     uint8_t *key0 = ws, *key1 = ws + L.total;
     uint8_t *q = ws + 2 * L.total;
     auto take = [&](size_t arrays) { uint64_t *r = (uint64_t *)q; q += arrays * L.s8; return r; };
-    uint64_t *d_rin = take(1), *d_rout = take(na), *d_xhat = take(1), *d_b0 = take(1), *d_b1 = take(1);
-    uint64_t *d_c0 = take(P->p), *d_c1 = take(P->p), *d_y0 = take(na), *d_y1 = take(na), *d_z0 = take(1), *d_z1 = take(1);
-    for (size_t first = 0; first < count; first += chunk) {
-        const size_t c = count - first < chunk ? count - first : chunk;
-        CU(cudaMemcpyAsync(d_rin, r_in + first, c * 8, cudaMemcpyHostToDevice, st));
-        CU(cudaMemcpyAsync(d_xhat, xhat + first, c * 8, cudaMemcpyHostToDevice, st));
+    uint64_t *d_b0 = take(1), *d_b1 = take(1), *d_c0 = take(P->p), *d_c1 = take(P->p);
+    struct Io { uint64_t *rin, *rout, *xhat, *y0, *y1, *z0, *z1; } io[2];
+    for (int b = 0; b < 2; ++b) io[b] = Io{take(1), take(na), take(1), take(na), take(na), take(1), take(1)};
+    const size_t n_chunks = (count + chunk - 1) / chunk;
+    auto upload = [&](size_t i) -> int {                       // [copy stream] inputs of chunk i
+        const size_t first = i * chunk, c = count - first < chunk ? count - first : chunk;
+        const Io &B = io[i & 1];
+        if (i >= 2) CU(cudaStreamWaitEvent(cs, hp->in_free[i & 1], 0));          // chunk i-2 has consumed this buffer
+        CU(cudaMemcpyAsync(B.rin, r_in + first, c * 8, cudaMemcpyHostToDevice, cs));
+        CU(cudaMemcpyAsync(B.xhat, xhat + first, c * 8, cudaMemcpyHostToDevice, cs));
         if (P->mask_output)
             for (int j = 0; j < P->n_out_a; ++j)
-                CU(cudaMemcpyAsync(d_rout + (size_t)j * c, r_out + (size_t)j * count + first, c * 8, cudaMemcpyHostToDevice, st));
-        int rc = fusefss_keygen(prog, d_rin, d_rout, seed, first, c, key0, key1, st); if (rc) return rc;
+                CU(cudaMemcpyAsync(B.rout + (size_t)j * c, r_out + (size_t)j * count + first, c * 8, cudaMemcpyHostToDevice, cs));
+        CU(cudaEventRecord(hp->in_ready[i & 1], cs));
+        return 0;
+    };
+    CU(cudaEventRecord(hp->out_free[0], st)); CU(cudaEventRecord(hp->out_free[1], st));
+    CU(cudaStreamWaitEvent(cs, hp->out_free[0], 0));           // order the copy stream after the caller's earlier work on `stream`
+    rc = upload(0); if (rc) return rc;
+    if (n_chunks > 1) { rc = upload(1); if (rc) return rc; }
+    for (size_t i = 0; i < n_chunks; ++i) {
+        const size_t first = i * chunk, c = count - first < chunk ? count - first : chunk;
+        const Io &B = io[i & 1];
+        CU(cudaStreamWaitEvent(st, hp->in_ready[i & 1], 0));
+        if (i >= 2) CU(cudaStreamWaitEvent(st, hp->out_free[i & 1], 0));         // chunk i-2's outputs have left this buffer
+        rc = fusefss_keygen(prog, B.rin, B.rout, seed, first, c, key0, key1, st); if (rc) return rc;
         if (P->T > 0 || P->has_lut) {
-            rc = fusefss_eval_fused_both(prog, key0, key1, d_xhat, c, d_b0, d_b1, d_c0, d_c1, st); if (rc) return rc;
+            rc = fusefss_eval_fused_both(prog, key0, key1, B.xhat, c, d_b0, d_b1, d_c0, d_c1, st); if (rc) return rc;
         }
-        rc = fusefss_post_fused(prog, key0, key1, d_xhat, d_b0, d_b1, d_c0, d_c1, c, d_y0, d_y1, d_z0, d_z1, st); if (rc) return rc;
+        rc = fusefss_post_fused(prog, key0, key1, B.xhat, d_b0, d_b1, d_c0, d_c1, c, B.y0, B.y1, B.z0, B.z1, st); if (rc) return rc;
+        CU(cudaEventRecord(hp->in_free[i & 1], st));
+        CU(cudaEventRecord(hp->out_ready[i & 1], st));
+        CU(cudaStreamWaitEvent(cs, hp->out_ready[i & 1], 0));                    // [copy stream] outputs of chunk i
         for (int j = 0; j < P->n_out_a; ++j) {
-            CU(cudaMemcpyAsync(y0 + (size_t)j * count + first, d_y0 + (size_t)j * c, c * 8, cudaMemcpyDeviceToHost, st));
-            CU(cudaMemcpyAsync(y1 + (size_t)j * count + first, d_y1 + (size_t)j * c, c * 8, cudaMemcpyDeviceToHost, st));
+            CU(cudaMemcpyAsync(y0 + (size_t)j * count + first, B.y0 + (size_t)j * c, c * 8, cudaMemcpyDeviceToHost, cs));
+            CU(cudaMemcpyAsync(y1 + (size_t)j * count + first, B.y1 + (size_t)j * c, c * 8, cudaMemcpyDeviceToHost, cs));
         }
         if (P->n_out_b > 0) {
-            CU(cudaMemcpyAsync(z0 + first, d_z0, c * 8, cudaMemcpyDeviceToHost, st));
-            CU(cudaMemcpyAsync(z1 + first, d_z1, c * 8, cudaMemcpyDeviceToHost, st));
+            CU(cudaMemcpyAsync(z0 + first, B.z0, c * 8, cudaMemcpyDeviceToHost, cs));
+            CU(cudaMemcpyAsync(z1 + first, B.z1, c * 8, cudaMemcpyDeviceToHost, cs));
         }
+        CU(cudaEventRecord(hp->out_free[i & 1], cs));
+        if (i + 2 < n_chunks) { rc = upload(i + 2); if (rc) return rc; }
     }
+    CU(cudaStreamSynchronize(cs));
     CU(cudaStreamSynchronize(st));
     return 0;
 }

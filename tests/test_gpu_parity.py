@@ -279,6 +279,33 @@ def test_gate_host_end_to_end(F, orc):
     assert np.array_equal(z0, exp["z"][0]) and np.array_equal(z1, exp["z"][1])
 
 
+@pytest.mark.parametrize("mk,count,chunk", [(lambda: specs.shared_prefix(specs.gelu()), 1000, 96), (lambda: specs.toy(8, 3, True), 777, 64),
+                                            (lambda: specs.shift_relu(), 2050, 1024)])
+def test_gate_host_many_chunks(F, orc, mk, count, chunk):
+    """fusefss_gate_host double-buffers its input / output arrays over an internal copy stream: many chunks, a ragged last one, pinned
+    host buffers (truly asynchronous copies), masked outputs (r_out travels too); every share equals the oracle's one-shot run, twice in
+    a row through the same workspace."""
+    import torch
+    spec = mk()
+    rng = np.random.default_rng(17)
+    N = 1 << spec.n if spec.n < 64 else None
+    u = (lambda k: rng.integers(0, N, k, dtype=np.uint64)) if N else \
+        (lambda k: rng.integers(0, 1 << 63, size=k, dtype=np.uint64) * np.uint64(2) + rng.integers(0, 2, size=k, dtype=np.uint64))
+    P, O = F.Program(spec), orc.Program(spec)
+    na = max(1, P.shape["n_out_a"])
+    x, r_in, r_out = u(count), u(count), u(na * count).reshape(na, count)
+    xhat = (x + r_in) & mask_of(spec.n)
+    pin = lambda a: torch.from_numpy(a.view(np.int64)).pin_memory().numpy().view(np.uint64)
+    ws = torch.empty(P.workspace_bytes(chunk), dtype=torch.uint8, device="cuda")
+    ok0, ok1 = O.keygen(r_in, r_out, 5)
+    exp = O.run_gate(ok0, ok1, xhat)
+    for _ in range(2):
+        y0, y1, z0, z1 = P.gate_host(pin(r_in), pin(r_out), pin(xhat), 5, chunk, ws)
+        assert np.array_equal(y0[:P.shape["n_out_a"]], exp["y"][0]) and np.array_equal(y1[:P.shape["n_out_a"]], exp["y"][1])
+        if P.shape["n_out_b"]:
+            assert np.array_equal(z0, exp["z"][0]) and np.array_equal(z1, exp["z"][1])
+
+
 FULL = [("relu16", 0), ("relu16", 1), ("relu16", 8), ("shift_relu", 8), ("shift_relu", 9), ("gelu", 8), ("gelu", 0), ("gelu", 1), ("gelu", 5), ("nexp", 0), ("nexp", 1), ("recip", 0), ("recip", 1),
         ("shift_relu", 0), ("shift_relu", 1), ("rsqrt", 0), ("rsqrt", 3), ("silu", 0), ("silu", 1)]
 
