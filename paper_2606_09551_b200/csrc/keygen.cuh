@@ -348,6 +348,121 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec(const __grid_constan
 
 
 // ---------------------------------------------------------------------------------------------------
+// k_gen_vec for SMALL launches (a few thousand elements: relu16, recip, rsqrt).  There the machine is far from full and what
+// bounds the dealer is the chain of one tree: n levels x the 4 (1+Q) PRG blocks a lane of k_gen_vec expands per level.  Here a
+// QUAD of lanes shares one element: lane 4 q + c expands child c = 2 b + d (party b, direction d) only, so a level's critical path
+// is 1+Q blocks, and the correction words are assembled with warp shuffles (about 35 per level).  A warp = (8-element tile, tree).
+// Same arithmetic, same bytes: every value below is the one k_gen_vec computes (DESIGN 4.2), only WHERE it is computed differs.
+// ---------------------------------------------------------------------------------------------------
+template <int P>
+__global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec_quad(const __grid_constant__ GenVecArgs a) {
+    constexpr int Q = (P + 1) / 2;
+    constexpr unsigned FULL = 0xffffffffu;
+    extern __shared__ uint32_t sT[];
+    const uint32_t tl = aes_fill_tables(sT);
+    const int lane = threadIdx.x & 31, c = lane & 3, b = c >> 1, d = c & 1, base = lane & ~3;
+    const size_t tiles = (a.count + 7) / 8;
+    const size_t items = tiles * (size_t)(a.M - 1);
+    const size_t warps = (size_t)gridDim.x * (blockDim.x >> 5);
+    for (size_t it = (size_t)(threadIdx.x >> 5) * gridDim.x + blockIdx.x; it < items; it += warps) {
+        const int j = 1 + (int)(it / tiles);
+        size_t e = (it - (size_t)(j - 1) * tiles) * 8 + (size_t)(lane >> 2);
+        const bool live = e < a.count;                                   // dead quads shadow the last element and store nothing
+        if (!live) e = a.count - 1;
+        const uint64_t r = a.r_in[e] & a.mask;
+        uint64_t alpha, beta[P];
+        if (a.sp) {
+            alpha = r << (64 - a.n);
+            beta[0] = 1;
+#pragma unroll
+            for (int w = 1; w < P; ++w) beta[w] = beta[w - 1] * (0ull - r);
+        } else {
+            P3 p3;
+            p3.init(a.alpha, a.m, a.n, a.mask, r, a.M);
+            alpha = p3.B(j) << (64 - a.n);
+            const uint64_t *va = a.payload + (size_t)p3.ord(j - 1) * P, *vb = a.payload + (size_t)p3.ord(j) * P;
+#pragma unroll
+            for (int w = 0; w < P; ++w) beta[w] = va[w] - vb[w];
+            if (a.xpoly) shift_payload<P>(beta, a.polys, a.d, 0ull - r);
+        }
+        uint32_t s[4];                                                   // this lane's party's seed
+        {
+            uint64_t lo, hi;
+            dealer_rand(tl, a.rk, a.first_elem + e, SLOT_VEC_ROOT + 2 * j + b, lo, hi);
+            s[0] = (uint32_t)lo & ~3u; s[1] = (uint32_t)(lo >> 32); s[2] = (uint32_t)hi; s[3] = (uint32_t)(hi >> 32);
+        }
+        uint8_t *tree0 = a.key0 + a.vt_first + (size_t)(j - 1) * a.vt_stride;
+        uint8_t *tree1 = a.key1 + a.vt_first + (size_t)(j - 1) * a.vt_stride;
+        uint8_t *mytree = (c & 1) ? tree1 : tree0;                       // lanes 0 / 1 store the seed words, lanes 2 / 3 the payload words
+        if (live && d == 0) st_stream16((b ? tree1 : tree0) + e * 16, make_uint4(s[0], s[1], s[2], s[3]));
+        uint32_t t0 = 0, t1 = 1;                                         // replicated in the four lanes
+        uint64_t Va[P];
+#pragma unroll
+        for (int w = 0; w < P; ++w) Va[w] = 0;
+        size_t lvl = a.vt_lvl_rel;
+        for (int i = 0; i < a.n; ++i, lvl += a.lvl_stride) {
+            const uint32_t abit = (uint32_t)(alpha >> 63);
+            alpha <<= 1;
+            const uint64_t am64 = 0ull - (uint64_t)abit;
+            const int keep_d = (int)abit, lose_d = 1 - keep_d;
+            uint32_t x[1][4] = {{s[0] | (uint32_t)d, s[1], s[2], s[3]}}, o[1][1 + Q][4];
+            prg_blocks<1, 1 + Q, 0, 1>(tl, x, o);
+            const uint32_t T = o[0][0][0] & 1u;
+            uint32_t S[4] = {o[0][0][0] & ~3u, o[0][0][1], o[0][0][2], o[0][0][3]};
+            uint32_t scw[4], keepS[4];
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const uint32_t sx = S[k] ^ __shfl_xor_sync(FULL, S[k], 2);           // S_0[d] ^ S_1[d]
+                scw[k] = __shfl_sync(FULL, sx, base + lose_d);
+                keepS[k] = __shfl_sync(FULL, S[k], base + 2 * b + keep_d);            // S_b[keep]
+            }
+            const uint32_t tx = T ^ __shfl_xor_sync(FULL, T, 2);                      // T_0[d] ^ T_1[d]
+            const uint32_t tcw0 = __shfl_sync(FULL, tx, base) ^ abit ^ 1u, tcw1 = __shfl_sync(FULL, tx, base + 1) ^ abit;
+            const uint32_t tcw_keep = abit ? tcw1 : tcw0;
+            const uint32_t Tk0 = __shfl_sync(FULL, T, base + keep_d), Tk1 = __shfl_sync(FULL, T, base + 2 + keep_d);
+            const uint64_t sgn = 0ull - (uint64_t)t1;
+            uint64_t vcw[P];
+#pragma unroll
+            for (int w = 0; w < P; ++w) {
+                const uint64_t W = (uint64_t)o[0][1 + w / 2][2 * (w & 1)] | ((uint64_t)o[0][1 + w / 2][2 * (w & 1) + 1] << 32);
+                const uint64_t Wp = __shfl_xor_sync(FULL, W, 2);
+                const uint64_t D = b ? W - Wp : Wp - W;                                // W_1[d] - W_0[d]
+                const uint64_t loseD = __shfl_sync(FULL, D, base + lose_d), keepD = __shfl_sync(FULL, D, base + keep_d);
+                uint64_t v = loseD - Va[w] + (beta[w] & am64);
+                v = ((v ^ sgn) - sgn) & a.mask;
+                vcw[w] = v;
+                Va[w] = Va[w] - keepD + ((v ^ sgn) - sgn);
+            }
+            if (live) {
+                if (c < 2) st_stream16(mytree + lvl + e * 16, make_uint4(scw[0] | tcw0 | (tcw1 << 1), scw[1], scw[2], scw[3]));
+                else {
+#pragma unroll
+                    for (int w = 0; w < P; ++w) st_stream8(mytree + lvl + a.s16 + (size_t)w * a.s8 + e * 8, vcw[w]);
+                }
+            }
+            const uint32_t tb = b ? t1 : t0, mb = 0u - tb;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) s[k] = keepS[k] ^ (scw[k] & mb);
+            const uint32_t nt0 = Tk0 ^ (t0 & tcw_keep), nt1 = Tk1 ^ (t1 & tcw_keep);
+            t0 = nt0; t1 = nt1;
+        }
+        // final correction word: fin = (-1)^{t_1} (conv(s_1) - conv(s_0) - Valpha)
+        uint32_t x[1][4] = {{s[0] | 2u, s[1], s[2], s[3]}}, o[1][Q][4];
+        prg_blocks<1, Q, 1, 1>(tl, x, o);
+        const uint64_t sgn = 0ull - (uint64_t)t1;
+#pragma unroll
+        for (int w = 0; w < P; ++w) {
+            const uint64_t C = (uint64_t)o[0][w / 2][2 * (w & 1)] | ((uint64_t)o[0][w / 2][2 * (w & 1) + 1] << 32);
+            const uint64_t Cp = __shfl_xor_sync(FULL, C, 2);
+            uint64_t v = (b ? C - Cp : Cp - C) - Va[w];
+            v = ((v ^ sgn) - sgn) & a.mask;
+            if (live && c < 2) st_stream8(mytree + a.vt_fin_rel + (size_t)w * a.s8 + e * 8, v);
+        }
+    }
+}
+
+
+// ---------------------------------------------------------------------------------------------------
 // a4: share splitting.  One lane per element: c_b of the lookup, [r_in], [r_out], kappa^A,
 // kappa^B (theta-atom carries of Lemma 4.3 + the spec's bits), Beaver / AND / B2A material.
 // ---------------------------------------------------------------------------------------------------

@@ -181,6 +181,28 @@ int launch_gen_vec_p(int p, int grid, int block, cudaStream_t st, const GenVecAr
     return FUSEFSS_E_SPEC;
 }
 
+// Tiny dealer launches (one warp per (32-element tile, tree) would leave at most 2 warps per SM: relu16, and the single tree per element
+// of recip / rsqrt in the single-key construction): the quad-lane kernel -- four lanes per element, one child each -- cuts the per-level
+// chain of a tree 4x (keygen.cuh): rsqrt v1 198 -> 72 us, relu16 v1 59 -> 27 us.  With more warps than that the SM's issue slots and lookup
+// pipe are shared anyway and the quads' shuffles and replicated setup cost more than they save (recip v0: 286 -> 426 us), so those
+// launches stay on k_gen_vec.
+std::atomic<int> g_gen_quad{1};               // fusefss_debug_set("gen_quad", 0): always the lane-per-element dealer kernel
+int launch_gen_vec(int p, size_t count, int trees, cudaStream_t st, const GenVecArgs &a) {
+    const size_t tiles = (count + 31) / 32, items = tiles * (size_t)trees;
+    if (g_gen_quad.load() && items <= (size_t)g_sms * 2) {
+        const size_t qitems = ((count + 7) / 8) * (size_t)trees;
+        const int th = threads_for(qitems, kGenThreads), grid = grid_for(qitems, th);
+        switch (p) {
+#define FSK_GQ_CASE(PP) case PP: return launch(k_gen_vec_quad<PP>, grid, th, kAesSmemBytes, st, a);
+        FSK_GQ_CASE(1) FSK_GQ_CASE(2) FSK_GQ_CASE(3) FSK_GQ_CASE(4) FSK_GQ_CASE(5) FSK_GQ_CASE(6) FSK_GQ_CASE(7) FSK_GQ_CASE(8)
+#undef FSK_GQ_CASE
+        }
+        return FUSEFSS_E_SPEC;
+    }
+    const int th = threads_for(items, kGenThreads);
+    return launch_gen_vec_p(p, grid_for(items, th), th, st, a);
+}
+
 // A launch is "small" when even with every tree of every element on its own warp it leaves at most 8 warps per SM: then the
 // 256-thread instantiation (255 registers per thread instead of 64) is used -- such launches live on the instruction-level
 // parallelism inside a warp, not on occupancy.
@@ -488,6 +510,7 @@ int fusefss_debug_set(const char *knob, long value) {
     if (k == "eval_threads") { g_eval_threads.store(value >= 32 && value <= kEvalThreads && value % 32 == 0 ? (int)value : kEvalThreads); return 0; }
     if (k == "small_kernels") { g_small_regs.store(value ? 1 : 0); return 0; }
     if (k == "sp_np") { g_sp_np.store(value >= 1 ? (int)value : 0); return 0; }
+    if (k == "gen_quad") { g_gen_quad.store(value ? 1 : 0); return 0; }
     return FUSEFSS_E_DEBUG;
 }
 uint64_t fusefss_launch_count(void) { return g_launches.load(); }
@@ -534,7 +557,7 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
             a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.vt_first = L.vt_first; a.vt_stride = L.vt_stride; a.lvl_stride = L.lvl_stride;
             a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel; a.first_elem = first_elem; a.mask = P->mask;
             a.n = (int)P->n; a.m = (int)P->m; a.M = 2; a.sp = 1; a.rk = rk;
-            { const int th = threads_for(tiles, kGenThreads); rc = launch_gen_vec_p(P->sp.pk, grid_for(tiles, th), th, st, a); }
+            rc = launch_gen_vec(P->sp.pk, count, 1, st, a);
             if (rc) return rc;
         }
     }
@@ -555,8 +578,7 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
         a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel; a.first_elem = first_elem; a.mask = P->mask;
         a.n = (int)P->n; a.m = (int)P->m; a.M = P->M; a.rk = rk;
         a.xpoly = (int)P->xpoly; a.polys = (int)P->r; a.d = (int)P->d;
-        const int th = threads_for(tiles * (size_t)(P->M - 1), kGenThreads), grid = grid_for(tiles * (size_t)(P->M - 1), th);
-        rc = launch_gen_vec_p(P->p, grid, th, st, a);
+        rc = launch_gen_vec(P->p, count, P->M - 1, st, a);
         if (rc) return rc;
     }
     if (parts & FUSEFSS_GEN_SHARES) {
