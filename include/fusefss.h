@@ -111,7 +111,8 @@ typedef struct {
 
 /* ---- a0: compile (host only; Protocol 3 steps (2)-(4); DESIGN 4.3) ------------------
  * Validates the spec (boundaries strictly increasing in (0,2^n), n in [1,64], m < 64, p <= 8, T <= 64,
- * <= 16 rounds, <= 64 AND gates, <= 64 B2A gates) and builds the immutable compiled gate type: atom list,
+ * <= 16 rounds, <= 64 AND gates, <= 64 B2A gates, <= 8 interactive A2B nodes, <= 64 opened bits per round -- an AND opens 2, a B2A 1 --,
+ * <= 48 live arithmetic and <= 128 live bit values) and builds the immutable compiled gate type: atom list,
  * (T, M, p), post-processing program, message shapes.  The spec's arrays are copied; the caller may free
  * them.  Compile once per gate type, reuse across tensors/layers (program caching). */
 int fusefss_compile(const fusefss_spec *spec, fusefss_program **out);

@@ -1039,6 +1039,9 @@ orc_prog *orc_compile(const orc_spec *S0)
         if (o->op == C_A_B2A) P->r_nbits[o->round] += 1;
         if (o->op == C_B_A2B) P->r_narr[o->round] += 1;
     }
+    /* a round's opened bits travel in ONE 64-bit word per element (message layout, DESIGN 4.6): more than 64 of them (e.g. 33 AND
+     * gates in one round) is over the format's limit -- reject instead of shifting past the word */
+    for (int q = 0; q < P->rounds; q++) if (P->r_nbits[q] > 64) { orc_destroy(P); return NULL; }
     P->ma_word[0] = 0;
     for (int i = 0; i < P->MA; i++) P->ma_word[i + 1] = P->ma_word[i] + (P->ma_is_x[i] ? 2 : 3);
     return P;

@@ -46,9 +46,12 @@ __global__ void __launch_bounds__(256) k_post_round(const __grid_constant__ Post
     const uint64_t mask = a.mask, xh = a.xhat[e] & mask;
     const bool p0 = a.party == 0;
     uint64_t A[kMaxAReg];
-    uint64_t Bw = 0, zword = 0, outbits = 0;
-    auto getb = [&](int r) -> uint64_t { return (Bw >> r) & 1ull; };
-    auto setb = [&](int r, uint64_t v) { Bw = (Bw & ~(1ull << r)) | ((v & 1ull) << r); };
+    uint64_t Bw0 = 0, Bw1 = 0, zword = 0, outbits = 0;                       // 128 bit registers (kMaxBReg) in two words
+    auto getb = [&](int r) -> uint64_t { return ((r < 64 ? Bw0 : Bw1) >> (r & 63)) & 1ull; };
+    auto setb = [&](int r, uint64_t v) {
+        const uint64_t m = 1ull << (r & 63), b = (v & 1ull) << (r & 63);
+        if (r < 64) Bw0 = (Bw0 & ~m) | b; else Bw1 = (Bw1 & ~m) | b;
+    };
     for (int pc = 0; pc < a.n_ins; ++pc) {
         const Ins o = a.ins[pc];
         switch (o.op) {
@@ -178,9 +181,12 @@ __global__ void __launch_bounds__(256) k_post_fused(const __grid_constant__ Post
     for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < a.count; e += (size_t)gridDim.x * blockDim.x) {
     const uint64_t mask = a.mask, xh = a.xhat[e] & mask;
     uint64_t A[2][kMaxAReg];
-    uint64_t Bw[2] = {0, 0}, zword[2] = {0, 0};
-    auto getb = [&](int b, int r) -> uint64_t { return (Bw[b] >> r) & 1ull; };
-    auto setb = [&](int b, int r, uint64_t v) { Bw[b] = (Bw[b] & ~(1ull << r)) | ((v & 1ull) << r); };
+    uint64_t Bw[2][2] = {{0, 0}, {0, 0}}, zword[2] = {0, 0};                   // per party: 128 bit registers in two words
+    auto getb = [&](int b, int r) -> uint64_t { return ((r < 64 ? Bw[b][0] : Bw[b][1]) >> (r & 63)) & 1ull; };
+    auto setb = [&](int b, int r, uint64_t v) {
+        const uint64_t m = 1ull << (r & 63), x = (v & 1ull) << (r & 63);
+        if (r < 64) Bw[b][0] = (Bw[b][0] & ~m) | x; else Bw[b][1] = (Bw[b][1] & ~m) | x;
+    };
     for (int pc = 0; pc < a.n_ins; ++pc) {
         const Ins o = a.ins[pc];
         switch (o.op) {

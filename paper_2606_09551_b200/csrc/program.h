@@ -16,7 +16,7 @@ constexpr int kMaxP = 8;           // payload words p
 constexpr int kMaxIntervals = 64;  // m < 64
 constexpr int kMaxRounds = 16;
 constexpr int kMaxAReg = 48;       // arithmetic registers after allocation (device local array)
-constexpr int kMaxBReg = 64;       // bit registers after allocation (one 64-bit word per party)
+constexpr int kMaxBReg = 128;      // bit registers after allocation (two 64-bit words per party)
 constexpr int kMaxA2B = 8;         // interactive A2B nodes per gate
 
 // One query of the packed comparison instance (Def I.1).

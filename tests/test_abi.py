@@ -42,6 +42,11 @@ ALL = ALL + [(nm + "_dense", (lambda mk=mk: specs.dense_table(mk()))) for nm, mk
 ALL = ALL + [(nm + "_et", (lambda mk=mk: specs.early_termination(mk()))) for nm, mk in ALL[:36] + ALL[-4:]]  # variant bit 3 (DESIGN 13)
 
 
+# gate types AT the compiled limits (m = 63, p = 8, T = 64, 63 output bits; 32 AND gates = one message bit word in one round)
+ALL = ALL + [("limits", specs.limits), ("limits_sp", lambda: specs.shared_prefix(specs.limits(n_pred=1))), ("limits_et", lambda: specs.early_termination(specs.limits())),
+             ("limits_pw", specs.limits_piecewise), ("limits_pw_sp", lambda: specs.shared_prefix(specs.limits_piecewise()))]
+
+
 @pytest.mark.parametrize("name,mk", ALL)
 def test_compile_matches_oracle_shape(F, orc, name, mk):
     """Two independent compilers (DESIGN 4.3): same L_shape, atoms, key size, message sizes."""
@@ -56,6 +61,19 @@ def test_compile_matches_oracle_shape(F, orc, name, mk):
             assert P.post_msg_bytes(count, q) == O.post_msg_bytes(count, q)
     assert P.post_rounds() == O.post_rounds()
     assert P.online_bits() == O.online_bits()
+
+
+@pytest.mark.parametrize("mk,kw", [(specs.limits, dict(m=64)), (specs.limits, dict(r=3, d=2)), (specs.limits, dict(n_pred=64)),
+                                   (specs.limits_piecewise, dict(m=33)), (lambda: specs.shared_prefix(specs.limits()), {})])
+def test_both_compilers_reject_beyond_the_limits(F, orc, mk, kw):
+    """one step past each limit (m = 64 intervals, p = 9 payload words, T = 65 atoms, 33 AND gates in one round): FUSEFSS_E_SPEC from
+    the library, NULL from the oracle's compiler -- never a truncated program; likewise the single-key construction of the T = 64 gate,
+    whose predicates and boundaries together would need 125 points"""
+    s = mk(**kw)
+    with pytest.raises(Exception):
+        F.Program(s)
+    with pytest.raises(Exception):
+        orc.Program(s)
 
 
 def test_appendix_N_shape(F):

@@ -434,6 +434,24 @@ def test_silu_all_chunks(F, orc):
     assert np.array_equal(np.concatenate(prop_z), pack_bits(ze))
 
 
+@pytest.mark.parametrize("mk,count", [(specs.limits, 45), (lambda: specs.early_termination(specs.limits()), 37),
+                                      (lambda: specs.shared_prefix(specs.limits(n_pred=1)), 70), (specs.limits_piecewise, 100),
+                                      (lambda: specs.shared_prefix(specs.limits_piecewise()), 100)])
+def test_compiled_limits(F, orc, mk, count):
+    """Gate types AT the compiled limits (workloads.specs.limits: m = 63 intervals -> 63 lookup trees, p = 8 payload words, T = 64 atoms
+    filling the packed comparison word, 63 output bits, 66 live bit registers; limits_piecewise: 32 AND gates = 64 opened bits = one full
+    message bit word in one round): keys, both calls, every round's messages, shares and reconstruction, ragged count."""
+    spec = mk()
+    rng = np.random.default_rng(31)
+    u = lambda k: rng.integers(0, 1 << 63, size=k, dtype=np.uint64) * np.uint64(2) + rng.integers(0, 2, size=k, dtype=np.uint64)
+    x = u(count)
+    a = np.array(spec.alpha, dtype=np.uint64)
+    x[:20] = np.concatenate([a[:10], a[-10:] - np.uint64(1)])
+    r_in = u(count)
+    r_in[20:23] = np.array([0, 2**64 - 1, 2**63], dtype=np.uint64)
+    _parity(F, orc, spec, x, r_in, u(2 * count), seed=13)
+
+
 @pytest.mark.parametrize("variant", [0, 1, 5])
 def test_many_scattered_boundaries(F, orc, variant):
     """m = 39 intervals spread over the whole ring (M = 40 lookup intervals for Protocol 3; 39 single-point clusters for

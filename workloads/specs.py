@@ -346,6 +346,28 @@ def a2b_demo(n=8, f=3):
                phi=phi, n_out_a=1, n_out_b=5, out_frac=2 * f)
 
 
+def limits(n=64, m=63, r=2, d=3, n_pred=63):
+    """A gate type AT the compiled limits (fusefss.h: m < 64, p <= 8, T <= 64, 64 output bits): m = 63 intervals spread over the ring,
+    r = 2 polynomials of degree 3 (p = 8 payload words) and 63 distinct thresholds C_beta, each its own output bit:
+    T = 1 r-atom + 63 theta-atoms = 64.  Stress / edge-case input, not an operator of the paper."""
+    N = 1 << n
+    alpha = [(i + 1) * (N // (m + 1)) + 3 * i for i in range(m - 1)]
+    coeff = [[[(7 * i + 3 * j + k + 1) * (1 if (i + k) % 3 else -1) for k in range(d + 1)] for j in range(r)] for i in range(m)]
+    nodes = [(BN_C, 0, 0, 0, 0, (t + 1) * (N // (n_pred + 2)) + 5 * t + 1) for t in range(n_pred)]
+    return _mk(f"limits_m{m}_p{r * (d + 1)}_T{n_pred + 1}", n, 12, alpha, coeff, nodes=nodes, bit_root=[list(range(n_pred))] * m,
+               n_out_a=r, out_frac=12)
+
+
+def limits_piecewise(n=64, m=32):
+    """m = 32 intervals with ONE piecewise output bit: Lemma D.2 spends m = 32 AND gates on it, all in one round -- 64 opened bits,
+    exactly one message bit word (the per-round limit); the 31 boundary comparisons become atoms."""
+    N = 1 << n
+    alpha = [(i + 1) * (N // (m + 1)) + i for i in range(m - 1)]
+    nodes = [(BN_C, 0, 0, 0, 0, N // 5 + 11), (BN_NOT, 0, 0, 0, 0, 0)]
+    return _mk(f"limits_pw_m{m}", n, 12, alpha, [[[i + 1, -i]] for i in range(m)], nodes=nodes, bit_root=[[i % 2] for i in range(m)],
+               n_out_a=1, out_frac=12)
+
+
 def plain_default(n=8, f=3):
     """No Phi (default: outputs are F's y and z), r = 1 degree-1, m = 3, one piecewise bit."""
     N = 1 << n
