@@ -295,7 +295,7 @@ int launch_eval_sp(const Program &P, int party, const void *const key[2], const 
     }
     if (const int f = g_force_g.load()) G = f < maxpts ? f : maxpts;
     a.G = G;
-    a.np = g_sp_np.load() ? g_sp_np.load() : 2;
+    a.np = g_sp_np.load() ? g_sp_np.load() : FFS_SP_NP_SMALL;      // clamped in the kernel to its compiled maximum (1 for large launches)
     a.zero_first = G > 1;
     const size_t items = tiles * (size_t)G * (size_t)a.n_parties;
     const bool small = small_launch(items);

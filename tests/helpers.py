@@ -90,6 +90,11 @@ def random_spec(seed, variant=0):
                     newB(op, int(rng.choice(B)), int(rng.integers(0, n)), int(rng.integers(0, 2)))
                 else:
                     newB(op, int(rng.choice(B)), int(rng.choice(B)))
+        rng_a2b = np.random.default_rng(seed + 7777)                # A2B nodes (own stream: the rest of the spec is as before)
+        for _ in range(int(rng_a2b.integers(0, 3))):
+            newB(S.PHI_B_A2B, int(rng_a2b.choice(A)), int(rng_a2b.integers(0, n)))
+            if rng_a2b.random() < 0.5:
+                newA(S.PHI_A_B2A, B[-1])                             # and back into arithmetic
         n_out_a, n_out_b = int(rng.integers(1, 3)), int(rng.integers(0, 4))
         for j in range(n_out_a):
             phi.append((S.PHI_A_OUT, j, int(rng.choice(A)), 0, 0))
