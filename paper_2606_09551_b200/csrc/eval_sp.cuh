@@ -31,6 +31,9 @@ struct EvalSpArgs {
 };
 
 // PK = payload words of the n-bit key: 1 (payload 1) or d+1 (payload (1, -r, .., (-r)^d), variant bit 2, DESIGN 11)
+#ifndef FFS_SP_UNR
+#define FFS_SP_UNR 3              // AES rounds per loop trip in this kernel (profiles/r1l_unroll.md)
+#endif
 template <int PK> struct SpState { uint32_t s[4]; uint32_t t; uint64_t V[PK]; };
 
 template <int PK>
@@ -38,7 +41,7 @@ __device__ __forceinline__ void sp_step(uint32_t tl, const uint4 cw, const uint6
     constexpr int QK = (PK + 1) / 2;
     uint32_t x[1][4] = {{st.s[0] | dbit, st.s[1], st.s[2], st.s[3]}};
     uint32_t o[1][1 + QK][4];
-    prg_blocks<1, 1 + QK, 0, true, 3>(tl, x, o);
+    prg_blocks<1, 1 + QK, 0, true, FFS_SP_UNR>(tl, x, o);
     const uint32_t tm = 0u - st.t;
     const uint64_t tm64 = 0ull - (uint64_t)st.t;
 #pragma unroll
@@ -120,7 +123,7 @@ __device__ __forceinline__ void sp_leaf(uint32_t tl, const SpState<PK> &st, cons
     constexpr int QK = (PK + 1) / 2;
     uint32_t x[1][4] = {{st.s[0] | 2u, st.s[1], st.s[2], st.s[3]}};
     uint32_t o[1][QK][4];
-    prg_blocks<1, QK, 1, true, 3>(tl, x, o);
+    prg_blocks<1, QK, 1, true, FFS_SP_UNR>(tl, x, o);
     const uint64_t tm64 = 0ull - (uint64_t)st.t;
 #pragma unroll
     for (int w = 0; w < PK; ++w) {
@@ -155,7 +158,7 @@ __device__ __forceinline__ void sp_walk_batch(uint32_t tl, const uint8_t *lvl, s
             ub[q] <<= 1;
             x[q][0] = st[q].s[0] | dbit[q]; x[q][1] = st[q].s[1]; x[q][2] = st[q].s[2]; x[q][3] = st[q].s[3];
         }
-        prg_blocks<NP, 1 + QK, 0, 2, 3>(tl, x, o);
+        prg_blocks<NP, 1 + QK, 0, 2, FFS_SP_UNR>(tl, x, o);
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
             const uint32_t tm = 0u - st[q].t;
