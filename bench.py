@@ -18,6 +18,7 @@ N > 1 (torchrun): --scaling weak (default): every rank runs its own full tensor,
 from __future__ import annotations
 
 import argparse
+import gc
 import json
 import os
 import statistics
@@ -197,6 +198,7 @@ class Gate:
         dev = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.int64)).cuda()
         self.r_in, self.r_out, self.xhat = dev(inp["r_in"]), dev(inp["r_out"]), dev(inp["xhat"])
         chunk = chunk or count
+        gc.collect()
         torch.cuda.empty_cache()
         free_b, _ = torch.cuda.mem_get_info()
         per_elem = 8 * (6 + 2 * self.sh["p"] + 3 * max(1, self.sh["n_out_a"]))
@@ -620,9 +622,13 @@ def main():
         dt = allmax(time.perf_counter() - t0)
         h2d = count * 8 * (2 + (na if spec.mask_output else 0))
         d2h = count * 8 * (2 * shp["n_out_a"] + (2 if shp["n_out_b"] else 0))
-        return {"value": eff_world * count * steps / dt, "unit": "elements/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "steps": steps, "api": "fusefss_gate_host (pinned host buffers, chunk=%d)" % chunk,
-                "checksum_y": int((hy[0][0, :4] + hy[1][0, :4]).sum().item()) & 0xFFFFFFFF}
+        out = {"value": eff_world * count * steps / dt, "unit": "elements/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "steps": steps, "api": "fusefss_gate_host (pinned host buffers, chunk=%d)" % chunk,
+               "checksum_y": int((hy[0][0, :4] + hy[1][0, :4]).sum().item()) & 0xFFFFFFFF}
+        del ws, one                                                 # the workspace (up to 103 GB) must be gone before the next leg sizes its buffers
+        gc.collect()
+        torch.cuda.empty_cache()
+        return out
     gate_chunk, gate_chunks, gate_first = gate.chunk, gate.n_chunks, gate.first_global
     gate.free()                                                     # the e2e workspace holds its own key buffers
     if not args.no_e2e:

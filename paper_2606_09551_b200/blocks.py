@@ -235,12 +235,12 @@ def bench(F, torch, steps: int = 3):
     x0h = U(xq.size)
     masks = {k: dev(U(c)) for k, c in (("nexp", xq.size), ("tr_e", xq.size), ("recip", rows), ("tr_t", rows), ("tr_y", xq.size))}
     blk = {}
-    for v in (3, 0):
-        B = Softmax(rows, cols, v)
+    for v, fo in ((3, False), (3, True), (0, False)):       # fo: gate -> gate edges through the opened yhat (DESIGN 16)
+        B = Softmax(rows, cols, v, fused_open=fo)
         res, t_deal, t_on = time_block(B, masks, dev(x0h), dev(xq - x0h))
         y = (res["y"][0] + res["y"][1]).cpu().numpy().astype(np.float64).reshape(rows, cols) / 4096.0
         ref = np.exp(xr) / np.exp(xr).sum(axis=1, keepdims=True)
-        blk["variant_%d" % v] = {"rows": rows, "cols": cols, "dealer_ms": t_deal, "online_ms": t_on, "online_elems_per_s": rows * cols / (t_on * 1e-3),
+        blk["variant_%d%s" % (v, "_fused_open" if fo else "")] = {"rows": rows, "cols": cols, "dealer_ms": t_deal, "online_ms": t_on, "online_elems_per_s": rows * cols / (t_on * 1e-3),
                                  "key_bytes_per_elem_per_party": B.key_bytes_per_party() / (rows * cols),
                                  "online_bytes_per_elem_per_party": B.online_bytes_per_party() / (rows * cols), "rounds": B.rounds(),
                                  "max_abs_err_vs_float_softmax": float(np.abs(y - ref).max())}
@@ -252,15 +252,18 @@ def bench(F, torch, steps: int = 3):
     xq = np.floor(xr.reshape(-1) * 4096 + 0.5).astype(np.int64).view(np.uint64)
     x0h = U(xq.size)
     masks = {k: dev(U(c)) for k, c in (("mean", rows), ("var", rows), ("rsqrt", rows), ("tr_g", rows), ("tr_y", xq.size))}
-    B = LayerNorm(rows, d, 3)
-    res, t_deal, t_on = time_block(B, masks, dev(x0h), dev(xq - x0h))
-    y = (res["y"][0] + res["y"][1]).cpu().numpy().astype(np.float64).reshape(rows, d) / 4096.0
     xf = xq.view(np.int64).astype(np.float64).reshape(rows, d) / 4096.0
     ref = (xf - xf.mean(axis=1, keepdims=True)) / xf.std(axis=1, keepdims=True)
-    out["layernorm_block"] = {"variant_3": {"rows": rows, "d": d, "dealer_ms": t_deal, "online_ms": t_on, "online_elems_per_s": rows * d / (t_on * 1e-3),
-                                            "key_bytes_per_elem_per_party": B.key_bytes_per_party() / (rows * d),
-                                            "online_bytes_per_elem_per_party": B.online_bytes_per_party() / (rows * d), "rounds": B.rounds(),
-                                            "max_abs_err_vs_float_layernorm": float(np.abs(y - ref).max())}}
-    del B
-    torch.cuda.empty_cache()
+    out["layernorm_block"] = {}
+    for fo in (False, True):
+        B = LayerNorm(rows, d, 3, fused_open=fo)
+        res, t_deal, t_on = time_block(B, masks, dev(x0h), dev(xq - x0h))
+        y = (res["y"][0] + res["y"][1]).cpu().numpy().astype(np.float64).reshape(rows, d) / 4096.0
+        out["layernorm_block"]["variant_3" + ("_fused_open" if fo else "")] = {
+            "rows": rows, "d": d, "dealer_ms": t_deal, "online_ms": t_on, "online_elems_per_s": rows * d / (t_on * 1e-3),
+            "key_bytes_per_elem_per_party": B.key_bytes_per_party() / (rows * d),
+            "online_bytes_per_elem_per_party": B.online_bytes_per_party() / (rows * d), "rounds": B.rounds(),
+            "max_abs_err_vs_float_layernorm": float(np.abs(y - ref).max())}
+        del B
+        torch.cuda.empty_cache()
     return out
