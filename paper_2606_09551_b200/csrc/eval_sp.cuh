@@ -31,9 +31,16 @@ struct EvalSpArgs {
 };
 
 // PK = payload words of the n-bit key: 1 (payload 1) or d+1 (payload (1, -r, .., (-r)^d), variant bit 2, DESIGN 11)
+#ifndef FFS_SP_PREFETCH_BIG
+#define FFS_SP_PREFETCH_BIG 0     // 1: the large-launch instantiation also prefetches the next level into registers
+#endif
 #ifndef FFS_SP_UNR
 #define FFS_SP_UNR 3              // AES rounds per loop trip in this kernel (profiles/r1l_unroll.md)
 #endif
+#ifndef FFS_SP_UNR_WIDE
+#define FFS_SP_UNR_WIDE FFS_SP_UNR // ... when the key's payload has >= 2 words (3 PRG blocks per level)
+#endif
+template <int PK> constexpr int sp_unr() { return PK >= 2 ? FFS_SP_UNR_WIDE : FFS_SP_UNR; }
 template <int PK> struct SpState { uint32_t s[4]; uint32_t t; uint64_t V[PK]; };
 
 template <int PK>
@@ -41,7 +48,7 @@ __device__ __forceinline__ void sp_step(uint32_t tl, const uint4 cw, const uint6
     constexpr int QK = (PK + 1) / 2;
     uint32_t x[1][4] = {{st.s[0] | dbit, st.s[1], st.s[2], st.s[3]}};
     uint32_t o[1][1 + QK][4];
-    prg_blocks<1, 1 + QK, 0, true, FFS_SP_UNR>(tl, x, o);
+    prg_blocks<1, 1 + QK, 0, true, sp_unr<PK>()>(tl, x, o);
     const uint32_t tm = 0u - st.t;
     const uint64_t tm64 = 0ull - (uint64_t)st.t;
 #pragma unroll
@@ -123,7 +130,7 @@ __device__ __forceinline__ void sp_leaf(uint32_t tl, const SpState<PK> &st, cons
     constexpr int QK = (PK + 1) / 2;
     uint32_t x[1][4] = {{st.s[0] | 2u, st.s[1], st.s[2], st.s[3]}};
     uint32_t o[1][QK][4];
-    prg_blocks<1, QK, 1, true, FFS_SP_UNR>(tl, x, o);
+    prg_blocks<1, QK, 1, true, sp_unr<PK>()>(tl, x, o);
     const uint64_t tm64 = 0ull - (uint64_t)st.t;
 #pragma unroll
     for (int w = 0; w < PK; ++w) {
@@ -141,16 +148,20 @@ template <int PK, int NPMAX, int NP, int HINT>
 __device__ __forceinline__ void sp_walk_batch(uint32_t tl, const uint8_t *lvl, size_t e, size_t s16, size_t s8, size_t lvl_stride,
                                               int from, int to, uint64_t (&ub)[NPMAX], SpState<PK> (&st)[NPMAX], uint64_t pol) {
     constexpr int QK = (PK + 1) / 2;
+    // register prefetch of the next level: only where a few warps per SM must hide the load latency themselves (the 256-thread
+    // instantiations, NPMAX > 1); with 32 warps per SM the other warps hide it and the 10 registers are better spent on the AES state
+    constexpr bool PF = NPMAX > 1 || FFS_SP_PREFETCH_BIG;
     if (from >= to) return;
     const uint8_t *pl = lvl + (size_t)from * lvl_stride;
     uint4 cw; uint64_t vcw[PK];
-    sp_load_level<PK, HINT>(pl, e, s16, s8, cw, vcw, pol);
+    if (PF) sp_load_level<PK, HINT>(pl, e, s16, s8, cw, vcw, pol);
     for (int i = from; i < to; ++i) {
+        if (!PF) sp_load_level<PK, HINT>(pl, e, s16, s8, cw, vcw, pol);
         pl += lvl_stride;
         uint4 cw_n = cw; uint64_t vcw_n[PK];
 #pragma unroll
         for (int w = 0; w < PK; ++w) vcw_n[w] = vcw[w];
-        if (i + 1 < to) sp_load_level<PK, HINT>(pl, e, s16, s8, cw_n, vcw_n, pol);
+        if (PF && i + 1 < to) sp_load_level<PK, HINT>(pl, e, s16, s8, cw_n, vcw_n, pol);
         uint32_t x[NP][4], o[NP][1 + QK][4], dbit[NP];
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
@@ -158,7 +169,7 @@ __device__ __forceinline__ void sp_walk_batch(uint32_t tl, const uint8_t *lvl, s
             ub[q] <<= 1;
             x[q][0] = st[q].s[0] | dbit[q]; x[q][1] = st[q].s[1]; x[q][2] = st[q].s[2]; x[q][3] = st[q].s[3];
         }
-        prg_blocks<NP, 1 + QK, 0, 2, FFS_SP_UNR>(tl, x, o);
+        prg_blocks<NP, 1 + QK, 0, 2, sp_unr<PK>()>(tl, x, o);
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
             const uint32_t tm = 0u - st[q].t;
