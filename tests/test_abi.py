@@ -34,12 +34,13 @@ ALL = [("relu16", lambda: specs.relu(16, 8)), ("gelu", specs.gelu), ("nexp", spe
        ("toy", lambda: specs.toy(8, 3)), ("toy_masked", lambda: specs.toy(8, 3, True)),
        ("plain", specs.plain_default), ("single", specs.single_interval), ("nobits", specs.no_bits),
        ("full", specs.full_partition), ("shift_relu8", lambda: specs.shift_relu(8, 3)), ("ars", lambda: specs.ars(64, 12)),
-       ("ars8", lambda: specs.ars(8, 3)), ("a2b8", lambda: specs.a2b_demo(8, 3)), ("a2b64", lambda: specs.a2b_demo(64, 12))]
+       ("ars8", lambda: specs.ars(8, 3)), ("a2b8", lambda: specs.a2b_demo(8, 3)), ("a2b64", lambda: specs.a2b_demo(64, 12)),
+       ("tiny1", lambda: specs.tiny_ring(1)), ("tiny2", lambda: specs.tiny_ring(2))]
 ALL = ALL + [(nm + "_sp", (lambda mk=mk: specs.shared_prefix(mk()))) for nm, mk in ALL]      # variant 1 (DESIGN 9)
 ALL = ALL + [(nm + "_xm", (lambda mk=mk: specs.input_masked_mul(mk()))) for nm, mk in ALL]  # variant bit 1 (DESIGN 10)
-ALL = ALL + [(nm + "_xp", (lambda mk=mk: specs.public_point_horner(mk()))) for nm, mk in ALL[:36]]  # variant bit 2 (DESIGN 11)
-ALL = ALL + [(nm + "_dense", (lambda mk=mk: specs.dense_table(mk()))) for nm, mk in ALL[:18] if nm in ("relu16", "toy", "toy_masked", "plain", "nobits", "full", "shift_relu8", "ars8")]  # variant bit 4 (DESIGN 14)
-ALL = ALL + [(nm + "_et", (lambda mk=mk: specs.early_termination(mk()))) for nm, mk in ALL[:36] + ALL[-4:]]  # variant bit 3 (DESIGN 13)
+ALL = ALL + [(nm + "_xp", (lambda mk=mk: specs.public_point_horner(mk()))) for nm, mk in ALL[:40]]  # variant bit 2 (DESIGN 11)
+ALL = ALL + [(nm + "_dense", (lambda mk=mk: specs.dense_table(mk()))) for nm, mk in ALL[:20] if nm in ("relu16", "toy", "toy_masked", "plain", "nobits", "full", "shift_relu8", "ars8")]  # variant bit 4 (DESIGN 14)
+ALL = ALL + [(nm + "_et", (lambda mk=mk: specs.early_termination(mk()))) for nm, mk in ALL[:40] + ALL[-4:]]  # variant bit 3 (DESIGN 13)
 
 
 # gate types AT the compiled limits (m = 63, p = 8, T = 64, 63 output bits; 32 AND gates = one message bit word in one round)

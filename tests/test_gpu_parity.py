@@ -116,7 +116,8 @@ def test_bitsliced_aes_matches_fips197_and_the_table_core(F):
 
 SMALL = [lambda: specs.relu(8, 4), lambda: specs.toy(8, 3), lambda: specs.toy(8, 3, True), specs.plain_default,
          specs.single_interval, specs.no_bits, specs.full_partition, lambda: specs.shift_relu(8, 3),
-         lambda: specs.toy(12, 4), lambda: specs.relu(12, 6), lambda: specs.ars(8, 3), lambda: specs.ars(12, 5)]
+         lambda: specs.toy(12, 4), lambda: specs.relu(12, 6), lambda: specs.ars(8, 3), lambda: specs.ars(12, 5),
+         lambda: specs.tiny_ring(1), lambda: specs.tiny_ring(2)]
 
 
 SMALL_SP = [(lambda mk=mk: specs.shared_prefix(mk())) for mk in SMALL]
@@ -249,6 +250,18 @@ def test_edge_masks_n64(F, orc, variant):
         x = np.concatenate([x, xh - r_in[-xh.size:]])
     r_out = np.arange(r_in.size, dtype=np.uint64)
     _parity(F, orc, spec, x, r_in, r_out, seed=9)
+
+
+@pytest.mark.parametrize("count", [1, 2, 31, 32, 33])
+@pytest.mark.parametrize("variant", [0, 1])
+def test_degenerate_counts(F, orc, count, variant):
+    """one element, a pair, and the counts around one 32-lane tile (the quad-lane dealer kernel works on 8-element tiles, the evaluation
+    on 32-element tiles; dead lanes shadow the last element and must store nothing)"""
+    spec = specs.CONFIGS["gelu"]()
+    if variant:
+        spec = specs.shared_prefix(spec)
+    inp = tensors.inputs("gelu", spec, count=count, seed=5)
+    _parity(F, orc, spec, inp["x"], inp["r_in"], inp["r_out"], seed=8)
 
 
 def test_chunked_keygen_equals_one_shot(F, orc):

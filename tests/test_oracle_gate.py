@@ -52,6 +52,22 @@ def test_reconstruct_all_r_sampled_x_n12(orc, mk):
     check_all_r(orc, spec, corner_inputs(spec, extra=3, seed=12))
 
 
+@pytest.mark.parametrize("n", [1, 2])
+@pytest.mark.parametrize("variant", [0, 1, 8, 9, 3, 5])
+def test_tiny_rings_exhaustive(orc, n, variant):
+    """Z_2 and Z_4 (M = min(m + 1, 2^n) binds: P:579): every x and every r, both constructions and the variant bits."""
+    spec = specs.tiny_ring(n)
+    if variant & 1:
+        spec = specs.shared_prefix(spec)
+    if variant & 2:
+        spec = specs.input_masked_mul(spec)
+    if variant & 4:
+        spec = specs.public_point_horner(spec)
+    if variant & 8:
+        spec = specs.early_termination(spec)
+    check_all_r(orc, spec, range(1 << n))
+
+
 def test_appendix_N_relu_golden(orc):
     """App. N (PAPER.md:961-1016): shape (T, M, p, #Beaver), atoms, and semantics (max(x,0), MSB(x))."""
     gold = {}

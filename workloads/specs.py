@@ -346,6 +346,15 @@ def a2b_demo(n=8, f=3):
                phi=phi, n_out_a=1, n_out_b=5, out_frac=2 * f)
 
 
+def tiny_ring(n=1):
+    """The smallest rings (n = 1: Z_2, two intervals, M = min(m + 1, 2^n) = 2; n = 2: three intervals, M = 4 = the whole ring):
+    degree-1 pieces, a threshold bit and the MSB.  Degenerate-size edge case for both constructions."""
+    m = 2 if n == 1 else 3
+    nodes = [(BN_C, 0, 0, 0, 0, 1), (BN_MSB, 0, 0, 0, 0, 0)]
+    return _mk(f"tiny_n{n}", n, 0, [1] if n == 1 else [1, 3], [[[i + 1, 1 - i]] for i in range(m)], nodes=nodes, bit_root=[[0, 1]] * m,
+               n_out_a=1, out_frac=0)
+
+
 def limits(n=64, m=63, r=2, d=3, n_pred=63):
     """A gate type AT the compiled limits (fusefss.h: m < 64, p <= 8, T <= 64, 64 output bits): m = 63 intervals spread over the ring,
     r = 2 polynomials of degree 3 (p = 8 payload words) and 63 distinct thresholds C_beta, each its own output bit:
