@@ -241,8 +241,8 @@ const char *fusefss_last_cuda_error(void);
 /* Test / tuning knobs (process-wide, not part of the method): "force_g" = v >= 1 forces the number of warps the trees / points of an
  * element are dealt to (0 = automatic); "eval_threads" = CTA size of the large evaluation launches (default 1024); "small_kernels"
  * = 0 disables the 256-thread instantiations used for small launches; "sp_np" = points the single-key evaluation walks in lock-step per
- * warp (0 = automatic); "gen_quad" = 0 disables the four-lanes-per-element dealer kernel used for small launches.  Unknown knob:
- * FUSEFSS_E_DEBUG. */
+ * warp (0 = automatic); "gen_quad" = 0 disables the four-lanes-per-element dealer kernel used for small launches; "sp_split" = 0 / 1 / 2: the lane-split
+ * single-key evaluation kernel never / for tiny launches (default) / for every small launch.  Unknown knob: FUSEFSS_E_DEBUG. */
 int fusefss_debug_set(const char *knob, long value);
 /* number of kernel launches this library has issued since load (bench.py's gpu_launches) */
 uint64_t fusefss_launch_count(void);

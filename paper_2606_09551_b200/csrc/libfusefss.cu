@@ -15,6 +15,7 @@
 #include "aes.cuh"
 #include "eval.cuh"
 #include "eval_sp.cuh"
+#include "eval_sp_split.cuh"
 #include "keygen.cuh"
 #include "post.cuh"
 #include "blocks.cuh"
@@ -29,6 +30,7 @@ thread_local int g_sms = 148;                 // SM count of the calling thread'
 std::atomic<int> g_force_g{0};                // fusefss_debug_set("force_g", v): v >= 1 forces the tree-group count (tests)
 std::atomic<int> g_eval_threads{kEvalThreads};// fusefss_debug_set("eval_threads", v): CTA size of the large eval launches
 std::atomic<int> g_sp_np{0};                  // fusefss_debug_set("sp_np", v): points walked in lock-step by k_eval_sp (0 = automatic)
+std::atomic<int> g_sp_split{1};                // fusefss_debug_set("sp_split", v): 0 = never the lane-split kernel, 1 = for tiny launches (default), 2 = for every small launch
 std::atomic<int> g_small_regs{1};             // fusefss_debug_set("small_kernels", 0): never pick the 256-thread instantiations
 const HostAes &host_aes() { static HostAes h; return h; }
 
@@ -274,9 +276,8 @@ int launch_eval_sp(const Program &P, int party, const void *const key[2], const 
     // chain(G) = sum over clusters (shared prefix + ceil(points / G) tails) levels; up to one warp per SM sub-partition the warps
     // run at the lone-warp rate, beyond that they share the sub-partition's issue slot and the SM's shared-memory pipe (and every
     // extra group re-walks the shared prefixes), so time ~ chain(G) * max(1, warps / (4 #SMs)).  Smallest G at the minimum.
-    const size_t units_sp = tiles * (size_t)a.n_parties;
-    int G = 1;
-    if (units_sp < (size_t)g_sms * (kEvalSpThreads / 32)) {
+    auto model_groups = [&](size_t units) {
+        int best_g = 1;
         double best = 0;
         for (int g = 1; g <= maxpts; ++g) {
             double chain = 0; int singles = 0;
@@ -288,23 +289,45 @@ int launch_eval_sp(const Program &P, int party, const void *const key[2], const 
             chain += (double)((singles + g - 1) / g) * (double)P.n;
             for (int w = 0; w < P.sp.n_w; ++w)
                 if (!P.sp.width[w].is_vec) chain += (double)((P.sp.width[w].n_points + g - 1) / g) * bit_tree_levels(P, P.sp.width[w].k);
-            const double load = (double)(units_sp * (size_t)g) / (4.0 * g_sms);
+            const double load = (double)(units * (size_t)g) / (4.0 * g_sms);
             const double cost = chain * (load > 1.0 ? load : 1.0);
-            if (g == 1 || cost < best - 1e-9) { best = cost; G = g; }
+            if (g == 1 || cost < best - 1e-9) { best = cost; best_g = g; }
         }
-    }
+        return best_g;
+    };
+    const size_t units_sp = tiles * (size_t)a.n_parties;
+    int G = units_sp < (size_t)g_sms * (kEvalSpThreads / 32) ? model_groups(units_sp) : 1;
     if (const int f = g_force_g.load()) G = f < maxpts ? f : maxpts;
-    a.G = G;
     a.np = g_sp_np.load() ? g_sp_np.load() : FFS_SP_NP_SMALL;      // clamped in the kernel to its compiled maximum (1 for large launches)
-    a.zero_first = G > 1;
-    const size_t items = tiles * (size_t)G * (size_t)a.n_parties;
+    size_t items = tiles * (size_t)G * (size_t)a.n_parties;
     const bool small = small_launch(items);
+    // TINY launches (even with every point of every element on its own warp at most one warp per SM sub-partition: a few hundred
+    // elements): the lane-split kernel (eval_sp_split.cuh) -- the 1 + QK blocks of a level on the lanes of a group, 32 / L elements per
+    // warp -- shortens the chain of one walk (one 32-element tile: 74 -> 57 us, variant 5: 107 -> 59 us).  Beyond that size the issue
+    // slots are all taken anyway and its shuffles / shared-memory round keys cost more than they save (recip 1,536 elements: 115 ->
+    // 125 us), so those launches stay on k_eval_sp (profiles/r2u_small_split.md).  sp_split = 2 forces it for every small launch (tests).
+    const int split_l = ((P.sp.pk + 1) / 2 == 1) ? 2 : 4;
+    const bool split = small && (g_sp_split.load() == 2 || (g_sp_split.load() == 1 && units_sp * (size_t)maxpts <= (size_t)g_sms * 4));
+    if (split) {
+        const size_t tiles_s = (count + (size_t)(32 / split_l) - 1) / (size_t)(32 / split_l);
+        G = model_groups(tiles_s * (size_t)a.n_parties);
+        if (const int f = g_force_g.load()) G = f < maxpts ? f : maxpts;
+        items = tiles_s * (size_t)G * (size_t)a.n_parties;
+    }
+    a.G = G;
+    a.zero_first = G > 1;
     const int cap_sp = g_eval_threads.load() < kEvalSpThreads ? g_eval_threads.load() : kEvalSpThreads;
     const int threads = small ? kEvalThreadsSmall : threads_for(items, cap_sp);
     const int grid = small ? (int)(items < (size_t)g_sms ? items : (size_t)g_sms) : grid_for(items, threads);   // small: spread the warps over ALL SMs
     const size_t sm = kAesSmemBytes;
     a.rpow = L.rpow;
     const bool coop = a.zero_first != 0;
+#define FSK_SPS_CASE(PP, KK) if (split && P.p == PP && P.sp.pk == KK) return launch(k_eval_sp_split<PP, KK>, grid, threads, sm, st, a, coop);
+#define FSK_SPS_ROW(KK) FSK_SPS_CASE(1, KK) FSK_SPS_CASE(2, KK) FSK_SPS_CASE(3, KK) FSK_SPS_CASE(4, KK) FSK_SPS_CASE(5, KK) \
+                        FSK_SPS_CASE(6, KK) FSK_SPS_CASE(7, KK) FSK_SPS_CASE(8, KK)
+    FSK_SPS_ROW(1) FSK_SPS_ROW(2) FSK_SPS_ROW(3)
+#undef FSK_SPS_ROW
+#undef FSK_SPS_CASE
 #define FSK_SP_CASE(PP, KK) if (P.p == PP && P.sp.pk == KK) return small ? launch(k_eval_sp<PP, KK, kEvalThreadsSmall>, grid, threads, sm, st, a, coop) \
                                                                          : launch(k_eval_sp<PP, KK, kEvalSpThreads>, grid, threads, sm, st, a, coop);
 #define FSK_SP_ROW(KK) FSK_SP_CASE(1, KK) FSK_SP_CASE(2, KK) FSK_SP_CASE(3, KK) FSK_SP_CASE(4, KK) FSK_SP_CASE(5, KK) \
@@ -511,6 +534,7 @@ int fusefss_debug_set(const char *knob, long value) {
     if (k == "small_kernels") { g_small_regs.store(value ? 1 : 0); return 0; }
     if (k == "sp_np") { g_sp_np.store(value >= 1 ? (int)value : 0); return 0; }
     if (k == "gen_quad") { g_gen_quad.store(value ? 1 : 0); return 0; }
+    if (k == "sp_split") { g_sp_split.store(value >= 0 && value <= 2 ? (int)value : 1); return 0; }
     return FUSEFSS_E_DEBUG;
 }
 uint64_t fusefss_launch_count(void) { return g_launches.load(); }

@@ -148,7 +148,7 @@ def knobs(F):
         for k, v in kw.items():
             F.debug_set(k, v)
     yield set_
-    F.debug_set("force_g", 0); F.debug_set("small_kernels", 1); F.debug_set("eval_threads", 1024); F.debug_set("gen_quad", 1)
+    F.debug_set("force_g", 0); F.debug_set("small_kernels", 1); F.debug_set("eval_threads", 1024); F.debug_set("gen_quad", 1); F.debug_set("sp_split", 1)
 
 
 @pytest.mark.parametrize("mk", SMALL + SMALL_SP + SMALL_XM + SMALL_XP + SMALL_ET + SMALL_DENSE + SMALL_A2B)
@@ -156,10 +156,10 @@ def knobs(F):
 def test_small_rings_all_masks(F, orc, mk, mode, knobs):
     """Every mask r (both Protocol 3 branches, incl. beta_0 = 0 and the dummy split) at n <= 8; a ragged count.
     auto: the launch configuration the library picks (small launches: every tree on its own warp, 256-thread kernels, in-kernel
-    zeroing + atomics; the dealer's quad-lane kernel k_gen_vec_quad); g1: one warp walks all trees of an element (no atomics); g2_big: two tree groups with the 1024-thread
+    zeroing + atomics; the dealer's quad-lane kernel k_gen_vec_quad; at these sizes the lane-split single-key kernel k_eval_sp_split); g1: one warp walks all trees of an element (no atomics); g2_big: two tree groups with the 1024-thread
     instantiations (the code path of large tensors whose last wave is split)."""
     if mode == "g1":
-        knobs(force_g=1, gen_quad=0)                        # and the lane-per-element dealer kernel instead of the quad-lane one
+        knobs(force_g=1, gen_quad=0, sp_split=0)            # and the lane-per-element kernels instead of the quad-lane dealer / lane-split evaluation
     if mode == "g2_big":
         knobs(force_g=2, small_kernels=0)
     spec = mk()
