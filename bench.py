@@ -249,9 +249,12 @@ class Gate:
         for first in range(0, self.count, self.chunk):
             e = [ev() for _ in range(6)] if events is not None else None
             rec = (lambda i: e[i].record()) if e else (lambda i: None)
-            rec(0); self.keygen(first, 1)            # the T bit-DCF keys (k_gen_bit)
-            rec(1); self.keygen(first, 2)            # the lookup keys (k_gen_vec)
-            rec(2); self.keygen(first, 4)            # share splitting (k_gen_misc)
+            if e is None and self.count <= SMALL_COUNT:      # small tensors: the user's call, fusefss_keygen (tiny ones: ONE dealer launch)
+                self.keygen(first, 7)
+            else:
+                rec(0); self.keygen(first, 1)            # the T bit-DCF keys (k_gen_bit)
+                rec(1); self.keygen(first, 2)            # the lookup keys (k_gen_vec)
+                rec(2); self.keygen(first, 4)            # share splitting (k_gen_misc)
             rec(3); bits, coeff = self.evaluate(first)
             rec(4); self.post(first, bits, coeff)
             rec(5)

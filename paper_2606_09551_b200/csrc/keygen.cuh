@@ -40,9 +40,8 @@ struct GenBitArgs {
     GenAtomDev atom[kMaxAtoms];
 };
 
-__global__ void __launch_bounds__(kGenThreads, 1) k_gen_bit(const __grid_constant__ GenBitArgs a) {
-    extern __shared__ uint32_t sT[];
-    const uint32_t tl = aes_fill_tables(sT);
+// the body of k_gen_bit (also run by k_gen_tiny, which makes ONE launch of a tiny tensor's whole dealer step)
+__device__ __forceinline__ void gen_bit_body(const GenBitArgs &a, const uint32_t tl) {
     const int lane = threadIdx.x & 31;
     const size_t tiles = (a.count + 31) / 32;
     const size_t items = tiles * (size_t)a.T;
@@ -149,6 +148,11 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_bit(const __grid_constan
         st_stream8(a.key0 + at.vb_off + e * 8, vbits);
         st_stream8(a.key1 + at.vb_off + e * 8, vbits);
     }
+}
+
+__global__ void __launch_bounds__(kGenThreads, 1) k_gen_bit(const __grid_constant__ GenBitArgs a) {
+    extern __shared__ uint32_t sT[];
+    gen_bit_body(a, aes_fill_tables(sT));
 }
 
 
@@ -355,11 +359,9 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec(const __grid_constan
 // Same arithmetic, same bytes: every value below is the one k_gen_vec computes (DESIGN 4.2), only WHERE it is computed differs.
 // ---------------------------------------------------------------------------------------------------
 template <int P>
-__global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec_quad(const __grid_constant__ GenVecArgs a) {
+__device__ __forceinline__ void gen_vec_quad_body(const GenVecArgs &a, const uint32_t tl) {
     constexpr int Q = (P + 1) / 2;
     constexpr unsigned FULL = 0xffffffffu;
-    extern __shared__ uint32_t sT[];
-    const uint32_t tl = aes_fill_tables(sT);
     const int lane = threadIdx.x & 31, c = lane & 3, b = c >> 1, d = c & 1, base = lane & ~3;
     const size_t tiles = (a.count + 7) / 8;
     const size_t items = tiles * (size_t)(a.M - 1);
@@ -461,6 +463,12 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec_quad(const __grid_co
     }
 }
 
+template <int P>
+__global__ void __launch_bounds__(kGenThreads, 1) k_gen_vec_quad(const __grid_constant__ GenVecArgs a) {
+    extern __shared__ uint32_t sT[];
+    gen_vec_quad_body<P>(a, aes_fill_tables(sT));
+}
+
 
 // ---------------------------------------------------------------------------------------------------
 // a4: share splitting.  One lane per element: c_b of the lookup, [r_in], [r_out], kappa^A,
@@ -479,9 +487,7 @@ struct GenMiscArgs {
     GenAtomDev atom[kMaxAtoms];
 };
 
-__global__ void __launch_bounds__(kGenThreads, 1) k_gen_misc(const __grid_constant__ GenMiscArgs a) {
-    extern __shared__ uint32_t sT[];
-    const uint32_t tl = aes_fill_tables(sT);
+__device__ __forceinline__ void gen_misc_body(const GenMiscArgs &a, const uint32_t tl) {
     for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < a.count; e += (size_t)gridDim.x * blockDim.x) {
         const uint64_t ge = a.first_elem + e;
         const uint64_t r = a.r_in[e] & a.mask;
@@ -610,6 +616,27 @@ __global__ void __launch_bounds__(kGenThreads, 1) k_gen_misc(const __grid_consta
             put(a.a2b_bits, b0, rbits ^ b0);
         }
     }
+}
+
+__global__ void __launch_bounds__(kGenThreads, 1) k_gen_misc(const __grid_constant__ GenMiscArgs a) {
+    extern __shared__ uint32_t sT[];
+    gen_misc_body(a, aes_fill_tables(sT));
+}
+
+// ---------------------------------------------------------------------------------------------------
+// The whole dealer step of a TINY tensor in ONE launch: bit trees, lookup trees (quad-lane) and share splitting run one after
+// the other on the same persistent CTAs, with one table fill (a launch costs 9-10 us of launch + fill, profiles/r2u_small_split.md,
+// which is most of a 4,096-element dealer pass).  The three parts write disjoint key sections, so no barrier separates them.
+// ---------------------------------------------------------------------------------------------------
+struct GenTinyArgs { GenBitArgs bit; GenVecArgs vec; GenMiscArgs misc; int has_bit, has_vec; };
+
+template <int P>
+__global__ void __launch_bounds__(kGenThreads, 1) k_gen_tiny(const __grid_constant__ GenTinyArgs a) {
+    extern __shared__ uint32_t sT[];
+    const uint32_t tl = aes_fill_tables(sT);
+    if (a.has_bit) gen_bit_body(a.bit, tl);
+    if (a.has_vec) gen_vec_quad_body<P>(a.vec, tl);
+    gen_misc_body(a.misc, tl);
 }
 
 }  // namespace fsk

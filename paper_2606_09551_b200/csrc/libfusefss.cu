@@ -561,52 +561,35 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
     const uint64_t *payload_dev = (const uint64_t *)(blob + P->dev_payload_off);
     const size_t tiles = (count + 31) / 32;
     const size_t smem = kAesSmemBytes;
+    // ---- arguments of the three dealer kernels (built unconditionally: host work only) -------------------------
+    bool has_bit = false, has_vec = false;
+    int vec_p = 1, vec_trees = 0;
+    GenBitArgs ab{};
+    ab.key0 = (uint8_t *)key0_dev; ab.key1 = (uint8_t *)key1_dev; ab.r_in = r_in_dev;
+    ab.count = count; ab.s16 = L.s16; ab.first_elem = first_elem; ab.mask = P->mask; ab.rk = rk; ab.et = (int)P->et;
+    GenVecArgs av{};
+    av.key0 = (uint8_t *)key0_dev; av.key1 = (uint8_t *)key1_dev; av.r_in = r_in_dev; av.alpha = alpha_dev; av.payload = payload_dev;
+    av.count = count; av.s16 = L.s16; av.s8 = L.s8; av.vt_first = L.vt_first; av.vt_stride = L.vt_stride; av.lvl_stride = L.lvl_stride;
+    av.vt_lvl_rel = L.vt_lvl_rel; av.vt_fin_rel = L.vt_fin_rel; av.first_elem = first_elem; av.mask = P->mask;
+    av.n = (int)P->n; av.m = (int)P->m; av.rk = rk;
     if (P->variant) {                                   // variant 1: one tree per view width (DESIGN 9)
-        bool any_bit = false, any_vec = false;
-        GenBitArgs ab{};
-        ab.key0 = (uint8_t *)key0_dev; ab.key1 = (uint8_t *)key1_dev; ab.r_in = r_in_dev;
-        ab.count = count; ab.s16 = L.s16; ab.first_elem = first_elem; ab.mask = P->mask; ab.T = P->sp.n_w; ab.rk = rk; ab.et = (int)P->et;
+        ab.T = P->sp.n_w;
         for (int w = 0; w < P->sp.n_w; ++w) {
             const bool vec = P->sp.width[w].is_vec != 0;
-            any_bit = any_bit || !vec; any_vec = any_vec || vec;
+            has_bit = has_bit || !vec; has_vec = has_vec || vec;
             ab.atom[w] = GenAtomDev{0, 0, L.bt_root[w], L.bt_cw[w], L.bt_vb[w], vec ? 0 : P->sp.width[w].k, 0};
         }
-        if (any_bit && (parts & FUSEFSS_GEN_CMP)) {
-            { const int th = threads_for(tiles * P->sp.n_w, kGenThreads); rc = launch(k_gen_bit, grid_for(tiles * P->sp.n_w, th), th, smem, st, ab); }
-            if (rc) return rc;
-        }
-        if (any_vec && (parts & FUSEFSS_GEN_LUT)) {
-            GenVecArgs a{};
-            a.key0 = (uint8_t *)key0_dev; a.key1 = (uint8_t *)key1_dev; a.r_in = r_in_dev; a.alpha = alpha_dev; a.payload = payload_dev;
-            a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.vt_first = L.vt_first; a.vt_stride = L.vt_stride; a.lvl_stride = L.lvl_stride;
-            a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel; a.first_elem = first_elem; a.mask = P->mask;
-            a.n = (int)P->n; a.m = (int)P->m; a.M = 2; a.sp = 1; a.rk = rk;
-            rc = launch_gen_vec(P->sp.pk, count, 1, st, a);
-            if (rc) return rc;
-        }
-    }
-    if (!P->variant && P->T > 0 && (parts & FUSEFSS_GEN_CMP)) {
-        GenBitArgs a{};
-        a.key0 = (uint8_t *)key0_dev; a.key1 = (uint8_t *)key1_dev; a.r_in = r_in_dev;
-        a.count = count; a.s16 = L.s16; a.first_elem = first_elem; a.mask = P->mask; a.T = P->T; a.rk = rk; a.et = (int)P->et;
+        av.M = 2; av.sp = 1; vec_p = P->sp.pk; vec_trees = 1;
+    } else {
+        has_bit = P->T > 0; has_vec = P->has_lut != 0;
+        ab.T = P->T;
         for (int t = 0; t < P->T; ++t)
-            a.atom[t] = GenAtomDev{P->atoms[t].c, P->atoms[t].beta, L.bt_root[t], L.bt_cw[t], L.bt_vb[t], P->atoms[t].k, P->atoms[t].is_theta};
-        const int th = threads_for(tiles * P->T, kGenThreads), grid = grid_for(tiles * P->T, th);
-        rc = launch(k_gen_bit, grid, th, kAesSmemBytes, st, a);
-        if (rc) return rc;
+            ab.atom[t] = GenAtomDev{P->atoms[t].c, P->atoms[t].beta, L.bt_root[t], L.bt_cw[t], L.bt_vb[t], P->atoms[t].k, P->atoms[t].is_theta};
+        av.M = P->M; av.xpoly = (int)P->xpoly; av.polys = (int)P->r; av.d = (int)P->d; vec_p = P->p; vec_trees = P->M - 1;
     }
-    if (!P->variant && P->has_lut && (parts & FUSEFSS_GEN_LUT)) {
-        GenVecArgs a{};
-        a.key0 = (uint8_t *)key0_dev; a.key1 = (uint8_t *)key1_dev; a.r_in = r_in_dev; a.alpha = alpha_dev; a.payload = payload_dev;
-        a.count = count; a.s16 = L.s16; a.s8 = L.s8; a.vt_first = L.vt_first; a.vt_stride = L.vt_stride; a.lvl_stride = L.lvl_stride;
-        a.vt_lvl_rel = L.vt_lvl_rel; a.vt_fin_rel = L.vt_fin_rel; a.first_elem = first_elem; a.mask = P->mask;
-        a.n = (int)P->n; a.m = (int)P->m; a.M = P->M; a.rk = rk;
-        a.xpoly = (int)P->xpoly; a.polys = (int)P->r; a.d = (int)P->d;
-        rc = launch_gen_vec(P->p, count, P->M - 1, st, a);
-        if (rc) return rc;
-    }
-    if (parts & FUSEFSS_GEN_SHARES) {
-        GenMiscArgs a{};
+    GenMiscArgs am{};
+    {
+        GenMiscArgs &a = am;
         a.key0 = (uint8_t *)key0_dev; a.key1 = (uint8_t *)key1_dev; a.r_in = r_in_dev; a.r_out = r_out_dev;
         a.alpha = alpha_dev; a.payload = payload_dev;
         a.count = count; a.s8 = L.s8; a.lut_c = L.lut_c; a.rin = L.rin; a.rout = L.rout; a.ka = L.ka; a.kb = L.kb;
@@ -624,8 +607,37 @@ int fusefss_keygen_parts(const fusefss_program *prog, const uint64_t *r_in_dev, 
             a.atom[t] = GenAtomDev{P->atoms[t].c, P->atoms[t].beta, 0, 0, 0, P->atoms[t].k, P->atoms[t].is_theta};
         a.a2b_rho = L.a2b_rho; a.a2b_bits = L.a2b_bits; a.GA2B = P->GA2B;
         for (int i = 0; i < P->GA2B; ++i) a.a2b_bit[i] = P->a2b_bit[i];
+    }
+    const size_t bit_items = tiles * (size_t)ab.T, vec_items = tiles * (size_t)vec_trees;
+    // TINY tensors, whole key at once: ONE launch for the three parts (k_gen_tiny) -- a launch costs 9-10 us of launch + table fill
+    const int all_parts = FUSEFSS_GEN_CMP | FUSEFSS_GEN_LUT | FUSEFSS_GEN_SHARES;
+    if (g_gen_quad.load() && (parts & all_parts) == all_parts && P->GA2B == 0 && (!has_vec || vec_items <= (size_t)g_sms * 2) &&
+        (!has_bit || bit_items <= (size_t)g_sms * 8)) {
+        GenTinyArgs t{};
+        t.bit = ab; t.vec = av; t.misc = am; t.has_bit = has_bit ? 1 : 0; t.has_vec = has_vec ? 1 : 0;
+        size_t items = tiles;
+        if (has_bit && bit_items > items) items = bit_items;
+        if (has_vec && ((count + 7) / 8) * (size_t)vec_trees > items) items = ((count + 7) / 8) * (size_t)vec_trees;
+        const int th = threads_for(items, kGenThreads), grid = grid_for(items, th);
+        switch (has_vec ? vec_p : 1) {
+#define FSK_GT_CASE(PP) case PP: return launch(k_gen_tiny<PP>, grid, th, smem, st, t);
+        FSK_GT_CASE(1) FSK_GT_CASE(2) FSK_GT_CASE(3) FSK_GT_CASE(4) FSK_GT_CASE(5) FSK_GT_CASE(6) FSK_GT_CASE(7) FSK_GT_CASE(8)
+#undef FSK_GT_CASE
+        }
+        return FUSEFSS_E_SPEC;
+    }
+    if (has_bit && (parts & FUSEFSS_GEN_CMP)) {
+        const int th = threads_for(bit_items, kGenThreads);
+        rc = launch(k_gen_bit, grid_for(bit_items, th), th, smem, st, ab);
+        if (rc) return rc;
+    }
+    if (has_vec && (parts & FUSEFSS_GEN_LUT)) {
+        rc = launch_gen_vec(vec_p, count, vec_trees, st, av);
+        if (rc) return rc;
+    }
+    if (parts & FUSEFSS_GEN_SHARES) {
         const int th = threads_for(tiles, kGenThreads), grid = grid_for(tiles, th);
-        rc = launch(k_gen_misc, grid, th, kAesSmemBytes, st, a);
+        rc = launch(k_gen_misc, grid, th, kAesSmemBytes, st, am);
         if (rc) return rc;
         if (P->GA2B > 0) {                              // the A2B nodes' comparison keys f_{rho_i mod 2^j, 1} (DESIGN 15): part of the shares section
             GenBitArgs ab{};
