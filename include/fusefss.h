@@ -35,7 +35,8 @@ enum {
     FUSEFSS_E_CUDA = -6,      /* a CUDA call failed (fusefss_last_cuda_error() has the text)  */
     FUSEFSS_E_OMITTED = -7,   /* eval_cmp with T = 0 / eval_lut with m = 1 (call omitted) */
     FUSEFSS_E_WORKSPACE = -8, /* fusefss_gate_host: workspace_bytes < fusefss_gate_workspace_bytes()  */
-    FUSEFSS_E_DEBUG = -9      /* fusefss_debug_set: unknown knob                                      */
+    FUSEFSS_E_DEBUG = -9,     /* fusefss_debug_set: unknown knob                                      */
+    FUSEFSS_E_STATIC = -10    /* fusefss_post_fused_noalloc: the lowered program has more than FUSEFSS_NOALLOC_MAX_INS instructions */
 };
 
 /* ---- operator specification (Def 4.1; grammar App. H) ------------------ */
@@ -186,6 +187,46 @@ int fusefss_post_fused(const fusefss_program *prog, const void *key0_dev, const 
                        const uint64_t *xhat_dev, const uint64_t *bits0_dev, const uint64_t *bits1_dev,
                        const uint64_t *coeff0_dev, const uint64_t *coeff1_dev, size_t count,
                        uint64_t *y0_dev, uint64_t *y1_dev, uint64_t *z0_dev, uint64_t *z1_dev, void *stream);
+
+/* ---- a7 without any device allocation ----------------------------------------------------------------------
+ * fusefss_post_fused_noalloc does exactly what fusefss_post_fused does (same arguments, same outputs bit for bit) but never
+ * calls cudaMalloc / cudaFree or any routine that allocates device memory.
+ *
+ * Who needs it.  fusefss_post_fused keeps the lowered post-processing program (the instruction table its kernel interprets)
+ * in a small device buffer that it cudaMalloc's the first time a program is used on a device.  Some hosts of this library
+ * cannot afford or are not allowed that call:
+ *   - an inference server whose tensor allocator has already reserved practically all of HBM for weights and caches, so a raw
+ *     cudaMalloc from a third-party library fails with out-of-memory (or is forbidden by the server's memory accounting);
+ *   - an online MPC loop with a latency budget: cudaMalloc synchronises the whole device, so a first-use allocation in the
+ *     middle of a layer stalls every other stream of the process;
+ *   - a party process confined to a fixed device-memory quota (MPS memory limit, container policy) sized in advance.
+ * For those callers the instruction table lives in a fixed array that is part of the library image itself
+ * (`static __device__`, FUSEFSS_NOALLOC_MAX_INS * 24 bytes = 48 KB): every GPU that loads libfusefss holds that array from
+ * module load until the process exits, whether or not this function is ever called.
+ *
+ * Limit.  A program whose lowered post-processing code is longer than FUSEFSS_NOALLOC_MAX_INS instructions is rejected with
+ * FUSEFSS_E_STATIC (every gate of the paper's benchmark suite lowers to well under 100).  That check needs no GPU and comes
+ * before the count check, so `fusefss_post_fused_noalloc(prog, k0, k1, xhat, ..., count = 0, ...)` answers at start-up:
+ * FUSEFSS_E_STATIC = does not fit, FUSEFSS_E_COUNT = fits.
+ *
+ * Set-up.  The first call on each device looks up the device address of the array (cudaGetSymbolAddress, with that device
+ * current) and, like every entry point, uploads the PRG constants once (a synchronous cudaMemcpyToSymbol).  Make that first
+ * call during start-up, before any stream capture begins on that device.
+ *
+ * Sharing.  There is ONE array per device, shared by every call, every program and every stream.  Each call copies its
+ * program's instructions into the front of the array on `stream` (a few hundred bytes to a few KB, ordered before its kernel)
+ * and whatever the previous call left behind stays there; nothing in the array has to start at zero, because the kernel reads
+ * exactly the n_ins entries this call wrote.  Two calls whose GPU work can overlap -- different streams, or different host
+ * threads on different streams -- race on the array and may interpret each other's program: serialise them (same stream, or an
+ * event between them).  Calls on one stream are safe back to back.
+ * Apart from that table the function uses no memory beyond the caller's inputs and outputs.  For the paper's Protocol-3
+ * construction (variant bit 0 clear) fusefss_eval_cmp / _lut / _fused / _fused_both never allocate either, so the whole online
+ * phase of a gate can run allocation-free. */
+#define FUSEFSS_NOALLOC_MAX_INS 2048
+int fusefss_post_fused_noalloc(const fusefss_program *prog, const void *key0_dev, const void *key1_dev,
+                               const uint64_t *xhat_dev, const uint64_t *bits0_dev, const uint64_t *bits1_dev,
+                               const uint64_t *coeff0_dev, const uint64_t *coeff1_dev, size_t count,
+                               uint64_t *y0_dev, uint64_t *y1_dev, uint64_t *z0_dev, uint64_t *z1_dev, void *stream);
 
 /* ---- vector-block glue (App. G: blocks = linear ops on shares + compiled scalar gates) ----------
  * fusefss_share_open: Protocol 1 for the input of gate `prog`: xhat = (x_0 + [r_in]_0) + (x_1 + [r_in]_1)

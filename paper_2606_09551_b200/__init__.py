@@ -20,7 +20,7 @@ LIB_PATH = os.path.join(_HERE, "libfusefss.so")
 SYMBOLS = (
     "fusefss_compile", "fusefss_destroy", "fusefss_shape", "fusefss_atom", "fusefss_key_bytes", "fusefss_keygen", "fusefss_keygen_parts",
     "fusefss_eval_cmp", "fusefss_eval_lut", "fusefss_eval_fused", "fusefss_eval_fused_both", "fusefss_post", "fusefss_post_rounds", "fusefss_post_msg_bytes",
-    "fusefss_online_bits", "fusefss_post_fused", "fusefss_cost", "fusefss_gate_workspace_bytes", "fusefss_gate_host",
+    "fusefss_online_bits", "fusefss_post_fused", "fusefss_post_fused_noalloc", "fusefss_cost", "fusefss_gate_workspace_bytes", "fusefss_gate_host",
     "fusefss_share_open", "fusefss_open_output", "fusefss_sub_bcast", "fusefss_row_sum", "fusefss_mul_triple_bytes", "fusefss_mul_keygen", "fusefss_mul_fused",
     "fusefss_strerror", "fusefss_last_cuda_error", "fusefss_debug_set", "fusefss_launch_count", "fusefss_aes_probe", "fusefss_aes_kat", "fusefss_pipe_probe", "fusefss_bitslice_kat", "fusefss_bitslice_probe",
 )
@@ -80,6 +80,7 @@ def _load():
         "fusefss_post_msg_bytes": (sz, [vp, sz, i32]),
         "fusefss_online_bits": (sz, [vp]),
         "fusefss_post_fused": (i32, [vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp, vp, vp, vp]),
+        "fusefss_post_fused_noalloc": (i32, [vp, vp, vp, vp, vp, vp, vp, vp, sz, vp, vp, vp, vp, vp]),
         "fusefss_cost": (i32, [vp, C.POINTER(Cost)]),
         "fusefss_gate_workspace_bytes": (sz, [vp, sz]),
         "fusefss_gate_host": (i32, [vp, vp, vp, vp, u64, sz, sz, vp, sz, vp, vp, vp, vp, vp]),
@@ -276,6 +277,16 @@ class Program:
                                                         self._empty(count), self._empty(count))
         _check(lib.fusefss_post_fused(self._h, _ptr(key0), _ptr(key1), _ptr(xhat), _ptr(bits0), _ptr(bits1),
                                       _ptr(coeff0), _ptr(coeff1), count, _ptr(y0), _ptr(y1), _ptr(z0), _ptr(z1), _stream()))
+        return y0, y1, z0, z1
+
+    def post_fused_noalloc(self, key0, key1, xhat, bits0, bits1, coeff0, coeff1, outs):
+        """fusefss_post_fused_noalloc: post_fused for hosts that must not allocate device memory (see include/fusefss.h).
+        To keep that promise on this side of the ABI too, the binding allocates nothing: `outs` = (y0, y1, z0, z1) are the
+        caller's tensors.  Calls share one table per device -- keep them on one stream."""
+        y0, y1, z0, z1 = outs
+        _check(lib.fusefss_post_fused_noalloc(self._h, _ptr(key0), _ptr(key1), _ptr(xhat), _ptr(bits0), _ptr(bits1),
+                                              _ptr(coeff0), _ptr(coeff1), xhat.numel(), _ptr(y0), _ptr(y1), _ptr(z0), _ptr(z1),
+                                              _stream()))
         return y0, y1, z0, z1
 
     def run_gate(self, key0, key1, xhat):

@@ -522,6 +522,7 @@ const char *fusefss_strerror(int code) {
     case FUSEFSS_E_OMITTED: return "call omitted for this gate type (T = 0 or m = 1)";
     case FUSEFSS_E_WORKSPACE: return "workspace smaller than fusefss_gate_workspace_bytes()";
     case FUSEFSS_E_DEBUG: return "unknown debug knob";
+    case FUSEFSS_E_STATIC: return "post-processing program longer than FUSEFSS_NOALLOC_MAX_INS instructions: use fusefss_post_fused";
     }
     return "unknown error";
 }
@@ -924,6 +925,76 @@ int fusefss_gate_host(const fusefss_program *prog, const uint64_t *r_in, const u
 }
 
 }  // extern "C"
+
+// ---- fusefss_post_fused_noalloc: the fused post-processing pass for callers that must not allocate ------------------------
+// (include/fusefss.h says who they are: servers whose allocator already owns all of HBM, latency-bound online loops that cannot
+// take cudaMalloc's device-wide synchronisation, processes under a fixed device-memory quota.)
+//
+// k_post_fused interprets the program's instruction table from global memory.  fusefss_post_fused keeps that table in a buffer it
+// cudaMalloc's on first use (ensure_blob); here the table goes into an array that is part of the module image instead, so it exists
+// on every GPU that loads the library, from module load to process exit: kStaticPostIns * sizeof(Ins) = 2048 * 24 B = 48 KB.
+//
+// One array per device, shared by all calls, programs and streams.  It keeps whatever the last call wrote; each call overwrites
+// the first n_ins entries on its own stream before its kernel and the kernel reads only those, so nothing needs clearing.  Calls
+// that can overlap on the GPU (different streams) race on it -- the header tells callers to serialise them.
+namespace fsk {
+constexpr int kStaticPostIns = FUSEFSS_NOALLOC_MAX_INS;
+// In HOST code this name is only a handle for the runtime's symbol calls, never a device address: passing it to a kernel would
+// fault (or quietly use host memory where the GPU can reach it).  static_post_table() below asks the runtime for the real address.
+static __device__ __align__(256) unsigned char g_static_post_ins[(size_t)kStaticPostIns * sizeof(Ins)];
+
+namespace {
+// Device address of g_static_post_ins on the CURRENT device: looked up once per device (the first noalloc call there, with that
+// device current), cached afterwards.  The map node is host memory; no device allocation happens here.
+int static_post_table(Ins **out) {
+    static std::mutex mu;
+    static std::map<int, Ins *> addr;
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lock(mu);
+    auto it = addr.find(dev);
+    if (it == addr.end()) {
+        void *p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_static_post_ins));
+        if (!p) return cuda_fail(cudaErrorInvalidSymbol, "cudaGetSymbolAddress(g_static_post_ins) returned null");
+        it = addr.emplace(dev, static_cast<Ins *>(p)).first;
+    }
+    *out = it->second;
+    return 0;
+}
+}  // namespace
+}  // namespace fsk
+
+extern "C" int fusefss_post_fused_noalloc(const fusefss_program *prog, const void *key0_dev, const void *key1_dev,
+                                          const uint64_t *xhat_dev, const uint64_t *bits0_dev, const uint64_t *bits1_dev,
+                                          const uint64_t *coeff0_dev, const uint64_t *coeff1_dev, size_t count, uint64_t *y0_dev,
+                                          uint64_t *y1_dev, uint64_t *z0_dev, uint64_t *z1_dev, void *stream) {
+    const Program *P = prog_of(prog);
+    if (!P || !key0_dev || !key1_dev || !xhat_dev) return FUSEFSS_E_NULL;
+    // the size limit is checked before anything touches the GPU (and before `count`), so a caller can probe it at start-up
+    if (P->ins.size() > (size_t)kStaticPostIns) return FUSEFSS_E_STATIC;
+    if (count == 0) return FUSEFSS_E_COUNT;
+    if ((P->T > 0 && (!bits0_dev || !bits1_dev)) || (P->has_lut && (!coeff0_dev || !coeff1_dev))) return FUSEFSS_E_NULL;
+    if ((P->n_out_a > 0 && (!y0_dev || !y1_dev)) || (P->n_out_b > 0 && (!z0_dev || !z1_dev))) return FUSEFSS_E_NULL;
+    int rc = init_device(); if (rc) return rc;
+    Ins *table = nullptr;
+    rc = static_post_table(&table); if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    // this call's instructions -> front of the shared table, ordered before the kernel on the same stream.  P->ins is pageable host
+    // memory owned by the program: the runtime has staged it by the time cudaMemcpyAsync returns, so the program may be destroyed
+    // as soon as this function has returned and the stream has drained.
+    if (!P->ins.empty())
+        CU(cudaMemcpyAsync(table, P->ins.data(), P->ins.size() * sizeof(Ins), cudaMemcpyHostToDevice, st));
+    Layout L; compute_layout(*P, count, &L);
+    PostFusedArgs a{};
+    a.ins = table; a.n_ins = (int)P->ins.size();
+    a.mask_output = (int)P->mask_output; a.n_out_a = P->n_out_a; a.n_out_b = P->n_out_b;
+    a.key[0] = (const uint8_t *)key0_dev; a.key[1] = (const uint8_t *)key1_dev; a.xhat = xhat_dev;
+    a.bits[0] = bits0_dev; a.bits[1] = bits1_dev; a.coeff[0] = coeff0_dev; a.coeff[1] = coeff1_dev;
+    a.y_out[0] = y0_dev; a.y_out[1] = y1_dev; a.z_out[0] = z0_dev; a.z_out[1] = z1_dev;
+    a.count = count; a.mask = P->mask; a.k = post_offsets(*P, L);
+    return launch_post(*P, k_post_fused<false>, k_post_fused<true>, count, st, a);
+}
 
 // ---- PRG micro-kernels: roofline denominator probe and FIPS-197 known-answer path --------------------
 namespace fsk {
