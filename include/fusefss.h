@@ -259,7 +259,9 @@ int fusefss_mul_fused(uint32_t n_bits, const uint64_t *x0_dev, const uint64_t *x
  * device workspace; r_in / r_out / xhat are copied to the device and y0, y1 [n_out_a][count], z0, z1 [count] back on an internal
  * copy stream, double-buffered, so the copies of chunk i+1 (in) and i-1 (out) overlap the kernels of chunk i (pin the host
  * buffers for that).  Returns after everything has completed.  workspace_dev must hold fusefss_gate_workspace_bytes(prog, chunk)
- * bytes; workspace_bytes is what the caller allocated (FUSEFSS_E_WORKSPACE if it is too small).  One call at a time per process. */
+ * bytes; workspace_bytes is what the caller allocated (FUSEFSS_E_WORKSPACE if it is too small).  Calls on one device are serialised
+ * (they share that device's copy stream and events); calls on different devices of one process run concurrently.  On an error return
+ * both streams have been drained first: no copy into the caller's host buffers is still in flight. */
 size_t fusefss_gate_workspace_bytes(const fusefss_program *prog, size_t chunk);
 int fusefss_gate_host(const fusefss_program *prog, const uint64_t *r_in, const uint64_t *r_out,
                       const uint64_t *xhat, uint64_t seed, size_t count, size_t chunk, void *workspace_dev,
@@ -282,7 +284,9 @@ const char *fusefss_last_cuda_error(void);
 /* Test / tuning knobs (process-wide, not part of the method): "force_g" = v >= 1 forces the number of warps the trees / points of an
  * element are dealt to (0 = automatic); "eval_threads" = CTA size of the large evaluation launches (default 1024); "small_kernels"
  * = 0 disables the 256-thread instantiations used for small launches; "sp_np" = points the single-key evaluation walks in lock-step per
- * warp (0 = automatic); "gen_quad" = 0 disables the four-lanes-per-element dealer kernel used for small launches; "sp_split" = 0 / 1 / 2: the lane-split
+ * warp (0 = automatic); "gen_quad" = 0 disables the four-lanes-per-element dealer kernel used for small launches; "coop" = 0: launches that accumulate with
+ * atomics clear their outputs with cudaMemsetAsync and launch normally instead of zeroing in-kernel behind a cooperative-launch grid barrier (the
+ * library takes that road by itself when the context refuses the cooperative launch); "sp_split" = 0 / 1 / 2: the lane-split
  * single-key evaluation kernel never / for tiny launches (default) / for every small launch.  Unknown knob: FUSEFSS_E_DEBUG. */
 int fusefss_debug_set(const char *knob, long value);
 /* number of kernel launches this library has issued since load (bench.py's gpu_launches) */

@@ -6,7 +6,7 @@
 // sits at shared-window offset  block*65536 + x*256 + half*128 + lane*4  (T0/T1 = halves of block 1, T2/T3 =
 // halves of block 2), so address = PRMT(state word, tl) = [tl.b0 | state byte k << 8 | tl.b2 | tl.b3] with
 // tl = 0x00010000 | lane*4, and (block, half) ride in the LDS immediate.  Per round and block: 16 PRMT + 16 LDS +
-// 8 LOP3 (r1a used SHF + LOP3 + IMAD per lookup and was issue-bound: profiles/r1a_launches_gelu.md).
+// 8 LOP3 (the first version of this core used SHF + LOP3 + IMAD per lookup and was issue-bound; no profile of it is kept).
 // State: 4 little-endian 32-bit words = the 4 columns (FIPS-197 3.4: byte r of word c is s[r][c]).
 #pragma once
 #include <cstdint>

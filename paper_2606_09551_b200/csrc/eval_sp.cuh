@@ -65,7 +65,10 @@ __device__ __forceinline__ void sp_step(uint32_t tl, const uint4 cw, const uint6
 // Cache behaviour of a level's correction words (HINT): the levels of a cluster's shared prefix (and every level of a lone point)
 // are read exactly once per element -- streamed (ld.global.cs, evict-first); the tail levels of a cluster are re-read once per
 // point of the cluster -- kept in L2 with an evict_last policy, so that the streamed prefix levels of the other 150,000 resident
-// lanes do not push them out to DRAM between two points (profiles/r2_eval_sp.md: DRAM reads 2.2x -> 1.0x the key size).
+// lanes do not push them out to DRAM between two points.  Measured (profiles/r2d_eval_sp_sweep.md, 1024 threads): DRAM bytes of the
+// gelu launch 2.72x -> 2.15x the key, of one silu chunk 4.01x -> 2.22x.  The hints do NOT bring the kernel to 1.0x: on the final
+// build profiles/traffic.md still has 2.2x on silu variant 1 and 6.5x on variant 5 (spill traffic of the 1024-thread instantiation
+// plus tail levels that fall out of L2 between the points of a cluster).
 #ifndef FFS_SP_L2HINT
 #define FFS_SP_L2HINT 1
 #endif

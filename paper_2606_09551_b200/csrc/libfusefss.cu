@@ -25,6 +25,7 @@ namespace fsk {
 namespace {
 
 thread_local char g_cuda_err[256] = "";
+thread_local cudaError_t g_cuda_code = cudaSuccess;   // code behind g_cuda_err (launch_accumulating asks for one specific failure)
 std::atomic<uint64_t> g_launches{0};
 thread_local int g_sms = 148;                 // SM count of the calling thread's current device (set by init_device)
 std::atomic<int> g_force_g{0};                // fusefss_debug_set("force_g", v): v >= 1 forces the tree-group count (tests)
@@ -32,10 +33,12 @@ std::atomic<int> g_eval_threads{kEvalThreads};// fusefss_debug_set("eval_threads
 std::atomic<int> g_sp_np{0};                  // fusefss_debug_set("sp_np", v): points walked in lock-step by k_eval_sp (0 = automatic)
 std::atomic<int> g_sp_split{1};                // fusefss_debug_set("sp_split", v): 0 = never the lane-split kernel, 1 = for tiny launches (default), 2 = for every small launch
 std::atomic<int> g_small_regs{1};             // fusefss_debug_set("small_kernels", 0): never pick the 256-thread instantiations
+std::atomic<int> g_coop{1};                   // fusefss_debug_set("coop", 0): G > 1 launches take the memset + plain-launch path (tests the fallback)
 const HostAes &host_aes() { static HostAes h; return h; }
 
 int cuda_fail(cudaError_t e, const char *what) {
     std::snprintf(g_cuda_err, sizeof g_cuda_err, "%s: %s", what, cudaGetErrorString(e));
+    g_cuda_code = e;
     return FUSEFSS_E_CUDA;
 }
 #define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(e_, #call); } while (0)
@@ -167,6 +170,26 @@ template <typename K, typename A> int launch(K kernel, int grid, int block, size
     return 0;
 }
 
+// Launches whose outputs are accumulated with atomics by G > 1 groups (a.zero_first): the kernel zeroes them itself behind ONE grid-wide
+// barrier, which needs a cooperative launch with every CTA co-resident (grid <= #SMs, one 192-KB CTA per SM).  A context that cannot
+// hold the grid -- an MPS client with an active-thread percentage, a green context or another SM partition, a co-running kernel that
+// pins shared memory -- refuses it with cudaErrorCooperativeLaunchTooLarge.  Then (and with the "coop" knob off): clear the
+// accumulators with cudaMemsetAsync on the same stream and launch the same kernel normally with zero_first = 0.  One more launch-sized
+// memset, same results bit for bit.
+template <typename K, typename A, typename Z>
+int launch_accumulating(K kernel, int grid, int block, size_t smem, cudaStream_t st, A a, Z clear_accumulators) {
+    if (!a.zero_first) return launch(kernel, grid, block, smem, st, a, false);
+    if (g_coop.load()) {
+        const int rc = launch(kernel, grid, block, smem, st, a, true);
+        if (rc == 0 || g_cuda_code != cudaErrorCooperativeLaunchTooLarge) return rc;
+        (void)cudaGetLastError();                  // the refusal is not sticky; clear it and take the other road
+    }
+    const int rc = clear_accumulators();
+    if (rc) return rc;
+    a.zero_first = 0;
+    return launch(kernel, grid, block, smem, st, a, false);
+}
+
 // ---- dispatch on P ---------------------------------------------------------------------------------
 int launch_gen_vec_p(int p, int grid, int block, cudaStream_t st, const GenVecArgs &a) {
     const size_t sm = kAesSmemBytes;
@@ -239,9 +262,15 @@ int launch_eval_p3(const Program &P, int party, const void *const key[2], const 
     const int threads = small ? kEvalThreadsSmall : threads_for(items, cap);
     const int grid = small ? (int)(items < (size_t)g_sms ? items : (size_t)g_sms) : grid_for(items, threads);   // small: spread the warps over ALL SMs
     const size_t sm = kAesSmemBytes;
-    const bool coop = a.zero_first != 0;
-#define FSK_P3_CASE(PP) case PP: return small ? launch(k_eval_p3<PP, kEvalThreadsSmall>, grid, threads, sm, st, a, coop) \
-                                              : launch(k_eval_p3<PP, p3_threads_for(PP)>, grid, threads, sm, st, a, coop);
+    auto clear = [&]() -> int {                    // what zero_outputs_and_sync would have zeroed
+        for (int sl = 0; sl < a.n_slots; ++sl) {
+            if (a.Gc > 1 && a.bits_out[sl]) CU(cudaMemsetAsync(a.bits_out[sl], 0, count * 8, st));
+            if (a.Gl > 1 && a.coeff_out[sl]) CU(cudaMemsetAsync(a.coeff_out[sl], 0, count * 8 * (size_t)P.p, st));
+        }
+        return 0;
+    };
+#define FSK_P3_CASE(PP) case PP: return small ? launch_accumulating(k_eval_p3<PP, kEvalThreadsSmall>, grid, threads, sm, st, a, clear) \
+                                              : launch_accumulating(k_eval_p3<PP, p3_threads_for(PP)>, grid, threads, sm, st, a, clear);
     switch (P.p) { FSK_P3_CASE(1) FSK_P3_CASE(2) FSK_P3_CASE(3) FSK_P3_CASE(4) FSK_P3_CASE(5) FSK_P3_CASE(6) FSK_P3_CASE(7) FSK_P3_CASE(8) }
 #undef FSK_P3_CASE
     return FUSEFSS_E_SPEC;
@@ -321,15 +350,21 @@ int launch_eval_sp(const Program &P, int party, const void *const key[2], const 
     const int grid = small ? (int)(items < (size_t)g_sms ? items : (size_t)g_sms) : grid_for(items, threads);   // small: spread the warps over ALL SMs
     const size_t sm = kAesSmemBytes;
     a.rpow = L.rpow;
-    const bool coop = a.zero_first != 0;
-#define FSK_SPS_CASE(PP, KK) if (split && P.p == PP && P.sp.pk == KK) return launch(k_eval_sp_split<PP, KK>, grid, threads, sm, st, a, coop);
+    auto clear = [&]() -> int {                    // what zero_outputs_and_sync would have zeroed
+        for (int sl = 0; sl < a.n_parties; ++sl) {
+            if (a.bits_out2[sl]) CU(cudaMemsetAsync(a.bits_out2[sl], 0, count * 8, st));
+            if (a.coeff_out2[sl]) CU(cudaMemsetAsync(a.coeff_out2[sl], 0, count * 8 * (size_t)P.p, st));
+        }
+        return 0;
+    };
+#define FSK_SPS_CASE(PP, KK) if (split && P.p == PP && P.sp.pk == KK) return launch_accumulating(k_eval_sp_split<PP, KK>, grid, threads, sm, st, a, clear);
 #define FSK_SPS_ROW(KK) FSK_SPS_CASE(1, KK) FSK_SPS_CASE(2, KK) FSK_SPS_CASE(3, KK) FSK_SPS_CASE(4, KK) FSK_SPS_CASE(5, KK) \
                         FSK_SPS_CASE(6, KK) FSK_SPS_CASE(7, KK) FSK_SPS_CASE(8, KK)
     FSK_SPS_ROW(1) FSK_SPS_ROW(2) FSK_SPS_ROW(3)
 #undef FSK_SPS_ROW
 #undef FSK_SPS_CASE
-#define FSK_SP_CASE(PP, KK) if (P.p == PP && P.sp.pk == KK) return small ? launch(k_eval_sp<PP, KK, kEvalThreadsSmall>, grid, threads, sm, st, a, coop) \
-                                                                         : launch(k_eval_sp<PP, KK, kEvalSpThreads>, grid, threads, sm, st, a, coop);
+#define FSK_SP_CASE(PP, KK) if (P.p == PP && P.sp.pk == KK) return small ? launch_accumulating(k_eval_sp<PP, KK, kEvalThreadsSmall>, grid, threads, sm, st, a, clear) \
+                                                                         : launch_accumulating(k_eval_sp<PP, KK, kEvalSpThreads>, grid, threads, sm, st, a, clear);
 #define FSK_SP_ROW(KK) FSK_SP_CASE(1, KK) FSK_SP_CASE(2, KK) FSK_SP_CASE(3, KK) FSK_SP_CASE(4, KK) FSK_SP_CASE(5, KK) \
                        FSK_SP_CASE(6, KK) FSK_SP_CASE(7, KK) FSK_SP_CASE(8, KK)
     FSK_SP_ROW(1) FSK_SP_ROW(2) FSK_SP_ROW(3)
@@ -535,6 +570,7 @@ int fusefss_debug_set(const char *knob, long value) {
     if (k == "small_kernels") { g_small_regs.store(value ? 1 : 0); return 0; }
     if (k == "sp_np") { g_sp_np.store(value >= 1 ? (int)value : 0); return 0; }
     if (k == "gen_quad") { g_gen_quad.store(value ? 1 : 0); return 0; }
+    if (k == "coop") { g_coop.store(value ? 1 : 0); return 0; }
     if (k == "sp_split") { g_sp_split.store(value >= 0 && value <= 2 ? (int)value : 1); return 0; }
     return FUSEFSS_E_DEBUG;
 }
@@ -830,7 +866,10 @@ size_t fusefss_gate_workspace_bytes(const fusefss_program *prog, size_t chunk) {
 
 namespace {
 // one copy stream and a few events per device for fusefss_gate_host, created on first use and kept for the life of the process
-struct HostPipe { cudaStream_t copy = nullptr; cudaEvent_t in_ready[2] = {}, in_free[2] = {}, out_ready[2] = {}, out_free[2] = {}; };
+struct HostPipe {
+    cudaStream_t copy = nullptr; cudaEvent_t in_ready[2] = {}, in_free[2] = {}, out_ready[2] = {}, out_free[2] = {};
+    std::mutex call_mu;                                        // the events are shared by the calls on THIS device: one call at a time per device
+};
 int host_pipe(HostPipe **out) {
     static std::mutex mu;
     static std::map<int, HostPipe> pipes;
@@ -866,8 +905,7 @@ int fusefss_gate_host(const fusefss_program *prog, const uint64_t *r_in, const u
     int rc = init_device(); if (rc) return rc;
     HostPipe *hp = nullptr;
     rc = host_pipe(&hp); if (rc) return rc;
-    static std::mutex call_mu;                                 // the pipe's events are shared: serialise calls
-    std::lock_guard<std::mutex> call_lock(call_mu);
+    std::lock_guard<std::mutex> call_lock(hp->call_mu);        // per device: calls on different GPUs of one process run concurrently
     cudaStream_t st = (cudaStream_t)stream, cs = hp->copy;
     Layout L; compute_layout(*P, chunk, &L);
     const int na = P->n_out_a > 0 ? P->n_out_a : 1;
@@ -891,6 +929,7 @@ int fusefss_gate_host(const fusefss_program *prog, const uint64_t *r_in, const u
         CU(cudaEventRecord(hp->in_ready[i & 1], cs));
         return 0;
     };
+    auto pipeline = [&]() -> int {
     CU(cudaEventRecord(hp->out_free[0], st)); CU(cudaEventRecord(hp->out_free[1], st));
     CU(cudaStreamWaitEvent(cs, hp->out_free[0], 0));           // order the copy stream after the caller's earlier work on `stream`
     rc = upload(0); if (rc) return rc;
@@ -922,6 +961,13 @@ int fusefss_gate_host(const fusefss_program *prog, const uint64_t *r_in, const u
     CU(cudaStreamSynchronize(cs));
     CU(cudaStreamSynchronize(st));
     return 0;
+    };
+    rc = pipeline();
+    if (rc) {                                                  // a step failed mid-pipeline: copies into / out of the caller's host buffers and kernels on the
+        (void)cudaStreamSynchronize(cs);                       // workspace may still be in flight.  Drain both streams before reporting, so that the caller
+        (void)cudaStreamSynchronize(st);                       // may free its buffers on error (the text of the first failure stays in fusefss_last_cuda_error)
+    }
+    return rc;
 }
 
 }  // extern "C"

@@ -148,7 +148,7 @@ def knobs(F):
         for k, v in kw.items():
             F.debug_set(k, v)
     yield set_
-    F.debug_set("force_g", 0); F.debug_set("small_kernels", 1); F.debug_set("eval_threads", 1024); F.debug_set("gen_quad", 1); F.debug_set("sp_split", 1)
+    F.debug_set("force_g", 0); F.debug_set("small_kernels", 1); F.debug_set("eval_threads", 1024); F.debug_set("gen_quad", 1); F.debug_set("sp_split", 1); F.debug_set("coop", 1)
 
 
 @pytest.mark.parametrize("mk", SMALL + SMALL_SP + SMALL_XM + SMALL_XP + SMALL_ET + SMALL_DENSE + SMALL_A2B)
@@ -200,6 +200,25 @@ def test_config_parity(F, orc, name, count, variant):
         spec = specs.early_termination(spec)                # bit trees cut 7 levels early (DESIGN 13)
     inp = tensors.inputs(name, spec, count=count, seed=0)
     _parity(F, orc, spec, inp["x"], inp["r_in"], inp["r_out"], seed=0)
+
+
+@pytest.mark.parametrize("variant", [0, 1, 5, 9])
+@pytest.mark.parametrize("name,count", [("relu16", 4096), ("recip", 130), ("rsqrt", 40), ("gelu", 333)])
+def test_no_cooperative_launch_fallback(F, orc, name, count, variant, knobs):
+    """Small launches accumulate the trees / points of an element with atomics from several warps and zero the outputs in-kernel behind
+    a cooperative-launch grid barrier.  Where the context refuses that launch (cudaErrorCooperativeLaunchTooLarge: MPS thread percentage,
+    SM partitions) the library clears the outputs with cudaMemsetAsync and launches normally; the "coop" = 0 knob takes that road on
+    purpose.  Same bits: the three evaluation kernels (k_eval_p3, k_eval_sp, k_eval_sp_split at the tiny counts) against the oracle."""
+    knobs(coop=0)
+    spec = specs.CONFIGS[name]()
+    if variant & 1:
+        spec = specs.shared_prefix(spec)
+    if variant & 4:
+        spec = specs.public_point_horner(spec)
+    if variant & 8:
+        spec = specs.early_termination(spec)
+    inp = tensors.inputs(name, spec, count=count, seed=6)
+    _parity(F, orc, spec, inp["x"], inp["r_in"], inp["r_out"], seed=2)
 
 
 def test_dense_table_relu16(F, orc):
