@@ -187,6 +187,8 @@ class Gate:
             spec = specs.public_point_horner(spec)
         if variant & 8:
             spec = specs.early_termination(spec)
+        if variant & 16:
+            spec = specs.dense_table(spec)                               # lookup by full-domain evaluation (needs bit 0, n <= 16; DESIGN 14)
         self.spec, self.P = spec, F.Program(spec)
         self.sh, self.cost = self.P.shape, self.P.cost()
         self.count, self.first_global = count, first_global
@@ -377,7 +379,12 @@ def measure(gate, M, steps, warmup, barrier, allmax, world=1, clocks_index=None)
         phases["keygen_bit"] = timed(graph_of(lambda: gate.keygen(0, 1))) if (sh["T"] and (not gate.variant & 1 or any(k < gate.spec.n for k in sh["k"]))) else 0.0
         phases["keygen_vec"] = timed(graph_of(lambda: gate.keygen(0, 2))) if sh["has_lut"] or gate.variant & 1 else 0.0
         phases["keygen_misc"] = timed(graph_of(lambda: gate.keygen(0, 4)))
+        # the dealer call the STEP makes (fusefss_keygen, all parts): for tiny tensors that is ONE k_gen_tiny launch, a different kernel
+        # from the three part launches above, which stay as a diagnostic (their sum exceeds this phase)
+        l_gen = F.launch_count()
         gate.keygen(0, 7)
+        dealer_launches = F.launch_count() - l_gen
+        keygen_all_ms = timed(graph_of(lambda: gate.keygen(0, 7)))
         phases["eval_both"] = timed(graph_of(ev_fn))
         bits, coeff = held["bc"]
         phases["post_fused"] = timed(graph_of(lambda: gate.post(0, bits, coeff)))
@@ -388,9 +395,21 @@ def measure(gate, M, steps, warmup, barrier, allmax, world=1, clocks_index=None)
         g1.keygen(0, 7)
         floor_ms = timed(graph_of(lambda: g1.evaluate(0)))
         g1.free()
+        # A floor that does NOT come from the kernel under test: one warp of the PRG probe (fusefss_aes_probe: no key loads, no tree logic)
+        # chaining n dependent trips of 3 AES blocks -- the PRG work on ONE root-to-leaf path of an n-level tree, which any evaluation of an
+        # element has to do in sequence -- plus what every launch pays (launch + filling the 128-KB table window).  Timed the same way.
+        pout = torch.empty(32 * 16, dtype=torch.uint8, device="cuda")
+        indep_floor_ms = timed(graph_of(lambda: F.aes_probe(32, 3 * gate.spec.n, pout)))
+        launch_fill_ms = timed(graph_of(lambda: F.aes_probe(32, 3, pout)))
         del flush
         l2 = "small tensor: CUDA-graph replay per step, a 256 MB L2 flush between timed replays (keys are read from HBM)"
     t_gen = phases["keygen_bit"] + phases["keygen_vec"] + phases["keygen_misc"]
+    parts_note = None
+    if small:                                                  # phases of the step as it runs: keygen_all + eval_both + post_fused
+        parts_note = {"keygen_bit": phases.pop("keygen_bit"), "keygen_vec": phases.pop("keygen_vec"), "keygen_misc": phases.pop("keygen_misc"),
+                      "what": "fusefss_keygen_parts launches timed alone (diagnostic: not the kernels the step runs when dealer_launches == 1)"}
+        phases = {"keygen_all": keygen_all_ms, **phases}
+        t_gen = keygen_all_ms
     t_eval, t_post = phases["eval_both"], phases["post_fused"]
     eval_aes = 2 * (cost["eval_cmp_aes"] + cost["eval_lut_aes"])
     eval_lk = 2 * (cost["eval_cmp_lookups"] + cost["eval_lut_lookups"])
@@ -398,7 +417,8 @@ def measure(gate, M, steps, warmup, barrier, allmax, world=1, clocks_index=None)
     gen_aes = cost["gen_cmp_aes"] + cost["gen_lut_aes"]
     n_launch = gate.n_chunks
     per_launch_elems = count / n_launch
-    eval_kernel = "k_eval_sp" if gate.variant & 1 else "k_eval_p3"
+    eval_kernel = ("k_eval_dense" if gate.variant & 16 else "k_eval_sp") if gate.variant & 1 else "k_eval_p3"
+    part_ms = parts_note or phases
 
     def roof(kernel, aes_elem, lk_elem, ms_total, bytes_elem):
         if not aes_elem or ms_total <= 0:
@@ -407,15 +427,25 @@ def measure(gate, M, steps, warmup, barrier, allmax, world=1, clocks_index=None)
         ach = aes_elem * per_launch_elems / (launch_ms * 1e-3) / 1e9
         peak = M.lookup_peak_gaes(lk_elem / aes_elem)
         gbs = bytes_elem * per_launch_elems / (launch_ms * 1e-3) / 1e9
-        return {"bound": "alu", "kernel": kernel, "achieved": ach, "peak": peak, "unit": "GAES/s (AES-128 blocks per second)",
+        return {"bound": "alu", "pipe": "lsu_shared (the shared-memory data pipe: T-table lookups; ncu pipe_lsu 96.6 %, pipe_alu 81 % on k_gen_vec<3>)",
+                "kernel": kernel, "achieved": ach, "peak": peak, "unit": "GAES/s (AES-128 blocks per second)",
                 "frac": ach / peak, "lookups_per_aes": lk_elem / aes_elem, "launch_ms": launch_ms, "aes_per_launch": aes_elem * per_launch_elems,
                 "share_of_step": ms_total / ms_step, "traffic": M.traffic_of(gate.name, gate.variant, int(per_launch_elems), kernel),
                 "algorithmic_bytes_per_launch": bytes_elem * per_launch_elems,
                 "hbm_achieved_gbs": gbs, "hbm_peak_gbs": M.hbm_gbs, "hbm_frac": gbs / M.hbm_gbs}
     roofs = {eval_kernel: roof(eval_kernel, eval_aes, eval_lk, t_eval, eval_key_bytes + 8 * (1 + 2 * (1 + sh["p"]))),
-             "k_gen_vec": roof("k_gen_vec", cost["gen_lut_aes"], cost["gen_lut_lookups"], phases["keygen_vec"], 2 * cost["eval_lut_key_bytes"]),
-             "k_gen_bit": roof("k_gen_bit", cost["gen_cmp_aes"], cost["gen_cmp_lookups"], phases["keygen_bit"], 2 * cost["eval_cmp_key_bytes"])}
+             "k_gen_vec": roof("k_gen_vec", cost["gen_lut_aes"], cost["gen_lut_lookups"], part_ms["keygen_vec"], 2 * cost["eval_lut_key_bytes"]),
+             "k_gen_bit": roof("k_gen_bit", cost["gen_cmp_aes"], cost["gen_cmp_lookups"], part_ms["keygen_bit"], 2 * cost["eval_cmp_key_bytes"])}
     roofs = {k: v for k, v in roofs.items() if v}
+    if small:                                                  # the whole dealer call against the roof of all its AES work; the part roofs are diagnostics
+        for k in ("k_gen_vec", "k_gen_bit"):
+            if k in roofs:
+                roofs[k]["note"] = "part launch timed alone (k_gen_vec_quad / k_gen_bit): the step itself runs fusefss_keygen, see keygen_all"
+        gen_lk = cost["gen_cmp_lookups"] + cost["gen_lut_lookups"]
+        r_all = roof("k_gen_tiny" if dealer_launches == 1 else "fusefss_keygen (%d launches)" % dealer_launches, gen_aes, gen_lk, keygen_all_ms,
+                     2 * (cost["eval_cmp_key_bytes"] + cost["eval_lut_key_bytes"]))
+        if r_all:
+            roofs["keygen_all"] = r_all
     key_b = P.key_bytes(1 << 20) / (1 << 20)
     res = {"count": count, "chunk": gate.chunk, "T": sh["T"], "M": sh["M"], "p": sh["p"], "rounds": P.post_rounds(),
            "value": world * count / (ms_step * 1e-3), "ms_per_step": ms_step,
@@ -430,6 +460,11 @@ def measure(gate, M, steps, warmup, barrier, allmax, world=1, clocks_index=None)
         res["clocks"] = clocks
     if floor_ms:
         res["eval_latency_floor_ms"] = floor_ms
+        res["eval_independent_floor_ms"] = indep_floor_ms
+        res["launch_and_table_fill_ms"] = launch_fill_ms
+    if parts_note:
+        res["keygen_parts_diagnostic_ms"] = parts_note
+        res["dealer_launches_per_step"] = dealer_launches
     return res
 
 
@@ -445,8 +480,58 @@ def compact(res):
             "eval_roof_frac": ek["frac"] if ek else None, "eval_kernel": res["eval_kernel"], "eval_launch_ms": ek["launch_ms"] if ek else None,
             "dominant_kernel": dom["kernel"] if dom else None, "dominant_roof_frac": dom["frac"] if dom else None,
             "traffic": ek["traffic"] if ek else None, "timing": "graph+flush" if res["l2"].startswith("small") else "events",
-            "eval_latency_floor_ms": res.get("eval_latency_floor_ms"),
-            "eval_floor_over_achieved": (res["eval_latency_floor_ms"] / ek["launch_ms"]) if (ek and res.get("eval_latency_floor_ms")) else None}
+            "eval_latency_floor_ms": res.get("eval_latency_floor_ms"), "dealer_launches_per_step": res.get("dealer_launches_per_step"),
+            "keygen_parts_diagnostic_ms": res.get("keygen_parts_diagnostic_ms"),
+            "eval_floor_over_achieved": (res["eval_latency_floor_ms"] / ek["launch_ms"]) if (ek and res.get("eval_latency_floor_ms")) else None,
+            # independent floor: one probe warp walking one n-level path (launch + table fill + n dependent 3-block trips), see measure()
+            "eval_independent_floor_ms": res.get("eval_independent_floor_ms"), "launch_and_table_fill_ms": res.get("launch_and_table_fill_ms"),
+            "eval_independent_floor_over_achieved": (res["eval_independent_floor_ms"] / ek["launch_ms"]) if (ek and res.get("eval_independent_floor_ms")) else None}
+
+
+def measure_a2b(F, torch, steps, count=1 << 20):
+    """A gate whose Phi has interactive A2B nodes (workloads.specs.a2b_demo on Z_2^64: three extractions at bits 63, 12 and 1 plus a local
+    one, DESIGN 15) on `count` uniform ring elements: dealer, both FSS calls, and the post-processing both ways -- one
+    fused launch for both parties (k_post_fused<true>) against the per-round API (k_post_round<true>: one launch per party per round, each
+    re-filling the 192-KB PRG table window because A2B rounds walk comparison keys)."""
+    from workloads import specs, tensors
+    spec = specs.a2b_demo(64, 12)
+    P = F.Program(spec)
+    rng = np.random.default_rng(0)
+    x, r_in = tensors.uniform_ring(rng, count, 64), tensors.uniform_ring(rng, count, 64)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.int64)).cuda()
+    d_rin, d_rout, d_xhat = dev(r_in), dev(tensors.uniform_ring(rng, count, 64).reshape(1, count)), dev(x + r_in)
+    keys = P.alloc_keys(count)
+    I = lambda *shape: torch.empty(shape, dtype=torch.int64, device="cuda")
+    bits, coeff = [I(count), I(count)], [I(P.shape["p"], count), I(P.shape["p"], count)]
+    outs = (I(1, count), I(1, count), I(count), I(count))
+    R = P.post_rounds()
+    msg = [torch.zeros(max(256, P.msg_total(count)), dtype=torch.uint8, device="cuda") for _ in (0, 1)]
+
+    def per_round():
+        for q in range(R + 1):
+            for b in (0, 1):
+                P.post(b, keys[b], d_xhat, bits[b], coeff[b], q, msg[1 - b], msg[b], y=outs[b], z=outs[2 + b])
+    legs = {"keygen": lambda: P.keygen(d_rin, d_rout, 0, keys=keys), "eval_both": lambda: P.eval_fused_both(keys[0], keys[1], d_xhat, bits, coeff),
+            "post_fused": lambda: P.post_fused(keys[0], keys[1], d_xhat, bits[0], bits[1], coeff[0], coeff[1], outs=outs), "post_per_round": per_round}
+    ms, launches = {}, {}
+    for nm, fn in legs.items():
+        for _ in range(2):
+            fn()
+        torch.cuda.synchronize()
+        l0 = F.launch_count()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(steps):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        ms[nm], launches[nm] = a.elapsed_time(b) / steps, (F.launch_count() - l0) // steps
+    step_ms = ms["keygen"] + ms["eval_both"] + ms["post_fused"]
+    return {"spec": "a2b_demo(n=64, f=12): m=3, p=%d, T=%d, %d interactive A2B nodes, %d rounds" % (P.shape["p"], P.shape["T"], 3, R), "count": count,
+            "ms": ms, "launches": launches, "step_elems_per_s": count / (step_ms * 1e-3),
+            "post_fused_elems_per_s": count / (ms["post_fused"] * 1e-3), "post_per_round_elems_per_s": count / (ms["post_per_round"] * 1e-3),
+            "key_bytes_per_elem_per_party": P.key_bytes(count) / count, "online_bytes_per_elem_per_party": P.online_bits() / 8,
+            "timing": "CUDA events around %d calls after 2 warm-up calls; inputs (%.1f GB of keys per party) exceed L2" % (steps, P.key_bytes(count) / 1e9)}
 
 
 def run_probes(F, torch, M, local):
@@ -636,10 +721,14 @@ def main():
     gate.free()                                                     # the e2e workspace holds its own key buffers
     if not args.no_e2e:
         e2e_chunk = gate_chunk if gate_chunks > 1 else min(count, 1 << 17)
-        line["e2e"] = e2e_of(P, sh, e2e_chunk, 1 if res["ms_per_step"] > 2000 else side_steps)
+        line["e2e"] = e2e_of(P, sh, e2e_chunk, max(3, side_steps) if res["ms_per_step"] > 2000 else side_steps)   # one untimed call, then >= 3 timed
 
     if not args.no_probes:
         line["prg_probe"] = run_probes(F, torch, M, local)
+        lds = line["prg_probe"].get("lds32_lanes_per_clk_per_sm")
+        if lds:                                                     # `frac` uses the nominal 32 lanes/clk/SM; this one the rate the pipe probe reached in this run
+            line["roofline"]["frac_vs_measured_lds"] = line["roofline"]["frac"] * LDS_LANES_PER_CLK_SM / lds
+            line["roofline"]["measured_lds_lanes_per_clk_per_sm"] = lds
 
     # ---- the same workload with the single-key shared-prefix construction (variants 1 and 5) ------------------
     if not args.no_sp and not (args.variant & 1):
@@ -668,13 +757,18 @@ def main():
             if other == name:
                 continue
             row = {}
-            for v in (0, 1):
+            # variants 8 / 9 = 0 / 1 with early-terminated bit trees (DESIGN 13), on the tensors whose gates have comparison atoms worth cutting;
+            # variant 17 = single key + dense-table lookup (DESIGN 14), on config 1 at its full 4,096 elements (n = 16)
+            extra = (8, 9) if other in ("relu16", "shift_relu", "gelu") else ()
+            extra += (17,) if other == "relu16" else ()
+            for v in (0, 1) + extra:
                 g3 = Gate(F, torch, other, v, tensors.FULL_COUNT[other], seed=0)
                 row["variant_%d" % v] = compact(measure(g3, M, side_steps, 3, barrier, allmax))
                 g3.free()
             cfgs[other] = row
         cfgs[name] = {"variant_%d" % args.variant: compact(res)}
         line["configs"] = cfgs
+        line["a2b_gate"] = measure_a2b(F, torch, side_steps)
 
     if args.blocks:
         from paper_2606_09551_b200 import blocks as gblocks

@@ -7,9 +7,12 @@
  *    fusefss_strerror() gives text.  Size queries return 0 on a null program.
  *  - Ring elements of Z_{2^n} (n <= 64) travel as uint64_t with bits >= n zero.
  *  - Pointers named *_dev are DEVICE pointers owned by the caller (e.g. torch tensors); pointers without
- *    the suffix are HOST pointers.  The library allocates no device memory of its own except a few KB per
- *    program (its post-processing code and descriptor tables, uploaded on first use, freed by _destroy).
- *  - `stream` is a cudaStream_t passed as void* (NULL = default stream); all launches are asynchronous on it.
+ *    the suffix are HOST pointers.  The library allocates no device memory of its own except one small buffer per
+ *    (program, device): its post-processing code and descriptor tables -- a few KB; for dense-table programs (variant bit 4) also the
+ *    2 x 2^n x p x 8-byte table, 2 MB at n = 16, p = 2.  fusefss_prepare() uploads it; otherwise the first call that needs it does
+ *    (one cudaMalloc + one synchronous cudaMemcpy, so call fusefss_prepare at start-up if first-use stalls matter).  Freed by _destroy.
+ *    fusefss_post_fused_noalloc needs no such buffer at all.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = default stream); once a program is prepared all launches are asynchronous on it.
  *  - party is 0 or 1.  xhat = x + r_in mod 2^n is public and identical for both parties (Protocol 1).
  *  - A key buffer is one-time material for exactly one xhat tensor; not enforced.
  *  - Key buffers are SoA over the chunk's elements; their size and layout depend on (program, count) only
@@ -118,6 +121,10 @@ typedef struct {
  * them.  Compile once per gate type, reuse across tensors/layers (program caching). */
 int fusefss_compile(const fusefss_spec *spec, fusefss_program **out);
 void fusefss_destroy(fusefss_program *prog);
+/* Uploads the program's device tables to the CURRENT device now (see Conventions) and initialises the library's per-device constants
+ * (PRG round keys and T-table seed in constant memory).  Idempotent and optional; after it no keygen / eval / post call with this program
+ * on this device allocates device memory or synchronises the device. */
+int fusefss_prepare(const fusefss_program *prog);
 int fusefss_shape(const fusefss_program *prog, fusefss_shape_t *out);
 /* atom t of the packed comparison instance Q = ((k_t, c_t, theta_t)) (Def I.1):
  * out4 = { k_t, c_t, is_theta, beta_t };  theta_t = (r mod 2^k + beta_t) mod 2^k, or r mod 2^k for an r-atom */

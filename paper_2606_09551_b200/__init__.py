@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libfusefss.so")
 
 # every symbol include/fusefss.h declares (tests check the library exports all of them)
 SYMBOLS = (
-    "fusefss_compile", "fusefss_destroy", "fusefss_shape", "fusefss_atom", "fusefss_key_bytes", "fusefss_keygen", "fusefss_keygen_parts",
+    "fusefss_compile", "fusefss_destroy", "fusefss_prepare", "fusefss_shape", "fusefss_atom", "fusefss_key_bytes", "fusefss_keygen", "fusefss_keygen_parts",
     "fusefss_eval_cmp", "fusefss_eval_lut", "fusefss_eval_fused", "fusefss_eval_fused_both", "fusefss_post", "fusefss_post_rounds", "fusefss_post_msg_bytes",
     "fusefss_online_bits", "fusefss_post_fused", "fusefss_post_fused_noalloc", "fusefss_cost", "fusefss_gate_workspace_bytes", "fusefss_gate_host",
     "fusefss_share_open", "fusefss_open_output", "fusefss_sub_bcast", "fusefss_row_sum", "fusefss_mul_triple_bytes", "fusefss_mul_keygen", "fusefss_mul_fused",
@@ -66,6 +66,7 @@ def _load():
     sig = {
         "fusefss_compile": (i32, [C.POINTER(Spec), C.POINTER(vp)]),
         "fusefss_destroy": (None, [vp]),
+        "fusefss_prepare": (i32, [vp]),
         "fusefss_shape": (i32, [vp, C.POINTER(Shape)]),
         "fusefss_atom": (i32, [vp, i32, C.POINTER(u64)]),
         "fusefss_key_bytes": (sz, [vp, sz]),
@@ -208,6 +209,11 @@ class Program:
         c = Cost()
         _check(lib.fusefss_cost(self._h, C.byref(c)))
         return {k: int(getattr(c, k)) for k, _ in Cost._fields_}
+
+    def prepare(self):
+        """fusefss_prepare: upload the program's tables to the current device now instead of on first use"""
+        _check(lib.fusefss_prepare(self._h))
+        return self
 
     def workspace_bytes(self, chunk):
         return lib.fusefss_gate_workspace_bytes(self._h, chunk)

@@ -450,6 +450,14 @@ void fusefss_destroy(fusefss_program *prog) {
     delete prog;
 }
 
+int fusefss_prepare(const fusefss_program *prog) {
+    const Program *P = prog_of(prog);
+    if (!P) return FUSEFSS_E_NULL;
+    int rc = init_device(); if (rc) return rc;
+    const uint8_t *blob = nullptr;
+    return ensure_blob(*P, &blob);
+}
+
 int fusefss_shape(const fusefss_program *prog, fusefss_shape_t *out) {
     const Program *P = prog_of(prog);
     if (!P || !out) return FUSEFSS_E_NULL;

@@ -11,7 +11,7 @@ if ROOT not in sys.path:
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
     config.addinivalue_line("markers", "slow: further exhaustive oracle pins (variant-bit x spec combinations beyond the default set); "
-                                       "run with `-m slow`; the recorded pass is profiles/r2_slow_pins.txt")
+                                       "run with `-m slow`; the recorded pass is profiles/r3_slow_pins.txt")
 
 
 def pytest_collection_modifyitems(config, items):

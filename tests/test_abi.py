@@ -139,3 +139,5 @@ def test_argument_errors_without_gpu(F):
     assert F.lib.fusefss_post(0, P._h, 1, 1, 1, 1, 10, 99, 1, 1, 1, 1, None) == -5
     assert F.lib.fusefss_gate_host(P._h, 1, 1, 1, 0, 10, 10, 1, 16, 1, 1, 1, 1, None) == -8    # workspace too small
     assert F.lib.fusefss_debug_set(b"no_such_knob", 1) == -9 and F.lib.fusefss_debug_set(b"force_g", 0) == 0
+    assert F.lib.fusefss_debug_set(b"coop", 1) == 0
+    assert F.lib.fusefss_prepare(None) == -1

@@ -221,6 +221,34 @@ def test_no_cooperative_launch_fallback(F, orc, name, count, variant, knobs):
     _parity(F, orc, spec, inp["x"], inp["r_in"], inp["r_out"], seed=2)
 
 
+def test_prepare_then_no_first_use_allocation(F):
+    """fusefss_prepare uploads the program's tables (2 MB for this dense-table program); with every tensor allocated beforehand, the dealer,
+    evaluation and post-processing calls that follow leave the device's free memory where it was: nothing allocates on first use."""
+    import torch
+    spec = specs.dense_table(specs.shared_prefix(specs.relu(16, 8)))
+    P = F.Program(spec)
+    count = 64
+    inp = tensors.inputs("relu16", spec, count=count, seed=1)
+    r_in, r_out, xhat = dev(inp["r_in"]), dev(inp["r_out"]), dev(inp["xhat"])
+    keys = P.alloc_keys(count)
+    I = lambda *shape: torch.empty(shape, dtype=torch.int64, device="cuda")
+    bits, coeff = [I(count), I(count)], [I(P.shape["p"], count), I(P.shape["p"], count)]
+    outs = (I(1, count), I(1, count), I(count), I(count))
+    F.Program(specs.relu(16, 8)).prepare()                   # per-device constants and module load are behind us
+    torch.cuda.synchronize()
+    P.prepare()
+    P.prepare()                                              # idempotent
+    free1 = torch.cuda.mem_get_info()[0]
+    P.keygen(r_in, r_out, 3, keys=keys)
+    P.eval_fused_both(keys[0], keys[1], xhat, bits, coeff)
+    P.post_fused(keys[0], keys[1], xhat, bits[0], bits[1], coeff[0], coeff[1], outs=outs)
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free1
+    y = (host(outs[0])[0] + host(outs[1])[0]) & mask_of(16)
+    x = inp["x"]
+    assert np.array_equal(y, np.where(x < (1 << 15), x, 0))  # ReLU on the 16-bit ring (PAPER.md:961-1016, App. N)
+
+
 def test_dense_table_relu16(F, orc):
     """config 1 (ReLU, n = 16) in the dense-table representation: 65,536-point full-domain evaluation per element and party; the
     oracle walks every point from the root, so a few dozen elements (a tile, a ragged tail, both parties in one launch)."""
