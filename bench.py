@@ -395,12 +395,20 @@ def measure(gate, M, steps, warmup, barrier, allmax, world=1, clocks_index=None)
         g1.keygen(0, 7)
         floor_ms = timed(graph_of(lambda: g1.evaluate(0)))
         g1.free()
-        # A floor that does NOT come from the kernel under test: one warp of the PRG probe (fusefss_aes_probe: no key loads, no tree logic)
-        # chaining n dependent trips of 3 AES blocks -- the PRG work on ONE root-to-leaf path of an n-level tree, which any evaluation of an
-        # element has to do in sequence -- plus what every launch pays (launch + filling the 128-KB table window).  Timed the same way.
+        # Floors that do NOT come from the kernel under test (fusefss_aes_chain_probe: one warp, no key loads, no tree logic): every evaluation
+        # of an element has to walk at least ONE root-to-leaf path of an n-level tree, level after level.  `independent`: a lane does all B blocks
+        # of a level itself (the lane-per-element mapping: B = 1 + Q payload blocks per node); `strict`: one block per level on the lane's
+        # dependent chain, the level's other blocks on other lanes (what any mapping short of splitting a single AES block across lanes can
+        # reach).  Both include what every launch pays (launch + filling the 128-KB table window of a 256-thread CTA), timed the same way.
+        if gate.variant & 1:
+            pk = (cost["eval_lut_key_bytes"] - 16 - 16 * gate.spec.n) // (8 * gate.spec.n + 8) if cost["eval_lut_key_bytes"] else 1
+        else:
+            pk = sh["p"]
+        level_blocks = min(5, 1 + (int(pk) + 1) // 2)
         pout = torch.empty(32 * 16, dtype=torch.uint8, device="cuda")
-        indep_floor_ms = timed(graph_of(lambda: F.aes_probe(32, 3 * gate.spec.n, pout)))
-        launch_fill_ms = timed(graph_of(lambda: F.aes_probe(32, 3, pout)))
+        indep_floor_ms = timed(graph_of(lambda: F.aes_chain_probe(level_blocks, gate.spec.n, pout)))
+        strict_floor_ms = timed(graph_of(lambda: F.aes_chain_probe(1, gate.spec.n, pout)))
+        launch_fill_ms = timed(graph_of(lambda: F.aes_chain_probe(1, 1, pout)))
         del flush
         l2 = "small tensor: CUDA-graph replay per step, a 256 MB L2 flush between timed replays (keys are read from HBM)"
     t_gen = phases["keygen_bit"] + phases["keygen_vec"] + phases["keygen_misc"]
@@ -461,6 +469,8 @@ def measure(gate, M, steps, warmup, barrier, allmax, world=1, clocks_index=None)
     if floor_ms:
         res["eval_latency_floor_ms"] = floor_ms
         res["eval_independent_floor_ms"] = indep_floor_ms
+        res["eval_strict_floor_ms"] = strict_floor_ms
+        res["floor_level_blocks"] = level_blocks
         res["launch_and_table_fill_ms"] = launch_fill_ms
     if parts_note:
         res["keygen_parts_diagnostic_ms"] = parts_note
@@ -485,7 +495,9 @@ def compact(res):
             "eval_floor_over_achieved": (res["eval_latency_floor_ms"] / ek["launch_ms"]) if (ek and res.get("eval_latency_floor_ms")) else None,
             # independent floor: one probe warp walking one n-level path (launch + table fill + n dependent 3-block trips), see measure()
             "eval_independent_floor_ms": res.get("eval_independent_floor_ms"), "launch_and_table_fill_ms": res.get("launch_and_table_fill_ms"),
-            "eval_independent_floor_over_achieved": (res["eval_independent_floor_ms"] / ek["launch_ms"]) if (ek and res.get("eval_independent_floor_ms")) else None}
+            "eval_independent_floor_over_achieved": (res["eval_independent_floor_ms"] / ek["launch_ms"]) if (ek and res.get("eval_independent_floor_ms")) else None,
+            "eval_strict_floor_ms": res.get("eval_strict_floor_ms"), "floor_level_blocks": res.get("floor_level_blocks"),
+            "eval_strict_floor_over_achieved": (res["eval_strict_floor_ms"] / ek["launch_ms"]) if (ek and res.get("eval_strict_floor_ms")) else None}
 
 
 def measure_a2b(F, torch, steps, count=1 << 20):
@@ -588,6 +600,9 @@ def main():
     ap.add_argument("--blocks", action="store_true", help="also time the softmax / LayerNorm vector blocks")
     ap.add_argument("--small-sweep", action="store_true", help="sweep the launch geometry of the small tensors' evaluation call (tuning evidence) and exit")
     ap.add_argument("--two-party", action="store_true", help="N = 2: party b on GPU b, real exchange of the opening buffers (two_party.run_party)")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"], help="process-group backend for N > 1 (gloo: exchanges staged through pinned host memory)")
+    ap.add_argument("--same-gpu", action="store_true", help="all ranks use cuda:0 (needs --backend gloo: NCCL refuses two ranks on one device).  A functional "
+                    "stand-in for a multi-GPU node where only one GPU is at hand: it exercises the sharding / exchange code, its timings say nothing about NVLink")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)                               # timing rule: W >= 3
     rank = int(os.environ.get("RANK", "0"))
@@ -615,19 +630,43 @@ def main():
     import paper_2606_09551_b200 as F
 
     assert torch.cuda.is_available(), "bench.py needs a CUDA device: the product has no CPU fallback"
+    if args.same_gpu:
+        assert args.backend == "gloo", "--same-gpu needs --backend gloo (NCCL refuses two ranks on one device)"
+        local = 0
     torch.cuda.set_device(local)
     use_dist = world > 1 or "LOCAL_RANK" in os.environ          # under torchrun the group exists even for one rank
+    red_dev = "cuda" if args.backend == "nccl" else "cpu"       # where the few scalars that cross ranks live
     if use_dist:
-        if os.environ.get("NCCL_DEBUG", "VERSION").upper() == "VERSION":
-            os.environ["NCCL_DEBUG"] = "WARN"                 # keep stdout to the one JSON line (no NCCL version banner)
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if args.backend == "nccl":
+            if os.environ.get("NCCL_DEBUG", "VERSION").upper() == "VERSION":
+                os.environ["NCCL_DEBUG"] = "WARN"             # keep stdout to the one JSON line (no NCCL version banner)
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group("gloo")
 
     def allmax(v):
         if use_dist:
-            t = torch.tensor([v], device="cuda", dtype=torch.float64)
+            t = torch.tensor([v], device=red_dev, dtype=torch.float64)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             return float(t.item())
         return v
+
+    def allsum32(v):
+        """sum over ranks of 32-bit checksums, mod 2^32"""
+        if use_dist:
+            t = torch.tensor([int(v)], device=red_dev, dtype=torch.int64)
+            dist.all_reduce(t, op=dist.ReduceOp.SUM)
+            return int(t.item()) & 0xFFFFFFFF
+        return int(v) & 0xFFFFFFFF
+
+    def checksum_of(g):
+        """32-bit checksum of the reconstructed outputs the gate's LAST chunk left on the device: sum_e (y0 + y1 mod 2^n) mod 2^32.  Randomness is
+        indexed by the global element, so a tensor sharded over ranks (one chunk per rank) sums to the one-rank value."""
+        c = g.count - (g.n_chunks - 1) * g.chunk
+        y = g.outs[0][0, :c] + g.outs[1][0, :c]                 # int64 arithmetic wraps mod 2^64
+        if g.spec.n < 64:
+            y = y & ((1 << g.spec.n) - 1)
+        return int((y & 0xFFFFFFFF).sum().item()) & 0xFFFFFFFF
 
     def barrier():
         torch.cuda.synchronize()
@@ -664,6 +703,7 @@ def main():
     res = measure(gate, M, args.steps, args.warmup, barrier, allmax, world=eff_world, clocks_index=local)
     if strong:
         res["value"] = full / (res["ms_per_step"] * 1e-3)
+    out_sum = allsum32(checksum_of(gate)) if (strong or world == 1) else checksum_of(gate)
     spec, sh, P = gate.spec, gate.sh, gate.P
     dominant = max(res["roofs"].values(), key=lambda r: r["share_of_step"])
     roofline = dict(dominant)
@@ -684,7 +724,11 @@ def main():
             "online_bytes_per_elem_per_party": res["online_bytes_per_elem_per_party"],
             "online_bytes_per_elem_per_party_input_masked_mul": F.Program(specs.input_masked_mul(spec)).online_bits() / 8,
             "aes_per_elem": res["aes_per_elem"], "projection": res["projection"], "gpu_launches": res["gpu_launches"],
-            "clocks": res.get("clocks"), "roofline": roofline}
+            "clocks": res.get("clocks"), "roofline": roofline,
+            "output_checksum": {"value": out_sum, "what": "sum over elements of (y0 + y1 mod 2^n) mod 2^32 of the last chunk" +
+                                (", summed over the ranks' shards" if strong else (" (rank 0's replica)" if world > 1 else ""))}}
+    if use_dist:
+        line["config"]["backend"] = args.backend + (", all ranks on cuda:0 (functional stand-in, not an NVLink measurement)" if args.same_gpu else "")
     side_steps = max(1, min(args.steps, args.side_steps))
     inp_host = gate.inp
 
@@ -722,6 +766,18 @@ def main():
     if not args.no_e2e:
         e2e_chunk = gate_chunk if gate_chunks > 1 else min(count, 1 << 17)
         line["e2e"] = e2e_of(P, sh, e2e_chunk, max(3, side_steps) if res["ms_per_step"] > 2000 else side_steps)   # one untimed call, then >= 3 timed
+
+    # ---- N > 1, replicas: the ONE tensor of the config sharded over the ranks as well, so that a scaling record carries a strong-scaling point
+    if world > 1 and not strong:
+        from paper_2606_09551_b200 import sharding
+        f2, c2 = sharding.shard_range(full, rank, world)
+        gs = Gate(F, torch, name, args.variant, c2, seed=0, first_global=f2, chunk=args.chunk, spec_count=full)
+        rs = measure(gs, M, side_steps, 3, barrier, allmax, world=1)
+        line["strong_scaling_leg"] = {"value": full / (rs["ms_per_step"] * 1e-3), "unit": "elements/s", "ms_per_step": rs["ms_per_step"], "steps": side_steps,
+                                      "what": f"the config's one {full}-element tensor sharded over {world} ranks by sharding.shard_range (contiguous, 32-aligned ranges; "
+                                              "randomness indexed by the global element; no collective); max-over-ranks time",
+                                      "output_checksum": allsum32(checksum_of(gs)) if gs.n_chunks == 1 else None}
+        gs.free()
 
     if not args.no_probes:
         line["prg_probe"] = run_probes(F, torch, M, local)

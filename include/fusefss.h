@@ -301,6 +301,11 @@ uint64_t fusefss_launch_count(void);
 /* PRG micro-kernel for the roofline denominator: each thread chains `iters` fixed-key AES-128 blocks starting
  * from its index and writes the last block to out_dev[threads*16 bytes]; blocks = threads*iters. */
 int fusefss_aes_probe(size_t threads, int iters, void *out_dev, void *stream);
+/* Latency probe for the small-tensor floor: ONE warp chains `trips` dependent trips, each expanding the lane's seed into blocks_per_trip
+ * (1..5) AES blocks that share their round-1 lookups -- the PRG work of one level of a tree with that many blocks per node, 32 elements in
+ * lock-step, with no key loads and no tree logic.  One 256-thread CTA (launch + table fill cost what a small evaluation launch pays).
+ * out_dev holds 32 * 16 bytes.  FUSEFSS_E_COUNT for trips <= 0 or blocks_per_trip outside 1..5. */
+int fusefss_aes_chain_probe(int blocks_per_trip, int trips, void *out_dev, void *stream);
 /* Pipe micro-probes for the roofline denominators: kind 0 = LOP3 issue (8 independent chains per thread), kind 1 =
  * conflict-free LDS.32 wavefronts (8 dependent-lookup chains per thread through the bank-replicated table).  One CTA of
  * 1024 threads per SM; out_dev holds SMs*1024 uint32.  Operations executed = SMs * 1024 * 8 * iters (lane-ops). */

@@ -22,7 +22,7 @@ SYMBOLS = (
     "fusefss_eval_cmp", "fusefss_eval_lut", "fusefss_eval_fused", "fusefss_eval_fused_both", "fusefss_post", "fusefss_post_rounds", "fusefss_post_msg_bytes",
     "fusefss_online_bits", "fusefss_post_fused", "fusefss_post_fused_noalloc", "fusefss_cost", "fusefss_gate_workspace_bytes", "fusefss_gate_host",
     "fusefss_share_open", "fusefss_open_output", "fusefss_sub_bcast", "fusefss_row_sum", "fusefss_mul_triple_bytes", "fusefss_mul_keygen", "fusefss_mul_fused",
-    "fusefss_strerror", "fusefss_last_cuda_error", "fusefss_debug_set", "fusefss_launch_count", "fusefss_aes_probe", "fusefss_aes_kat", "fusefss_pipe_probe", "fusefss_bitslice_kat", "fusefss_bitslice_probe",
+    "fusefss_strerror", "fusefss_last_cuda_error", "fusefss_debug_set", "fusefss_launch_count", "fusefss_aes_probe", "fusefss_aes_chain_probe", "fusefss_aes_kat", "fusefss_pipe_probe", "fusefss_bitslice_kat", "fusefss_bitslice_probe",
 )
 
 
@@ -97,6 +97,7 @@ def _load():
         "fusefss_debug_set": (i32, [C.c_char_p, C.c_long]),
         "fusefss_launch_count": (u64, []),
         "fusefss_aes_probe": (i32, [sz, i32, vp, vp]),
+        "fusefss_aes_chain_probe": (i32, [i32, i32, vp, vp]),
         "fusefss_aes_kat": (i32, [C.c_char_p, C.c_char_p, vp, vp]),
         "fusefss_pipe_probe": (i32, [i32, i32, vp, vp]),
         "fusefss_bitslice_kat": (i32, [C.c_char_p, vp, vp, vp]),
@@ -364,6 +365,12 @@ def bitslice_probe(threads: int = 0, iters: int = 24):
     torch.cuda.synchronize()
     return {"gaes": threads * 32 * iters / (a.elapsed_time(b) * 1e-3) / 1e9,
             "what": "fusefss_bitslice_probe: 32 blocks per thread as 128 bit-planes, composite-field S-box circuit (152 XOR + 36 AND per byte), no tables"}
+
+
+def aes_chain_probe(blocks_per_trip: int, trips: int, out):
+    """fusefss_aes_chain_probe: one warp, `trips` dependent trips of `blocks_per_trip` AES blocks; out = 512-byte CUDA tensor"""
+    _check(lib.fusefss_aes_chain_probe(blocks_per_trip, trips, _ptr(out), _stream()))
+    return out
 
 
 def aes_probe(threads: int, iters: int, out=None):

@@ -1094,6 +1094,28 @@ __global__ void __launch_bounds__(kEvalThreads, 1) k_pipe_probe(const PipeArgs a
     for (int j = 0; j < 8; ++j) acc ^= v[j];
     a.out[(size_t)blockIdx.x * blockDim.x + threadIdx.x] = acc;
 }
+// Latency probe for the small-tensor floor (bench.py, DESIGN 6): ONE warp of a 256-thread CTA (the CTA size of the small evaluation kernels,
+// so launch + table fill cost the same) chains `iters` dependent trips; a trip expands the lane's seed into B blocks that share their
+// round-1 lookups -- the PRG work of one tree level with B blocks per node, 32 elements in lock-step -- and folds them into the next seed.
+template <int B>
+__global__ void __launch_bounds__(kEvalThreadsSmall, 1) k_aes_chain_probe(const ProbeArgs a) {
+    extern __shared__ uint32_t sT[];
+    const uint32_t tl = aes_fill_tables(sT);
+    if (threadIdx.x >= 32) return;
+    uint32_t x[1][4] = {{threadIdx.x * 2654435761u, 0x9e3779b9u, 0x7f4a7c15u, 0xf39cc060u}};
+    for (int it = 0; it < a.iters; ++it) {
+        uint32_t o[1][B][4];
+        prg_blocks<1, B, 0, 1>(tl, x, o);
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            uint32_t v = 0;
+#pragma unroll
+            for (int k = 0; k < B; ++k) v ^= o[0][k][(c + k) & 3];
+            x[0][c] = v;
+        }
+    }
+    a.out[threadIdx.x] = make_uint4(x[0][0], x[0][1], x[0][2], x[0][3]);
+}
 struct KatArgs { uint4 *out; uint32_t in[4]; RoundKeys rk; };
 __global__ void k_aes_kat(const KatArgs a) {
     extern __shared__ uint32_t sT[];
@@ -1115,6 +1137,19 @@ int fusefss_aes_probe(size_t threads, int iters, void *out_dev, void *stream) {
     ProbeArgs a{(uint4 *)out_dev, threads, iters};
     const int grid = grid_for((threads + 31) / 32, kEvalThreads);
     return launch(k_aes_probe, grid, kEvalThreads, kAesSmemBytes, (cudaStream_t)stream, a);
+}
+
+int fusefss_aes_chain_probe(int blocks_per_trip, int trips, void *out_dev, void *stream) {
+    if (!out_dev) return FUSEFSS_E_NULL;
+    if (trips <= 0 || blocks_per_trip < 1 || blocks_per_trip > 5) return FUSEFSS_E_COUNT;
+    int rc = init_device(); if (rc) return rc;
+    ProbeArgs a{(uint4 *)out_dev, 32, trips};
+    switch (blocks_per_trip) {
+#define FSK_CH_CASE(BB) case BB: return launch(k_aes_chain_probe<BB>, 1, kEvalThreadsSmall, kAesSmemBytes, (cudaStream_t)stream, a);
+    FSK_CH_CASE(1) FSK_CH_CASE(2) FSK_CH_CASE(3) FSK_CH_CASE(4) FSK_CH_CASE(5)
+#undef FSK_CH_CASE
+    }
+    return FUSEFSS_E_COUNT;
 }
 
 int fusefss_pipe_probe(int kind, int iters, void *out_dev, void *stream) {

@@ -102,11 +102,21 @@ def bench(F, torch, dist, args, rank, world, M):
         y, z, sent = run_party_cuda(P, rank, key, xhat)
     b.record()
     torch.cuda.synchronize(); dist.barrier(); torch.cuda.synchronize()
-    t = torch.tensor([a.elapsed_time(b)], device="cuda", dtype=torch.float64)
+    nccl = dist.get_backend() == "nccl"
+    t = torch.tensor([a.elapsed_time(b)], device="cuda" if nccl else "cpu", dtype=torch.float64)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms = float(t.item()) / args.steps
-    return {"metric": "online elements/s, one GPU per party (FSS calls + post-processing rounds with NCCL exchange)", "value": count / (ms * 1e-3),
+    # reconstruct on rank 0: the two parties' output shares must add up to the plaintext gate (the check a user of the online phase would make)
+    y_other = exchange(y.contiguous(), 1 - rank, rank)
+    mask = (1 << spec.n) - 1
+    rec = y[0] + y_other[0]
+    if spec.n < 64:
+        rec = rec & mask
+    checksum = int((rec & 0xFFFFFFFF).sum().item()) & 0xFFFFFFFF
+    how = "NCCL send/recv of the device buffers" if nccl else "gloo, staged through pinned host memory (two processes; a stand-in for NVLink when both ranks share one GPU)"
+    return {"metric": "online elements/s, one process per party (FSS calls + post-processing rounds with a real exchange: %s)" % how, "value": count / (ms * 1e-3),
             "unit": "elements/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
             "scaling": "two-party", "vs_baseline": None, "dtype": "u64", "data": "synthetic",
             "config": {"workload": f"{name} n={spec.n} f={spec.f} count={count}", "construction": f"variant {v}", "parallelism": "party b on GPU b, send/recv of the opening buffers"},
-            "online_bytes_sent_per_party_per_step": sent, "rounds": P.post_rounds()}
+            "online_bytes_sent_per_party_per_step": sent, "rounds": P.post_rounds(), "exchange": how,
+            "output_checksum": {"value": checksum, "what": "sum over elements of (y0 + y1 mod 2^n) mod 2^32, y1 received from the peer"}}

@@ -64,3 +64,40 @@ def test_two_ranks_gloo():
     assert ranges[0][0] == 0 and ranges[0][0] + ranges[0][1] == ranges[1][0]
     assert ranges[1][0] + ranges[1][1] == total and ranges[1][0] % 32 == 0
     assert tmax == 11.0
+
+
+# ---- the N > 1 paths of bench.py on ONE GPU: two processes over gloo (NCCL refuses two ranks on one device) ------------------------------
+def _bench_line(extra, nproc=1, port=0):
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    common = ["--workload", "gelu", "--count", "65536", "--steps", "2", "--warmup", "3", "--no-cpu", "--no-e2e", "--no-sp", "--no-configs", "--no-probes"]
+    if nproc == 1:
+        cmd = [sys.executable, os.path.join(root, "bench.py"), "--gpus", "1"] + common + extra
+    else:
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(nproc), "--master-addr", "127.0.0.1",
+               "--master-port", str(port), os.path.join(root, "bench.py"), "--gpus", str(nproc), "--backend", "gloo", "--same-gpu"] + common + extra
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=900, cwd=root)
+    assert out.returncode == 0, out.stderr[-3000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, out.stdout[-2000:]
+    return json.loads(lines[0])
+
+
+@pytest.mark.gpu
+def test_bench_multi_rank_paths_on_one_gpu():
+    """bench.py's strong-scaling, replica and party-per-process legs have only ever had one GPU to run on.  Two processes sharing cuda:0 over a
+    gloo group run the same code (sharding.shard_range, max-over-ranks timing, the per-round exchange of two_party.run_party); the outputs they
+    leave must reconstruct to the same values as the one-process run: equal 32-bit checksums of y0 + y1."""
+    one = _bench_line([])
+    ref = one["output_checksum"]["value"]
+    strong = _bench_line(["--scaling", "strong"], nproc=2, port=29731)
+    assert strong["n_gpus"] == 2 and strong["scaling"] == "strong" and "gloo" in strong["config"]["backend"]
+    assert strong["output_checksum"]["value"] == ref
+    weak = _bench_line([], nproc=2, port=29732)
+    assert weak["scaling"] == "weak" and weak["output_checksum"]["value"] == ref          # rank 0's replica = the one-process tensor (seed 0)
+    assert weak["strong_scaling_leg"]["output_checksum"] == ref and weak["strong_scaling_leg"]["value"] > 0
+    two = _bench_line(["--two-party"], nproc=2, port=29733)
+    assert two["scaling"] == "two-party" and two["rounds"] >= 1 and two["online_bytes_sent_per_party_per_step"] > 0
+    assert two["output_checksum"]["value"] == ref
